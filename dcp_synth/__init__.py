@@ -1,0 +1,195 @@
+"""Seeded synthetic inputs for the pair-bias attention layer (Design-CP's one-GPU core).
+
+This module is the ONLY code shared by the CPU oracle (`oracle/`) and the CUDA path
+(`paper_2607_05439_b200/`).  It holds no arithmetic of the method itself: it only draws
+random tensors with the shapes, value distributions and copy/residue block structure of
+the paper's icosahedral workloads (PAPER.md:118-120 "60 x 210 residues", :152, :323;
+BASELINE.json `configs`), and rounds them once to the storage dtype.
+
+Recipe:
+  * token index  i = copy * n + res,  copy in [0, copies), res in [0, n)   (copies = 60)
+  * s[i]   = a[res] + 0.1 * N(0,1)                 a ~ N(0,1)  [n, c_s]
+  * z[i,j] = E[copy(i), copy(j)] + R[res(i), res(j)] + 0.1 * N(0,1)
+             E ~ N(0,1) [copies, copies, c_z],  R ~ N(0,1) [n, n, c_z]
+  * weights: W_q, W_k, W_v, W_g [c_s, H*c], W_o [H*c, c_s], W_b [c_z, H]  ~ N(0, 1/fan_in)
+             (variance 1/fan_in), gamma = 1 + 0.1 N(0,1), beta = 0.1 N(0,1)
+  * config 0 is iid: s ~ N(0,1), z ~ N(0,1), no block structure.
+
+Everything is generated with `torch` generators so the same code runs on the CPU (tests,
+oracle) and on the GPU (z of 2.3-36.9 GB must be born in HBM).  CPU and CUDA generators give
+different bit streams; each is deterministic per seed.  Parity tests always hand the oracle
+the exact stored bits (read back from the device), never a re-generation.
+"""
+from __future__ import annotations
+
+import dataclasses
+import math
+from typing import Dict, Optional
+
+import torch
+
+COPIES = 60  # icosahedral point group order: 60 ASU copies
+
+
+@dataclasses.dataclass(frozen=True)
+class LayerConfig:
+    """Shape of one pair-bias attention layer call (BASELINE.json `configs`)."""
+
+    name: str
+    I: int          # tokens (or L atoms)
+    c_s: int        # single-track width (c_atom for the atom variant)
+    c_z: int        # pair width (c_atompair for the atom variant)
+    H: int          # heads
+    c: int          # head dim
+    dtype: str      # "f32" | "bf16"  storage type
+    seed: int
+    structured: bool = True   # icosahedral copy/residue block structure
+    copies: int = COPIES
+
+    @property
+    def D(self) -> int:
+        return self.H * self.c
+
+    @property
+    def n_res(self) -> int:
+        return self.I // self.copies if self.structured else self.I
+
+    def z_bytes(self) -> int:
+        return self.I * self.I * self.c_z * (4 if self.dtype == "f32" else 2)
+
+
+# BASELINE.json configs 0..4 (C0..C4)
+CONFIGS: Dict[str, LayerConfig] = {
+    "C0": LayerConfig("C0", I=64, c_s=128, c_z=64, H=4, c=32, dtype="f32", seed=0, structured=False),
+    "C1": LayerConfig("C1", I=600, c_s=384, c_z=128, H=16, c=24, dtype="bf16", seed=1),
+    "C2": LayerConfig("C2", I=3000, c_s=384, c_z=128, H=16, c=48, dtype="bf16", seed=2),
+    "C3": LayerConfig("C3", I=12000, c_s=384, c_z=128, H=16, c=48, dtype="bf16", seed=3),
+    "C4": LayerConfig("C4", I=24000, c_s=128, c_z=16, H=4, c=32, dtype="bf16", seed=4),
+}
+
+
+def torch_dtype(name: str) -> torch.dtype:
+    return {"f32": torch.float32, "bf16": torch.bfloat16}[name]
+
+
+def _gen(seed: int, device) -> torch.Generator:
+    g = torch.Generator(device=device)
+    g.manual_seed(int(seed))
+    return g
+
+
+def make_weights(cfg: LayerConfig, device="cpu", with_ln_s: bool = False,
+                 with_b_q: bool = False) -> Dict[str, torch.Tensor]:
+    """Layer weights, drawn on the CPU in fp32 (tiny), rounded once to the storage dtype.
+
+    Draw order is fixed: W_q, W_k, W_v, W_g, W_b, W_o, gamma_z, beta_z, gamma_s, beta_s, b_q.
+    """
+    g = _gen(cfg.seed * 1000003 + 17, "cpu")
+    dt = torch_dtype(cfg.dtype)
+    D = cfg.D
+
+    def n(*shape, std=1.0):
+        return torch.randn(*shape, generator=g, dtype=torch.float32) * std
+
+    w = {}
+    for k in ("w_q", "w_k", "w_v", "w_g"):
+        w[k] = n(cfg.c_s, D, std=1.0 / math.sqrt(cfg.c_s))
+    w["w_b"] = n(cfg.c_z, cfg.H, std=1.0 / math.sqrt(cfg.c_z))
+    w["w_o"] = n(D, cfg.c_s, std=1.0 / math.sqrt(D))
+    w["ln_z_gamma"] = 1.0 + 0.1 * n(cfg.c_z)
+    w["ln_z_beta"] = 0.1 * n(cfg.c_z)
+    gs, bs, bq = 1.0 + 0.1 * n(cfg.c_s), 0.1 * n(cfg.c_s), 0.1 * n(D)
+    if with_ln_s:
+        w["ln_s_gamma"], w["ln_s_beta"] = gs, bs
+    if with_b_q:
+        w["b_q"] = bq
+    return {k: v.to(dt).to(device).contiguous() for k, v in w.items()}
+
+
+def make_s(cfg: LayerConfig, device="cpu") -> torch.Tensor:
+    """Single track s [I, c_s] in the storage dtype."""
+    g = _gen(cfg.seed * 1000003 + 1, "cpu")
+    if not cfg.structured:
+        s = torch.randn(cfg.I, cfg.c_s, generator=g, dtype=torch.float32)
+    else:
+        n = cfg.n_res
+        assert n * cfg.copies == cfg.I, "structured configs need I = copies * n_res"
+        a = torch.randn(n, cfg.c_s, generator=g, dtype=torch.float32)
+        s = a.repeat(cfg.copies, 1) + 0.1 * torch.randn(cfg.I, cfg.c_s, generator=g, dtype=torch.float32)
+    return s.to(torch_dtype(cfg.dtype)).to(device).contiguous()
+
+
+def _tables(cfg: LayerConfig, device):
+    g = _gen(cfg.seed * 1000003 + 2, "cpu")
+    n = cfg.n_res
+    E = torch.randn(cfg.copies, cfg.copies, cfg.c_z, generator=g, dtype=torch.float32)
+    R = torch.randn(n, n, cfg.c_z, generator=g, dtype=torch.float32)
+    return E.to(device), R.to(device)
+
+
+def fill_z(cfg: LayerConfig, out: torch.Tensor, chunk_rows: int = 0,
+           noise: float = 0.1, cyclic_copy_table: bool = False) -> torch.Tensor:
+    """Fill `out` ([I, I, c_z], storage dtype, on any device) with the pair tensor, in row chunks.
+
+    Chunk r (rows [r*chunk, (r+1)*chunk)) draws its noise from a generator seeded
+    (seed, r) on out's device, so a fill is repeatable for a fixed device type and chunk size.
+    `cyclic_copy_table` replaces E[a,b] by F[(b-a) mod copies] (used by the oracle's
+    copy-shift invariance pin; SURVEY.md 8c "Symmetry").
+    """
+    I, cz = cfg.I, cfg.c_z
+    assert tuple(out.shape) == (I, I, cz)
+    dev = out.device
+    if not cfg.structured:
+        chunk = chunk_rows or I
+        for r, i0 in enumerate(range(0, I, chunk)):
+            i1 = min(I, i0 + chunk)
+            g = _gen(cfg.seed * 1000003 + 1000 + r, dev)
+            out[i0:i1] = torch.randn(i1 - i0, I, cz, generator=g, device=dev, dtype=torch.float32).to(out.dtype)
+        return out
+    n = cfg.n_res
+    E, R = _tables(cfg, dev)
+    if cyclic_copy_table:
+        F = E[0]  # [copies, c_z]
+        a = torch.arange(cfg.copies, device=dev)
+        E = F[(a[None, :] - a[:, None]) % cfg.copies]
+    idx = torch.arange(I, device=dev)
+    copy_j, res_j = idx // n, idx % n
+    if chunk_rows <= 0:
+        # ~256 MB of fp32 temporaries per chunk
+        chunk_rows = max(1, min(I, (64 << 20) // max(1, I * cz)))
+    for r, i0 in enumerate(range(0, I, chunk_rows)):
+        i1 = min(I, i0 + chunk_rows)
+        ci, ri = copy_j[i0:i1], res_j[i0:i1]
+        blk = E[ci][:, copy_j] + R[ri][:, res_j]
+        if noise != 0.0:
+            g = _gen(cfg.seed * 1000003 + 1000 + r, dev)
+            blk += noise * torch.randn(i1 - i0, I, cz, generator=g, device=dev, dtype=torch.float32)
+        out[i0:i1] = blk.to(out.dtype)
+        del blk
+    return out
+
+
+def make_z(cfg: LayerConfig, device="cpu", **kw) -> torch.Tensor:
+    out = torch.empty(cfg.I, cfg.I, cfg.c_z, dtype=torch_dtype(cfg.dtype), device=device)
+    return fill_z(cfg, out, **kw)
+
+
+def small_config(name: str, I: int, c_s: int, c_z: int, H: int, c: int, dtype: str = "f32",
+                 seed: int = 7, structured: bool = False, copies: int = COPIES) -> LayerConfig:
+    """Helper for tests: arbitrary small shapes (ragged tails, odd sizes)."""
+    return LayerConfig(name, I=I, c_s=c_s, c_z=c_z, H=H, c=c, dtype=dtype, seed=seed,
+                       structured=structured, copies=copies)
+
+
+def sample_rows(I: int, count: int, boundaries=(), seed: int = 0):
+    """Query rows for sampled parity at sizes the oracle cannot cover in full: first/last row,
+    both sides of every given boundary, plus seeded random rows."""
+    rows = {0, I - 1}
+    for b in boundaries:
+        for r in (b - 1, b):
+            if 0 <= r < I:
+                rows.add(int(r))
+    g = _gen(seed + 99, "cpu")
+    while len(rows) < min(count, I):
+        rows.add(int(torch.randint(0, I, (1,), generator=g)))
+    return sorted(rows)

@@ -1,0 +1,320 @@
+"""Pins for the CPU fp64 oracle (`-m "not gpu"`): each test fixes the oracle against something
+other than itself -- a hand-derived worked example, brute force, closed forms, invariants,
+library routines -- so that a dropped term, a wrong sign/index or a transposed operand fails.
+Citations: PAPER.md:58, :72 (Eq. 1), :83 (Eq. 2), :90, :337 (Eq. 5); SURVEY.md section 8(c).
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import brute
+from oracle import decompositions as dec
+from oracle import pair_bias_attention as orc
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def rand_problem(rng, I, c_s, c_z, H, c, ln_s=False, b_q=False):
+    D = H * c
+    w = {
+        "w_q": rng.normal(size=(c_s, D)) / math.sqrt(c_s),
+        "w_k": rng.normal(size=(c_s, D)) / math.sqrt(c_s),
+        "w_v": rng.normal(size=(c_s, D)) / math.sqrt(c_s),
+        "w_g": rng.normal(size=(c_s, D)) / math.sqrt(c_s),
+        "w_b": rng.normal(size=(c_z, H)) / math.sqrt(c_z),
+        "w_o": rng.normal(size=(D, c_s)) / math.sqrt(D),
+        "ln_z_gamma": 1 + 0.1 * rng.normal(size=c_z),
+        "ln_z_beta": 0.1 * rng.normal(size=c_z),
+    }
+    if ln_s:
+        w["ln_s_gamma"] = 1 + 0.1 * rng.normal(size=c_s)
+        w["ln_s_beta"] = 0.1 * rng.normal(size=c_s)
+    if b_q:
+        w["b_q"] = 0.1 * rng.normal(size=D)
+    s = rng.normal(size=(I, c_s))
+    z = rng.normal(size=(I, I, c_z))
+    return s, z, w
+
+
+# ---------------------------------------------------------------- worked example (golden file)
+def _golden():
+    vals = {}
+    with open(os.path.join(HERE, "golden", "worked_example.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            k, v = line.split()
+            vals[k] = float(v)
+    return vals
+
+
+def _worked_problem():
+    s = np.array([[1.0], [-0.5]])
+    z = np.array([[[1.0, 3.0], [2.0, 0.0]], [[0.0, 4.0], [5.0, 1.0]]])
+    w = {"w_q": [[2.0]], "w_k": [[1.0]], "w_v": [[3.0]], "w_g": [[0.0]], "w_o": [[2.0]],
+         "w_b": [[0.75], [-0.25]], "ln_z_gamma": [1.0, 1.0], "ln_z_beta": [0.0, 0.0]}
+    return s, z, w
+
+
+def test_worked_example_matches_golden():
+    g = _golden()
+    s, z, w = _worked_problem()
+    out = orc.pair_bias_attention(s, z, w, H=1, c=1, eps=1e-5)
+    assert out.shape == (2, 1)
+    assert abs(out[0, 0] - g["out0"]) < 1e-13
+    assert abs(out[1, 0] - g["out1"]) < 1e-13
+    # the golden values themselves follow the hand derivation written in the file header
+    r, rp = 1 / math.sqrt(1 + 1e-5 / 1.0), 1 / math.sqrt(1 + 1e-5 / 4.0)
+    assert abs(r - g["r"]) < 1e-15 and abs(rp - g["r_prime"]) < 1e-15
+    a00 = 1 / (1 + math.exp((-1 + r) - (2 - r)))
+    a10 = 1 / (1 + math.exp((0.5 + rp) - (-1 - rp)))
+    assert abs(a00 - g["a00"]) < 1e-15 and abs(a10 - g["a10"]) < 1e-15
+    assert abs(4.5 * a00 - 1.5 - g["out0"]) < 1e-13 and abs(4.5 * a10 - 1.5 - g["out1"]) < 1e-13
+    # bias rows of the worked example: b00=-r, b01=+r, b10=-r', b11=+r'
+    b0 = orc.pair_bias_row(z[0], w, 1e-5)[:, 0]
+    b1 = orc.pair_bias_row(z[1], w, 1e-5)[:, 0]
+    assert np.allclose(b0, [-r, r], atol=1e-15) and np.allclose(b1, [-rp, rp], atol=1e-15)
+
+
+# ---------------------------------------------------------------- brute force on tiny inputs
+@pytest.mark.parametrize("I,c_s,c_z,H,c,ln_s,b_q", [
+    (5, 6, 3, 2, 4, False, False),     # H*c != c_s, c_z not a power of two
+    (16, 8, 5, 3, 2, True, True),      # optional LN_s and b_q
+    (7, 4, 1, 1, 3, False, False),     # c_z = 1
+    (1, 3, 4, 2, 2, False, False),     # single token
+])
+def test_brute_force_agreement(I, c_s, c_z, H, c, ln_s, b_q):
+    rng = np.random.default_rng(100 + I)
+    s, z, w = rand_problem(rng, I, c_s, c_z, H, c, ln_s, b_q)
+    out = orc.pair_bias_attention(s, z, w, H, c)
+    ref = brute.brute_force(
+        s.tolist(), z.tolist(), w["w_q"].tolist(), w["w_k"].tolist(), w["w_v"].tolist(),
+        w["w_g"].tolist(), w["w_b"].tolist(), w["w_o"].tolist(), w["ln_z_gamma"].tolist(),
+        w["ln_z_beta"].tolist(), H, c,
+        ln_s=(w["ln_s_gamma"].tolist(), w["ln_s_beta"].tolist()) if ln_s else None,
+        b_q=w["b_q"].tolist() if b_q else None)
+    ref = np.array(ref)
+    assert np.max(np.abs(out - ref)) <= 1e-12 * max(1.0, np.max(np.abs(ref)))
+
+
+# ---------------------------------------------------------------- closed forms
+def test_uniform_attention_closed_form():
+    """W_b = 0 and identical keys (W_k = 0) => uniform attention => out_i = (g_i * mean_j v_j) W_o."""
+    rng = np.random.default_rng(1)
+    I, c_s, c_z, H, c = 23, 12, 6, 3, 4
+    s, z, w = rand_problem(rng, I, c_s, c_z, H, c)
+    w["w_b"] = np.zeros_like(w["w_b"])
+    w["ln_z_beta"] = np.zeros_like(w["ln_z_beta"])
+    w["w_k"] = np.zeros_like(w["w_k"])
+    out = orc.pair_bias_attention(s, z, w, H, c)
+    g = 1 / (1 + np.exp(-(s @ w["w_g"])))
+    ref = (g * (s @ w["w_v"]).mean(axis=0)) @ w["w_o"]
+    assert np.max(np.abs(out - ref)) < 1e-13
+
+
+def test_constant_values_closed_form():
+    """All v_j equal u (rows of s equal except through W_v... use W_v rows so that v_j=u) => o_i = u."""
+    rng = np.random.default_rng(2)
+    I, c_s, c_z, H, c = 11, 5, 4, 2, 3
+    s, z, w = rand_problem(rng, I, c_s, c_z, H, c)
+    s[:, 0] = 1.0                       # constant feature
+    w["w_v"][1:, :] = 0.0               # v_j = W_v[0,:] for every j
+    out = orc.pair_bias_attention(s, z, w, H, c)
+    g = 1 / (1 + np.exp(-(s @ w["w_g"])))
+    ref = (g * w["w_v"][0]) @ w["w_o"]
+    assert np.max(np.abs(out - ref)) < 1e-13
+
+
+def test_single_key_limit():
+    rng = np.random.default_rng(3)
+    s, z, w = rand_problem(rng, 1, 7, 5, 2, 3)
+    out = orc.pair_bias_attention(s, z, w, 2, 3)
+    g = 1 / (1 + np.exp(-(s @ w["w_g"])))
+    assert np.max(np.abs(out - (g * (s @ w["w_v"])) @ w["w_o"])) < 1e-14
+
+
+def test_one_hot_limit_pins_orientation_of_z():
+    """Bias +50 at j = pi(i), -50 elsewhere => out_i -> (g_i * v_pi(i)) W_o; a transposed z fails."""
+    rng = np.random.default_rng(4)
+    I, c_s, c_z, H, c = 9, 6, 2, 2, 3
+    s, _, w = rand_problem(rng, I, c_s, c_z, H, c)
+    pi = np.roll(np.arange(I), 2)                    # non-involutive permutation (a 9-cycle shift)
+    assert not np.array_equal(pi[pi], np.arange(I))
+    # c_z = 2: LN(z) = (+r, -r) or (-r, +r); with W_b = (A, -A) the bias is +-2 A r for every head
+    z = np.zeros((I, I, 2))
+    z[..., 0], z[..., 1] = -1.0, 1.0                  # bias = -2Ar
+    for i in range(I):
+        z[i, pi[i]] = (1.0, -1.0)                     # bias = +2Ar at j = pi(i)
+    w["ln_z_gamma"] = np.ones(2)
+    w["ln_z_beta"] = np.zeros(2)
+    w["w_b"] = np.tile(np.array([[25.0], [-25.0]]), (1, H))
+    out = orc.pair_bias_attention(s, z, w, H, c)
+    g = 1 / (1 + np.exp(-(s @ w["w_g"])))
+    v = s @ w["w_v"]
+    ref = (g * v[pi]) @ w["w_o"]
+    assert np.max(np.abs(out - ref)) < 1e-12
+    wrong = (g * v[np.argsort(pi)]) @ w["w_o"]       # what a transposed read of z would give
+    assert np.max(np.abs(out - wrong)) > 1e-3
+    out_t = orc.pair_bias_attention(s, np.swapaxes(z, 0, 1).copy(), w, H, c)
+    assert np.max(np.abs(out_t - ref)) > 1e-3
+
+
+def test_layernorm_invariances():
+    """z_ij -> a_ij z_ij + t_ij 1 (a > 0) leaves the bias unchanged for eps = 0; c_z = 1 => zhat = beta."""
+    rng = np.random.default_rng(5)
+    I, c_s, c_z, H, c = 8, 5, 7, 2, 2
+    s, z, w = rand_problem(rng, I, c_s, c_z, H, c)
+    a = rng.uniform(0.5, 3.0, size=(I, I, 1))
+    t = rng.normal(size=(I, I, 1))
+    o1 = orc.pair_bias_attention(s, z, w, H, c, eps=0.0)
+    o2 = orc.pair_bias_attention(s, a * z + t, w, H, c, eps=0.0)
+    assert np.max(np.abs(o1 - o2)) < 1e-12
+    # c_z = 1: constant bias per head => equals bias-free attention (softmax shift invariance)
+    s, z, w = rand_problem(rng, I, c_s, 1, H, c)
+    w0 = dict(w)
+    w0["w_b"] = np.zeros_like(w["w_b"])
+    assert np.max(np.abs(orc.pair_bias_attention(s, z, w, H, c)
+                         - orc.pair_bias_attention(s, z, w0, H, c))) < 1e-13
+
+
+def test_library_composition_torch_fp64():
+    """Third independent check: torch fp64 layer_norm + linear + scaled_dot_product_attention."""
+    rng = np.random.default_rng(6)
+    I, c_s, c_z, H, c = 96, 24, 16, 4, 6
+    s, z, w = rand_problem(rng, I, c_s, c_z, H, c, ln_s=True, b_q=True)
+    out = orc.pair_bias_attention(s, z, w, H, c, eps=1e-5)
+    T = lambda x: torch.tensor(np.asarray(x), dtype=torch.float64)
+    F = torch.nn.functional
+    st = F.layer_norm(T(s), (c_s,), T(w["ln_s_gamma"]), T(w["ln_s_beta"]), 1e-5)
+    q = (st @ T(w["w_q"]) + T(w["b_q"])).view(I, H, c).transpose(0, 1)
+    k = (st @ T(w["w_k"])).view(I, H, c).transpose(0, 1)
+    v = (st @ T(w["w_v"])).view(I, H, c).transpose(0, 1)
+    b = F.layer_norm(T(z), (c_z,), T(w["ln_z_gamma"]), T(w["ln_z_beta"]), 1e-5) @ T(w["w_b"])
+    o = F.scaled_dot_product_attention(q[None], k[None], v[None], attn_mask=b.permute(2, 0, 1)[None])[0]
+    o = o.transpose(0, 1).reshape(I, H * c)
+    ref = (torch.sigmoid(st @ T(w["w_g"])) * o) @ T(w["w_o"])
+    assert np.max(np.abs(out - ref.numpy())) < 1e-12
+
+
+# ---------------------------------------------------------------- symmetry
+def test_permutation_equivariance():
+    rng = np.random.default_rng(7)
+    I, c_s, c_z, H, c = 17, 6, 5, 2, 3
+    s, z, w = rand_problem(rng, I, c_s, c_z, H, c)
+    pi = rng.permutation(I)
+    o = orc.pair_bias_attention(s, z, w, H, c)
+    op = orc.pair_bias_attention(s[pi], z[pi][:, pi], w, H, c)
+    assert np.max(np.abs(op - o[pi])) < 1e-12
+
+
+def test_cyclic_copy_shift_invariance():
+    """Noise-free generator with a cyclic copy table E[a,b] = F[(b-a) mod C] is invariant under
+    copy shifts => the output is periodic over copies (echoes the paper's symmetric assemblies,
+    PAPER.md:325-327)."""
+    import dcp_synth as syn
+    cfg = syn.small_config("cyc", I=5 * 4, c_s=6, c_z=4, H=2, c=3, structured=True, copies=5, seed=11)
+    w = {k: v.double().numpy() for k, v in syn.make_weights(cfg).items()}
+    # noise-free s: repeat the ASU block exactly
+    rng = np.random.default_rng(8)
+    a = rng.normal(size=(cfg.n_res, cfg.c_s))
+    s = np.tile(a, (cfg.copies, 1))
+    z = syn.make_z(cfg, noise=0.0, cyclic_copy_table=True).double().numpy()
+    o = orc.pair_bias_attention(s, z, w, cfg.H, cfg.c)
+    o = o.reshape(cfg.copies, cfg.n_res, -1)
+    assert np.max(np.abs(o - o[0:1])) < 1e-12
+
+
+# ---------------------------------------------------------------- Eq. 5 planner
+def test_shard_range_closed_form_exhaustive():
+    for n in range(0, 201):
+        for P in range(1, 18):
+            tot, prev_end, sizes = 0, 0, []
+            for p in range(P):
+                st, ln = dec.shard_range(n, P, p)
+                assert st == prev_end                      # start_{p+1} = start_p + I_p
+                assert ln == n // P + (1 if p < n % P else 0)   # Eq. 1
+                prev_end = st + ln
+                tot += ln
+                sizes.append(ln)
+            assert tot == n and max(sizes) - min(sizes) <= 1
+    # the paper's examples of uneven splits
+    assert [dec.shard_range(67, 4, p)[1] for p in range(4)] == [17, 17, 17, 16]
+    assert [dec.shard_range(600, 7, p)[1] for p in range(7)] == [86, 86, 86, 86, 86, 85, 85]
+
+
+def test_grid_needs_perfect_square():
+    assert dec.grid_side(16) == 4 and dec.grid_side(1) == 1
+    for bad in (2, 3, 8, 15):
+        with pytest.raises(ValueError):
+            dec.grid_side(bad)
+
+
+# ---------------------------------------------------------------- merge operator
+def test_merge_algebra_and_extremes():
+    rng = np.random.default_rng(9)
+    R, H, c = 4, 3, 5
+
+    def state(shift):
+        m = rng.normal(size=(R, H)) + shift
+        return m, rng.uniform(0.5, 2, size=(R, H)), rng.normal(size=(R, H, c))
+
+    a, b, cst = state(0), state(80.0), state(-80.0)
+    ab_c = dec.merge(dec.merge(a, b), cst)
+    a_bc = dec.merge(a, dec.merge(b, cst))
+    ba = dec.merge(b, a)
+    for x, y in zip(ab_c, a_bc):
+        assert np.all(np.isfinite(x)) and np.allclose(x, y, rtol=1e-12, atol=0)
+    for x, y in zip(dec.merge(a, b), ba):
+        assert np.allclose(x, y, rtol=1e-14, atol=0)
+    m2, l2, acc2 = dec.merge(a, a)                       # self-merge doubles l and acc, keeps m
+    assert np.array_equal(m2, a[0]) and np.allclose(l2, 2 * a[1]) and np.allclose(acc2, 2 * a[2])
+
+
+# ---------------------------------------------------------------- decompositions agree with the dense definition
+@pytest.mark.parametrize("I", [12, 13, 30])
+def test_row_and_grid_agree_with_dense(I):
+    rng = np.random.default_rng(10 + I)
+    c_s, c_z, H, c = 6, 5, 2, 3
+    s, z, w = rand_problem(rng, I, c_s, c_z, H, c)
+    o = orc.pair_bias_attention(s, z, w, H, c)
+    scale = np.max(np.abs(o))
+    for P in list(range(1, I + 1, max(1, I // 6))) + [I]:
+        assert np.max(np.abs(dec.row_decomposition(s, z, w, H, c, P) - o)) <= 1e-12 * scale
+    for P in (1, 4, 9, 16):
+        if math.isqrt(P) <= I:
+            assert np.max(np.abs(dec.grid_decomposition(s, z, w, H, c, P) - o)) <= 1e-12 * scale
+            assert np.max(np.abs(dec.grid_decomposition(s, z, w, H, c, P, first_block_offset=True) - o)) \
+                <= 1e-12 * scale
+    with pytest.raises(ValueError):
+        dec.grid_decomposition(s, z, w, H, c, 8)
+
+
+def test_key_split_states_merge_to_dense():
+    rng = np.random.default_rng(11)
+    I, c_s, c_z, H, c = 21, 6, 4, 2, 3
+    s, z, w = rand_problem(rng, I, c_s, c_z, H, c)
+    rows = [0, 5, 20]
+    states = dec.key_split_states(s, z[rows], rows, w, H, c, key_chunks=4)
+    st = states[0]
+    for nxt in states[1:]:
+        st = dec.merge(st, nxt)
+    _, _, _, g = orc.single_track(s, w, H, c)
+    out = dec.finalize(st, g[rows], w["w_o"])
+    ref = orc.pair_bias_attention_rows(s, z[rows], rows, w, H, c)
+    assert np.max(np.abs(out - ref)) < 1e-12
+
+
+# ---------------------------------------------------------------- generator determinism
+def test_input_generator_is_seed_deterministic():
+    import dcp_synth as syn
+    cfg = syn.small_config("g", I=60 * 2, c_s=8, c_z=4, H=2, c=4, dtype="bf16", structured=True, seed=5)
+    z1, z2 = syn.make_z(cfg, chunk_rows=16), syn.make_z(cfg, chunk_rows=16)
+    assert torch.equal(z1, z2)
+    assert torch.equal(syn.make_s(cfg), syn.make_s(cfg))
+    w1, w2 = syn.make_weights(cfg), syn.make_weights(cfg)
+    assert all(torch.equal(w1[k], w2[k]) for k in w1)
+    cfg2 = syn.small_config("g", I=60 * 2, c_s=8, c_z=4, H=2, c=4, dtype="bf16", structured=True, seed=6)
+    assert not torch.equal(z1, syn.make_z(cfg2, chunk_rows=16))
