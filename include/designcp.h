@@ -1,0 +1,148 @@
+/* libdesigncp -- attention with pair bias on one B200 (sm_100a): the one-GPU core that Design-CP
+ * (arxiv/paper_2607_05439) distributes.  Plain C ABI: pointers and sizes only, no torch types.
+ *
+ * The layer (citations are lines of /root/reference/PAPER.md; readings in DESIGN.md):
+ *   PAPER.md:58  (sec 3.1)  "a learned projection of Z produces a per-head pair bias B in R^{IxIxH} that is
+ *                            added to the attention logits before the softmax, softmax(QK^T/sqrt(d) + B)"
+ *   PAPER.md:83  (Eq. 2)    Attn^(p) = softmax(Q^(p) K^T / sqrt(d) + B^(p)) V,  B^(p) = f_B(Z^(p)) in R^{I_p x I x H}
+ *   BASELINE.json config 0  out = W_o ( sigmoid(s W_g) (.) softmax(Q K^T/sqrt(c) + LN(z) W_b) V )
+ *   PAPER.md:72 (Eq. 1), :337 (Eq. 5)  row shards  I_p = floor(I/P)+[p < I mod P], start_p = p floor(I/P)+min(p, I mod P)
+ *   PAPER.md:90 (sec 3.3), :446 (C.2)  sqrt(P) x sqrt(P) grid; partial outputs merged by an online softmax
+ *
+ * Layout: every tensor is row-major, last index fastest.
+ *   s   [I, c_s]        single track                        z   [I, I, c_z]   z[i, j, :] biases query i <- key j
+ *   W_q, W_k, W_v, W_g [c_s, H*c] (column h*c+d = head h, channel d)   W_b [c_z, H]   W_o [H*c, c_s]
+ *   out [I, c_s]
+ * dtype is the STORAGE type of s, z, the weights and out (DCP_F32 or DCP_BF16); all accumulation is fp32.
+ *
+ * Ownership: the caller owns every buffer.  The library allocates nothing persistent, keeps no global state
+ * (except a one-time cudaFuncSetAttribute per kernel) and is re-entrant.  Inputs are read-only and must not
+ * alias out/workspace.  Unless a function says HOST, pointers are DEVICE pointers on the current device.
+ * Asynchrony: work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = default stream) and the
+ * call returns after the launches.  DCP_ERR_CUDA reports launch-time errors; execution errors surface at the
+ * caller's next synchronisation.  No function aborts or throws.
+ */
+#ifndef DESIGNCP_H
+#define DESIGNCP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  DCP_OK = 0,
+  DCP_ERR_INVALID_ARG = 1, /* null pointer, non-positive size, parts > I, GRID with non-square parts,
+                              misaligned pointer / pitch (16 B), c_z*sizeof(elt) % 16 != 0                         */
+  DCP_ERR_UNSUPPORTED = 2, /* a (dtype, H, c, c_z) the kernels are not instantiated for                           */
+  DCP_ERR_WORKSPACE = 3,   /* workspace too small (see dcp_workspace_bytes)                                       */
+  DCP_ERR_CUDA = 4         /* a CUDA runtime / driver call failed at launch time                                  */
+} dcp_status;
+
+typedef enum { DCP_F32 = 0, DCP_BF16 = 1 } dcp_dtype;
+
+/* How the layer is cut (the on-device emulation of Design-CP's schemes):
+ *   MONOLITHIC  one problem; keys processed as `key_split` Eq.-5 chunks merged left to right
+ *   ROW         PAPER.md:72-86: `parts` query stripes (Eq. 5), each against ALL keys, one launch per stripe
+ *   GRID        PAPER.md:90: G x G quadrants, G = sqrt(parts) (parts must be a perfect square), one launch per
+ *               quadrant producing a partial (m, l, acc); the G key blocks of a row are merged left to right  */
+typedef enum { DCP_MONOLITHIC = 0, DCP_ROW = 1, DCP_GRID = 2 } dcp_decomp;
+
+/* Which fused kernel runs the (query-tile, key-tile) loop. */
+typedef enum {
+  DCP_KERNEL_AUTO = 0,   /* fastest kernel instantiated for the shape                                            */
+  DCP_KERNEL_GENERIC = 1,/* fp32 CUDA-core kernel: any shape with H <= 16, H*c % 32 == 0, H*c <= 768             */
+  DCP_KERNEL_MMA = 2     /* bf16 tensor-core kernel (TMA-streamed z): DCP_BF16 only, shapes of configs 1-4       */
+} dcp_kernel;
+
+typedef struct {
+  const void *w_q, *w_k, *w_v, *w_g; /* [c_s, H*c]                                                */
+  const void *w_b;                   /* [c_z, H]                                                  */
+  const void *w_o;                   /* [H*c, c_s]                                                */
+  const void *ln_z_gamma, *ln_z_beta;/* [c_z]    LayerNorm over the channel axis of z             */
+  const void *ln_s_gamma, *ln_s_beta;/* [c_s] or both NULL = no LayerNorm on s (BASELINE formula) */
+  const void *b_q;                   /* [H*c] or NULL                                             */
+  float ln_eps;                      /* <= 0 means 1e-5                                           */
+} dcp_weights;
+
+typedef struct {
+  int parts;     /* ROW: number of stripes, 1 <= parts <= I.  GRID: P, a perfect square with sqrt(P) <= I.
+                    MONOLITHIC: ignored.                                                                 */
+  int key_split; /* MONOLITHIC / ROW: key chunks (Eq. 5) merged left to right; <= 0 means 1.  GRID: ignored
+                    (the key axis is cut into sqrt(parts) blocks).                                       */
+  int kernel;    /* a dcp_kernel                                                                         */
+  void *ev_fused_begin, *ev_fused_end; /* optional cudaEvent_t (from dcp_event_create): recorded on `stream` just
+                    before the first and just after the last fused-kernel launch of the call (bench.py times the
+                    dominant kernel with them); NULL = not recorded                                       */
+} dcp_plan;
+
+/* Bytes of device workspace dcp_pair_bias_attention needs for this problem (q,k,v,g, the partial states
+ * [chunks][I][H] x2 and [chunks][I][H*c] fp32, the gated activations, folded weights).  `plan` may be NULL
+ * (MONOLITHIC defaults). */
+dcp_status dcp_workspace_bytes(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype,
+                               dcp_decomp decomp, const dcp_plan *plan, size_t *bytes);
+
+/* The layer.  z is read exactly once; the I*I*H logits never reach memory.
+ * ldz = elements between z[i,0,0] and z[i+1,0,0] (0 means I*c_z); lets z be a view of a larger tensor.
+ * workspace: device, 256-byte aligned, >= dcp_workspace_bytes(...).  The result does not depend on `decomp`
+ * beyond rounding. */
+dcp_status dcp_pair_bias_attention(const void *s, const void *z, int64_t ldz, const dcp_weights *w, void *out,
+                                   int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype,
+                                   dcp_decomp decomp, const dcp_plan *plan,
+                                   void *workspace, size_t workspace_bytes, void *stream);
+
+/* Atom-level dense variant ("an analogous pair representation P in R^{LxLxc_atompair}";
+ * BASELINE.json config 4): the same computation with (L, c_atom, c_atompair) for (I, c_s, c_z). */
+dcp_status dcp_atom_pair_bias_attention(const void *a, const void *p, int64_t ldp, const dcp_weights *w,
+                                        void *out, int64_t L, int c_atom, int H, int c, int c_atompair,
+                                        dcp_dtype dtype, dcp_decomp decomp, const dcp_plan *plan,
+                                        void *workspace, size_t workspace_bytes, void *stream);
+
+/* End-to-end entry with HOST inputs/outputs: s_host, z_host, out_host are HOST pointers (pinned memory gives
+ * full PCIe rate); weights stay device-resident (they are parameters, not per-step inputs).  Copies s and z
+ * to the device staging buffers s_dev [I,c_s], z_dev [I,I,c_z], runs the layer, copies out back, all on
+ * `stream`.  Returns after enqueueing; synchronise the stream before reading out_host. */
+dcp_status dcp_pair_bias_attention_host(const void *s_host, const void *z_host, const dcp_weights *w,
+                                        void *out_host, void *s_dev, void *z_dev, void *out_dev,
+                                        int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype,
+                                        dcp_decomp decomp, const dcp_plan *plan,
+                                        void *workspace, size_t workspace_bytes, void *stream);
+
+/* Diagnostic: the partial online-softmax state of query rows [q0,q1) against keys [k0,k1) only:
+ * m [q1-q0, H] = max_j logit, l [q1-q0, H] = sum_j e^{logit-m}, acc [q1-q0, H*c] = sum_j e^{logit-m} v_j (fp32). */
+dcp_status dcp_partial_states(const void *s, const void *z, int64_t ldz, const dcp_weights *w,
+                              int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype, int kernel,
+                              int64_t q0, int64_t q1, int64_t k0, int64_t k1,
+                              float *m, float *l, float *acc,
+                              void *workspace, size_t workspace_bytes, void *stream);
+
+/* The merge kernel alone: left fold over `n_parts` partial states of `rows` rows:
+ * m' = max(m_a, m_b), l' = l_a e^{m_a-m'} + l_b e^{m_b-m'}, acc' likewise.  m, l: [n_parts, rows, H];
+ * acc: [n_parts, rows, H*c]; outputs m_out, l_out [rows, H], acc_out [rows, H*c].  All fp32, device. */
+dcp_status dcp_merge_states(int n_parts, int64_t rows, int H, int c, const float *m, const float *l,
+                            const float *acc, float *m_out, float *l_out, float *acc_out, void *stream);
+
+/* Eq. 5, host only: shard p of n items over `parts` shards. */
+dcp_status dcp_shard_range(int64_t n, int parts, int p, int64_t *start, int64_t *len);
+
+/* 1 if fused kernel `kernel` (a dcp_kernel, not AUTO) is instantiated for this (dtype, H, c, c_z), else 0. Host only. */
+int dcp_kernel_supported(int kernel, dcp_dtype dtype, int H, int c, int c_z);
+
+/* CUDA-event helpers for callers without a CUDA runtime binding (bench.py): timing-enabled events. */
+dcp_status dcp_event_create(void **ev);
+dcp_status dcp_event_record(void *ev, void *stream);
+dcp_status dcp_event_elapsed_ms(void *ev_begin, void *ev_end, float *ms); /* synchronises on ev_end */
+dcp_status dcp_event_destroy(void *ev);
+
+/* Number of kernels the last dcp_pair_bias_attention* call on this thread launched (bench.py's gpu_launches). */
+int dcp_last_launch_count(void);
+
+const char *dcp_status_string(dcp_status st);
+int dcp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DESIGNCP_H */

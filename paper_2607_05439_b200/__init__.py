@@ -1,0 +1,11 @@
+"""paper_2607_05439_b200 -- B200-native pair-bias attention (the one-GPU core of Design-CP).
+
+`csrc/` holds the CUDA kernels and the C ABI (include/designcp.h); `binding.py` is the thin
+ctypes layer with the same names.  Importing the package requires the built library
+(`python paper_2607_05439_b200/build.py`); there is no CPU fallback.
+"""
+from .binding import (  # noqa: F401
+    DcpError, Event, dcp_atom_pair_bias_attention, dcp_kernel_supported, dcp_last_launch_count, dcp_merge_states,
+    dcp_pair_bias_attention, dcp_pair_bias_attention_host, dcp_partial_states, dcp_shard_range,
+    dcp_workspace_bytes, status_string, version,
+)

@@ -1,0 +1,266 @@
+"""Thin ctypes binding of libdesigncp (include/designcp.h): argument marshalling only.
+
+Every step of the hot path runs inside the library's CUDA kernels; torch is used here only to
+hold device memory and to name the current stream.  There is NO CPU fallback: importing this
+module raises if libdesigncp.so is missing, and every call raises on a non-OK status.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional
+
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libdesigncp.so")
+
+DCP_OK = 0
+DCP_ERR_INVALID_ARG, DCP_ERR_UNSUPPORTED, DCP_ERR_WORKSPACE, DCP_ERR_CUDA = 1, 2, 3, 4
+DCP_F32, DCP_BF16 = 0, 1
+DCP_MONOLITHIC, DCP_ROW, DCP_GRID = 0, 1, 2
+DCP_KERNEL_AUTO, DCP_KERNEL_GENERIC, DCP_KERNEL_MMA = 0, 1, 2
+
+DECOMP = {"monolithic": DCP_MONOLITHIC, "row": DCP_ROW, "grid": DCP_GRID}
+KERNEL = {"auto": DCP_KERNEL_AUTO, "generic": DCP_KERNEL_GENERIC, "mma": DCP_KERNEL_MMA}
+
+EXPORTS = [
+    "dcp_workspace_bytes", "dcp_pair_bias_attention", "dcp_atom_pair_bias_attention",
+    "dcp_pair_bias_attention_host", "dcp_partial_states", "dcp_merge_states", "dcp_shard_range",
+    "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
+    "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
+]
+
+
+class DcpError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {status_string(status)}")
+
+
+class dcp_weights(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in (
+        "w_q", "w_k", "w_v", "w_g", "w_b", "w_o", "ln_z_gamma", "ln_z_beta", "ln_s_gamma", "ln_s_beta", "b_q")]
+    _fields_ += [("ln_eps", C.c_float)]
+
+
+class dcp_plan(C.Structure):
+    _fields_ = [("parts", C.c_int), ("key_split", C.c_int), ("kernel", C.c_int),
+                ("ev_fused_begin", C.c_void_p), ("ev_fused_end", C.c_void_p)]
+
+
+def _load() -> C.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python paper_2607_05439_b200/build.py` "
+            "(there is no CPU fallback for the product path)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i64, i32, sz = C.c_void_p, C.c_int64, C.c_int, C.c_size_t
+    lib.dcp_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, i32, i32, C.POINTER(dcp_plan), C.POINTER(sz)]
+    layer_args = [vp, vp, i64, C.POINTER(dcp_weights), vp, i64, i32, i32, i32, i32, i32, i32,
+                  C.POINTER(dcp_plan), vp, sz, vp]
+    lib.dcp_pair_bias_attention.argtypes = layer_args
+    lib.dcp_atom_pair_bias_attention.argtypes = layer_args
+    lib.dcp_pair_bias_attention_host.argtypes = [vp, vp, C.POINTER(dcp_weights), vp, vp, vp, vp, i64, i32, i32, i32,
+                                                 i32, i32, i32, C.POINTER(dcp_plan), vp, sz, vp]
+    lib.dcp_partial_states.argtypes = [vp, vp, i64, C.POINTER(dcp_weights), i64, i32, i32, i32, i32, i32, i32,
+                                       i64, i64, i64, i64, vp, vp, vp, vp, sz, vp]
+    lib.dcp_merge_states.argtypes = [i32, i64, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.dcp_shard_range.argtypes = [i64, i32, i32, C.POINTER(i64), C.POINTER(i64)]
+    lib.dcp_event_create.argtypes = [C.POINTER(vp)]
+    lib.dcp_event_record.argtypes = [vp, vp]
+    lib.dcp_event_elapsed_ms.argtypes = [vp, vp, C.POINTER(C.c_float)]
+    lib.dcp_event_destroy.argtypes = [vp]
+    for n in ("dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy"):
+        getattr(lib, n).restype = i32
+    lib.dcp_kernel_supported.argtypes = [i32, i32, i32, i32, i32]
+    lib.dcp_kernel_supported.restype = i32
+    lib.dcp_last_launch_count.restype = i32
+    lib.dcp_status_string.argtypes = [i32]
+    lib.dcp_status_string.restype = C.c_char_p
+    lib.dcp_version.restype = i32
+    for n in EXPORTS[:7]:
+        getattr(lib, n).restype = i32
+    return lib
+
+
+_lib = _load()
+
+
+def status_string(st: int) -> str:
+    return _lib.dcp_status_string(int(st)).decode()
+
+
+def version() -> int:
+    return int(_lib.dcp_version())
+
+
+def _check(st: int, where: str):
+    if st != DCP_OK:
+        raise DcpError(st, where)
+
+
+def _dtype_code(t: torch.dtype) -> int:
+    if t == torch.float32:
+        return DCP_F32
+    if t == torch.bfloat16:
+        return DCP_BF16
+    raise TypeError(f"libdesigncp stores f32 or bf16, not {t}")
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream_ptr(stream=None):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def _weights_struct(w: Dict[str, torch.Tensor], eps: float) -> dcp_weights:
+    ws = dcp_weights()
+    for name in ("w_q", "w_k", "w_v", "w_g", "w_b", "w_o", "ln_z_gamma", "ln_z_beta"):
+        t = w[name]
+        assert t.is_cuda and t.is_contiguous(), name
+        setattr(ws, name, t.data_ptr())
+    for name in ("ln_s_gamma", "ln_s_beta", "b_q"):
+        t = w.get(name)
+        setattr(ws, name, None if t is None else t.data_ptr())
+    ws.ln_eps = float(eps)
+    return ws
+
+
+def _plan(parts: int, key_split: int, kernel, events=None) -> dcp_plan:
+    k = KERNEL[kernel] if isinstance(kernel, str) else int(kernel)
+    e0, e1 = (events if events is not None else (None, None))
+    return dcp_plan(int(parts), int(key_split), k, e0, e1)
+
+
+class Event:
+    """A timing-enabled cudaEvent_t owned through the C ABI (dcp_event_*)."""
+
+    def __init__(self):
+        h = C.c_void_p()
+        _check(_lib.dcp_event_create(C.byref(h)), "dcp_event_create")
+        self.handle = h
+
+    def record(self, stream=None):
+        _check(_lib.dcp_event_record(self.handle, _stream_ptr(stream)), "dcp_event_record")
+
+    def elapsed_ms(self, end: "Event") -> float:
+        ms = C.c_float()
+        _check(_lib.dcp_event_elapsed_ms(self.handle, end.handle, C.byref(ms)), "dcp_event_elapsed_ms")
+        return float(ms.value)
+
+    def __del__(self):
+        try:
+            _lib.dcp_event_destroy(self.handle)
+        except Exception:
+            pass
+
+
+def dcp_shard_range(n: int, parts: int, p: int):
+    """Eq. 5, host only."""
+    s, l = C.c_int64(), C.c_int64()
+    _check(_lib.dcp_shard_range(n, parts, p, C.byref(s), C.byref(l)), "dcp_shard_range")
+    return s.value, l.value
+
+
+def dcp_workspace_bytes(I, c_s, H, c, c_z, dtype: torch.dtype, decomp="monolithic", parts=1, key_split=1,
+                        kernel="auto") -> int:
+    out = C.c_size_t()
+    pl = _plan(parts, key_split, kernel)
+    _check(_lib.dcp_workspace_bytes(I, c_s, H, c, c_z, _dtype_code(dtype), DECOMP[decomp], C.byref(pl),
+                                    C.byref(out)), "dcp_workspace_bytes")
+    return int(out.value)
+
+
+def dcp_kernel_supported(kernel, dtype: torch.dtype, H: int, c: int, c_z: int) -> bool:
+    k = KERNEL[kernel] if isinstance(kernel, str) else int(kernel)
+    return bool(_lib.dcp_kernel_supported(k, _dtype_code(dtype), H, c, c_z))
+
+
+def dcp_last_launch_count() -> int:
+    return int(_lib.dcp_last_launch_count())
+
+
+def _alloc_ws(nbytes: int, device) -> torch.Tensor:
+    return torch.empty(max(nbytes, 256), dtype=torch.uint8, device=device)
+
+
+def dcp_pair_bias_attention(s, z, w, H, c, decomp="monolithic", parts=1, key_split=1, kernel="auto", eps=1e-5,
+                            out=None, workspace=None, stream=None, atom=False, ldz=0, fused_events=None):
+    """out[I, c_s] = W_o (sigmoid(s W_g) (.) softmax(Q K^T/sqrt(c) + LN(z) W_b) V)  on the current CUDA device."""
+    assert s.is_cuda and z.is_cuda and s.is_contiguous()
+    I, c_s = s.shape
+    c_z = z.shape[-1]
+    dt = _dtype_code(s.dtype)
+    assert z.dtype == s.dtype
+    if out is None:
+        out = torch.empty(I, c_s, dtype=s.dtype, device=s.device)
+    pl = _plan(parts, key_split, kernel,
+               None if fused_events is None else (fused_events[0].handle, fused_events[1].handle))
+    if workspace is None:
+        workspace = _alloc_ws(dcp_workspace_bytes(I, c_s, H, c, c_z, s.dtype, decomp, parts, key_split, kernel), s.device)
+    ws = _weights_struct(w, eps)
+    fn = _lib.dcp_atom_pair_bias_attention if atom else _lib.dcp_pair_bias_attention
+    st = fn(_ptr(s), _ptr(z), int(ldz), C.byref(ws), _ptr(out), I, c_s, H, c, c_z, dt, DECOMP[decomp], C.byref(pl),
+            _ptr(workspace), workspace.numel(), _stream_ptr(stream))
+    _check(st, "dcp_atom_pair_bias_attention" if atom else "dcp_pair_bias_attention")
+    return out
+
+
+def dcp_atom_pair_bias_attention(a, p, w, H, c, **kw):
+    """Atom-level dense variant (BASELINE.json config 4): (L, c_atom, c_atompair) for (I, c_s, c_z)."""
+    return dcp_pair_bias_attention(a, p, w, H, c, atom=True, **kw)
+
+
+def dcp_pair_bias_attention_host(s_host, z_host, w, H, c, out_host, s_dev, z_dev, out_dev, workspace,
+                                 decomp="monolithic", parts=1, key_split=1, kernel="auto", eps=1e-5, stream=None):
+    """End-to-end entry: HOST s, z, out (pinned tensors); device staging buffers supplied by the caller."""
+    assert not s_host.is_cuda and not z_host.is_cuda and not out_host.is_cuda
+    I, c_s = s_host.shape
+    c_z = z_host.shape[-1]
+    pl = _plan(parts, key_split, kernel)
+    ws = _weights_struct(w, eps)
+    st = _lib.dcp_pair_bias_attention_host(_ptr(s_host), _ptr(z_host), C.byref(ws), _ptr(out_host), _ptr(s_dev),
+                                           _ptr(z_dev), _ptr(out_dev), I, c_s, H, c, c_z, _dtype_code(s_host.dtype),
+                                           DECOMP[decomp], C.byref(pl), _ptr(workspace), workspace.numel(),
+                                           _stream_ptr(stream))
+    _check(st, "dcp_pair_bias_attention_host")
+    return out_host
+
+
+def dcp_partial_states(s, z, w, H, c, q0, q1, k0, k1, kernel="auto", eps=1e-5, stream=None):
+    """Partial (m, l, acc) of query rows [q0,q1) against keys [k0,k1)."""
+    I, c_s = s.shape
+    c_z = z.shape[-1]
+    R, D = q1 - q0, H * c
+    m = torch.empty(max(R, 0), H, dtype=torch.float32, device=s.device)
+    l = torch.empty_like(m)
+    acc = torch.empty(max(R, 0), D, dtype=torch.float32, device=s.device)
+    workspace = _alloc_ws(dcp_workspace_bytes(I, c_s, H, c, c_z, s.dtype), s.device)
+    ws = _weights_struct(w, eps)
+    k = KERNEL[kernel] if isinstance(kernel, str) else int(kernel)
+    st = _lib.dcp_partial_states(_ptr(s), _ptr(z), 0, C.byref(ws), I, c_s, H, c, c_z, _dtype_code(s.dtype), k,
+                                 q0, q1, k0, k1, _ptr(m), _ptr(l), _ptr(acc), _ptr(workspace), workspace.numel(),
+                                 _stream_ptr(stream))
+    _check(st, "dcp_partial_states")
+    return m, l, acc
+
+
+def dcp_merge_states(m, l, acc, H, c, stream=None):
+    """Left fold over partial states: m, l [n, rows, H], acc [n, rows, H*c] (fp32, device)."""
+    n, rows = m.shape[0], m.shape[1]
+    m_out = torch.empty(rows, H, dtype=torch.float32, device=m.device)
+    l_out = torch.empty_like(m_out)
+    acc_out = torch.empty(rows, H * c, dtype=torch.float32, device=m.device)
+    st = _lib.dcp_merge_states(n, rows, H, c, _ptr(m.contiguous()), _ptr(l.contiguous()), _ptr(acc.contiguous()),
+                               _ptr(m_out), _ptr(l_out), _ptr(acc_out), _stream_ptr(stream))
+    _check(st, "dcp_merge_states")
+    return m_out, l_out, acc_out
+
+
+def raw():
+    """The ctypes library handle (tests call error paths with raw arguments)."""
+    return _lib

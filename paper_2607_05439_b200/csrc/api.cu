@@ -1,0 +1,395 @@
+// libdesigncp C ABI (include/designcp.h): validation, the Eq.-5 planner, workspace carving and the
+// launch sequence  prologue (a1) -> fused kernel per sub-problem (a2-a7) -> merge + gate (a8) -> W_o (a9).
+// Decomposition emulation (PAPER.md:72-86 row stripes, :90 grid): one fused launch per stripe / quadrant on a
+// strided view of z (a base-pointer offset, no copy), partial states merged left to right by one kernel.
+#include <cstdio>
+#include <cstring>
+
+#include "kernels.h"
+
+namespace dcp {
+namespace {
+
+thread_local int g_launches = 0;
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+inline int elt_size(dcp_dtype dt) { return dt == DCP_F32 ? 4 : 2; }
+
+struct Carve {
+  size_t q, k, v, g, gated, s_ln, wg, c0, wfold, c1, st_m, st_l, st_acc, total;
+};
+
+Carve carve(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dt, int slots) {
+  Carve w{};
+  const size_t D = (size_t)H * c, e = elt_size(dt);
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+  w.q = take((size_t)I * D * e);
+  w.k = take((size_t)I * D * e);
+  w.v = take((size_t)I * D * e);
+  w.g = take((size_t)I * D * e);
+  w.gated = take((size_t)I * D * e);
+  w.s_ln = take((size_t)I * c_s * sizeof(float));
+  w.wg = take((size_t)c_z * H * sizeof(float));
+  w.c0 = take(kMaxHeads * sizeof(float));
+  w.wfold = take((size_t)32 * c_z * 2);
+  w.c1 = take(32 * sizeof(float));
+  w.st_m = take((size_t)slots * I * H * sizeof(float));
+  w.st_l = take((size_t)slots * I * H * sizeof(float));
+  w.st_acc = take((size_t)slots * I * D * sizeof(float));
+  w.total = off;
+  return w;
+}
+
+int isqrt_exact(int p) {
+  int g = 0;
+  while ((int64_t)(g + 1) * (g + 1) <= p) ++g;
+  return (g * g == p) ? g : -1;
+}
+
+struct Plan {
+  dcp_decomp decomp;
+  int parts, key_split, slots, G, kernel;
+  cudaEvent_t ev_begin, ev_end;
+};
+
+dcp_status make_plan(int64_t I, dcp_decomp decomp, const dcp_plan* in, Plan* out) {
+  Plan p{};
+  p.decomp = decomp;
+  p.parts = in ? in->parts : 1;
+  p.key_split = (in && in->key_split > 0) ? in->key_split : 1;
+  p.kernel = in ? in->kernel : DCP_KERNEL_AUTO;
+  p.ev_begin = in ? (cudaEvent_t)in->ev_fused_begin : nullptr;
+  p.ev_end = in ? (cudaEvent_t)in->ev_fused_end : nullptr;
+  p.G = 1;
+  if (p.kernel < DCP_KERNEL_AUTO || p.kernel > DCP_KERNEL_MMA) return DCP_ERR_INVALID_ARG;
+  switch (decomp) {
+    case DCP_MONOLITHIC:
+      p.parts = 1;
+      break;
+    case DCP_ROW:
+      if (p.parts < 1 || p.parts > I) return DCP_ERR_INVALID_ARG;
+      break;
+    case DCP_GRID:
+      // "this 2D grid scheme applies only when the available GPU count P is a perfect square"
+      if (p.parts < 1) return DCP_ERR_INVALID_ARG;
+      p.G = isqrt_exact(p.parts);
+      if (p.G < 1 || p.G > I) return DCP_ERR_INVALID_ARG;
+      p.key_split = p.G;
+      break;
+    default:
+      return DCP_ERR_INVALID_ARG;
+  }
+  if (p.key_split > I) return DCP_ERR_INVALID_ARG;
+  p.slots = p.key_split;
+  *out = p;
+  return DCP_OK;
+}
+
+dcp_status check_shape(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dt) {
+  if (I <= 0 || c_s <= 0 || H <= 0 || c <= 0 || c_z <= 0) return DCP_ERR_INVALID_ARG;
+  if (dt != DCP_F32 && dt != DCP_BF16) return DCP_ERR_INVALID_ARG;
+  if (I > (int64_t)1 << 30) return DCP_ERR_INVALID_ARG;
+  if ((c_z * elt_size(dt)) % 16 != 0) return DCP_ERR_INVALID_ARG;
+  if (!fused_generic_supports(dt, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
+  return DCP_OK;
+}
+
+inline bool misaligned(const void* p, size_t a = 16) { return (reinterpret_cast<uintptr_t>(p) % a) != 0; }
+
+#define DCP_CUDA(expr)                         \
+  do {                                         \
+    cudaError_t _e = (expr);                   \
+    if (_e != cudaSuccess) return DCP_ERR_CUDA; \
+    ++g_launches;                              \
+  } while (0)
+
+struct Ctx {
+  int64_t I;
+  int c_s, H, c, c_z, D;
+  dcp_dtype dt;
+  const dcp_weights* w;
+  float eps;
+  char* ws;
+  Carve cv;
+  cudaStream_t st;
+  bool use_mma;
+};
+
+// a1: (optional LN_s) + q, k, v, g projections for ALL rows (keys/values come from the full S),
+// plus the folded LayerNorm(z) affine.
+dcp_status run_prologue(const Ctx& x, const void* s) {
+  const void* a = s;
+  bool a_f32 = false;
+  if (x.w->ln_s_gamma != nullptr) {
+    DCP_CUDA(launch_layernorm_rows(x.dt, s, x.w->ln_s_gamma, x.w->ln_s_beta, (float*)(x.ws + x.cv.s_ln), x.I, x.c_s,
+                                   x.eps, x.st));
+    a = x.ws + x.cv.s_ln;
+    a_f32 = x.dt != DCP_F32;
+  }
+  DCP_CUDA(launch_gemm(x.dt, a_f32, a, x.c_s, x.w->w_q, x.w->b_q, x.ws + x.cv.q, x.D, x.I, x.D, x.c_s, EPI_NONE, x.st));
+  DCP_CUDA(launch_gemm(x.dt, a_f32, a, x.c_s, x.w->w_k, nullptr, x.ws + x.cv.k, x.D, x.I, x.D, x.c_s, EPI_NONE, x.st));
+  DCP_CUDA(launch_gemm(x.dt, a_f32, a, x.c_s, x.w->w_v, nullptr, x.ws + x.cv.v, x.D, x.I, x.D, x.c_s, EPI_NONE, x.st));
+  DCP_CUDA(launch_gemm(x.dt, a_f32, a, x.c_s, x.w->w_g, nullptr, x.ws + x.cv.g, x.D, x.I, x.D, x.c_s, EPI_SIGMOID, x.st));
+  DCP_CUDA(launch_fold_ln_z(x.dt, x.w->w_b, x.w->ln_z_gamma, x.w->ln_z_beta, (float*)(x.ws + x.cv.wg),
+                            (float*)(x.ws + x.cv.c0), x.c_z, x.H, x.st));
+  return DCP_OK;
+}
+
+FusedParams base_params(const Ctx& x, const void* z, int64_t ldz) {
+  FusedParams p{};
+  p.z = z;
+  p.ldz = ldz;
+  p.q = x.ws + x.cv.q;
+  p.k = x.ws + x.cv.k;
+  p.v = x.ws + x.cv.v;
+  p.wg = (const float*)(x.ws + x.cv.wg);
+  p.c0 = (const float*)(x.ws + x.cv.c0);
+  p.I = (int)x.I;
+  p.c_z = x.c_z;
+  p.H = x.H;
+  p.c = x.c;
+  p.D = x.D;
+  p.eps = x.eps;
+  p.scale = 1.0f / sqrtf((float)x.c);
+  return p;
+}
+
+dcp_status run_fused(const Ctx& x, const FusedParams& p) {
+  DCP_CUDA(launch_fused_generic(x.dt, p, x.st));
+  return DCP_OK;
+}
+
+dcp_status validate_weights(const dcp_weights* w) {
+  if (!w || !w->w_q || !w->w_k || !w->w_v || !w->w_g || !w->w_b || !w->w_o || !w->ln_z_gamma || !w->ln_z_beta)
+    return DCP_ERR_INVALID_ARG;
+  if ((w->ln_s_gamma == nullptr) != (w->ln_s_beta == nullptr)) return DCP_ERR_INVALID_ARG;
+  return DCP_OK;
+}
+
+dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w, void* out, int64_t I, int c_s, int H,
+                 int c, int c_z, dcp_dtype dt, dcp_decomp decomp, const dcp_plan* plan_in, void* workspace,
+                 size_t workspace_bytes, void* stream) {
+  g_launches = 0;
+  if (!s || !z || !out || !workspace) return DCP_ERR_INVALID_ARG;
+  dcp_status st = validate_weights(w);
+  if (st != DCP_OK) return st;
+  st = check_shape(I, c_s, H, c, c_z, dt);
+  if (st != DCP_OK) return st;
+  Plan plan;
+  st = make_plan(I, decomp, plan_in, &plan);
+  if (st != DCP_OK) return st;
+  if (plan.kernel == DCP_KERNEL_MMA) return DCP_ERR_UNSUPPORTED;
+  const int e = elt_size(dt);
+  if (ldz == 0) ldz = I * (int64_t)c_z;
+  if (ldz < I * (int64_t)c_z) return DCP_ERR_INVALID_ARG;
+  if (misaligned(s) || misaligned(z) || misaligned(out) || misaligned(workspace, 256) || (ldz * e) % 16 != 0)
+    return DCP_ERR_INVALID_ARG;
+  Ctx x{};
+  x.I = I; x.c_s = c_s; x.H = H; x.c = c; x.c_z = c_z; x.D = H * c; x.dt = dt; x.w = w;
+  x.eps = w->ln_eps > 0.f ? w->ln_eps : 1e-5f;
+  x.ws = (char*)workspace;
+  x.cv = carve(I, c_s, H, c, c_z, dt, plan.slots);
+  x.st = (cudaStream_t)stream;
+  if (workspace_bytes < x.cv.total) return DCP_ERR_WORKSPACE;
+
+  st = run_prologue(x, s);
+  if (st != DCP_OK) return st;
+
+  FusedParams bp = base_params(x, z, ldz);
+  bp.st_m = (float*)(x.ws + x.cv.st_m);
+  bp.st_l = (float*)(x.ws + x.cv.st_l);
+  bp.st_acc = (float*)(x.ws + x.cv.st_acc);
+  bp.state_rows = I;
+  bp.state_row0 = 0;
+
+  if (plan.ev_begin && cudaEventRecord(plan.ev_begin, x.st) != cudaSuccess) return DCP_ERR_CUDA;
+  if (plan.decomp == DCP_GRID) {
+    // quadrant (r, cb): rows of block r against keys of block cb, bias from Z^(r,cb) only; slot = cb
+    for (int r = 0; r < plan.G; ++r) {
+      for (int cb = 0; cb < plan.G; ++cb) {
+        FusedParams p = bp;
+        int64_t len;
+        shard_range(I, plan.G, r, &p.q0, &len);
+        p.q1 = p.q0 + len;
+        shard_range(I, plan.G, cb, &p.k0, &len);
+        p.k1 = p.k0 + len;
+        p.n_chunks = 1;
+        p.slot0 = cb;
+        st = run_fused(x, p);
+        if (st != DCP_OK) return st;
+      }
+    }
+  } else {
+    // stripe p: its query rows against ALL keys (cross-attention); MONOLITHIC is one stripe
+    for (int sp = 0; sp < plan.parts; ++sp) {
+      FusedParams p = bp;
+      int64_t len;
+      shard_range(I, plan.parts, sp, &p.q0, &len);
+      p.q1 = p.q0 + len;
+      p.k0 = 0;
+      p.k1 = I;
+      p.n_chunks = plan.key_split;
+      p.slot0 = 0;
+      st = run_fused(x, p);
+      if (st != DCP_OK) return st;
+    }
+  }
+
+  if (plan.ev_end && cudaEventRecord(plan.ev_end, x.st) != cudaSuccess) return DCP_ERR_CUDA;
+
+  MergeParams mp{};
+  mp.st_m = bp.st_m; mp.st_l = bp.st_l; mp.st_acc = bp.st_acc;
+  mp.g = x.ws + x.cv.g;
+  mp.gated = x.ws + x.cv.gated;
+  mp.rows = I; mp.n_slots = plan.slots; mp.H = H; mp.c = c; mp.D = x.D;
+  DCP_CUDA(launch_merge(dt, mp, x.st));
+  DCP_CUDA(launch_gemm(dt, false, x.ws + x.cv.gated, x.D, w->w_o, nullptr, out, c_s, I, c_s, x.D, EPI_NONE, x.st));
+  return DCP_OK;
+}
+
+}  // namespace
+}  // namespace dcp
+
+using namespace dcp;
+
+extern "C" {
+
+dcp_status dcp_workspace_bytes(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype, dcp_decomp decomp,
+                               const dcp_plan* plan_in, size_t* bytes) {
+  if (!bytes) return DCP_ERR_INVALID_ARG;
+  dcp_status st = check_shape(I, c_s, H, c, c_z, dtype);
+  if (st != DCP_OK) return st;
+  Plan plan;
+  st = make_plan(I, decomp, plan_in, &plan);
+  if (st != DCP_OK) return st;
+  *bytes = carve(I, c_s, H, c, c_z, dtype, plan.slots).total;
+  return DCP_OK;
+}
+
+dcp_status dcp_pair_bias_attention(const void* s, const void* z, int64_t ldz, const dcp_weights* w, void* out, int64_t I,
+                                   int c_s, int H, int c, int c_z, dcp_dtype dtype, dcp_decomp decomp,
+                                   const dcp_plan* plan, void* workspace, size_t workspace_bytes, void* stream) {
+  return layer(s, z, ldz, w, out, I, c_s, H, c, c_z, dtype, decomp, plan, workspace, workspace_bytes, stream);
+}
+
+dcp_status dcp_atom_pair_bias_attention(const void* a, const void* p, int64_t ldp, const dcp_weights* w, void* out,
+                                        int64_t L, int c_atom, int H, int c, int c_atompair, dcp_dtype dtype,
+                                        dcp_decomp decomp, const dcp_plan* plan, void* workspace,
+                                        size_t workspace_bytes, void* stream) {
+  return layer(a, p, ldp, w, out, L, c_atom, H, c, c_atompair, dtype, decomp, plan, workspace, workspace_bytes, stream);
+}
+
+dcp_status dcp_pair_bias_attention_host(const void* s_host, const void* z_host, const dcp_weights* w, void* out_host,
+                                        void* s_dev, void* z_dev, void* out_dev, int64_t I, int c_s, int H, int c,
+                                        int c_z, dcp_dtype dtype, dcp_decomp decomp, const dcp_plan* plan,
+                                        void* workspace, size_t workspace_bytes, void* stream) {
+  if (!s_host || !z_host || !out_host || !s_dev || !z_dev || !out_dev) return DCP_ERR_INVALID_ARG;
+  dcp_status st = check_shape(I, c_s, H, c, c_z, dtype);
+  if (st != DCP_OK) return st;
+  const size_t e = elt_size(dtype);
+  cudaStream_t cs = (cudaStream_t)stream;
+  if (cudaMemcpyAsync(s_dev, s_host, (size_t)I * c_s * e, cudaMemcpyHostToDevice, cs) != cudaSuccess) return DCP_ERR_CUDA;
+  if (cudaMemcpyAsync(z_dev, z_host, (size_t)I * I * c_z * e, cudaMemcpyHostToDevice, cs) != cudaSuccess)
+    return DCP_ERR_CUDA;
+  st = layer(s_dev, z_dev, 0, w, out_dev, I, c_s, H, c, c_z, dtype, decomp, plan, workspace, workspace_bytes, stream);
+  if (st != DCP_OK) return st;
+  if (cudaMemcpyAsync(out_host, out_dev, (size_t)I * c_s * e, cudaMemcpyDeviceToHost, cs) != cudaSuccess)
+    return DCP_ERR_CUDA;
+  return DCP_OK;
+}
+
+dcp_status dcp_partial_states(const void* s, const void* z, int64_t ldz, const dcp_weights* w, int64_t I, int c_s, int H,
+                              int c, int c_z, dcp_dtype dtype, int kernel, int64_t q0, int64_t q1, int64_t k0,
+                              int64_t k1, float* m, float* l, float* acc, void* workspace, size_t workspace_bytes,
+                              void* stream) {
+  g_launches = 0;
+  if (!s || !z || !m || !l || !acc || !workspace) return DCP_ERR_INVALID_ARG;
+  dcp_status st = validate_weights(w);
+  if (st != DCP_OK) return st;
+  st = check_shape(I, c_s, H, c, c_z, dtype);
+  if (st != DCP_OK) return st;
+  if (q0 < 0 || q1 > I || q0 >= q1 || k0 < 0 || k1 > I || k0 >= k1) return DCP_ERR_INVALID_ARG;
+  if (kernel == DCP_KERNEL_MMA) return DCP_ERR_UNSUPPORTED;
+  if (ldz == 0) ldz = I * (int64_t)c_z;
+  if (misaligned(s) || misaligned(z) || misaligned(workspace, 256)) return DCP_ERR_INVALID_ARG;
+  Ctx x{};
+  x.I = I; x.c_s = c_s; x.H = H; x.c = c; x.c_z = c_z; x.D = H * c; x.dt = dtype; x.w = w;
+  x.eps = w->ln_eps > 0.f ? w->ln_eps : 1e-5f;
+  x.ws = (char*)workspace;
+  x.cv = carve(I, c_s, H, c, c_z, dtype, 1);
+  x.st = (cudaStream_t)stream;
+  if (workspace_bytes < x.cv.total) return DCP_ERR_WORKSPACE;
+  st = run_prologue(x, s);
+  if (st != DCP_OK) return st;
+  FusedParams p = base_params(x, z, ldz);
+  p.st_m = m; p.st_l = l; p.st_acc = acc;
+  p.state_rows = q1 - q0;
+  p.state_row0 = q0;
+  p.q0 = q0; p.q1 = q1; p.k0 = k0; p.k1 = k1;
+  p.n_chunks = 1;
+  p.slot0 = 0;
+  return run_fused(x, p);
+}
+
+dcp_status dcp_merge_states(int n_parts, int64_t rows, int H, int c, const float* m, const float* l, const float* acc,
+                            float* m_out, float* l_out, float* acc_out, void* stream) {
+  if (n_parts < 1 || rows < 1 || H < 1 || c < 1 || !m || !l || !acc || !m_out || !l_out || !acc_out)
+    return DCP_ERR_INVALID_ARG;
+  MergeParams mp{};
+  mp.st_m = m; mp.st_l = l; mp.st_acc = acc;
+  mp.g = nullptr;
+  mp.m_out = m_out; mp.l_out = l_out; mp.acc_out = acc_out;
+  mp.rows = rows; mp.n_slots = n_parts; mp.H = H; mp.c = c; mp.D = H * c;
+  if (launch_merge(DCP_F32, mp, (cudaStream_t)stream) != cudaSuccess) return DCP_ERR_CUDA;
+  return DCP_OK;
+}
+
+dcp_status dcp_shard_range(int64_t n, int parts, int p, int64_t* start, int64_t* len) {
+  if (n < 0 || parts < 1 || p < 0 || p >= parts || !start || !len) return DCP_ERR_INVALID_ARG;
+  shard_range(n, parts, p, start, len);
+  return DCP_OK;
+}
+
+int dcp_kernel_supported(int kernel, dcp_dtype dtype, int H, int c, int c_z) {
+  if (kernel == DCP_KERNEL_GENERIC) return fused_generic_supports(dtype, H, c, c_z) ? 1 : 0;
+  return 0;
+}
+
+dcp_status dcp_event_create(void** ev) {
+  if (!ev) return DCP_ERR_INVALID_ARG;
+  cudaEvent_t e;
+  if (cudaEventCreate(&e) != cudaSuccess) return DCP_ERR_CUDA;
+  *ev = (void*)e;
+  return DCP_OK;
+}
+dcp_status dcp_event_record(void* ev, void* stream) {
+  if (!ev) return DCP_ERR_INVALID_ARG;
+  return cudaEventRecord((cudaEvent_t)ev, (cudaStream_t)stream) == cudaSuccess ? DCP_OK : DCP_ERR_CUDA;
+}
+dcp_status dcp_event_elapsed_ms(void* ev_begin, void* ev_end, float* ms) {
+  if (!ev_begin || !ev_end || !ms) return DCP_ERR_INVALID_ARG;
+  if (cudaEventSynchronize((cudaEvent_t)ev_end) != cudaSuccess) return DCP_ERR_CUDA;
+  return cudaEventElapsedTime(ms, (cudaEvent_t)ev_begin, (cudaEvent_t)ev_end) == cudaSuccess ? DCP_OK : DCP_ERR_CUDA;
+}
+dcp_status dcp_event_destroy(void* ev) {
+  if (!ev) return DCP_ERR_INVALID_ARG;
+  return cudaEventDestroy((cudaEvent_t)ev) == cudaSuccess ? DCP_OK : DCP_ERR_CUDA;
+}
+
+int dcp_last_launch_count(void) { return g_launches; }
+
+const char* dcp_status_string(dcp_status st) {
+  switch (st) {
+    case DCP_OK: return "DCP_OK";
+    case DCP_ERR_INVALID_ARG: return "DCP_ERR_INVALID_ARG";
+    case DCP_ERR_UNSUPPORTED: return "DCP_ERR_UNSUPPORTED";
+    case DCP_ERR_WORKSPACE: return "DCP_ERR_WORKSPACE";
+    case DCP_ERR_CUDA: return "DCP_ERR_CUDA";
+    default: return "DCP_ERR_UNKNOWN";
+  }
+}
+
+int dcp_version(void) { return 100; }
+
+}  // extern "C"
