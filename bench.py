@@ -1,0 +1,359 @@
+#!/usr/bin/env python
+"""bench.py -- one B200, attention with pair bias (Design-CP's one-GPU core), BASELINE.json's metric:
+"pair-bias attention Gpair-entries/s at I=3000; % of HBM roofline".
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C1|C3|C4] [--decomp monolithic|row|grid]
+    python bench.py --impl reference ...      # the fp64 CPU oracle on the same config (bounded sample per step)
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N ...                 # N independent replicas ("replicas only")
+
+A "step" is one pass of the whole hot path (prologue projections, fused
+LayerNorm + bias projection + QK^T + online softmax + PV, merge, gate, W_o) over one synthetic layer input.
+One JSON line on stdout (rank 0).  `value` = I^2 * steps / t with z resident in HBM; `e2e` = the same metric
+through dcp_pair_bias_attention_host with HOST (pinned) s, z, out -- copies inside the timed region;
+`roofline` = the fused kernel's algorithmic bytes (z once: c_z * 2 B per pair) / its CUDA-event duration
+against the measured HBM copy bandwidth; `cpu_baseline` = the oracle on this box's host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "pair_bias_attention_gpair_per_s"
+UNIT = "Gpair/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/, named per round); None = not captured for that kernel / workload.
+NCU_TRAFFIC_BYTES = {
+    # (kernel, workload): bytes
+}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="native", choices=["native", "reference"])
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--decomp", default="monolithic", choices=["monolithic", "row", "grid"])
+    ap.add_argument("--parts", type=int, default=0, help="row stripes / grid cells (0: 8 rows, 16 grid)")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "mma"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-rows", type=int, default=0, help="oracle sample rows (0: sized for ~10-20 s)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def default_parts(decomp, parts):
+    if parts:
+        return parts
+    return {"monolithic": 1, "row": 8, "grid": 16}[decomp]
+
+
+def oracle_sample(cfg, s, z, w, n_rows, seed=0):
+    """Time the fp64 oracle, as it stands, on `n_rows` sampled query rows x all I keys of this workload.
+    Returns (pairs, seconds, threads, rows)."""
+    import numpy as np
+    import torch
+    import dcp_synth as syn
+    from oracle import pair_bias_attention as orc
+    rows = syn.sample_rows(cfg.I, n_rows, seed=seed)
+    idx = torch.as_tensor(rows, device=z.device)
+    f64 = lambda t: t.detach().float().cpu().double().numpy()
+    z_rows = z.index_select(0, idx).float().cpu().numpy()
+    s64, w64 = f64(s), {k: f64(v) for k, v in w.items()}
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
+    except Exception:
+        threads = 1
+    t0 = time.perf_counter()
+    out = orc.pair_bias_attention_rows(s64, z_rows, rows, w64, cfg.H, cfg.c)
+    dt = time.perf_counter() - t0
+    assert np.all(np.isfinite(out))
+    return len(rows) * cfg.I, dt, threads, rows, out
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle (test infrastructure) timed as the baseline arm; rank 0 only."""
+    if rank != 0:
+        return
+    import torch
+    import dcp_synth as syn
+    cfg = syn.CONFIGS[args.workload]
+    dev = "cuda:0" if torch.cuda.is_available() else "cpu"
+    # generate on the GPU when there is one (z of 2.3 GB), else on the CPU for small workloads
+    w = syn.make_weights(cfg, dev)
+    s = syn.make_s(cfg, dev)
+    z = syn.make_z(cfg, dev)
+    n_rows = args.cpu_rows or max(2, min(cfg.I, int(2.0e6 / cfg.I)))   # ~2 M pairs per step
+    for _ in range(max(0, min(args.warmup, 1))):
+        oracle_sample(cfg, s, z, w, 2)
+    pairs = secs = 0.0
+    threads = 1
+    for k in range(args.steps):
+        p, dt, threads, _, _ = oracle_sample(cfg, s, z, w, n_rows, seed=k)
+        pairs += p
+        secs += dt
+    value = pairs / secs / 1e9
+    sample = f"{n_rows} sampled query rows x {cfg.I} keys per step ({args.steps} steps), fp64 numpy oracle"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / max(args.steps, 1) * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(cfg), "decomposition": "monolithic", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg):
+    kind = "atom-level" if cfg.name == "C4" else "token-level"
+    return (f"{cfg.name}: {kind} pair-bias attention I={cfg.I} c_s={cfg.c_s} c_z={cfg.c_z} H={cfg.H} c={cfg.c} "
+            f"{cfg.dtype} (icosahedral 60 x {cfg.n_res})" if cfg.structured else
+            f"{cfg.name}: {kind} pair-bias attention I={cfg.I} c_s={cfg.c_s} c_z={cfg.c_z} H={cfg.H} c={cfg.c} {cfg.dtype}")
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as ge
+    if rank == 0 or world == 1:
+        ge.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    import dcp_synth as syn
+    import paper_2607_05439_b200 as dcp
+
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    cfg = syn.CONFIGS[args.workload]
+    # every rank runs its own replica of the layer on its own inputs (seed offset by rank): no data-path collective
+    if world > 1:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    parts = default_parts(args.decomp, args.parts)
+    atom = cfg.name == "C4"
+    w = syn.make_weights(cfg, dev)
+    s = syn.make_s(cfg, dev)
+    z = syn.make_z(cfg, dev)
+    tdt = s.dtype
+    ws_bytes = dcp.dcp_workspace_bytes(cfg.I, cfg.c_s, cfg.H, cfg.c, cfg.c_z, tdt, args.decomp, parts, 1, args.kernel)
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+    out = torch.empty(cfg.I, cfg.c_s, dtype=tdt, device=dev)
+    stream = torch.cuda.current_stream()
+    z_bytes = z.numel() * z.element_size()
+    l2_note = "z (%.0f MB) larger than the 126 MB L2: no flush needed" % (z_bytes / 1e6)
+    flush = None
+    if z_bytes < 400e6:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+        l2_note = "L2 flushed between steps by writing a 256 MiB buffer (outside the fused-kernel events)"
+
+    def step(ev=None):
+        dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, decomp=args.decomp, parts=parts, kernel=args.kernel,
+                                    out=out, workspace=ws, atom=atom, fused_events=ev)
+
+    for _ in range(max(args.warmup, 3)):
+        if flush is not None:
+            flush.zero_()
+        step()
+    launches_per_step = dcp.dcp_last_launch_count()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    evs = [(dcp.Event(), dcp.Event()) for _ in range(args.steps)]
+    t_begin, t_end = dcp.Event(), dcp.Event()
+    step_ms = []
+    torch.cuda.synchronize()
+    if flush is None:
+        t_begin.record()
+        for k in range(args.steps):
+            step(evs[k])
+        t_end.record()
+        torch.cuda.synchronize()
+        total_ms = t_begin.elapsed_ms(t_end)
+    else:
+        # small workload: flush L2 between steps, time each step with its own event pair
+        total_ms = 0.0
+        for k in range(args.steps):
+            flush.zero_()
+            a, b = dcp.Event(), dcp.Event()
+            a.record()
+            step(evs[k])
+            b.record()
+            torch.cuda.synchronize()
+            total_ms += a.elapsed_ms(b)
+    clocks = sampler.stop() if rank == 0 else None
+    fused_ms = [a.elapsed_ms(b) for a, b in evs]
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    pairs_per_step = float(cfg.I) * cfg.I
+    value = pairs_per_step * args.steps * world / (total_ms * 1e-3) / 1e9
+
+    # ---- roofline of the dominant (fused) kernel: algorithmic bytes = z once = c_z * elt bytes per pair
+    peak, peak_how = measured_peaks()
+    fused_avg_ms = sum(fused_ms) / len(fused_ms)
+    alg_bytes = pairs_per_step * cfg.c_z * z.element_size()
+    achieved = alg_bytes / (fused_avg_ms * 1e-3) / 1e9
+    kname = {"auto": None, "generic": "fused_generic_kernel", "mma": "fused_mma_kernel"}[args.kernel]
+    if kname is None:
+        kname = "fused_mma_kernel" if dcp.dcp_kernel_supported("mma", tdt, cfg.H, cfg.c, cfg.c_z) else "fused_generic_kernel"
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES.get((kname, cfg.name)), "kernel": kname, "peak_source": peak_how,
+                "kernel_ms": fused_avg_ms, "kernel_share_of_step": fused_avg_ms * args.steps / total_ms,
+                "algorithmic_bytes_per_launch": alg_bytes,
+                "fused_launches_per_step": 1 if args.decomp == "monolithic" else None}
+
+    # ---- e2e: HOST (pinned) s, z, out through dcp_pair_bias_attention_host, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        try:
+            sh = torch.empty(s.shape, dtype=tdt).pin_memory(); sh.copy_(s)
+            zh = torch.empty(z.shape, dtype=tdt).pin_memory(); zh.copy_(z)
+            oh = torch.empty(out.shape, dtype=tdt).pin_memory()
+            s_dev, out_dev = torch.empty_like(s), torch.empty_like(out)
+            ne = max(1, args.e2e_steps)
+            dcp.dcp_pair_bias_attention_host(sh, zh, w, cfg.H, cfg.c, oh, s_dev, z, out_dev, ws, decomp=args.decomp,
+                                             parts=parts, kernel=args.kernel)   # warm-up (z_dev = z: same bits)
+            torch.cuda.synchronize()
+            if world > 1:
+                dist.barrier()
+            a, b = dcp.Event(), dcp.Event()
+            a.record()
+            for _ in range(ne):
+                dcp.dcp_pair_bias_attention_host(sh, zh, w, cfg.H, cfg.c, oh, s_dev, z, out_dev, ws,
+                                                 decomp=args.decomp, parts=parts, kernel=args.kernel)
+            b.record()
+            torch.cuda.synchronize()
+            ms = a.elapsed_ms(b)
+            if world > 1:
+                t = torch.tensor([ms], dtype=torch.float64, device=dev)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                ms = float(t.item())
+            assert torch.equal(oh.to(dev), out), "host entry disagrees with the device entry"
+            e2e = {"value": pairs_per_step * ne * world / (ms * 1e-3) / 1e9, "unit": UNIT,
+                   "h2d_bytes_per_step": (sh.numel() + zh.numel()) * sh.element_size(),
+                   "d2h_bytes_per_step": oh.numel() * oh.element_size(), "steps": ne,
+                   "note": "PCIe host->device copy of z dominates"}
+            del zh
+        except Exception as exc:  # e.g. not enough pinned host memory for z
+            e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None,
+                   "error": repr(exc)[:200]}
+
+    # ---- cpu_baseline: the oracle on this box's host cores, rank 0 at N=1 only, on a bounded sample
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n_rows = args.cpu_rows or max(2, min(cfg.I, int(4.0e6 / cfg.I)))
+        oracle_sample(cfg, s, z, w, 2)  # page in numpy/BLAS
+        pairs, dt, threads, rows, ref = oracle_sample(cfg, s, z, w, n_rows)
+        import numpy as np
+        got = out.index_select(0, torch.as_tensor(rows, device=dev)).float().cpu().double().numpy()
+        rel = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
+        cpu = {"value": pairs / dt / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"{len(rows)} sampled query rows x {cfg.I} keys of this workload ({dt:.1f} s), fp64 numpy oracle",
+               "gpu_vs_oracle_rel_l2_on_sample": rel, "gpu_vs_oracle_max_abs_on_sample": float(np.abs(got - ref).max())}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16" if cfg.dtype == "bf16" else "f32", "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "decomposition": args.decomp, "parts": parts,
+                       "kernel": kname, "l2": l2_note, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "peak_device_bytes": int(torch.cuda.max_memory_allocated())},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": launches_per_step * args.steps, "clocks": clocks,
+            "hbm_roofline_gpair_per_s": peak * 1e9 / (cfg.c_z * z.element_size()) / 1e9,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
