@@ -22,16 +22,18 @@ struct Carve {
 Carve carve(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dt, int slots) {
   Carve w{};
   const size_t D = (size_t)H * c, e = elt_size(dt);
+  // the tensor-core path keeps q, k zero-padded per head ([I][H][cp]) and v transposed ([D][ldv])
+  const size_t Dp = (size_t)H * mma_head_pad(c), ldv = (size_t)mma_ldv(I);
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
-  w.q = take((size_t)I * D * e);
-  w.k = take((size_t)I * D * e);
-  w.v = take((size_t)I * D * e);
+  w.q = take((size_t)I * Dp * e);
+  w.k = take((size_t)I * Dp * e);
+  w.v = take(D * ldv * e);
   w.g = take((size_t)I * D * e);
   w.gated = take((size_t)I * D * e);
   w.s_ln = take((size_t)I * c_s * sizeof(float));
   w.wg = take((size_t)c_z * H * sizeof(float));
-  w.c0 = take(kMaxHeads * sizeof(float));
+  w.c0 = take(32 * sizeof(float));
   w.wfold = take((size_t)32 * c_z * 2);
   w.c1 = take(32 * sizeof(float));
   w.st_m = take((size_t)slots * I * H * sizeof(float));
@@ -50,10 +52,12 @@ int isqrt_exact(int p) {
 struct Plan {
   dcp_decomp decomp;
   int parts, key_split, slots, G, kernel;
+  bool use_mma;   // bf16 tensor-core path (fused_mma.cu) instead of the generic fp32 CUDA-core kernel
+  int nseg;       // tensor-core path: Eq.-5 segments per key chunk (a pure function of I and the chunk count)
   cudaEvent_t ev_begin, ev_end;
 };
 
-dcp_status make_plan(int64_t I, dcp_decomp decomp, const dcp_plan* in, Plan* out) {
+dcp_status make_plan(int64_t I, int H, int c, int c_z, dcp_dtype dt, dcp_decomp decomp, const dcp_plan* in, Plan* out) {
   Plan p{};
   p.decomp = decomp;
   p.parts = in ? in->parts : 1;
@@ -81,7 +85,12 @@ dcp_status make_plan(int64_t I, dcp_decomp decomp, const dcp_plan* in, Plan* out
       return DCP_ERR_INVALID_ARG;
   }
   if (p.key_split > I) return DCP_ERR_INVALID_ARG;
-  p.slots = p.key_split;
+  const bool mma_ok = fused_mma_supports(dt, H, c, c_z);
+  if (p.kernel == DCP_KERNEL_MMA && !mma_ok) return DCP_ERR_UNSUPPORTED;
+  if (p.kernel == DCP_KERNEL_GENERIC && !fused_generic_supports(dt, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
+  p.use_mma = mma_ok && p.kernel != DCP_KERNEL_GENERIC;
+  p.nseg = p.use_mma ? mma_num_segments(I, p.key_split) : 1;
+  p.slots = p.key_split * p.nseg;
   *out = p;
   return DCP_OK;
 }
@@ -91,7 +100,7 @@ dcp_status check_shape(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dt) 
   if (dt != DCP_F32 && dt != DCP_BF16) return DCP_ERR_INVALID_ARG;
   if (I > (int64_t)1 << 30) return DCP_ERR_INVALID_ARG;
   if ((c_z * elt_size(dt)) % 16 != 0) return DCP_ERR_INVALID_ARG;
-  if (!fused_generic_supports(dt, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
+  if (!fused_generic_supports(dt, H, c, c_z) && !fused_mma_supports(dt, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
   return DCP_OK;
 }
 
@@ -155,6 +164,53 @@ FusedParams base_params(const Ctx& x, const void* z, int64_t ldz) {
   return p;
 }
 
+// a1 on tensor cores (bf16 path): one GEMM launch for q, k, v, g in the layouts the fused MMA kernel reads.
+dcp_status run_prologue_mma(const Ctx& x, const void* s) {
+  const void* a = s;
+  if (x.w->ln_s_gamma != nullptr) {
+    DCP_CUDA(launch_layernorm_rows_bf16(s, x.w->ln_s_gamma, x.w->ln_s_beta, x.ws + x.cv.s_ln, x.I, x.c_s, x.eps, x.st));
+    a = x.ws + x.cv.s_ln;
+  }
+  const int cp = mma_head_pad(x.c);
+  const int64_t ldv = mma_ldv(x.I);
+  if (cp != x.c) {   // zero the per-head padding of q and k
+    if (cudaMemsetAsync(x.ws + x.cv.q, 0, (size_t)x.I * x.H * cp * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
+    if (cudaMemsetAsync(x.ws + x.cv.k, 0, (size_t)x.I * x.H * cp * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
+  }
+  if (ldv != x.I) {  // zero V^T beyond the last key (0 * finite in PV)
+    if (cudaMemsetAsync(x.ws + x.cv.v, 0, (size_t)x.D * ldv * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
+  }
+  GemmMmaParams gp{};
+  gp.A = a; gp.lda = x.c_s; gp.M = x.I; gp.N = x.D; gp.K = x.c_s; gp.nseg = 4;
+  gp.W[0] = x.w->w_q; gp.W[1] = x.w->w_k; gp.W[2] = x.w->w_v; gp.W[3] = x.w->w_g;
+  gp.bias[0] = x.w->b_q;
+  gp.C[0] = x.ws + x.cv.q; gp.C[1] = x.ws + x.cv.k; gp.C[2] = x.ws + x.cv.v; gp.C[3] = x.ws + x.cv.g;
+  gp.mode[0] = GEMM_OUT_HEADPAD; gp.mode[1] = GEMM_OUT_HEADPAD; gp.mode[2] = GEMM_OUT_TRANSPOSED; gp.mode[3] = GEMM_OUT_SIGMOID;
+  gp.scale[0] = 1.4426950408889634f / sqrtf((float)x.c);   // log2(e)/sqrt(c): the softmax runs in the exp2 domain
+  gp.scale[1] = 1.f;
+  gp.ldc[2] = ldv; gp.ldc[3] = x.D;
+  gp.H = x.H; gp.c = x.c; gp.cp = cp;
+  DCP_CUDA(launch_gemm_mma(gp, x.st));
+  DCP_CUDA(launch_fold_ln_z_mma(x.w->w_b, x.w->ln_z_gamma, x.w->ln_z_beta, x.ws + x.cv.wfold, (float*)(x.ws + x.cv.c1),
+                                (float*)(x.ws + x.cv.c0), x.c_z, x.H, 16, x.st));
+  return DCP_OK;
+}
+
+MmaParams base_params_mma(const Ctx& x) {
+  MmaParams p{};
+  p.qp = x.ws + x.cv.q;
+  p.kp = x.ws + x.cv.k;
+  p.vt = x.ws + x.cv.v;
+  p.ldv = mma_ldv(x.I);
+  p.wfold = x.ws + x.cv.wfold;
+  p.c1 = (const float*)(x.ws + x.cv.c1);
+  p.c0 = (const float*)(x.ws + x.cv.c0);
+  p.I = (int)x.I;
+  p.c = x.c;
+  p.eps = x.eps;
+  return p;
+}
+
 dcp_status run_fused(const Ctx& x, const FusedParams& p) {
   DCP_CUDA(launch_fused_generic(x.dt, p, x.st));
   return DCP_OK;
@@ -177,9 +233,8 @@ dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w
   st = check_shape(I, c_s, H, c, c_z, dt);
   if (st != DCP_OK) return st;
   Plan plan;
-  st = make_plan(I, decomp, plan_in, &plan);
+  st = make_plan(I, H, c, c_z, dt, decomp, plan_in, &plan);
   if (st != DCP_OK) return st;
-  if (plan.kernel == DCP_KERNEL_MMA) return DCP_ERR_UNSUPPORTED;
   const int e = elt_size(dt);
   if (ldz == 0) ldz = I * (int64_t)c_z;
   if (ldz < I * (int64_t)c_z) return DCP_ERR_INVALID_ARG;
@@ -193,13 +248,31 @@ dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w
   x.st = (cudaStream_t)stream;
   if (workspace_bytes < x.cv.total) return DCP_ERR_WORKSPACE;
 
+  float* st_m = (float*)(x.ws + x.cv.st_m);
+  float* st_l = (float*)(x.ws + x.cv.st_l);
+  float* st_acc = (float*)(x.ws + x.cv.st_acc);
+
+  if (plan.use_mma) {
+    st = run_prologue_mma(x, s);
+    if (st != DCP_OK) return st;
+    // ONE persistent launch over every (stripe | grid row block, 32-query tile, key chunk, segment) unit; each unit
+    // reads only its own block of z and writes its own partial state (no cross-unit communication).
+    MmaParams mp = base_params_mma(x);
+    mp.st_m = st_m; mp.st_l = st_l; mp.st_acc = st_acc;
+    mp.state_rows = I; mp.state_row0 = 0;
+    mp.q_begin = 0; mp.q_end = (int)I; mp.n_qparts = plan.decomp == DCP_GRID ? plan.G : plan.parts;
+    mp.k_begin = 0; mp.k_end = (int)I; mp.n_kparts = plan.key_split;
+    mp.nseg = plan.nseg; mp.slot0 = 0;
+    if (plan.ev_begin && cudaEventRecord(plan.ev_begin, x.st) != cudaSuccess) return DCP_ERR_CUDA;
+    DCP_CUDA(launch_fused_mma(mp, z, ldz, x.st));
+  } else {
   st = run_prologue(x, s);
   if (st != DCP_OK) return st;
 
   FusedParams bp = base_params(x, z, ldz);
-  bp.st_m = (float*)(x.ws + x.cv.st_m);
-  bp.st_l = (float*)(x.ws + x.cv.st_l);
-  bp.st_acc = (float*)(x.ws + x.cv.st_acc);
+  bp.st_m = st_m;
+  bp.st_l = st_l;
+  bp.st_acc = st_acc;
   bp.state_rows = I;
   bp.state_row0 = 0;
 
@@ -235,16 +308,24 @@ dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w
       if (st != DCP_OK) return st;
     }
   }
+  }
 
   if (plan.ev_end && cudaEventRecord(plan.ev_end, x.st) != cudaSuccess) return DCP_ERR_CUDA;
 
   MergeParams mp{};
-  mp.st_m = bp.st_m; mp.st_l = bp.st_l; mp.st_acc = bp.st_acc;
+  mp.st_m = st_m; mp.st_l = st_l; mp.st_acc = st_acc;
   mp.g = x.ws + x.cv.g;
   mp.gated = x.ws + x.cv.gated;
   mp.rows = I; mp.n_slots = plan.slots; mp.H = H; mp.c = c; mp.D = x.D;
   DCP_CUDA(launch_merge(dt, mp, x.st));
-  DCP_CUDA(launch_gemm(dt, false, x.ws + x.cv.gated, x.D, w->w_o, nullptr, out, c_s, I, c_s, x.D, EPI_NONE, x.st));
+  if (plan.use_mma) {
+    GemmMmaParams gp{};
+    gp.A = x.ws + x.cv.gated; gp.lda = x.D; gp.M = I; gp.N = c_s; gp.K = x.D; gp.nseg = 1;
+    gp.W[0] = w->w_o; gp.C[0] = out; gp.mode[0] = GEMM_OUT_PLAIN; gp.ldc[0] = c_s;
+    DCP_CUDA(launch_gemm_mma(gp, x.st));
+  } else {
+    DCP_CUDA(launch_gemm(dt, false, x.ws + x.cv.gated, x.D, w->w_o, nullptr, out, c_s, I, c_s, x.D, EPI_NONE, x.st));
+  }
   return DCP_OK;
 }
 
@@ -261,7 +342,7 @@ dcp_status dcp_workspace_bytes(int64_t I, int c_s, int H, int c, int c_z, dcp_dt
   dcp_status st = check_shape(I, c_s, H, c, c_z, dtype);
   if (st != DCP_OK) return st;
   Plan plan;
-  st = make_plan(I, decomp, plan_in, &plan);
+  st = make_plan(I, H, c, c_z, dtype, decomp, plan_in, &plan);
   if (st != DCP_OK) return st;
   *bytes = carve(I, c_s, H, c, c_z, dtype, plan.slots).total;
   return DCP_OK;
@@ -310,7 +391,10 @@ dcp_status dcp_partial_states(const void* s, const void* z, int64_t ldz, const d
   st = check_shape(I, c_s, H, c, c_z, dtype);
   if (st != DCP_OK) return st;
   if (q0 < 0 || q1 > I || q0 >= q1 || k0 < 0 || k1 > I || k0 >= k1) return DCP_ERR_INVALID_ARG;
-  if (kernel == DCP_KERNEL_MMA) return DCP_ERR_UNSUPPORTED;
+  const bool mma_ok = fused_mma_supports(dtype, H, c, c_z);
+  if (kernel == DCP_KERNEL_MMA && !mma_ok) return DCP_ERR_UNSUPPORTED;
+  if (kernel == DCP_KERNEL_GENERIC && !fused_generic_supports(dtype, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
+  const bool use_mma = mma_ok && kernel != DCP_KERNEL_GENERIC;
   if (ldz == 0) ldz = I * (int64_t)c_z;
   if (misaligned(s) || misaligned(z) || misaligned(workspace, 256)) return DCP_ERR_INVALID_ARG;
   Ctx x{};
@@ -320,6 +404,18 @@ dcp_status dcp_partial_states(const void* s, const void* z, int64_t ldz, const d
   x.cv = carve(I, c_s, H, c, c_z, dtype, 1);
   x.st = (cudaStream_t)stream;
   if (workspace_bytes < x.cv.total) return DCP_ERR_WORKSPACE;
+  if (use_mma) {
+    st = run_prologue_mma(x, s);
+    if (st != DCP_OK) return st;
+    MmaParams mp = base_params_mma(x);
+    mp.st_m = m; mp.st_l = l; mp.st_acc = acc;
+    mp.state_rows = q1 - q0; mp.state_row0 = q0;
+    mp.q_begin = (int)q0; mp.q_end = (int)q1; mp.n_qparts = 1;
+    mp.k_begin = (int)k0; mp.k_end = (int)k1; mp.n_kparts = 1;
+    mp.nseg = 1; mp.slot0 = 0;
+    DCP_CUDA(launch_fused_mma(mp, z, ldz, x.st));
+    return DCP_OK;
+  }
   st = run_prologue(x, s);
   if (st != DCP_OK) return st;
   FusedParams p = base_params(x, z, ldz);
@@ -353,6 +449,7 @@ dcp_status dcp_shard_range(int64_t n, int parts, int p, int64_t* start, int64_t*
 
 int dcp_kernel_supported(int kernel, dcp_dtype dtype, int H, int c, int c_z) {
   if (kernel == DCP_KERNEL_GENERIC) return fused_generic_supports(dtype, H, c, c_z) ? 1 : 0;
+  if (kernel == DCP_KERNEL_MMA) return fused_mma_supports(dtype, H, c, c_z) ? 1 : 0;
   return 0;
 }
 

@@ -1,0 +1,539 @@
+// bf16 tensor-core fused kernel (steps a2-a7 of SURVEY.md section 8(a)) for c_z = 128, H = 16 heads.
+//   per pair (i, j):  LayerNorm(z_ij) -> bias_h = zhat . W_b[:,h]          ("learned projection of Z")
+//   logit_h = q_i^h . k_j^h / sqrt(c) + bias_h                             (PAPER.md:83 Eq. 2; i = row of z, :81)
+//   online softmax over keys with running (m, l, acc)
+// z is streamed from HBM exactly once by TMA (cp.async.bulk.tensor, 128-byte swizzle) through a 4-stage
+// mbarrier ring; the I*I*H logits and the LayerNorm output never leave the SM.
+//
+// One persistent CTA per SM, 16 warps, warp-specialised (register budgets moved with setmaxnreg):
+//   warp 0        TMA producer: z boxes of (64 ch, 16 keys, 8 queries) x 2 channel halves = 32 KB per stage
+//   warps 4-7     bias projection: per (query, 16 keys) one m16 block; A = raw z tile (ldmatrix from the swizzled
+//                 stage), B = (gamma (.) W_b log2 e)^T bf16, fp32 accumulate; LayerNorm statistics (two-pass, fp32)
+//                 come from the same A fragments; bias = rstd*(z.W' - mu*c1) + c0 goes to a double-buffered
+//                 shared-memory tile bias[h][32 queries][16 keys] fp32  (the layout change projection -> logits)
+//   warps 8-15    attention: warp w owns heads 2w, 2w+1 for the tile's 32 queries (two m16 blocks): the MMA
+//                 accumulator is initialised with the bias, S += Q K^T, online softmax in the exp2 domain
+//                 (q is pre-scaled by log2 e / sqrt(c)), P (bf16) feeds PV straight from registers,
+//                 K / V^T fragments are read from L2 with 64-bit loads (a per-16 key permutation makes each
+//                 thread's fragment contiguous), O stays in registers (96 per thread).
+// Work unit = (32-query tile) x (key segment); key tiles are aligned to absolute multiples of 16 and a row's
+// arithmetic depends only on its key segments, so row(P) == monolithic and grid(GxG) == monolithic(key_split=G)
+// bitwise.  No atomics.
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
+#include "kernels.h"
+
+namespace dcp {
+
+namespace {
+
+constexpr int kCz = 128;
+constexpr int kH = 16;
+constexpr int kTileQ = 32;          // queries per work unit
+constexpr int kTileK = 16;          // keys per attention tile
+constexpr int kSubQ = 8;            // queries per z stage
+constexpr int kNZ = 4;              // z stages
+constexpr int kStageBytes = kSubQ * kTileK * kCz * 2;   // 32 KB
+constexpr int kHalfBytes = kStageBytes / 2;
+constexpr int kBiasHeadPitch = kTileQ * kTileK + 4;     // floats; +4: conflict-free projection stores
+constexpr int kBiasBufFloats = kH * kBiasHeadPitch;
+constexpr int kWtPitch = kCz / 2 + 4;                   // 32-bit words per head row of W'^T (+4: conflict-free)
+constexpr int kThreads = 512;
+constexpr int kProjWarp0 = 4, kNumProjWarps = 4, kAttnWarp0 = 8, kNumAttnWarps = 8;
+
+constexpr size_t kSmemZ = 0;
+constexpr size_t kSmemBias = kSmemZ + (size_t)kNZ * kStageBytes;
+constexpr size_t kSmemWt = kSmemBias + 2 * (size_t)kBiasBufFloats * 4;
+constexpr size_t kSmemBar = kSmemWt + (size_t)kH * kWtPitch * 4;
+constexpr size_t kSmemTotal = kSmemBar + (2 * kNZ + 4) * 8;
+constexpr size_t kSmemAlloc = kSmemTotal + 1024;        // slack for 1024-byte alignment of the swizzled stages
+
+// ------------------------------------------------------------------ PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tmap, int c0, int c1, int c2, uint32_t bar,
+                                            uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(policy)
+      : "memory");
+}
+__device__ __forceinline__ void ldmatrix_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+__device__ __forceinline__ void mma_bf16(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
+                                         uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, "
+               "{%0, %1, %2, %3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ float bf_lo(uint32_t x) { return __uint_as_float(x << 16); }
+__device__ __forceinline__ float bf_hi(uint32_t x) { return __uint_as_float(x & 0xffff0000u); }
+__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+__device__ __forceinline__ float fast_exp2(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ uint2 ldg_u2(const void* p) { return __ldg(reinterpret_cast<const uint2*>(p)); }
+__device__ __forceinline__ float quad_max(float v) {
+  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1));
+  return fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 2));
+}
+__device__ __forceinline__ float quad_sum(float v) {
+  v += __shfl_xor_sync(0xffffffffu, v, 1);
+  return v + __shfl_xor_sync(0xffffffffu, v, 2);
+}
+
+// ------------------------------------------------------------------ work units
+struct Unit {
+  int q0;      // first query row of the 32-row tile
+  int q_end;   // end of the query part the tile belongs to (rows >= q_end are not computed / stored)
+  int ks, ke;  // key segment
+  int slot;    // partial-state slot
+};
+
+// Eq. 5 in 32-bit (I <= 2^30)
+__device__ __forceinline__ void shard32(int n, int parts, int p, int* start, int* len) {
+  const int base = n / parts, rem = n % parts;
+  *len = base + (p < rem ? 1 : 0);
+  *start = p * base + (p < rem ? p : rem);
+}
+
+__host__ __device__ inline int64_t mma_num_units(int n, int n_qparts, int n_kparts, int nseg) {
+  // query parts have sizes floor(n/P) or floor(n/P)+1 (Eq. 5): count their 32-row tiles in closed form
+  const int base = n / n_qparts, rem = n % n_qparts;
+  const int t_big = (base + 1 + kTileQ - 1) / kTileQ, t_small = (base + kTileQ - 1) / kTileQ;
+  return ((int64_t)rem * t_big + (int64_t)(n_qparts - rem) * t_small) * n_kparts * nseg;
+}
+
+__device__ __forceinline__ Unit decode_unit(const MmaParams& p, int u) {
+  const int n = p.q_end - p.q_begin;
+  const int base = n / p.n_qparts, rem = n % p.n_qparts;
+  const int t_big = (base + 1 + kTileQ - 1) / kTileQ, t_small = (base + kTileQ - 1) / kTileQ;
+  const int per_tile = p.n_kparts * p.nseg;
+  int tile = u / per_tile;
+  const int r = u - tile * per_tile;
+  int part, tq;
+  if (tile < rem * t_big) { part = tile / t_big; tq = tile - part * t_big; }
+  else { tile -= rem * t_big; part = tile / t_small; tq = tile - part * t_small; part += rem; }
+  int ps, pl;
+  shard32(n, p.n_qparts, part, &ps, &pl);
+  Unit un;
+  un.q0 = p.q_begin + ps + tq * kTileQ;
+  un.q_end = p.q_begin + ps + pl;
+  const int cb = r / p.nseg, sg = r - cb * p.nseg;
+  int cs, cl, ss, sl;
+  shard32(p.k_end - p.k_begin, p.n_kparts, cb, &cs, &cl);
+  shard32(cl, p.nseg, sg, &ss, &sl);
+  un.ks = p.k_begin + cs + ss;
+  un.ke = un.ks + sl;
+  un.slot = p.slot0 + r;
+  return un;
+}
+
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+
+// ------------------------------------------------------------------ the kernel
+// C = head dim, CP = C rounded up to a multiple of 16 (q/k rows are zero-padded to CP by the prologue)
+template <int C, int CP>
+__global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_constant__ CUtensorMap tmap_z,
+                                                                const MmaParams p) {
+  extern __shared__ unsigned char smem_dyn[];
+  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
+  const uint32_t s_z = smem_u32(smem + kSmemZ);
+  float* s_bias = reinterpret_cast<float*>(smem + kSmemBias);
+  uint32_t* s_wt = reinterpret_cast<uint32_t*>(smem + kSmemWt);
+  const uint32_t s_bar = smem_u32(smem + kSmemBar);
+  const uint32_t bar_zfull = s_bar, bar_zempty = s_bar + 8 * kNZ, bar_bfull = s_bar + 16 * kNZ,
+                 bar_bempty = s_bar + 16 * kNZ + 16;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int g = lane >> 2, t = lane & 3;
+
+  // W'^T table [16 heads][64 words] (two bf16 channels per word), row pitch kWtPitch words
+  for (int e = threadIdx.x; e < kH * (kCz / 2); e += kThreads) {
+    const int h = e / (kCz / 2), wd = e % (kCz / 2);
+    s_wt[h * kWtPitch + wd] = reinterpret_cast<const uint32_t*>(p.wfold)[h * (kCz / 2) + wd];
+  }
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, kNumProjWarps); }
+    for (int b = 0; b < 2; ++b) { mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+
+  const int n_units = (int)mma_num_units(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
+
+  if (warp < kProjWarp0) {
+    // =============================================================== TMA producer (warp 0, one lane)
+    reg_dec<24>();
+    if (warp == 0 && lane == 0) {
+      uint64_t policy;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const Unit un = decode_unit(p, u);
+        const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
+        const int nsub = (rows + kSubQ - 1) / kSubQ;
+        for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
+          for (int sub = 0; sub < nsub; ++sub) {
+            mbar_wait(bar_zempty + 8 * stage, phase ^ 1);
+            mbar_expect_tx(bar_zfull + 8 * stage, kStageBytes);
+            const uint32_t dst = s_z + stage * kStageBytes;
+            const int qrow = un.q0 + sub * kSubQ;
+            tma_load_3d(dst, &tmap_z, 0, j0, qrow, bar_zfull + 8 * stage, policy);
+            tma_load_3d(dst + kHalfBytes, &tmap_z, 64, j0, qrow, bar_zfull + 8 * stage, policy);
+            if (++stage == kNZ) { stage = 0; phase ^= 1; }
+          }
+        }
+      }
+    }
+  } else if (warp < kAttnWarp0) {
+    // =============================================================== bias projection + LayerNorm statistics
+    reg_dec<88>();
+    const int pw = warp - kProjWarp0;
+    // the 4 heads this thread finalises: 2t, 2t+1 (n-block 0) and 8+2t, 8+2t+1 (n-block 1)
+    float c1h[4], c0h[4];
+#pragma unroll
+    for (int x = 0; x < 4; ++x) {
+      const int h = (x >> 1) * 8 + 2 * t + (x & 1);
+      c1h[x] = p.c1[h];
+      c0h[x] = p.c0[h];
+    }
+    // ldmatrix source row of this lane inside an m16 block, and its swizzle phase
+    const int lrow = (lane & 7) + ((lane >> 3) & 1) * 8;
+    const int lchunk = lane >> 4;
+    int stage = 0, bbuf = 0;
+    uint32_t phase = 0, bphase = 0;
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+      const Unit un = decode_unit(p, u);
+      const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
+      const int nsub = (rows + kSubQ - 1) / kSubQ;
+      for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
+        mbar_wait(bar_bempty + 8 * bbuf, bphase ^ 1);
+        float* bias_buf = s_bias + bbuf * kBiasBufFloats;
+        for (int sub = 0; sub < nsub; ++sub) {
+          mbar_wait(bar_zfull + 8 * stage, phase);
+          const uint32_t zs = s_z + stage * kStageBytes;
+#pragma unroll 1
+          for (int mb = 0; mb < 2; ++mb) {
+            const int ql = pw * 2 + mb;                  // query inside the stage (0..7)
+            const int row = ql * kTileK + lrow;          // smem row of this lane's ldmatrix address
+            uint32_t a[8][4];
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+              const int chunk = (ks & 3) * 2 + lchunk;
+              const uint32_t addr = zs + (ks >> 2) * kHalfBytes + row * 128 + ((chunk ^ (row & 7)) << 4);
+              ldmatrix_x4(addr, a[ks][0], a[ks][1], a[ks][2], a[ks][3]);
+            }
+            // ---- a2: LayerNorm statistics, two-pass in fp32 (rows g and g+8 of the block)
+            float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+              s0 += bf_lo(a[ks][0]) + bf_hi(a[ks][0]) + bf_lo(a[ks][2]) + bf_hi(a[ks][2]);
+              s1 += bf_lo(a[ks][1]) + bf_hi(a[ks][1]) + bf_lo(a[ks][3]) + bf_hi(a[ks][3]);
+            }
+            const float mu0 = quad_sum(s0) * (1.f / kCz), mu1 = quad_sum(s1) * (1.f / kCz);
+            float v0 = 0.f, v1 = 0.f;
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+              float d;
+              d = bf_lo(a[ks][0]) - mu0; v0 = fmaf(d, d, v0);
+              d = bf_hi(a[ks][0]) - mu0; v0 = fmaf(d, d, v0);
+              d = bf_lo(a[ks][2]) - mu0; v0 = fmaf(d, d, v0);
+              d = bf_hi(a[ks][2]) - mu0; v0 = fmaf(d, d, v0);
+              d = bf_lo(a[ks][1]) - mu1; v1 = fmaf(d, d, v1);
+              d = bf_hi(a[ks][1]) - mu1; v1 = fmaf(d, d, v1);
+              d = bf_lo(a[ks][3]) - mu1; v1 = fmaf(d, d, v1);
+              d = bf_hi(a[ks][3]) - mu1; v1 = fmaf(d, d, v1);
+            }
+            const float rstd0 = rsqrtf(quad_sum(v0) * (1.f / kCz) + p.eps);
+            const float rstd1 = rsqrtf(quad_sum(v1) * (1.f / kCz) + p.eps);
+            // ---- a3: raw z . W'   (W' = gamma (.) W_b * log2 e, bf16)
+            float acc0[4] = {0.f, 0.f, 0.f, 0.f}, acc1[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+              const uint32_t* w0 = s_wt + g * kWtPitch + ks * 8 + t;
+              const uint32_t* w1 = w0 + 8 * kWtPitch;
+              mma_bf16(acc0, a[ks][0], a[ks][1], a[ks][2], a[ks][3], w0[0], w0[4]);
+              mma_bf16(acc1, a[ks][0], a[ks][1], a[ks][2], a[ks][3], w1[0], w1[4]);
+            }
+            // ---- LN(z) W_b = rstd * (z.W' - mu * c1) + c0 ; store to bias[h][query][key]
+            const float nm0 = -mu0 * rstd0, nm1 = -mu1 * rstd1;
+            float* brow = bias_buf + (sub * kSubQ + ql) * kTileK;
+            {
+              float* b = brow + (2 * t) * kBiasHeadPitch;
+              b[g] = fmaf(acc0[0], rstd0, fmaf(nm0, c1h[0], c0h[0]));
+              b[g + 8] = fmaf(acc0[2], rstd1, fmaf(nm1, c1h[0], c0h[0]));
+              b += kBiasHeadPitch;
+              b[g] = fmaf(acc0[1], rstd0, fmaf(nm0, c1h[1], c0h[1]));
+              b[g + 8] = fmaf(acc0[3], rstd1, fmaf(nm1, c1h[1], c0h[1]));
+              b = brow + (8 + 2 * t) * kBiasHeadPitch;
+              b[g] = fmaf(acc1[0], rstd0, fmaf(nm0, c1h[2], c0h[2]));
+              b[g + 8] = fmaf(acc1[2], rstd1, fmaf(nm1, c1h[2], c0h[2]));
+              b += kBiasHeadPitch;
+              b[g] = fmaf(acc1[1], rstd0, fmaf(nm0, c1h[3], c0h[3]));
+              b[g + 8] = fmaf(acc1[3], rstd1, fmaf(nm1, c1h[3], c0h[3]));
+            }
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_zempty + 8 * stage);
+          if (++stage == kNZ) { stage = 0; phase ^= 1; }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_bfull + 8 * bbuf);
+        bbuf ^= 1;
+        if (bbuf == 0) bphase ^= 1;
+      }
+    }
+  } else {
+    // =============================================================== attention: QK^T + bias, online softmax, PV
+    reg_inc<200>();
+    const int aw = warp - kAttnWarp0;
+    constexpr int KK = CP / 16;     // k-steps of QK^T
+    constexpr int ND = C / 8;       // n-blocks of PV
+    const __nv_bfloat16* qp = reinterpret_cast<const __nv_bfloat16*>(p.qp);
+    const __nv_bfloat16* kp = reinterpret_cast<const __nv_bfloat16*>(p.kp);
+    const __nv_bfloat16* vt = reinterpret_cast<const __nv_bfloat16*>(p.vt);
+    int bbuf = 0;
+    uint32_t bphase = 0;
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+      const Unit un = decode_unit(p, u);
+      // Q fragments: [head][m-block][k-step] -> (a0,a2) of row g and (a1,a3) of row g+8
+      uint2 qa[2][2][KK], qb[2][2][KK];
+#pragma unroll
+      for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+        for (int mb = 0; mb < 2; ++mb) {
+          int r0i = un.q0 + mb * 16 + g, r1i = r0i + 8;
+          const int64_t r0 = r0i < p.I ? r0i : p.I - 1;
+          const int64_t r1 = r1i < p.I ? r1i : p.I - 1;
+          const int h = 2 * aw + hh;
+#pragma unroll
+          for (int kk = 0; kk < KK; ++kk) {
+            qa[hh][mb][kk] = ldg_u2(qp + (r0 * kH + h) * CP + kk * 16 + 4 * t);
+            qb[hh][mb][kk] = ldg_u2(qp + (r1 * kH + h) * CP + kk * 16 + 4 * t);
+          }
+        }
+      float o[2][2][ND][4];
+      float m_run[2][2][2], l_run[2][2][2];
+#pragma unroll
+      for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+        for (int mb = 0; mb < 2; ++mb) {
+          m_run[hh][mb][0] = m_run[hh][mb][1] = -INFINITY;
+          l_run[hh][mb][0] = l_run[hh][mb][1] = 0.f;
+#pragma unroll
+          for (int nd = 0; nd < ND; ++nd)
+#pragma unroll
+            for (int x = 0; x < 4; ++x) o[hh][mb][nd][x] = 0.f;
+        }
+
+      for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
+        const bool partial = (j0 < un.ks) || (j0 + kTileK > un.ke);
+        // key of S column: n-block A col c <-> j0 + 4*(c/2) + c%2, n-block B col c <-> that + 2
+        const int kAi = j0 + 4 * (g >> 1) + (g & 1);
+        const int64_t keyA = kAi < p.I ? kAi : p.I - 1;
+        const int64_t keyB = kAi + 2 < p.I ? kAi + 2 : p.I - 1;
+        mbar_wait(bar_bfull + 8 * bbuf, bphase);
+        const float* bias_buf = s_bias + bbuf * kBiasBufFloats;
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+          const int h = 2 * aw + hh;
+          uint2 kA[KK], kB[KK], vf[ND];
+#pragma unroll
+          for (int kk = 0; kk < KK; ++kk) {
+            kA[kk] = ldg_u2(kp + (keyA * kH + h) * CP + kk * 16 + 4 * t);
+            kB[kk] = ldg_u2(kp + (keyB * kH + h) * CP + kk * 16 + 4 * t);
+          }
+#pragma unroll
+          for (int nd = 0; nd < ND; ++nd) vf[nd] = ldg_u2(vt + ((int64_t)(h * C + nd * 8 + g)) * p.ldv + j0 + 4 * t);
+#pragma unroll
+          for (int mb = 0; mb < 2; ++mb) {
+            const float4 b0 = *reinterpret_cast<const float4*>(bias_buf + h * kBiasHeadPitch + (mb * 16 + g) * kTileK + 4 * t);
+            const float4 b1 = *reinterpret_cast<const float4*>(bias_buf + h * kBiasHeadPitch + (mb * 16 + g + 8) * kTileK + 4 * t);
+            float sA[4] = {b0.x, b0.y, b1.x, b1.y};
+            float sB[4] = {b0.z, b0.w, b1.z, b1.w};
+#pragma unroll
+            for (int kk = 0; kk < KK; ++kk) {
+              mma_bf16(sA, qa[hh][mb][kk].x, qb[hh][mb][kk].x, qa[hh][mb][kk].y, qb[hh][mb][kk].y, kA[kk].x, kA[kk].y);
+              mma_bf16(sB, qa[hh][mb][kk].x, qb[hh][mb][kk].x, qa[hh][mb][kk].y, qb[hh][mb][kk].y, kB[kk].x, kB[kk].y);
+            }
+            if (partial) {
+              const int k0 = j0 + 4 * t;
+              if (k0 < un.ks || k0 >= un.ke) { sA[0] = -INFINITY; sA[2] = -INFINITY; }
+              if (k0 + 1 < un.ks || k0 + 1 >= un.ke) { sA[1] = -INFINITY; sA[3] = -INFINITY; }
+              if (k0 + 2 < un.ks || k0 + 2 >= un.ke) { sB[0] = -INFINITY; sB[2] = -INFINITY; }
+              if (k0 + 3 < un.ks || k0 + 3 >= un.ke) { sB[1] = -INFINITY; sB[3] = -INFINITY; }
+            }
+            // ---- a5: online softmax (exp2 domain), rows g (x = 0) and g+8 (x = 1)
+            const float mx0 = quad_max(fmaxf(fmaxf(sA[0], sA[1]), fmaxf(sB[0], sB[1])));
+            const float mx1 = quad_max(fmaxf(fmaxf(sA[2], sA[3]), fmaxf(sB[2], sB[3])));
+            const float mn0 = fmaxf(m_run[hh][mb][0], mx0), mn1 = fmaxf(m_run[hh][mb][1], mx1);
+            const float al0 = fast_exp2(m_run[hh][mb][0] - mn0), al1 = fast_exp2(m_run[hh][mb][1] - mn1);
+            m_run[hh][mb][0] = mn0;
+            m_run[hh][mb][1] = mn1;
+            sA[0] = fast_exp2(sA[0] - mn0); sA[1] = fast_exp2(sA[1] - mn0);
+            sB[0] = fast_exp2(sB[0] - mn0); sB[1] = fast_exp2(sB[1] - mn0);
+            sA[2] = fast_exp2(sA[2] - mn1); sA[3] = fast_exp2(sA[3] - mn1);
+            sB[2] = fast_exp2(sB[2] - mn1); sB[3] = fast_exp2(sB[3] - mn1);
+            l_run[hh][mb][0] = fmaf(l_run[hh][mb][0], al0, (sA[0] + sA[1]) + (sB[0] + sB[1]));
+            l_run[hh][mb][1] = fmaf(l_run[hh][mb][1], al1, (sA[2] + sA[3]) + (sB[2] + sB[3]));
+            const uint32_t p0 = pack_bf16(sA[0], sA[1]), p1 = pack_bf16(sA[2], sA[3]);
+            const uint32_t p2 = pack_bf16(sB[0], sB[1]), p3 = pack_bf16(sB[2], sB[3]);
+            // ---- a6: acc = acc * alpha + P V
+#pragma unroll
+            for (int nd = 0; nd < ND; ++nd) {
+              o[hh][mb][nd][0] *= al0; o[hh][mb][nd][1] *= al0;
+              o[hh][mb][nd][2] *= al1; o[hh][mb][nd][3] *= al1;
+              mma_bf16(o[hh][mb][nd], p0, p1, p2, p3, vf[nd].x, vf[nd].y);
+            }
+          }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_bempty + 8 * bbuf);
+        bbuf ^= 1;
+        if (bbuf == 0) bphase ^= 1;
+      }
+
+      // ---- a7: partial state of (rows, key segment) -> slot   (m back in natural-log units)
+      constexpr float kLn2 = 0.6931471805599453f;
+#pragma unroll
+      for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+        for (int mb = 0; mb < 2; ++mb)
+#pragma unroll
+          for (int x = 0; x < 2; ++x) {
+            const float l = quad_sum(l_run[hh][mb][x]);
+            const int row = un.q0 + mb * 16 + g + 8 * x;
+            if (row < un.q_end) {
+              const int h = 2 * aw + hh;
+              const int64_t srow = (int64_t)un.slot * p.state_rows + (row - p.state_row0);
+              if (t == 0) {
+                p.st_m[srow * kH + h] = m_run[hh][mb][x] * kLn2;
+                p.st_l[srow * kH + h] = l;
+              }
+              float* dst = p.st_acc + srow * (kH * C) + h * C + 2 * t;
+#pragma unroll
+              for (int nd = 0; nd < ND; ++nd)
+                *reinterpret_cast<float2*>(dst + nd * 8) = make_float2(o[hh][mb][nd][2 * x], o[hh][mb][nd][2 * x + 1]);
+            }
+          }
+    }
+  }
+}
+
+// ------------------------------------------------------------------ host side
+PFN_cuTensorMapEncodeTiled get_encode_fn() {
+  static PFN_cuTensorMapEncodeTiled fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* ptr = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(ptr);
+  }
+  return fn;
+}
+
+template <int C, int CP>
+cudaError_t launch_c(const CUtensorMap& tm, const MmaParams& p, int64_t units, cudaStream_t st) {
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(fused_mma_kernel<C, CP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemAlloc);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (sms <= 0) sms = 148;
+  const unsigned grid = (unsigned)(units < sms ? units : sms);
+  fused_mma_kernel<C, CP><<<grid, kThreads, kSmemAlloc, st>>>(tm, p);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
+bool fused_mma_supports(dcp_dtype dt, int H, int c, int c_z) {
+  return dt == DCP_BF16 && H == kH && c_z == kCz && (c == 24 || c == 32 || c == 48);
+}
+
+int mma_head_pad(int c) { return (c + 15) / 16 * 16; }
+int64_t mma_ldv(int64_t I) { return (I + 15) / 16 * 16; }
+
+// Segments per key chunk: a pure function of (I, n_kparts) so every decomposition cuts a row's keys alike.
+// Picks the count that best fills 148 SMs with (32-query tile) x (segment) units, charging the partial-state
+// round trip (~25 * segments / I of the z bytes) and keeping segments >= 64 keys.
+int mma_num_segments(int64_t I, int n_kparts) {
+  const int64_t qtiles = (I + kTileQ - 1) / kTileQ;
+  const int64_t chunk = I / n_kparts;
+  int best = 1;
+  double best_score = -1.0;
+  for (int s = 1; s <= 16; ++s) {
+    if (s > 1 && chunk / s < 64) break;
+    const int64_t units = qtiles * n_kparts * s;
+    const int64_t waves = (units + 147) / 148;
+    const double fill = (double)units / (double)(waves * 148);
+    const double extra = 25.0 * s * n_kparts / (double)I;
+    const double score = fill / (1.0 + extra);
+    if (score > best_score + 1e-9) { best_score = score; best = s; }
+  }
+  return best;
+}
+
+cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st) {
+  if (p.q_end <= p.q_begin || p.k_end <= p.k_begin) return cudaSuccess;
+  PFN_cuTensorMapEncodeTiled enc = get_encode_fn();
+  if (!enc) return cudaErrorNotSupported;
+  CUtensorMap tm;
+  const cuuint64_t gdim[3] = {(cuuint64_t)kCz, (cuuint64_t)p.I, (cuuint64_t)p.I};
+  const cuuint64_t gstr[2] = {(cuuint64_t)kCz * 2, (cuuint64_t)ldz * 2};
+  const cuuint32_t box[3] = {64, kTileK, kSubQ};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(z), gdim, gstr, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  const int64_t units = mma_num_units(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
+  if (units > 0x7fffffff) return cudaErrorInvalidValue;
+  switch (p.c) {
+    case 24: return launch_c<24, 32>(tm, p, units, st);
+    case 32: return launch_c<32, 32>(tm, p, units, st);
+    case 48: return launch_c<48, 48>(tm, p, units, st);
+    default: return cudaErrorInvalidValue;
+  }
+}
+
+}  // namespace dcp

@@ -1,0 +1,223 @@
+// Tensor-core GEMMs of the bf16 path: the single-track projections (step a1) and the output projection (step a9).
+//   PAPER.md:77-81 (sec 3.2): Q^(p) = f_Q(S^(p)); "keys and values are projected from the full single-track S"
+//   BASELINE.json config 0:  out = W_o (sigmoid(s W_g) (.) softmax(...) V)
+// C[M, N] = A[M, K] (bf16, row-major) x W[K, N] (bf16, row-major), fp32 accumulate, mma.sync m16n8k16,
+// 128 x 128 x 32 CTA tiles, cp.async double buffering.  The four projections run as ONE launch over
+// N = 4 D columns; the epilogue writes each segment in the layout the fused kernel reads:
+//   q -> qp [I][H][CP]  scaled by log2(e)/sqrt(c) (exp2-domain softmax), head rows zero-padded to CP
+//   k -> kp [I][H][CP]
+//   v -> vt [H*c][ldv]  transposed (key index contiguous) so PV's B fragments are 64-bit loads
+//   g -> g  [I][D]      sigmoid gate
+// Every output element is accumulated over k in a fixed order that does not depend on the tile it falls in.
+#include "kernels.h"
+
+namespace dcp {
+
+namespace {
+
+constexpr int BM = 128, BN = 128, BK = 32;
+constexpr int LDA_S = BK + 8;    // padded smem rows: conflict-free ldmatrix
+constexpr int LDB_S = BN + 8;
+
+__device__ __forceinline__ void cp_async16(void* dst, const void* src, bool ok) {
+  const uint32_t d = (uint32_t)__cvta_generic_to_shared(dst);
+  const int n = ok ? 16 : 0;
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
+}
+__device__ __forceinline__ void mma16816(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, "
+               "{%0, %1, %2, %3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+__global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
+  __shared__ __align__(16) __nv_bfloat16 As[2][BM * LDA_S];
+  __shared__ __align__(16) __nv_bfloat16 Bs[2][BK * LDB_S];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int wm = warp >> 2, wn = warp & 3;            // 2 x 4 warps, warp tile 64 x 32
+  const int nb_per_seg = (p.N + BN - 1) / BN;
+  const int seg = blockIdx.x / nb_per_seg;
+  const int n0 = (blockIdx.x % nb_per_seg) * BN;
+  const int64_t m0 = (int64_t)blockIdx.y * BM;
+  const __nv_bfloat16* A = reinterpret_cast<const __nv_bfloat16*>(p.A);
+  const __nv_bfloat16* W = reinterpret_cast<const __nv_bfloat16*>(p.W[seg]);
+
+  float acc[4][4][4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+#pragma unroll
+      for (int x = 0; x < 4; ++x) acc[i][j][x] = 0.f;
+
+  auto load_tile = [&](int buf, int k0) {
+#pragma unroll
+    for (int it = 0; it < 2; ++it) {
+      const int e = tid + it * 256;
+      {   // A: 128 rows x 4 chunks of 8 elements
+        const int r = e >> 2, ch = e & 3;
+        const int64_t gm = m0 + r;
+        const int gk = k0 + ch * 8;
+        const bool ok = gm < p.M && gk < p.K;
+        cp_async16(&As[buf][r * LDA_S + ch * 8], ok ? (const void*)(A + gm * p.lda + gk) : (const void*)A, ok);
+      }
+      {   // W: 32 rows x 16 chunks
+        const int r = e >> 4, ch = e & 15;
+        const int gk = k0 + r, gn = n0 + ch * 8;
+        const bool ok = gk < p.K && gn < p.N;
+        cp_async16(&Bs[buf][r * LDB_S + ch * 8], ok ? (const void*)(W + (int64_t)gk * p.N + gn) : (const void*)W, ok);
+      }
+    }
+    cp_async_commit();
+  };
+
+  const int nk = (p.K + BK - 1) / BK;
+  load_tile(0, 0);
+  for (int kt = 0; kt < nk; ++kt) {
+    const int buf = kt & 1;
+    if (kt + 1 < nk) { load_tile(buf ^ 1, (kt + 1) * BK); cp_async_wait<1>(); }
+    else cp_async_wait<0>();
+    __syncthreads();
+#pragma unroll
+    for (int ks = 0; ks < BK / 16; ++ks) {
+      uint32_t af[4][4], bf[4][2];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const int row = wm * 64 + i * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+        const int col = ks * 16 + (lane >> 4) * 8;
+        ldsm_x4((uint32_t)__cvta_generic_to_shared(&As[buf][row * LDA_S + col]), af[i][0], af[i][1], af[i][2], af[i][3]);
+      }
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const int krow = ks * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+        const int col = wn * 32 + j * 16 + (lane >> 4) * 8;
+        ldsm_x4_t((uint32_t)__cvta_generic_to_shared(&Bs[buf][krow * LDB_S + col]), bf[2 * j][0], bf[2 * j][1],
+                  bf[2 * j + 1][0], bf[2 * j + 1][1]);
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) mma16816(acc[i][j], af[i], bf[j][0], bf[j][1]);
+    }
+    __syncthreads();
+  }
+
+  // ---- epilogue
+  const int g = lane >> 2, t = lane & 3;
+  const int mode = p.mode[seg];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int x = 0; x < 2; ++x) {
+      const int64_t row = m0 + wm * 64 + i * 16 + g + 8 * x;
+      if (row >= p.M) continue;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int col = n0 + wn * 32 + j * 8 + 2 * t;
+        if (col >= p.N) continue;
+        float v0 = acc[i][j][2 * x], v1 = acc[i][j][2 * x + 1];
+        if (p.bias[seg] != nullptr) {
+          const __nv_bfloat16* b = reinterpret_cast<const __nv_bfloat16*>(p.bias[seg]);
+          v0 += __bfloat162float(b[col]);
+          v1 += __bfloat162float(b[col + 1]);
+        }
+        __nv_bfloat16* C = reinterpret_cast<__nv_bfloat16*>(p.C[seg]);
+        if (mode == GEMM_OUT_PLAIN) {
+          *reinterpret_cast<__nv_bfloat162*>(C + row * p.ldc[seg] + col) = __floats2bfloat162_rn(v0, v1);
+        } else if (mode == GEMM_OUT_SIGMOID) {
+          v0 = 1.f / (1.f + expf(-v0));
+          v1 = 1.f / (1.f + expf(-v1));
+          *reinterpret_cast<__nv_bfloat162*>(C + row * p.ldc[seg] + col) = __floats2bfloat162_rn(v0, v1);
+        } else if (mode == GEMM_OUT_HEADPAD) {
+          const int h = col / p.c, d = col % p.c;   // c even, col even: the pair stays inside one head
+          *reinterpret_cast<__nv_bfloat162*>(C + (row * p.H + h) * p.cp + d) = __floats2bfloat162_rn(v0 * p.scale[seg], v1 * p.scale[seg]);
+        } else {   // GEMM_OUT_TRANSPOSED: vt[col][row]
+          C[(int64_t)col * p.ldc[seg] + row] = __float2bfloat16_rn(v0);
+          C[(int64_t)(col + 1) * p.ldc[seg] + row] = __float2bfloat16_rn(v1);
+        }
+      }
+    }
+}
+
+__global__ void layernorm_rows_bf16_kernel(const __nv_bfloat16* __restrict__ x, const __nv_bfloat16* __restrict__ gamma,
+                                           const __nv_bfloat16* __restrict__ beta, __nv_bfloat16* __restrict__ y,
+                                           int64_t rows, int width, float eps) {
+  // one warp per row; two-pass, population variance (reading #2 in DESIGN.md); output rounded to bf16
+  int64_t row = (int64_t)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;
+  int lane = threadIdx.x % 32;
+  if (row >= rows) return;
+  const __nv_bfloat16* xr = x + row * width;
+  float s = 0.f;
+  for (int k = lane; k < width; k += 32) s += to_f32(xr[k]);
+  float mu = warp_sum(s) / (float)width;
+  float v = 0.f;
+  for (int k = lane; k < width; k += 32) {
+    float d = to_f32(xr[k]) - mu;
+    v = fmaf(d, d, v);
+  }
+  float rstd = rsqrtf(warp_sum(v) / (float)width + eps);
+  for (int k = lane; k < width; k += 32)
+    y[row * width + k] = __float2bfloat16_rn((to_f32(xr[k]) - mu) * rstd * to_f32(gamma[k]) + to_f32(beta[k]));
+}
+
+__global__ void fold_ln_z_mma_kernel(const __nv_bfloat16* __restrict__ w_b, const __nv_bfloat16* __restrict__ gamma,
+                                     const __nv_bfloat16* __restrict__ beta, __nv_bfloat16* __restrict__ wfold,
+                                     float* __restrict__ c1, float* __restrict__ c0, int c_z, int H, int H_pad) {
+  // wfold[h][k] = bf16(gamma_k W_b[k,h] log2 e)   (K-major rows: the B operand of the projection MMA)
+  // c1[h] = sum_k wfold[h][k] (the rounded values, ascending k), c0[h] = log2 e * sum_k beta_k W_b[k,h]
+  constexpr float kLog2e = 1.4426950408889634f;
+  for (int e = threadIdx.x; e < H_pad * c_z; e += blockDim.x) {
+    const int h = e / c_z, k = e % c_z;
+    const float v = h < H ? to_f32(gamma[k]) * to_f32(w_b[k * H + h]) * kLog2e : 0.f;
+    wfold[e] = __float2bfloat16_rn(v);
+  }
+  __syncthreads();
+  if (threadIdx.x < H_pad) {
+    const int h = threadIdx.x;
+    float a1 = 0.f, a0 = 0.f;
+    for (int k = 0; k < c_z; ++k) {
+      a1 += to_f32(wfold[h * c_z + k]);
+      if (h < H) a0 = fmaf(to_f32(beta[k]), to_f32(w_b[k * H + h]), a0);
+    }
+    c1[h] = a1;
+    c0[h] = a0 * kLog2e;
+  }
+}
+
+}  // namespace
+
+cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st) {
+  if (p.M <= 0 || p.N <= 0 || p.K <= 0) return cudaSuccess;
+  if (p.K % 8 != 0 || p.N % 8 != 0 || p.lda % 8 != 0) return cudaErrorInvalidValue;
+  dim3 grid((unsigned)(p.nseg * ((p.N + BN - 1) / BN)), (unsigned)((p.M + BM - 1) / BM));
+  gemm_mma_kernel<<<grid, 256, 0, st>>>(p);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_layernorm_rows_bf16(const void* x, const void* gamma, const void* beta, void* y, int64_t rows,
+                                       int width, float eps, cudaStream_t st) {
+  unsigned blocks = (unsigned)((rows + 7) / 8);
+  layernorm_rows_bf16_kernel<<<blocks, 256, 0, st>>>((const __nv_bfloat16*)x, (const __nv_bfloat16*)gamma,
+                                                     (const __nv_bfloat16*)beta, (__nv_bfloat16*)y, rows, width, eps);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_fold_ln_z_mma(const void* w_b, const void* gamma, const void* beta, void* wfold, float* c1, float* c0,
+                                 int c_z, int H, int H_pad, cudaStream_t st) {
+  fold_ln_z_mma_kernel<<<1, 256, 0, st>>>((const __nv_bfloat16*)w_b, (const __nv_bfloat16*)gamma,
+                                          (const __nv_bfloat16*)beta, (__nv_bfloat16*)wfold, c1, c0, c_z, H, H_pad);
+  return cudaGetLastError();
+}
+
+}  // namespace dcp

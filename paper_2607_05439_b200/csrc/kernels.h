@@ -11,10 +11,6 @@ enum GemmEpilogue { EPI_NONE = 0, EPI_SIGMOID = 1 };
 cudaError_t launch_gemm(dcp_dtype dt, bool a_is_f32, const void* A, int64_t lda, const void* W, const void* bias,
                         void* C, int64_t ldc, int64_t M, int N, int K, GemmEpilogue epi, cudaStream_t st);
 
-// Tensor-core (mma.sync bf16) version of the same GEMM for the bf16 path; A, W, C bf16.
-cudaError_t launch_gemm_bf16_mma(const void* A, int64_t lda, const void* W, const void* bias, void* C, int64_t ldc,
-                                 int64_t M, int N, int K, GemmEpilogue epi, cudaStream_t st);
-
 // s~ = LayerNorm(s; gamma, beta) -> float [rows, width]      (optional LN_s, reading #3 in DESIGN.md)
 cudaError_t launch_layernorm_rows(dcp_dtype dt, const void* x, const void* gamma, const void* beta, float* y,
                                   int64_t rows, int width, float eps, cudaStream_t st);
@@ -27,17 +23,57 @@ cudaError_t launch_fold_ln_z(dcp_dtype dt, const void* w_b, const void* gamma, c
 cudaError_t launch_fused_generic(dcp_dtype dt, const FusedParams& p, cudaStream_t st);
 bool fused_generic_supports(dcp_dtype dt, int H, int c, int c_z);
 
-// bf16 tensor-core fused kernel (TMA-streamed z).  Workspace for folded bf16 weights is carved by api.cu.
-struct MmaAux {
-  const void* wfold;    // [H_pad, c_z] bf16: (gamma (.) W_b)^T, K-major
-  const float* c1;      // [H] sum_k wfold[h,k]  (for the -mu*c1 term)
-  const float* c0;      // [H]
-  void* tmap_z;         // host pointer to a CUtensorMap for z (128 B, passed by value into the kernel)
+// ---- bf16 tensor-core path (fused_mma.cu, gemm_mma.cu)
+enum GemmOutMode { GEMM_OUT_PLAIN = 0, GEMM_OUT_SIGMOID = 1, GEMM_OUT_HEADPAD = 2, GEMM_OUT_TRANSPOSED = 3 };
+
+// C_seg = epi(A[M,K] * W_seg[K,N] + bias_seg) for seg < nseg, all bf16 with fp32 accumulation (one launch).
+struct GemmMmaParams {
+  const void* A;        // [M, K] bf16, row pitch lda
+  int64_t lda, M;
+  int N, K, nseg;
+  const void* W[4];     // [K, N] bf16 row-major
+  const void* bias[4];  // [N] bf16 or nullptr
+  void* C[4];
+  int mode[4];          // GemmOutMode
+  float scale[4];       // HEADPAD only
+  int64_t ldc[4];       // PLAIN / SIGMOID: row pitch; TRANSPOSED: pitch of the transposed rows
+  int H, c, cp;         // HEADPAD: C[(row*H + h)*cp + d] for column h*c + d
 };
-cudaError_t launch_fused_mma(const FusedParams& p, const MmaAux& aux, cudaStream_t st);
-bool fused_mma_supports(dcp_dtype dt, int H, int c, int c_z);
+cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st);
+cudaError_t launch_layernorm_rows_bf16(const void* x, const void* gamma, const void* beta, void* y, int64_t rows,
+                                       int width, float eps, cudaStream_t st);
+// wfold [H_pad][c_z] bf16 = (gamma (.) W_b * log2 e)^T, c1[h] = sum_k wfold[h][k], c0[h] = log2 e * sum_k beta_k W_b[k,h]
 cudaError_t launch_fold_ln_z_mma(const void* w_b, const void* gamma, const void* beta, void* wfold, float* c1,
-                                 float* c0, int c_z, int H, cudaStream_t st);
+                                 float* c0, int c_z, int H, int H_pad, cudaStream_t st);
+
+// One launch of the persistent fused kernel over every (query part, 32-query tile, key chunk, key segment) unit:
+// query rows [q_begin, q_end) cut into n_qparts Eq.-5 parts (row stripes / grid row blocks), keys [k_begin, k_end)
+// into n_kparts Eq.-5 chunks (key_split / grid key blocks), each chunk into nseg Eq.-5 segments; unit
+// (chunk cb, segment sg) writes partial-state slot slot0 + cb*nseg + sg.
+struct MmaParams {
+  const void* qp;       // [I][H][cp] bf16, scaled by log2(e)/sqrt(c)
+  const void* kp;       // [I][H][cp] bf16
+  const void* vt;       // [H*c][ldv] bf16 (key index contiguous, zero beyond I)
+  int64_t ldv;
+  const void* wfold;    // [16][c_z] bf16
+  const float* c1;      // [16]
+  const float* c0;      // [16]
+  float* st_m;          // [slots, state_rows, H]   (natural-log units)
+  float* st_l;          // [slots, state_rows, H]
+  float* st_acc;        // [slots, state_rows, H*c]
+  int64_t state_rows, state_row0;
+  int I;
+  int q_begin, q_end, n_qparts;
+  int k_begin, k_end, n_kparts;
+  int nseg, slot0;
+  int c;
+  float eps;
+};
+cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st);
+bool fused_mma_supports(dcp_dtype dt, int H, int c, int c_z);
+int mma_head_pad(int c);
+int64_t mma_ldv(int64_t I);
+int mma_num_segments(int64_t I, int n_kparts);
 
 // Merge (step a8) + normalise + gate (first half of a9); or raw merged state out.
 cudaError_t launch_merge(dcp_dtype dt, const MergeParams& p, cudaStream_t st);

@@ -55,6 +55,10 @@ def test_c0_fp32_all_decompositions():
     ("f32", 5, 24, 8, 2, 16, False, False),      # I smaller than any tile
     ("bf16", 131, 64, 32, 4, 24, False, False),  # ragged, c = 24
     ("bf16", 200, 128, 16, 4, 32, True, False),  # atom-like widths
+    ("bf16", 131, 64, 128, 16, 24, False, False),  # tensor-core kernel shapes: ragged I, c = 24 (padded to 32)
+    ("bf16", 77, 96, 128, 16, 48, True, True),     # tensor-core kernel, c = 48, LN_s + b_q, I < 3 tiles
+    ("bf16", 200, 64, 128, 16, 32, False, False),  # tensor-core kernel, c = 32
+    ("bf16", 9, 32, 128, 16, 48, False, False),    # tensor-core kernel, I smaller than a tile
 ])
 def test_small_shapes_all_decompositions(dtype, I, c_s, c_z, H, c, ln_s, b_q):
     dcp = _dcp()
@@ -133,11 +137,11 @@ def test_full_size_sampled_rows(name, decomps):
 
 
 # ------------------------------------------------------------------ partial states and the merge kernel
-@pytest.mark.parametrize("dtype", ["f32", "bf16"])
-def test_partial_states_and_merge(dtype):
+@pytest.mark.parametrize("dtype,c_z,H", [("f32", 32, 4), ("bf16", 32, 4), ("bf16", 128, 16)])
+def test_partial_states_and_merge(dtype, c_z, H):
     from oracle import decompositions as dec
     dcp = _dcp()
-    cfg = syn.small_config("ps", I=150, c_s=64, c_z=32, H=4, c=24, dtype=dtype, seed=33)
+    cfg = syn.small_config("ps", I=150, c_s=64, c_z=c_z, H=H, c=24, dtype=dtype, seed=33)
     s, z, w = util.make_problem(cfg, DEV)
     q0, q1 = 37, 101
     rows = list(range(q0, q1))
