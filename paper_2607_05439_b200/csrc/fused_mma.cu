@@ -38,14 +38,12 @@ constexpr int kStageBytes = kSubQ * kTileK * kCz * 2;   // 32 KB
 constexpr int kHalfBytes = kStageBytes / 2;
 constexpr int kBiasHeadPitch = kTileQ * kTileK + 4;     // floats; +4: conflict-free projection stores
 constexpr int kBiasBufFloats = kH * kBiasHeadPitch;
-constexpr int kWtPitch = kCz / 2 + 4;                   // 32-bit words per head row of W'^T (+4: conflict-free)
 constexpr int kThreads = 512;
 constexpr int kProjWarp0 = 4, kNumProjWarps = 4, kAttnWarp0 = 8, kNumAttnWarps = 8;
 
 constexpr size_t kSmemZ = 0;
 constexpr size_t kSmemBias = kSmemZ + (size_t)kNZ * kStageBytes;
-constexpr size_t kSmemWt = kSmemBias + 2 * (size_t)kBiasBufFloats * 4;
-constexpr size_t kSmemBar = kSmemWt + (size_t)kH * kWtPitch * 4;
+constexpr size_t kSmemBar = kSmemBias + 2 * (size_t)kBiasBufFloats * 4;
 constexpr size_t kSmemTotal = kSmemBar + (2 * kNZ + 4) * 8;
 constexpr size_t kSmemAlloc = kSmemTotal + 1024;        // slack for 1024-byte alignment of the swizzled stages
 
@@ -169,7 +167,6 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
   const uint32_t s_z = smem_u32(smem + kSmemZ);
   float* s_bias = reinterpret_cast<float*>(smem + kSmemBias);
-  uint32_t* s_wt = reinterpret_cast<uint32_t*>(smem + kSmemWt);
   const uint32_t s_bar = smem_u32(smem + kSmemBar);
   const uint32_t bar_zfull = s_bar, bar_zempty = s_bar + 8 * kNZ, bar_bfull = s_bar + 16 * kNZ,
                  bar_bempty = s_bar + 16 * kNZ + 16;
@@ -177,11 +174,6 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
 
-  // W'^T table [16 heads][64 words] (two bf16 channels per word), row pitch kWtPitch words
-  for (int e = threadIdx.x; e < kH * (kCz / 2); e += kThreads) {
-    const int h = e / (kCz / 2), wd = e % (kCz / 2);
-    s_wt[h * kWtPitch + wd] = reinterpret_cast<const uint32_t*>(p.wfold)[h * (kCz / 2) + wd];
-  }
   if (threadIdx.x == 0) {
     for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, kNumProjWarps); }
     for (int b = 0; b < 2; ++b) { mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps); }
@@ -229,9 +221,24 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
       c1h[x] = p.c1[h];
       c0h[x] = p.c0[h];
     }
+    // B fragments of W'^T (heads 8*nb + g, channels 16*ks + 2t.. and + 8) stay in registers for the whole kernel
+    uint32_t wf[2][8][2];
+    {
+      const uint32_t* wsrc = reinterpret_cast<const uint32_t*>(p.wfold);
+#pragma unroll
+      for (int nb = 0; nb < 2; ++nb)
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks) {
+          wf[nb][ks][0] = __ldg(wsrc + (nb * 8 + g) * (kCz / 2) + ks * 8 + t);
+          wf[nb][ks][1] = __ldg(wsrc + (nb * 8 + g) * (kCz / 2) + ks * 8 + t + 4);
+        }
+    }
+    constexpr uint32_t kOnes = 0x3f803f80u;   // bf16x2 (1, 1)
     // ldmatrix source row of this lane inside an m16 block, and its swizzle phase
     const int lrow = (lane & 7) + ((lane >> 3) & 1) * 8;
     const int lchunk = lane >> 4;
+    const int diag_src = (lane & ~3) | (g >> 1);   // lane of this quad that holds the Gram diagonal of rows g, g+8
+    const bool diag_odd = (g & 1) != 0;
     int stage = 0, bbuf = 0;
     uint32_t phase = 0, bphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
@@ -244,49 +251,34 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
         for (int sub = 0; sub < nsub; ++sub) {
           mbar_wait(bar_zfull + 8 * stage, phase);
           const uint32_t zs = s_z + stage * kStageBytes;
-#pragma unroll 1
+#pragma unroll
           for (int mb = 0; mb < 2; ++mb) {
             const int ql = pw * 2 + mb;                  // query inside the stage (0..7)
             const int row = ql * kTileK + lrow;          // smem row of this lane's ldmatrix address
-            uint32_t a[8][4];
+            // One m16 block = (query ql) x (16 keys).  Five accumulator chains over the 8 k-steps, all on the
+            // tensor pipe:  a3 = raw z . W' (2 n-blocks);  sum z = z . 1;  sum z^2 = diag(z z^T) (the A fragments
+            // of rows 0-7 / 8-15 are exactly the B fragments of the Gram product).
+            float acc0[4] = {0.f, 0.f, 0.f, 0.f}, acc1[4] = {0.f, 0.f, 0.f, 0.f};
+            float accs[4] = {0.f, 0.f, 0.f, 0.f}, gr0[4] = {0.f, 0.f, 0.f, 0.f}, gr1[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
             for (int ks = 0; ks < 8; ++ks) {
               const int chunk = (ks & 3) * 2 + lchunk;
               const uint32_t addr = zs + (ks >> 2) * kHalfBytes + row * 128 + ((chunk ^ (row & 7)) << 4);
-              ldmatrix_x4(addr, a[ks][0], a[ks][1], a[ks][2], a[ks][3]);
+              uint32_t a0, a1, a2, a3;
+              ldmatrix_x4(addr, a0, a1, a2, a3);
+              mma_bf16(acc0, a0, a1, a2, a3, wf[0][ks][0], wf[0][ks][1]);
+              mma_bf16(acc1, a0, a1, a2, a3, wf[1][ks][0], wf[1][ks][1]);
+              mma_bf16(accs, a0, a1, a2, a3, kOnes, kOnes);
+              mma_bf16(gr0, a0, a1, a2, a3, a0, a2);
+              mma_bf16(gr1, a0, a1, a2, a3, a1, a3);
             }
-            // ---- a2: LayerNorm statistics, two-pass in fp32 (rows g and g+8 of the block)
-            float s0 = 0.f, s1 = 0.f;
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-              s0 += bf_lo(a[ks][0]) + bf_hi(a[ks][0]) + bf_lo(a[ks][2]) + bf_hi(a[ks][2]);
-              s1 += bf_lo(a[ks][1]) + bf_hi(a[ks][1]) + bf_lo(a[ks][3]) + bf_hi(a[ks][3]);
-            }
-            const float mu0 = quad_sum(s0) * (1.f / kCz), mu1 = quad_sum(s1) * (1.f / kCz);
-            float v0 = 0.f, v1 = 0.f;
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-              float d;
-              d = bf_lo(a[ks][0]) - mu0; v0 = fmaf(d, d, v0);
-              d = bf_hi(a[ks][0]) - mu0; v0 = fmaf(d, d, v0);
-              d = bf_lo(a[ks][2]) - mu0; v0 = fmaf(d, d, v0);
-              d = bf_hi(a[ks][2]) - mu0; v0 = fmaf(d, d, v0);
-              d = bf_lo(a[ks][1]) - mu1; v1 = fmaf(d, d, v1);
-              d = bf_hi(a[ks][1]) - mu1; v1 = fmaf(d, d, v1);
-              d = bf_lo(a[ks][3]) - mu1; v1 = fmaf(d, d, v1);
-              d = bf_hi(a[ks][3]) - mu1; v1 = fmaf(d, d, v1);
-            }
-            const float rstd0 = rsqrtf(quad_sum(v0) * (1.f / kCz) + p.eps);
-            const float rstd1 = rsqrtf(quad_sum(v1) * (1.f / kCz) + p.eps);
-            // ---- a3: raw z . W'   (W' = gamma (.) W_b * log2 e, bf16)
-            float acc0[4] = {0.f, 0.f, 0.f, 0.f}, acc1[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-              const uint32_t* w0 = s_wt + g * kWtPitch + ks * 8 + t;
-              const uint32_t* w1 = w0 + 8 * kWtPitch;
-              mma_bf16(acc0, a[ks][0], a[ks][1], a[ks][2], a[ks][3], w0[0], w0[4]);
-              mma_bf16(acc1, a[ks][0], a[ks][1], a[ks][2], a[ks][3], w1[0], w1[4]);
-            }
+            // ---- a2: LayerNorm statistics (fp32): mu = sum/c_z, var = sum z^2 / c_z - mu^2
+            const float sq0 = __shfl_sync(0xffffffffu, diag_odd ? gr0[1] : gr0[0], diag_src);
+            const float sq1 = __shfl_sync(0xffffffffu, diag_odd ? gr1[3] : gr1[2], diag_src);
+            const float mu0 = accs[0] * (1.f / kCz), mu1 = accs[2] * (1.f / kCz);
+            const float var0 = fmaxf(fmaf(sq0, 1.f / kCz, -mu0 * mu0), 0.f);
+            const float var1 = fmaxf(fmaf(sq1, 1.f / kCz, -mu1 * mu1), 0.f);
+            const float rstd0 = rsqrtf(var0 + p.eps), rstd1 = rsqrtf(var1 + p.eps);
             // ---- LN(z) W_b = rstd * (z.W' - mu * c1) + c0 ; store to bias[h][query][key]
             const float nm0 = -mu0 * rstd0, nm1 = -mu1 * rstd1;
             float* brow = bias_buf + (sub * kSubQ + ql) * kTileK;
