@@ -86,6 +86,12 @@ __device__ __forceinline__ void mma_bf16(float (&d)[4], uint32_t a0, uint32_t a1
                "{%0, %1, %2, %3};"
                : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
+__device__ __forceinline__ void sts_f32(uint32_t addr, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory"); }
+__device__ __forceinline__ float4 lds_f32x4(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
+}
 __device__ __forceinline__ float bf_lo(uint32_t x) { return __uint_as_float(x << 16); }
 __device__ __forceinline__ float bf_hi(uint32_t x) { return __uint_as_float(x & 0xffff0000u); }
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
@@ -211,7 +217,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     }
   } else if (warp < kAttnWarp0) {
     // =============================================================== bias projection + LayerNorm statistics
-    reg_dec<88>();
+    reg_dec<104>();
     const int pw = warp - kProjWarp0;
     // the 4 heads this thread finalises: 2t, 2t+1 (n-block 0) and 8+2t, 8+2t+1 (n-block 1)
     float c1h[4], c0h[4];
@@ -247,55 +253,62 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
       const int nsub = (rows + kSubQ - 1) / kSubQ;
       for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
         mbar_wait(bar_bempty + 8 * bbuf, bphase ^ 1);
-        float* bias_buf = s_bias + bbuf * kBiasBufFloats;
+        const uint32_t bias_buf = smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4);
         for (int sub = 0; sub < nsub; ++sub) {
           mbar_wait(bar_zfull + 8 * stage, phase);
           const uint32_t zs = s_z + stage * kStageBytes;
+          // Two m16 blocks at once (queries 2pw, 2pw+1 of the stage) x (16 keys): ten independent accumulator
+          // chains over the 8 k-steps, all on the tensor pipe:  a3 = raw z . W' (2 n-blocks);  sum z = z . 1;
+          // sum z^2 = diag(z z^T) (the A fragments of rows 0-7 / 8-15 are exactly the B fragments of the Gram product).
+          float acc0[2][4], acc1[2][4], accs[2][4], gr0[2][4], gr1[2][4];
+#pragma unroll
+          for (int mb = 0; mb < 2; ++mb)
+#pragma unroll
+            for (int x = 0; x < 4; ++x) acc0[mb][x] = acc1[mb][x] = accs[mb][x] = gr0[mb][x] = gr1[mb][x] = 0.f;
+          const int row0 = (pw * 2) * kTileK + lrow;     // smem row of this lane's ldmatrix address (block 0)
+          const uint32_t zrow = zs + row0 * 128;
+          const int sw = row0 & 7;                       // block 1 is 16 rows further: same swizzle phase
+#pragma unroll
+          for (int ks = 0; ks < 8; ++ks) {
+            const int chunk = (ks & 3) * 2 + lchunk;
+            const uint32_t addr = zrow + (ks >> 2) * kHalfBytes + ((chunk ^ sw) << 4);
+            uint32_t a[2][4];
+            ldmatrix_x4(addr, a[0][0], a[0][1], a[0][2], a[0][3]);
+            ldmatrix_x4(addr + kTileK * 128, a[1][0], a[1][1], a[1][2], a[1][3]);
+#pragma unroll
+            for (int mb = 0; mb < 2; ++mb) {
+              mma_bf16(acc0[mb], a[mb][0], a[mb][1], a[mb][2], a[mb][3], wf[0][ks][0], wf[0][ks][1]);
+              mma_bf16(acc1[mb], a[mb][0], a[mb][1], a[mb][2], a[mb][3], wf[1][ks][0], wf[1][ks][1]);
+              mma_bf16(accs[mb], a[mb][0], a[mb][1], a[mb][2], a[mb][3], kOnes, kOnes);
+              mma_bf16(gr0[mb], a[mb][0], a[mb][1], a[mb][2], a[mb][3], a[mb][0], a[mb][2]);
+              mma_bf16(gr1[mb], a[mb][0], a[mb][1], a[mb][2], a[mb][3], a[mb][1], a[mb][3]);
+            }
+          }
 #pragma unroll
           for (int mb = 0; mb < 2; ++mb) {
             const int ql = pw * 2 + mb;                  // query inside the stage (0..7)
-            const int row = ql * kTileK + lrow;          // smem row of this lane's ldmatrix address
-            // One m16 block = (query ql) x (16 keys).  Five accumulator chains over the 8 k-steps, all on the
-            // tensor pipe:  a3 = raw z . W' (2 n-blocks);  sum z = z . 1;  sum z^2 = diag(z z^T) (the A fragments
-            // of rows 0-7 / 8-15 are exactly the B fragments of the Gram product).
-            float acc0[4] = {0.f, 0.f, 0.f, 0.f}, acc1[4] = {0.f, 0.f, 0.f, 0.f};
-            float accs[4] = {0.f, 0.f, 0.f, 0.f}, gr0[4] = {0.f, 0.f, 0.f, 0.f}, gr1[4] = {0.f, 0.f, 0.f, 0.f};
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-              const int chunk = (ks & 3) * 2 + lchunk;
-              const uint32_t addr = zs + (ks >> 2) * kHalfBytes + row * 128 + ((chunk ^ (row & 7)) << 4);
-              uint32_t a0, a1, a2, a3;
-              ldmatrix_x4(addr, a0, a1, a2, a3);
-              mma_bf16(acc0, a0, a1, a2, a3, wf[0][ks][0], wf[0][ks][1]);
-              mma_bf16(acc1, a0, a1, a2, a3, wf[1][ks][0], wf[1][ks][1]);
-              mma_bf16(accs, a0, a1, a2, a3, kOnes, kOnes);
-              mma_bf16(gr0, a0, a1, a2, a3, a0, a2);
-              mma_bf16(gr1, a0, a1, a2, a3, a1, a3);
-            }
             // ---- a2: LayerNorm statistics (fp32): mu = sum/c_z, var = sum z^2 / c_z - mu^2
-            const float sq0 = __shfl_sync(0xffffffffu, diag_odd ? gr0[1] : gr0[0], diag_src);
-            const float sq1 = __shfl_sync(0xffffffffu, diag_odd ? gr1[3] : gr1[2], diag_src);
-            const float mu0 = accs[0] * (1.f / kCz), mu1 = accs[2] * (1.f / kCz);
+            const float sq0 = __shfl_sync(0xffffffffu, diag_odd ? gr0[mb][1] : gr0[mb][0], diag_src);
+            const float sq1 = __shfl_sync(0xffffffffu, diag_odd ? gr1[mb][3] : gr1[mb][2], diag_src);
+            const float mu0 = accs[mb][0] * (1.f / kCz), mu1 = accs[mb][2] * (1.f / kCz);
             const float var0 = fmaxf(fmaf(sq0, 1.f / kCz, -mu0 * mu0), 0.f);
             const float var1 = fmaxf(fmaf(sq1, 1.f / kCz, -mu1 * mu1), 0.f);
             const float rstd0 = rsqrtf(var0 + p.eps), rstd1 = rsqrtf(var1 + p.eps);
             // ---- LN(z) W_b = rstd * (z.W' - mu * c1) + c0 ; store to bias[h][query][key]
             const float nm0 = -mu0 * rstd0, nm1 = -mu1 * rstd1;
-            float* brow = bias_buf + (sub * kSubQ + ql) * kTileK;
-            {
-              float* b = brow + (2 * t) * kBiasHeadPitch;
-              b[g] = fmaf(acc0[0], rstd0, fmaf(nm0, c1h[0], c0h[0]));
-              b[g + 8] = fmaf(acc0[2], rstd1, fmaf(nm1, c1h[0], c0h[0]));
-              b += kBiasHeadPitch;
-              b[g] = fmaf(acc0[1], rstd0, fmaf(nm0, c1h[1], c0h[1]));
-              b[g + 8] = fmaf(acc0[3], rstd1, fmaf(nm1, c1h[1], c0h[1]));
-              b = brow + (8 + 2 * t) * kBiasHeadPitch;
-              b[g] = fmaf(acc1[0], rstd0, fmaf(nm0, c1h[2], c0h[2]));
-              b[g + 8] = fmaf(acc1[2], rstd1, fmaf(nm1, c1h[2], c0h[2]));
-              b += kBiasHeadPitch;
-              b[g] = fmaf(acc1[1], rstd0, fmaf(nm0, c1h[3], c0h[3]));
-              b[g + 8] = fmaf(acc1[3], rstd1, fmaf(nm1, c1h[3], c0h[3]));
-            }
+            const uint32_t brow = bias_buf + ((sub * kSubQ + ql) * kTileK + g) * 4;
+            uint32_t b = brow + (2 * t) * (kBiasHeadPitch * 4);
+            sts_f32(b, fmaf(acc0[mb][0], rstd0, fmaf(nm0, c1h[0], c0h[0])));
+            sts_f32(b + 32, fmaf(acc0[mb][2], rstd1, fmaf(nm1, c1h[0], c0h[0])));
+            b += kBiasHeadPitch * 4;
+            sts_f32(b, fmaf(acc0[mb][1], rstd0, fmaf(nm0, c1h[1], c0h[1])));
+            sts_f32(b + 32, fmaf(acc0[mb][3], rstd1, fmaf(nm1, c1h[1], c0h[1])));
+            b = brow + (8 + 2 * t) * (kBiasHeadPitch * 4);
+            sts_f32(b, fmaf(acc1[mb][0], rstd0, fmaf(nm0, c1h[2], c0h[2])));
+            sts_f32(b + 32, fmaf(acc1[mb][2], rstd1, fmaf(nm1, c1h[2], c0h[2])));
+            b += kBiasHeadPitch * 4;
+            sts_f32(b, fmaf(acc1[mb][1], rstd0, fmaf(nm0, c1h[3], c0h[3])));
+            sts_f32(b + 32, fmaf(acc1[mb][3], rstd1, fmaf(nm1, c1h[3], c0h[3])));
           }
           __syncwarp();
           if (lane == 0) mbar_arrive(bar_zempty + 8 * stage);
@@ -309,7 +322,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     }
   } else {
     // =============================================================== attention: QK^T + bias, online softmax, PV
-    reg_inc<200>();
+    reg_inc<192>();
     const int aw = warp - kAttnWarp0;
     constexpr int KK = CP / 16;     // k-steps of QK^T
     constexpr int ND = C / 8;       // n-blocks of PV
@@ -357,7 +370,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
         const int64_t keyA = kAi < p.I ? kAi : p.I - 1;
         const int64_t keyB = kAi + 2 < p.I ? kAi + 2 : p.I - 1;
         mbar_wait(bar_bfull + 8 * bbuf, bphase);
-        const float* bias_buf = s_bias + bbuf * kBiasBufFloats;
+        const uint32_t bias_buf = smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4) + (g * kTileK + 4 * t) * 4;
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
           const int h = 2 * aw + hh;
@@ -371,8 +384,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           for (int nd = 0; nd < ND; ++nd) vf[nd] = ldg_u2(vt + ((int64_t)(h * C + nd * 8 + g)) * p.ldv + j0 + 4 * t);
 #pragma unroll
           for (int mb = 0; mb < 2; ++mb) {
-            const float4 b0 = *reinterpret_cast<const float4*>(bias_buf + h * kBiasHeadPitch + (mb * 16 + g) * kTileK + 4 * t);
-            const float4 b1 = *reinterpret_cast<const float4*>(bias_buf + h * kBiasHeadPitch + (mb * 16 + g + 8) * kTileK + 4 * t);
+            const float4 b0 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + mb * 16 * kTileK) * 4);
+            const float4 b1 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + (mb * 16 + 8) * kTileK) * 4);
             float sA[4] = {b0.x, b0.y, b1.x, b1.y};
             float sB[4] = {b0.z, b0.w, b1.z, b1.w};
 #pragma unroll
