@@ -43,8 +43,13 @@ constexpr int kProjWarp0 = 4, kNumProjWarps = 4, kAttnWarp0 = 8, kNumAttnWarps =
 
 constexpr size_t kSmemZ = 0;
 constexpr size_t kSmemBias = kSmemZ + (size_t)kNZ * kStageBytes;
-constexpr size_t kSmemBar = kSmemBias + 2 * (size_t)kBiasBufFloats * 4;
-constexpr size_t kSmemTotal = kSmemBar + (2 * kNZ + 4) * 8;
+constexpr int kProjN = 32;                               // projection MMA N: 16 heads, the ones row (sum z), zero rows
+constexpr int kWtHalfBytes = kProjN * 128;               // W'' tile: 32 rows x 64 channels bf16 per channel half
+constexpr int kTmemCols = 512;                           // 2 buffers x (32 projection + 128 Gram columns), power of two
+constexpr int kTmemBufCols = 256, kTmemGramCol = 128;
+constexpr size_t kSmemWt = (kSmemBias + 2 * (size_t)kBiasBufFloats * 4 + 1023) / 1024 * 1024;   // 1024-aligned (swizzle)
+constexpr size_t kSmemBar = kSmemWt + 2 * (size_t)kWtHalfBytes;
+constexpr size_t kSmemTotal = kSmemBar + (2 * kNZ + 8) * 8 + 16;
 constexpr size_t kSmemAlloc = kSmemTotal + 1024;        // slack for 1024-byte alignment of the swizzled stages
 
 // ------------------------------------------------------------------ PTX helpers
@@ -61,14 +66,76 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   uint32_t done;
+  uint32_t spins = 0;
   do {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    // watchdog: a pipeline bug must surface as a CUDA error, never as a hung GPU (each failed try_wait already
+    // sleeps for the hardware time limit, so 2^24 failures is seconds)
+    if (!done && ++spins == (1u << 24)) __trap();
   } while (!done);
 }
+// ---- tcgen05 / TMEM (5th-generation tensor cores): single-thread MMA issue, accumulators in tensor memory
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+// K-major operand tile, 128-byte swizzle: rows of 64 bf16 (128 B), 8-row groups 1024 B apart (SBO), descriptor
+// version 1 (sm_100), layout type 2 = SWIZZLE_128B.  `addr` may be advanced by 32 B per K = 16 step inside the atom.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t addr) {
+  return (uint64_t)((addr & 0x3ffffu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) |
+         ((uint64_t)2 << 61);
+}
+// instruction descriptor, kind::f16: D = f32, A = B = bf16, both K-major, M x N
+__host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_x16(uint32_t taddr, float (&v)[16]) {
+  uint32_t r[16];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+                 "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+               : "r"(taddr));
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ float tmem_ld_x1(uint32_t taddr) {
+  uint32_t r;
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(r) : "r"(taddr));
+  return __uint_as_float(r);
+}
+__device__ __forceinline__ void tmem_ld_x32(uint32_t taddr, float (&v)[32]) {
+  uint32_t r[32];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+      "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+#pragma unroll
+  for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tmap, int c0, int c1, int c2, uint32_t bar,
                                             uint64_t policy) {
   asm volatile(
@@ -173,20 +240,40 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
   const uint32_t s_z = smem_u32(smem + kSmemZ);
   float* s_bias = reinterpret_cast<float*>(smem + kSmemBias);
+  const uint32_t s_wt = smem_u32(smem + kSmemWt);
   const uint32_t s_bar = smem_u32(smem + kSmemBar);
   const uint32_t bar_zfull = s_bar, bar_zempty = s_bar + 8 * kNZ, bar_bfull = s_bar + 16 * kNZ,
-                 bar_bempty = s_bar + 16 * kNZ + 16;
+                 bar_bempty = s_bar + 16 * kNZ + 16, bar_tfull = s_bar + 16 * kNZ + 32, bar_tempty = s_bar + 16 * kNZ + 48;
+  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + kSmemBar + (2 * kNZ + 8) * 8);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, kNumProjWarps); }
-    for (int b = 0; b < 2; ++b) { mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps); }
+    // zempty / tfull are arrived on by tcgen05.commit (the MMAs that read the stage / wrote the accumulators are done)
+    for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1); }
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps);
+      mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, kNumProjWarps);
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
+  // W'' = B operand of the projection MMA, K-major, 128-byte swizzled by hand: row n < 16 = head n of
+  // (gamma (.) W_b log2 e)^T, row 16 = ones (its accumulator column is sum_k z), rows 17..31 = 0.
+  for (int e = threadIdx.x; e < kProjN * (kCz / 8); e += kThreads) {
+    const int n = e / (kCz / 8), ch16 = e % (kCz / 8);          // 16-byte chunk = 8 channels
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (n < kH) v = __ldg(reinterpret_cast<const uint4*>(p.wfold) + n * (kCz / 8) + ch16);
+    else if (n == kH) v = make_uint4(0x3f803f80u, 0x3f803f80u, 0x3f803f80u, 0x3f803f80u);
+    const int half = ch16 >> 3, c = ch16 & 7;
+    *reinterpret_cast<uint4*>(smem + kSmemWt + half * kWtHalfBytes + n * 128 + ((c ^ (n & 7)) << 4)) = v;
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to TMA / tcgen05
+  if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), kTmemCols);
+  tc_fence_before();
   __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *s_tmem;
 
   const int n_units = (int)mma_num_units(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
 
@@ -214,39 +301,58 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           }
         }
       }
+    } else if (warp == 1 && lane == 0) {
+      // ============================================================= tcgen05 issuer (one thread)
+      // Per z stage (128 pair rows = 8 queries x 16 keys, K-major, exactly as TMA wrote it) two accumulator chains
+      // over the 8 K = 16 steps:   P[128 x 32]  = z . W''^T   (a3: 16 heads; column 16 = sum_k z)
+      //                            G[128 x 128] = z . z^T     (a2: its diagonal is sum_k z^2)
+      // into TMEM buffer tb; tcgen05.commit then releases the smem stage and publishes the accumulators.
+      constexpr uint32_t idesc_p = umma_idesc_bf16(128, kProjN), idesc_g = umma_idesc_bf16(128, 128);
+      int stage = 0, tb = 0;
+      uint32_t phase = 0, tphase = 0;
+      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const Unit un = decode_unit(p, u);
+        const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
+        const int nsub = (rows + kSubQ - 1) / kSubQ;
+        for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
+          for (int sub = 0; sub < nsub; ++sub) {
+            mbar_wait(bar_tempty + 8 * tb, tphase ^ 1);
+            mbar_wait(bar_zfull + 8 * stage, phase);
+            tc_fence_after();
+            const uint32_t zs = s_z + stage * kStageBytes;
+            const uint32_t d_p = tmem_base + tb * kTmemBufCols, d_g = d_p + kTmemGramCol;
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+              const uint64_t a = umma_desc_sw128(zs + (ks >> 2) * kHalfBytes + (ks & 3) * 32);
+              const uint64_t b = umma_desc_sw128(s_wt + (ks >> 2) * kWtHalfBytes + (ks & 3) * 32);
+              umma_bf16(d_p, a, b, idesc_p, ks > 0);
+            }
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks) {
+              const uint64_t a = umma_desc_sw128(zs + (ks >> 2) * kHalfBytes + (ks & 3) * 32);
+              umma_bf16(d_g, a, a, idesc_g, ks > 0);
+            }
+            umma_commit(bar_zempty + 8 * stage);
+            umma_commit(bar_tfull + 8 * tb);
+            if (++stage == kNZ) { stage = 0; phase ^= 1; }
+            tb ^= 1;
+            if (tb == 0) tphase ^= 1;
+          }
+        }
+      }
     }
   } else if (warp < kAttnWarp0) {
-    // =============================================================== bias projection + LayerNorm statistics
+    // =============================================================== LayerNorm statistics + bias epilogue (TMEM -> smem)
+    // Thread = one pair row of the stage: TMEM lane 32*pw + lane = (query 2pw + lane/16 of the stage, key lane%16).
     reg_dec<104>();
-    const int pw = warp - kProjWarp0;
-    // the 4 heads this thread finalises: 2t, 2t+1 (n-block 0) and 8+2t, 8+2t+1 (n-block 1)
-    float c1h[4], c0h[4];
+    const int pw = warp - kProjWarp0;                       // == warp % 4: the TMEM lane quadrant this warp may read
+    float c1h[kH], c0h[kH];
 #pragma unroll
-    for (int x = 0; x < 4; ++x) {
-      const int h = (x >> 1) * 8 + 2 * t + (x & 1);
-      c1h[x] = p.c1[h];
-      c0h[x] = p.c0[h];
-    }
-    // B fragments of W'^T (heads 8*nb + g, channels 16*ks + 2t.. and + 8) stay in registers for the whole kernel
-    uint32_t wf[2][8][2];
-    {
-      const uint32_t* wsrc = reinterpret_cast<const uint32_t*>(p.wfold);
-#pragma unroll
-      for (int nb = 0; nb < 2; ++nb)
-#pragma unroll
-        for (int ks = 0; ks < 8; ++ks) {
-          wf[nb][ks][0] = __ldg(wsrc + (nb * 8 + g) * (kCz / 2) + ks * 8 + t);
-          wf[nb][ks][1] = __ldg(wsrc + (nb * 8 + g) * (kCz / 2) + ks * 8 + t + 4);
-        }
-    }
-    constexpr uint32_t kOnes = 0x3f803f80u;   // bf16x2 (1, 1)
-    // ldmatrix source row of this lane inside an m16 block, and its swizzle phase
-    const int lrow = (lane & 7) + ((lane >> 3) & 1) * 8;
-    const int lchunk = lane >> 4;
-    const int diag_src = (lane & ~3) | (g >> 1);   // lane of this quad that holds the Gram diagonal of rows g, g+8
-    const bool diag_odd = (g & 1) != 0;
-    int stage = 0, bbuf = 0;
-    uint32_t phase = 0, bphase = 0;
+    for (int h = 0; h < kH; ++h) { c1h[h] = __ldg(p.c1 + h); c0h[h] = __ldg(p.c0 + h); }
+    const uint32_t t_lane = tmem_base + ((uint32_t)(pw * 32) << 16);
+    const int prow = pw * 32 + lane;                        // pair row inside the stage
+    int tb = 0, bbuf = 0;
+    uint32_t tphase = 0, bphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
       const Unit un = decode_unit(p, u);
       const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
@@ -255,64 +361,39 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
         mbar_wait(bar_bempty + 8 * bbuf, bphase ^ 1);
         const uint32_t bias_buf = smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4);
         for (int sub = 0; sub < nsub; ++sub) {
-          mbar_wait(bar_zfull + 8 * stage, phase);
-          const uint32_t zs = s_z + stage * kStageBytes;
-          // Two m16 blocks at once (queries 2pw, 2pw+1 of the stage) x (16 keys): ten independent accumulator
-          // chains over the 8 k-steps, all on the tensor pipe:  a3 = raw z . W' (2 n-blocks);  sum z = z . 1;
-          // sum z^2 = diag(z z^T) (the A fragments of rows 0-7 / 8-15 are exactly the B fragments of the Gram product).
-          float acc0[2][4], acc1[2][4], accs[2][4], gr0[2][4], gr1[2][4];
-#pragma unroll
-          for (int mb = 0; mb < 2; ++mb)
-#pragma unroll
-            for (int x = 0; x < 4; ++x) acc0[mb][x] = acc1[mb][x] = accs[mb][x] = gr0[mb][x] = gr1[mb][x] = 0.f;
-          const int row0 = (pw * 2) * kTileK + lrow;     // smem row of this lane's ldmatrix address (block 0)
-          const uint32_t zrow = zs + row0 * 128;
-          const int sw = row0 & 7;                       // block 1 is 16 rows further: same swizzle phase
-#pragma unroll
-          for (int ks = 0; ks < 8; ++ks) {
-            const int chunk = (ks & 3) * 2 + lchunk;
-            const uint32_t addr = zrow + (ks >> 2) * kHalfBytes + ((chunk ^ sw) << 4);
-            uint32_t a[2][4];
-            ldmatrix_x4(addr, a[0][0], a[0][1], a[0][2], a[0][3]);
-            ldmatrix_x4(addr + kTileK * 128, a[1][0], a[1][1], a[1][2], a[1][3]);
-#pragma unroll
-            for (int mb = 0; mb < 2; ++mb) {
-              mma_bf16(acc0[mb], a[mb][0], a[mb][1], a[mb][2], a[mb][3], wf[0][ks][0], wf[0][ks][1]);
-              mma_bf16(acc1[mb], a[mb][0], a[mb][1], a[mb][2], a[mb][3], wf[1][ks][0], wf[1][ks][1]);
-              mma_bf16(accs[mb], a[mb][0], a[mb][1], a[mb][2], a[mb][3], kOnes, kOnes);
-              mma_bf16(gr0[mb], a[mb][0], a[mb][1], a[mb][2], a[mb][3], a[mb][0], a[mb][2]);
-              mma_bf16(gr1[mb], a[mb][0], a[mb][1], a[mb][2], a[mb][3], a[mb][1], a[mb][3]);
-            }
-          }
-#pragma unroll
-          for (int mb = 0; mb < 2; ++mb) {
-            const int ql = pw * 2 + mb;                  // query inside the stage (0..7)
-            // ---- a2: LayerNorm statistics (fp32): mu = sum/c_z, var = sum z^2 / c_z - mu^2
-            const float sq0 = __shfl_sync(0xffffffffu, diag_odd ? gr0[mb][1] : gr0[mb][0], diag_src);
-            const float sq1 = __shfl_sync(0xffffffffu, diag_odd ? gr1[mb][3] : gr1[mb][2], diag_src);
-            const float mu0 = accs[mb][0] * (1.f / kCz), mu1 = accs[mb][2] * (1.f / kCz);
-            const float var0 = fmaxf(fmaf(sq0, 1.f / kCz, -mu0 * mu0), 0.f);
-            const float var1 = fmaxf(fmaf(sq1, 1.f / kCz, -mu1 * mu1), 0.f);
-            const float rstd0 = rsqrtf(var0 + p.eps), rstd1 = rsqrtf(var1 + p.eps);
-            // ---- LN(z) W_b = rstd * (z.W' - mu * c1) + c0 ; store to bias[h][query][key]
-            const float nm0 = -mu0 * rstd0, nm1 = -mu1 * rstd1;
-            const uint32_t brow = bias_buf + ((sub * kSubQ + ql) * kTileK + g) * 4;
-            uint32_t b = brow + (2 * t) * (kBiasHeadPitch * 4);
-            sts_f32(b, fmaf(acc0[mb][0], rstd0, fmaf(nm0, c1h[0], c0h[0])));
-            sts_f32(b + 32, fmaf(acc0[mb][2], rstd1, fmaf(nm1, c1h[0], c0h[0])));
-            b += kBiasHeadPitch * 4;
-            sts_f32(b, fmaf(acc0[mb][1], rstd0, fmaf(nm0, c1h[1], c0h[1])));
-            sts_f32(b + 32, fmaf(acc0[mb][3], rstd1, fmaf(nm1, c1h[1], c0h[1])));
-            b = brow + (8 + 2 * t) * (kBiasHeadPitch * 4);
-            sts_f32(b, fmaf(acc1[mb][0], rstd0, fmaf(nm0, c1h[2], c0h[2])));
-            sts_f32(b + 32, fmaf(acc1[mb][2], rstd1, fmaf(nm1, c1h[2], c0h[2])));
-            b += kBiasHeadPitch * 4;
-            sts_f32(b, fmaf(acc1[mb][1], rstd0, fmaf(nm0, c1h[3], c0h[3])));
-            sts_f32(b + 32, fmaf(acc1[mb][3], rstd1, fmaf(nm1, c1h[3], c0h[3])));
-          }
+          mbar_wait(bar_tfull + 8 * tb, tphase);
+          tc_fence_after();
+          const uint32_t t_p = t_lane + tb * kTmemBufCols;
+          float acc[16], gr[32];
+          tmem_ld_x16(t_p, acc);                              // z . W' for the 16 heads
+          const float zsum = tmem_ld_x1(t_p + kH);            // sum_k z
+          tmem_ld_x32(t_p + kTmemGramCol + pw * 32, gr);      // Gram columns 32pw..32pw+31 of this row
+          tmem_ld_wait();
+          tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(bar_zempty + 8 * stage);
-          if (++stage == kNZ) { stage = 0; phase ^= 1; }
+          if (lane == 0) mbar_arrive(bar_tempty + 8 * tb);    // accumulators are in registers: buffer free
+          tb ^= 1;
+          if (tb == 0) tphase ^= 1;
+          // diagonal element: register index == lane (select tree, no local-memory indexing)
+#pragma unroll
+          for (int i = 0; i < 16; ++i) gr[i] = (lane & 16) ? gr[i + 16] : gr[i];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) gr[i] = (lane & 8) ? gr[i + 8] : gr[i];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) gr[i] = (lane & 4) ? gr[i + 4] : gr[i];
+#pragma unroll
+          for (int i = 0; i < 2; ++i) gr[i] = (lane & 2) ? gr[i + 2] : gr[i];
+          const float zsq = (lane & 1) ? gr[1] : gr[0];       // sum_k z^2
+          // ---- a2: LayerNorm statistics (fp32): mu = sum/c_z, var = sum z^2 / c_z - mu^2
+          const float mu = zsum * (1.f / kCz);
+          const float var = fmaxf(fmaf(zsq, 1.f / kCz, -mu * mu), 0.f);
+          const float rstd = rsqrtf(var + p.eps);
+          const float nm = -mu * rstd;
+          // ---- LN(z) W_b = rstd * (z.W' - mu * c1) + c0 ; store to bias[h][query][key] (32 lanes = 128 contiguous bytes)
+          const uint32_t brow = bias_buf + ((sub * kSubQ) * kTileK + prow) * 4;
+#pragma unroll
+          for (int h = 0; h < kH; ++h)
+            sts_f32(brow + h * (kBiasHeadPitch * 4), fmaf(acc[h], rstd, fmaf(nm, c1h[h], c0h[h])));
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_bfull + 8 * bbuf);
@@ -454,6 +535,13 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             }
           }
     }
+  }
+  // teardown: every role is done with tensor memory before the allocating warp frees it
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    __syncwarp();
+    tmem_dealloc(tmem_base, kTmemCols);
   }
 }
 
