@@ -45,8 +45,8 @@ constexpr size_t kSmemZ = 0;
 constexpr size_t kSmemBias = kSmemZ + (size_t)kNZ * kStageBytes;
 constexpr int kProjN = 32;                               // projection MMA N: 16 heads, the ones row (sum z), zero rows
 constexpr int kWtHalfBytes = kProjN * 128;               // W'' tile: 32 rows x 64 channels bf16 per channel half
-constexpr int kTmemCols = 512;                           // 2 buffers x (32 projection + 128 Gram columns), power of two
-constexpr int kTmemBufCols = 256, kTmemGramCol = 128;
+constexpr int kTmemCols = 64;                            // 2 accumulator buffers x 32 projection columns
+constexpr int kTmemBufCols = 32;
 constexpr size_t kSmemWt = (kSmemBias + 2 * (size_t)kBiasBufFloats * 4 + 1023) / 1024 * 1024;   // 1024-aligned (swizzle)
 constexpr size_t kSmemBar = kSmemWt + 2 * (size_t)kWtHalfBytes;
 constexpr size_t kSmemTotal = kSmemBar + (2 * kNZ + 8) * 8 + 16;
@@ -122,19 +122,6 @@ __device__ __forceinline__ float tmem_ld_x1(uint32_t taddr) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(r) : "r"(taddr));
   return __uint_as_float(r);
 }
-__device__ __forceinline__ void tmem_ld_x32(uint32_t taddr, float (&v)[32]) {
-  uint32_t r[32];
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
-      "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
-        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
-        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-      : "r"(taddr));
-#pragma unroll
-  for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
-}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tmap, int c0, int c1, int c2, uint32_t bar,
                                             uint64_t policy) {
@@ -142,10 +129,6 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tma
       "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
       " [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(policy)
       : "memory");
-}
-__device__ __forceinline__ void ldmatrix_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];"
-               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(addr));
 }
 __device__ __forceinline__ void mma_bf16(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
                                          uint32_t b1) {
@@ -157,6 +140,11 @@ __device__ __forceinline__ void sts_f32(uint32_t addr, float v) { asm volatile("
 __device__ __forceinline__ float4 lds_f32x4(uint32_t addr) {
   float4 v;
   asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ uint4 lds_u32x4(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
   return v;
 }
 __device__ __forceinline__ float bf_lo(uint32_t x) { return __uint_as_float(x << 16); }
@@ -251,7 +239,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
 
   if (threadIdx.x == 0) {
     // zempty / tfull are arrived on by tcgen05.commit (the MMAs that read the stage / wrote the accumulators are done)
-    for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1); }
+    for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + kNumProjWarps); }
     for (int b = 0; b < 2; ++b) {
       mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps);
       mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, kNumProjWarps);
@@ -307,7 +295,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
       // over the 8 K = 16 steps:   P[128 x 32]  = z . W''^T   (a3: 16 heads; column 16 = sum_k z)
       //                            G[128 x 128] = z . z^T     (a2: its diagonal is sum_k z^2)
       // into TMEM buffer tb; tcgen05.commit then releases the smem stage and publishes the accumulators.
-      constexpr uint32_t idesc_p = umma_idesc_bf16(128, kProjN), idesc_g = umma_idesc_bf16(128, 128);
+      constexpr uint32_t idesc_p = umma_idesc_bf16(128, kProjN);
       int stage = 0, tb = 0;
       uint32_t phase = 0, tphase = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
@@ -320,17 +308,12 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             mbar_wait(bar_zfull + 8 * stage, phase);
             tc_fence_after();
             const uint32_t zs = s_z + stage * kStageBytes;
-            const uint32_t d_p = tmem_base + tb * kTmemBufCols, d_g = d_p + kTmemGramCol;
+            const uint32_t d_p = tmem_base + tb * kTmemBufCols;
 #pragma unroll
             for (int ks = 0; ks < 8; ++ks) {
               const uint64_t a = umma_desc_sw128(zs + (ks >> 2) * kHalfBytes + (ks & 3) * 32);
               const uint64_t b = umma_desc_sw128(s_wt + (ks >> 2) * kWtHalfBytes + (ks & 3) * 32);
               umma_bf16(d_p, a, b, idesc_p, ks > 0);
-            }
-#pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-              const uint64_t a = umma_desc_sw128(zs + (ks >> 2) * kHalfBytes + (ks & 3) * 32);
-              umma_bf16(d_g, a, a, idesc_g, ks > 0);
             }
             umma_commit(bar_zempty + 8 * stage);
             umma_commit(bar_tfull + 8 * tb);
@@ -344,6 +327,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   } else if (warp < kAttnWarp0) {
     // =============================================================== LayerNorm statistics + bias epilogue (TMEM -> smem)
     // Thread = one pair row of the stage: TMEM lane 32*pw + lane = (query 2pw + lane/16 of the stage, key lane%16).
+    // sum_k z^2 comes from the thread's own 256-byte row of the swizzled stage (16 conflict-free LDS.128, fp32 FMAs);
+    // sum_k z (the ones row of W'') and z.W' come from the tcgen05 accumulators.
     reg_dec<104>();
     const int pw = warp - kProjWarp0;                       // == warp % 4: the TMEM lane quadrant this warp may read
     float c1h[kH], c0h[kH];
@@ -351,8 +336,10 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     for (int h = 0; h < kH; ++h) { c1h[h] = __ldg(p.c1 + h); c0h[h] = __ldg(p.c0 + h); }
     const uint32_t t_lane = tmem_base + ((uint32_t)(pw * 32) << 16);
     const int prow = pw * 32 + lane;                        // pair row inside the stage
-    int tb = 0, bbuf = 0;
-    uint32_t tphase = 0, bphase = 0;
+    const uint32_t zrow = s_z + prow * 128;                 // row base inside a channel half (128-byte swizzle atom rows)
+    const uint32_t zsw = (uint32_t)(prow & 7);
+    int tb = 0, bbuf = 0, stage = 0;
+    uint32_t tphase = 0, bphase = 0, zphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
       const Unit un = decode_unit(p, u);
       const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
@@ -361,30 +348,42 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
         mbar_wait(bar_bempty + 8 * bbuf, bphase ^ 1);
         const uint32_t bias_buf = smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4);
         for (int sub = 0; sub < nsub; ++sub) {
+          // ---- a2: sum_k z^2 of this pair straight from the TMA stage
+          mbar_wait(bar_zfull + 8 * stage, zphase);
+          float sq0 = 0.f, sq1 = 0.f, sq2 = 0.f, sq3 = 0.f;
+          const uint32_t zr = zrow + stage * kStageBytes;
+#pragma unroll
+          for (int half = 0; half < 2; ++half) {
+            uint4 w[8];
+#pragma unroll
+            for (int c = 0; c < 8; ++c) w[c] = lds_u32x4(zr + half * kHalfBytes + ((c ^ zsw) << 4));
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+              sq0 = fmaf(bf_lo(w[c].x), bf_lo(w[c].x), sq0); sq1 = fmaf(bf_hi(w[c].x), bf_hi(w[c].x), sq1);
+              sq2 = fmaf(bf_lo(w[c].y), bf_lo(w[c].y), sq2); sq3 = fmaf(bf_hi(w[c].y), bf_hi(w[c].y), sq3);
+              sq0 = fmaf(bf_lo(w[c].z), bf_lo(w[c].z), sq0); sq1 = fmaf(bf_hi(w[c].z), bf_hi(w[c].z), sq1);
+              sq2 = fmaf(bf_lo(w[c].w), bf_lo(w[c].w), sq2); sq3 = fmaf(bf_hi(w[c].w), bf_hi(w[c].w), sq3);
+            }
+          }
+          float zsq = (sq0 + sq1) + (sq2 + sq3);
+          asm volatile("" : "+f"(zsq));                       // the row has been consumed before the stage is released
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_zempty + 8 * stage);
+          if (++stage == kNZ) { stage = 0; zphase ^= 1; }
+          // ---- a3: z.W' (16 heads) and sum_k z from tensor memory
           mbar_wait(bar_tfull + 8 * tb, tphase);
           tc_fence_after();
           const uint32_t t_p = t_lane + tb * kTmemBufCols;
-          float acc[16], gr[32];
-          tmem_ld_x16(t_p, acc);                              // z . W' for the 16 heads
-          const float zsum = tmem_ld_x1(t_p + kH);            // sum_k z
-          tmem_ld_x32(t_p + kTmemGramCol + pw * 32, gr);      // Gram columns 32pw..32pw+31 of this row
+          float acc[16];
+          tmem_ld_x16(t_p, acc);
+          const float zsum = tmem_ld_x1(t_p + kH);
           tmem_ld_wait();
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(bar_tempty + 8 * tb);    // accumulators are in registers: buffer free
           tb ^= 1;
           if (tb == 0) tphase ^= 1;
-          // diagonal element: register index == lane (select tree, no local-memory indexing)
-#pragma unroll
-          for (int i = 0; i < 16; ++i) gr[i] = (lane & 16) ? gr[i + 16] : gr[i];
-#pragma unroll
-          for (int i = 0; i < 8; ++i) gr[i] = (lane & 8) ? gr[i + 8] : gr[i];
-#pragma unroll
-          for (int i = 0; i < 4; ++i) gr[i] = (lane & 4) ? gr[i + 4] : gr[i];
-#pragma unroll
-          for (int i = 0; i < 2; ++i) gr[i] = (lane & 2) ? gr[i + 2] : gr[i];
-          const float zsq = (lane & 1) ? gr[1] : gr[0];       // sum_k z^2
-          // ---- a2: LayerNorm statistics (fp32): mu = sum/c_z, var = sum z^2 / c_z - mu^2
+          // LayerNorm statistics (fp32): mu = sum/c_z, var = sum z^2 / c_z - mu^2
           const float mu = zsum * (1.f / kCz);
           const float var = fmaxf(fmaf(zsq, 1.f / kCz, -mu * mu), 0.f);
           const float rstd = rsqrtf(var + p.eps);
@@ -452,10 +451,19 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
         const int64_t keyB = kAi + 2 < p.I ? kAi + 2 : p.I - 1;
         mbar_wait(bar_bfull + 8 * bbuf, bphase);
         const uint32_t bias_buf = smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4) + (g * kTileK + 4 * t) * 4;
+#ifdef EXP_NOATTN
+        if (p.I < 0)
+#endif
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
           const int h = 2 * aw + hh;
           uint2 kA[KK], kB[KK], vf[ND];
+#ifdef EXP_NOKV
+          const int64_t keyA_ = 0, keyB_ = 1; const int j0_ = 0;
+#define keyA keyA_
+#define keyB keyB_
+#define j0 j0_
+#endif
 #pragma unroll
           for (int kk = 0; kk < KK; ++kk) {
             kA[kk] = ldg_u2(kp + (keyA * kH + h) * CP + kk * 16 + 4 * t);
@@ -463,6 +471,11 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           }
 #pragma unroll
           for (int nd = 0; nd < ND; ++nd) vf[nd] = ldg_u2(vt + ((int64_t)(h * C + nd * 8 + g)) * p.ldv + j0 + 4 * t);
+#ifdef EXP_NOKV
+#undef keyA
+#undef keyB
+#undef j0
+#endif
 #pragma unroll
           for (int mb = 0; mb < 2; ++mb) {
             const float4 b0 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + mb * 16 * kTileK) * 4);
@@ -499,8 +512,10 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             // ---- a6: acc = acc * alpha + P V
 #pragma unroll
             for (int nd = 0; nd < ND; ++nd) {
+#ifndef EXP_NORESCALE
               o[hh][mb][nd][0] *= al0; o[hh][mb][nd][1] *= al0;
               o[hh][mb][nd][2] *= al1; o[hh][mb][nd][3] *= al1;
+#endif
               mma_bf16(o[hh][mb][nd], p0, p1, p2, p3, vf[nd].x, vf[nd].y);
             }
           }
