@@ -33,7 +33,7 @@ constexpr int kH = 16;
 constexpr int kTileQ = 32;          // queries per work unit
 constexpr int kTileK = 16;          // keys per attention tile
 constexpr int kSubQ = 8;            // queries per z stage
-constexpr int kNZ = 4;              // z stages
+constexpr int kNZ = 3;              // z stages
 constexpr int kStageBytes = kSubQ * kTileK * kCz * 2;   // 32 KB
 constexpr int kHalfBytes = kStageBytes / 2;
 constexpr int kBiasHeadPitch = kTileQ * kTileK + 4;     // floats; +4: conflict-free projection stores
@@ -49,8 +49,9 @@ constexpr int kTmemCols = 64;                            // 2 accumulator buffer
 constexpr int kTmemBufCols = 32;
 constexpr size_t kSmemWt = (kSmemBias + 2 * (size_t)kBiasBufFloats * 4 + 1023) / 1024 * 1024;   // 1024-aligned (swizzle)
 constexpr size_t kSmemBar = kSmemWt + 2 * (size_t)kWtHalfBytes;
-constexpr size_t kSmemTotal = kSmemBar + (2 * kNZ + 8) * 8 + 16;
-constexpr size_t kSmemAlloc = kSmemTotal + 1024;        // slack for 1024-byte alignment of the swizzled stages
+constexpr size_t kSmemQ = (kSmemBar + (2 * kNZ + 8) * 8 + 16 + 15) / 16 * 16;   // Q tile [32 rows][H][CP] bf16, padded rows
+__host__ __device__ constexpr int q_pitch(int CP) { return kH * CP * 2 + 32; }      // bytes; +32: conflict-free 64-bit loads
+__host__ __device__ constexpr size_t smem_alloc(int CP) { return kSmemQ + (size_t)kTileQ * q_pitch(CP) + 1024; }  // + alignment slack
 
 // ------------------------------------------------------------------ PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -147,8 +148,20 @@ __device__ __forceinline__ uint4 lds_u32x4(uint32_t addr) {
   asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
   return v;
 }
-__device__ __forceinline__ float bf_lo(uint32_t x) { return __uint_as_float(x << 16); }
-__device__ __forceinline__ float bf_hi(uint32_t x) { return __uint_as_float(x & 0xffff0000u); }
+__device__ __forceinline__ uint2 lds_u32x2(uint32_t addr) {
+  uint2 v;
+  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+  return v;
+}
+// acc_lo += lo(w)^2, acc_hi += hi(w)^2 for a bf16x2 word: mixed-precision FMA (bf16 x bf16 + f32, PTX ISA 8.6, sm_100:
+// SASS FHFMA.BF16 with .H0/.H1 operand selectors), exact products, fp32 accumulation, no unpacking instructions
+__device__ __forceinline__ void fma_sq_bf16x2(float& acc_lo, float& acc_hi, uint32_t w) {
+  asm("{\n\t.reg .b16 l, h;\n\t"
+      "mov.b32 {l, h}, %2;\n\t"
+      "fma.rn.f32.bf16 %0, l, l, %0;\n\t"
+      "fma.rn.f32.bf16 %1, h, h, %1;\n\t}"
+      : "+f"(acc_lo), "+f"(acc_hi) : "r"(w));
+}
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
   uint32_t r;
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
@@ -230,6 +243,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   float* s_bias = reinterpret_cast<float*>(smem + kSmemBias);
   const uint32_t s_wt = smem_u32(smem + kSmemWt);
   const uint32_t s_bar = smem_u32(smem + kSmemBar);
+  const uint32_t s_q = smem_u32(smem + kSmemQ);
   const uint32_t bar_zfull = s_bar, bar_zempty = s_bar + 8 * kNZ, bar_bfull = s_bar + 16 * kNZ,
                  bar_bempty = s_bar + 16 * kNZ + 16, bar_tfull = s_bar + 16 * kNZ + 32, bar_tempty = s_bar + 16 * kNZ + 48;
   volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + kSmemBar + (2 * kNZ + 8) * 8);
@@ -359,10 +373,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             for (int c = 0; c < 8; ++c) w[c] = lds_u32x4(zr + half * kHalfBytes + ((c ^ zsw) << 4));
 #pragma unroll
             for (int c = 0; c < 8; ++c) {
-              sq0 = fmaf(bf_lo(w[c].x), bf_lo(w[c].x), sq0); sq1 = fmaf(bf_hi(w[c].x), bf_hi(w[c].x), sq1);
-              sq2 = fmaf(bf_lo(w[c].y), bf_lo(w[c].y), sq2); sq3 = fmaf(bf_hi(w[c].y), bf_hi(w[c].y), sq3);
-              sq0 = fmaf(bf_lo(w[c].z), bf_lo(w[c].z), sq0); sq1 = fmaf(bf_hi(w[c].z), bf_hi(w[c].z), sq1);
-              sq2 = fmaf(bf_lo(w[c].w), bf_lo(w[c].w), sq2); sq3 = fmaf(bf_hi(w[c].w), bf_hi(w[c].w), sq3);
+              fma_sq_bf16x2(sq0, sq1, w[c].x); fma_sq_bf16x2(sq2, sq3, w[c].y);
+              fma_sq_bf16x2(sq0, sq1, w[c].z); fma_sq_bf16x2(sq2, sq3, w[c].w);
             }
           }
           float zsq = (sq0 + sq1) + (sq2 + sq3);
@@ -413,22 +425,20 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     uint32_t bphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
       const Unit un = decode_unit(p, u);
-      // Q fragments: [head][m-block][k-step] -> (a0,a2) of row g and (a1,a3) of row g+8
-      uint2 qa[2][2][KK], qb[2][2][KK];
-#pragma unroll
-      for (int hh = 0; hh < 2; ++hh)
-#pragma unroll
-        for (int mb = 0; mb < 2; ++mb) {
-          int r0i = un.q0 + mb * 16 + g, r1i = r0i + 8;
-          const int64_t r0 = r0i < p.I ? r0i : p.I - 1;
-          const int64_t r1 = r1i < p.I ? r1i : p.I - 1;
-          const int h = 2 * aw + hh;
-#pragma unroll
-          for (int kk = 0; kk < KK; ++kk) {
-            qa[hh][mb][kk] = ldg_u2(qp + (r0 * kH + h) * CP + kk * 16 + 4 * t);
-            qb[hh][mb][kk] = ldg_u2(qp + (r1 * kH + h) * CP + kk * 16 + 4 * t);
-          }
-        }
+      // Q tile -> shared memory (rows of the tile, all heads), shared by the 8 attention warps; row pitch padded so the
+      // per-thread 64-bit fragment loads are conflict-free.  Named barrier 1 = the 256 attention threads.
+      constexpr int kQP = q_pitch(CP);
+      constexpr int kQRowChunks = kH * CP * 2 / 16;
+      asm volatile("bar.sync 1, 256;" ::: "memory");          // every warp is done with the previous unit's Q
+      for (int e = threadIdx.x - kAttnWarp0 * 32; e < kTileQ * kQRowChunks; e += kNumAttnWarps * 32) {
+        const int r = e / kQRowChunks, ch = e - r * kQRowChunks;
+        const int64_t row = (un.q0 + r) < p.I ? (un.q0 + r) : p.I - 1;
+        const uint4 v = __ldg(reinterpret_cast<const uint4*>(qp + row * (kH * CP)) + ch);
+        *reinterpret_cast<uint4*>(smem + kSmemQ + r * kQP + ch * 16) = v;
+      }
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      // fragment address of (row g, head 2aw, k-step 0): + mb*16*kQP (+8 rows: +8*kQP), + hh*CP*2, + kk*32
+      const uint32_t q_frag = s_q + g * kQP + (2 * aw) * (CP * 2) + 8 * t;
       float o[2][2][ND][4];
       float m_run[2][2][2], l_run[2][2][2];
 #pragma unroll
@@ -443,82 +453,104 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             for (int x = 0; x < 4; ++x) o[hh][mb][nd][x] = 0.f;
         }
 
-      for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
-        const bool partial = (j0 < un.ks) || (j0 + kTileK > un.ke);
-        // key of S column: n-block A col c <-> j0 + 4*(c/2) + c%2, n-block B col c <-> that + 2
-        const int kAi = j0 + 4 * (g >> 1) + (g & 1);
+      // K / V^T fragments of (key tile j, head h) are read from L2 into the registers the previous block just released:
+      // K right after the last QK^T MMA that used it, V^T right after the last PV MMA (software pipelining, no extra
+      // registers).  key of S column: n-block A col c <-> j + 4*(c/2) + c%2, n-block B col c <-> that + 2
+      uint2 kA[KK], kB[KK], vf[ND];
+      auto load_k = [&](int j, int h) {
+        const int kAi = j + 4 * (g >> 1) + (g & 1);
         const int64_t keyA = kAi < p.I ? kAi : p.I - 1;
         const int64_t keyB = kAi + 2 < p.I ? kAi + 2 : p.I - 1;
+#pragma unroll
+        for (int kk = 0; kk < KK; ++kk) {
+          kA[kk] = ldg_u2(kp + (keyA * kH + h) * CP + kk * 16 + 4 * t);
+          kB[kk] = ldg_u2(kp + (keyB * kH + h) * CP + kk * 16 + 4 * t);
+        }
+      };
+      auto load_v = [&](int j, int h) {
+#pragma unroll
+        for (int nd = 0; nd < ND; ++nd) vf[nd] = ldg_u2(vt + ((int64_t)(h * C + nd * 8 + g)) * p.ldv + j + 4 * t);
+      };
+      load_k(un.ks & ~(kTileK - 1), 2 * aw);
+      load_v(un.ks & ~(kTileK - 1), 2 * aw);
+
+      for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
+        const bool partial = (j0 < un.ks) || (j0 + kTileK > un.ke);
+        const int jn = j0 + kTileK < un.ke ? j0 + kTileK : j0;     // next tile (the last one re-reads itself: harmless)
         mbar_wait(bar_bfull + 8 * bbuf, bphase);
         const uint32_t bias_buf = smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4) + (g * kTileK + 4 * t) * 4;
-#ifdef EXP_NOATTN
-        if (p.I < 0)
-#endif
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
           const int h = 2 * aw + hh;
-          uint2 kA[KK], kB[KK], vf[ND];
-#ifdef EXP_NOKV
-          const int64_t keyA_ = 0, keyB_ = 1; const int j0_ = 0;
-#define keyA keyA_
-#define keyB keyB_
-#define j0 j0_
-#endif
-#pragma unroll
-          for (int kk = 0; kk < KK; ++kk) {
-            kA[kk] = ldg_u2(kp + (keyA * kH + h) * CP + kk * 16 + 4 * t);
-            kB[kk] = ldg_u2(kp + (keyB * kH + h) * CP + kk * 16 + 4 * t);
-          }
-#pragma unroll
-          for (int nd = 0; nd < ND; ++nd) vf[nd] = ldg_u2(vt + ((int64_t)(h * C + nd * 8 + g)) * p.ldv + j0 + 4 * t);
-#ifdef EXP_NOKV
-#undef keyA
-#undef keyB
-#undef j0
-#endif
+          // ---- a4: S = bias + Q K^T for both 16-row blocks (four independent accumulator chains)
+          float sA[2][4], sB[2][4];
 #pragma unroll
           for (int mb = 0; mb < 2; ++mb) {
             const float4 b0 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + mb * 16 * kTileK) * 4);
             const float4 b1 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + (mb * 16 + 8) * kTileK) * 4);
-            float sA[4] = {b0.x, b0.y, b1.x, b1.y};
-            float sB[4] = {b0.z, b0.w, b1.z, b1.w};
+            sA[mb][0] = b0.x; sA[mb][1] = b0.y; sA[mb][2] = b1.x; sA[mb][3] = b1.y;
+            sB[mb][0] = b0.z; sB[mb][1] = b0.w; sB[mb][2] = b1.z; sB[mb][3] = b1.w;
+          }
 #pragma unroll
-            for (int kk = 0; kk < KK; ++kk) {
-              mma_bf16(sA, qa[hh][mb][kk].x, qb[hh][mb][kk].x, qa[hh][mb][kk].y, qb[hh][mb][kk].y, kA[kk].x, kA[kk].y);
-              mma_bf16(sB, qa[hh][mb][kk].x, qb[hh][mb][kk].x, qa[hh][mb][kk].y, qb[hh][mb][kk].y, kB[kk].x, kB[kk].y);
+          for (int kk = 0; kk < KK; ++kk)
+#pragma unroll
+            for (int mb = 0; mb < 2; ++mb) {
+              const uint2 qa = lds_u32x2(q_frag + (mb * 16) * kQP + hh * (CP * 2) + kk * 32);
+              const uint2 qb = lds_u32x2(q_frag + (mb * 16 + 8) * kQP + hh * (CP * 2) + kk * 32);
+              mma_bf16(sA[mb], qa.x, qb.x, qa.y, qb.y, kA[kk].x, kA[kk].y);
+              mma_bf16(sB[mb], qa.x, qb.x, qa.y, qb.y, kB[kk].x, kB[kk].y);
             }
+          if (hh == 0) load_k(j0, h + 1); else load_k(jn, h - 1);
+          uint32_t pf[2][4];
+#pragma unroll
+          for (int mb = 0; mb < 2; ++mb) {
             if (partial) {
               const int k0 = j0 + 4 * t;
-              if (k0 < un.ks || k0 >= un.ke) { sA[0] = -INFINITY; sA[2] = -INFINITY; }
-              if (k0 + 1 < un.ks || k0 + 1 >= un.ke) { sA[1] = -INFINITY; sA[3] = -INFINITY; }
-              if (k0 + 2 < un.ks || k0 + 2 >= un.ke) { sB[0] = -INFINITY; sB[2] = -INFINITY; }
-              if (k0 + 3 < un.ks || k0 + 3 >= un.ke) { sB[1] = -INFINITY; sB[3] = -INFINITY; }
+              if (k0 < un.ks || k0 >= un.ke) { sA[mb][0] = -INFINITY; sA[mb][2] = -INFINITY; }
+              if (k0 + 1 < un.ks || k0 + 1 >= un.ke) { sA[mb][1] = -INFINITY; sA[mb][3] = -INFINITY; }
+              if (k0 + 2 < un.ks || k0 + 2 >= un.ke) { sB[mb][0] = -INFINITY; sB[mb][2] = -INFINITY; }
+              if (k0 + 3 < un.ks || k0 + 3 >= un.ke) { sB[mb][1] = -INFINITY; sB[mb][3] = -INFINITY; }
             }
-            // ---- a5: online softmax (exp2 domain), rows g (x = 0) and g+8 (x = 1)
-            const float mx0 = quad_max(fmaxf(fmaxf(sA[0], sA[1]), fmaxf(sB[0], sB[1])));
-            const float mx1 = quad_max(fmaxf(fmaxf(sA[2], sA[3]), fmaxf(sB[2], sB[3])));
-            const float mn0 = fmaxf(m_run[hh][mb][0], mx0), mn1 = fmaxf(m_run[hh][mb][1], mx1);
-            const float al0 = fast_exp2(m_run[hh][mb][0] - mn0), al1 = fast_exp2(m_run[hh][mb][1] - mn1);
+            // ---- a5: online softmax (exp2 domain), rows g (x = 0) and g+8 (x = 1).  The reference m of a row moves only
+            // when the tile maximum exceeds it by more than kLazy (P <= 2^kLazy stays well inside bf16 / fp32 range); a
+            // state (m, l, acc) is defined up to its reference (reading 19).  Rows that keep their reference
+            // have alpha == 1 exactly, so skipping the rescale when no row of the warp moved changes no bit.
+            constexpr float kLazy = 8.f;
+            const float mx0 = quad_max(fmaxf(fmaxf(sA[mb][0], sA[mb][1]), fmaxf(sB[mb][0], sB[mb][1])));
+            const float mx1 = quad_max(fmaxf(fmaxf(sA[mb][2], sA[mb][3]), fmaxf(sB[mb][2], sB[mb][3])));
+            const float mo0 = m_run[hh][mb][0], mo1 = m_run[hh][mb][1];
+            const bool mv0 = mx0 > mo0 + kLazy, mv1 = mx1 > mo1 + kLazy;
+            const float mn0 = mv0 ? mx0 : mo0, mn1 = mv1 ? mx1 : mo1;
             m_run[hh][mb][0] = mn0;
             m_run[hh][mb][1] = mn1;
-            sA[0] = fast_exp2(sA[0] - mn0); sA[1] = fast_exp2(sA[1] - mn0);
-            sB[0] = fast_exp2(sB[0] - mn0); sB[1] = fast_exp2(sB[1] - mn0);
-            sA[2] = fast_exp2(sA[2] - mn1); sA[3] = fast_exp2(sA[3] - mn1);
-            sB[2] = fast_exp2(sB[2] - mn1); sB[3] = fast_exp2(sB[3] - mn1);
-            l_run[hh][mb][0] = fmaf(l_run[hh][mb][0], al0, (sA[0] + sA[1]) + (sB[0] + sB[1]));
-            l_run[hh][mb][1] = fmaf(l_run[hh][mb][1], al1, (sA[2] + sA[3]) + (sB[2] + sB[3]));
-            const uint32_t p0 = pack_bf16(sA[0], sA[1]), p1 = pack_bf16(sA[2], sA[3]);
-            const uint32_t p2 = pack_bf16(sB[0], sB[1]), p3 = pack_bf16(sB[2], sB[3]);
-            // ---- a6: acc = acc * alpha + P V
+            sA[mb][0] = fast_exp2(sA[mb][0] - mn0); sA[mb][1] = fast_exp2(sA[mb][1] - mn0);
+            sB[mb][0] = fast_exp2(sB[mb][0] - mn0); sB[mb][1] = fast_exp2(sB[mb][1] - mn0);
+            sA[mb][2] = fast_exp2(sA[mb][2] - mn1); sA[mb][3] = fast_exp2(sA[mb][3] - mn1);
+            sB[mb][2] = fast_exp2(sB[mb][2] - mn1); sB[mb][3] = fast_exp2(sB[mb][3] - mn1);
+            const float sum0 = (sA[mb][0] + sA[mb][1]) + (sB[mb][0] + sB[mb][1]);
+            const float sum1 = (sA[mb][2] + sA[mb][3]) + (sB[mb][2] + sB[mb][3]);
+            if (__any_sync(0xffffffffu, mv0 || mv1)) {
+              const float al0 = mv0 ? fast_exp2(mo0 - mn0) : 1.f, al1 = mv1 ? fast_exp2(mo1 - mn1) : 1.f;
+              l_run[hh][mb][0] *= al0;
+              l_run[hh][mb][1] *= al1;
 #pragma unroll
-            for (int nd = 0; nd < ND; ++nd) {
-#ifndef EXP_NORESCALE
-              o[hh][mb][nd][0] *= al0; o[hh][mb][nd][1] *= al0;
-              o[hh][mb][nd][2] *= al1; o[hh][mb][nd][3] *= al1;
-#endif
-              mma_bf16(o[hh][mb][nd], p0, p1, p2, p3, vf[nd].x, vf[nd].y);
+              for (int nd = 0; nd < ND; ++nd) {
+                o[hh][mb][nd][0] *= al0; o[hh][mb][nd][1] *= al0;
+                o[hh][mb][nd][2] *= al1; o[hh][mb][nd][3] *= al1;
+              }
             }
+            l_run[hh][mb][0] += sum0;
+            l_run[hh][mb][1] += sum1;
+            pf[mb][0] = pack_bf16(sA[mb][0], sA[mb][1]); pf[mb][1] = pack_bf16(sA[mb][2], sA[mb][3]);
+            pf[mb][2] = pack_bf16(sB[mb][0], sB[mb][1]); pf[mb][3] = pack_bf16(sB[mb][2], sB[mb][3]);
           }
+          // ---- a6: acc += P V
+#pragma unroll
+          for (int nd = 0; nd < ND; ++nd)
+#pragma unroll
+            for (int mb = 0; mb < 2; ++mb)
+              mma_bf16(o[hh][mb][nd], pf[mb][0], pf[mb][1], pf[mb][2], pf[mb][3], vf[nd].x, vf[nd].y);
+          if (hh == 0) load_v(j0, h + 1); else load_v(jn, h - 1);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_bempty + 8 * bbuf);
@@ -579,7 +611,7 @@ template <int C, int CP>
 cudaError_t launch_c(const CUtensorMap& tm, const MmaParams& p, int64_t units, cudaStream_t st) {
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(fused_mma_kernel<C, CP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemAlloc);
+    cudaError_t e = cudaFuncSetAttribute(fused_mma_kernel<C, CP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_alloc(CP));
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
@@ -588,7 +620,7 @@ cudaError_t launch_c(const CUtensorMap& tm, const MmaParams& p, int64_t units, c
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (sms <= 0) sms = 148;
   const unsigned grid = (unsigned)(units < sms ? units : sms);
-  fused_mma_kernel<C, CP><<<grid, kThreads, kSmemAlloc, st>>>(tm, p);
+  fused_mma_kernel<C, CP><<<grid, kThreads, smem_alloc(CP), st>>>(tm, p);
   return cudaGetLastError();
 }
 

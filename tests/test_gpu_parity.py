@@ -161,9 +161,15 @@ def test_partial_states_and_merge(dtype, c_z, H):
                 raise
             got.append((m, l, acc))
             om, ol, oacc = states[cb]
-            # the state is defined up to the reference max: compare m, and l/acc rescaled to the oracle's m
+            # the state is defined up to its reference m (reading 19): l/acc are compared after rescaling to
+            # the oracle's m.  fp32 kernel: m is the row maximum.  bf16 tensor-core kernel: the reference follows the
+            # running maximum lazily -- never above it, at most 8 log2 units (8 ln 2) below it.
             f = np.exp(util.np64(m) - om)
-            assert np.max(np.abs(util.np64(m) - om)) <= (1e-4 if dtype == "f32" else 0.1)
+            dm = util.np64(m) - om
+            if dtype == "f32":
+                assert np.max(np.abs(dm)) <= 1e-4
+            else:
+                assert dm.max() <= 0.1 and dm.min() >= -(8.0 * np.log(2.0) + 0.1)
             assert np.max(np.abs(util.np64(l) * f - ol) / ol) <= tol
             a = util.np64(acc).reshape(len(rows), cfg.H, cfg.c) * f[..., None]
             assert np.max(np.abs(a - oacc)) <= tol * max(1.0, np.max(np.abs(oacc)))
