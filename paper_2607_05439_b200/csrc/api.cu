@@ -2,6 +2,7 @@
 // launch sequence  prologue (a1) -> fused kernel per sub-problem (a2-a7) -> merge + gate (a8) -> W_o (a9).
 // Decomposition emulation (PAPER.md:72-86 row stripes, :90 grid): one fused launch per stripe / quadrant on a
 // strided view of z (a base-pointer offset, no copy), partial states merged left to right by one kernel.
+#include <algorithm>
 #include <cstdio>
 #include <cstring>
 
@@ -23,12 +24,12 @@ Carve carve(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dt, int slots) 
   Carve w{};
   const size_t D = (size_t)H * c, e = elt_size(dt);
   // the tensor-core path keeps q, k zero-padded per head ([I][H][cp]) and v transposed ([D][ldv])
-  const size_t Dp = (size_t)H * mma_head_pad(c), ldv = (size_t)mma_ldv(I);
+  const size_t Dp = (size_t)H * mma_head_pad(c), frag = (size_t)mma_frag_elems(I, H, c);
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
   w.q = take((size_t)I * Dp * e);
-  w.k = take((size_t)I * Dp * e);
-  w.v = take(D * ldv * e);
+  w.k = take(std::max((size_t)I * Dp, frag) * e);
+  w.v = take(std::max((size_t)I * D, frag) * e);
   w.g = take((size_t)I * D * e);
   w.gated = take((size_t)I * D * e);
   w.s_ln = take((size_t)I * c_s * sizeof(float));
@@ -172,23 +173,23 @@ dcp_status run_prologue_mma(const Ctx& x, const void* s) {
     a = x.ws + x.cv.s_ln;
   }
   const int cp = mma_head_pad(x.c);
-  const int64_t ldv = mma_ldv(x.I);
-  if (cp != x.c) {   // zero the per-head padding of q and k
+  const size_t frag = (size_t)mma_frag_elems(x.I, x.H, x.c);
+  if (cp != x.c) {   // zero the per-head padding of q
     if (cudaMemsetAsync(x.ws + x.cv.q, 0, (size_t)x.I * x.H * cp * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
-    if (cudaMemsetAsync(x.ws + x.cv.k, 0, (size_t)x.I * x.H * cp * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
   }
-  if (ldv != x.I) {  // zero V^T beyond the last key (0 * finite in PV)
-    if (cudaMemsetAsync(x.ws + x.cv.v, 0, (size_t)x.D * ldv * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
+  if (cp != x.c || x.I % 16 != 0) {   // zero the head-dim padding and the keys beyond I (0 * finite in PV)
+    if (cudaMemsetAsync(x.ws + x.cv.k, 0, frag * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
+    if (cudaMemsetAsync(x.ws + x.cv.v, 0, frag * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
   }
   GemmMmaParams gp{};
   gp.A = a; gp.lda = x.c_s; gp.M = x.I; gp.N = x.D; gp.K = x.c_s; gp.nseg = 4;
   gp.W[0] = x.w->w_q; gp.W[1] = x.w->w_k; gp.W[2] = x.w->w_v; gp.W[3] = x.w->w_g;
   gp.bias[0] = x.w->b_q;
   gp.C[0] = x.ws + x.cv.q; gp.C[1] = x.ws + x.cv.k; gp.C[2] = x.ws + x.cv.v; gp.C[3] = x.ws + x.cv.g;
-  gp.mode[0] = GEMM_OUT_HEADPAD; gp.mode[1] = GEMM_OUT_HEADPAD; gp.mode[2] = GEMM_OUT_TRANSPOSED; gp.mode[3] = GEMM_OUT_SIGMOID;
+  gp.mode[0] = GEMM_OUT_HEADPAD; gp.mode[1] = GEMM_OUT_KFRAG; gp.mode[2] = GEMM_OUT_VFRAG; gp.mode[3] = GEMM_OUT_SIGMOID;
   gp.scale[0] = 1.4426950408889634f / sqrtf((float)x.c);   // log2(e)/sqrt(c): the softmax runs in the exp2 domain
   gp.scale[1] = 1.f;
-  gp.ldc[2] = ldv; gp.ldc[3] = x.D;
+  gp.ldc[3] = x.D;
   gp.H = x.H; gp.c = x.c; gp.cp = cp;
   DCP_CUDA(launch_gemm_mma(gp, x.st));
   DCP_CUDA(launch_fold_ln_z_mma(x.w->w_b, x.w->ln_z_gamma, x.w->ln_z_beta, x.ws + x.cv.wfold, (float*)(x.ws + x.cv.c1),
@@ -199,9 +200,8 @@ dcp_status run_prologue_mma(const Ctx& x, const void* s) {
 MmaParams base_params_mma(const Ctx& x) {
   MmaParams p{};
   p.qp = x.ws + x.cv.q;
-  p.kp = x.ws + x.cv.k;
-  p.vt = x.ws + x.cv.v;
-  p.ldv = mma_ldv(x.I);
+  p.kfr = x.ws + x.cv.k;
+  p.vfr = x.ws + x.cv.v;
   p.wfold = x.ws + x.cv.wfold;
   p.c1 = (const float*)(x.ws + x.cv.c1);
   p.c0 = (const float*)(x.ws + x.cv.c0);

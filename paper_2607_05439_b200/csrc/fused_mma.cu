@@ -419,8 +419,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     constexpr int KK = CP / 16;     // k-steps of QK^T
     constexpr int ND = C / 8;       // n-blocks of PV
     const __nv_bfloat16* qp = reinterpret_cast<const __nv_bfloat16*>(p.qp);
-    const __nv_bfloat16* kp = reinterpret_cast<const __nv_bfloat16*>(p.kp);
-    const __nv_bfloat16* vt = reinterpret_cast<const __nv_bfloat16*>(p.vt);
+    const uint4* kfr = reinterpret_cast<const uint4*>(p.kfr);
+    const uint4* vfr = reinterpret_cast<const uint4*>(p.vfr);
     int bbuf = 0;
     uint32_t bphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
@@ -453,23 +453,22 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             for (int x = 0; x < 4; ++x) o[hh][mb][nd][x] = 0.f;
         }
 
-      // K / V^T fragments of (key tile j, head h) are read from L2 into the registers the previous block just released:
-      // K right after the last QK^T MMA that used it, V^T right after the last PV MMA (software pipelining, no extra
-      // registers).  key of S column: n-block A col c <-> j + 4*(c/2) + c%2, n-block B col c <-> that + 2
-      uint2 kA[KK], kB[KK], vf[ND];
+      // K / V fragments of (key tile j, head h) are read from L2 into the registers the previous block just released:
+      // K right after the last QK^T MMA that used it, V right after the last PV MMA (software pipelining, no extra
+      // registers).  Both live in MMA B-fragment order (gemm_mma.cu), so every load is one coalesced 128-bit access per
+      // lane: K k-step kk -> (n-block A, n-block B) fragments, V n-block pair ndp -> fragments of nd = 2 ndp, 2 ndp + 1.
+      // key of S column: n-block A col c <-> j + 4*(c/2) + c%2, n-block B col c <-> that + 2
+      constexpr int NDP = CP / 16;
+      uint4 kq[KK], vq[NDP];
       auto load_k = [&](int j, int h) {
-        const int kAi = j + 4 * (g >> 1) + (g & 1);
-        const int64_t keyA = kAi < p.I ? kAi : p.I - 1;
-        const int64_t keyB = kAi + 2 < p.I ? kAi + 2 : p.I - 1;
+        const uint4* src = kfr + ((int64_t)((j >> 4) * kH + h) * KK) * 32 + lane;
 #pragma unroll
-        for (int kk = 0; kk < KK; ++kk) {
-          kA[kk] = ldg_u2(kp + (keyA * kH + h) * CP + kk * 16 + 4 * t);
-          kB[kk] = ldg_u2(kp + (keyB * kH + h) * CP + kk * 16 + 4 * t);
-        }
+        for (int kk = 0; kk < KK; ++kk) kq[kk] = __ldg(src + kk * 32);
       };
       auto load_v = [&](int j, int h) {
+        const uint4* src = vfr + ((int64_t)((j >> 4) * kH + h) * NDP) * 32 + lane;
 #pragma unroll
-        for (int nd = 0; nd < ND; ++nd) vf[nd] = ldg_u2(vt + ((int64_t)(h * C + nd * 8 + g)) * p.ldv + j + 4 * t);
+        for (int ndp = 0; ndp < NDP; ++ndp) vq[ndp] = __ldg(src + ndp * 32);
       };
       load_k(un.ks & ~(kTileK - 1), 2 * aw);
       load_v(un.ks & ~(kTileK - 1), 2 * aw);
@@ -497,8 +496,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             for (int mb = 0; mb < 2; ++mb) {
               const uint2 qa = lds_u32x2(q_frag + (mb * 16) * kQP + hh * (CP * 2) + kk * 32);
               const uint2 qb = lds_u32x2(q_frag + (mb * 16 + 8) * kQP + hh * (CP * 2) + kk * 32);
-              mma_bf16(sA[mb], qa.x, qb.x, qa.y, qb.y, kA[kk].x, kA[kk].y);
-              mma_bf16(sB[mb], qa.x, qb.x, qa.y, qb.y, kB[kk].x, kB[kk].y);
+              mma_bf16(sA[mb], qa.x, qb.x, qa.y, qb.y, kq[kk].x, kq[kk].y);
+              mma_bf16(sB[mb], qa.x, qb.x, qa.y, qb.y, kq[kk].z, kq[kk].w);
             }
           if (hh == 0) load_k(j0, h + 1); else load_k(jn, h - 1);
           uint32_t pf[2][4];
@@ -549,7 +548,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           for (int nd = 0; nd < ND; ++nd)
 #pragma unroll
             for (int mb = 0; mb < 2; ++mb)
-              mma_bf16(o[hh][mb][nd], pf[mb][0], pf[mb][1], pf[mb][2], pf[mb][3], vf[nd].x, vf[nd].y);
+              mma_bf16(o[hh][mb][nd], pf[mb][0], pf[mb][1], pf[mb][2], pf[mb][3],
+                       (nd & 1) ? vq[nd >> 1].z : vq[nd >> 1].x, (nd & 1) ? vq[nd >> 1].w : vq[nd >> 1].y);
           if (hh == 0) load_v(j0, h + 1); else load_v(jn, h - 1);
         }
         __syncwarp();
@@ -631,7 +631,7 @@ bool fused_mma_supports(dcp_dtype dt, int H, int c, int c_z) {
 }
 
 int mma_head_pad(int c) { return (c + 15) / 16 * 16; }
-int64_t mma_ldv(int64_t I) { return (I + 15) / 16 * 16; }
+int64_t mma_frag_elems(int64_t I, int H, int c) { return (I + 15) / 16 * H * (mma_head_pad(c) / 16) * 256; }
 
 // Segments per key chunk: a pure function of (I, n_kparts) so every decomposition cuts a row's keys alike.
 // Picks the count that best fills 148 SMs with (32-query tile) x (segment) units, charging the partial-state

@@ -5,8 +5,7 @@
 // 128 x 128 x 32 CTA tiles, cp.async double buffering.  The four projections run as ONE launch over
 // N = 4 D columns; the epilogue writes each segment in the layout the fused kernel reads:
 //   q -> qp [I][H][CP]  scaled by log2(e)/sqrt(c) (exp2-domain softmax), head rows zero-padded to CP
-//   k -> kp [I][H][CP]
-//   v -> vt [H*c][ldv]  transposed (key index contiguous) so PV's B fragments are 64-bit loads
+//   k -> kfr, v -> vfr  in the MMA B-fragment order of the fused kernel (one coalesced 128-bit load per lane)
 //   g -> g  [I][D]      sigmoid gate
 // Every output element is accumulated over k in a fixed order that does not depend on the tile it falls in.
 #include "kernels.h"
@@ -142,6 +141,24 @@ __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
         } else if (mode == GEMM_OUT_HEADPAD) {
           const int h = col / p.c, d = col % p.c;   // c even, col even: the pair stays inside one head
           *reinterpret_cast<__nv_bfloat162*>(C + (row * p.H + h) * p.cp + d) = __floats2bfloat162_rn(v0 * p.scale[seg], v1 * p.scale[seg]);
+        } else if (mode == GEMM_OUT_KFRAG) {
+          // K as the B operand of S = Q K^T (m16n8k16): lane (g, t) of key tile `row / 16` holds, for k-step kk, the
+          // 4 head dims 16 kk + 4t .. + 3 of key 4 (g / 2) + g % 2 (n-block A) and of that key + 2 (n-block B)
+          const int h = col / p.c, d = col % p.c, r = (int)(row & 15);
+          const int lane_f = (2 * (r >> 2) + (r & 1)) * 4 + ((d & 15) >> 2);
+          const int64_t idx = ((((row >> 4) * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + lane_f) * 8 + ((r >> 1) & 1) * 4 + (d & 3);
+          *reinterpret_cast<__nv_bfloat162*>(C + idx) = __floats2bfloat162_rn(v0, v1);
+        } else if (mode == GEMM_OUT_VFRAG) {
+          // V as the B operand of acc += P V: lane (g, t) holds, for the n-block pair ndp, keys 4t .. 4t + 3 of the tile
+          // for head dims 16 ndp + g and 16 ndp + 8 + g
+          const int h = col / p.c, r = (int)(row & 15);
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int d = col % p.c + e;
+            const int lane_f = (d & 7) * 4 + (r >> 2);
+            const int64_t idx = ((((row >> 4) * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + lane_f) * 8 + ((d >> 3) & 1) * 4 + (r & 3);
+            C[idx] = __float2bfloat16_rn(e == 0 ? v0 : v1);
+          }
         } else {   // GEMM_OUT_TRANSPOSED: vt[col][row]
           C[(int64_t)col * p.ldc[seg] + row] = __float2bfloat16_rn(v0);
           C[(int64_t)(col + 1) * p.ldc[seg] + row] = __float2bfloat16_rn(v1);

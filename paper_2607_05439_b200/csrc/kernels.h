@@ -24,7 +24,8 @@ cudaError_t launch_fused_generic(dcp_dtype dt, const FusedParams& p, cudaStream_
 bool fused_generic_supports(dcp_dtype dt, int H, int c, int c_z);
 
 // ---- bf16 tensor-core path (fused_mma.cu, gemm_mma.cu)
-enum GemmOutMode { GEMM_OUT_PLAIN = 0, GEMM_OUT_SIGMOID = 1, GEMM_OUT_HEADPAD = 2, GEMM_OUT_TRANSPOSED = 3 };
+enum GemmOutMode { GEMM_OUT_PLAIN = 0, GEMM_OUT_SIGMOID = 1, GEMM_OUT_HEADPAD = 2, GEMM_OUT_TRANSPOSED = 3,
+                   GEMM_OUT_KFRAG = 4, GEMM_OUT_VFRAG = 5 };
 
 // C_seg = epi(A[M,K] * W_seg[K,N] + bias_seg) for seg < nseg, all bf16 with fp32 accumulation (one launch).
 struct GemmMmaParams {
@@ -37,7 +38,7 @@ struct GemmMmaParams {
   int mode[4];          // GemmOutMode
   float scale[4];       // HEADPAD only
   int64_t ldc[4];       // PLAIN / SIGMOID: row pitch; TRANSPOSED: pitch of the transposed rows
-  int H, c, cp;         // HEADPAD: C[(row*H + h)*cp + d] for column h*c + d
+  int H, c, cp;         // HEADPAD: C[(row*H + h)*cp + d] for column h*c + d; KFRAG / VFRAG: MMA-fragment order (fused_mma.cu)
 };
 cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st);
 cudaError_t launch_layernorm_rows_bf16(const void* x, const void* gamma, const void* beta, void* y, int64_t rows,
@@ -52,9 +53,8 @@ cudaError_t launch_fold_ln_z_mma(const void* w_b, const void* gamma, const void*
 // (chunk cb, segment sg) writes partial-state slot slot0 + cb*nseg + sg.
 struct MmaParams {
   const void* qp;       // [I][H][cp] bf16, scaled by log2(e)/sqrt(c)
-  const void* kp;       // [I][H][cp] bf16
-  const void* vt;       // [H*c][ldv] bf16 (key index contiguous, zero beyond I)
-  int64_t ldv;
+  const void* kfr;      // K in QK^T B-fragment order: [key tile of 16][H][cp/16][32 lanes][8] bf16 (zero padded)
+  const void* vfr;      // V in PV B-fragment order:   [key tile of 16][H][cp/16][32 lanes][8] bf16 (zero padded)
   const void* wfold;    // [16][c_z] bf16
   const float* c1;      // [16]
   const float* c0;      // [16]
@@ -72,7 +72,7 @@ struct MmaParams {
 cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st);
 bool fused_mma_supports(dcp_dtype dt, int H, int c, int c_z);
 int mma_head_pad(int c);
-int64_t mma_ldv(int64_t I);
+int64_t mma_frag_elems(int64_t I, int H, int c);   // bf16 elements of kfr (= of vfr)
 int mma_num_segments(int64_t I, int n_kparts);
 
 // Merge (step a8) + normalise + gate (first half of a9); or raw merged state out.
