@@ -14,7 +14,7 @@ namespace dcp {
 
 namespace {
 
-constexpr int BM = 128, BN = 128, BK = 32;
+constexpr int BN = 128, BK = 32;   // BM = 32 MI: 128 (MI = 4) or 64 (MI = 2, for grids that would not fill the GPU)
 constexpr int LDA_S = BK + 8;    // padded smem rows: conflict-free ldmatrix
 constexpr int LDB_S = BN + 8;
 
@@ -40,11 +40,13 @@ __device__ __forceinline__ void mma16816(float (&d)[4], const uint32_t (&a)[4], 
                : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
 
+template <int MI>
 __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
+  constexpr int BM = 32 * MI;
   __shared__ __align__(16) __nv_bfloat16 As[2][BM * LDA_S];
   __shared__ __align__(16) __nv_bfloat16 Bs[2][BK * LDB_S];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int wm = warp >> 2, wn = warp & 3;            // 2 x 4 warps, warp tile 64 x 32
+  const int wm = warp >> 2, wn = warp & 3;            // 2 x 4 warps, warp tile (16 MI) x 32
   const int nb_per_seg = (p.N + BN - 1) / BN;
   const int seg = blockIdx.x / nb_per_seg;
   const int n0 = (blockIdx.x % nb_per_seg) * BN;
@@ -52,9 +54,9 @@ __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
   const __nv_bfloat16* A = reinterpret_cast<const __nv_bfloat16*>(p.A);
   const __nv_bfloat16* W = reinterpret_cast<const __nv_bfloat16*>(p.W[seg]);
 
-  float acc[4][4][4];
+  float acc[MI][4][4];
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+  for (int i = 0; i < MI; ++i)
 #pragma unroll
     for (int j = 0; j < 4; ++j)
 #pragma unroll
@@ -64,7 +66,7 @@ __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
 #pragma unroll
     for (int it = 0; it < 2; ++it) {
       const int e = tid + it * 256;
-      {   // A: 128 rows x 4 chunks of 8 elements
+      if (e < BM * 4) {   // A: BM rows x 4 chunks of 8 elements
         const int r = e >> 2, ch = e & 3;
         const int64_t gm = m0 + r;
         const int gk = k0 + ch * 8;
@@ -90,10 +92,10 @@ __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
     __syncthreads();
 #pragma unroll
     for (int ks = 0; ks < BK / 16; ++ks) {
-      uint32_t af[4][4], bf[4][2];
+      uint32_t af[MI][4], bf[4][2];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const int row = wm * 64 + i * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
+      for (int i = 0; i < MI; ++i) {
+        const int row = wm * (16 * MI) + i * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
         const int col = ks * 16 + (lane >> 4) * 8;
         ldsm_x4((uint32_t)__cvta_generic_to_shared(&As[buf][row * LDA_S + col]), af[i][0], af[i][1], af[i][2], af[i][3]);
       }
@@ -105,7 +107,7 @@ __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
                   bf[2 * j + 1][0], bf[2 * j + 1][1]);
       }
 #pragma unroll
-      for (int i = 0; i < 4; ++i)
+      for (int i = 0; i < MI; ++i)
 #pragma unroll
         for (int j = 0; j < 4; ++j) mma16816(acc[i][j], af[i], bf[j][0], bf[j][1]);
     }
@@ -116,10 +118,10 @@ __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
   const int g = lane >> 2, t = lane & 3;
   const int mode = p.mode[seg];
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+  for (int i = 0; i < MI; ++i)
 #pragma unroll
     for (int x = 0; x < 2; ++x) {
-      const int64_t row = m0 + wm * 64 + i * 16 + g + 8 * x;
+      const int64_t row = m0 + wm * (16 * MI) + i * 16 + g + 8 * x;
       if (row >= p.M) continue;
 #pragma unroll
       for (int j = 0; j < 4; ++j) {
@@ -192,7 +194,7 @@ __global__ void fold_ln_z_mma_kernel(const __nv_bfloat16* __restrict__ w_b, cons
                                      const __nv_bfloat16* __restrict__ beta, __nv_bfloat16* __restrict__ wfold,
                                      float* __restrict__ c1, float* __restrict__ c0, int c_z, int H, int H_pad) {
   // wfold[h][k] = bf16(gamma_k W_b[k,h] log2 e)   (K-major rows: the B operand of the projection MMA)
-  // c1[h] = sum_k wfold[h][k] (the rounded values, ascending k), c0[h] = log2 e * sum_k beta_k W_b[k,h]
+  // c1[h] = sum_k wfold[h][k] (the rounded values), c0[h] = log2 e * sum_k beta_k W_b[k,h]
   constexpr float kLog2e = 1.4426950408889634f;
   for (int e = threadIdx.x; e < H_pad * c_z; e += blockDim.x) {
     const int h = e / c_z, k = e % c_z;
@@ -200,15 +202,16 @@ __global__ void fold_ln_z_mma_kernel(const __nv_bfloat16* __restrict__ w_b, cons
     wfold[e] = __float2bfloat16_rn(v);
   }
   __syncthreads();
-  if (threadIdx.x < H_pad) {
-    const int h = threadIdx.x;
+  // one warp per head: lane-strided partial sums, then a butterfly reduction (fixed order: run-to-run repeatable)
+  for (int h = threadIdx.x >> 5; h < H_pad; h += blockDim.x >> 5) {
     float a1 = 0.f, a0 = 0.f;
-    for (int k = 0; k < c_z; ++k) {
+    for (int k = threadIdx.x & 31; k < c_z; k += 32) {
       a1 += to_f32(wfold[h * c_z + k]);
       if (h < H) a0 = fmaf(to_f32(beta[k]), to_f32(w_b[k * H + h]), a0);
     }
-    c1[h] = a1;
-    c0[h] = a0 * kLog2e;
+    a1 = warp_sum(a1);
+    a0 = warp_sum(a0);
+    if ((threadIdx.x & 31) == 0) { c1[h] = a1; c0[h] = a0 * kLog2e; }
   }
 }
 
@@ -217,8 +220,14 @@ __global__ void fold_ln_z_mma_kernel(const __nv_bfloat16* __restrict__ w_b, cons
 cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st) {
   if (p.M <= 0 || p.N <= 0 || p.K <= 0) return cudaSuccess;
   if (p.K % 8 != 0 || p.N % 8 != 0 || p.lda % 8 != 0) return cudaErrorInvalidValue;
-  dim3 grid((unsigned)(p.nseg * ((p.N + BN - 1) / BN)), (unsigned)((p.M + BM - 1) / BM));
-  gemm_mma_kernel<<<grid, 256, 0, st>>>(p);
+  const int64_t nb = (int64_t)p.nseg * ((p.N + BN - 1) / BN);
+  if (nb * ((p.M + 127) / 128) >= 2 * 148) {   // enough 128-row tiles for two CTAs per SM
+    dim3 grid((unsigned)nb, (unsigned)((p.M + 127) / 128));
+    gemm_mma_kernel<4><<<grid, 256, 0, st>>>(p);
+  } else {
+    dim3 grid((unsigned)nb, (unsigned)((p.M + 63) / 64));
+    gemm_mma_kernel<2><<<grid, 256, 0, st>>>(p);
+  }
   return cudaGetLastError();
 }
 
