@@ -90,7 +90,7 @@ dcp_status make_plan(int64_t I, int H, int c, int c_z, dcp_dtype dt, dcp_decomp 
   if (p.kernel == DCP_KERNEL_MMA && !mma_ok) return DCP_ERR_UNSUPPORTED;
   if (p.kernel == DCP_KERNEL_GENERIC && !fused_generic_supports(dt, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
   p.use_mma = mma_ok && p.kernel != DCP_KERNEL_GENERIC;
-  p.nseg = p.use_mma ? mma_num_segments(I, p.key_split) : 1;
+  p.nseg = p.use_mma ? mma_num_segments(I, H, p.key_split) : 1;
   p.slots = p.key_split * p.nseg;
   *out = p;
   return DCP_OK;
@@ -177,7 +177,7 @@ dcp_status run_prologue_mma(const Ctx& x, const void* s) {
   if (cp != x.c) {   // zero the per-head padding of q
     if (cudaMemsetAsync(x.ws + x.cv.q, 0, (size_t)x.I * x.H * cp * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
   }
-  if (cp != x.c || x.I % 16 != 0) {   // zero the head-dim padding and the keys beyond I (0 * finite in PV)
+  if (cp != x.c || x.I % 32 != 0) {   // zero the head-dim padding and the keys beyond I (0 * finite in PV)
     if (cudaMemsetAsync(x.ws + x.cv.k, 0, frag * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
     if (cudaMemsetAsync(x.ws + x.cv.v, 0, frag * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
   }
@@ -206,7 +206,9 @@ MmaParams base_params_mma(const Ctx& x) {
   p.c1 = (const float*)(x.ws + x.cv.c1);
   p.c0 = (const float*)(x.ws + x.cv.c0);
   p.I = (int)x.I;
+  p.H = x.H;
   p.c = x.c;
+  p.c_z = x.c_z;
   p.eps = x.eps;
   return p;
 }

@@ -19,10 +19,8 @@
 // Work unit = (32-query tile) x (key segment); key tiles are aligned to absolute multiples of 16 and a row's
 // arithmetic depends only on its key segments, so row(P) == monolithic and grid(GxG) == monolithic(key_split=G)
 // bitwise.  No atomics.
-#include <cuda.h>
-#include <cudaTypedefs.h>
-
 #include "kernels.h"
+#include "mma_ptx.cuh"
 
 namespace dcp {
 
@@ -52,185 +50,6 @@ constexpr size_t kSmemBar = kSmemWt + 2 * (size_t)kWtHalfBytes;
 constexpr size_t kSmemQ = (kSmemBar + (2 * kNZ + 8) * 8 + 16 + 15) / 16 * 16;   // Q tile [32 rows][H][CP] bf16, padded rows
 __host__ __device__ constexpr int q_pitch(int CP) { return kH * CP * 2 + 32; }      // bytes; +32: conflict-free 64-bit loads
 __host__ __device__ constexpr size_t smem_alloc(int CP) { return kSmemQ + (size_t)kTileQ * q_pitch(CP) + 1024; }  // + alignment slack
-
-// ------------------------------------------------------------------ PTX helpers
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t done;
-  uint32_t spins = 0;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-    // watchdog: a pipeline bug must surface as a CUDA error, never as a hung GPU (each failed try_wait already
-    // sleeps for the hardware time limit, so 2^24 failures is seconds)
-    if (!done && ++spins == (1u << 24)) __trap();
-  } while (!done);
-}
-// ---- tcgen05 / TMEM (5th-generation tensor cores): single-thread MMA issue, accumulators in tensor memory
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
-  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
-  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
-  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
-}
-// K-major operand tile, 128-byte swizzle: rows of 64 bf16 (128 B), 8-row groups 1024 B apart (SBO), descriptor
-// version 1 (sm_100), layout type 2 = SWIZZLE_128B.  `addr` may be advanced by 32 B per K = 16 step inside the atom.
-__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t addr) {
-  return (uint64_t)((addr & 0x3ffffu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) |
-         ((uint64_t)2 << 61);
-}
-// instruction descriptor, kind::f16: D = f32, A = B = bf16, both K-major, M x N
-__host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
-}
-__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "setp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-      ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
-__device__ __forceinline__ void tmem_ld_x16(uint32_t taddr, float (&v)[16]) {
-  uint32_t r[16];
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-                 "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-               : "r"(taddr));
-#pragma unroll
-  for (int i = 0; i < 16; ++i) v[i] = __uint_as_float(r[i]);
-}
-__device__ __forceinline__ float tmem_ld_x1(uint32_t taddr) {
-  uint32_t r;
-  asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(r) : "r"(taddr));
-  return __uint_as_float(r);
-}
-__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tmap, int c0, int c1, int c2, uint32_t bar,
-                                            uint64_t policy) {
-  asm volatile(
-      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
-      " [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(policy)
-      : "memory");
-}
-__device__ __forceinline__ void mma_bf16(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
-                                         uint32_t b1) {
-  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, "
-               "{%0, %1, %2, %3};"
-               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
-}
-__device__ __forceinline__ void sts_f32(uint32_t addr, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory"); }
-__device__ __forceinline__ float4 lds_f32x4(uint32_t addr) {
-  float4 v;
-  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ uint4 lds_u32x4(uint32_t addr) {
-  uint4 v;
-  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
-  return v;
-}
-__device__ __forceinline__ uint2 lds_u32x2(uint32_t addr) {
-  uint2 v;
-  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
-  return v;
-}
-// acc_lo += lo(w)^2, acc_hi += hi(w)^2 for a bf16x2 word: mixed-precision FMA (bf16 x bf16 + f32, PTX ISA 8.6, sm_100:
-// SASS FHFMA.BF16 with .H0/.H1 operand selectors), exact products, fp32 accumulation, no unpacking instructions
-__device__ __forceinline__ void fma_sq_bf16x2(float& acc_lo, float& acc_hi, uint32_t w) {
-  asm("{\n\t.reg .b16 l, h;\n\t"
-      "mov.b32 {l, h}, %2;\n\t"
-      "fma.rn.f32.bf16 %0, l, l, %0;\n\t"
-      "fma.rn.f32.bf16 %1, h, h, %1;\n\t}"
-      : "+f"(acc_lo), "+f"(acc_hi) : "r"(w));
-}
-__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
-  uint32_t r;
-  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
-  return r;
-}
-__device__ __forceinline__ float fast_exp2(float x) {
-  float y;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-__device__ __forceinline__ uint2 ldg_u2(const void* p) { return __ldg(reinterpret_cast<const uint2*>(p)); }
-__device__ __forceinline__ float quad_max(float v) {
-  v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1));
-  return fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 2));
-}
-__device__ __forceinline__ float quad_sum(float v) {
-  v += __shfl_xor_sync(0xffffffffu, v, 1);
-  return v + __shfl_xor_sync(0xffffffffu, v, 2);
-}
-
-// ------------------------------------------------------------------ work units
-struct Unit {
-  int q0;      // first query row of the 32-row tile
-  int q_end;   // end of the query part the tile belongs to (rows >= q_end are not computed / stored)
-  int ks, ke;  // key segment
-  int slot;    // partial-state slot
-};
-
-// Eq. 5 in 32-bit (I <= 2^30)
-__device__ __forceinline__ void shard32(int n, int parts, int p, int* start, int* len) {
-  const int base = n / parts, rem = n % parts;
-  *len = base + (p < rem ? 1 : 0);
-  *start = p * base + (p < rem ? p : rem);
-}
-
-__host__ __device__ inline int64_t mma_num_units(int n, int n_qparts, int n_kparts, int nseg) {
-  // query parts have sizes floor(n/P) or floor(n/P)+1 (Eq. 5): count their 32-row tiles in closed form
-  const int base = n / n_qparts, rem = n % n_qparts;
-  const int t_big = (base + 1 + kTileQ - 1) / kTileQ, t_small = (base + kTileQ - 1) / kTileQ;
-  return ((int64_t)rem * t_big + (int64_t)(n_qparts - rem) * t_small) * n_kparts * nseg;
-}
-
-__device__ __forceinline__ Unit decode_unit(const MmaParams& p, int u) {
-  const int n = p.q_end - p.q_begin;
-  const int base = n / p.n_qparts, rem = n % p.n_qparts;
-  const int t_big = (base + 1 + kTileQ - 1) / kTileQ, t_small = (base + kTileQ - 1) / kTileQ;
-  const int per_tile = p.n_kparts * p.nseg;
-  int tile = u / per_tile;
-  const int r = u - tile * per_tile;
-  int part, tq;
-  if (tile < rem * t_big) { part = tile / t_big; tq = tile - part * t_big; }
-  else { tile -= rem * t_big; part = tile / t_small; tq = tile - part * t_small; part += rem; }
-  int ps, pl;
-  shard32(n, p.n_qparts, part, &ps, &pl);
-  Unit un;
-  un.q0 = p.q_begin + ps + tq * kTileQ;
-  un.q_end = p.q_begin + ps + pl;
-  const int cb = r / p.nseg, sg = r - cb * p.nseg;
-  int cs, cl, ss, sl;
-  shard32(p.k_end - p.k_begin, p.n_kparts, cb, &cs, &cl);
-  shard32(cl, p.nseg, sg, &ss, &sl);
-  un.ks = p.k_begin + cs + ss;
-  un.ke = un.ks + sl;
-  un.slot = p.slot0 + r;
-  return un;
-}
-
-template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
-template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
 // ------------------------------------------------------------------ the kernel
 // C = head dim, CP = C rounded up to a multiple of 16 (q/k rows are zero-padded to CP by the prologue)
@@ -277,7 +96,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   tc_fence_after();
   const uint32_t tmem_base = *s_tmem;
 
-  const int n_units = (int)mma_num_units(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
+  const int n_units = (int)mma_num_units<kTileQ>(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
 
   if (warp < kProjWarp0) {
     // =============================================================== TMA producer (warp 0, one lane)
@@ -288,7 +107,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
       int stage = 0;
       uint32_t phase = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const Unit un = decode_unit(p, u);
+        const Unit un = decode_unit<kTileQ>(p, u);
         const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
         const int nsub = (rows + kSubQ - 1) / kSubQ;
         for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
@@ -313,7 +132,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
       int stage = 0, tb = 0;
       uint32_t phase = 0, tphase = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const Unit un = decode_unit(p, u);
+        const Unit un = decode_unit<kTileQ>(p, u);
         const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
         const int nsub = (rows + kSubQ - 1) / kSubQ;
         for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
@@ -355,7 +174,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     int tb = 0, bbuf = 0, stage = 0;
     uint32_t tphase = 0, bphase = 0, zphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const Unit un = decode_unit(p, u);
+      const Unit un = decode_unit<kTileQ>(p, u);
       const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
       const int nsub = (rows + kSubQ - 1) / kSubQ;
       for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
@@ -424,7 +243,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     int bbuf = 0;
     uint32_t bphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const Unit un = decode_unit(p, u);
+      const Unit un = decode_unit<kTileQ>(p, u);
       // Q tile -> shared memory (rows of the tile, all heads), shared by the 8 attention warps; row pitch padded so the
       // per-thread 64-bit fragment loads are conflict-free.  Named barrier 1 = the 256 attention threads.
       constexpr int kQP = q_pitch(CP);
@@ -593,20 +412,6 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
 }
 
 // ------------------------------------------------------------------ host side
-PFN_cuTensorMapEncodeTiled get_encode_fn() {
-  static PFN_cuTensorMapEncodeTiled fn = nullptr;
-  static bool tried = false;
-  if (!tried) {
-    tried = true;
-    void* ptr = nullptr;
-    cudaDriverEntryPointQueryResult qres;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &qres) == cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
-      fn = reinterpret_cast<PFN_cuTensorMapEncodeTiled>(ptr);
-  }
-  return fn;
-}
-
 template <int C, int CP>
 cudaError_t launch_c(const CUtensorMap& tm, const MmaParams& p, int64_t units, cudaStream_t st) {
   static bool attr_set = false;
@@ -627,17 +432,19 @@ cudaError_t launch_c(const CUtensorMap& tm, const MmaParams& p, int64_t units, c
 }  // namespace
 
 bool fused_mma_supports(dcp_dtype dt, int H, int c, int c_z) {
-  return dt == DCP_BF16 && H == kH && c_z == kCz && (c == 24 || c == 32 || c == 48);
+  return (dt == DCP_BF16 && H == kH && c_z == kCz && (c == 24 || c == 32 || c == 48)) || fused_atom_supports(dt, H, c, c_z);
 }
 
 int mma_head_pad(int c) { return (c + 15) / 16 * 16; }
-int64_t mma_frag_elems(int64_t I, int H, int c) { return (I + 15) / 16 * H * (mma_head_pad(c) / 16) * 256; }
+// keys rounded up to 32: the atom kernel reads K / V two 16-key blocks at a time
+int64_t mma_frag_elems(int64_t I, int H, int c) { return (I + 31) / 32 * 2 * H * (mma_head_pad(c) / 16) * 256; }
 
 // Segments per key chunk: a pure function of (I, n_kparts) so every decomposition cuts a row's keys alike.
 // Picks the count that best fills 148 SMs with (32-query tile) x (segment) units, charging the partial-state
 // round trip (~25 * segments / I of the z bytes) and keeping segments >= 64 keys.
-int mma_num_segments(int64_t I, int n_kparts) {
-  const int64_t qtiles = (I + kTileQ - 1) / kTileQ;
+int mma_num_segments(int64_t I, int H, int n_kparts) {
+  const int tile_q = H == kH ? kTileQ : fused_atom_tile_q();
+  const int64_t qtiles = (I + tile_q - 1) / tile_q;
   const int64_t chunk = I / n_kparts;
   int best = 1;
   double best_score = -1.0;
@@ -654,6 +461,7 @@ int mma_num_segments(int64_t I, int n_kparts) {
 }
 
 cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st) {
+  if (p.H != kH) return launch_fused_atom(p, z, ldz, st);
   if (p.q_end <= p.q_begin || p.k_end <= p.k_begin) return cudaSuccess;
   PFN_cuTensorMapEncodeTiled enc = get_encode_fn();
   if (!enc) return cudaErrorNotSupported;
@@ -666,7 +474,7 @@ cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cud
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
-  const int64_t units = mma_num_units(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
+  const int64_t units = mma_num_units<kTileQ>(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
   if (units > 0x7fffffff) return cudaErrorInvalidValue;
   switch (p.c) {
     case 24: return launch_c<24, 32>(tm, p, units, st);

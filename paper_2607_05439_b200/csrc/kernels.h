@@ -66,14 +66,18 @@ struct MmaParams {
   int q_begin, q_end, n_qparts;
   int k_begin, k_end, n_kparts;
   int nseg, slot0;
-  int c;
+  int H, c, c_z;
   float eps;
 };
 cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st);
 bool fused_mma_supports(dcp_dtype dt, int H, int c, int c_z);
 int mma_head_pad(int c);
 int64_t mma_frag_elems(int64_t I, int H, int c);   // bf16 elements of kfr (= of vfr)
-int mma_num_segments(int64_t I, int n_kparts);
+int mma_num_segments(int64_t I, int H, int n_kparts);
+// atom-level shape (c_atompair = 16, H = 4, c = 32): fused_atom.cu, dispatched to by launch_fused_mma
+cudaError_t launch_fused_atom(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st);
+bool fused_atom_supports(dcp_dtype dt, int H, int c, int c_z);
+int fused_atom_tile_q();
 
 // Merge (step a8) + normalise + gate (first half of a9); or raw merged state out.
 cudaError_t launch_merge(dcp_dtype dt, const MergeParams& p, cudaStream_t st);
