@@ -52,6 +52,9 @@ def parse():
     ap.add_argument("--cpu-rows", type=int, default=0, help="oracle sample rows (0: sized for ~10-20 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--ceiling", action="store_true",
+                    help="memory-ceiling mode (BASELINE.json config 3): largest I (multiple of 60, C3's widths) whose z, "
+                         "workspace, s and out fit one GPU; runs the layer there and checks sampled rows against the oracle")
     return ap.parse_args()
 
 
@@ -116,14 +119,15 @@ def default_parts(decomp, parts):
     return {"monolithic": 1, "row": 8, "grid": 16}[decomp]
 
 
-def oracle_sample(cfg, s, z, w, n_rows, seed=0):
+def oracle_sample(cfg, s, z, w, n_rows, seed=0, rows=None):
     """Time the fp64 oracle, as it stands, on `n_rows` sampled query rows x all I keys of this workload.
     Returns (pairs, seconds, threads, rows)."""
     import numpy as np
     import torch
     import dcp_synth as syn
     from oracle import pair_bias_attention as orc
-    rows = syn.sample_rows(cfg.I, n_rows, seed=seed)
+    if rows is None:
+        rows = syn.sample_rows(cfg.I, n_rows, seed=seed)
     idx = torch.as_tensor(rows, device=z.device)
     f64 = lambda t: t.detach().float().cpu().double().numpy()
     z_rows = z.index_select(0, idx).float().cpu().numpy()
@@ -175,6 +179,72 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def run_ceiling(args):
+    """Largest I = 60 n (C3's widths: c_s 384, c_z 128, H 16, c 48, bf16) that fits this GPU: bisection over n on
+    "z [I, I, c_z] + workspace + s + out allocate", then one warm-up + timed run of the layer at that size and a
+    sampled-row parity check against the oracle.  One JSON line with a `ceiling` object."""
+    import dataclasses
+    import numpy as np
+    import torch
+    import __graft_entry__ as ge
+    ge.build()
+    import dcp_synth as syn
+    import paper_2607_05439_b200 as dcp
+    dev = "cuda:0"
+    base = syn.CONFIGS["C3"]
+    free0, total = torch.cuda.mem_get_info()
+
+    def try_alloc(I):
+        try:
+            ws_bytes = dcp.dcp_workspace_bytes(I, base.c_s, base.H, base.c, base.c_z, torch.bfloat16, "monolithic", 1, 1, "auto")
+            z = torch.empty(I, I, base.c_z, dtype=torch.bfloat16, device=dev)
+            ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+            # room for the input generator's per-chunk fp32 temporaries and for s, out, weights
+            spare = torch.empty(768 << 20, dtype=torch.uint8, device=dev)
+            del spare
+            return z, ws
+        except torch.OutOfMemoryError:
+            return None
+
+    lo, hi = base.I // 60, 32000 // 60          # lo fits (C3 itself), hi cannot (245 GB of z)
+    while hi - lo > 1:
+        mid = (lo + hi) // 2
+        got = try_alloc(60 * mid)
+        ok = got is not None
+        del got
+        torch.cuda.empty_cache()
+        lo, hi = (mid, hi) if ok else (lo, mid)
+    I = 60 * lo
+    cfg = dataclasses.replace(base, name="ceiling", I=I, seed=base.seed + 7)
+    z, ws = try_alloc(I)
+    syn.fill_z(cfg, z, chunk_rows=8)
+    w = syn.make_weights(cfg, dev)
+    s = syn.make_s(cfg, dev)
+    out = torch.empty(I, cfg.c_s, dtype=torch.bfloat16, device=dev)
+    e0, e1 = dcp.Event(), dcp.Event()
+    for k in range(2):
+        e0.record()
+        dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, out=out, workspace=ws)
+        e1.record()
+        torch.cuda.synchronize()
+    ms = e0.elapsed_ms(e1)
+    peak_bytes = int(torch.cuda.max_memory_allocated())
+    rows = syn.sample_rows(I, 24, boundaries=[32, I // 2, I - 32], seed=5)
+    _, _, _, _, ref = oracle_sample(cfg, s, z, w, 0, rows=rows)
+    got = out.index_select(0, torch.as_tensor(rows, device=dev)).float().cpu().double().numpy()
+    rel = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
+    mab = float(np.abs(got - ref).max())
+    line = {"metric": METRIC, "unit": UNIT, "n_gpus": 1, "data": "synthetic", "dtype": "bf16",
+            "ceiling": {"I_max": I, "step": 60, "z_bytes": int(z.numel() * 2), "workspace_bytes": int(ws.numel()),
+                        "peak_device_bytes": peak_bytes, "device_total_bytes": int(total), "device_free_bytes_at_start": int(free0),
+                        "ms": ms, "value": I * float(I) / (ms * 1e-3) / 1e9,
+                        "hbm_frac": I * float(I) * cfg.c_z * 2 / (ms * 1e-3) / 1e9 / measured_peaks()[0],
+                        "sampled_rows": len(rows), "rel_l2_vs_oracle": rel, "max_abs_vs_oracle": mab,
+                        "parity_ok": bool(rel <= 1e-2 and mab <= 2e-2),
+                        "next_I_fails": 60 * hi}}
+    print(json.dumps(line), flush=True)
+
+
 def workload_name(cfg):
     kind = "atom-level" if cfg.name == "C4" else "token-level"
     return (f"{cfg.name}: {kind} pair-bias attention I={cfg.I} c_s={cfg.c_s} c_z={cfg.c_z} H={cfg.H} c={cfg.c} "
@@ -189,6 +259,10 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+        return
+    if args.ceiling:
+        if rank == 0:
+            run_ceiling(args)
         return
 
     import torch
@@ -278,9 +352,11 @@ def main():
     fused_avg_ms = sum(fused_ms) / len(fused_ms)
     alg_bytes = pairs_per_step * cfg.c_z * z.element_size()
     achieved = alg_bytes / (fused_avg_ms * 1e-3) / 1e9
-    kname = {"auto": None, "generic": "fused_generic_kernel", "mma": "fused_mma_kernel"}[args.kernel]
+    kname = {"auto": None, "generic": "fused_generic_kernel", "mma": "fused_mma_kernel" if cfg.H == 16 else "fused_atom_kernel"}[args.kernel]
     if kname is None:
-        kname = "fused_mma_kernel" if dcp.dcp_kernel_supported("mma", tdt, cfg.H, cfg.c, cfg.c_z) else "fused_generic_kernel"
+        kname = "fused_generic_kernel"
+        if dcp.dcp_kernel_supported("mma", tdt, cfg.H, cfg.c, cfg.c_z):
+            kname = "fused_mma_kernel" if cfg.H == 16 else "fused_atom_kernel"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES.get((kname, cfg.name)), "kernel": kname, "peak_source": peak_how,
                 "kernel_ms": fused_avg_ms, "kernel_share_of_step": fused_avg_ms * args.steps / total_ms,

@@ -177,7 +177,7 @@ dcp_status run_prologue_mma(const Ctx& x, const void* s) {
   if (cp != x.c) {   // zero the per-head padding of q
     if (cudaMemsetAsync(x.ws + x.cv.q, 0, (size_t)x.I * x.H * cp * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
   }
-  if (cp != x.c || x.I % 32 != 0) {   // zero the head-dim padding and the keys beyond I (0 * finite in PV)
+  if (cp != x.c) {   // zero the head-dim padding of the K / V fragments (keys beyond I are zero-filled by the GEMM)
     if (cudaMemsetAsync(x.ws + x.cv.k, 0, frag * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
     if (cudaMemsetAsync(x.ws + x.cv.v, 0, frag * 2, x.st) != cudaSuccess) return DCP_ERR_CUDA;
   }

@@ -43,8 +43,11 @@ __device__ __forceinline__ void mma16816(float (&d)[4], const uint32_t (&a)[4], 
 template <int MI>
 __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
   constexpr int BM = 32 * MI;
-  __shared__ __align__(16) __nv_bfloat16 As[2][BM * LDA_S];
-  __shared__ __align__(16) __nv_bfloat16 Bs[2][BK * LDB_S];
+  // pipeline buffers; after the main loop the same memory stages the C tile of the fragment-order outputs
+  constexpr int kAElems = 2 * BM * LDA_S, kBElems = 2 * BK * LDB_S, kCElems = BM * LDB_S;
+  __shared__ __align__(16) __nv_bfloat16 smem_raw[(kAElems + kBElems) > kCElems ? (kAElems + kBElems) : kCElems];
+  __nv_bfloat16 (*As)[BM * LDA_S] = reinterpret_cast<__nv_bfloat16 (*)[BM * LDA_S]>(smem_raw);
+  __nv_bfloat16 (*Bs)[BK * LDB_S] = reinterpret_cast<__nv_bfloat16 (*)[BK * LDB_S]>(smem_raw + kAElems);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int wm = warp >> 2, wn = warp & 3;            // 2 x 4 warps, warp tile (16 MI) x 32
   const int nb_per_seg = (p.N + BN - 1) / BN;
@@ -114,6 +117,53 @@ __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
     __syncthreads();
   }
 
+  // ---- epilogue, fragment-order outputs (k, v): the C tile goes through shared memory so that the global stores are
+  // 8-byte units written in destination order (256 contiguous bytes per warp) instead of scattered 2- / 4-byte stores
+  if (p.mode[seg] == GEMM_OUT_KFRAG || p.mode[seg] == GEMM_OUT_VFRAG) {
+    __nv_bfloat16* Cs = smem_raw;                       // [BM][LDB_S]; the main loop ended with __syncthreads()
+    const int g = lane >> 2, t = lane & 3;
+#pragma unroll
+    for (int i = 0; i < MI; ++i)
+#pragma unroll
+      for (int x = 0; x < 2; ++x) {
+        const int rl = wm * (16 * MI) + i * 16 + g + 8 * x;
+        const bool live = m0 + rl < p.M;                // rows beyond M are written as zeros (0 * finite in PV)
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+          *reinterpret_cast<__nv_bfloat162*>(Cs + rl * LDB_S + wn * 32 + j * 8 + 2 * t) =
+              live ? __floats2bfloat162_rn(acc[i][j][2 * x], acc[i][j][2 * x + 1]) : __floats2bfloat162_rn(0.f, 0.f);
+      }
+    __syncthreads();
+    __nv_bfloat16* C = reinterpret_cast<__nv_bfloat16*>(p.C[seg]);
+    const int64_t tile_end = (p.M + 31) / 32 * 2;       // key tiles the fragment buffers hold (mma_frag_elems)
+    const bool is_k = p.mode[seg] == GEMM_OUT_KFRAG;
+    for (int u = tid; u < BM * BN / 4; u += 256) {
+      // unit = [key tile kt][16-column group][g][t][b]: 8 bytes of lane (g, t)'s fragment
+      const int b = u & 1, tt = (u >> 1) & 3, gg = (u >> 3) & 7, grp = (u >> 6) & 7, kt = u >> 9;
+      const int64_t tile = (m0 >> 4) + kt;
+      if (tile >= tile_end) continue;
+      uint2 v;
+      int col;
+      if (is_k) {   // K: 4 head dims of key 4 (g / 2) + g % 2 + 2 b   (b = n-block A / B)
+        col = grp * 16 + 4 * tt;
+        v = *reinterpret_cast<const uint2*>(Cs + (kt * 16 + 4 * (gg >> 1) + (gg & 1) + 2 * b) * LDB_S + col);
+      } else {      // V: keys 4 t .. 4 t + 3 of head dim 8 b + g of the group
+        col = grp * 16 + 8 * b + gg;
+        const __nv_bfloat16* src = Cs + (kt * 16 + 4 * tt) * LDB_S + col;
+        const uint32_t e0 = *reinterpret_cast<const unsigned short*>(src), e1 = *reinterpret_cast<const unsigned short*>(src + LDB_S);
+        const uint32_t e2 = *reinterpret_cast<const unsigned short*>(src + 2 * LDB_S), e3 = *reinterpret_cast<const unsigned short*>(src + 3 * LDB_S);
+        v = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
+      }
+      const int ca = n0 + col;
+      if (ca >= p.N) continue;
+      const int h = ca / p.c, d = ca % p.c;
+      int64_t idx;
+      if (is_k) idx = (((tile * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + gg * 4 + ((d & 15) >> 2)) * 8 + b * 4;
+      else idx = (((tile * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + (d & 7) * 4 + tt) * 8 + ((d >> 3) & 1) * 4;
+      *reinterpret_cast<uint2*>(C + idx) = v;
+    }
+    return;
+  }
   // ---- epilogue
   const int g = lane >> 2, t = lane & 3;
   const int mode = p.mode[seg];
@@ -143,24 +193,6 @@ __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
         } else if (mode == GEMM_OUT_HEADPAD) {
           const int h = col / p.c, d = col % p.c;   // c even, col even: the pair stays inside one head
           *reinterpret_cast<__nv_bfloat162*>(C + (row * p.H + h) * p.cp + d) = __floats2bfloat162_rn(v0 * p.scale[seg], v1 * p.scale[seg]);
-        } else if (mode == GEMM_OUT_KFRAG) {
-          // K as the B operand of S = Q K^T (m16n8k16): lane (g, t) of key tile `row / 16` holds, for k-step kk, the
-          // 4 head dims 16 kk + 4t .. + 3 of key 4 (g / 2) + g % 2 (n-block A) and of that key + 2 (n-block B)
-          const int h = col / p.c, d = col % p.c, r = (int)(row & 15);
-          const int lane_f = (2 * (r >> 2) + (r & 1)) * 4 + ((d & 15) >> 2);
-          const int64_t idx = ((((row >> 4) * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + lane_f) * 8 + ((r >> 1) & 1) * 4 + (d & 3);
-          *reinterpret_cast<__nv_bfloat162*>(C + idx) = __floats2bfloat162_rn(v0, v1);
-        } else if (mode == GEMM_OUT_VFRAG) {
-          // V as the B operand of acc += P V: lane (g, t) holds, for the n-block pair ndp, keys 4t .. 4t + 3 of the tile
-          // for head dims 16 ndp + g and 16 ndp + 8 + g
-          const int h = col / p.c, r = (int)(row & 15);
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const int d = col % p.c + e;
-            const int lane_f = (d & 7) * 4 + (r >> 2);
-            const int64_t idx = ((((row >> 4) * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + lane_f) * 8 + ((d >> 3) & 1) * 4 + (r & 3);
-            C[idx] = __float2bfloat16_rn(e == 0 ? v0 : v1);
-          }
         } else {   // GEMM_OUT_TRANSPOSED: vt[col][row]
           C[(int64_t)col * p.ldc[seg] + row] = __float2bfloat16_rn(v0);
           C[(int64_t)(col + 1) * p.ldc[seg] + row] = __float2bfloat16_rn(v1);

@@ -110,7 +110,7 @@ def test_c1_bf16_full():
 @pytest.mark.parametrize("name,decomps", [
     ("C2", [("monolithic", 1), ("row", 8), ("grid", 16)]),   # stripes of 375, 4x4 grid of 750^2 quadrants
     ("C3", [("monolithic", 1), ("grid", 16)]),
-    ("C4", [("monolithic", 1), ("row", 16)]),
+    ("C4", [("monolithic", 1), ("row", 16), ("grid", 16)]),
 ])
 def test_full_size_sampled_rows(name, decomps):
     dcp = _dcp()
@@ -137,11 +137,12 @@ def test_full_size_sampled_rows(name, decomps):
 
 
 # ------------------------------------------------------------------ partial states and the merge kernel
-@pytest.mark.parametrize("dtype,c_z,H", [("f32", 32, 4), ("bf16", 32, 4), ("bf16", 128, 16)])
-def test_partial_states_and_merge(dtype, c_z, H):
+@pytest.mark.parametrize("dtype,c_z,H,c", [("f32", 32, 4, 24), ("bf16", 32, 4, 24), ("bf16", 128, 16, 24),
+                                           ("bf16", 16, 4, 32)])   # last: the atom-level tensor-core kernel
+def test_partial_states_and_merge(dtype, c_z, H, c):
     from oracle import decompositions as dec
     dcp = _dcp()
-    cfg = syn.small_config("ps", I=150, c_s=64, c_z=c_z, H=H, c=24, dtype=dtype, seed=33)
+    cfg = syn.small_config("ps", I=150, c_s=64, c_z=c_z, H=H, c=c, dtype=dtype, seed=33)
     s, z, w = util.make_problem(cfg, DEV)
     q0, q1 = 37, 101
     rows = list(range(q0, q1))
