@@ -245,6 +245,30 @@ def run_ceiling(args):
     print(json.dumps(line), flush=True)
 
 
+def replica_config(cfg, rank, world):
+    """"Replicas only": rank r runs its own copy of the layer on its own inputs."""
+    if world <= 1:
+        return cfg
+    import dataclasses
+    return dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+
+
+def max_over_ranks_ms(ms, world, device):
+    """Timing rule of the bench contract: a multi-rank number is the MAX over ranks of the device time."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_gpairs(I, steps, world, ms):
+    """Whole-job throughput: every rank processed I^2 pairs per step (weak scaling), in max-over-ranks time."""
+    return float(I) * I * steps * world / (ms * 1e-3) / 1e9
+
+
 def workload_name(cfg):
     kind = "atom-level" if cfg.name == "C4" else "token-level"
     return (f"{cfg.name}: {kind} pair-bias attention I={cfg.I} c_s={cfg.c_s} c_z={cfg.c_z} H={cfg.H} c={cfg.c} "
@@ -280,9 +304,7 @@ def main():
     dev = f"cuda:{local_rank}"
     cfg = syn.CONFIGS[args.workload]
     # every rank runs its own replica of the layer on its own inputs (seed offset by rank): no data-path collective
-    if world > 1:
-        import dataclasses
-        cfg = dataclasses.replace(cfg, seed=cfg.seed + 1000 * rank)
+    cfg = replica_config(cfg, rank, world)
     parts = default_parts(args.decomp, args.parts)
     atom = cfg.name == "C4"
     w = syn.make_weights(cfg, dev)
@@ -340,12 +362,9 @@ def main():
             total_ms += a.elapsed_ms(b)
     clocks = sampler.stop() if rank == 0 else None
     fused_ms = [a.elapsed_ms(b) for a, b in evs]
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks_ms(total_ms, world, dev)
     pairs_per_step = float(cfg.I) * cfg.I
-    value = pairs_per_step * args.steps * world / (total_ms * 1e-3) / 1e9
+    value = aggregate_gpairs(cfg.I, args.steps, world, total_ms)
 
     # ---- roofline of the dominant (fused) kernel: algorithmic bytes = z once = c_z * elt bytes per pair
     peak, peak_how = measured_peaks()
@@ -385,12 +404,9 @@ def main():
             b.record()
             torch.cuda.synchronize()
             ms = a.elapsed_ms(b)
-            if world > 1:
-                t = torch.tensor([ms], dtype=torch.float64, device=dev)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                ms = float(t.item())
+            ms = max_over_ranks_ms(ms, world, dev)
             assert torch.equal(oh.to(dev), out), "host entry disagrees with the device entry"
-            e2e = {"value": pairs_per_step * ne * world / (ms * 1e-3) / 1e9, "unit": UNIT,
+            e2e = {"value": aggregate_gpairs(cfg.I, ne, world, ms), "unit": UNIT,
                    "h2d_bytes_per_step": (sh.numel() + zh.numel()) * sh.element_size(),
                    "d2h_bytes_per_step": oh.numel() * oh.element_size(), "steps": ne,
                    "note": "PCIe host->device copy of z dominates"}
