@@ -251,6 +251,7 @@ __global__ void fold_ln_z_mma_kernel(const __nv_bfloat16* __restrict__ w_b, cons
 
 cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st) {
   if (p.M <= 0 || p.N <= 0 || p.K <= 0) return cudaSuccess;
+  if (gemm_tc_supports(p)) return launch_gemm_tc(p, st);
   if (p.K % 8 != 0 || p.N % 8 != 0 || p.lda % 8 != 0) return cudaErrorInvalidValue;
   const int64_t nb = (int64_t)p.nseg * ((p.N + BN - 1) / BN);
   if (nb * ((p.M + 127) / 128) >= 2 * 148) {   // enough 128-row tiles for two CTAs per SM

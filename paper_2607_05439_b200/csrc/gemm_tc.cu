@@ -1,0 +1,251 @@
+// tcgen05 GEMMs of the bf16 path: the single-track projections (step a1) and the output projection (step a9).
+//   PAPER.md:77-81 (sec 3.2): Q^(p) = f_Q(S^(p)); "keys and values are projected from the full single-track S"
+//   BASELINE.json config 0:  out = W_o (sigmoid(s W_g) (.) softmax(...) V)
+// C_seg[M, N] = A[M, K] (bf16 row-major = K-major) x W_seg[K, N] (bf16 row-major = MN-major B operand), fp32
+// accumulation in tensor memory.  One 128 x 128 output tile per CTA, K streamed in 64-wide blocks through a 3-stage
+// TMA / mbarrier ring (128-byte swizzle); two CTAs per SM overlap one tile's epilogue with the other's main loop.
+//   warp 0   TMA producer: A box (64 k, 128 rows), W boxes (64 n, 64 k) x 2
+//   warp 1   tcgen05 issuer (one lane): 4 x tcgen05.mma kind::f16 (M = 128, N = 128, K = 16) per k-block
+//   warps 2-5 epilogue: tcgen05.ld (thread = row) -> bias / scale / sigmoid -> bf16 -> shared C tile -> coalesced
+//            global stores in the layout the fused kernel reads (gemm_mma.cu lists the output modes)
+// The launcher falls back to the mma.sync kernel (gemm_mma.cu) for shapes this tiling does not cover
+// (N % 128, K % 64, unaligned pitches).  Every output element is accumulated over k in one fixed order.
+#include "kernels.h"
+#include "mma_ptx.cuh"
+
+namespace dcp {
+
+namespace {
+
+constexpr int TBM = 128, TBN = 128, TBK = 64, TST = 3;
+constexpr int kABytes = TBM * TBK * 2;                   // 16 KB
+constexpr int kBBytes = TBN * TBK * 2;                   // 16 KB: two (64 n x 64 k) boxes
+constexpr int kTcStage = kABytes + kBBytes;
+constexpr int kCsPitch = TBN + 8;                        // bf16 elements; +8: conflict-free 16-byte row writes
+constexpr size_t kTcSmemBar = (size_t)TST * kTcStage;
+constexpr size_t kTcSmemTotal = kTcSmemBar + (2 * TST + 2) * 8 + 16;
+constexpr size_t kTcSmemAlloc = kTcSmemTotal + 1024;
+static_assert(TBM * kCsPitch * 2 <= TST * kTcStage, "C tile is staged in the pipeline buffers");
+
+struct GemmTcMaps {
+  CUtensorMap a;
+  CUtensorMap w[4];
+};
+
+// MN-major operand tile (W[K][N], n contiguous), 128-byte swizzle: 64 n x 8 k atoms of 1024 B; atoms along k are
+// SBO = 1024 B apart, the second 64-n block of the tile LBO = 64 k-rows * 128 B = 8192 B further
+__device__ __forceinline__ uint64_t umma_desc_mn_sw128(uint32_t addr) {
+  return (uint64_t)((addr & 0x3ffffu) >> 4) | ((uint64_t)(8192 >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) |
+         ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tmap, int c0, int c1, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+               ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_ld_x32(uint32_t taddr, float (&v)[32]) {
+  uint32_t r[32];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+      "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+#pragma unroll
+  for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+__global__ void __launch_bounds__(192, 2) gemm_tc_kernel(const __grid_constant__ GemmTcMaps maps, const GemmMmaParams p) {
+  extern __shared__ unsigned char smem_dyn[];
+  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
+  const uint32_t s_base = smem_u32(smem);
+  const uint32_t s_bar = smem_u32(smem + kTcSmemBar);
+  const uint32_t bar_full = s_bar, bar_empty = s_bar + 8 * TST, bar_acc = s_bar + 16 * TST;
+  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + kTcSmemBar + (2 * TST + 2) * 8);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nb_per_seg = p.N / TBN;
+  const int seg = blockIdx.x / nb_per_seg;
+  const int n0 = (blockIdx.x % nb_per_seg) * TBN;
+  const int m0 = blockIdx.y * TBM;
+  const int nk = p.K / TBK;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < TST; ++s) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 1); }
+    mbar_init(bar_acc, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), TBN);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *s_tmem;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      // =============================================================== TMA producer
+      const CUtensorMap* wmap = &maps.w[seg];
+      for (int kb = 0; kb < nk; ++kb) {
+        const int stage = kb % TST;
+        mbar_wait(bar_empty + 8 * stage, ((kb / TST) & 1) ^ 1);
+        mbar_expect_tx(bar_full + 8 * stage, kTcStage);
+        const uint32_t dst = s_base + stage * kTcStage;
+        tma_load_2d(dst, &maps.a, kb * TBK, m0, bar_full + 8 * stage);
+        tma_load_2d(dst + kABytes, wmap, n0, kb * TBK, bar_full + 8 * stage);
+        tma_load_2d(dst + kABytes + kBBytes / 2, wmap, n0 + 64, kb * TBK, bar_full + 8 * stage);
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      // =============================================================== tcgen05 issuer
+      // instruction descriptor: D = f32, A = B = bf16, A K-major, B MN-major (bit 16), M = 128, N = 128
+      constexpr uint32_t idesc = umma_idesc_bf16(TBM, TBN) | (1u << 16);
+      for (int kb = 0; kb < nk; ++kb) {
+        const int stage = kb % TST;
+        mbar_wait(bar_full + 8 * stage, (kb / TST) & 1);
+        tc_fence_after();
+        const uint32_t a0 = s_base + stage * kTcStage, b0 = a0 + kABytes;
+#pragma unroll
+        for (int ks = 0; ks < TBK / 16; ++ks)
+          umma_bf16(tmem_base, umma_desc_sw128(a0 + ks * 32), umma_desc_mn_sw128(b0 + ks * 2048), idesc, (kb | ks) != 0);
+        umma_commit(bar_empty + 8 * stage);
+      }
+      umma_commit(bar_acc);
+    }
+  } else {
+    // =============================================================== epilogue (warps 2-5: TMEM lane quadrant = warp % 4)
+    const int quad = warp & 3, et = threadIdx.x - 64;      // et: 0..127 among the epilogue threads
+    const int row = quad * 32 + lane;                       // tile row of this thread = its TMEM lane
+    const int mode = p.mode[seg];
+    __nv_bfloat16* Cs = reinterpret_cast<__nv_bfloat16*>(smem);   // [128][kCsPitch], aliases the drained pipeline stages
+    mbar_wait(bar_acc, 0);
+    tc_fence_after();
+    const __nv_bfloat16* bias = reinterpret_cast<const __nv_bfloat16*>(p.bias[seg]);
+    const float scale = mode == GEMM_OUT_HEADPAD ? p.scale[seg] : 1.f;
+#pragma unroll
+    for (int ch = 0; ch < TBN / 32; ++ch) {
+      float v[32];
+      tmem_ld_x32(tmem_base + ((uint32_t)(quad * 32) << 16) + ch * 32, v);
+      tmem_ld_wait();
+      uint32_t w[16];
+#pragma unroll
+      for (int i = 0; i < 16; ++i) {
+        float v0 = v[2 * i], v1 = v[2 * i + 1];
+        if (bias != nullptr) {
+          v0 += __bfloat162float(bias[n0 + ch * 32 + 2 * i]);
+          v1 += __bfloat162float(bias[n0 + ch * 32 + 2 * i + 1]);
+        }
+        if (mode == GEMM_OUT_SIGMOID) {
+          v0 = 1.f / (1.f + expf(-v0));
+          v1 = 1.f / (1.f + expf(-v1));
+        }
+        w[i] = pack_bf16(v0 * scale, v1 * scale);
+      }
+      uint4* dst = reinterpret_cast<uint4*>(Cs + row * kCsPitch + ch * 32);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) dst[i] = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+    }
+    tc_fence_before();
+    asm volatile("bar.sync 1, 128;" ::: "memory");
+    __nv_bfloat16* C = reinterpret_cast<__nv_bfloat16*>(p.C[seg]);
+    if (mode == GEMM_OUT_PLAIN || mode == GEMM_OUT_SIGMOID || (mode == GEMM_OUT_HEADPAD && p.cp == p.c)) {
+      // row-major rows (HEADPAD without padding is [row][H * c]): 16 lanes store one 256-byte row segment
+      const int64_t ldc = mode == GEMM_OUT_HEADPAD ? (int64_t)p.H * p.c : p.ldc[seg];
+      for (int u = et; u < TBM * (TBN / 8); u += 128) {
+        const int r = u >> 4, c8 = u & 15;
+        if (m0 + r < p.M)
+          *reinterpret_cast<uint4*>(C + (int64_t)(m0 + r) * ldc + n0 + c8 * 8) = *reinterpret_cast<const uint4*>(Cs + r * kCsPitch + c8 * 8);
+      }
+    } else if (mode == GEMM_OUT_HEADPAD) {
+      for (int u = et; u < TBM * (TBN / 2); u += 128) {
+        const int r = u >> 6, col = (u & 63) * 2, ca = n0 + col;
+        if (m0 + r < p.M) {
+          const int h = ca / p.c, d = ca % p.c;    // c even, col even: the pair stays inside one head
+          *reinterpret_cast<uint32_t*>(C + ((int64_t)(m0 + r) * p.H + h) * p.cp + d) = *reinterpret_cast<const uint32_t*>(Cs + r * kCsPitch + col);
+        }
+      }
+    } else {
+      // K / V in the MMA B-fragment order of the fused kernels (see gemm_mma.cu): 8-byte units in destination order
+      const int64_t tile_end = (p.M + 31) / 32 * 2;
+      const bool is_k = mode == GEMM_OUT_KFRAG;
+      for (int u = et; u < TBM * TBN / 4; u += 128) {
+        const int b = u & 1, tt = (u >> 1) & 3, gg = (u >> 3) & 7, grp = (u >> 6) & 7, kt = u >> 9;
+        const int64_t tile = (m0 >> 4) + kt;
+        if (tile >= tile_end) continue;
+        uint2 v;
+        int col;
+        if (is_k) {
+          col = grp * 16 + 4 * tt;
+          v = *reinterpret_cast<const uint2*>(Cs + (kt * 16 + 4 * (gg >> 1) + (gg & 1) + 2 * b) * kCsPitch + col);
+        } else {
+          col = grp * 16 + 8 * b + gg;
+          const unsigned short* src = reinterpret_cast<const unsigned short*>(Cs + (kt * 16 + 4 * tt) * kCsPitch + col);
+          const uint32_t e0 = src[0], e1 = src[kCsPitch], e2 = src[2 * kCsPitch], e3 = src[3 * kCsPitch];
+          v = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
+        }
+        const int ca = n0 + col, h = ca / p.c, d = ca % p.c;
+        int64_t idx;
+        if (is_k) idx = (((tile * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + gg * 4 + ((d & 15) >> 2)) * 8 + b * 4;
+        else idx = (((tile * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + (d & 7) * 4 + tt) * 8 + ((d >> 3) & 1) * 4;
+        *reinterpret_cast<uint2*>(C + idx) = v;
+      }
+    }
+  }
+  // teardown: the epilogue has drained tensor memory before the allocating warp frees it
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    __syncwarp();
+    tmem_dealloc(tmem_base, TBN);
+  }
+}
+
+}  // namespace
+
+bool gemm_tc_supports(const GemmMmaParams& p) {
+  if (p.M <= 0 || p.N % TBN != 0 || p.K % TBK != 0 || p.lda % 8 != 0 || ((uintptr_t)p.A & 15) != 0) return false;
+  for (int s = 0; s < p.nseg; ++s) {
+    if (((uintptr_t)p.W[s] & 15) != 0 || ((uintptr_t)p.C[s] & 15) != 0) return false;
+    if ((p.mode[s] == GEMM_OUT_PLAIN || p.mode[s] == GEMM_OUT_SIGMOID) && p.ldc[s] % 8 != 0) return false;
+    if (p.mode[s] == GEMM_OUT_TRANSPOSED) return false;
+  }
+  return get_encode_fn() != nullptr;
+}
+
+cudaError_t launch_gemm_tc(const GemmMmaParams& p, cudaStream_t st) {
+  PFN_cuTensorMapEncodeTiled enc = get_encode_fn();
+  if (!enc) return cudaErrorNotSupported;
+  GemmTcMaps maps;
+  const cuuint32_t estr[2] = {1, 1};
+  {
+    const cuuint64_t gdim[2] = {(cuuint64_t)p.K, (cuuint64_t)p.M};
+    const cuuint64_t gstr[1] = {(cuuint64_t)p.lda * 2};
+    const cuuint32_t box[2] = {TBK, TBM};
+    if (enc(&maps.a, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(p.A), gdim, gstr, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
+  for (int s = 0; s < 4; ++s) {
+    const void* w = p.W[s < p.nseg ? s : 0];
+    const cuuint64_t gdim[2] = {(cuuint64_t)p.N, (cuuint64_t)p.K};
+    const cuuint64_t gstr[1] = {(cuuint64_t)p.N * 2};
+    const cuuint32_t box[2] = {64, TBK};
+    if (enc(&maps.w[s], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(w), gdim, gstr, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+  }
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemAlloc);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  dim3 grid((unsigned)(p.nseg * (p.N / TBN)), (unsigned)((p.M + TBM - 1) / TBM));
+  gemm_tc_kernel<<<grid, 192, kTcSmemAlloc, st>>>(maps, p);
+  return cudaGetLastError();
+}
+
+}  // namespace dcp
