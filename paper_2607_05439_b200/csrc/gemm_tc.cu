@@ -17,15 +17,19 @@ namespace dcp {
 
 namespace {
 
-constexpr int TBM = 128, TBN = 128, TBK = 64, TST = 3;
+constexpr int TBM = 128, TBK = 64, TST = 3;
 constexpr int kABytes = TBM * TBK * 2;                   // 16 KB
-constexpr int kBBytes = TBN * TBK * 2;                   // 16 KB: two (64 n x 64 k) boxes
-constexpr int kTcStage = kABytes + kBBytes;
-constexpr int kCsPitch = TBN + 8;                        // bf16 elements; +8: conflict-free 16-byte row writes
-constexpr size_t kTcSmemBar = (size_t)TST * kTcStage;
-constexpr size_t kTcSmemTotal = kTcSmemBar + (2 * TST + 2) * 8 + 16;
-constexpr size_t kTcSmemAlloc = kTcSmemTotal + 1024;
-static_assert(TBM * kCsPitch * 2 <= TST * kTcStage, "C tile is staged in the pipeline buffers");
+constexpr int kTcThreads = 64 + 256;                     // producer warp, issuer warp, 8 epilogue warps
+// per output-tile width TBN (128, or 64 for grids that would not fill the GPU)
+template <int TBN> struct TcCfg {
+  static constexpr int kBBytes = TBN * TBK * 2;          // TBN / 64 boxes of (64 n x 64 k)
+  static constexpr int kStage = kABytes + kBBytes;
+  static constexpr int kCsPitch = TBN + 8;               // bf16 elements; +8: conflict-free 16-byte row writes
+  static constexpr size_t kSmemBar = (size_t)TST * kStage;
+  static constexpr size_t kSmemHd = kSmemBar + (2 * TST + 2) * 8 + 16;   // (head, head dim) of the tile's columns
+  static constexpr size_t kSmemAlloc = kSmemHd + TBN * 4 + 1024;
+  static_assert(TBM * kCsPitch * 2 <= TST * kStage, "C tile is staged in the pipeline buffers");
+};
 
 struct GemmTcMaps {
   CUtensorMap a;
@@ -56,7 +60,11 @@ __device__ __forceinline__ void tmem_ld_x32(uint32_t taddr, float (&v)[32]) {
   for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
 }
 
-__global__ void __launch_bounds__(192, 2) gemm_tc_kernel(const __grid_constant__ GemmTcMaps maps, const GemmMmaParams p) {
+template <int TBN>
+__global__ void __launch_bounds__(kTcThreads, 2) gemm_tc_kernel(const __grid_constant__ GemmTcMaps maps, const GemmMmaParams p) {
+  using Cfg = TcCfg<TBN>;
+  constexpr int kTcStage = Cfg::kStage, kCsPitch = Cfg::kCsPitch;
+  constexpr size_t kTcSmemBar = Cfg::kSmemBar;
   extern __shared__ unsigned char smem_dyn[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
   const uint32_t s_base = smem_u32(smem);
@@ -92,8 +100,9 @@ __global__ void __launch_bounds__(192, 2) gemm_tc_kernel(const __grid_constant__
         mbar_expect_tx(bar_full + 8 * stage, kTcStage);
         const uint32_t dst = s_base + stage * kTcStage;
         tma_load_2d(dst, &maps.a, kb * TBK, m0, bar_full + 8 * stage);
-        tma_load_2d(dst + kABytes, wmap, n0, kb * TBK, bar_full + 8 * stage);
-        tma_load_2d(dst + kABytes + kBBytes / 2, wmap, n0 + 64, kb * TBK, bar_full + 8 * stage);
+#pragma unroll
+        for (int nb = 0; nb < TBN / 64; ++nb)
+          tma_load_2d(dst + kABytes + nb * 8192, wmap, n0 + 64 * nb, kb * TBK, bar_full + 8 * stage);
       }
     }
   } else if (warp == 1) {
@@ -114,54 +123,54 @@ __global__ void __launch_bounds__(192, 2) gemm_tc_kernel(const __grid_constant__
       umma_commit(bar_acc);
     }
   } else {
-    // =============================================================== epilogue (warps 2-5: TMEM lane quadrant = warp % 4)
-    const int quad = warp & 3, et = threadIdx.x - 64;      // et: 0..127 among the epilogue threads
+    // =============================================================== epilogue (warps 2-9: TMEM lane quadrant = warp % 4,
+    // the two warps of a quadrant take one half of the tile's columns each)
+    const int quad = warp & 3, half = (warp - 2) >> 2, et = threadIdx.x - 64;   // et: 0..255 among the epilogue threads
     const int row = quad * 32 + lane;                       // tile row of this thread = its TMEM lane
     const int mode = p.mode[seg];
     __nv_bfloat16* Cs = reinterpret_cast<__nv_bfloat16*>(smem);   // [128][kCsPitch], aliases the drained pipeline stages
+    short2* hd = reinterpret_cast<short2*>(smem + Cfg::kSmemHd);
+    if (et < TBN && p.c > 0) hd[et] = make_short2((short)((n0 + et) / p.c), (short)((n0 + et) % p.c));   // one division per column
     mbar_wait(bar_acc, 0);
     tc_fence_after();
     const __nv_bfloat16* bias = reinterpret_cast<const __nv_bfloat16*>(p.bias[seg]);
     const float scale = mode == GEMM_OUT_HEADPAD ? p.scale[seg] : 1.f;
 #pragma unroll
-    for (int ch = 0; ch < TBN / 32; ++ch) {
+    for (int c32 = 0; c32 < TBN / 64; ++c32) {
+      const int ch = half * (TBN / 64) + c32;               // 32-column chunk of the tile
       float v[32];
       tmem_ld_x32(tmem_base + ((uint32_t)(quad * 32) << 16) + ch * 32, v);
       tmem_ld_wait();
-      uint32_t w[16];
+      if (bias != nullptr) {
 #pragma unroll
-      for (int i = 0; i < 16; ++i) {
-        float v0 = v[2 * i], v1 = v[2 * i + 1];
-        if (bias != nullptr) {
-          v0 += __bfloat162float(bias[n0 + ch * 32 + 2 * i]);
-          v1 += __bfloat162float(bias[n0 + ch * 32 + 2 * i + 1]);
-        }
-        if (mode == GEMM_OUT_SIGMOID) {
-          v0 = 1.f / (1.f + expf(-v0));
-          v1 = 1.f / (1.f + expf(-v1));
-        }
-        w[i] = pack_bf16(v0 * scale, v1 * scale);
+        for (int i = 0; i < 32; ++i) v[i] += __bfloat162float(bias[n0 + ch * 32 + i]);
+      }
+      if (mode == GEMM_OUT_SIGMOID) {
+#pragma unroll
+        for (int i = 0; i < 32; ++i) v[i] = 1.f / (1.f + expf(-v[i]));
       }
       uint4* dst = reinterpret_cast<uint4*>(Cs + row * kCsPitch + ch * 32);
 #pragma unroll
-      for (int i = 0; i < 4; ++i) dst[i] = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+      for (int i = 0; i < 4; ++i)
+        dst[i] = make_uint4(pack_bf16(v[8 * i] * scale, v[8 * i + 1] * scale), pack_bf16(v[8 * i + 2] * scale, v[8 * i + 3] * scale),
+                            pack_bf16(v[8 * i + 4] * scale, v[8 * i + 5] * scale), pack_bf16(v[8 * i + 6] * scale, v[8 * i + 7] * scale));
     }
     tc_fence_before();
-    asm volatile("bar.sync 1, 128;" ::: "memory");
+    asm volatile("bar.sync 1, 256;" ::: "memory");
     __nv_bfloat16* C = reinterpret_cast<__nv_bfloat16*>(p.C[seg]);
     if (mode == GEMM_OUT_PLAIN || mode == GEMM_OUT_SIGMOID || (mode == GEMM_OUT_HEADPAD && p.cp == p.c)) {
-      // row-major rows (HEADPAD without padding is [row][H * c]): 16 lanes store one 256-byte row segment
+      // row-major rows (HEADPAD without padding is [row][H * c]): TBN / 8 lanes store one row segment of the tile
       const int64_t ldc = mode == GEMM_OUT_HEADPAD ? (int64_t)p.H * p.c : p.ldc[seg];
-      for (int u = et; u < TBM * (TBN / 8); u += 128) {
-        const int r = u >> 4, c8 = u & 15;
+      for (int u = et; u < TBM * (TBN / 8); u += 256) {
+        const int r = u / (TBN / 8), c8 = u % (TBN / 8);
         if (m0 + r < p.M)
           *reinterpret_cast<uint4*>(C + (int64_t)(m0 + r) * ldc + n0 + c8 * 8) = *reinterpret_cast<const uint4*>(Cs + r * kCsPitch + c8 * 8);
       }
     } else if (mode == GEMM_OUT_HEADPAD) {
-      for (int u = et; u < TBM * (TBN / 2); u += 128) {
-        const int r = u >> 6, col = (u & 63) * 2, ca = n0 + col;
+      for (int u = et; u < TBM * (TBN / 2); u += 256) {
+        const int r = u / (TBN / 2), col = (u % (TBN / 2)) * 2;
         if (m0 + r < p.M) {
-          const int h = ca / p.c, d = ca % p.c;    // c even, col even: the pair stays inside one head
+          const int h = hd[col].x, d = hd[col].y;  // c even, col even: the pair stays inside one head
           *reinterpret_cast<uint32_t*>(C + ((int64_t)(m0 + r) * p.H + h) * p.cp + d) = *reinterpret_cast<const uint32_t*>(Cs + r * kCsPitch + col);
         }
       }
@@ -169,8 +178,8 @@ __global__ void __launch_bounds__(192, 2) gemm_tc_kernel(const __grid_constant__
       // K / V in the MMA B-fragment order of the fused kernels (see gemm_mma.cu): 8-byte units in destination order
       const int64_t tile_end = (p.M + 31) / 32 * 2;
       const bool is_k = mode == GEMM_OUT_KFRAG;
-      for (int u = et; u < TBM * TBN / 4; u += 128) {
-        const int b = u & 1, tt = (u >> 1) & 3, gg = (u >> 3) & 7, grp = (u >> 6) & 7, kt = u >> 9;
+      for (int u = et; u < TBM * TBN / 4; u += 256) {
+        const int b = u & 1, tt = (u >> 1) & 3, gg = (u >> 3) & 7, grp = (u >> 6) % (TBN / 16), kt = u / (TBN * 4);
         const int64_t tile = (m0 >> 4) + kt;
         if (tile >= tile_end) continue;
         uint2 v;
@@ -184,7 +193,7 @@ __global__ void __launch_bounds__(192, 2) gemm_tc_kernel(const __grid_constant__
           const uint32_t e0 = src[0], e1 = src[kCsPitch], e2 = src[2 * kCsPitch], e3 = src[3 * kCsPitch];
           v = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
         }
-        const int ca = n0 + col, h = ca / p.c, d = ca % p.c;
+        const int h = hd[col].x, d = hd[col].y;
         int64_t idx;
         if (is_k) idx = (((tile * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + gg * 4 + ((d & 15) >> 2)) * 8 + b * 4;
         else idx = (((tile * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + (d & 7) * 4 + tt) * 8 + ((d >> 3) & 1) * 4;
@@ -204,7 +213,7 @@ __global__ void __launch_bounds__(192, 2) gemm_tc_kernel(const __grid_constant__
 }  // namespace
 
 bool gemm_tc_supports(const GemmMmaParams& p) {
-  if (p.M <= 0 || p.N % TBN != 0 || p.K % TBK != 0 || p.lda % 8 != 0 || ((uintptr_t)p.A & 15) != 0) return false;
+  if (p.M <= 0 || p.N % 64 != 0 || p.K % TBK != 0 || p.lda % 8 != 0 || ((uintptr_t)p.A & 15) != 0) return false;
   for (int s = 0; s < p.nseg; ++s) {
     if (((uintptr_t)p.W[s] & 15) != 0 || ((uintptr_t)p.C[s] & 15) != 0) return false;
     if ((p.mode[s] == GEMM_OUT_PLAIN || p.mode[s] == GEMM_OUT_SIGMOID) && p.ldc[s] % 8 != 0) return false;
@@ -239,12 +248,21 @@ cudaError_t launch_gemm_tc(const GemmMmaParams& p, cudaStream_t st) {
   }
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTcSmemAlloc);
+    cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TcCfg<128>::kSmemAlloc);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(gemm_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TcCfg<64>::kSmemAlloc);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  dim3 grid((unsigned)(p.nseg * (p.N / TBN)), (unsigned)((p.M + TBM - 1) / TBM));
-  gemm_tc_kernel<<<grid, 192, kTcSmemAlloc, st>>>(maps, p);
+  const unsigned mt = (unsigned)((p.M + TBM - 1) / TBM);
+  // 128-wide tiles when they give every SM two CTAs (or N does not split into 64s evenly enough to matter)
+  if (p.N % 128 == 0 && (int64_t)p.nseg * (p.N / 128) * mt >= 2 * 148) {
+    dim3 grid((unsigned)(p.nseg * (p.N / 128)), mt);
+    gemm_tc_kernel<128><<<grid, kTcThreads, TcCfg<128>::kSmemAlloc, st>>>(maps, p);
+  } else {
+    dim3 grid((unsigned)(p.nseg * (p.N / 64)), mt);
+    gemm_tc_kernel<64><<<grid, kTcThreads, TcCfg<64>::kSmemAlloc, st>>>(maps, p);
+  }
   return cudaGetLastError();
 }
 
