@@ -34,7 +34,9 @@ UNIT = "Gpair/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/, named per round); None = not captured for that kernel / workload.
 NCU_TRAFFIC_BYTES = {
-    # (kernel, workload): bytes
+    # (kernel, workload): bytes   -- profiles/r01_fused_c2_ncu_full.txt, profiles/r01_fused_atom_c4_ncu_full.txt
+    ("fused_mma_kernel", "C2"): 2330531000 + 7912448,
+    ("fused_atom_kernel", "C4"): 18746721000 + 124210176,
 }
 
 
