@@ -43,11 +43,12 @@ constexpr size_t kSmemZ = 0;
 constexpr size_t kSmemBias = kSmemZ + (size_t)kNZ * kStageBytes;
 constexpr int kProjN = 32;                               // projection MMA N: 16 heads, the ones row (sum z), zero rows
 constexpr int kWtHalfBytes = kProjN * 128;               // W'' tile: 32 rows x 64 channels bf16 per channel half
-constexpr int kTmemCols = 64;                            // 2 accumulator buffers x 32 projection columns
-constexpr int kTmemBufCols = 32;
+constexpr int kNT = 4;                                   // TMEM accumulator buffers
+constexpr int kTmemBufCols = 32;                         // projection columns per buffer
+constexpr int kTmemCols = kNT * kTmemBufCols;            // 128 (a power of two >= 32)
 constexpr size_t kSmemWt = (kSmemBias + 2 * (size_t)kBiasBufFloats * 4 + 1023) / 1024 * 1024;   // 1024-aligned (swizzle)
 constexpr size_t kSmemBar = kSmemWt + 2 * (size_t)kWtHalfBytes;
-constexpr size_t kSmemQ = (kSmemBar + (2 * kNZ + 8) * 8 + 16 + 15) / 16 * 16;   // Q tile [32 rows][H][CP] bf16, padded rows
+constexpr size_t kSmemQ = (kSmemBar + (2 * kNZ + 4 + 2 * kNT) * 8 + 16 + 15) / 16 * 16;   // Q tile [32 rows][H][CP] bf16, padded rows
 __host__ __device__ constexpr int q_pitch(int CP) { return kH * CP * 2 + 32; }      // bytes; +32: conflict-free 64-bit loads
 __host__ __device__ constexpr size_t smem_alloc(int CP) { return kSmemQ + (size_t)kTileQ * q_pitch(CP) + 1024; }  // + alignment slack
 
@@ -64,8 +65,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   const uint32_t s_bar = smem_u32(smem + kSmemBar);
   const uint32_t s_q = smem_u32(smem + kSmemQ);
   const uint32_t bar_zfull = s_bar, bar_zempty = s_bar + 8 * kNZ, bar_bfull = s_bar + 16 * kNZ,
-                 bar_bempty = s_bar + 16 * kNZ + 16, bar_tfull = s_bar + 16 * kNZ + 32, bar_tempty = s_bar + 16 * kNZ + 48;
-  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + kSmemBar + (2 * kNZ + 8) * 8);
+                 bar_bempty = s_bar + 16 * kNZ + 16, bar_tfull = s_bar + 16 * kNZ + 32, bar_tempty = bar_tfull + 8 * kNT;
+  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + kSmemBar + (2 * kNZ + 4 + 2 * kNT) * 8);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
@@ -73,10 +74,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   if (threadIdx.x == 0) {
     // zempty / tfull are arrived on by tcgen05.commit (the MMAs that read the stage / wrote the accumulators are done)
     for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + kNumProjWarps); }
-    for (int b = 0; b < 2; ++b) {
-      mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps);
-      mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, kNumProjWarps);
-    }
+    for (int b = 0; b < 2; ++b) { mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps); }
+    for (int b = 0; b < kNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, kNumProjWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   // W'' = B operand of the projection MMA, K-major, 128-byte swizzled by hand: row n < 16 = head n of
@@ -151,8 +150,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             umma_commit(bar_zempty + 8 * stage);
             umma_commit(bar_tfull + 8 * tb);
             if (++stage == kNZ) { stage = 0; phase ^= 1; }
-            tb ^= 1;
-            if (tb == 0) tphase ^= 1;
+            if (++tb == kNT) { tb = 0; tphase ^= 1; }
           }
         }
       }
@@ -212,8 +210,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(bar_tempty + 8 * tb);    // accumulators are in registers: buffer free
-          tb ^= 1;
-          if (tb == 0) tphase ^= 1;
+          if (++tb == kNT) { tb = 0; tphase ^= 1; }
           // LayerNorm statistics (fp32): mu = sum/c_z, var = sum z^2 / c_z - mu^2
           const float mu = zsum * (1.f / kCz);
           const float var = fmaxf(fmaf(zsq, 1.f / kCz, -mu * mu), 0.f);
