@@ -448,11 +448,9 @@ cudaError_t launch_fused_atom(const MmaParams& p, const void* z, int64_t ldz, cu
   if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
   const int64_t units = mma_num_units<aTileQ>(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
   if (units > 0x7fffffff) return cudaErrorInvalidValue;
-  static bool attr_set = false;
-  if (!attr_set) {
+  {   // per-device function attribute: set on every launch (cheap), so a process may use several GPUs
     cudaError_t e = cudaFuncSetAttribute(fused_atom_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aSmemAlloc);
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   int dev = 0, sms = 0;
   cudaGetDevice(&dev);

@@ -411,11 +411,9 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
 // ------------------------------------------------------------------ host side
 template <int C, int CP>
 cudaError_t launch_c(const CUtensorMap& tm, const MmaParams& p, int64_t units, cudaStream_t st) {
-  static bool attr_set = false;
-  if (!attr_set) {
+  {   // per-device function attribute: set on every launch (cheap), so a process may use several GPUs
     cudaError_t e = cudaFuncSetAttribute(fused_mma_kernel<C, CP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_alloc(CP));
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   int dev = 0, sms = 0;
   cudaGetDevice(&dev);

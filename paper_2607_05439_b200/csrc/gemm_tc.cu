@@ -2,14 +2,16 @@
 //   PAPER.md:77-81 (sec 3.2): Q^(p) = f_Q(S^(p)); "keys and values are projected from the full single-track S"
 //   BASELINE.json config 0:  out = W_o (sigmoid(s W_g) (.) softmax(...) V)
 // C_seg[M, N] = A[M, K] (bf16 row-major = K-major) x W_seg[K, N] (bf16 row-major = MN-major B operand), fp32
-// accumulation in tensor memory.  One 128 x 128 output tile per CTA, K streamed in 64-wide blocks through a 3-stage
-// TMA / mbarrier ring (128-byte swizzle); two CTAs per SM overlap one tile's epilogue with the other's main loop.
-//   warp 0   TMA producer: A box (64 k, 128 rows), W boxes (64 n, 64 k) x 2
-//   warp 1   tcgen05 issuer (one lane): 4 x tcgen05.mma kind::f16 (M = 128, N = 128, K = 16) per k-block
-//   warps 2-5 epilogue: tcgen05.ld (thread = row) -> bias / scale / sigmoid -> bf16 -> shared C tile -> coalesced
-//            global stores in the layout the fused kernel reads (gemm_mma.cu lists the output modes)
+// accumulation in tensor memory.  One 128 x TBN output tile per CTA (TBN = 128, or 64 when 128-wide tiles would not
+// give every SM two CTAs), K streamed in 64-wide blocks through a 3-stage TMA / mbarrier ring (128-byte swizzle);
+// two CTAs per SM overlap one tile's epilogue with the other's main loop.
+//   warp 0    TMA producer: A box (64 k, 128 rows), W boxes (64 n, 64 k) x TBN / 64
+//   warp 1    tcgen05 issuer (one lane): 4 x tcgen05.mma kind::f16 (M = 128, N = TBN, K = 16) per k-block
+//   warps 2-9 epilogue: tcgen05.ld (thread = row, two warps per TMEM lane quadrant) -> bias / scale / sigmoid -> bf16
+//             -> shared C tile -> coalesced global stores in the layout the fused kernel reads (gemm_mma.cu lists
+//             the output modes)
 // The launcher falls back to the mma.sync kernel (gemm_mma.cu) for shapes this tiling does not cover
-// (N % 128, K % 64, unaligned pitches).  Every output element is accumulated over k in one fixed order.
+// (N % 64, K % 64, unaligned pitches).  Every output element is accumulated over k in one fixed order.
 #include "kernels.h"
 #include "mma_ptx.cuh"
 
@@ -246,13 +248,11 @@ cudaError_t launch_gemm_tc(const GemmMmaParams& p, cudaStream_t st) {
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
   }
-  static bool attr_set = false;
-  if (!attr_set) {
+  {   // per-device function attribute: set on every launch (cheap), so a process may use several GPUs
     cudaError_t e = cudaFuncSetAttribute(gemm_tc_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TcCfg<128>::kSmemAlloc);
     if (e == cudaSuccess)
       e = cudaFuncSetAttribute(gemm_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TcCfg<64>::kSmemAlloc);
     if (e != cudaSuccess) return e;
-    attr_set = true;
   }
   const unsigned mt = (unsigned)((p.M + TBM - 1) / TBM);
   // 128-wide tiles when they give every SM two CTAs (or N does not split into 64s evenly enough to matter)
