@@ -57,3 +57,40 @@ def brute_force(s, z, w_q, w_k, w_v, w_g, w_b, w_o, gamma, beta, H, c, eps=1e-5,
                 gated[h * c + d] = g[i][h * c + d] * o
         out.append([sum(gated[e] * w_o[e][t] for e in range(D)) for t in range(len(w_o[0]))])
     return out
+
+
+def brute_force_sparse(a, p_slice, idx, w_q, w_k, w_v, w_g, w_b, w_o, gamma, beta, H, c, eps=1e-5):
+    """Sparse k-neighbour atom attention, same naive style: nested loops over Python
+    lists, `math.exp`.  a [L][c_atom], p_slice [L][k][c_atompair], idx [L][k] (negative = unused slot).
+    Pins `oracle/sparse_atom_attention.py` (tests/test_oracle_pins.py::test_sparse_brute_force)."""
+    L, c_s = len(a), len(a[0])
+    c_p = len(p_slice[0][0])
+    D = H * c
+
+    def proj(W, i, col):
+        return sum(a[i][t] * W[t][col] for t in range(c_s))
+
+    out = []
+    for l in range(L):
+        gated = [0.0] * D
+        slots = [j for j in range(len(idx[l])) if idx[l][j] >= 0]
+        for h in range(H):
+            if not slots:
+                continue
+            logit = []
+            for j in slots:
+                m = idx[l][j]
+                pp = p_slice[l][j]
+                mu = sum(pp) / c_p
+                var = sum((x - mu) ** 2 for x in pp) / c_p
+                bias = sum(((pp[t] - mu) / math.sqrt(var + eps) * gamma[t] + beta[t]) * w_b[t][h] for t in range(c_p))
+                dot = sum(proj(w_q, l, h * c + d) * proj(w_k, m, h * c + d) for d in range(c))
+                logit.append(dot / math.sqrt(c) + bias)
+            mx = max(logit)
+            ex = [math.exp(x - mx) for x in logit]
+            tot = sum(ex)
+            for d in range(c):
+                o = sum(ex[n] / tot * proj(w_v, idx[l][j], h * c + d) for n, j in enumerate(slots))
+                gated[h * c + d] = o / (1.0 + math.exp(-proj(w_g, l, h * c + d)))
+        out.append([sum(gated[e] * w_o[e][t] for e in range(D)) for t in range(len(w_o[0]))])
+    return out

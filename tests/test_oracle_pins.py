@@ -318,3 +318,69 @@ def test_input_generator_is_seed_deterministic():
     assert all(torch.equal(w1[k], w2[k]) for k in w1)
     cfg2 = syn.small_config("g", I=60 * 2, c_s=8, c_z=4, H=2, c=4, dtype="bf16", structured=True, seed=6)
     assert not torch.equal(z1, syn.make_z(cfg2, chunk_rows=16))
+
+
+# ---------------------------------------------------------------- sparse k-neighbour atom attention
+def _sparse_problem(rng, L, k, c_s=12, c_p=6, H=2, c=4):
+    from oracle import sparse_atom_attention as spo  # noqa: F401
+    a, P, w = rand_problem(rng, L, c_s, c_p, H, c)
+    idx = np.stack([rng.choice(L, size=k, replace=False) for _ in range(L)])
+    p_slice = np.stack([P[l, idx[l]] for l in range(L)])
+    return a, P, p_slice, idx, w
+
+
+def test_sparse_full_budget_equals_dense_oracle():
+    """idx[l] = a permutation of ALL atoms, p_slice the matching gather of a dense P  =>  the dense layer."""
+    from oracle import sparse_atom_attention as spo
+    rng = np.random.default_rng(41)
+    L, H, c = 17, 3, 4
+    a, P, p_slice, idx, w = _sparse_problem(rng, L, L, H=H, c=c)
+    dense = orc.pair_bias_attention(a, P, w, H, c)
+    sparse = spo.sparse_atom_attention(a, p_slice, idx, w, H, c)
+    assert np.max(np.abs(dense - sparse)) <= 1e-12 * max(1.0, np.max(np.abs(dense)))
+
+
+def test_sparse_brute_force():
+    from oracle import sparse_atom_attention as spo
+    rng = np.random.default_rng(42)
+    L, k, H, c = 7, 3, 2, 3
+    a, P, p_slice, idx, w = _sparse_problem(rng, L, k, c_s=5, c_p=4, H=H, c=c)
+    idx[2, 1] = -1                      # an unused slot
+    idx[4, :] = -1                      # an atom without neighbours: out = 0
+    idx[5, 2] = idx[5, 0]               # a neighbour listed twice counts twice
+    p_slice[5, 2] = p_slice[5, 0]
+    tl = lambda x: np.asarray(x).tolist()
+    ref = brute.brute_force_sparse(tl(a), tl(p_slice), tl(idx), tl(w["w_q"]), tl(w["w_k"]), tl(w["w_v"]), tl(w["w_g"]),
+                                   tl(w["w_b"]), tl(w["w_o"]), tl(w["ln_z_gamma"]), tl(w["ln_z_beta"]), H, c)
+    got = spo.sparse_atom_attention(a, p_slice, idx, w, H, c)
+    assert np.max(np.abs(got - np.asarray(ref))) <= 1e-12
+    assert np.all(got[4] == 0.0)
+
+
+def test_sparse_slot_permutation_and_masking():
+    from oracle import sparse_atom_attention as spo
+    rng = np.random.default_rng(43)
+    L, k, H, c = 11, 5, 2, 4
+    a, P, p_slice, idx, w = _sparse_problem(rng, L, k, H=H, c=c)
+    base = spo.sparse_atom_attention(a, p_slice, idx, w, H, c)
+    perm = rng.permutation(k)
+    assert np.max(np.abs(spo.sparse_atom_attention(a, p_slice[:, perm], idx[:, perm], w, H, c) - base)) <= 1e-13
+    # a masked slot == a shorter list (whatever the pair features stored in the masked slot)
+    idx2, p2 = idx.copy(), p_slice.copy()
+    idx2[:, 3] = -1
+    p2[:, 3] = 1e6
+    keep = [0, 1, 2, 4]
+    short = spo.sparse_atom_attention(a, p_slice[:, keep], idx[:, keep], w, H, c)
+    assert np.max(np.abs(spo.sparse_atom_attention(a, p2, idx2, w, H, c) - short)) <= 1e-13
+
+
+def test_sparse_single_neighbour_closed_form():
+    """k = 1: softmax over one slot is 1, so out_l = (sigmoid(a_l W_g) (.) a_m W_v) W_o with m = idx[l, 0]."""
+    from oracle import sparse_atom_attention as spo
+    rng = np.random.default_rng(44)
+    L, H, c = 9, 2, 3
+    a, P, p_slice, idx, w = _sparse_problem(rng, L, 1, H=H, c=c)
+    got = spo.sparse_atom_attention(a, p_slice, idx, w, H, c)
+    gate = 1.0 / (1.0 + np.exp(-(a @ w["w_g"])))
+    ref = (gate * (a[idx[:, 0]] @ w["w_v"])) @ w["w_o"]
+    assert np.max(np.abs(got - ref)) <= 1e-12
