@@ -193,3 +193,62 @@ def sample_rows(I: int, count: int, boundaries=(), seed: int = 0):
     while len(rows) < min(count, I):
         rows.add(int(torch.randint(0, I, (1,), generator=g)))
     return sorted(rows)
+
+
+# ------------------------------------------------------------------ sparse k-neighbour atom attention
+def make_atom_coords(cfg: LayerConfig, device="cpu") -> torch.Tensor:
+    """Synthetic atom coordinates [L, 3] (fp32) of an icosahedral-shaped assembly: one ASU chain drawn as a
+    self-avoiding-ish random walk (1.5 A steps), copied `copies` times with seeded random rotations and centres on
+    a sphere whose radius keeps neighbouring copies in contact.  Input recipe only (stands in for the noised
+    coordinates X^(t) of PAPER.md:303); nothing of the method's arithmetic."""
+    g = _gen(cfg.seed * 1000003 + 5, "cpu")
+    n = cfg.n_res if cfg.structured else cfg.I
+    copies = cfg.copies if cfg.structured else 1
+    steps = torch.randn(n, 3, generator=g, dtype=torch.float32)
+    steps = 1.5 * steps / steps.norm(dim=1, keepdim=True)
+    asu = torch.cumsum(steps, dim=0)
+    asu = asu - asu.mean(dim=0, keepdim=True)
+    rad = float(asu.norm(dim=1).max())
+    out = []
+    for _ in range(copies):
+        qm, _r = torch.linalg.qr(torch.randn(3, 3, generator=g, dtype=torch.float32))
+        ctr = torch.randn(3, generator=g, dtype=torch.float32)
+        ctr = ctr / ctr.norm() * (rad * math.sqrt(copies) / 2.0 if copies > 1 else 0.0)
+        out.append(asu @ qm.T + ctr)
+    return torch.cat(out, dim=0).to(device).contiguous()
+
+
+def make_knn_idx(cfg: LayerConfig, k: int, device="cpu", chunk: int = 2048) -> torch.Tensor:
+    """Neighbour lists idx [L, k] int32: the k spatially closest atoms of each query atom (itself included), from
+    make_atom_coords by a chunked distance matrix + top-k.  Stands in for the paper's budget of sequence-local plus
+    spatially closest atoms; k = min(k, L)."""
+    x = make_atom_coords(cfg, device)
+    L = x.shape[0]
+    k = min(k, L)
+    idx = torch.empty(L, k, dtype=torch.int32, device=device)
+    for i0 in range(0, L, chunk):
+        d = torch.cdist(x[i0:i0 + chunk], x)
+        idx[i0:i0 + chunk] = torch.topk(d, k, dim=1, largest=False).indices.to(torch.int32)
+    return idx.contiguous()
+
+
+def make_p_slice(cfg: LayerConfig, idx: torch.Tensor, device="cpu", noise: float = 0.1, chunk: int = 4096) -> torch.Tensor:
+    """Pair features of the listed neighbours, p_slice[l, j] = P[l, idx[l, j]] with the same recipe as the dense
+    pair tensor (E[copy, copy] + R[atom, atom] + 0.1 N(0, 1)), built directly in slice form [L, k, c_z]."""
+    L, k = idx.shape
+    out = torch.empty(L, k, cfg.c_z, dtype=torch_dtype(cfg.dtype), device=device)
+    if not cfg.structured:
+        g = _gen(cfg.seed * 1000003 + 6, device)
+        out.copy_(torch.randn(L, k, cfg.c_z, generator=g, device=device, dtype=torch.float32))
+        return out
+    n = cfg.n_res
+    E, R = _tables(cfg, device)
+    for r, i0 in enumerate(range(0, L, chunk)):
+        i1 = min(L, i0 + chunk)
+        rows = torch.arange(i0, i1, device=device)
+        m = idx[i0:i1].long().clamp(min=0)
+        blk = E[(rows // n)[:, None], m // n] + R[(rows % n)[:, None], m % n]
+        g = _gen(cfg.seed * 1000003 + 2000 + r, device)
+        blk += noise * torch.randn(i1 - i0, k, cfg.c_z, generator=g, device=device, dtype=torch.float32)
+        out[i0:i1] = blk.to(out.dtype)
+    return out

@@ -100,6 +100,21 @@ dcp_status dcp_atom_pair_bias_attention(const void *a, const void *p, int64_t ld
                                         dcp_dtype dtype, dcp_decomp decomp, const dcp_plan *plan,
                                         void *workspace, size_t workspace_bytes, void *stream);
 
+/* Sparse k-neighbour atom-level attention ("each query atom attends to a budget of k neighbours ... The
+ * relevant slice of P is gathered at those k indices and then projected to the per-head bias"; :303 the block
+ * consumes a [L, k, c_atompair] slice, k = n_attn-keys, default 128; :456 K/V/B entries gathered at the indices).
+ * For query atom l: keys m = idx[l, j] (j < k), logit_j^h = q_l^h.k_m^h/sqrt(c) + LN(p_slice[l, j, :]).W_b[:, h],
+ * softmax over the VALID slots, out_l = (sigmoid(a_l W_g) (.) sum_j a_j v_m) W_o.
+ *   a [L, c_atom], p_slice [L, k, c_atompair], out [L, c_atom]: device, storage dtype, row-major, 16-byte aligned;
+ *   idx [L, k]: device int32; idx < 0 marks an unused slot (an atom without valid slots gets out = 0); a neighbour
+ *   listed twice counts twice; indices >= L are undefined behaviour.
+ * Instantiated for DCP_BF16, c = 32, c_atompair = 16, H <= 16, k <= 512, c_atom % 8 == 0 (DCP_ERR_UNSUPPORTED
+ * otherwise).  workspace >= dcp_sparse_atom_workspace_bytes(...), 256-byte aligned.  Enqueues on `stream`. */
+dcp_status dcp_sparse_atom_workspace_bytes(int64_t L, int c_atom, int H, int c, dcp_dtype dtype, size_t *bytes);
+dcp_status dcp_sparse_atom_attention(const void *a, const void *p_slice, const int32_t *idx, const dcp_weights *w,
+                                     void *out, int64_t L, int k, int c_atom, int H, int c, int c_atompair,
+                                     dcp_dtype dtype, void *workspace, size_t workspace_bytes, void *stream);
+
 /* End-to-end entry with HOST inputs/outputs: s_host, z_host, out_host are HOST pointers (pinned memory gives
  * full PCIe rate); weights stay device-resident (they are parameters, not per-step inputs).  Copies s and z
  * to the device staging buffers s_dev [I,c_s], z_dev [I,I,c_z], runs the layer, copies out back, all on

@@ -27,6 +27,7 @@ KERNEL = {"auto": DCP_KERNEL_AUTO, "generic": DCP_KERNEL_GENERIC, "mma": DCP_KER
 EXPORTS = [
     "dcp_workspace_bytes", "dcp_pair_bias_attention", "dcp_atom_pair_bias_attention",
     "dcp_pair_bias_attention_host", "dcp_partial_states", "dcp_merge_states", "dcp_shard_range",
+    "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention",
     "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
     "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
 ]
@@ -79,7 +80,10 @@ def _load() -> C.CDLL:
     lib.dcp_status_string.argtypes = [i32]
     lib.dcp_status_string.restype = C.c_char_p
     lib.dcp_version.restype = i32
-    for n in EXPORTS[:7]:
+    lib.dcp_sparse_atom_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, C.POINTER(sz)]
+    lib.dcp_sparse_atom_attention.argtypes = [vp, vp, vp, C.POINTER(dcp_weights), vp, i64, i32, i32, i32, i32, i32, i32,
+                                              vp, sz, vp]
+    for n in EXPORTS[:9]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -213,6 +217,32 @@ def dcp_pair_bias_attention(s, z, w, H, c, decomp="monolithic", parts=1, key_spl
 def dcp_atom_pair_bias_attention(a, p, w, H, c, **kw):
     """Atom-level dense variant (BASELINE.json config 4): (L, c_atom, c_atompair) for (I, c_s, c_z)."""
     return dcp_pair_bias_attention(a, p, w, H, c, atom=True, **kw)
+
+
+def dcp_sparse_atom_workspace_bytes(L, c_atom, H, c, dtype: torch.dtype) -> int:
+    n = C.c_size_t(0)
+    _check(_lib.dcp_sparse_atom_workspace_bytes(int(L), int(c_atom), int(H), int(c), _dtype_code(dtype), C.byref(n)),
+           "dcp_sparse_atom_workspace_bytes")
+    return int(n.value)
+
+
+def dcp_sparse_atom_attention(a, p_slice, idx, w, H, c, eps=1e-5, out=None, workspace=None, stream=None):
+    """Sparse k-neighbour atom attention: a [L, c_atom], p_slice [L, k, c_atompair],
+    idx [L, k] int32 (negative = unused slot) -> out [L, c_atom]."""
+    assert a.is_cuda and p_slice.is_cuda and idx.is_cuda and a.is_contiguous() and p_slice.is_contiguous()
+    assert idx.dtype == torch.int32 and idx.is_contiguous() and p_slice.dtype == a.dtype
+    L, c_atom = a.shape
+    k, c_p = p_slice.shape[1], p_slice.shape[2]
+    assert tuple(idx.shape) == (L, k) and p_slice.shape[0] == L
+    if out is None:
+        out = torch.empty(L, c_atom, dtype=a.dtype, device=a.device)
+    if workspace is None:
+        workspace = _alloc_ws(dcp_sparse_atom_workspace_bytes(L, c_atom, H, c, a.dtype), a.device)
+    ws = _weights_struct(w, eps)
+    st = _lib.dcp_sparse_atom_attention(_ptr(a), _ptr(p_slice), _ptr(idx), C.byref(ws), _ptr(out), L, k, c_atom, H, c, c_p,
+                                        _dtype_code(a.dtype), _ptr(workspace), workspace.numel(), _stream_ptr(stream))
+    _check(st, "dcp_sparse_atom_attention")
+    return out
 
 
 def dcp_pair_bias_attention_host(s_host, z_host, w, H, c, out_host, s_dev, z_dev, out_dev, workspace,

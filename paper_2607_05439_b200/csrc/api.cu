@@ -363,6 +363,73 @@ dcp_status dcp_atom_pair_bias_attention(const void* a, const void* p, int64_t ld
   return layer(a, p, ldp, w, out, L, c_atom, H, c, c_atompair, dtype, decomp, plan, workspace, workspace_bytes, stream);
 }
 
+// ---- sparse k-neighbour atom attention
+namespace {
+struct SparseCarve { size_t q, k, v, g, gated, s_ln, wfold, c1, c0, total; };
+SparseCarve sparse_carve(int64_t L, int c_atom, int H, int c) {
+  SparseCarve w{};
+  const size_t D = (size_t)H * c;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+  w.q = take((size_t)L * D * 2); w.k = take((size_t)L * D * 2); w.v = take((size_t)L * D * 2);
+  w.g = take((size_t)L * D * 2); w.gated = take((size_t)L * D * 2);
+  w.s_ln = take((size_t)L * c_atom * 2);
+  w.wfold = take(16 * 16 * 2); w.c1 = take(16 * sizeof(float)); w.c0 = take(16 * sizeof(float));
+  w.total = off;
+  return w;
+}
+}  // namespace
+
+dcp_status dcp_sparse_atom_workspace_bytes(int64_t L, int c_atom, int H, int c, dcp_dtype dtype, size_t* bytes) {
+  if (!bytes || L <= 0 || c_atom <= 0 || H <= 0 || c <= 0) return DCP_ERR_INVALID_ARG;
+  if (dtype != DCP_BF16) return DCP_ERR_UNSUPPORTED;
+  *bytes = sparse_carve(L, c_atom, H, c).total;
+  return DCP_OK;
+}
+
+dcp_status dcp_sparse_atom_attention(const void* a, const void* p_slice, const int32_t* idx, const dcp_weights* w,
+                                     void* out, int64_t L, int k, int c_atom, int H, int c, int c_atompair,
+                                     dcp_dtype dtype, void* workspace, size_t workspace_bytes, void* stream) {
+  g_launches = 0;
+  if (!a || !p_slice || !idx || !out || !workspace) return DCP_ERR_INVALID_ARG;
+  if (!w || !w->w_q || !w->w_k || !w->w_v || !w->w_g || !w->w_b || !w->w_o || !w->ln_z_gamma || !w->ln_z_beta)
+    return DCP_ERR_INVALID_ARG;
+  if ((w->ln_s_gamma == nullptr) != (w->ln_s_beta == nullptr)) return DCP_ERR_INVALID_ARG;
+  if (L <= 0 || k <= 0 || c_atom <= 0 || H <= 0 || c <= 0 || c_atompair <= 0 || L > 0x7fffffff) return DCP_ERR_INVALID_ARG;
+  if (dtype != DCP_BF16 || !sparse_atom_supports(dtype, H, c, c_atompair, k) || c_atom % 8 != 0) return DCP_ERR_UNSUPPORTED;
+  if ((((uintptr_t)a | (uintptr_t)p_slice | (uintptr_t)out | (uintptr_t)workspace) & 15) != 0) return DCP_ERR_INVALID_ARG;
+  const SparseCarve cv = sparse_carve(L, c_atom, H, c);
+  if (workspace_bytes < cv.total) return DCP_ERR_WORKSPACE;
+  char* ws = (char*)workspace;
+  cudaStream_t st = (cudaStream_t)stream;
+  const float eps = w->ln_eps > 0.f ? w->ln_eps : 1e-5f;
+  const int D = H * c;
+  const void* x = a;
+  if (w->ln_s_gamma != nullptr) {
+    DCP_CUDA(launch_layernorm_rows_bf16(a, w->ln_s_gamma, w->ln_s_beta, ws + cv.s_ln, L, c_atom, eps, st));
+    x = ws + cv.s_ln;
+  }
+  GemmMmaParams gp{};
+  gp.A = x; gp.lda = c_atom; gp.M = L; gp.N = D; gp.K = c_atom; gp.nseg = 4;
+  gp.W[0] = w->w_q; gp.W[1] = w->w_k; gp.W[2] = w->w_v; gp.W[3] = w->w_g;
+  gp.bias[0] = w->b_q;
+  gp.C[0] = ws + cv.q; gp.C[1] = ws + cv.k; gp.C[2] = ws + cv.v; gp.C[3] = ws + cv.g;
+  gp.mode[0] = GEMM_OUT_HEADPAD; gp.mode[1] = GEMM_OUT_PLAIN; gp.mode[2] = GEMM_OUT_PLAIN; gp.mode[3] = GEMM_OUT_SIGMOID;
+  gp.scale[0] = 1.4426950408889634f / sqrtf((float)c);   // exp2-domain softmax
+  gp.ldc[1] = D; gp.ldc[2] = D; gp.ldc[3] = D;
+  gp.H = H; gp.c = c; gp.cp = c;
+  DCP_CUDA(launch_gemm_mma(gp, st));
+  DCP_CUDA(launch_fold_ln_z_mma(w->w_b, w->ln_z_gamma, w->ln_z_beta, ws + cv.wfold, (float*)(ws + cv.c1),
+                                (float*)(ws + cv.c0), c_atompair, H, 16, st));
+  DCP_CUDA(launch_sparse_atom(ws + cv.q, ws + cv.k, ws + cv.v, ws + cv.g, p_slice, idx, ws + cv.wfold,
+                              (const float*)(ws + cv.c1), (const float*)(ws + cv.c0), ws + cv.gated, L, k, H, eps, st));
+  GemmMmaParams go{};
+  go.A = ws + cv.gated; go.lda = D; go.M = L; go.N = c_atom; go.K = D; go.nseg = 1;
+  go.W[0] = w->w_o; go.C[0] = out; go.mode[0] = GEMM_OUT_PLAIN; go.ldc[0] = c_atom;
+  DCP_CUDA(launch_gemm_mma(go, st));
+  return DCP_OK;
+}
+
 dcp_status dcp_pair_bias_attention_host(const void* s_host, const void* z_host, const dcp_weights* w, void* out_host,
                                         void* s_dev, void* z_dev, void* out_dev, int64_t I, int c_s, int H, int c,
                                         int c_z, dcp_dtype dtype, dcp_decomp decomp, const dcp_plan* plan,

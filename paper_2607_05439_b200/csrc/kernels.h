@@ -82,6 +82,13 @@ cudaError_t launch_fused_atom(const MmaParams& p, const void* z, int64_t ldz, cu
 bool fused_atom_supports(dcp_dtype dt, int H, int c, int c_z);
 int fused_atom_tile_q();
 
+// Sparse k-neighbour atom attention (sparse_atom.cu): q, k, v, g [L][H*32] bf16 from the prologue
+// GEMM, p_slice [L][kn][16], idx [L][kn] (negative = unused slot) -> gated [L][H*32]
+bool sparse_atom_supports(dcp_dtype dt, int H, int c, int c_z, int kn);
+cudaError_t launch_sparse_atom(const void* q, const void* k, const void* v, const void* g, const void* p_slice,
+                               const int32_t* idx, const void* wfold, const float* c1, const float* c0, void* gated,
+                               int64_t L, int kn, int H, float eps, cudaStream_t st);
+
 // Merge (step a8) + normalise + gate (first half of a9); or raw merged state out.
 cudaError_t launch_merge(dcp_dtype dt, const MergeParams& p, cudaStream_t st);
 
