@@ -46,7 +46,9 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4"])
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4"],
+                    help="C0..C4: BASELINE.json configs (dense layer); S4: sparse k-neighbour atom attention on C4's atoms")
+    ap.add_argument("--neighbours", type=int, default=128, help="S4: budget k (PAPER.md:303 default 128)")
     ap.add_argument("--decomp", default="monolithic", choices=["monolithic", "row", "grid"])
     ap.add_argument("--parts", type=int, default=0, help="row stripes / grid cells (0: 8 rows, 16 grid)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "mma"])
@@ -152,6 +154,9 @@ def run_reference(args, rank, world):
         return
     import torch
     import dcp_synth as syn
+    if args.workload == "S4":
+        run_reference_sparse(args)
+        return
     cfg = syn.CONFIGS[args.workload]
     dev = "cuda:0" if torch.cuda.is_available() else "cpu"
     # generate on the GPU when there is one (z of 2.3 GB), else on the CPU for small workloads
@@ -271,6 +276,164 @@ def aggregate_gpairs(I, steps, world, ms):
     return float(I) * I * steps * world / (ms * 1e-3) / 1e9
 
 
+def run_reference_sparse(args):
+    """--impl reference --workload S4: the sparse fp64 oracle on sampled query atoms of the same inputs."""
+    import torch
+    import dcp_synth as syn
+    from oracle import sparse_atom_attention as spo
+    cfg = syn.CONFIGS["C4"]
+    dev = "cuda:0" if torch.cuda.is_available() else "cpu"
+    k = args.neighbours
+    w = syn.make_weights(cfg, dev)
+    a = syn.make_s(cfg, dev)
+    idx = syn.make_knn_idx(cfg, k, dev)
+    p = syn.make_p_slice(cfg, idx, dev)
+    f64 = lambda t: t.detach().float().cpu().double().numpy()
+    a64, w64 = f64(a), {kk: f64(v) for kk, v in w.items()}
+    n_rows = args.cpu_rows or cfg.I
+    pairs = secs = 0.0
+    for step in range(args.steps + min(args.warmup, 1)):
+        rows = syn.sample_rows(cfg.I, n_rows, seed=step)
+        r = torch.as_tensor(rows, device=dev)
+        p_rows, i_rows = p.index_select(0, r).float().cpu().numpy(), idx.index_select(0, r).cpu().numpy()
+        t0 = time.perf_counter()
+        spo.sparse_atom_attention_rows(a64, p_rows, i_rows, rows, w64, cfg.H, cfg.c)
+        if step >= min(args.warmup, 1):
+            secs += time.perf_counter() - t0
+            pairs += len(rows) * k
+    value = pairs / secs / 1e9
+    sample = f"{n_rows} sampled query atoms x {k} neighbours per step ({args.steps} steps), fp64 numpy oracle"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": secs / max(args.steps, 1) * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"S4: sparse k-neighbour atom attention L={cfg.I} k={k}", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}), flush=True)
+
+
+def run_sparse(args, rank, world, local_rank):
+    """--workload S4: sparse k-neighbour atom attention on C4's atoms (L = 24000, c_atom = 128,
+    c_atompair = 16, H = 4, c = 32), budget k = --neighbours.  One pair = one (query atom, neighbour slot)."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as ge
+    if rank == 0 or world == 1:
+        ge.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    import dcp_synth as syn
+    import paper_2607_05439_b200 as dcp
+    from oracle import sparse_atom_attention as spo
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    cfg = replica_config(syn.CONFIGS["C4"], rank, world)
+    k = args.neighbours
+    w = syn.make_weights(cfg, dev)
+    a = syn.make_s(cfg, dev)
+    idx = syn.make_knn_idx(cfg, k, dev)
+    p = syn.make_p_slice(cfg, idx, dev)
+    L = cfg.I
+    ws = torch.empty(dcp.dcp_sparse_atom_workspace_bytes(L, cfg.c_s, cfg.H, cfg.c, a.dtype), dtype=torch.uint8, device=dev)
+    out = torch.empty(L, cfg.c_s, dtype=a.dtype, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # inputs (115 MB) fit L2: flush between steps
+
+    def step(ev=None):
+        dcp.dcp_sparse_atom_attention(a, p, idx, w, cfg.H, cfg.c, out=out, workspace=ws, fused_events=ev)
+
+    for _ in range(max(args.warmup, 3)):
+        flush.zero_()
+        step()
+    launches = dcp.dcp_last_launch_count()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    total_ms, fused_ms = 0.0, []
+    for _ in range(args.steps):
+        flush.zero_()
+        e0, e1, f0, f1 = dcp.Event(), dcp.Event(), dcp.Event(), dcp.Event()
+        torch.cuda.synchronize()
+        e0.record()
+        step((f0, f1))
+        e1.record()
+        torch.cuda.synchronize()
+        total_ms += e0.elapsed_ms(e1)
+        fused_ms.append(f0.elapsed_ms(f1))
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = max_over_ranks_ms(total_ms, world, dev)
+    pairs = float(L) * k
+    value = pairs * args.steps * world / (total_ms * 1e-3) / 1e9
+    kms = sum(fused_ms) / len(fused_ms)
+    # the gather kernel's bytes: every slot reads a 64-byte K slice and a 64-byte V slice per head (from L2: K and V
+    # are 12 MB), its 32-byte p row and its index; bound = L2 -> SM gather, reported against the HBM copy peak
+    peak, peak_how = measured_peaks()
+    gather_bytes = pairs * (2 * cfg.H * cfg.c * 2 + cfg.c_z * 2 + 4)
+    hbm_bytes = pairs * (cfg.c_z * 2 + 4) + 5 * L * cfg.D * 2
+    roofline = {"bound": "hbm", "achieved": hbm_bytes / (kms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                "frac": hbm_bytes / (kms * 1e-3) / 1e9 / peak, "traffic": None, "kernel": "sparse_atom_kernel",
+                "peak_source": peak_how, "kernel_ms": kms, "kernel_share_of_step": kms * args.steps / total_ms,
+                "algorithmic_bytes_per_launch": hbm_bytes,
+                "l2_gather_bytes_per_launch": gather_bytes, "l2_gather_gbs": gather_bytes / (kms * 1e-3) / 1e9,
+                "note": "K / V rows are gathered from L2 (12 MB resident): the compulsory HBM bytes are p_slice + idx + "
+                        "q, k, v, g, gated; the kernel is L2-gather / issue bound, see DESIGN.md"}
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        rows = syn.sample_rows(L, args.cpu_rows or L, seed=0)     # every atom: ~2 s of oracle time
+        r = torch.as_tensor(rows, device=dev)
+        f64 = lambda t: t.detach().float().cpu().double().numpy()
+        a64, w64 = f64(a), {kk: f64(v) for kk, v in w.items()}
+        p_rows, i_rows = p.index_select(0, r).float().cpu().numpy(), idx.index_select(0, r).cpu().numpy()
+        t0 = time.perf_counter()
+        ref = spo.sparse_atom_attention_rows(a64, p_rows, i_rows, rows, w64, cfg.H, cfg.c)
+        dt = time.perf_counter() - t0
+        got = f64(out.index_select(0, r))
+        cpu = {"value": len(rows) * k / dt / 1e9, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+               "sample": f"{len(rows)} sampled query atoms x {k} neighbours ({dt:.1f} s incl. the single-track projections "
+                         "of all atoms), fp64 numpy oracle",
+               "gpu_vs_oracle_rel_l2_on_sample": float(np.linalg.norm(got - ref) / np.linalg.norm(ref)),
+               "gpu_vs_oracle_max_abs_on_sample": float(np.abs(got - ref).max())}
+    e2e = None
+    if not args.no_e2e:
+        # host (pinned) a, p_slice, idx -> device, the layer, out -> host, per step
+        ah, ph, ih = a.cpu().pin_memory(), p.cpu().pin_memory(), idx.cpu().pin_memory()
+        oh = torch.empty(out.shape, dtype=out.dtype).pin_memory()
+        a_d, p_d, i_d = torch.empty_like(a), torch.empty_like(p), torch.empty_like(idx)
+        ne = max(1, args.e2e_steps)
+        e0, e1 = dcp.Event(), dcp.Event()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(ne):
+            a_d.copy_(ah, non_blocking=True); p_d.copy_(ph, non_blocking=True); i_d.copy_(ih, non_blocking=True)
+            dcp.dcp_sparse_atom_attention(a_d, p_d, i_d, w, cfg.H, cfg.c, out=out, workspace=ws)
+            oh.copy_(out, non_blocking=True)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = max_over_ranks_ms(e0.elapsed_ms(e1), world, dev)
+        e2e = {"value": pairs * ne * world / (ms * 1e-3) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": ah.numel() * 2 + ph.numel() * 2 + ih.numel() * 4, "d2h_bytes_per_step": oh.numel() * 2,
+               "steps": ne}
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "bf16", "data": "synthetic",
+                "config": {"workload": f"S4: sparse k-neighbour atom attention L={L} k={k} c_atom={cfg.c_s} c_atompair={cfg.c_z} "
+                                       f"H={cfg.H} c={cfg.c} bf16 (icosahedral 60 x {cfg.n_res}, kNN of synthetic coordinates)",
+                           "pair": "one (query atom, neighbour slot)", "kernel": "sparse_atom_kernel",
+                           "l2": "L2 flushed between steps by writing a 256 MiB buffer",
+                           "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "peak_device_bytes": int(torch.cuda.max_memory_allocated())},
+                "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches * (args.steps + max(args.warmup, 3)),
+                "clocks": clocks}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def workload_name(cfg):
     kind = "atom-level" if cfg.name == "C4" else "token-level"
     return (f"{cfg.name}: {kind} pair-bias attention I={cfg.I} c_s={cfg.c_s} c_z={cfg.c_z} H={cfg.H} c={cfg.c} "
@@ -289,6 +452,9 @@ def main():
     if args.ceiling:
         if rank == 0:
             run_ceiling(args)
+        return
+    if args.workload == "S4":
+        run_sparse(args, rank, world, local_rank)
         return
 
     import torch

@@ -109,11 +109,13 @@ dcp_status dcp_atom_pair_bias_attention(const void *a, const void *p, int64_t ld
  *   idx [L, k]: device int32; idx < 0 marks an unused slot (an atom without valid slots gets out = 0); a neighbour
  *   listed twice counts twice; indices >= L are undefined behaviour.
  * Instantiated for DCP_BF16, c = 32, c_atompair = 16, H <= 16, k <= 512, c_atom % 8 == 0 (DCP_ERR_UNSUPPORTED
- * otherwise).  workspace >= dcp_sparse_atom_workspace_bytes(...), 256-byte aligned.  Enqueues on `stream`. */
+ * otherwise).  workspace >= dcp_sparse_atom_workspace_bytes(...), 256-byte aligned.  Enqueues on `stream`.
+ * `plan` may be NULL; only its ev_fused_begin / ev_fused_end (recorded around the gather kernel) are used. */
 dcp_status dcp_sparse_atom_workspace_bytes(int64_t L, int c_atom, int H, int c, dcp_dtype dtype, size_t *bytes);
 dcp_status dcp_sparse_atom_attention(const void *a, const void *p_slice, const int32_t *idx, const dcp_weights *w,
                                      void *out, int64_t L, int k, int c_atom, int H, int c, int c_atompair,
-                                     dcp_dtype dtype, void *workspace, size_t workspace_bytes, void *stream);
+                                     dcp_dtype dtype, const dcp_plan *plan, void *workspace, size_t workspace_bytes,
+                                     void *stream);
 
 /* End-to-end entry with HOST inputs/outputs: s_host, z_host, out_host are HOST pointers (pinned memory gives
  * full PCIe rate); weights stay device-resident (they are parameters, not per-step inputs).  Copies s and z

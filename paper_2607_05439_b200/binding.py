@@ -82,7 +82,7 @@ def _load() -> C.CDLL:
     lib.dcp_version.restype = i32
     lib.dcp_sparse_atom_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, C.POINTER(sz)]
     lib.dcp_sparse_atom_attention.argtypes = [vp, vp, vp, C.POINTER(dcp_weights), vp, i64, i32, i32, i32, i32, i32, i32,
-                                              vp, sz, vp]
+                                              C.POINTER(dcp_plan), vp, sz, vp]
     for n in EXPORTS[:9]:
         getattr(lib, n).restype = i32
     return lib
@@ -226,7 +226,8 @@ def dcp_sparse_atom_workspace_bytes(L, c_atom, H, c, dtype: torch.dtype) -> int:
     return int(n.value)
 
 
-def dcp_sparse_atom_attention(a, p_slice, idx, w, H, c, eps=1e-5, out=None, workspace=None, stream=None):
+def dcp_sparse_atom_attention(a, p_slice, idx, w, H, c, eps=1e-5, out=None, workspace=None, stream=None,
+                              fused_events=None):
     """Sparse k-neighbour atom attention: a [L, c_atom], p_slice [L, k, c_atompair],
     idx [L, k] int32 (negative = unused slot) -> out [L, c_atom]."""
     assert a.is_cuda and p_slice.is_cuda and idx.is_cuda and a.is_contiguous() and p_slice.is_contiguous()
@@ -239,8 +240,10 @@ def dcp_sparse_atom_attention(a, p_slice, idx, w, H, c, eps=1e-5, out=None, work
     if workspace is None:
         workspace = _alloc_ws(dcp_sparse_atom_workspace_bytes(L, c_atom, H, c, a.dtype), a.device)
     ws = _weights_struct(w, eps)
+    pl = _plan(1, 1, "auto", None if fused_events is None else (fused_events[0].handle, fused_events[1].handle))
     st = _lib.dcp_sparse_atom_attention(_ptr(a), _ptr(p_slice), _ptr(idx), C.byref(ws), _ptr(out), L, k, c_atom, H, c, c_p,
-                                        _dtype_code(a.dtype), _ptr(workspace), workspace.numel(), _stream_ptr(stream))
+                                        _dtype_code(a.dtype), C.byref(pl), _ptr(workspace), workspace.numel(),
+                                        _stream_ptr(stream))
     _check(st, "dcp_sparse_atom_attention")
     return out
 

@@ -389,7 +389,8 @@ dcp_status dcp_sparse_atom_workspace_bytes(int64_t L, int c_atom, int H, int c, 
 
 dcp_status dcp_sparse_atom_attention(const void* a, const void* p_slice, const int32_t* idx, const dcp_weights* w,
                                      void* out, int64_t L, int k, int c_atom, int H, int c, int c_atompair,
-                                     dcp_dtype dtype, void* workspace, size_t workspace_bytes, void* stream) {
+                                     dcp_dtype dtype, const dcp_plan* plan, void* workspace, size_t workspace_bytes,
+                                     void* stream) {
   g_launches = 0;
   if (!a || !p_slice || !idx || !out || !workspace) return DCP_ERR_INVALID_ARG;
   if (!w || !w->w_q || !w->w_k || !w->w_v || !w->w_g || !w->w_b || !w->w_o || !w->ln_z_gamma || !w->ln_z_beta)
@@ -421,8 +422,10 @@ dcp_status dcp_sparse_atom_attention(const void* a, const void* p_slice, const i
   DCP_CUDA(launch_gemm_mma(gp, st));
   DCP_CUDA(launch_fold_ln_z_mma(w->w_b, w->ln_z_gamma, w->ln_z_beta, ws + cv.wfold, (float*)(ws + cv.c1),
                                 (float*)(ws + cv.c0), c_atompair, H, 16, st));
+  if (plan && plan->ev_fused_begin && cudaEventRecord((cudaEvent_t)plan->ev_fused_begin, st) != cudaSuccess) return DCP_ERR_CUDA;
   DCP_CUDA(launch_sparse_atom(ws + cv.q, ws + cv.k, ws + cv.v, ws + cv.g, p_slice, idx, ws + cv.wfold,
                               (const float*)(ws + cv.c1), (const float*)(ws + cv.c0), ws + cv.gated, L, k, H, eps, st));
+  if (plan && plan->ev_fused_end && cudaEventRecord((cudaEvent_t)plan->ev_fused_end, st) != cudaSuccess) return DCP_ERR_CUDA;
   GemmMmaParams go{};
   go.A = ws + cv.gated; go.lda = D; go.M = L; go.N = c_atom; go.K = D; go.nseg = 1;
   go.W[0] = w->w_o; go.C[0] = out; go.mode[0] = GEMM_OUT_PLAIN; go.ldc[0] = c_atom;

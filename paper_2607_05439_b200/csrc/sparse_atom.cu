@@ -166,6 +166,153 @@ __global__ void __launch_bounds__(128) sparse_atom_kernel(const SparseParams p) 
   out[lane] = __float2bfloat16_rn(gate * (acc[0] / lsum));
 }
 
+// ---- row-coalesced variant for H in {2, 4, 8}: one warp per atom, ALL heads.  A K / V row of the atom's neighbour is
+// H * 64 bytes; LPR = 4 H lanes read it as 16-byte chunks (lane chunk ch -> head ch / 4, head dims 8 (ch % 4) .. + 7), so
+// one warp-level load covers 32 / LPR whole rows = a few fully used 128-byte lines.  The slot-per-lane kernel above
+// touches 32 different lines per load instruction and is bound by L1 tag throughput (one wavefront per line); this one
+// needs ~8x fewer wavefronts.  Per warp: (A) lane = slot: bias of all heads from the p row -> shared logits[slot][h];
+// (B) QK^T row by row, 4-lane shuffle reduction per head, added to the logits; (C) softmax statistics over the slots;
+// (D) acc += P v row by row, the partial sums of the 32 / LPR row groups combined by shuffles at the end.
+template <int H>
+__global__ void __launch_bounds__(128) sparse_atom_rows_kernel(const SparseParams p) {
+  constexpr int LPR = 4 * H;            // lanes per K / V row
+  constexpr int RPL = 32 / LPR;         // rows per warp-level load
+  constexpr int D = H * sC;
+  extern __shared__ float smem_f[];
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int kpad = (p.kn + 31) & ~31;
+  float* s_logit = smem_f + (size_t)wib * kpad * (H + 1);          // [kpad][H]
+  int* s_idx = reinterpret_cast<int*>(s_logit + (size_t)kpad * H);  // [kpad]
+  const int64_t l = (int64_t)blockIdx.x * 4 + wib;
+  if (l >= p.L) return;
+  const int ch = lane % LPR, grp = lane / LPR, hd = ch >> 2;        // chunk of the row, row group, head of the chunk
+  const uint4 qv = __ldg(reinterpret_cast<const uint4*>(p.q + l * D) + ch);
+  const uint32_t ones = 0x3f803f80u;
+
+  // ---- (A) lane = slot: neighbour index, LayerNorm statistics of the p row, bias of every head
+  for (int j0 = 0; j0 < kpad; j0 += 32) {
+    const int j = j0 + lane;
+    const int m = j < p.kn ? __ldg(p.idx + l * p.kn + j) : -1;
+    s_idx[j] = m;
+    if (m >= 0) {
+      const uint4* pr = reinterpret_cast<const uint4*>(p.p + (l * p.kn + j) * sCz);
+      const uint4 p0 = __ldg(pr), p1 = __ldg(pr + 1);
+      const uint32_t pw_[8] = {p0.x, p0.y, p0.z, p0.w, p1.x, p1.y, p1.z, p1.w};
+      float sm = 0.f, sq = 0.f;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) { dot_bf16x2(sm, pw_[i], ones); dot_bf16x2(sq, pw_[i], pw_[i]); }
+      const float mu = sm * (1.f / sCz);
+      const float rstd = rsqrtf(fmaxf(fmaf(sq, 1.f / sCz, -mu * mu), 0.f) + p.eps);
+#pragma unroll
+      for (int h = 0; h < H; ++h) {
+        const uint4 w0 = __ldg(reinterpret_cast<const uint4*>(p.wfold + h * sCz));
+        const uint4 w1 = __ldg(reinterpret_cast<const uint4*>(p.wfold + h * sCz) + 1);
+        const uint32_t wf_[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+        float pw = 0.f;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) dot_bf16x2(pw, pw_[i], wf_[i]);
+        s_logit[j * H + h] = fmaf(rstd, pw - mu * __ldg(p.c1 + h), __ldg(p.c0 + h));
+      }
+    } else {
+#pragma unroll
+      for (int h = 0; h < H; ++h) s_logit[j * H + h] = -INFINITY;
+    }
+  }
+  __syncwarp();
+  // ---- (B) logits += q . k, RPL rows per load, four loads in flight
+  for (int j0 = 0; j0 < p.kn; j0 += 4 * RPL) {
+    uint4 kv[4];
+    int mm[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int j = j0 + u * RPL + grp;
+      mm[u] = j < p.kn ? s_idx[j] : -1;
+      if (mm[u] >= 0) kv[u] = __ldg(reinterpret_cast<const uint4*>(p.k + (int64_t)mm[u] * D) + ch);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      float d0 = 0.f, d1 = 0.f;
+      if (mm[u] >= 0) {
+        dot_bf16x2(d0, kv[u].x, qv.x); dot_bf16x2(d1, kv[u].y, qv.y);
+        dot_bf16x2(d0, kv[u].z, qv.z); dot_bf16x2(d1, kv[u].w, qv.w);
+      }
+      float d = d0 + d1;
+      d += __shfl_xor_sync(0xffffffffu, d, 1);
+      d += __shfl_xor_sync(0xffffffffu, d, 2);
+      if (mm[u] >= 0 && (ch & 3) == 0) s_logit[(j0 + u * RPL + grp) * H + hd] += d;
+    }
+  }
+  __syncwarp();
+  // ---- (C) softmax statistics per head over the slots (lane = slot), numerators back to shared memory
+  float mx[H], sum[H];
+#pragma unroll
+  for (int h = 0; h < H; ++h) { mx[h] = -INFINITY; sum[h] = 0.f; }
+  for (int j = lane; j < kpad; j += 32)
+#pragma unroll
+    for (int h = 0; h < H; ++h) mx[h] = fmaxf(mx[h], s_logit[j * H + h]);
+#pragma unroll
+  for (int h = 0; h < H; ++h) mx[h] = warp_max(mx[h]);
+  if (mx[0] == -INFINITY) {             // no valid neighbour (a slot is valid for all heads or for none): o = 0
+    for (int e = lane; e < D; e += 32) p.gated[l * D + e] = __float2bfloat16_rn(0.f);
+    return;
+  }
+  for (int j = lane; j < kpad; j += 32)
+#pragma unroll
+    for (int h = 0; h < H; ++h) {
+      const float pe = fast_exp2(s_logit[j * H + h] - mx[h]);    // exp2(-inf) = 0 for unused slots
+      sum[h] += pe;
+      s_logit[j * H + h] = pe;
+    }
+#pragma unroll
+  for (int h = 0; h < H; ++h) sum[h] = warp_sum(sum[h]);
+  __syncwarp();
+  // ---- (D) acc += P v, RPL rows per load, four loads in flight
+  float acc[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) acc[i] = 0.f;
+  for (int j0 = 0; j0 < p.kn; j0 += 4 * RPL) {
+    uint4 vv[4];
+    int mm[4];
+    float pe[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int j = j0 + u * RPL + grp;
+      mm[u] = j < p.kn ? s_idx[j] : -1;
+      if (mm[u] >= 0) {
+        vv[u] = __ldg(reinterpret_cast<const uint4*>(p.v + (int64_t)mm[u] * D) + ch);
+        pe[u] = s_logit[j * H + hd];
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      if (mm[u] >= 0) {
+        const uint32_t pb = pack_bf16(pe[u], 0.f);     // P rounded to bf16 for PV, like the dense kernels
+        axpy_bf16x2(acc[0], acc[1], vv[u].x, pb); axpy_bf16x2(acc[2], acc[3], vv[u].y, pb);
+        axpy_bf16x2(acc[4], acc[5], vv[u].z, pb); axpy_bf16x2(acc[6], acc[7], vv[u].w, pb);
+      }
+  }
+  // the RPL row groups hold partial sums of the same output chunk
+#pragma unroll
+  for (int off = LPR; off < 32; off <<= 1)
+#pragma unroll
+    for (int i = 0; i < 8; ++i) acc[i] += __shfl_xor_sync(0xffffffffu, acc[i], off);
+  if (grp == 0) {
+    float lh = sum[0];
+#pragma unroll
+    for (int h = 1; h < H; ++h) lh = hd == h ? sum[h] : lh;
+    const float inv = 1.f / lh;
+    const uint4 gv = __ldg(reinterpret_cast<const uint4*>(p.g + l * D) + ch);
+    const uint32_t gw[4] = {gv.x, gv.y, gv.z, gv.w};
+    uint32_t ow[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float g0 = __uint_as_float(gw[i] << 16), g1 = __uint_as_float(gw[i] & 0xffff0000u);
+      ow[i] = pack_bf16(g0 * (acc[2 * i] * inv), g1 * (acc[2 * i + 1] * inv));
+    }
+    *reinterpret_cast<uint4*>(p.gated + l * D + ch * 8) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+  }
+}
+
 }  // namespace
 
 bool sparse_atom_supports(dcp_dtype dt, int H, int c, int c_z, int kn) {
@@ -181,6 +328,23 @@ cudaError_t launch_sparse_atom(const void* q, const void* k, const void* v, cons
   sp.g = (const __nv_bfloat16*)g; sp.p = (const __nv_bfloat16*)p_slice; sp.idx = idx;
   sp.wfold = (const __nv_bfloat16*)wfold; sp.c1 = c1; sp.c0 = c0; sp.gated = (__nv_bfloat16*)gated;
   sp.L = L; sp.kn = kn; sp.H = H; sp.eps = eps;
+  if (H == 2 || H == 4 || H == 8) {   // row-coalesced kernel: one warp per atom, dynamic smem = logits + indices
+    const int kpad = (kn + 31) & ~31;
+    const size_t smem = (size_t)4 * kpad * (H + 1) * sizeof(float);
+    const unsigned blocks = (unsigned)((L + 3) / 4);
+    cudaError_t e = cudaSuccess;
+    if (H == 2) {
+      e = cudaFuncSetAttribute(sparse_atom_rows_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (e == cudaSuccess) sparse_atom_rows_kernel<2><<<blocks, 128, smem, st>>>(sp);
+    } else if (H == 4) {
+      e = cudaFuncSetAttribute(sparse_atom_rows_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (e == cudaSuccess) sparse_atom_rows_kernel<4><<<blocks, 128, smem, st>>>(sp);
+    } else {
+      e = cudaFuncSetAttribute(sparse_atom_rows_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+      if (e == cudaSuccess) sparse_atom_rows_kernel<8><<<blocks, 128, smem, st>>>(sp);
+    }
+    return e != cudaSuccess ? e : cudaGetLastError();
+  }
   const int64_t warps = L * H;
   sparse_atom_kernel<<<(unsigned)((warps + 3) / 4), 128, 0, st>>>(sp);
   return cudaGetLastError();

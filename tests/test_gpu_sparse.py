@@ -40,6 +40,8 @@ def _oracle(cfg, a, p, idx, w, rows=None):
     (40, 40, 2, 128, False, False),     # k = L: every atom attends to all atoms
     (129, 1, 3, 72, False, False),      # single neighbour, odd head count, c_atom not a multiple of 64
     (600, 512, 4, 128, False, False),   # the largest supported budget
+    (200, 64, 8, 128, False, False),    # H = 8: one 512-byte row per warp-level load
+    (90, 48, 16, 64, False, False),     # H = 16: slot-per-lane kernel
 ])
 def test_sparse_small_shapes(L, k, H, c_atom, ln_s, b_q):
     dcp = _dcp()
