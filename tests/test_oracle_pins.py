@@ -384,3 +384,53 @@ def test_sparse_single_neighbour_closed_form():
     gate = 1.0 / (1.0 + np.exp(-(a @ w["w_g"])))
     ref = (gate * (a[idx[:, 0]] @ w["w_v"])) @ w["w_o"]
     assert np.max(np.abs(got - ref)) <= 1e-12
+
+
+# ---------------------------------------------------------------- k nearest neighbours
+def test_knn_integer_lattice_closed_form():
+    """Points on the integer line 0..n-1 (exact binary32 distances): the neighbours of l are l, then l-1 / l+1
+    (the smaller index first on the tie), l-2 / l+2, ..."""
+    from oracle import knn as ko
+    n, k = 23, 7
+    x = np.zeros((n, 3), dtype=np.float32)
+    x[:, 1] = np.arange(n)
+    got = ko.knn(x, k)
+    for l in range(n):
+        cand = sorted(range(n), key=lambda m: (abs(m - l), m))[:k]
+        assert got[l].tolist() == cand
+
+
+def test_knn_brute_force_binary32():
+    """Pure-Python brute force with every operation rounded to binary32 through struct (independent of numpy)."""
+    import struct
+    from oracle import knn as ko
+    f32 = lambda v: struct.unpack("f", struct.pack("f", v))[0]
+    rng = np.random.default_rng(51)
+    L, k = 40, 9
+    x = (rng.normal(size=(L, 3)) * 7).astype(np.float32)
+    x[7] = x[3]                                    # an exact duplicate point: tie broken by index
+    got = ko.knn(x, k)
+    xs = [[float(v) for v in row] for row in x]
+    for l in range(L):
+        d = []
+        for m in range(L):
+            t = [f32(xs[m][a] - xs[l][a]) for a in range(3)]
+            s = [f32(t[a] * t[a]) for a in range(3)]
+            d.append((f32(f32(s[0] + s[1]) + s[2]), m))
+        assert got[l].tolist() == [m for _, m in sorted(d)[:k]]
+
+
+def test_knn_matches_kdtree_and_is_translation_invariant():
+    from scipy.spatial import cKDTree
+    from oracle import knn as ko
+    rng = np.random.default_rng(52)
+    L, k = 300, 16
+    x = rng.uniform(-20, 20, size=(L, 3)).astype(np.float32)
+    got = ko.knn(x, k)
+    _, ref = cKDTree(x.astype(np.float64)).query(x.astype(np.float64), k=k)
+    for l in range(L):                             # fp64 vs binary32 can only differ on near-ties: compare as sets
+        assert len(set(got[l].tolist()) ^ set(ref[l].tolist())) <= 2
+    assert np.array_equal(got[:, 0], np.arange(L))                 # the query itself comes first (d2 = 0)
+    xi = np.round(x * 8) / 8                        # multiples of 1/8: a shift by 64 is exact in binary32
+    assert np.array_equal(ko.knn(xi, k), ko.knn((xi + np.float32(64.0)).astype(np.float32), k))
+    assert np.array_equal(ko.knn(x, 1)[:, 0], np.arange(L))
