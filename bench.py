@@ -46,8 +46,9 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4"],
-                    help="C0..C4: BASELINE.json configs (dense layer); S4: sparse k-neighbour atom attention on C4's atoms")
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4", "K4"],
+                    help="C0..C4: BASELINE.json configs (dense layer); S4: sparse k-neighbour atom attention on C4's atoms; "
+                         "K4: the k-nearest-neighbour lists of C4's atoms (dcp_knn)")
     ap.add_argument("--neighbours", type=int, default=128, help="S4: budget k (PAPER.md:303 default 128)")
     ap.add_argument("--decomp", default="monolithic", choices=["monolithic", "row", "grid"])
     ap.add_argument("--parts", type=int, default=0, help="row stripes / grid cells (0: 8 rows, 16 grid)")
@@ -156,6 +157,27 @@ def run_reference(args, rank, world):
     import dcp_synth as syn
     if args.workload == "S4":
         run_reference_sparse(args)
+        return
+    if args.workload == "K4":
+        from oracle import knn as ko
+        cfg = syn.CONFIGS["C4"]
+        xh = syn.make_atom_coords(cfg, "cpu").numpy()
+        n_rows = args.cpu_rows or 2000
+        secs = 0.0
+        for step in range(args.steps):
+            rows = syn.sample_rows(cfg.I, n_rows, seed=step)
+            t0 = time.perf_counter()
+            ko.knn_rows(xh, args.neighbours, rows)
+            secs += time.perf_counter() - t0
+        value = n_rows * float(cfg.I) * args.steps / secs / 1e9
+        sample = f"{n_rows} sampled query atoms x {cfg.I} candidates per step ({args.steps} steps), binary32 numpy oracle"
+        print(json.dumps({"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / max(args.steps, 1) * 1e3,
+                          "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                          "config": {"workload": f"K4: k-nearest-neighbour lists L={cfg.I} k={args.neighbours}", "sample": sample},
+                          "cpu_baseline": {"value": value, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
+                          "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                          "gpu_launches": 0}), flush=True)
         return
     cfg = syn.CONFIGS[args.workload]
     dev = "cuda:0" if torch.cuda.is_available() else "cpu"
@@ -312,6 +334,98 @@ def run_reference_sparse(args):
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}), flush=True)
 
 
+def run_knn(args, rank, world, local_rank):
+    """--workload K4: neighbour lists of C4's 24000 synthetic atoms, k = --neighbours.
+    One pair = one (query atom, candidate atom) distance: L^2 per call.  Single GPU (or independent replicas)."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as ge
+    if rank == 0 or world == 1:
+        ge.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    import dcp_synth as syn
+    import paper_2607_05439_b200 as dcp
+    from oracle import knn as ko
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    cfg = replica_config(syn.CONFIGS["C4"], rank, world)
+    k, L = args.neighbours, syn.CONFIGS["C4"].I
+    x = syn.make_atom_coords(cfg, dev)
+    out = torch.empty(L, k, dtype=torch.int32, device=dev)
+    for _ in range(max(args.warmup, 3)):
+        dcp.dcp_knn(x, k, out=out)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = dcp.Event(), dcp.Event()
+    e0.record()
+    for _ in range(args.steps):
+        dcp.dcp_knn(x, k, out=out)
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = max_over_ranks_ms(e0.elapsed_ms(e1), world, dev)
+    pairs = float(L) * L
+    value = pairs * args.steps * world / (total_ms * 1e-3) / 1e9
+    kms = total_ms / args.steps
+    # ALU bound: the scan needs >= 12 thread-instructions per candidate (3 LDS, 3 FSUB, 3 FMUL, 2 FADD, 1 compare);
+    # peak = 148 SMs x 128 lanes x sm clock / 12 (DESIGN.md 6.5); insertions into the sorted list come on top
+    sm_clock_ghz = 1.965
+    peak = 148 * 128 * sm_clock_ghz / 12.0
+    roofline = {"bound": "alu", "achieved": pairs / (kms * 1e-3) / 1e9, "peak": peak, "unit": "Gpair/s",
+                "frac": pairs / (kms * 1e-3) / 1e9 / peak, "traffic": None, "kernel": "knn_kernel",
+                "peak_source": "derived: 148 SMs x 128 FP32 lanes x 1.965 GHz / 12 instructions per candidate",
+                "kernel_ms": kms, "kernel_share_of_step": 1.0}
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        rows = syn.sample_rows(L, args.cpu_rows or 3000, seed=0)
+        xh = x.cpu().numpy()
+        t0 = time.perf_counter()
+        ref = ko.knn_rows(xh, k, rows)
+        dt = time.perf_counter() - t0
+        got = out.index_select(0, torch.as_tensor(rows, device=dev)).cpu().numpy()
+        cpu = {"value": len(rows) * float(L) / dt / 1e9, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+               "sample": f"{len(rows)} sampled query atoms x {L} candidates ({dt:.1f} s), binary32 numpy oracle",
+               "gpu_vs_oracle_bit_exact_on_sample": bool(np.array_equal(got, ref))}
+    e2e = None
+    if not args.no_e2e:
+        xh, oh = x.cpu().pin_memory(), torch.empty(L, k, dtype=torch.int32).pin_memory()
+        xd = torch.empty_like(x)
+        ne = max(1, args.e2e_steps)
+        a, b = dcp.Event(), dcp.Event()
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(ne):
+            xd.copy_(xh, non_blocking=True)
+            dcp.dcp_knn(xd, k, out=out)
+            oh.copy_(out, non_blocking=True)
+        b.record()
+        torch.cuda.synchronize()
+        ms = max_over_ranks_ms(a.elapsed_ms(b), world, dev)
+        e2e = {"value": pairs * ne * world / (ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": xh.numel() * 4,
+               "d2h_bytes_per_step": oh.numel() * 4, "steps": ne}
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": kms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": f"K4: k-nearest-neighbour lists L={L} k={k} (icosahedral 60 x {cfg.n_res} synthetic atoms)",
+                       "pair": "one (query atom, candidate atom) distance", "kernel": "knn_kernel",
+                       "l2": "inputs (288 KB) are cache resident by nature; nothing to flush",
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "peak_device_bytes": int(torch.cuda.max_memory_allocated())},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": args.steps + max(args.warmup, 3), "clocks": clocks}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_sparse(args, rank, world, local_rank):
     """--workload S4: sparse k-neighbour atom attention on C4's atoms (L = 24000, c_atom = 128,
     c_atompair = 16, H = 4, c = 32), budget k = --neighbours.  One pair = one (query atom, neighbour slot)."""
@@ -455,6 +569,9 @@ def main():
         return
     if args.workload == "S4":
         run_sparse(args, rank, world, local_rank)
+        return
+    if args.workload == "K4":
+        run_knn(args, rank, world, local_rank)
         return
 
     import torch

@@ -117,6 +117,15 @@ dcp_status dcp_sparse_atom_attention(const void *a, const void *p_slice, const i
                                      dcp_dtype dtype, const dcp_plan *plan, void *workspace, size_t workspace_bytes,
                                      void *stream);
 
+/* Neighbour lists for dcp_sparse_atom_attention ("The kNN indices are computed once per denoising step
+ * from the current noised coordinates X^(t) via a single cdist call"; :454 distance matrix + top-k per row, here
+ * without the [L, L] matrix).  x [L, 3] fp32 device; idx [L, k] int32 device: the k atoms with the smallest squared
+ * Euclidean distance to atom l (itself included), ordered by (distance, atom index) ascending -- unique, and
+ * bit-exact against the oracle: distances in binary32, t = x_m - x_l, d2 = (t0 t0 + t1 t1) + t2 t2, no FMA.
+ * 1 <= k <= min(L, 512) (DCP_ERR_INVALID_ARG / DCP_ERR_UNSUPPORTED otherwise).  The paper's sequence-local and
+ * inter-chain quotas are not part of this call. */
+dcp_status dcp_knn(const float *x, int32_t *idx, int64_t L, int k, void *stream);
+
 /* End-to-end entry with HOST inputs/outputs: s_host, z_host, out_host are HOST pointers (pinned memory gives
  * full PCIe rate); weights stay device-resident (they are parameters, not per-step inputs).  Copies s and z
  * to the device staging buffers s_dev [I,c_s], z_dev [I,I,c_z], runs the layer, copies out back, all on

@@ -27,7 +27,7 @@ KERNEL = {"auto": DCP_KERNEL_AUTO, "generic": DCP_KERNEL_GENERIC, "mma": DCP_KER
 EXPORTS = [
     "dcp_workspace_bytes", "dcp_pair_bias_attention", "dcp_atom_pair_bias_attention",
     "dcp_pair_bias_attention_host", "dcp_partial_states", "dcp_merge_states", "dcp_shard_range",
-    "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention",
+    "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention", "dcp_knn",
     "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
     "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
 ]
@@ -83,7 +83,8 @@ def _load() -> C.CDLL:
     lib.dcp_sparse_atom_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, C.POINTER(sz)]
     lib.dcp_sparse_atom_attention.argtypes = [vp, vp, vp, C.POINTER(dcp_weights), vp, i64, i32, i32, i32, i32, i32, i32,
                                               C.POINTER(dcp_plan), vp, sz, vp]
-    for n in EXPORTS[:9]:
+    lib.dcp_knn.argtypes = [vp, vp, i64, i32, vp]
+    for n in EXPORTS[:10]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -217,6 +218,16 @@ def dcp_pair_bias_attention(s, z, w, H, c, decomp="monolithic", parts=1, key_spl
 def dcp_atom_pair_bias_attention(a, p, w, H, c, **kw):
     """Atom-level dense variant (BASELINE.json config 4): (L, c_atom, c_atompair) for (I, c_s, c_z)."""
     return dcp_pair_bias_attention(a, p, w, H, c, atom=True, **kw)
+
+
+def dcp_knn(x, k, out=None, stream=None):
+    """idx [L, k] int32: the k nearest atoms of every atom of x [L, 3] fp32 (itself included), by (distance, index)."""
+    assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.shape[1] == 3
+    L = x.shape[0]
+    if out is None:
+        out = torch.empty(L, k, dtype=torch.int32, device=x.device)
+    _check(_lib.dcp_knn(_ptr(x), _ptr(out), L, int(k), _stream_ptr(stream)), "dcp_knn")
+    return out
 
 
 def dcp_sparse_atom_workspace_bytes(L, c_atom, H, c, dtype: torch.dtype) -> int:

@@ -433,6 +433,14 @@ dcp_status dcp_sparse_atom_attention(const void* a, const void* p_slice, const i
   return DCP_OK;
 }
 
+dcp_status dcp_knn(const float* x, int32_t* idx, int64_t L, int k, void* stream) {
+  g_launches = 0;
+  if (!x || !idx || L <= 0 || k <= 0 || k > L) return DCP_ERR_INVALID_ARG;
+  if (!knn_supports(L, k)) return DCP_ERR_UNSUPPORTED;
+  DCP_CUDA(launch_knn(x, idx, L, k, (cudaStream_t)stream));
+  return DCP_OK;
+}
+
 dcp_status dcp_pair_bias_attention_host(const void* s_host, const void* z_host, const dcp_weights* w, void* out_host,
                                         void* s_dev, void* z_dev, void* out_dev, int64_t I, int c_s, int H, int c,
                                         int c_z, dcp_dtype dtype, dcp_decomp decomp, const dcp_plan* plan,

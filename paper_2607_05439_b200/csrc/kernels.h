@@ -89,6 +89,10 @@ cudaError_t launch_sparse_atom(const void* q, const void* k, const void* v, cons
                                const int32_t* idx, const void* wfold, const float* c1, const float* c0, void* gated,
                                int64_t L, int kn, int H, float eps, cudaStream_t st);
 
+// k nearest neighbours of every atom (knn.cu): x [L][3] fp32 -> idx [L][k], ordered by (d2, index)
+bool knn_supports(int64_t L, int k);
+cudaError_t launch_knn(const float* x, int32_t* idx, int64_t L, int k, cudaStream_t st);
+
 // Merge (step a8) + normalise + gate (first half of a9); or raw merged state out.
 cudaError_t launch_merge(dcp_dtype dt, const MergeParams& p, cudaStream_t st);
 
