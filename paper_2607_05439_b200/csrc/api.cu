@@ -191,9 +191,14 @@ dcp_status run_prologue_mma(const Ctx& x, const void* s) {
   gp.scale[1] = 1.f;
   gp.ldc[3] = x.D;
   gp.H = x.H; gp.c = x.c; gp.cp = cp;
-  DCP_CUDA(launch_gemm_mma(gp, x.st));
-  DCP_CUDA(launch_fold_ln_z_mma(x.w->w_b, x.w->ln_z_gamma, x.w->ln_z_beta, x.ws + x.cv.wfold, (float*)(x.ws + x.cv.c1),
-                                (float*)(x.ws + x.cv.c0), x.c_z, x.H, 16, x.st));
+  gp.fold_w_b = x.w->w_b; gp.fold_gamma = x.w->ln_z_gamma; gp.fold_beta = x.w->ln_z_beta;
+  gp.fold_wfold = x.ws + x.cv.wfold; gp.fold_c1 = (float*)(x.ws + x.cv.c1); gp.fold_c0 = (float*)(x.ws + x.cv.c0);
+  gp.fold_c_z = x.c_z; gp.fold_H = x.H; gp.fold_H_pad = 16;
+  bool folded = false;
+  DCP_CUDA(launch_gemm_mma(gp, x.st, &folded));
+  if (!folded)
+    DCP_CUDA(launch_fold_ln_z_mma(x.w->w_b, x.w->ln_z_gamma, x.w->ln_z_beta, x.ws + x.cv.wfold, (float*)(x.ws + x.cv.c1),
+                                  (float*)(x.ws + x.cv.c0), x.c_z, x.H, 16, x.st));
   return DCP_OK;
 }
 

@@ -9,6 +9,7 @@
 //   g -> g  [I][D]      sigmoid gate
 // Every output element is accumulated over k in a fixed order that does not depend on the tile it falls in.
 #include "kernels.h"
+#include "fold.cuh"
 
 namespace dcp {
 
@@ -225,33 +226,18 @@ __global__ void layernorm_rows_bf16_kernel(const __nv_bfloat16* __restrict__ x, 
 __global__ void fold_ln_z_mma_kernel(const __nv_bfloat16* __restrict__ w_b, const __nv_bfloat16* __restrict__ gamma,
                                      const __nv_bfloat16* __restrict__ beta, __nv_bfloat16* __restrict__ wfold,
                                      float* __restrict__ c1, float* __restrict__ c0, int c_z, int H, int H_pad) {
-  // wfold[h][k] = bf16(gamma_k W_b[k,h] log2 e)   (K-major rows: the B operand of the projection MMA)
-  // c1[h] = sum_k wfold[h][k] (the rounded values), c0[h] = log2 e * sum_k beta_k W_b[k,h]
-  constexpr float kLog2e = 1.4426950408889634f;
-  for (int e = threadIdx.x; e < H_pad * c_z; e += blockDim.x) {
-    const int h = e / c_z, k = e % c_z;
-    const float v = h < H ? to_f32(gamma[k]) * to_f32(w_b[k * H + h]) * kLog2e : 0.f;
-    wfold[e] = __float2bfloat16_rn(v);
-  }
-  __syncthreads();
-  // one warp per head: lane-strided partial sums, then a butterfly reduction (fixed order: run-to-run repeatable)
-  for (int h = threadIdx.x >> 5; h < H_pad; h += blockDim.x >> 5) {
-    float a1 = 0.f, a0 = 0.f;
-    for (int k = threadIdx.x & 31; k < c_z; k += 32) {
-      a1 += to_f32(wfold[h * c_z + k]);
-      if (h < H) a0 = fmaf(to_f32(beta[k]), to_f32(w_b[k * H + h]), a0);
-    }
-    a1 = warp_sum(a1);
-    a0 = warp_sum(a0);
-    if ((threadIdx.x & 31) == 0) { c1[h] = a1; c0[h] = a0 * kLog2e; }
-  }
+  fold_ln_z_mma_device(w_b, gamma, beta, wfold, c1, c0, c_z, H, H_pad, threadIdx.x, blockDim.x);
 }
 
 }  // namespace
 
-cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st) {
+cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st, bool* fold_done) {
+  if (fold_done) *fold_done = false;
   if (p.M <= 0 || p.N <= 0 || p.K <= 0) return cudaSuccess;
-  if (gemm_tc_supports(p)) return launch_gemm_tc(p, st);
+  if (gemm_tc_supports(p)) {
+    if (fold_done) *fold_done = p.fold_w_b != nullptr;
+    return launch_gemm_tc(p, st);
+  }
   if (p.K % 8 != 0 || p.N % 8 != 0 || p.lda % 8 != 0) return cudaErrorInvalidValue;
   const int64_t nb = (int64_t)p.nseg * ((p.N + BN - 1) / BN);
   if (nb * ((p.M + 127) / 128) >= 2 * 148) {   // enough 128-row tiles for two CTAs per SM

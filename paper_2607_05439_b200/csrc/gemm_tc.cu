@@ -12,6 +12,7 @@
 //             the output modes)
 // The launcher falls back to the mma.sync kernel (gemm_mma.cu) for shapes this tiling does not cover
 // (N % 64, K % 64, unaligned pitches).  Every output element is accumulated over k in one fixed order.
+#include "fold.cuh"
 #include "kernels.h"
 #include "mma_ptx.cuh"
 
@@ -74,6 +75,13 @@ __global__ void __launch_bounds__(kTcThreads, 2) gemm_tc_kernel(const __grid_con
   const uint32_t bar_full = s_bar, bar_empty = s_bar + 8 * TST, bar_acc = s_bar + 16 * TST;
   volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + kTcSmemBar + (2 * TST + 2) * 8);
 
+  if (blockIdx.y == gridDim.y - 1 && p.fold_w_b != nullptr) {
+    // the extra CTA row of the launch: CTA 0 folds LayerNorm(z) into the bias projection weights, the others leave
+    if (blockIdx.x == 0 && threadIdx.x < 256)
+      fold_ln_z_mma_device(p.fold_w_b, p.fold_gamma, p.fold_beta, p.fold_wfold, p.fold_c1, p.fold_c0, p.fold_c_z, p.fold_H,
+                           p.fold_H_pad, threadIdx.x, 256);
+    return;
+  }
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nb_per_seg = p.N / TBN;
   const int seg = blockIdx.x / nb_per_seg;
@@ -254,9 +262,10 @@ cudaError_t launch_gemm_tc(const GemmMmaParams& p, cudaStream_t st) {
       e = cudaFuncSetAttribute(gemm_tc_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TcCfg<64>::kSmemAlloc);
     if (e != cudaSuccess) return e;
   }
-  const unsigned mt = (unsigned)((p.M + TBM - 1) / TBM);
+  const unsigned mt_tiles = (unsigned)((p.M + TBM - 1) / TBM);
+  const unsigned mt = mt_tiles + (p.fold_w_b != nullptr ? 1u : 0u);     // + the row that carries the LayerNorm(z) fold
   // 128-wide tiles when they give every SM two CTAs (or N does not split into 64s evenly enough to matter)
-  if (p.N % 128 == 0 && (int64_t)p.nseg * (p.N / 128) * mt >= 2 * 148) {
+  if (p.N % 128 == 0 && (int64_t)p.nseg * (p.N / 128) * mt_tiles >= 2 * 148) {
     dim3 grid((unsigned)(p.nseg * (p.N / 128)), mt);
     gemm_tc_kernel<128><<<grid, kTcThreads, TcCfg<128>::kSmemAlloc, st>>>(maps, p);
   } else {

@@ -39,11 +39,17 @@ struct GemmMmaParams {
   float scale[4];       // HEADPAD only
   int64_t ldc[4];       // PLAIN / SIGMOID: row pitch; TRANSPOSED: pitch of the transposed rows
   int H, c, cp;         // HEADPAD: C[(row*H + h)*cp + d] for column h*c + d; KFRAG / VFRAG: MMA-fragment order (fused_mma.cu)
+  // optional: the LayerNorm(z) fold (fold_ln_z_mma) rides along as one extra CTA of the tcgen05 GEMM launch
+  // (fold_w_b == nullptr: not requested; launch_gemm_mma reports through `fold_done` whether it was done)
+  const void *fold_w_b, *fold_gamma, *fold_beta;
+  void* fold_wfold;
+  float *fold_c1, *fold_c0;
+  int fold_c_z, fold_H, fold_H_pad;
 };
-cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st);   // dispatches to launch_gemm_tc when it applies
+cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st, bool* fold_done = nullptr);   // dispatches to launch_gemm_tc when it applies
 // tcgen05 / TMA GEMM (gemm_tc.cu): N % 128 == 0, K % 64 == 0, 16-byte aligned operands
 bool gemm_tc_supports(const GemmMmaParams& p);
-cudaError_t launch_gemm_tc(const GemmMmaParams& p, cudaStream_t st);
+cudaError_t launch_gemm_tc(const GemmMmaParams& p, cudaStream_t st);   // also runs the requested LayerNorm(z) fold
 cudaError_t launch_layernorm_rows_bf16(const void* x, const void* gamma, const void* beta, void* y, int64_t rows,
                                        int width, float eps, cudaStream_t st);
 // wfold [H_pad][c_z] bf16 = (gamma (.) W_b * log2 e)^T, c1[h] = sum_k wfold[h][k], c0[h] = log2 e * sum_k beta_k W_b[k,h]

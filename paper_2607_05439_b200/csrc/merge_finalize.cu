@@ -46,7 +46,9 @@ __global__ void __launch_bounds__(256) merge_kernel(const MergeParams p) {
 // Same fold, four consecutive channels of one head per thread (c % 4 == 0): 128-bit state loads, the rescale
 // factors e^{m_a-m'}, e^{m_b-m'} computed once per thread instead of once per channel.  Element arithmetic and
 // order are identical to merge_kernel, so both produce the same bits.
-template <typename T>
+// NS > 0: the slot count is a compile-time constant, so all slots' loads are issued before the fold (the fold itself,
+// its order and every operation are the same as in the runtime-count version: same bits).
+template <typename T, int NS>
 __global__ void __launch_bounds__(256) merge_vec4_kernel(const MergeParams p) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int dq = p.D >> 2;
@@ -54,20 +56,44 @@ __global__ void __launch_bounds__(256) merge_vec4_kernel(const MergeParams p) {
   const int64_t row = idx / dq;
   const int e = (int)(idx - row * dq) << 2;
   const int h = e / p.c;
-  float m = p.st_m[row * p.H + h];
-  float l = p.st_l[row * p.H + h];
-  float4 a = *reinterpret_cast<const float4*>(p.st_acc + row * p.D + e);
-  for (int s = 1; s < p.n_slots; ++s) {
-    const int64_t srow = (int64_t)s * p.rows + row;
-    const float mb = p.st_m[srow * p.H + h];
-    const float lb = p.st_l[srow * p.H + h];
-    const float4 ab = *reinterpret_cast<const float4*>(p.st_acc + srow * p.D + e);
-    const float mn = fmaxf(m, mb);
-    const float fa = expf(m - mn), fb = expf(mb - mn);
-    l = l * fa + lb * fb;
-    a.x = a.x * fa + ab.x * fb; a.y = a.y * fa + ab.y * fb;
-    a.z = a.z * fa + ab.z * fb; a.w = a.w * fa + ab.w * fb;
-    m = mn;
+  float m, l;
+  float4 a;
+  if constexpr (NS > 0) {
+    float ms[NS], ls[NS];
+    float4 as[NS];
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+      const int64_t srow = (int64_t)s * p.rows + row;
+      ms[s] = p.st_m[srow * p.H + h];
+      ls[s] = p.st_l[srow * p.H + h];
+      as[s] = *reinterpret_cast<const float4*>(p.st_acc + srow * p.D + e);
+    }
+    m = ms[0]; l = ls[0]; a = as[0];
+#pragma unroll
+    for (int s = 1; s < NS; ++s) {
+      const float mn = fmaxf(m, ms[s]);
+      const float fa = expf(m - mn), fb = expf(ms[s] - mn);
+      l = l * fa + ls[s] * fb;
+      a.x = a.x * fa + as[s].x * fb; a.y = a.y * fa + as[s].y * fb;
+      a.z = a.z * fa + as[s].z * fb; a.w = a.w * fa + as[s].w * fb;
+      m = mn;
+    }
+  } else {
+    m = p.st_m[row * p.H + h];
+    l = p.st_l[row * p.H + h];
+    a = *reinterpret_cast<const float4*>(p.st_acc + row * p.D + e);
+    for (int s = 1; s < p.n_slots; ++s) {
+      const int64_t srow = (int64_t)s * p.rows + row;
+      const float mb = p.st_m[srow * p.H + h];
+      const float lb = p.st_l[srow * p.H + h];
+      const float4 ab = *reinterpret_cast<const float4*>(p.st_acc + srow * p.D + e);
+      const float mn = fmaxf(m, mb);
+      const float fa = expf(m - mn), fb = expf(mb - mn);
+      l = l * fa + lb * fb;
+      a.x = a.x * fa + ab.x * fb; a.y = a.y * fa + ab.y * fb;
+      a.z = a.z * fa + ab.z * fb; a.w = a.w * fa + ab.w * fb;
+      m = mn;
+    }
   }
   if (p.g != nullptr) {
     const T* gp = reinterpret_cast<const T*>(p.g) + row * p.D + e;
@@ -82,6 +108,17 @@ __global__ void __launch_bounds__(256) merge_vec4_kernel(const MergeParams p) {
   }
 }
 
+template <typename T>
+void launch_vec4(const MergeParams& p, unsigned blocks, cudaStream_t st) {
+  switch (p.n_slots) {
+    case 1: merge_vec4_kernel<T, 1><<<blocks, 256, 0, st>>>(p); break;
+    case 2: merge_vec4_kernel<T, 2><<<blocks, 256, 0, st>>>(p); break;
+    case 3: merge_vec4_kernel<T, 3><<<blocks, 256, 0, st>>>(p); break;
+    case 4: merge_vec4_kernel<T, 4><<<blocks, 256, 0, st>>>(p); break;
+    default: merge_vec4_kernel<T, 0><<<blocks, 256, 0, st>>>(p); break;
+  }
+}
+
 }  // namespace
 
 cudaError_t launch_merge(dcp_dtype dt, const MergeParams& p, cudaStream_t st) {
@@ -89,8 +126,8 @@ cudaError_t launch_merge(dcp_dtype dt, const MergeParams& p, cudaStream_t st) {
   if (total <= 0) return cudaSuccess;
   if (p.c % 4 == 0 && ((uintptr_t)p.st_acc & 15) == 0 && (p.g != nullptr || ((uintptr_t)p.acc_out & 15) == 0)) {
     const unsigned vblocks = (unsigned)((total / 4 + 255) / 256);
-    if (dt == DCP_F32) merge_vec4_kernel<float><<<vblocks, 256, 0, st>>>(p);
-    else merge_vec4_kernel<__nv_bfloat16><<<vblocks, 256, 0, st>>>(p);
+    if (dt == DCP_F32) launch_vec4<float>(p, vblocks, st);
+    else launch_vec4<__nv_bfloat16>(p, vblocks, st);
     return cudaGetLastError();
   }
   unsigned blocks = (unsigned)((total + 255) / 256);
