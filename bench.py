@@ -379,7 +379,8 @@ def run_knn(args, rank, world, local_rank):
     sm_clock_ghz = 1.965
     peak = 148 * 128 * sm_clock_ghz / 12.0
     roofline = {"bound": "alu", "achieved": pairs / (kms * 1e-3) / 1e9, "peak": peak, "unit": "Gpair/s",
-                "frac": pairs / (kms * 1e-3) / 1e9 / peak, "traffic": None, "kernel": "knn_kernel",
+                "frac": pairs / (kms * 1e-3) / 1e9 / peak, "traffic": None,
+                "kernel": "knn_select_kernel" if k <= 256 else "knn_kernel",
                 "peak_source": "derived: 148 SMs x 128 FP32 lanes x 1.965 GHz / 12 instructions per candidate",
                 "kernel_ms": kms, "kernel_share_of_step": 1.0}
     cpu = None
@@ -416,7 +417,8 @@ def run_knn(args, rank, world, local_rank):
             "ms_per_step": kms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": {"workload": f"K4: k-nearest-neighbour lists L={L} k={k} (icosahedral 60 x {cfg.n_res} synthetic atoms)",
-                       "pair": "one (query atom, candidate atom) distance", "kernel": "knn_kernel",
+                       "pair": "one (query atom, candidate atom) distance",
+                       "kernel": "knn_select_kernel" if k <= 256 else "knn_kernel",
                        "l2": "inputs (288 KB) are cache resident by nature; nothing to flush",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "peak_device_bytes": int(torch.cuda.max_memory_allocated())},

@@ -10,7 +10,8 @@
 // arithmetic is pinned: IEEE binary32, round to nearest, NO fused multiply-add, t = x_m - x_l per coordinate,
 // d2 = (t0 t0 + t1 t1) + t2 t2 -- the oracle (oracle/knn.py) uses the same operations and the result is bit-exact.
 //
-// One warp per query.  The list of k (d2, index) pairs, sorted lexicographically, lives in registers, NR = k / 32
+// knn_kernel (k > 256; knn_select_kernel below serves k <= 256): one warp per query.  The list of k (d2, index)
+// pairs, sorted lexicographically, lives in registers, NR = k / 32
 // (rounded up) consecutive positions per lane.  Candidates are visited 128 at a time; a ballot picks those that beat
 // the current k-th entry, and each is inserted by a ballot-count of its position and a one-place shift (register
 // moves + one shuffle).  A window of indices around the query is scanned first, which tightens the k-th distance
@@ -126,6 +127,187 @@ __global__ void __launch_bounds__(256) knn_kernel(const float* __restrict__ x, i
   }
 }
 
+// ---- threshold-select variant (k <= 256): no sorted list is maintained while scanning.
+//   1. the warp computes the distances to the 2048 atoms of the block's own tile (64 registers per lane) and bisects
+//      the binary32 bit pattern (non-negative floats order like unsigned integers) for a threshold T with at least k
+//      of those distances <= T: an upper bound of the final k-th distance, a few percent above the tile's own k-th;
+//   2. one scan over all L candidates appends every (d2, index) with d2 <= T to a per-warp shared-memory buffer
+//      (one ballot + one prefix popcount per 32 candidates; typically 1.5 k .. 2 k entries);
+//   3. the buffer is sorted by (d2, index) with a bitonic network and its first k entries are the answer.
+// Same distances, same (d2, index) order as knn_kernel: the result is identical.  A query whose buffer overflows
+// (more than kCap candidates within T: a very dense neighbourhood) falls back to the insertion scan over global memory.
+constexpr int kCap = 512;
+
+template <int NR>
+__device__ __noinline__ void knn_insert_global(const float* __restrict__ x, int32_t* __restrict__ idx, int L, int k, int l,
+                                               int lane) {
+  const float q0 = __ldg(x + 3 * (int64_t)l), q1 = __ldg(x + 3 * (int64_t)l + 1), q2 = __ldg(x + 3 * (int64_t)l + 2);
+  float ld[NR];
+  int li[NR];
+#pragma unroll
+  for (int r = 0; r < NR; ++r) { ld[r] = kInf; li[r] = 0x7fffffff; }
+  const int last_lane = (k - 1) / NR, last_r = (k - 1) % NR;
+  float tau = kInf;
+  int tau_i = 0x7fffffff;
+  for (int c0 = 0; c0 < L; c0 += 32) {
+    const int m = c0 + lane;
+    float d = kInf;
+    if (m < L) {
+      const float a0 = __fsub_rn(__ldg(x + 3 * (int64_t)m), q0), a1 = __fsub_rn(__ldg(x + 3 * (int64_t)m + 1), q1);
+      const float a2 = __fsub_rn(__ldg(x + 3 * (int64_t)m + 2), q2);
+      d = __fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2));
+    }
+    unsigned mask = __ballot_sync(0xffffffffu, d < tau || (d == tau && m < tau_i));
+    while (mask) {
+      const int b = __ffs(mask) - 1;
+      mask &= mask - 1;
+      const float dn = __shfl_sync(0xffffffffu, d, b);
+      const int mn = c0 + b;
+      if (!(dn < tau || (dn == tau && mn < tau_i))) continue;
+      int pos = 0;
+#pragma unroll
+      for (int r = 0; r < NR; ++r) pos += __popc(__ballot_sync(0xffffffffu, ld[r] < dn || (ld[r] == dn && li[r] < mn)));
+      const int pl = pos / NR, pr = pos % NR;
+      const float up_d = __shfl_up_sync(0xffffffffu, ld[NR - 1], 1);
+      const int up_i = __shfl_up_sync(0xffffffffu, li[NR - 1], 1);
+      if (lane > pl) {
+#pragma unroll
+        for (int r = NR - 1; r > 0; --r) { ld[r] = ld[r - 1]; li[r] = li[r - 1]; }
+        ld[0] = up_d; li[0] = up_i;
+      } else if (lane == pl) {
+#pragma unroll
+        for (int r = NR - 1; r > 0; --r)
+          if (r > pr) { ld[r] = ld[r - 1]; li[r] = li[r - 1]; }
+#pragma unroll
+        for (int r = 0; r < NR; ++r)
+          if (r == pr) { ld[r] = dn; li[r] = mn; }
+      }
+      float tl = ld[0];
+      int ti = li[0];
+#pragma unroll
+      for (int r = 1; r < NR; ++r) { tl = r == last_r ? ld[r] : tl; ti = r == last_r ? li[r] : ti; }
+      tau = __shfl_sync(0xffffffffu, tl, last_lane);
+      tau_i = __shfl_sync(0xffffffffu, ti, last_lane);
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < NR; ++r) {
+    const int pos = lane * NR + r;
+    if (pos < k) idx[(int64_t)l * k + pos] = li[r];
+  }
+}
+
+__global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict__ x, int32_t* __restrict__ idx, int L, int k) {
+  extern __shared__ float smem_knn[];
+  float* sx = smem_knn;
+  float* sy = sx + kTile;
+  float* sz = sy + kTile;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  float* bd = sz + kTile + wib * (2 * kCap);                   // per-warp buffer: kCap distances, kCap indices
+  int* bi = reinterpret_cast<int*>(bd + kCap);
+  const int lq = blockIdx.x * 8 + wib;
+  const bool active = lq < L;
+  const int l = active ? lq : L - 1;
+  const float q0 = __ldg(x + 3 * (int64_t)l), q1 = __ldg(x + 3 * (int64_t)l + 1), q2 = __ldg(x + 3 * (int64_t)l + 2);
+  const int n_tiles = (L + kTile - 1) / kTile;
+  const int own = (blockIdx.x * 8) / kTile;
+  unsigned thr = 0x7f800000u;                                  // bit pattern of the threshold T
+  int cnt = 0;
+  const unsigned lt_mask = (1u << lane) - 1u;
+
+  for (int tt = 0; tt < n_tiles; ++tt) {
+    const int tile = tt == 0 ? own : (tt <= own ? tt - 1 : tt);
+    const int t0 = tile * kTile;
+    __syncthreads();
+    for (int e = threadIdx.x; e < kTile; e += blockDim.x) {
+      const int m = t0 + e;
+      sx[e] = m < L ? __ldg(x + 3 * (int64_t)m) : 0.f;
+      sy[e] = m < L ? __ldg(x + 3 * (int64_t)m + 1) : 0.f;
+      sz[e] = m < L ? __ldg(x + 3 * (int64_t)m + 2) : 0.f;
+    }
+    __syncthreads();
+    const int n_here = (L - t0 < kTile ? L - t0 : kTile);
+    if (tt == 0) {
+      // ---- 1. distances to the own tile in registers, bisection for T
+      unsigned db[kTile / 32];
+#pragma unroll
+      for (int i = 0; i < kTile / 32; ++i) {
+        const int e = 32 * i + lane;
+        const float a0 = __fsub_rn(sx[e], q0), a1 = __fsub_rn(sy[e], q1), a2 = __fsub_rn(sz[e], q2);
+        const float dd = __fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2));
+        db[i] = e < n_here ? __float_as_uint(dd) : 0x7f800000u;
+      }
+      unsigned lo = 0u, hi = 0x7f800000u;                      // invariant: #{db <= hi} >= min(k, n_here)
+      const int need = k < n_here ? k : n_here;
+      for (int it = 0; it < 14 && lo < hi; ++it) {
+        const unsigned mid = lo + ((hi - lo) >> 1);
+        int c = 0;
+#pragma unroll
+        for (int i = 0; i < kTile / 32; ++i) c += db[i] <= mid ? 1 : 0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+        if (c >= need) hi = mid; else lo = mid + 1;
+      }
+      thr = n_here >= k ? hi : 0x7f800000u;                    // fewer than k atoms in the tile: no bound from it
+      // ---- 2a. the own tile's candidates come straight from the registers
+#pragma unroll
+      for (int i = 0; i < kTile / 32; ++i) {
+        const bool pass = db[i] <= thr && 32 * i + lane < n_here;
+        const unsigned mask = __ballot_sync(0xffffffffu, pass);
+        const int slot = cnt + __popc(mask & lt_mask);
+        if (pass && slot < kCap) { bd[slot] = __uint_as_float(db[i]); bi[slot] = t0 + 32 * i + lane; }
+        cnt += __popc(mask);
+      }
+    } else {
+      // ---- 2b. every other tile: four chunks per step
+      for (int c0 = 0; c0 < n_here; c0 += 128) {
+        unsigned dbv[4], mk[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int e = (c0 + 32 * u + lane) & (kTile - 1);
+          const float a0 = __fsub_rn(sx[e], q0), a1 = __fsub_rn(sy[e], q1), a2 = __fsub_rn(sz[e], q2);
+          const float dd = __fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2));
+          dbv[u] = __float_as_uint(dd);
+          mk[u] = __ballot_sync(0xffffffffu, dbv[u] <= thr && c0 + 32 * u + lane < n_here);
+        }
+        if ((mk[0] | mk[1] | mk[2] | mk[3]) == 0) continue;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const bool pass = (mk[u] >> lane) & 1u;
+          const int slot = cnt + __popc(mk[u] & lt_mask);
+          if (pass && slot < kCap) { bd[slot] = __uint_as_float(dbv[u]); bi[slot] = t0 + c0 + 32 * u + lane; }
+          cnt += __popc(mk[u]);
+        }
+      }
+    }
+  }
+  if (!active) return;
+  if (cnt > kCap) {                                            // very dense neighbourhood: exact fallback
+    knn_insert_global<8>(x, idx, L, k, l, lane);
+    return;
+  }
+  // ---- 3. bitonic sort of the buffer by (d2, index), padded to a power of two
+  int P = 32;
+  while (P < cnt) P <<= 1;
+  for (int e = cnt + lane; e < P; e += 32) { bd[e] = kInf; bi[e] = 0x7fffffff; }
+  __syncwarp();
+  for (int size = 2; size <= P; size <<= 1) {
+    for (int stride = size >> 1; stride > 0; stride >>= 1) {
+      for (int i = lane; i < (P >> 1); i += 32) {
+        const int pos = 2 * i - (i & (stride - 1));
+        const int par = pos + stride;
+        const bool asc = (pos & size) == 0;
+        const float da = bd[pos], dbb = bd[par];
+        const int ia = bi[pos], ib = bi[par];
+        const bool a_after_b = da > dbb || (da == dbb && ia > ib);
+        if (a_after_b == asc) { bd[pos] = dbb; bd[par] = da; bi[pos] = ib; bi[par] = ia; }
+      }
+      __syncwarp();
+    }
+  }
+  for (int j = lane; j < k; j += 32) idx[(int64_t)l * k + j] = bi[j];
+}
+
 }  // namespace
 
 bool knn_supports(int64_t L, int k) { return L >= 1 && L <= 0x7fffffff && k >= 1 && k <= 512 && k <= L; }
@@ -133,6 +315,13 @@ bool knn_supports(int64_t L, int k) { return L >= 1 && L <= 0x7fffffff && k >= 1
 cudaError_t launch_knn(const float* x, int32_t* idx, int64_t L, int k, cudaStream_t st) {
   const int nr = (k + 31) / 32;
   const unsigned blocks = (unsigned)((L + 7) / 8);
+  if (k <= 256) {   // threshold-select kernel: shared tiles (24 KB) + 8 per-warp candidate buffers (4 KB each)
+    const size_t smem = (size_t)(3 * kTile + 8 * 2 * kCap) * sizeof(float);
+    cudaError_t e = cudaFuncSetAttribute(knn_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    knn_select_kernel<<<blocks, 256, smem, st>>>(x, idx, (int)L, k);
+    return cudaGetLastError();
+  }
   if (nr <= 1) knn_kernel<1><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);
   else if (nr <= 2) knn_kernel<2><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);
   else if (nr <= 4) knn_kernel<4><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);

@@ -33,6 +33,18 @@ def test_knn_ties_and_duplicates():
     assert np.array_equal(got, ko.knn(x.cpu().numpy(), 96))
 
 
+def test_knn_dense_cluster_takes_the_exact_fallback():
+    """3000 coincident points + a few others: far more than the select kernel's candidate buffer lie within the
+    threshold, so every query takes the insertion fallback; the order is then purely by index."""
+    dcp = _dcp()
+    x = torch.zeros(3100, 3)
+    x[3000:] = torch.arange(100, dtype=torch.float32)[:, None] + 5.0
+    x = x.to(DEV)
+    got = dcp.dcp_knn(x, 128).cpu().numpy()
+    assert np.array_equal(got, ko.knn(x.cpu().numpy(), 128))
+    assert np.array_equal(got[7], np.arange(128))
+
+
 def test_knn_structured_atoms_sampled_rows():
     """C4's synthetic assembly (L = 24000), k = 128: sampled queries against the oracle, and against the torch
     cdist + topk lists the input generator builds (same sets wherever no near-tie decides)."""
