@@ -117,6 +117,13 @@ dcp_status dcp_sparse_atom_attention(const void *a, const void *p_slice, const i
                                      dcp_dtype dtype, const dcp_plan *plan, void *workspace, size_t workspace_bytes,
                                      void *stream);
 
+/* p_slice[l, j, :] = p[l, idx[l, j], :] ("The relevant slice of P is gathered at those k indices"): the
+ * dense atom-pair tensor p [L, L, c_atompair] (row pitch ldp elements, 0 = L * c_atompair) -> the slice
+ * [L, k, c_atompair] that dcp_sparse_atom_attention consumes; slots with idx < 0 are filled with zeros.  Device
+ * pointers, c_atompair * element size a multiple of 16 bytes, 16-byte aligned (DCP_ERR_INVALID_ARG otherwise). */
+dcp_status dcp_gather_pair_slice(const void *p, int64_t ldp, const int32_t *idx, void *p_slice, int64_t L, int k,
+                                 int c_atompair, dcp_dtype dtype, void *stream);
+
 /* Neighbour lists for dcp_sparse_atom_attention ("The kNN indices are computed once per denoising step
  * from the current noised coordinates X^(t) via a single cdist call"; :454 distance matrix + top-k per row, here
  * without the [L, L] matrix).  x [L, 3] fp32 device; idx [L, k] int32 device: the k atoms with the smallest squared

@@ -27,7 +27,7 @@ KERNEL = {"auto": DCP_KERNEL_AUTO, "generic": DCP_KERNEL_GENERIC, "mma": DCP_KER
 EXPORTS = [
     "dcp_workspace_bytes", "dcp_pair_bias_attention", "dcp_atom_pair_bias_attention",
     "dcp_pair_bias_attention_host", "dcp_partial_states", "dcp_merge_states", "dcp_shard_range",
-    "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention", "dcp_knn",
+    "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention", "dcp_knn", "dcp_gather_pair_slice",
     "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
     "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
 ]
@@ -84,7 +84,8 @@ def _load() -> C.CDLL:
     lib.dcp_sparse_atom_attention.argtypes = [vp, vp, vp, C.POINTER(dcp_weights), vp, i64, i32, i32, i32, i32, i32, i32,
                                               C.POINTER(dcp_plan), vp, sz, vp]
     lib.dcp_knn.argtypes = [vp, vp, i64, i32, vp]
-    for n in EXPORTS[:10]:
+    lib.dcp_gather_pair_slice.argtypes = [vp, i64, vp, vp, i64, i32, i32, i32, vp]
+    for n in EXPORTS[:11]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -218,6 +219,17 @@ def dcp_pair_bias_attention(s, z, w, H, c, decomp="monolithic", parts=1, key_spl
 def dcp_atom_pair_bias_attention(a, p, w, H, c, **kw):
     """Atom-level dense variant (BASELINE.json config 4): (L, c_atom, c_atompair) for (I, c_s, c_z)."""
     return dcp_pair_bias_attention(a, p, w, H, c, atom=True, **kw)
+
+
+def dcp_gather_pair_slice(p, idx, out=None, stream=None):
+    """p_slice [L, k, c] = p[l, idx[l, j], :] from the dense pair tensor p [L, L, c] (zeros where idx < 0)."""
+    assert p.is_cuda and idx.is_cuda and p.is_contiguous() and idx.is_contiguous() and idx.dtype == torch.int32
+    L, k, c_p = p.shape[0], idx.shape[1], p.shape[2]
+    if out is None:
+        out = torch.empty(L, k, c_p, dtype=p.dtype, device=p.device)
+    _check(_lib.dcp_gather_pair_slice(_ptr(p), 0, _ptr(idx), _ptr(out), L, k, c_p, _dtype_code(p.dtype), _stream_ptr(stream)),
+           "dcp_gather_pair_slice")
+    return out
 
 
 def dcp_knn(x, k, out=None, stream=None):

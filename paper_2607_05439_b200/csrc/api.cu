@@ -438,6 +438,18 @@ dcp_status dcp_sparse_atom_attention(const void* a, const void* p_slice, const i
   return DCP_OK;
 }
 
+dcp_status dcp_gather_pair_slice(const void* p, int64_t ldp, const int32_t* idx, void* p_slice, int64_t L, int k,
+                                 int c_atompair, dcp_dtype dtype, void* stream) {
+  g_launches = 0;
+  if (!p || !idx || !p_slice || L <= 0 || k <= 0 || c_atompair <= 0) return DCP_ERR_INVALID_ARG;
+  const int64_t e = elt_size(dtype);
+  if (ldp == 0) ldp = L * (int64_t)c_atompair;
+  if ((c_atompair * e) % 16 != 0 || (ldp * e) % 16 != 0 || (((uintptr_t)p | (uintptr_t)p_slice) & 15) != 0)
+    return DCP_ERR_INVALID_ARG;
+  DCP_CUDA(launch_gather_pair_slice(p, ldp * e, idx, p_slice, L, k, (int)(c_atompair * e), (cudaStream_t)stream));
+  return DCP_OK;
+}
+
 dcp_status dcp_knn(const float* x, int32_t* idx, int64_t L, int k, void* stream) {
   g_launches = 0;
   if (!x || !idx || L <= 0 || k <= 0 || k > L) return DCP_ERR_INVALID_ARG;

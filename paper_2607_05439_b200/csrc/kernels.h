@@ -95,6 +95,10 @@ cudaError_t launch_sparse_atom(const void* q, const void* k, const void* v, cons
                                const int32_t* idx, const void* wfold, const float* c1, const float* c0, void* gated,
                                int64_t L, int kn, int H, float eps, cudaStream_t st);
 
+// p_slice[l, j, :] = P[l, idx[l, j], :] (row_bytes = c_atompair * element size, a multiple of 16; zeros for idx < 0)
+cudaError_t launch_gather_pair_slice(const void* P, int64_t ldp_bytes, const int32_t* idx, void* out, int64_t L, int kn,
+                                     int row_bytes, cudaStream_t st);
+
 // k nearest neighbours of every atom (knn.cu): x [L][3] fp32 -> idx [L][k], ordered by (d2, index)
 bool knn_supports(int64_t L, int k);
 cudaError_t launch_knn(const float* x, int32_t* idx, int64_t L, int k, cudaStream_t st);

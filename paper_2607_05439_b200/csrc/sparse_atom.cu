@@ -313,6 +313,21 @@ __global__ void __launch_bounds__(128) sparse_atom_rows_kernel(const SparseParam
   }
 }
 
+// p_slice[l, j, :] = P[l, idx[l, j], :]  ("The relevant slice of P is gathered at those k indices"):
+// 16-byte chunks, the chunks of one slot on adjacent lanes; unused slots (idx < 0) are filled with zeros.
+__global__ void __launch_bounds__(256) gather_pair_slice_kernel(const uint4* __restrict__ P, int64_t ldp16,
+                                                                const int32_t* __restrict__ idx, uint4* __restrict__ out,
+                                                                int64_t L, int kn, int chunks) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t total = L * kn * chunks;
+  if (e >= total) return;
+  const int ch = (int)(e % chunks);
+  const int64_t slot = e / chunks;
+  const int64_t l = slot / kn;
+  const int m = __ldg(idx + slot);
+  out[e] = m >= 0 ? __ldg(P + l * ldp16 + (int64_t)m * chunks + ch) : make_uint4(0u, 0u, 0u, 0u);
+}
+
 }  // namespace
 
 bool sparse_atom_supports(dcp_dtype dt, int H, int c, int c_z, int kn) {
@@ -350,4 +365,16 @@ cudaError_t launch_sparse_atom(const void* q, const void* k, const void* v, cons
   return cudaGetLastError();
 }
 
+}  // namespace dcp
+
+namespace dcp {
+cudaError_t launch_gather_pair_slice(const void* P, int64_t ldp_bytes, const int32_t* idx, void* out, int64_t L, int kn,
+                                     int row_bytes, cudaStream_t st) {
+  const int chunks = row_bytes / 16;
+  const int64_t total = L * kn * chunks;
+  if (total <= 0) return cudaSuccess;
+  gather_pair_slice_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>((const uint4*)P, ldp_bytes / 16, idx, (uint4*)out,
+                                                                            L, kn, chunks);
+  return cudaGetLastError();
+}
 }  // namespace dcp

@@ -83,6 +83,27 @@ def test_sparse_full_budget_matches_dense_layer():
     util.check_close(dense, ref, "bf16", "dense")
 
 
+def test_gather_pair_slice_and_full_chain():
+    """coordinates -> dcp_knn -> dcp_gather_pair_slice (dense P) -> dcp_sparse_atom_attention, against the oracles:
+    the gather is byte work (bit-exact against torch.gather), the chain is checked against the sparse oracle."""
+    dcp = _dcp()
+    cfg = syn.small_config("chain", I=480, c_s=128, c_z=16, H=4, c=32, dtype="bf16", seed=13, structured=True, copies=60)
+    w = syn.make_weights(cfg, DEV)
+    a = syn.make_s(cfg, DEV)
+    P = syn.make_z(cfg, DEV)
+    x = syn.make_atom_coords(cfg, DEV)
+    idx = dcp.dcp_knn(x, 64)
+    idx[3, 10:] = -1                                        # a partly filled budget
+    p_slice = dcp.dcp_gather_pair_slice(P, idx)
+    ref_slice = torch.gather(P, 1, idx.long().clamp(min=0)[..., None].expand(-1, -1, cfg.c_z))
+    ref_slice = torch.where((idx < 0)[..., None], torch.zeros_like(ref_slice), ref_slice)
+    assert torch.equal(p_slice, ref_slice)
+    out = dcp.dcp_sparse_atom_attention(a, p_slice, idx, w, cfg.H, cfg.c)
+    util.check_close(out, _oracle(cfg, a, p_slice, idx, w), "bf16", "knn -> gather -> sparse attention")
+    pf = dcp.dcp_gather_pair_slice(P.float(), idx)          # fp32 rows (64 bytes) gather too
+    assert torch.equal(pf, ref_slice.float())
+
+
 def test_sparse_c4_sampled_rows():
     """C4's atoms (L = 24000, c_atom 128, H 4, c 32) with the paper's budget k = 128: sampled rows vs the oracle."""
     dcp = _dcp()
