@@ -136,7 +136,6 @@ __global__ void __launch_bounds__(256) knn_kernel(const float* __restrict__ x, i
 //   3. the buffer is sorted by (d2, index) with a bitonic network and its first k entries are the answer.
 // Same distances, same (d2, index) order as knn_kernel: the result is identical.  A query whose buffer overflows
 // (more than kCap candidates within T: a very dense neighbourhood) falls back to the insertion scan over global memory.
-constexpr int kCap = 512;
 
 template <int NR>
 __device__ __noinline__ void knn_insert_global(const float* __restrict__ x, int32_t* __restrict__ idx, int L, int k, int l,
@@ -197,6 +196,8 @@ __device__ __noinline__ void knn_insert_global(const float* __restrict__ x, int3
   }
 }
 
+// kCap = candidate-buffer entries per warp; NRF = list registers per lane of the exact fallback
+template <int kCap, int NRF>
 __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict__ x, int32_t* __restrict__ idx, int L, int k) {
   extern __shared__ float smem_knn[];
   float* sx = smem_knn;
@@ -283,7 +284,7 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
   }
   if (!active) return;
   if (cnt > kCap) {                                            // very dense neighbourhood: exact fallback
-    knn_insert_global<8>(x, idx, L, k, l, lane);
+    knn_insert_global<NRF>(x, idx, L, k, l, lane);
     return;
   }
   // ---- 3. bitonic sort of the buffer by (d2, index), padded to a power of two
@@ -315,13 +316,15 @@ bool knn_supports(int64_t L, int k) { return L >= 1 && L <= 0x7fffffff && k >= 1
 cudaError_t launch_knn(const float* x, int32_t* idx, int64_t L, int k, cudaStream_t st) {
   const int nr = (k + 31) / 32;
   const unsigned blocks = (unsigned)((L + 7) / 8);
-  if (k <= 256) {   // threshold-select kernel: shared tiles (24 KB) + 8 per-warp candidate buffers (4 KB each)
-    const size_t smem = (size_t)(3 * kTile + 8 * 2 * kCap) * sizeof(float);
-    cudaError_t e = cudaFuncSetAttribute(knn_select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  // threshold-select kernel: shared tiles (24 KB) + 8 per-warp candidate buffers (8 bytes per entry)
+  if (k <= 256) {
+    const size_t smem = (size_t)(3 * kTile + 8 * 2 * 512) * sizeof(float);
+    cudaError_t e = cudaFuncSetAttribute(knn_select_kernel<512, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    knn_select_kernel<<<blocks, 256, smem, st>>>(x, idx, (int)L, k);
+    knn_select_kernel<512, 8><<<blocks, 256, smem, st>>>(x, idx, (int)L, k);
     return cudaGetLastError();
   }
+  // k > 256: the buffered candidates would outgrow shared memory too often; the register-list kernel serves them
   if (nr <= 1) knn_kernel<1><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);
   else if (nr <= 2) knn_kernel<2><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);
   else if (nr <= 4) knn_kernel<4><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);
