@@ -434,3 +434,59 @@ def test_knn_matches_kdtree_and_is_translation_invariant():
     xi = np.round(x * 8) / 8                        # multiples of 1/8: a shift by 64 is exact in binary32
     assert np.array_equal(ko.knn(xi, k), ko.knn((xi + np.float32(64.0)).astype(np.float32), k))
     assert np.array_equal(ko.knn(x, 1)[:, 0], np.arange(L))
+
+
+# ---------------------------------------------------------------- pairwise SwiGLU transition (Eq. 6, Alg. 1)
+def _transition_problem(rng, n_pairs=37, c_z=12):
+    z = rng.normal(size=(n_pairs, c_z)) * 1.5 + 0.3
+    w1 = rng.normal(size=(c_z, 4 * c_z)) / math.sqrt(c_z)
+    w2 = rng.normal(size=(c_z, 4 * c_z)) / math.sqrt(c_z)
+    w3 = rng.normal(size=(4 * c_z, c_z)) / math.sqrt(4 * c_z)
+    gamma, beta = 1 + 0.1 * rng.normal(size=c_z), 0.1 * rng.normal(size=c_z)
+    return z, w1, w2, w3, gamma, beta
+
+
+def test_transition_matches_torch_composition():
+    from oracle import pair_transition as pto
+    z, w1, w2, w3, gamma, beta = _transition_problem(np.random.default_rng(61))
+    tz = torch.from_numpy(z)
+    n = torch.nn.functional.layer_norm(tz, (z.shape[-1],), torch.from_numpy(gamma), torch.from_numpy(beta), 1e-5)
+    ref = tz + (torch.nn.functional.silu(n @ torch.from_numpy(w1)) * (n @ torch.from_numpy(w2))) @ torch.from_numpy(w3)
+    assert np.max(np.abs(pto.pair_transition(z, w1, w2, w3, gamma, beta) - ref.numpy())) <= 1e-12
+
+
+def test_transition_brute_force():
+    from oracle import pair_transition as pto
+    z, w1, w2, w3, gamma, beta = _transition_problem(np.random.default_rng(62), n_pairs=5, c_z=3)
+    got = pto.pair_transition(z, w1, w2, w3, gamma, beta)
+    c = z.shape[1]
+    for p in range(z.shape[0]):
+        row = [float(v) for v in z[p]]
+        mu = sum(row) / c
+        var = sum((v - mu) ** 2 for v in row) / c
+        n = [(row[t] - mu) / math.sqrt(var + 1e-5) * gamma[t] + beta[t] for t in range(c)]
+        h = []
+        for j in range(4 * c):
+            a = sum(n[t] * w1[t][j] for t in range(c))
+            b = sum(n[t] * w2[t][j] for t in range(c))
+            h.append(a / (1.0 + math.exp(-a)) * b)
+        for t in range(c):
+            assert abs(got[p][t] - (row[t] + sum(h[j] * w3[j][t] for j in range(4 * c)))) <= 1e-12
+
+
+def test_transition_special_cases():
+    from oracle import pair_transition as pto
+    rng = np.random.default_rng(63)
+    z, w1, w2, w3, gamma, beta = _transition_problem(rng)
+    assert np.array_equal(pto.pair_transition(z, w1, w2, 0 * w3, gamma, beta), z)          # W_3 = 0: the residual only
+    assert np.max(np.abs(pto.pair_transition(z, 0 * w1, w2, w3, gamma, beta) - z)) <= 1e-15  # SiLU(0) = 0
+    t1 = pto.pair_transition(z, w1, w2, w3, gamma, beta) - z
+    t2 = pto.pair_transition(z, w1, w2, 2.5 * w3, gamma, beta) - z
+    assert np.max(np.abs(t2 - 2.5 * t1)) <= 1e-12                                            # linear in W_3
+    perm = rng.permutation(z.shape[0])                                                       # pairs are independent
+    assert np.max(np.abs(pto.pair_transition(z[perm], w1, w2, w3, gamma, beta)
+                         - pto.pair_transition(z, w1, w2, w3, gamma, beta)[perm])) <= 1e-13
+    # LayerNorm invariance: a per-pair affine rescale of z changes only the residual term (up to the eps term)
+    zs = 3.0 * z + 7.0
+    t3 = pto.pair_transition(zs, w1, w2, w3, gamma, beta, eps=0.0) - zs
+    assert np.max(np.abs(t3 - (pto.pair_transition(z, w1, w2, w3, gamma, beta, eps=0.0) - z))) <= 1e-11
