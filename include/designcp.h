@@ -117,6 +117,18 @@ dcp_status dcp_sparse_atom_attention(const void *a, const void *p_slice, const i
                                      dcp_dtype dtype, const dcp_plan *plan, void *workspace, size_t workspace_bytes,
                                      void *stream);
 
+/* Pairwise SwiGLU transition (PAPER.md:381-385 Eq. 6, :387-409 Algorithm 1):
+ *     z_out = z + ( SiLU(LN(z) W_1) (.) LN(z) W_2 ) W_3        for every pair (row of z) independently,
+ * LN = LayerNorm over the channel axis with affine ln_gamma, ln_beta (population variance, eps; <= 0 means 1e-5).
+ *   z, z_out [n_pairs, c_z] row-major device (n_pairs = I * I for the token-pair tensor); z_out may be z (in place);
+ *   w1, w2 [c_z, 4 c_z], w3 [4 c_z, c_z] row-major device, ln_gamma, ln_beta [c_z]; all in the storage dtype, 16-byte
+ *   aligned.  Instantiated for DCP_BF16, c_z = 128 (DCP_ERR_UNSUPPORTED otherwise); n_pairs < 2^31.
+ * workspace >= dcp_pair_transition_workspace_bytes (folded weights), 256-byte aligned.  Enqueues on `stream`. */
+dcp_status dcp_pair_transition_workspace_bytes(int c_z, dcp_dtype dtype, size_t *bytes);
+dcp_status dcp_pair_transition(const void *z, void *z_out, int64_t n_pairs, int c_z, const void *w1, const void *w2,
+                               const void *w3, const void *ln_gamma, const void *ln_beta, float ln_eps, dcp_dtype dtype,
+                               void *workspace, size_t workspace_bytes, void *stream);
+
 /* p_slice[l, j, :] = p[l, idx[l, j], :] ("The relevant slice of P is gathered at those k indices"): the
  * dense atom-pair tensor p [L, L, c_atompair] (row pitch ldp elements, 0 = L * c_atompair) -> the slice
  * [L, k, c_atompair] that dcp_sparse_atom_attention consumes; slots with idx < 0 are filled with zeros.  Device

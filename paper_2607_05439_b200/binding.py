@@ -28,6 +28,7 @@ EXPORTS = [
     "dcp_workspace_bytes", "dcp_pair_bias_attention", "dcp_atom_pair_bias_attention",
     "dcp_pair_bias_attention_host", "dcp_partial_states", "dcp_merge_states", "dcp_shard_range",
     "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention", "dcp_knn", "dcp_gather_pair_slice",
+    "dcp_pair_transition_workspace_bytes", "dcp_pair_transition",
     "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
     "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
 ]
@@ -85,7 +86,9 @@ def _load() -> C.CDLL:
                                               C.POINTER(dcp_plan), vp, sz, vp]
     lib.dcp_knn.argtypes = [vp, vp, i64, i32, vp]
     lib.dcp_gather_pair_slice.argtypes = [vp, i64, vp, vp, i64, i32, i32, i32, vp]
-    for n in EXPORTS[:11]:
+    lib.dcp_pair_transition_workspace_bytes.argtypes = [i32, i32, C.POINTER(sz)]
+    lib.dcp_pair_transition.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, C.c_float, i32, vp, sz, vp]
+    for n in EXPORTS[:13]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -219,6 +222,23 @@ def dcp_pair_bias_attention(s, z, w, H, c, decomp="monolithic", parts=1, key_spl
 def dcp_atom_pair_bias_attention(a, p, w, H, c, **kw):
     """Atom-level dense variant (BASELINE.json config 4): (L, c_atom, c_atompair) for (I, c_s, c_z)."""
     return dcp_pair_bias_attention(a, p, w, H, c, atom=True, **kw)
+
+
+def dcp_pair_transition(z, w1, w2, w3, ln_gamma, ln_beta, eps=1e-5, out=None, workspace=None, stream=None):
+    """z_out = z + (SiLU(LN(z) W1) * (LN(z) W2)) W3 over the last axis of z (Eq. 6); out may be z (in place)."""
+    assert z.is_cuda and z.is_contiguous()
+    c_z = z.shape[-1]
+    n_pairs = z.numel() // c_z
+    if out is None:
+        out = torch.empty_like(z)
+    if workspace is None:
+        n = C.c_size_t(0)
+        _check(_lib.dcp_pair_transition_workspace_bytes(c_z, _dtype_code(z.dtype), C.byref(n)), "dcp_pair_transition_workspace_bytes")
+        workspace = _alloc_ws(int(n.value), z.device)
+    st = _lib.dcp_pair_transition(_ptr(z), _ptr(out), n_pairs, c_z, _ptr(w1), _ptr(w2), _ptr(w3), _ptr(ln_gamma), _ptr(ln_beta),
+                                  C.c_float(eps), _dtype_code(z.dtype), _ptr(workspace), workspace.numel(), _stream_ptr(stream))
+    _check(st, "dcp_pair_transition")
+    return out
 
 
 def dcp_gather_pair_slice(p, idx, out=None, stream=None):

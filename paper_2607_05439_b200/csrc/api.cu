@@ -450,6 +450,30 @@ dcp_status dcp_gather_pair_slice(const void* p, int64_t ldp, const int32_t* idx,
   return DCP_OK;
 }
 
+dcp_status dcp_pair_transition_workspace_bytes(int c_z, dcp_dtype dtype, size_t* bytes) {
+  if (!bytes || c_z <= 0) return DCP_ERR_INVALID_ARG;
+  if (!pair_transition_supports(dtype, c_z)) return DCP_ERR_UNSUPPORTED;
+  *bytes = align_up(pair_transition_workspace_bytes());
+  return DCP_OK;
+}
+
+dcp_status dcp_pair_transition(const void* z, void* z_out, int64_t n_pairs, int c_z, const void* w1, const void* w2,
+                               const void* w3, const void* ln_gamma, const void* ln_beta, float ln_eps, dcp_dtype dtype,
+                               void* workspace, size_t workspace_bytes, void* stream) {
+  g_launches = 0;
+  if (!z || !z_out || !w1 || !w2 || !w3 || !ln_gamma || !ln_beta || !workspace || n_pairs <= 0 || c_z <= 0)
+    return DCP_ERR_INVALID_ARG;
+  if (!pair_transition_supports(dtype, c_z)) return DCP_ERR_UNSUPPORTED;
+  if (n_pairs > 0x7fffff00ll) return DCP_ERR_INVALID_ARG;
+  if ((((uintptr_t)z | (uintptr_t)z_out | (uintptr_t)w1 | (uintptr_t)w2 | (uintptr_t)w3 | (uintptr_t)workspace) & 15) != 0)
+    return DCP_ERR_INVALID_ARG;
+  if (workspace_bytes < pair_transition_workspace_bytes()) return DCP_ERR_WORKSPACE;
+  DCP_CUDA(launch_pair_transition(z, z_out, n_pairs, w1, w2, w3, ln_gamma, ln_beta, ln_eps > 0.f ? ln_eps : 1e-5f, workspace,
+                                  (cudaStream_t)stream));
+  ++g_launches;   // the weight-fold launch
+  return DCP_OK;
+}
+
 dcp_status dcp_knn(const float* x, int32_t* idx, int64_t L, int k, void* stream) {
   g_launches = 0;
   if (!x || !idx || L <= 0 || k <= 0 || k > L) return DCP_ERR_INVALID_ARG;

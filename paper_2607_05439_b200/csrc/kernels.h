@@ -103,6 +103,13 @@ cudaError_t launch_gather_pair_slice(const void* P, int64_t ldp_bytes, const int
 bool knn_supports(int64_t L, int k);
 cudaError_t launch_knn(const float* x, int32_t* idx, int64_t L, int k, cudaStream_t st);
 
+// Pairwise SwiGLU transition z <- z + W3 (SiLU(W1 LN z) (.) W2 LN z) (pair_transition.cu)
+bool pair_transition_supports(dcp_dtype dt, int c_z);
+size_t pair_transition_workspace_bytes();
+cudaError_t launch_pair_transition(const void* z_in, void* z_out, int64_t n_pairs, const void* w1, const void* w2,
+                                   const void* w3, const void* gamma, const void* beta, float eps, void* workspace,
+                                   cudaStream_t st);
+
 // Merge (step a8) + normalise + gate (first half of a9); or raw merged state out.
 cudaError_t launch_merge(dcp_dtype dt, const MergeParams& p, cudaStream_t st);
 

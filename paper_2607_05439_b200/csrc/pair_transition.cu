@@ -1,0 +1,388 @@
+// Pairwise SwiGLU transition on the pair tensor, bf16, c_z = 128, hidden 4 c_z = 512.
+//   PAPER.md:381-385 (Eq. 6)   Transition(Z) = W_3 ( SiLU(W_1 LN(Z)) (.) W_2 LN(Z) ),  Z <- Z + Transition(Z)
+//   PAPER.md:387-409 (Alg. 1)  the memory-friendly order N, A, B, SiLU, (.), W_3, residual -- here per 128-pair tile,
+//                              so the 4 c_z-wide intermediates never leave the SM at all.
+// ~393 kflop per pair over 512 bytes of traffic (read + write z): tensor bound.
+//
+// LayerNorm is folded into the first GEMM exactly as in the attention kernels:
+//   LN(z) W = rstd (z . W' - mu c1) + c0,  W' = diag(gamma) W (bf16), c1[j] = sum_k W'[k][j], c0[j] = sum_k beta_k W[k][j]
+// so the raw z tile, as TMA wrote it (K-major, 128-byte swizzle), is the A operand, and mu / rstd are applied per row
+// by the thread that owns the row in tensor memory.
+//
+// One persistent CTA per SM, 10 warps:
+//   warp 0     TMA producer: z tiles (128 pairs x 128 ch = 32 KB, double buffered) and, per 128-wide hidden chunk c,
+//              the weight tiles W1'[:, c], W2'[:, c] (64 KB) and W3[c, :] (32 KB) -- row-major weights are MN-major B operands
+//   warp 1     tcgen05 issuer: G1(c): [A1 | A2] (128 x 256, TMEM) = z . [W1'c | W2'c]   (8 k-steps, N = 256)
+//                              G2(c): OUT (128 x 128, TMEM) += H_c . W3_c              (8 k-steps, N = 128)
+//              issued as G1(0), G1(1), G2(0), G1(2), G2(1), G1(3), G2(2), G2(3): the tensor pipe works on the next
+//              chunk while the epilogue warps turn the previous one into H
+//   warps 2-9  epilogue (TMEM lane quadrant = warp % 4, two warps per quadrant = two 64-column halves): per chunk
+//              tcgen05.ld A1, A2 -> a = rstd (A - mu c1) + c0 -> h = SiLU(a1) a2 -> bf16 -> the H tile in shared memory
+//              (K-major, 128-byte swizzle by hand: the A operand of G2); per tile OUT + z -> bf16 -> TMA store.
+#include "kernels.h"
+#include "mma_ptx.cuh"
+
+namespace dcp {
+
+namespace {
+
+constexpr int tCz = 128, tHid = 512, tNC = 128, tChunks = tHid / tNC, tM = 128;
+constexpr int tThreads = 64 + 256;
+constexpr int tZBytes = tM * tCz * 2;          // 32 KB, two 64-channel halves of 16 KB
+constexpr int tW12Bytes = 2 * tCz * tNC * 2;   // 64 KB: per k-block of 64: [W1 n-half 0][W1 n-half 1][W2 n-half 0][W2 n-half 1]
+constexpr int tW3Bytes = tNC * tCz * 2;        // 32 KB: per k-block of 64: [n-half 0][n-half 1]
+constexpr int tHBytes = tM * tNC * 2;          // 32 KB
+constexpr size_t tSmemZ = 0;
+constexpr size_t tSmemW12 = tSmemZ + 2 * (size_t)tZBytes;
+constexpr size_t tSmemW3 = tSmemW12 + tW12Bytes;
+constexpr size_t tSmemH = tSmemW3 + tW3Bytes;
+constexpr size_t tSmemC = tSmemH + tHBytes;                 // float4 {c1_1, c0_1, c1_2, c0_2} per hidden unit: 8 KB
+constexpr size_t tSmemBar = tSmemC + (size_t)tHid * 16;
+constexpr size_t tSmemAlloc = tSmemBar + 16 * 8 + 16 + 1024;
+constexpr int tColA1 = 0, tColOut = 256;                    // TMEM columns: A1 [0,128) A2 [128,256) OUT [256,384)
+
+struct TransMaps {
+  CUtensorMap z_in, z_out, w1, w2, w3;
+};
+
+// MN-major B tile, 128-byte swizzle, 64-n blocks `lbo` bytes apart, 8-k-row atoms 1024 B apart
+__device__ __forceinline__ uint64_t umma_desc_mn(uint32_t addr, uint32_t lbo) {
+  return (uint64_t)((addr & 0x3ffffu) >> 4) | ((uint64_t)(lbo >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) |
+         ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+__device__ __forceinline__ void tma_load_2d_t(uint32_t dst, const CUtensorMap* tmap, int c0, int c1, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+               ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* tmap, int c0, int c1, uint32_t src) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+               ::"l"(tmap), "r"(c0), "r"(c1), "r"(src) : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+      "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ float tanh_fast(float x) {
+  float y;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// acc_s += lo(w) + hi(w), acc_q += lo(w)^2 + hi(w)^2  (bf16x2 word, mixed-precision FMAs)
+__device__ __forceinline__ void stats_bf16x2(float& acc_s, float& acc_q, uint32_t w) {
+  asm("{\n\t.reg .b16 l, h, o;\n\t"
+      "mov.b32 {l, h}, %2;\n\t"
+      "mov.b16 o, 0x3f80;\n\t"
+      "fma.rn.f32.bf16 %0, l, o, %0;\n\t"
+      "fma.rn.f32.bf16 %0, h, o, %0;\n\t"
+      "fma.rn.f32.bf16 %1, l, l, %1;\n\t"
+      "fma.rn.f32.bf16 %1, h, h, %1;\n\t}"
+      : "+f"(acc_s), "+f"(acc_q) : "r"(w));
+}
+
+__global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __grid_constant__ TransMaps maps,
+                                                                      const float4* __restrict__ consts, int64_t n_pairs,
+                                                                      float eps) {
+  extern __shared__ unsigned char smem_dyn[];
+  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
+  const uint32_t s_z = smem_u32(smem + tSmemZ), s_w12 = smem_u32(smem + tSmemW12), s_w3 = smem_u32(smem + tSmemW3);
+  const uint32_t s_h = smem_u32(smem + tSmemH), s_bar = smem_u32(smem + tSmemBar);
+  float4* s_c = reinterpret_cast<float4*>(smem + tSmemC);
+  // barriers
+  const uint32_t b_zfull = s_bar, b_zempty = s_bar + 16, b_w12full = s_bar + 32, b_w12empty = s_bar + 40, b_w3full = s_bar + 48,
+                 b_w3empty = s_bar + 56, b_afull = s_bar + 64, b_aempty = s_bar + 72, b_hfull = s_bar + 80,
+                 b_hempty = s_bar + 88, b_ofull = s_bar + 96, b_oempty = s_bar + 104;
+  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + tSmemBar + 16 * 8);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int b = 0; b < 2; ++b) { mbar_init(b_zfull + 8 * b, 1); mbar_init(b_zempty + 8 * b, 8); }
+    mbar_init(b_w12full, 1); mbar_init(b_w12empty, 1); mbar_init(b_w3full, 1); mbar_init(b_w3empty, 1);
+    mbar_init(b_afull, 1); mbar_init(b_aempty, 8); mbar_init(b_hfull, 8); mbar_init(b_hempty, 1);
+    mbar_init(b_ofull, 1); mbar_init(b_oempty, 8);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  for (int e = threadIdx.x; e < tHid; e += tThreads) s_c[e] = __ldg(consts + e);
+  if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), 512);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *s_tmem;
+  const int64_t n_tiles = (n_pairs + tM - 1) / tM;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      // =============================================================== TMA producer
+      uint32_t n12 = 0, n3 = 0;
+      auto load_z = [&](int64_t tile, int it) {
+        const int zb = it & 1;
+        mbar_wait(b_zempty + 8 * zb, ((it >> 1) & 1) ^ 1);
+        mbar_expect_tx(b_zfull + 8 * zb, tZBytes);
+        tma_load_2d_t(s_z + zb * tZBytes, &maps.z_in, 0, (int)(tile * tM), b_zfull + 8 * zb);
+        tma_load_2d_t(s_z + zb * tZBytes + tZBytes / 2, &maps.z_in, 64, (int)(tile * tM), b_zfull + 8 * zb);
+      };
+      int it = 0;
+      if ((int64_t)blockIdx.x < n_tiles) load_z(blockIdx.x, 0);
+      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        for (int c = 0; c < tChunks; ++c) {
+          mbar_wait(b_w12empty, (n12 & 1) ^ 1);
+          mbar_expect_tx(b_w12full, tW12Bytes);
+#pragma unroll
+          for (int kb = 0; kb < 2; ++kb)
+#pragma unroll
+            for (int nh = 0; nh < 2; ++nh) {
+              tma_load_2d_t(s_w12 + kb * 32768 + nh * 8192, &maps.w1, c * tNC + 64 * nh, 64 * kb, b_w12full);
+              tma_load_2d_t(s_w12 + kb * 32768 + 16384 + nh * 8192, &maps.w2, c * tNC + 64 * nh, 64 * kb, b_w12full);
+            }
+          ++n12;
+          mbar_wait(b_w3empty, (n3 & 1) ^ 1);
+          mbar_expect_tx(b_w3full, tW3Bytes);
+#pragma unroll
+          for (int kb = 0; kb < 2; ++kb)
+#pragma unroll
+            for (int nh = 0; nh < 2; ++nh)
+              tma_load_2d_t(s_w3 + kb * 16384 + nh * 8192, &maps.w3, 64 * nh, c * tNC + 64 * kb, b_w3full);
+          ++n3;
+          if (c == 1 && tile + gridDim.x < n_tiles) load_z(tile + gridDim.x, it + 1);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      // =============================================================== tcgen05 issuer
+      constexpr uint32_t idesc1 = umma_idesc_bf16(tM, 256) | (1u << 16);     // B MN-major
+      constexpr uint32_t idesc2 = umma_idesc_bf16(tM, 128) | (1u << 16);
+      uint32_t n12 = 0, n3 = 0, na = 0, nh = 0, nout = 0;
+      int it = 0;
+      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int zb = it & 1;
+        const uint32_t zs = s_z + zb * tZBytes;
+        mbar_wait(b_zfull + 8 * zb, (it >> 1) & 1);
+        auto g1 = [&]() {
+          mbar_wait(b_w12full, n12 & 1);
+          mbar_wait(b_aempty, (na & 1) ^ 1);
+          tc_fence_after();
+#pragma unroll
+          for (int ks = 0; ks < 8; ++ks)
+            umma_bf16(tmem_base + tColA1, umma_desc_sw128(zs + (ks >> 2) * (tZBytes / 2) + (ks & 3) * 32),
+                      umma_desc_mn(s_w12 + (ks >> 2) * 32768 + (ks & 3) * 2048, 8192), idesc1, ks != 0);
+          umma_commit(b_afull);
+          umma_commit(b_w12empty);
+          ++n12; ++na;
+        };
+        auto g2 = [&](int c) {
+          mbar_wait(b_hfull, nh & 1);
+          mbar_wait(b_w3full, n3 & 1);
+          if (c == 0) mbar_wait(b_oempty, (nout & 1) ^ 1);
+          tc_fence_after();
+#pragma unroll
+          for (int ks = 0; ks < 8; ++ks)
+            umma_bf16(tmem_base + tColOut, umma_desc_sw128(s_h + (ks >> 2) * (tHBytes / 2) + (ks & 3) * 32),
+                      umma_desc_mn(s_w3 + (ks >> 2) * 16384 + (ks & 3) * 2048, 8192), idesc2, (c | ks) != 0);
+          umma_commit(b_hempty);
+          umma_commit(b_w3empty);
+          if (c == tChunks - 1) { umma_commit(b_ofull); ++nout; }
+          ++nh; ++n3;
+        };
+        g1();
+        for (int c = 0; c < tChunks; ++c) {
+          if (c + 1 < tChunks) g1();
+          g2(c);
+        }
+      }
+    }
+  } else {
+    // =============================================================== epilogue warps
+    const int quad = warp & 3, half = (warp - 2) >> 2, et = threadIdx.x - 64;
+    const int r = quad * 32 + lane;                         // tile row = TMEM lane of this thread
+    const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16);
+    const uint32_t sw = (uint32_t)(r & 7);
+    uint32_t na = 0, nh = 0, nout = 0;
+    int it = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      const int zb = it & 1;
+      const uint32_t zrow = s_z + zb * tZBytes + r * 128;   // row base inside a 64-channel half
+      mbar_wait(b_zfull + 8 * zb, (it >> 1) & 1);
+      // ---- LayerNorm statistics of the thread's pair (fp32): mu = sum / c_z, var = sum z^2 / c_z - mu^2
+      float sm = 0.f, sq = 0.f;
+#pragma unroll
+      for (int hf = 0; hf < 2; ++hf)
+#pragma unroll
+        for (int ch = 0; ch < 8; ++ch) {
+          const uint4 w = lds_u32x4(zrow + hf * (tZBytes / 2) + ((ch ^ sw) << 4));
+          stats_bf16x2(sm, sq, w.x); stats_bf16x2(sm, sq, w.y); stats_bf16x2(sm, sq, w.z); stats_bf16x2(sm, sq, w.w);
+        }
+      const float mu = sm * (1.f / tCz);
+      const float rstd = rsqrtf(fmaxf(fmaf(sq, 1.f / tCz, -mu * mu), 0.f) + eps);
+      const float nm = -mu * rstd;
+
+      for (int c = 0; c < tChunks; ++c) {
+        mbar_wait(b_afull, na & 1);
+        tc_fence_after();
+        uint32_t hw[32];                                     // the thread's 64 h values of this chunk, bf16x2
+#pragma unroll
+        for (int sb = 0; sb < 2; ++sb) {
+          uint32_t a1[32], a2[32];
+          tmem_ld32(t_lane + tColA1 + half * 64 + sb * 32, a1);
+          tmem_ld32(t_lane + tColA1 + 128 + half * 64 + sb * 32, a2);
+          tmem_ld_wait();
+          if (sb == 1) {                                     // A1 / A2 are in registers: the next G1 may overwrite them
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(b_aempty);
+          }
+#pragma unroll
+          for (int i = 0; i < 32; i += 2) {
+            float hv[2];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+              const float4 k = s_c[c * tNC + half * 64 + sb * 32 + i + e];     // {c1_1, c0_1, c1_2, c0_2}: broadcast read
+              const float x1 = fmaf(__uint_as_float(a1[i + e]), rstd, fmaf(nm, k.x, k.y));
+              const float x2 = fmaf(__uint_as_float(a2[i + e]), rstd, fmaf(nm, k.z, k.w));
+              // SiLU(x) = x sigmoid(x) = 0.5 x (1 + tanh(x / 2))
+              const float hx = 0.5f * x1;
+              hv[e] = fmaf(hx, tanh_fast(hx), hx) * x2;
+            }
+            hw[sb * 16 + (i >> 1)] = pack_bf16(hv[0], hv[1]);
+          }
+        }
+        ++na;
+        // ---- H tile (the A operand of G2): row r of the 64-column k-half `half`, 128-byte swizzle
+        mbar_wait(b_hempty, (nh & 1) ^ 1);                   // G2 of the previous chunk has finished reading H
+        const uint32_t hrow = s_h + half * (tHBytes / 2) + r * 128;
+#pragma unroll
+        for (int ch = 0; ch < 8; ++ch)
+          asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(hrow + ((ch ^ sw) << 4)), "r"(hw[4 * ch]),
+                       "r"(hw[4 * ch + 1]), "r"(hw[4 * ch + 2]), "r"(hw[4 * ch + 3]) : "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(b_hfull);
+        ++nh;
+      }
+
+      // ---- residual: z + OUT -> bf16 -> staging tile (the H buffer, same swizzled layout) -> TMA store
+      mbar_wait(b_ofull, nout & 1);
+      tc_fence_after();
+      uint32_t ow[32];
+#pragma unroll
+      for (int sb = 0; sb < 2; ++sb) {
+        uint32_t o[32];
+        tmem_ld32(t_lane + tColOut + half * 64 + sb * 32, o);
+        tmem_ld_wait();
+        if (sb == 1) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(b_oempty);
+        }
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          const uint4 zv = lds_u32x4(zrow + half * (tZBytes / 2) + (((sb * 4 + ch) ^ sw) << 4));
+          const uint32_t zw[4] = {zv.x, zv.y, zv.z, zv.w};
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const float z0 = __uint_as_float(zw[q] << 16), z1 = __uint_as_float(zw[q] & 0xffff0000u);
+            ow[sb * 16 + ch * 4 + q] = pack_bf16(z0 + __uint_as_float(o[ch * 8 + 2 * q]), z1 + __uint_as_float(o[ch * 8 + 2 * q + 1]));
+          }
+        }
+      }
+      ++nout;
+      // out_full implies that every G2 of the tile is complete, so the H buffer is free for staging
+      const uint32_t orow = s_h + half * (tHBytes / 2) + r * 128;
+#pragma unroll
+      for (int ch = 0; ch < 8; ++ch)
+        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(orow + ((ch ^ sw) << 4)), "r"(ow[4 * ch]),
+                     "r"(ow[4 * ch + 1]), "r"(ow[4 * ch + 2]), "r"(ow[4 * ch + 3]) : "memory");
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      __syncwarp();
+      if (lane == 0) mbar_arrive(b_zempty + 8 * zb);          // this warp is done with the z tile
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      if (et == 0) {
+        tma_store_2d(&maps.z_out, 0, (int)(tile * tM), s_h);
+        tma_store_2d(&maps.z_out, 64, (int)(tile * tM), s_h + tHBytes / 2);
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the staging tile has been read
+      }
+      asm volatile("bar.sync 1, 256;" ::: "memory");          // ... before the next tile's chunk 0 overwrites it
+    }
+    if (et == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    __syncwarp();
+    tmem_dealloc(tmem_base, 512);
+  }
+}
+
+// W'[k][j] = bf16(gamma_k W[k][j]) for W1 and W2, consts[j] = {sum_k W1'[k][j], sum_k beta_k W1[k][j], same for W2}
+__global__ void __launch_bounds__(128) transition_fold_kernel(const __nv_bfloat16* __restrict__ w1, const __nv_bfloat16* __restrict__ w2,
+                                                             const __nv_bfloat16* __restrict__ gamma, const __nv_bfloat16* __restrict__ beta,
+                                                             __nv_bfloat16* __restrict__ w1f, __nv_bfloat16* __restrict__ w2f,
+                                                             float4* __restrict__ consts) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= tHid) return;
+  float c11 = 0.f, c01 = 0.f, c12 = 0.f, c02 = 0.f;
+  for (int k = 0; k < tCz; ++k) {
+    const float g = to_f32(gamma[k]), b = to_f32(beta[k]);
+    const float a = to_f32(w1[k * tHid + j]), c = to_f32(w2[k * tHid + j]);
+    const __nv_bfloat16 af = __float2bfloat16_rn(g * a), cf = __float2bfloat16_rn(g * c);
+    w1f[k * tHid + j] = af;
+    w2f[k * tHid + j] = cf;
+    c11 += to_f32(af); c12 += to_f32(cf);
+    c01 = fmaf(b, a, c01); c02 = fmaf(b, c, c02);
+  }
+  consts[j] = make_float4(c11, c01, c12, c02);
+}
+
+CUresult encode2d(PFN_cuTensorMapEncodeTiled enc, CUtensorMap* m, const void* base, uint64_t d0, uint64_t d1, uint32_t b0,
+                  uint32_t b1) {
+  const cuuint64_t gdim[2] = {d0, d1};
+  const cuuint64_t gstr[1] = {d0 * 2};
+  const cuuint32_t box[2] = {b0, b1};
+  const cuuint32_t estr[2] = {1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstr, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+}
+
+}  // namespace
+
+bool pair_transition_supports(dcp_dtype dt, int c_z) { return dt == DCP_BF16 && c_z == tCz; }
+size_t pair_transition_workspace_bytes() { return (size_t)2 * tCz * tHid * 2 + (size_t)tHid * 16; }
+
+cudaError_t launch_pair_transition(const void* z_in, void* z_out, int64_t n_pairs, const void* w1, const void* w2,
+                                   const void* w3, const void* gamma, const void* beta, float eps, void* workspace,
+                                   cudaStream_t st) {
+  if (n_pairs <= 0) return cudaSuccess;
+  PFN_cuTensorMapEncodeTiled enc = get_encode_fn();
+  if (!enc) return cudaErrorNotSupported;
+  __nv_bfloat16* w1f = reinterpret_cast<__nv_bfloat16*>(workspace);
+  __nv_bfloat16* w2f = w1f + tCz * tHid;
+  float4* consts = reinterpret_cast<float4*>(w2f + tCz * tHid);
+  transition_fold_kernel<<<tHid / 128, 128, 0, st>>>((const __nv_bfloat16*)w1, (const __nv_bfloat16*)w2,
+                                                     (const __nv_bfloat16*)gamma, (const __nv_bfloat16*)beta, w1f, w2f, consts);
+  TransMaps maps;
+  if (encode2d(enc, &maps.z_in, z_in, tCz, (uint64_t)n_pairs, 64, tM) != CUDA_SUCCESS ||
+      encode2d(enc, &maps.z_out, z_out, tCz, (uint64_t)n_pairs, 64, tM) != CUDA_SUCCESS ||
+      encode2d(enc, &maps.w1, w1f, tHid, tCz, 64, 64) != CUDA_SUCCESS ||
+      encode2d(enc, &maps.w2, w2f, tHid, tCz, 64, 64) != CUDA_SUCCESS ||
+      encode2d(enc, &maps.w3, w3, tCz, tHid, 64, 64) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  cudaError_t e = cudaFuncSetAttribute(pair_transition_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tSmemAlloc);
+  if (e != cudaSuccess) return e;
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (sms <= 0) sms = 148;
+  const int64_t n_tiles = (n_pairs + tM - 1) / tM;
+  const unsigned grid = (unsigned)(n_tiles < sms ? n_tiles : sms);
+  pair_transition_kernel<<<grid, tThreads, tSmemAlloc, st>>>(maps, consts, n_pairs, eps);
+  return cudaGetLastError();
+}
+
+}  // namespace dcp
