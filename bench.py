@@ -46,9 +46,10 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4", "K4"],
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4", "K4", "T2", "T3"],
                     help="C0..C4: BASELINE.json configs (dense layer); S4: sparse k-neighbour atom attention on C4's atoms; "
-                         "K4: the k-nearest-neighbour lists of C4's atoms (dcp_knn)")
+                         "K4: the k-nearest-neighbour lists of C4's atoms (dcp_knn); T2 / T3: the pairwise SwiGLU transition on "
+                         "C2's / C3's pair tensor (dcp_pair_transition)")
     ap.add_argument("--neighbours", type=int, default=128, help="S4: budget k (PAPER.md:303 default 128)")
     ap.add_argument("--decomp", default="monolithic", choices=["monolithic", "row", "grid"])
     ap.add_argument("--parts", type=int, default=0, help="row stripes / grid cells (0: 8 rows, 16 grid)")
@@ -334,6 +335,112 @@ def run_reference_sparse(args):
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}), flush=True)
 
 
+def run_transition(args, rank, world, local_rank):
+    """--workload T2 | T3: z <- z + W3 (SiLU(W1 LN z) (.) W2 LN z) on C2's (I = 3000) or C3's
+    (I = 12000) pair tensor, c_z = 128, bf16, in place.  One pair = one row of z; tensor bound (393 kflop per pair)."""
+    import math
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as ge
+    if rank == 0 or world == 1:
+        ge.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    import dcp_synth as syn
+    import paper_2607_05439_b200 as dcp
+    from oracle import pair_transition as pto
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    cfg = replica_config(syn.CONFIGS["C2" if args.workload == "T2" else "C3"], rank, world)
+    c_z = cfg.c_z
+    g = torch.Generator(device="cpu").manual_seed(cfg.seed * 1000003 + 31)
+    rn = lambda *s, std=1.0: (torch.randn(*s, generator=g) * std).to(torch.bfloat16).to(dev)
+    w = (rn(c_z, 4 * c_z, std=1 / math.sqrt(c_z)), rn(c_z, 4 * c_z, std=1 / math.sqrt(c_z)),
+         rn(4 * c_z, c_z, std=1 / math.sqrt(4 * c_z)), (1 + 0.1 * torch.randn(c_z, generator=g)).to(torch.bfloat16).to(dev),
+         (0.1 * torch.randn(c_z, generator=g)).to(torch.bfloat16).to(dev))
+    z = syn.make_z(cfg, dev)
+    out = torch.empty_like(z)
+    n_pairs = float(cfg.I) * cfg.I
+    for _ in range(max(args.warmup, 3)):
+        dcp.dcp_pair_transition(z, *w, out=out)
+    launches = dcp.dcp_last_launch_count()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = dcp.Event(), dcp.Event()
+    e0.record()
+    for _ in range(args.steps):
+        dcp.dcp_pair_transition(z, *w, out=out)
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = max_over_ranks_ms(e0.elapsed_ms(e1), world, dev)
+    kms = total_ms / args.steps
+    value = n_pairs * args.steps * world / (total_ms * 1e-3) / 1e9
+    flops = n_pairs * (2.0 * c_z * 4 * c_z * 2 + 2.0 * 4 * c_z * c_z)       # 393216 per pair
+    with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+        pk = json.load(f)
+    peak_tf = float(pk["bf16_tflops_sustained" if kms > 2.0 else "bf16_tflops"])
+    roofline = {"bound": "tensor", "achieved": flops / (kms * 1e-3) / 1e12, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": flops / (kms * 1e-3) / 1e12 / peak_tf, "traffic": None, "kernel": "pair_transition_kernel",
+                "peak_source": "measured (MEASURED_PEAKS.json, cuBLAS bf16 8192^3: sustained for a > 2 ms kernel, else burst)",
+                "kernel_ms": kms, "kernel_share_of_step": 1.0, "algorithmic_flops_per_launch": flops,
+                "hbm_bytes_per_launch": n_pairs * c_z * 2 * 2, "hbm_gbs": n_pairs * c_z * 4 / (kms * 1e-3) / 1e9}
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        n_s = args.cpu_rows or 200000
+        idx = torch.randint(0, cfg.I * cfg.I, (n_s,), generator=torch.Generator().manual_seed(1)).to(dev)
+        zs = z.reshape(-1, c_z).index_select(0, idx)
+        f64 = lambda t: t.detach().float().cpu().double().numpy()
+        z64, w64 = f64(zs), [f64(t) for t in w]
+        t0 = time.perf_counter()
+        ref = pto.pair_transition(z64, *w64)
+        dt = time.perf_counter() - t0
+        got = f64(out.reshape(-1, c_z).index_select(0, idx))
+        cpu = {"value": n_s / dt / 1e9, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+               "sample": f"{n_s} sampled pairs ({dt:.1f} s), fp64 numpy oracle",
+               "gpu_vs_oracle_rel_l2_on_sample": float(np.linalg.norm(got - ref) / np.linalg.norm(ref)),
+               "gpu_vs_oracle_max_abs_on_sample": float(np.abs(got - ref).max()),
+               "gpu_vs_oracle_within_tolerance": bool(np.all(np.abs(got - ref) <= 2e-2 + 2.0 ** -8 * np.abs(ref))),
+               "tolerance": "rel-L2 <= 1e-2 and |got - ref| <= 2e-2 + 2^-8 |ref| (bf16 output of z + update, DESIGN.md 6.6)"}
+    e2e = None
+    if not args.no_e2e and args.workload == "T2":
+        zh, oh = z.cpu().pin_memory(), torch.empty(z.shape, dtype=z.dtype).pin_memory()
+        zd = torch.empty_like(z)
+        ne = max(1, args.e2e_steps)
+        a, b = dcp.Event(), dcp.Event()
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(ne):
+            zd.copy_(zh, non_blocking=True)
+            dcp.dcp_pair_transition(zd, *w, out=zd)
+            oh.copy_(zd, non_blocking=True)
+        b.record()
+        torch.cuda.synchronize()
+        ms = max_over_ranks_ms(a.elapsed_ms(b), world, dev)
+        e2e = {"value": n_pairs * ne * world / (ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": zh.numel() * 2,
+               "d2h_bytes_per_step": oh.numel() * 2, "steps": ne, "note": "PCIe copies of z in both directions dominate"}
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": kms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic",
+            "config": {"workload": f"{args.workload}: pairwise SwiGLU transition on the pair tensor I={cfg.I} c_z={c_z} hidden={4 * c_z} "
+                                   f"bf16 (icosahedral 60 x {cfg.n_res})", "pair": "one row of z (one token pair)",
+                       "kernel": "pair_transition_kernel", "l2": "z (%.0f MB) larger than the 126 MB L2: no flush needed" % (z.numel() * 2 / 1e6),
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "peak_device_bytes": int(torch.cuda.max_memory_allocated())},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches * (args.steps + max(args.warmup, 3)),
+            "clocks": clocks}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_knn(args, rank, world, local_rank):
     """--workload K4: neighbour lists of C4's 24000 synthetic atoms, k = --neighbours.
     One pair = one (query atom, candidate atom) distance: L^2 per call.  Single GPU (or independent replicas)."""
@@ -574,6 +681,9 @@ def main():
         return
     if args.workload == "K4":
         run_knn(args, rank, world, local_rank)
+        return
+    if args.workload in ("T2", "T3"):
+        run_transition(args, rank, world, local_rank)
         return
 
     import torch
