@@ -4,10 +4,11 @@
 //                              so the 4 c_z-wide intermediates never leave the SM at all.
 // ~393 kflop per pair over 512 bytes of traffic (read + write z): tensor bound.
 //
-// LayerNorm is folded into the first GEMM exactly as in the attention kernels:
-//   LN(z) W = rstd (z . W' - mu c1) + c0,  W' = diag(gamma) W (bf16), c1[j] = sum_k W'[k][j], c0[j] = sum_k beta_k W[k][j]
-// so the raw z tile, as TMA wrote it (K-major, 128-byte swizzle), is the A operand, and mu / rstd are applied per row
-// by the thread that owns the row in tensor memory.
+// LayerNorm is folded into the first GEMM:
+//   LN(z) W = rstd (z . W' - mu c1 + (1 / rstd) c0),  W' = diag(gamma) W, c1[j] = sum_k W'[k][j], c0[j] = sum_k beta_k W[k][j]
+// The raw z tile, as TMA wrote it (K-major, 128-byte swizzle), is the A operand of 8 k-steps; a ninth k-step multiplies
+// the K extension [-mu, 1 / rstd, 0 ...] (written per row by the epilogue warps) with the weight rows [c1; c0; 0 ...],
+// so the accumulator only has to be scaled by the row's rstd: no per-column constants in the epilogue.
 //
 // One persistent CTA per SM, 10 warps:
 //   warp 0     TMA producer: z tiles (128 pairs x 128 ch = 32 KB, double buffered) and, per 128-wide hidden chunk c,
@@ -32,18 +33,28 @@ constexpr int tZBytes = tM * tCz * 2;          // 32 KB, two 64-channel halves o
 constexpr int tW12Bytes = 2 * tCz * tNC * 2;   // 64 KB: per k-block of 64: [W1 n-half 0][W1 n-half 1][W2 n-half 0][W2 n-half 1]
 constexpr int tW3Bytes = tNC * tCz * 2;        // 32 KB: per k-block of 64: [n-half 0][n-half 1]
 constexpr int tHBytes = tM * tNC * 2;          // 32 KB
+constexpr int tKx = 16;                        // the K extension: channels 128 (-mu), 129 (1 / rstd), 130..143 (zero)
+constexpr int tZxBytes = tM * tKx * 2;         // 4 KB per z buffer, K-major, 32-byte swizzle
+constexpr int tW12xBytes = 4 * 64 * tKx * 2;   // 8 KB: rows k = 128..143 of [W1'c | W2'c], four 64-n blocks of 2 KB
 constexpr size_t tSmemZ = 0;
 constexpr size_t tSmemW12 = tSmemZ + 2 * (size_t)tZBytes;
 constexpr size_t tSmemW3 = tSmemW12 + tW12Bytes;
 constexpr size_t tSmemH = tSmemW3 + tW3Bytes;
-constexpr size_t tSmemC = tSmemH + tHBytes;                 // float4 {c1_1, c0_1, c1_2, c0_2} per hidden unit: 8 KB
-constexpr size_t tSmemBar = tSmemC + (size_t)tHid * 16;
+constexpr size_t tSmemZx = tSmemH + tHBytes;
+constexpr size_t tSmemW12x = tSmemZx + 2 * (size_t)tZxBytes;
+constexpr size_t tSmemBar = tSmemW12x + tW12xBytes;
 constexpr size_t tSmemAlloc = tSmemBar + 16 * 8 + 16 + 1024;
 constexpr int tColA1 = 0, tColOut = 256;                    // TMEM columns: A1 [0,128) A2 [128,256) OUT [256,384)
 
 struct TransMaps {
-  CUtensorMap z_in, z_out, w1, w2, w3;
+  CUtensorMap z_in, z_out, w1, w2, w3, w1x, w2x;   // w1x / w2x: the same folded weights with a (64 n, 16 k) box
 };
+
+// K-major A tile, 32-byte swizzle (rows of 16 bf16, 8-row groups 256 B apart): the K extension of the z tile
+__device__ __forceinline__ uint64_t umma_desc_k_sw32(uint32_t addr) {
+  return (uint64_t)((addr & 0x3ffffu) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(256 >> 4) << 32) | ((uint64_t)1 << 46) |
+         ((uint64_t)6 << 61);
+}
 
 // MN-major B tile, 128-byte swizzle, 64-n blocks `lbo` bytes apart, 8-k-row atoms 1024 B apart
 __device__ __forceinline__ uint64_t umma_desc_mn(uint32_t addr, uint32_t lbo) {
@@ -86,17 +97,16 @@ __device__ __forceinline__ void stats_bf16x2(float& acc_s, float& acc_q, uint32_
 }
 
 __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __grid_constant__ TransMaps maps,
-                                                                      const float4* __restrict__ consts, int64_t n_pairs,
-                                                                      float eps) {
+                                                                      int64_t n_pairs, float eps) {
   extern __shared__ unsigned char smem_dyn[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
   const uint32_t s_z = smem_u32(smem + tSmemZ), s_w12 = smem_u32(smem + tSmemW12), s_w3 = smem_u32(smem + tSmemW3);
   const uint32_t s_h = smem_u32(smem + tSmemH), s_bar = smem_u32(smem + tSmemBar);
-  float4* s_c = reinterpret_cast<float4*>(smem + tSmemC);
+  const uint32_t s_zx = smem_u32(smem + tSmemZx), s_w12x = smem_u32(smem + tSmemW12x);
   // barriers
   const uint32_t b_zfull = s_bar, b_zempty = s_bar + 16, b_w12full = s_bar + 32, b_w12empty = s_bar + 40, b_w3full = s_bar + 48,
                  b_w3empty = s_bar + 56, b_afull = s_bar + 64, b_aempty = s_bar + 72, b_hfull = s_bar + 80,
-                 b_hempty = s_bar + 88, b_ofull = s_bar + 96, b_oempty = s_bar + 104;
+                 b_hempty = s_bar + 88, b_ofull = s_bar + 96, b_oempty = s_bar + 104, b_xfull = s_bar + 112;   // b_xfull: 2 barriers
   volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + tSmemBar + 16 * 8);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -105,9 +115,9 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
     mbar_init(b_w12full, 1); mbar_init(b_w12empty, 1); mbar_init(b_w3full, 1); mbar_init(b_w3empty, 1);
     mbar_init(b_afull, 1); mbar_init(b_aempty, 8); mbar_init(b_hfull, 8); mbar_init(b_hempty, 1);
     mbar_init(b_ofull, 1); mbar_init(b_oempty, 8);
+    mbar_init(b_xfull, 4); mbar_init(b_xfull + 8, 4);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  for (int e = threadIdx.x; e < tHid; e += tThreads) s_c[e] = __ldg(consts + e);
   if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), 512);
   tc_fence_before();
   __syncthreads();
@@ -131,7 +141,7 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
       for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
         for (int c = 0; c < tChunks; ++c) {
           mbar_wait(b_w12empty, (n12 & 1) ^ 1);
-          mbar_expect_tx(b_w12full, tW12Bytes);
+          mbar_expect_tx(b_w12full, tW12Bytes + tW12xBytes);
 #pragma unroll
           for (int kb = 0; kb < 2; ++kb)
 #pragma unroll
@@ -139,6 +149,11 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
               tma_load_2d_t(s_w12 + kb * 32768 + nh * 8192, &maps.w1, c * tNC + 64 * nh, 64 * kb, b_w12full);
               tma_load_2d_t(s_w12 + kb * 32768 + 16384 + nh * 8192, &maps.w2, c * tNC + 64 * nh, 64 * kb, b_w12full);
             }
+#pragma unroll
+          for (int nh = 0; nh < 2; ++nh) {
+            tma_load_2d_t(s_w12x + nh * 2048, &maps.w1x, c * tNC + 64 * nh, tCz, b_w12full);
+            tma_load_2d_t(s_w12x + 4096 + nh * 2048, &maps.w2x, c * tNC + 64 * nh, tCz, b_w12full);
+          }
           ++n12;
           mbar_wait(b_w3empty, (n3 & 1) ^ 1);
           mbar_expect_tx(b_w3full, tW3Bytes);
@@ -163,6 +178,7 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
         const int zb = it & 1;
         const uint32_t zs = s_z + zb * tZBytes;
         mbar_wait(b_zfull + 8 * zb, (it >> 1) & 1);
+        mbar_wait(b_xfull + 8 * zb, (it >> 1) & 1);          // the epilogue has written this tile's K extension
         auto g1 = [&]() {
           mbar_wait(b_w12full, n12 & 1);
           mbar_wait(b_aempty, (na & 1) ^ 1);
@@ -171,6 +187,7 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
           for (int ks = 0; ks < 8; ++ks)
             umma_bf16(tmem_base + tColA1, umma_desc_sw128(zs + (ks >> 2) * (tZBytes / 2) + (ks & 3) * 32),
                       umma_desc_mn(s_w12 + (ks >> 2) * 32768 + (ks & 3) * 2048, 8192), idesc1, ks != 0);
+          umma_bf16(tmem_base + tColA1, umma_desc_k_sw32(s_zx + zb * tZxBytes), umma_desc_mn(s_w12x, 2048), idesc1, 1);
           umma_commit(b_afull);
           umma_commit(b_w12empty);
           ++n12; ++na;
@@ -203,12 +220,13 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
     const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16);
     const uint32_t sw = (uint32_t)(r & 7);
     uint32_t na = 0, nh = 0, nout = 0;
-    int it = 0;
-    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-      const int zb = it & 1;
-      const uint32_t zrow = s_z + zb * tZBytes + r * 128;   // row base inside a 64-channel half
-      mbar_wait(b_zfull + 8 * zb, (it >> 1) & 1);
-      // ---- LayerNorm statistics of the thread's pair (fp32): mu = sum / c_z, var = sum z^2 / c_z - mu^2
+    // LayerNorm statistics of the thread's pair of tile number `jt` (fp32: mu = sum / c_z, var = sum z^2 / c_z - mu^2)
+    // and the K extension row [-mu, 1 / rstd, 0 ...] of that z buffer (32-byte swizzle: 16-byte chunk ^ bit 2 of the
+    // row); returns rstd.  Called one tile ahead, so that the issuer never waits for it.
+    auto prepare = [&](int jt) -> float {
+      const int zb = jt & 1;
+      const uint32_t zrow = s_z + zb * tZBytes + r * 128;
+      mbar_wait(b_zfull + 8 * zb, (jt >> 1) & 1);
       float sm = 0.f, sq = 0.f;
 #pragma unroll
       for (int hf = 0; hf < 2; ++hf)
@@ -218,8 +236,24 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
           stats_bf16x2(sm, sq, w.x); stats_bf16x2(sm, sq, w.y); stats_bf16x2(sm, sq, w.z); stats_bf16x2(sm, sq, w.w);
         }
       const float mu = sm * (1.f / tCz);
-      const float rstd = rsqrtf(fmaxf(fmaf(sq, 1.f / tCz, -mu * mu), 0.f) + eps);
-      const float nm = -mu * rstd;
+      const float vpe = fmaxf(fmaf(sq, 1.f / tCz, -mu * mu), 0.f) + eps;
+      if (half == 0) {
+        const uint32_t xrow = s_zx + zb * tZxBytes + r * 32;
+        const uint32_t c0 = ((uint32_t)(r >> 2) & 1u) << 4;
+        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %2, %2};" ::"r"(xrow + c0), "r"(pack_bf16(-mu, sqrtf(vpe))), "r"(0u) : "memory");
+        asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(xrow + (c0 ^ 16u)), "r"(0u) : "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(b_xfull + 8 * zb);
+      }
+      return rsqrtf(vpe);
+    };
+    int it = 0;
+    float rstd_next = (int64_t)blockIdx.x < n_tiles ? prepare(0) : 0.f;
+    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      const int zb = it & 1;
+      const uint32_t zrow = s_z + zb * tZBytes + r * 128;   // row base inside a 64-channel half
+      const float rstd = rstd_next, hrstd = 0.5f * rstd_next;
 
       for (int c = 0; c < tChunks; ++c) {
         mbar_wait(b_afull, na & 1);
@@ -241,12 +275,9 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
             float hv[2];
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-              const float4 k = s_c[c * tNC + half * 64 + sb * 32 + i + e];     // {c1_1, c0_1, c1_2, c0_2}: broadcast read
-              const float x1 = fmaf(__uint_as_float(a1[i + e]), rstd, fmaf(nm, k.x, k.y));
-              const float x2 = fmaf(__uint_as_float(a2[i + e]), rstd, fmaf(nm, k.z, k.w));
-              // SiLU(x) = x sigmoid(x) = 0.5 x (1 + tanh(x / 2))
-              const float hx = 0.5f * x1;
-              hv[e] = fmaf(hx, tanh_fast(hx), hx) * x2;
+              // a = rstd * accumulator (the K extension carried -mu c1 + c0 / rstd);  SiLU(x) = 0.5 x (1 + tanh(x / 2))
+              const float hx = __uint_as_float(a1[i + e]) * hrstd;
+              hv[e] = fmaf(hx, tanh_fast(hx), hx) * (__uint_as_float(a2[i + e]) * rstd);
             }
             hw[sb * 16 + (i >> 1)] = pack_bf16(hv[0], hv[1]);
           }
@@ -263,6 +294,7 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
         __syncwarp();
         if (lane == 0) mbar_arrive(b_hfull);
         ++nh;
+        if (c == 2 && tile + gridDim.x < n_tiles) rstd_next = prepare(it + 1);   // the next tile's statistics, early
       }
 
       // ---- residual: z + OUT -> bf16 -> staging tile (the H buffer, same swizzled layout) -> TMA store
@@ -319,11 +351,11 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
   }
 }
 
-// W'[k][j] = bf16(gamma_k W[k][j]) for W1 and W2, consts[j] = {sum_k W1'[k][j], sum_k beta_k W1[k][j], same for W2}
+// Folded weights [c_z + 16][4 c_z] for W1 and W2: rows k < c_z: bf16(gamma_k W[k][j]); row c_z: c1[j] = sum_k of those
+// rounded values; row c_z + 1: c0[j] = sum_k beta_k W[k][j]; rows c_z + 2 ..: zero (the K extension of the first GEMM)
 __global__ void __launch_bounds__(128) transition_fold_kernel(const __nv_bfloat16* __restrict__ w1, const __nv_bfloat16* __restrict__ w2,
                                                              const __nv_bfloat16* __restrict__ gamma, const __nv_bfloat16* __restrict__ beta,
-                                                             __nv_bfloat16* __restrict__ w1f, __nv_bfloat16* __restrict__ w2f,
-                                                             float4* __restrict__ consts) {
+                                                             __nv_bfloat16* __restrict__ w1f, __nv_bfloat16* __restrict__ w2f) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= tHid) return;
   float c11 = 0.f, c01 = 0.f, c12 = 0.f, c02 = 0.f;
@@ -336,7 +368,9 @@ __global__ void __launch_bounds__(128) transition_fold_kernel(const __nv_bfloat1
     c11 += to_f32(af); c12 += to_f32(cf);
     c01 = fmaf(b, a, c01); c02 = fmaf(b, c, c02);
   }
-  consts[j] = make_float4(c11, c01, c12, c02);
+  w1f[tCz * tHid + j] = __float2bfloat16_rn(c11); w1f[(tCz + 1) * tHid + j] = __float2bfloat16_rn(c01);
+  w2f[tCz * tHid + j] = __float2bfloat16_rn(c12); w2f[(tCz + 1) * tHid + j] = __float2bfloat16_rn(c02);
+  for (int k = tCz + 2; k < tCz + tKx; ++k) { w1f[k * tHid + j] = __float2bfloat16_rn(0.f); w2f[k * tHid + j] = __float2bfloat16_rn(0.f); }
 }
 
 CUresult encode2d(PFN_cuTensorMapEncodeTiled enc, CUtensorMap* m, const void* base, uint64_t d0, uint64_t d1, uint32_t b0,
@@ -353,7 +387,7 @@ CUresult encode2d(PFN_cuTensorMapEncodeTiled enc, CUtensorMap* m, const void* ba
 }  // namespace
 
 bool pair_transition_supports(dcp_dtype dt, int c_z) { return dt == DCP_BF16 && c_z == tCz; }
-size_t pair_transition_workspace_bytes() { return (size_t)2 * tCz * tHid * 2 + (size_t)tHid * 16; }
+size_t pair_transition_workspace_bytes() { return (size_t)2 * (tCz + tKx) * tHid * 2; }
 
 cudaError_t launch_pair_transition(const void* z_in, void* z_out, int64_t n_pairs, const void* w1, const void* w2,
                                    const void* w3, const void* gamma, const void* beta, float eps, void* workspace,
@@ -362,15 +396,16 @@ cudaError_t launch_pair_transition(const void* z_in, void* z_out, int64_t n_pair
   PFN_cuTensorMapEncodeTiled enc = get_encode_fn();
   if (!enc) return cudaErrorNotSupported;
   __nv_bfloat16* w1f = reinterpret_cast<__nv_bfloat16*>(workspace);
-  __nv_bfloat16* w2f = w1f + tCz * tHid;
-  float4* consts = reinterpret_cast<float4*>(w2f + tCz * tHid);
+  __nv_bfloat16* w2f = w1f + (tCz + tKx) * tHid;
   transition_fold_kernel<<<tHid / 128, 128, 0, st>>>((const __nv_bfloat16*)w1, (const __nv_bfloat16*)w2,
-                                                     (const __nv_bfloat16*)gamma, (const __nv_bfloat16*)beta, w1f, w2f, consts);
+                                                     (const __nv_bfloat16*)gamma, (const __nv_bfloat16*)beta, w1f, w2f);
   TransMaps maps;
   if (encode2d(enc, &maps.z_in, z_in, tCz, (uint64_t)n_pairs, 64, tM) != CUDA_SUCCESS ||
       encode2d(enc, &maps.z_out, z_out, tCz, (uint64_t)n_pairs, 64, tM) != CUDA_SUCCESS ||
-      encode2d(enc, &maps.w1, w1f, tHid, tCz, 64, 64) != CUDA_SUCCESS ||
-      encode2d(enc, &maps.w2, w2f, tHid, tCz, 64, 64) != CUDA_SUCCESS ||
+      encode2d(enc, &maps.w1, w1f, tHid, tCz + tKx, 64, 64) != CUDA_SUCCESS ||
+      encode2d(enc, &maps.w2, w2f, tHid, tCz + tKx, 64, 64) != CUDA_SUCCESS ||
+      encode2d(enc, &maps.w1x, w1f, tHid, tCz + tKx, 64, tKx) != CUDA_SUCCESS ||
+      encode2d(enc, &maps.w2x, w2f, tHid, tCz + tKx, 64, tKx) != CUDA_SUCCESS ||
       encode2d(enc, &maps.w3, w3, tCz, tHid, 64, 64) != CUDA_SUCCESS)
     return cudaErrorInvalidValue;
   cudaError_t e = cudaFuncSetAttribute(pair_transition_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tSmemAlloc);
@@ -381,7 +416,7 @@ cudaError_t launch_pair_transition(const void* z_in, void* z_out, int64_t n_pair
   if (sms <= 0) sms = 148;
   const int64_t n_tiles = (n_pairs + tM - 1) / tM;
   const unsigned grid = (unsigned)(n_tiles < sms ? n_tiles : sms);
-  pair_transition_kernel<<<grid, tThreads, tSmemAlloc, st>>>(maps, consts, n_pairs, eps);
+  pair_transition_kernel<<<grid, tThreads, tSmemAlloc, st>>>(maps, n_pairs, eps);
   return cudaGetLastError();
 }
 
