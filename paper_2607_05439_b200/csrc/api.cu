@@ -424,9 +424,14 @@ dcp_status dcp_sparse_atom_attention(const void* a, const void* p_slice, const i
   gp.scale[0] = 1.4426950408889634f / sqrtf((float)c);   // exp2-domain softmax
   gp.ldc[1] = D; gp.ldc[2] = D; gp.ldc[3] = D;
   gp.H = H; gp.c = c; gp.cp = c;
-  DCP_CUDA(launch_gemm_mma(gp, st));
-  DCP_CUDA(launch_fold_ln_z_mma(w->w_b, w->ln_z_gamma, w->ln_z_beta, ws + cv.wfold, (float*)(ws + cv.c1),
-                                (float*)(ws + cv.c0), c_atompair, H, 16, st));
+  gp.fold_w_b = w->w_b; gp.fold_gamma = w->ln_z_gamma; gp.fold_beta = w->ln_z_beta;
+  gp.fold_wfold = ws + cv.wfold; gp.fold_c1 = (float*)(ws + cv.c1); gp.fold_c0 = (float*)(ws + cv.c0);
+  gp.fold_c_z = c_atompair; gp.fold_H = H; gp.fold_H_pad = 16;
+  bool folded = false;
+  DCP_CUDA(launch_gemm_mma(gp, st, &folded));
+  if (!folded)
+    DCP_CUDA(launch_fold_ln_z_mma(w->w_b, w->ln_z_gamma, w->ln_z_beta, ws + cv.wfold, (float*)(ws + cv.c1),
+                                  (float*)(ws + cv.c0), c_atompair, H, 16, st));
   if (plan && plan->ev_fused_begin && cudaEventRecord((cudaEvent_t)plan->ev_fused_begin, st) != cudaSuccess) return DCP_ERR_CUDA;
   DCP_CUDA(launch_sparse_atom(ws + cv.q, ws + cv.k, ws + cv.v, ws + cv.g, p_slice, idx, ws + cv.wfold,
                               (const float*)(ws + cv.c1), (const float*)(ws + cv.c0), ws + cv.gated, L, k, H, eps, st));
