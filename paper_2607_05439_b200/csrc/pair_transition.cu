@@ -37,14 +37,15 @@ constexpr int tKx = 16;                        // the K extension: channels 128 
 constexpr int tZxBytes = tM * tKx * 2;         // 4 KB per z buffer, K-major, 32-byte swizzle
 constexpr int tW12xBytes = 4 * 64 * tKx * 2;   // 8 KB: rows k = 128..143 of [W1'c | W2'c], four 64-n blocks of 2 KB
 constexpr size_t tSmemZ = 0;
+constexpr int tW12Slot = tW12Bytes / 2;         // 32 KB: one k-block of a chunk; a ring of three slots
 constexpr size_t tSmemW12 = tSmemZ + 2 * (size_t)tZBytes;
-constexpr size_t tSmemW3 = tSmemW12 + tW12Bytes;
-constexpr size_t tSmemH = tSmemW3 + tW3Bytes;
-constexpr size_t tSmemZx = tSmemH + tHBytes;
+constexpr size_t tSmemW3 = tSmemW12 + 3 * (size_t)tW12Slot;
+constexpr size_t tSmemZx = tSmemW3 + tW3Bytes;
 constexpr size_t tSmemW12x = tSmemZx + 2 * (size_t)tZxBytes;
-constexpr size_t tSmemBar = tSmemW12x + tW12xBytes;
-constexpr size_t tSmemAlloc = tSmemBar + 16 * 8 + 16 + 1024;
-constexpr int tColA1 = 0, tColOut = 256;                    // TMEM columns: A1 [0,128) A2 [128,256) OUT [256,384)
+constexpr size_t tSmemBar = tSmemW12x + 2 * (size_t)tW12xBytes;
+constexpr size_t tSmemAlloc = tSmemBar + 24 * 8 + 1024;
+constexpr int tColA1 = 0, tColOut = 256, tColH = 384;       // TMEM columns: A1 [0,128) A2 [128,256) OUT [256,384)
+                                                            // H (bf16x2, the A operand of G2) [384,448) and [448,512)
 
 struct TransMaps {
   CUtensorMap z_in, z_out, w1, w2, w3, w1x, w2x;   // w1x / w2x: the same folded weights with a (64 n, 16 k) box
@@ -79,6 +80,21 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
         "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
       : "r"(taddr));
 }
+// 16 consecutive 32-bit columns of the thread's TMEM lane
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+        "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]) : "memory");
+}
+// D[tmem] (+)= A[tmem: lane = row, one column = two consecutive k] . B[smem]
+__device__ __forceinline__ void umma_bf16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
 __device__ __forceinline__ float tanh_fast(float x) {
   float y;
   asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -101,19 +117,22 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
   extern __shared__ unsigned char smem_dyn[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
   const uint32_t s_z = smem_u32(smem + tSmemZ), s_w12 = smem_u32(smem + tSmemW12), s_w3 = smem_u32(smem + tSmemW3);
-  const uint32_t s_h = smem_u32(smem + tSmemH), s_bar = smem_u32(smem + tSmemBar);
+  const uint32_t s_bar = smem_u32(smem + tSmemBar);
   const uint32_t s_zx = smem_u32(smem + tSmemZx), s_w12x = smem_u32(smem + tSmemW12x);
   // barriers
-  const uint32_t b_zfull = s_bar, b_zempty = s_bar + 16, b_w12full = s_bar + 32, b_w12empty = s_bar + 40, b_w3full = s_bar + 48,
-                 b_w3empty = s_bar + 56, b_afull = s_bar + 64, b_aempty = s_bar + 72, b_hfull = s_bar + 80,
-                 b_hempty = s_bar + 88, b_ofull = s_bar + 96, b_oempty = s_bar + 104, b_xfull = s_bar + 112;   // b_xfull: 2 barriers
-  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + tSmemBar + 16 * 8);
+  // (8 bytes each; z, x, h: one per buffer; w12: one per ring slot)
+  const uint32_t b_zfull = s_bar, b_zempty = s_bar + 16, b_w12full = s_bar + 32, b_w12empty = s_bar + 56, b_w3full = s_bar + 80,
+                 b_w3empty = s_bar + 88, b_afull = s_bar + 96, b_aempty = s_bar + 104, b_hfull = s_bar + 112,
+                 b_hempty = s_bar + 128, b_ofull = s_bar + 144, b_oempty = s_bar + 152, b_xfull = s_bar + 160;
+  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + tSmemBar + 22 * 8);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
-    for (int b = 0; b < 2; ++b) { mbar_init(b_zfull + 8 * b, 1); mbar_init(b_zempty + 8 * b, 8); }
-    mbar_init(b_w12full, 1); mbar_init(b_w12empty, 1); mbar_init(b_w3full, 1); mbar_init(b_w3empty, 1);
-    mbar_init(b_afull, 1); mbar_init(b_aempty, 8); mbar_init(b_hfull, 8); mbar_init(b_hempty, 1);
+    for (int b = 0; b < 2; ++b) { mbar_init(b_zfull + 8 * b, 1); mbar_init(b_zempty + 8 * b, 1); }
+    for (int b = 0; b < 3; ++b) { mbar_init(b_w12full + 8 * b, 1); mbar_init(b_w12empty + 8 * b, 1); }
+    mbar_init(b_w3full, 1); mbar_init(b_w3empty, 1);
+    mbar_init(b_afull, 1); mbar_init(b_aempty, 8);
+    for (int b = 0; b < 2; ++b) { mbar_init(b_hfull + 8 * b, 8); mbar_init(b_hempty + 8 * b, 1); }
     mbar_init(b_ofull, 1); mbar_init(b_oempty, 8);
     mbar_init(b_xfull, 4); mbar_init(b_xfull + 8, 4);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -128,7 +147,6 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
   if (warp == 0) {
     if (lane == 0) {
       // =============================================================== TMA producer
-      uint32_t n12 = 0, n3 = 0;
       auto load_z = [&](int64_t tile, int it) {
         const int zb = it & 1;
         mbar_wait(b_zempty + 8 * zb, ((it >> 1) & 1) ^ 1);
@@ -136,33 +154,48 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
         tma_load_2d_t(s_z + zb * tZBytes, &maps.z_in, 0, (int)(tile * tM), b_zfull + 8 * zb);
         tma_load_2d_t(s_z + zb * tZBytes + tZBytes / 2, &maps.z_in, 64, (int)(tile * tM), b_zfull + 8 * zb);
       };
-      int it = 0;
-      if ((int64_t)blockIdx.x < n_tiles) load_z(blockIdx.x, 0);
-      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
-        for (int c = 0; c < tChunks; ++c) {
-          mbar_wait(b_w12empty, (n12 & 1) ^ 1);
-          mbar_expect_tx(b_w12full, tW12Bytes + tW12xBytes);
+      // The CTA's chunks are numbered g = 4 it + c across its tiles; the weights of chunk g are those of c = g & 3.
+      // k-block j = 2 g + kb of [W1'c | W2'c] goes to ring slot j % 3 (use number j / 3); the K-extension rows of chunk g
+      // ride on the kb = 1 load (buffer g & 1: free because slot j - 3's release follows every MMA of chunk g - 2).
+      const uint32_t my_tiles = (int64_t)blockIdx.x < n_tiles ? (uint32_t)((n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0u;
+      const uint32_t n_kblocks = my_tiles * tChunks * 2;
+      auto load_w12 = [&](uint32_t j) {
+        if (j >= n_kblocks) return;
+        const uint32_t g = j >> 1, kb = j & 1, c = g & 3, slot = j % 3, use = j / 3;
+        mbar_wait(b_w12empty + 8 * slot, (use & 1) ^ 1);
+        mbar_expect_tx(b_w12full + 8 * slot, tW12Slot + (kb ? tW12xBytes : 0));
+        const uint32_t base = s_w12 + slot * tW12Slot;
 #pragma unroll
-          for (int kb = 0; kb < 2; ++kb)
-#pragma unroll
-            for (int nh = 0; nh < 2; ++nh) {
-              tma_load_2d_t(s_w12 + kb * 32768 + nh * 8192, &maps.w1, c * tNC + 64 * nh, 64 * kb, b_w12full);
-              tma_load_2d_t(s_w12 + kb * 32768 + 16384 + nh * 8192, &maps.w2, c * tNC + 64 * nh, 64 * kb, b_w12full);
-            }
+        for (int nh = 0; nh < 2; ++nh) {
+          tma_load_2d_t(base + nh * 8192, &maps.w1, c * tNC + 64 * nh, 64 * kb, b_w12full + 8 * slot);
+          tma_load_2d_t(base + 16384 + nh * 8192, &maps.w2, c * tNC + 64 * nh, 64 * kb, b_w12full + 8 * slot);
+        }
+        if (kb) {
+          const uint32_t xb = s_w12x + (g & 1) * tW12xBytes;
 #pragma unroll
           for (int nh = 0; nh < 2; ++nh) {
-            tma_load_2d_t(s_w12x + nh * 2048, &maps.w1x, c * tNC + 64 * nh, tCz, b_w12full);
-            tma_load_2d_t(s_w12x + 4096 + nh * 2048, &maps.w2x, c * tNC + 64 * nh, tCz, b_w12full);
+            tma_load_2d_t(xb + nh * 2048, &maps.w1x, c * tNC + 64 * nh, tCz, b_w12full + 8 * slot);
+            tma_load_2d_t(xb + 4096 + nh * 2048, &maps.w2x, c * tNC + 64 * nh, tCz, b_w12full + 8 * slot);
           }
-          ++n12;
-          mbar_wait(b_w3empty, (n3 & 1) ^ 1);
+        }
+      };
+      if (my_tiles) load_z(blockIdx.x, 0);
+      load_w12(0); load_w12(1); load_w12(2);
+      uint32_t g = 0;
+      int it = 0;
+      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        for (int c = 0; c < tChunks; ++c, ++g) {
+          // in the order in which the tensor pipe frees the buffers: k-block (g, 0) -> (g + 1, 1), (g, 1) -> (g + 2, 0),
+          // G2(g - 1) -> W3(g)
+          load_w12(2 * g + 3);
+          load_w12(2 * g + 4);
+          mbar_wait(b_w3empty, (g & 1) ^ 1);
           mbar_expect_tx(b_w3full, tW3Bytes);
 #pragma unroll
           for (int kb = 0; kb < 2; ++kb)
 #pragma unroll
             for (int nh = 0; nh < 2; ++nh)
               tma_load_2d_t(s_w3 + kb * 16384 + nh * 8192, &maps.w3, 64 * nh, c * tNC + 64 * kb, b_w3full);
-          ++n3;
           if (c == 1 && tile + gridDim.x < n_tiles) load_z(tile + gridDim.x, it + 1);
         }
       }
@@ -172,36 +205,46 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
       // =============================================================== tcgen05 issuer
       constexpr uint32_t idesc1 = umma_idesc_bf16(tM, 256) | (1u << 16);     // B MN-major
       constexpr uint32_t idesc2 = umma_idesc_bf16(tM, 128) | (1u << 16);
-      uint32_t n12 = 0, n3 = 0, na = 0, nh = 0, nout = 0;
+      uint32_t g = 0, n3 = 0, na = 0, nh = 0, nout = 0;
       int it = 0;
       for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
         const int zb = it & 1;
         const uint32_t zs = s_z + zb * tZBytes;
         mbar_wait(b_zfull + 8 * zb, (it >> 1) & 1);
         mbar_wait(b_xfull + 8 * zb, (it >> 1) & 1);          // the epilogue has written this tile's K extension
+        // G1 of the CTA's chunk number g: [A1 | A2] = [z | -mu, 1 / rstd] . [W1'c | W2'c ; c1 ; c0], k-block by k-block
         auto g1 = [&]() {
-          mbar_wait(b_w12full, n12 & 1);
-          mbar_wait(b_aempty, (na & 1) ^ 1);
-          tc_fence_after();
 #pragma unroll
-          for (int ks = 0; ks < 8; ++ks)
-            umma_bf16(tmem_base + tColA1, umma_desc_sw128(zs + (ks >> 2) * (tZBytes / 2) + (ks & 3) * 32),
-                      umma_desc_mn(s_w12 + (ks >> 2) * 32768 + (ks & 3) * 2048, 8192), idesc1, ks != 0);
-          umma_bf16(tmem_base + tColA1, umma_desc_k_sw32(s_zx + zb * tZxBytes), umma_desc_mn(s_w12x, 2048), idesc1, 1);
-          umma_commit(b_afull);
-          umma_commit(b_w12empty);
-          ++n12; ++na;
+          for (int kb = 0; kb < 2; ++kb) {
+            const uint32_t j = 2 * g + kb, slot = j % 3, use = j / 3;
+            mbar_wait(b_w12full + 8 * slot, use & 1);
+            if (kb == 0) mbar_wait(b_aempty, (na & 1) ^ 1);
+            tc_fence_after();
+            const uint32_t wb = s_w12 + slot * tW12Slot;
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks)
+              umma_bf16(tmem_base + tColA1, umma_desc_sw128(zs + kb * (tZBytes / 2) + ks * 32), umma_desc_mn(wb + ks * 2048, 8192),
+                        idesc1, (kb | ks) != 0);
+            if (kb == 1) {
+              umma_bf16(tmem_base + tColA1, umma_desc_k_sw32(s_zx + zb * tZxBytes), umma_desc_mn(s_w12x + (g & 1) * tW12xBytes, 2048),
+                        idesc1, 1);
+              umma_commit(b_afull);
+            }
+            umma_commit(b_w12empty + 8 * slot);
+          }
+          ++g; ++na;
         };
         auto g2 = [&](int c) {
-          mbar_wait(b_hfull, nh & 1);
+          const uint32_t hb = nh & 1;
+          mbar_wait(b_hfull + 8 * hb, (nh >> 1) & 1);
           mbar_wait(b_w3full, n3 & 1);
           if (c == 0) mbar_wait(b_oempty, (nout & 1) ^ 1);
           tc_fence_after();
 #pragma unroll
           for (int ks = 0; ks < 8; ++ks)
-            umma_bf16(tmem_base + tColOut, umma_desc_sw128(s_h + (ks >> 2) * (tHBytes / 2) + (ks & 3) * 32),
-                      umma_desc_mn(s_w3 + (ks >> 2) * 16384 + (ks & 3) * 2048, 8192), idesc2, (c | ks) != 0);
-          umma_commit(b_hempty);
+            umma_bf16_ts(tmem_base + tColOut, tmem_base + tColH + 64 * hb + 8 * ks,
+                         umma_desc_mn(s_w3 + (ks >> 2) * 16384 + (ks & 3) * 2048, 8192), idesc2, (c | ks) != 0);
+          umma_commit(b_hempty + 8 * hb);
           umma_commit(b_w3empty);
           if (c == tChunks - 1) { umma_commit(b_ofull); ++nout; }
           ++nh; ++n3;
@@ -258,9 +301,10 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
       for (int c = 0; c < tChunks; ++c) {
         mbar_wait(b_afull, na & 1);
         tc_fence_after();
-        uint32_t hw[32];                                     // the thread's 64 h values of this chunk, bf16x2
+        const uint32_t hb = nh & 1;                          // H buffer of this chunk: TMEM columns tColH + 64 hb ..
 #pragma unroll
         for (int sb = 0; sb < 2; ++sb) {
+          uint32_t hw[16];                                   // 32 h values of the thread's row, bf16x2
           uint32_t a1[32], a2[32];
           tmem_ld32(t_lane + tColA1 + half * 64 + sb * 32, a1);
           tmem_ld32(t_lane + tColA1 + 128 + half * 64 + sb * 32, a2);
@@ -279,25 +323,27 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
               const float hx = __uint_as_float(a1[i + e]) * hrstd;
               hv[e] = fmaf(hx, tanh_fast(hx), hx) * (__uint_as_float(a2[i + e]) * rstd);
             }
-            hw[sb * 16 + (i >> 1)] = pack_bf16(hv[0], hv[1]);
+            hw[i >> 1] = pack_bf16(hv[0], hv[1]);
           }
+          // ---- H (the A operand of G2, read from TMEM): lane = row, column = two consecutive hidden units
+          if (sb == 0) mbar_wait(b_hempty + 8 * hb, ((nh >> 1) & 1) ^ 1);   // G2 two chunks back has finished reading it
+          tmem_st16(t_lane + tColH + 64 * hb + half * 32 + sb * 16, hw);
         }
         ++na;
-        // ---- H tile (the A operand of G2): row r of the 64-column k-half `half`, 128-byte swizzle
-        mbar_wait(b_hempty, (nh & 1) ^ 1);                   // G2 of the previous chunk has finished reading H
-        const uint32_t hrow = s_h + half * (tHBytes / 2) + r * 128;
-#pragma unroll
-        for (int ch = 0; ch < 8; ++ch)
-          asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(hrow + ((ch ^ sw) << 4)), "r"(hw[4 * ch]),
-                       "r"(hw[4 * ch + 1]), "r"(hw[4 * ch + 2]), "r"(hw[4 * ch + 3]) : "memory");
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(b_hfull);
+        if (lane == 0) mbar_arrive(b_hfull + 8 * hb);
         ++nh;
+        if (c == 0 && it > 0 && et == 0) {                   // the previous tile's store has read its buffer: free for z
+          asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+          mbar_arrive(b_zempty + 8 * (zb ^ 1));
+        }
         if (c == 2 && tile + gridDim.x < n_tiles) rstd_next = prepare(it + 1);   // the next tile's statistics, early
       }
 
-      // ---- residual: z + OUT -> bf16 -> staging tile (the H buffer, same swizzled layout) -> TMA store
+      // ---- residual: z + OUT -> bf16, written over the thread's own bytes of the z tile (every G1 of the tile is
+      // complete once out_full is) -> TMA store from there
       mbar_wait(b_ofull, nout & 1);
       tc_fence_after();
       uint32_t ow[32];
@@ -323,23 +369,18 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
         }
       }
       ++nout;
-      // out_full implies that every G2 of the tile is complete, so the H buffer is free for staging
-      const uint32_t orow = s_h + half * (tHBytes / 2) + r * 128;
+      const uint32_t orow = zrow + half * (tZBytes / 2);
 #pragma unroll
       for (int ch = 0; ch < 8; ++ch)
         asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(orow + ((ch ^ sw) << 4)), "r"(ow[4 * ch]),
                      "r"(ow[4 * ch + 1]), "r"(ow[4 * ch + 2]), "r"(ow[4 * ch + 3]) : "memory");
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      __syncwarp();
-      if (lane == 0) mbar_arrive(b_zempty + 8 * zb);          // this warp is done with the z tile
       asm volatile("bar.sync 1, 256;" ::: "memory");
       if (et == 0) {
-        tma_store_2d(&maps.z_out, 0, (int)(tile * tM), s_h);
-        tma_store_2d(&maps.z_out, 64, (int)(tile * tM), s_h + tHBytes / 2);
+        tma_store_2d(&maps.z_out, 0, (int)(tile * tM), s_z + zb * tZBytes);
+        tma_store_2d(&maps.z_out, 64, (int)(tile * tM), s_z + zb * tZBytes + tZBytes / 2);
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the staging tile has been read
       }
-      asm volatile("bar.sync 1, 256;" ::: "memory");          // ... before the next tile's chunk 0 overwrites it
     }
     if (et == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
   }
