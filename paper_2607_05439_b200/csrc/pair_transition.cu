@@ -10,16 +10,23 @@
 // the K extension [-mu, 1 / rstd, 0 ...] (written per row by the epilogue warps) with the weight rows [c1; c0; 0 ...],
 // so the accumulator only has to be scaled by the row's rstd: no per-column constants in the epilogue.
 //
-// One persistent CTA per SM, 10 warps:
+// One persistent CTA per SM, 10 warps, CTAs launched as clusters of two that walk the weight chunks in lockstep:
 //   warp 0     TMA producer: z tiles (128 pairs x 128 ch = 32 KB, double buffered) and, per 128-wide hidden chunk c,
-//              the weight tiles W1'[:, c], W2'[:, c] (64 KB) and W3[c, :] (32 KB) -- row-major weights are MN-major B operands
-//   warp 1     tcgen05 issuer: G1(c): [A1 | A2] (128 x 256, TMEM) = z . [W1'c | W2'c]   (8 k-steps, N = 256)
-//                              G2(c): OUT (128 x 128, TMEM) += H_c . W3_c              (8 k-steps, N = 128)
+//              the weight tiles W1'[:, c], W2'[:, c] (two 64-row k-blocks of 32 KB in a three-slot ring, refilled in the
+//              order in which the tensor pipe frees them) and W3[c, :] (32 KB) -- row-major weights are MN-major B
+//              operands.  Each CTA of the pair fetches half of every weight tile and multicasts it to both, so a weight
+//              byte leaves L2 once per tile pair; the slot-free barriers collect one tcgen05.commit from each CTA.
+//   warp 1     tcgen05 issuer: G1(c): [A1 | A2] (128 x 256, TMEM) = [z | -mu, 1/rstd] . [W1'c | W2'c ; c1 ; c0]  (9 k-steps)
+//                              G2(c): OUT (128 x 128, TMEM) += H_c . W3_c   (8 k-steps, H_c read from TMEM: A-in-TMEM form)
 //              issued as G1(0), G1(1), G2(0), G1(2), G2(1), G1(3), G2(2), G2(3): the tensor pipe works on the next
 //              chunk while the epilogue warps turn the previous one into H
 //   warps 2-9  epilogue (TMEM lane quadrant = warp % 4, two warps per quadrant = two 64-column halves): per chunk
-//              tcgen05.ld A1, A2 -> a = rstd (A - mu c1) + c0 -> h = SiLU(a1) a2 -> bf16 -> the H tile in shared memory
-//              (K-major, 128-byte swizzle by hand: the A operand of G2); per tile OUT + z -> bf16 -> TMA store.
+//              tcgen05.ld A1, A2 -> h = SiLU(rstd A1) rstd A2 -> bf16x2 -> tcgen05.st into the H columns of TMEM
+//              (lane = row, one column = two hidden units; double buffered); per tile OUT + z -> bf16, written over
+//              the thread's own bytes of the z tile -> TMA store from there.
+// TMEM: A1 [0,128) A2 [128,256) OUT [256,384) H [384,448) [448,512).  Shared memory: z 64 KB, W12 ring 96 KB, W3 32 KB,
+// K extension 8 + 16 KB.  What limits it (what-if builds): the weight bytes every SM has to take in per
+// tile (416 KB) and the accumulator hand-offs between the tensor pipe and the epilogue warps.
 #include "kernels.h"
 #include "mma_ptx.cuh"
 
@@ -29,10 +36,11 @@ namespace {
 
 constexpr int tCz = 128, tHid = 512, tNC = 128, tChunks = tHid / tNC, tM = 128;
 constexpr int tThreads = 64 + 256;
+constexpr int tCluster = 2;                    // CTA pair: every weight tile is read from L2 once and multicast to both
+constexpr uint16_t tClusterMask = (1u << tCluster) - 1;
 constexpr int tZBytes = tM * tCz * 2;          // 32 KB, two 64-channel halves of 16 KB
 constexpr int tW12Bytes = 2 * tCz * tNC * 2;   // 64 KB: per k-block of 64: [W1 n-half 0][W1 n-half 1][W2 n-half 0][W2 n-half 1]
 constexpr int tW3Bytes = tNC * tCz * 2;        // 32 KB: per k-block of 64: [n-half 0][n-half 1]
-constexpr int tHBytes = tM * tNC * 2;          // 32 KB
 constexpr int tKx = 16;                        // the K extension: channels 128 (-mu), 129 (1 / rstd), 130..143 (zero)
 constexpr int tZxBytes = tM * tKx * 2;         // 4 KB per z buffer, K-major, 32-byte swizzle
 constexpr int tW12xBytes = 4 * 64 * tKx * 2;   // 8 KB: rows k = 128..143 of [W1'c | W2'c], four 64-n blocks of 2 KB
@@ -65,6 +73,19 @@ __device__ __forceinline__ uint64_t umma_desc_mn(uint32_t addr, uint32_t lbo) {
 __device__ __forceinline__ void tma_load_2d_t(uint32_t dst, const CUtensorMap* tmap, int c0, int c1, uint32_t bar) {
   asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
                ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+// the same load written to the same shared-memory offset (and signalled on the same barrier offset) of every CTA in cta_mask
+__device__ __forceinline__ void tma_load_2d_mc(uint32_t dst, const CUtensorMap* tmap, int c0, int c1, uint32_t bar, uint16_t cta_mask) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1, {%2, %3}], [%4], %5;"
+               ::"r"(dst), "l"(tmap), "r"(c0), "r"(c1), "r"(bar), "h"(cta_mask) : "memory");
+}
+// tcgen05.commit arriving on the barrier at this offset in every CTA of cta_mask
+__device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t cta_mask) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"(cta_mask) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void tma_store_2d(const CUtensorMap* tmap, int c0, int c1, uint32_t src) {
   asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
@@ -112,7 +133,7 @@ __device__ __forceinline__ void stats_bf16x2(float& acc_s, float& acc_q, uint32_
       : "+f"(acc_s), "+f"(acc_q) : "r"(w));
 }
 
-__global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __grid_constant__ TransMaps maps,
+__global__ void __cluster_dims__(tCluster, 1, 1) __launch_bounds__(tThreads, 1) pair_transition_kernel(const __grid_constant__ TransMaps maps,
                                                                       int64_t n_pairs, float eps) {
   extern __shared__ unsigned char smem_dyn[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
@@ -129,8 +150,8 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
 
   if (threadIdx.x == 0) {
     for (int b = 0; b < 2; ++b) { mbar_init(b_zfull + 8 * b, 1); mbar_init(b_zempty + 8 * b, 1); }
-    for (int b = 0; b < 3; ++b) { mbar_init(b_w12full + 8 * b, 1); mbar_init(b_w12empty + 8 * b, 1); }
-    mbar_init(b_w3full, 1); mbar_init(b_w3empty, 1);
+    for (int b = 0; b < 3; ++b) { mbar_init(b_w12full + 8 * b, 1); mbar_init(b_w12empty + 8 * b, tCluster); }
+    mbar_init(b_w3full, 1); mbar_init(b_w3empty, tCluster);
     mbar_init(b_afull, 1); mbar_init(b_aempty, 8);
     for (int b = 0; b < 2; ++b) { mbar_init(b_hfull + 8 * b, 8); mbar_init(b_hempty + 8 * b, 1); }
     mbar_init(b_ofull, 1); mbar_init(b_oempty, 8);
@@ -140,9 +161,18 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
   if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), 512);
   tc_fence_before();
   __syncthreads();
+  cluster_sync_all();                                        // the peer's barriers are initialised before anything arrives on them
   tc_fence_after();
   const uint32_t tmem_base = *s_tmem;
+  // Tiles go to CTA pairs: pair p of tiles (2 p, 2 p + 1) to cluster p % n_clusters, tile 2 p + rank to the CTA of
+  // that rank, so that both CTAs of a cluster walk the weight chunks in lockstep.  A tile index == n_tiles (odd tile
+  // count) is a phantom: its loads are zero-filled and its store is clipped by the tensor map.
   const int64_t n_tiles = (n_pairs + tM - 1) / tM;
+  uint32_t rank;
+  asm("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+  const int64_t n_clusters = gridDim.x / tCluster, cid = blockIdx.x / tCluster, n_tpairs = (n_tiles + tCluster - 1) / tCluster;
+  const int n_it = cid < n_tpairs ? (int)((n_tpairs - cid + n_clusters - 1) / n_clusters) : 0;
+  auto tile_of = [&](int it) -> int64_t { return (cid + (int64_t)it * n_clusters) * tCluster + rank; };
 
   if (warp == 0) {
     if (lane == 0) {
@@ -157,33 +187,30 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
       // The CTA's chunks are numbered g = 4 it + c across its tiles; the weights of chunk g are those of c = g & 3.
       // k-block j = 2 g + kb of [W1'c | W2'c] goes to ring slot j % 3 (use number j / 3); the K-extension rows of chunk g
       // ride on the kb = 1 load (buffer g & 1: free because slot j - 3's release follows every MMA of chunk g - 2).
-      const uint32_t my_tiles = (int64_t)blockIdx.x < n_tiles ? (uint32_t)((n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x) : 0u;
-      const uint32_t n_kblocks = my_tiles * tChunks * 2;
+      const uint32_t n_kblocks = (uint32_t)n_it * tChunks * 2;
       auto load_w12 = [&](uint32_t j) {
         if (j >= n_kblocks) return;
         const uint32_t g = j >> 1, kb = j & 1, c = g & 3, slot = j % 3, use = j / 3;
         mbar_wait(b_w12empty + 8 * slot, (use & 1) ^ 1);
         mbar_expect_tx(b_w12full + 8 * slot, tW12Slot + (kb ? tW12xBytes : 0));
         const uint32_t base = s_w12 + slot * tW12Slot;
+        // rank 0 fetches the W1' boxes, rank 1 the W2' boxes, each for both CTAs
+        const CUtensorMap* wm = rank ? &maps.w2 : &maps.w1;
+        const CUtensorMap* wxm = rank ? &maps.w2x : &maps.w1x;
 #pragma unroll
-        for (int nh = 0; nh < 2; ++nh) {
-          tma_load_2d_t(base + nh * 8192, &maps.w1, c * tNC + 64 * nh, 64 * kb, b_w12full + 8 * slot);
-          tma_load_2d_t(base + 16384 + nh * 8192, &maps.w2, c * tNC + 64 * nh, 64 * kb, b_w12full + 8 * slot);
-        }
+        for (int nh = 0; nh < 2; ++nh)
+          tma_load_2d_mc(base + rank * 16384 + nh * 8192, wm, c * tNC + 64 * nh, 64 * kb, b_w12full + 8 * slot, tClusterMask);
         if (kb) {
           const uint32_t xb = s_w12x + (g & 1) * tW12xBytes;
 #pragma unroll
-          for (int nh = 0; nh < 2; ++nh) {
-            tma_load_2d_t(xb + nh * 2048, &maps.w1x, c * tNC + 64 * nh, tCz, b_w12full + 8 * slot);
-            tma_load_2d_t(xb + 4096 + nh * 2048, &maps.w2x, c * tNC + 64 * nh, tCz, b_w12full + 8 * slot);
-          }
+          for (int nh = 0; nh < 2; ++nh)
+            tma_load_2d_mc(xb + rank * 4096 + nh * 2048, wxm, c * tNC + 64 * nh, tCz, b_w12full + 8 * slot, tClusterMask);
         }
       };
-      if (my_tiles) load_z(blockIdx.x, 0);
+      if (n_it) load_z(tile_of(0), 0);
       load_w12(0); load_w12(1); load_w12(2);
       uint32_t g = 0;
-      int it = 0;
-      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      for (int it = 0; it < n_it; ++it) {
         for (int c = 0; c < tChunks; ++c, ++g) {
           // in the order in which the tensor pipe frees the buffers: k-block (g, 0) -> (g + 1, 1), (g, 1) -> (g + 2, 0),
           // G2(g - 1) -> W3(g)
@@ -192,11 +219,9 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
           mbar_wait(b_w3empty, (g & 1) ^ 1);
           mbar_expect_tx(b_w3full, tW3Bytes);
 #pragma unroll
-          for (int kb = 0; kb < 2; ++kb)
-#pragma unroll
-            for (int nh = 0; nh < 2; ++nh)
-              tma_load_2d_t(s_w3 + kb * 16384 + nh * 8192, &maps.w3, 64 * nh, c * tNC + 64 * kb, b_w3full);
-          if (c == 1 && tile + gridDim.x < n_tiles) load_z(tile + gridDim.x, it + 1);
+          for (int nh = 0; nh < 2; ++nh)                     // k-block `rank` of W3's chunk, for both CTAs
+            tma_load_2d_mc(s_w3 + rank * 16384 + nh * 8192, &maps.w3, 64 * nh, c * tNC + 64 * (int)rank, b_w3full, tClusterMask);
+          if (c == 1 && it + 1 < n_it) load_z(tile_of(it + 1), it + 1);
         }
       }
     }
@@ -206,8 +231,7 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
       constexpr uint32_t idesc1 = umma_idesc_bf16(tM, 256) | (1u << 16);     // B MN-major
       constexpr uint32_t idesc2 = umma_idesc_bf16(tM, 128) | (1u << 16);
       uint32_t g = 0, n3 = 0, na = 0, nh = 0, nout = 0;
-      int it = 0;
-      for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      for (int it = 0; it < n_it; ++it) {
         const int zb = it & 1;
         const uint32_t zs = s_z + zb * tZBytes;
         mbar_wait(b_zfull + 8 * zb, (it >> 1) & 1);
@@ -230,7 +254,7 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
                         idesc1, 1);
               umma_commit(b_afull);
             }
-            umma_commit(b_w12empty + 8 * slot);
+            umma_commit_mc(b_w12empty + 8 * slot, tClusterMask);   // both CTAs write into this slot
           }
           ++g; ++na;
         };
@@ -245,7 +269,7 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
             umma_bf16_ts(tmem_base + tColOut, tmem_base + tColH + 64 * hb + 8 * ks,
                          umma_desc_mn(s_w3 + (ks >> 2) * 16384 + (ks & 3) * 2048, 8192), idesc2, (c | ks) != 0);
           umma_commit(b_hempty + 8 * hb);
-          umma_commit(b_w3empty);
+          umma_commit_mc(b_w3empty, tClusterMask);
           if (c == tChunks - 1) { umma_commit(b_ofull); ++nout; }
           ++nh; ++n3;
         };
@@ -292,8 +316,9 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
       return rsqrtf(vpe);
     };
     int it = 0;
-    float rstd_next = (int64_t)blockIdx.x < n_tiles ? prepare(0) : 0.f;
-    for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+    float rstd_next = n_it ? prepare(0) : 0.f;
+    for (; it < n_it; ++it) {
+      const int64_t tile = tile_of(it);
       const int zb = it & 1;
       const uint32_t zrow = s_z + zb * tZBytes + r * 128;   // row base inside a 64-channel half
       const float rstd = rstd_next, hrstd = 0.5f * rstd_next;
@@ -339,7 +364,7 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
           asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
           mbar_arrive(b_zempty + 8 * (zb ^ 1));
         }
-        if (c == 2 && tile + gridDim.x < n_tiles) rstd_next = prepare(it + 1);   // the next tile's statistics, early
+        if (c == 2 && it + 1 < n_it) rstd_next = prepare(it + 1);   // the next tile's statistics, early
       }
 
       // ---- residual: z + OUT -> bf16, written over the thread's own bytes of the z tile (every G1 of the tile is
@@ -386,6 +411,7 @@ __global__ void __launch_bounds__(tThreads, 1) pair_transition_kernel(const __gr
   }
   tc_fence_before();
   __syncthreads();
+  cluster_sync_all();                                        // no CTA leaves while its peer may still signal its barriers
   if (warp == 1) {
     __syncwarp();
     tmem_dealloc(tmem_base, 512);
@@ -456,7 +482,8 @@ cudaError_t launch_pair_transition(const void* z_in, void* z_out, int64_t n_pair
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (sms <= 0) sms = 148;
   const int64_t n_tiles = (n_pairs + tM - 1) / tM;
-  const unsigned grid = (unsigned)(n_tiles < sms ? n_tiles : sms);
+  const int64_t n_tpairs = (n_tiles + tCluster - 1) / tCluster, max_clusters = sms / tCluster;
+  const unsigned grid = (unsigned)((n_tpairs < max_clusters ? n_tpairs : max_clusters) * tCluster);
   pair_transition_kernel<<<grid, tThreads, tSmemAlloc, st>>>(maps, n_pairs, eps);
   return cudaGetLastError();
 }
