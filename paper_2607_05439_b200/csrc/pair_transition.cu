@@ -35,7 +35,7 @@ namespace dcp {
 namespace {
 
 constexpr int tCz = 128, tHid = 512, tNC = 128, tChunks = tHid / tNC, tM = 128;
-constexpr int tThreads = 64 + 256;
+constexpr int tThreads = 64 + 256 + 128;     // producer, issuer, 8 epilogue warps, 4 output warps
 constexpr int tCluster = 2;                    // CTA pair: every weight tile is read from L2 once and multicast to both
 constexpr uint16_t tClusterMask = (1u << tCluster) - 1;
 constexpr int tZBytes = tM * tCz * 2;          // 32 KB, two 64-channel halves of 16 KB
@@ -154,7 +154,7 @@ __global__ void __cluster_dims__(tCluster, 1, 1) __launch_bounds__(tThreads, 1) 
     mbar_init(b_w3full, 1); mbar_init(b_w3empty, tCluster);
     mbar_init(b_afull, 1); mbar_init(b_aempty, 8);
     for (int b = 0; b < 2; ++b) { mbar_init(b_hfull + 8 * b, 8); mbar_init(b_hempty + 8 * b, 1); }
-    mbar_init(b_ofull, 1); mbar_init(b_oempty, 8);
+    mbar_init(b_ofull, 1); mbar_init(b_oempty, 4);
     mbar_init(b_xfull, 4); mbar_init(b_xfull + 8, 4);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -230,63 +230,113 @@ __global__ void __cluster_dims__(tCluster, 1, 1) __launch_bounds__(tThreads, 1) 
       // =============================================================== tcgen05 issuer
       constexpr uint32_t idesc1 = umma_idesc_bf16(tM, 256) | (1u << 16);     // B MN-major
       constexpr uint32_t idesc2 = umma_idesc_bf16(tM, 128) | (1u << 16);
-      uint32_t g = 0, n3 = 0, na = 0, nh = 0, nout = 0;
-      for (int it = 0; it < n_it; ++it) {
-        const int zb = it & 1;
+      const uint32_t n_chunks = (uint32_t)n_it * tChunks;
+      // G1 of the CTA's chunk number g (tile g / 4): [A1 | A2] = [z | -mu, 1 / rstd] . [W1'c | W2'c ; c1 ; c0], k-block by k-block
+      auto g1 = [&](uint32_t g) {
+        const uint32_t it = g / tChunks, zb = it & 1;
         const uint32_t zs = s_z + zb * tZBytes;
-        mbar_wait(b_zfull + 8 * zb, (it >> 1) & 1);
-        mbar_wait(b_xfull + 8 * zb, (it >> 1) & 1);          // the epilogue has written this tile's K extension
-        // G1 of the CTA's chunk number g: [A1 | A2] = [z | -mu, 1 / rstd] . [W1'c | W2'c ; c1 ; c0], k-block by k-block
-        auto g1 = [&]() {
-#pragma unroll
-          for (int kb = 0; kb < 2; ++kb) {
-            const uint32_t j = 2 * g + kb, slot = j % 3, use = j / 3;
-            mbar_wait(b_w12full + 8 * slot, use & 1);
-            if (kb == 0) mbar_wait(b_aempty, (na & 1) ^ 1);
-            tc_fence_after();
-            const uint32_t wb = s_w12 + slot * tW12Slot;
-#pragma unroll
-            for (int ks = 0; ks < 4; ++ks)
-              umma_bf16(tmem_base + tColA1, umma_desc_sw128(zs + kb * (tZBytes / 2) + ks * 32), umma_desc_mn(wb + ks * 2048, 8192),
-                        idesc1, (kb | ks) != 0);
-            if (kb == 1) {
-              umma_bf16(tmem_base + tColA1, umma_desc_k_sw32(s_zx + zb * tZxBytes), umma_desc_mn(s_w12x + (g & 1) * tW12xBytes, 2048),
-                        idesc1, 1);
-              umma_commit(b_afull);
-            }
-            umma_commit_mc(b_w12empty + 8 * slot, tClusterMask);   // both CTAs write into this slot
-          }
-          ++g; ++na;
-        };
-        auto g2 = [&](int c) {
-          const uint32_t hb = nh & 1;
-          mbar_wait(b_hfull + 8 * hb, (nh >> 1) & 1);
-          mbar_wait(b_w3full, n3 & 1);
-          if (c == 0) mbar_wait(b_oempty, (nout & 1) ^ 1);
-          tc_fence_after();
-#pragma unroll
-          for (int ks = 0; ks < 8; ++ks)
-            umma_bf16_ts(tmem_base + tColOut, tmem_base + tColH + 64 * hb + 8 * ks,
-                         umma_desc_mn(s_w3 + (ks >> 2) * 16384 + (ks & 3) * 2048, 8192), idesc2, (c | ks) != 0);
-          umma_commit(b_hempty + 8 * hb);
-          umma_commit_mc(b_w3empty, tClusterMask);
-          if (c == tChunks - 1) { umma_commit(b_ofull); ++nout; }
-          ++nh; ++n3;
-        };
-        g1();
-        for (int c = 0; c < tChunks; ++c) {
-          if (c + 1 < tChunks) g1();
-          g2(c);
+        if ((g & (tChunks - 1)) == 0) {
+          mbar_wait(b_zfull + 8 * zb, (it >> 1) & 1);
+          mbar_wait(b_xfull + 8 * zb, (it >> 1) & 1);        // the epilogue has written this tile's K extension
         }
+#pragma unroll
+        for (int kb = 0; kb < 2; ++kb) {
+          const uint32_t j = 2 * g + kb, slot = j % 3, use = j / 3;
+          mbar_wait(b_w12full + 8 * slot, use & 1);
+          if (kb == 0) mbar_wait(b_aempty, (g & 1) ^ 1);
+          tc_fence_after();
+          const uint32_t wb = s_w12 + slot * tW12Slot;
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks)
+            umma_bf16(tmem_base + tColA1, umma_desc_sw128(zs + kb * (tZBytes / 2) + ks * 32), umma_desc_mn(wb + ks * 2048, 8192),
+                      idesc1, (kb | ks) != 0);
+          if (kb == 1) {
+            umma_bf16(tmem_base + tColA1, umma_desc_k_sw32(s_zx + zb * tZxBytes), umma_desc_mn(s_w12x + (g & 1) * tW12xBytes, 2048),
+                      idesc1, 1);
+            umma_commit(b_afull);
+          }
+          umma_commit_mc(b_w12empty + 8 * slot, tClusterMask);   // both CTAs write into this slot
+        }
+      };
+      // G2 of chunk g: OUT (+)= H . W3[rows of the chunk]
+      auto g2 = [&](uint32_t g) {
+        const uint32_t hb = g & 1, c = g & (tChunks - 1);
+        mbar_wait(b_hfull + 8 * hb, (g >> 1) & 1);
+        mbar_wait(b_w3full, g & 1);
+        if (c == 0) mbar_wait(b_oempty, ((g / tChunks) & 1) ^ 1);   // the output warps have read the previous tile's OUT
+        tc_fence_after();
+#pragma unroll
+        for (int ks = 0; ks < 8; ++ks)
+          umma_bf16_ts(tmem_base + tColOut, tmem_base + tColH + 64 * hb + 8 * ks,
+                       umma_desc_mn(s_w3 + (ks >> 2) * 16384 + (ks & 3) * 2048, 8192), idesc2, (c | ks) != 0);
+        umma_commit(b_hempty + 8 * hb);
+        umma_commit_mc(b_w3empty, tClusterMask);
+        if (c == tChunks - 1) umma_commit(b_ofull);
+      };
+      // G1(g + 1) ahead of G2(g), across tile boundaries too: the tensor pipe works on the next chunk while the
+      // epilogue warps turn the previous one into H
+      if (n_chunks) g1(0);
+      for (uint32_t g = 0; g < n_chunks; ++g) {
+        if (g + 1 < n_chunks) g1(g + 1);
+        g2(g);
       }
     }
+  } else if (warp >= 10) {
+    // =============================================================== output warps (one per TMEM lane quadrant)
+    // residual: z + OUT -> bf16, written over the thread's own row of the z tile (every G1 of the tile is complete
+    // once out_full is, and the epilogue warps read a z tile only before its first G1) -> TMA store from there
+    const int quad = warp & 3, ot = threadIdx.x - 320;
+    const int r = quad * 32 + lane;
+    const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16);
+    const uint32_t sw = (uint32_t)(r & 7);
+    for (int it = 0; it < n_it; ++it) {
+      const int64_t tile = tile_of(it);
+      const int zb = it & 1;
+      const uint32_t zrow = s_z + zb * tZBytes + r * 128;   // row base inside a 64-channel half
+      mbar_wait(b_ofull, it & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int sb = 0; sb < 4; ++sb) {                       // 32 channels at a time
+        uint32_t o[32];
+        tmem_ld32(t_lane + tColOut + sb * 32, o);
+        tmem_ld_wait();
+        if (sb == 3) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(b_oempty);              // OUT is in registers: the next tile's G2 may overwrite it
+        }
+#pragma unroll
+        for (int ch = 0; ch < 4; ++ch) {
+          const uint32_t addr = zrow + (sb >> 1) * (tZBytes / 2) + ((((sb & 1) * 4 + ch) ^ sw) << 4);
+          const uint4 zv = lds_u32x4(addr);
+          const uint32_t zw[4] = {zv.x, zv.y, zv.z, zv.w};
+          uint32_t ow[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const float z0 = __uint_as_float(zw[q] << 16), z1 = __uint_as_float(zw[q] & 0xffff0000u);
+            ow[q] = pack_bf16(z0 + __uint_as_float(o[ch * 8 + 2 * q]), z1 + __uint_as_float(o[ch * 8 + 2 * q + 1]));
+          }
+          asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(ow[0]), "r"(ow[1]), "r"(ow[2]), "r"(ow[3]) : "memory");
+        }
+      }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      if (ot == 0) {
+        tma_store_2d(&maps.z_out, 0, (int)(tile * tM), s_z + zb * tZBytes);
+        tma_store_2d(&maps.z_out, 64, (int)(tile * tM), s_z + zb * tZBytes + tZBytes / 2);
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the store has read the buffer: free for z
+        mbar_arrive(b_zempty + 8 * zb);
+      }
+    }
+    if (ot == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
   } else {
     // =============================================================== epilogue warps
-    const int quad = warp & 3, half = (warp - 2) >> 2, et = threadIdx.x - 64;
+    const int quad = warp & 3, half = (warp - 2) >> 2;
     const int r = quad * 32 + lane;                         // tile row = TMEM lane of this thread
     const uint32_t t_lane = tmem_base + ((uint32_t)(quad * 32) << 16);
     const uint32_t sw = (uint32_t)(r & 7);
-    uint32_t na = 0, nh = 0, nout = 0;
+    uint32_t na = 0, nh = 0;
     // LayerNorm statistics of the thread's pair of tile number `jt` (fp32: mu = sum / c_z, var = sum z^2 / c_z - mu^2)
     // and the K extension row [-mu, 1 / rstd, 0 ...] of that z buffer (32-byte swizzle: 16-byte chunk ^ bit 2 of the
     // row); returns rstd.  Called one tile ahead, so that the issuer never waits for it.
@@ -318,9 +368,6 @@ __global__ void __cluster_dims__(tCluster, 1, 1) __launch_bounds__(tThreads, 1) 
     int it = 0;
     float rstd_next = n_it ? prepare(0) : 0.f;
     for (; it < n_it; ++it) {
-      const int64_t tile = tile_of(it);
-      const int zb = it & 1;
-      const uint32_t zrow = s_z + zb * tZBytes + r * 128;   // row base inside a 64-channel half
       const float rstd = rstd_next, hrstd = 0.5f * rstd_next;
 
       for (int c = 0; c < tChunks; ++c) {
@@ -360,54 +407,10 @@ __global__ void __cluster_dims__(tCluster, 1, 1) __launch_bounds__(tThreads, 1) 
         __syncwarp();
         if (lane == 0) mbar_arrive(b_hfull + 8 * hb);
         ++nh;
-        if (c == 0 && it > 0 && et == 0) {                   // the previous tile's store has read its buffer: free for z
-          asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-          mbar_arrive(b_zempty + 8 * (zb ^ 1));
-        }
         if (c == 2 && it + 1 < n_it) rstd_next = prepare(it + 1);   // the next tile's statistics, early
       }
 
-      // ---- residual: z + OUT -> bf16, written over the thread's own bytes of the z tile (every G1 of the tile is
-      // complete once out_full is) -> TMA store from there
-      mbar_wait(b_ofull, nout & 1);
-      tc_fence_after();
-      uint32_t ow[32];
-#pragma unroll
-      for (int sb = 0; sb < 2; ++sb) {
-        uint32_t o[32];
-        tmem_ld32(t_lane + tColOut + half * 64 + sb * 32, o);
-        tmem_ld_wait();
-        if (sb == 1) {
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(b_oempty);
-        }
-#pragma unroll
-        for (int ch = 0; ch < 4; ++ch) {
-          const uint4 zv = lds_u32x4(zrow + half * (tZBytes / 2) + (((sb * 4 + ch) ^ sw) << 4));
-          const uint32_t zw[4] = {zv.x, zv.y, zv.z, zv.w};
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const float z0 = __uint_as_float(zw[q] << 16), z1 = __uint_as_float(zw[q] & 0xffff0000u);
-            ow[sb * 16 + ch * 4 + q] = pack_bf16(z0 + __uint_as_float(o[ch * 8 + 2 * q]), z1 + __uint_as_float(o[ch * 8 + 2 * q + 1]));
-          }
-        }
-      }
-      ++nout;
-      const uint32_t orow = zrow + half * (tZBytes / 2);
-#pragma unroll
-      for (int ch = 0; ch < 8; ++ch)
-        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(orow + ((ch ^ sw) << 4)), "r"(ow[4 * ch]),
-                     "r"(ow[4 * ch + 1]), "r"(ow[4 * ch + 2]), "r"(ow[4 * ch + 3]) : "memory");
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-      if (et == 0) {
-        tma_store_2d(&maps.z_out, 0, (int)(tile * tM), s_z + zb * tZBytes);
-        tma_store_2d(&maps.z_out, 64, (int)(tile * tM), s_z + zb * tZBytes + tZBytes / 2);
-        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-      }
     }
-    if (et == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
   }
   tc_fence_before();
   __syncthreads();
