@@ -37,6 +37,8 @@ NCU_TRAFFIC_BYTES = {
     # (kernel, workload): bytes   -- profiles/r01_fused_c2_ncu_full.txt, profiles/r01_fused_atom_c4_ncu_full.txt
     ("fused_mma_kernel", "C2"): 2330531000 + 7912448,
     ("fused_atom_kernel", "C4"): 18746721000 + 124210176,
+    # profiles/r01_pair_transition_t2_ncu_full.txt (z read once, written once)
+    ("pair_transition_kernel", "T2"): 2305023000 + 2259754000,
 }
 
 
@@ -387,7 +389,7 @@ def run_transition(args, rank, world, local_rank):
         pk = json.load(f)
     peak_tf = float(pk["bf16_tflops_sustained" if kms > 2.0 else "bf16_tflops"])
     roofline = {"bound": "tensor", "achieved": flops / (kms * 1e-3) / 1e12, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": flops / (kms * 1e-3) / 1e12 / peak_tf, "traffic": None, "kernel": "pair_transition_kernel",
+                "frac": flops / (kms * 1e-3) / 1e12 / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(("pair_transition_kernel", args.workload)), "kernel": "pair_transition_kernel",
                 "peak_source": "measured (MEASURED_PEAKS.json, cuBLAS bf16 8192^3: sustained for a > 2 ms kernel, else burst)",
                 "kernel_ms": kms, "kernel_share_of_step": 1.0, "algorithmic_flops_per_launch": flops,
                 "hbm_bytes_per_launch": n_pairs * c_z * 2 * 2, "hbm_gbs": n_pairs * c_z * 4 / (kms * 1e-3) / 1e9}

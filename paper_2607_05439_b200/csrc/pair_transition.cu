@@ -423,12 +423,13 @@ __global__ void __cluster_dims__(tCluster, 1, 1) __launch_bounds__(tThreads, 1) 
 
 // Folded weights [c_z + 16][4 c_z] for W1 and W2: rows k < c_z: bf16(gamma_k W[k][j]); row c_z: c1[j] = sum_k of those
 // rounded values; row c_z + 1: c0[j] = sum_k beta_k W[k][j]; rows c_z + 2 ..: zero (the K extension of the first GEMM)
-__global__ void __launch_bounds__(128) transition_fold_kernel(const __nv_bfloat16* __restrict__ w1, const __nv_bfloat16* __restrict__ w2,
+__global__ void __launch_bounds__(32) transition_fold_kernel(const __nv_bfloat16* __restrict__ w1, const __nv_bfloat16* __restrict__ w2,
                                                              const __nv_bfloat16* __restrict__ gamma, const __nv_bfloat16* __restrict__ beta,
                                                              __nv_bfloat16* __restrict__ w1f, __nv_bfloat16* __restrict__ w2f) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= tHid) return;
   float c11 = 0.f, c01 = 0.f, c12 = 0.f, c02 = 0.f;
+#pragma unroll 16
   for (int k = 0; k < tCz; ++k) {
     const float g = to_f32(gamma[k]), b = to_f32(beta[k]);
     const float a = to_f32(w1[k * tHid + j]), c = to_f32(w2[k * tHid + j]);
@@ -467,7 +468,7 @@ cudaError_t launch_pair_transition(const void* z_in, void* z_out, int64_t n_pair
   if (!enc) return cudaErrorNotSupported;
   __nv_bfloat16* w1f = reinterpret_cast<__nv_bfloat16*>(workspace);
   __nv_bfloat16* w2f = w1f + (tCz + tKx) * tHid;
-  transition_fold_kernel<<<tHid / 128, 128, 0, st>>>((const __nv_bfloat16*)w1, (const __nv_bfloat16*)w2,
+  transition_fold_kernel<<<tHid / 32, 32, 0, st>>>((const __nv_bfloat16*)w1, (const __nv_bfloat16*)w2,
                                                      (const __nv_bfloat16*)gamma, (const __nv_bfloat16*)beta, w1f, w2f);
   TransMaps maps;
   if (encode2d(enc, &maps.z_in, z_in, tCz, (uint64_t)n_pairs, 64, tM) != CUDA_SUCCESS ||
