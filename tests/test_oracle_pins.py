@@ -490,3 +490,65 @@ def test_transition_special_cases():
     zs = 3.0 * z + 7.0
     t3 = pto.pair_transition(zs, w1, w2, w3, gamma, beta, eps=0.0) - zs
     assert np.max(np.abs(t3 - (pto.pair_transition(z, w1, w2, w3, gamma, beta, eps=0.0) - z))) <= 1e-11
+
+
+# ---------------------------------------------------------------- Pairformer stack (oracle/pairformer_stack.py)
+def _stack_problem(rng, I=5, c_s=6, c_z=4, H=2, c=3, n_blocks=2):
+    s, z, _ = rand_problem(rng, I, c_s, c_z, H, c)
+    blocks = []
+    for _ in range(n_blocks):
+        _, _, w = rand_problem(rng, I, c_s, c_z, H, c)
+        _, w1, w2, w3, gamma, beta = _transition_problem(rng, n_pairs=1, c_z=c_z)
+        blocks.append((w, {"w1": w1, "w2": w2, "w3": 3.0 * w3, "gamma": gamma, "beta": beta}))   # a transition that moves z a lot
+    return s, z, blocks
+
+
+def _brute_attention(s, z, w, H, c):
+    tl = lambda x: np.asarray(x).tolist()
+    return np.array(brute.brute_force(tl(s), tl(z), tl(w["w_q"]), tl(w["w_k"]), tl(w["w_v"]), tl(w["w_g"]), tl(w["w_b"]),
+                                      tl(w["w_o"]), tl(w["ln_z_gamma"]), tl(w["ln_z_beta"]), H, c))
+
+
+def test_stack_identity_when_output_weights_vanish():
+    from oracle import pairformer_stack as pso
+    s, z, blocks = _stack_problem(np.random.default_rng(71), n_blocks=3)
+    for w, t in blocks:
+        w["w_o"] = np.zeros_like(w["w_o"])
+        t["w3"] = np.zeros_like(t["w3"])
+    s3, z3 = pso.pairformer_stack(s, z, blocks, 2, 3)
+    assert np.array_equal(s3, s) and np.array_equal(z3, z)
+
+
+def test_stack_order_against_brute_force():
+    """Attention of block b reads the Z that block b - 1 left (not the original, not the one its own transition writes)."""
+    from oracle import pairformer_stack as pso
+    H, c = 2, 3
+    s, z, blocks = _stack_problem(np.random.default_rng(72), n_blocks=2)
+    s1, z1 = pso.pairformer_stack(s, z, blocks[:1], H, c)
+    s2, z2 = pso.pairformer_stack(s, z, blocks, H, c)
+    t0, t1 = blocks[0][1], blocks[1][1]
+    # the transition really moves z (otherwise the order pins below would be vacuous)
+    assert np.max(np.abs(z1 - z)) > 0.5
+    assert np.max(np.abs(s1 - (s + _brute_attention(s, z, blocks[0][0], H, c)))) <= 1e-12      # block 1: original z
+    assert np.max(np.abs(s1 - (s + _brute_attention(s, z1, blocks[0][0], H, c)))) > 1e-3       # ... not the updated one
+    assert np.max(np.abs(s2 - (s1 + _brute_attention(s1, z1, blocks[1][0], H, c)))) <= 1e-12   # block 2: (s1, z1)
+    # the pair track: the transition applied block by block (torch composition as the independent routine)
+    def tr(zz, t):
+        tz = torch.from_numpy(zz)
+        n = torch.nn.functional.layer_norm(tz, (zz.shape[-1],), torch.from_numpy(t["gamma"]), torch.from_numpy(t["beta"]), 1e-5)
+        return (tz + (torch.nn.functional.silu(n @ torch.from_numpy(t["w1"])) * (n @ torch.from_numpy(t["w2"])))
+                @ torch.from_numpy(t["w3"])).numpy()
+    assert np.max(np.abs(z1 - tr(z, t0))) <= 1e-12
+    assert np.max(np.abs(z2 - tr(tr(z, t0), t1))) <= 1e-11
+
+
+def test_stack_round_store_is_applied_once_per_block():
+    from oracle import pairformer_stack as pso
+    H, c = 2, 3
+    s, z, blocks = _stack_problem(np.random.default_rng(73), n_blocks=2)
+    bf = lambda x: torch.from_numpy(np.asarray(x)).to(torch.bfloat16).double().numpy()
+    s2, z2 = pso.pairformer_stack(bf(s), bf(z), blocks, H, c, round_store=bf)
+    assert np.array_equal(bf(s2), s2) and np.array_equal(bf(z2), z2)
+    s1, z1 = pso.pairformer_block(bf(s), bf(z), *blocks[0], H, c, round_store=bf)
+    s2b, z2b = pso.pairformer_block(s1, z1, *blocks[1], H, c, round_store=bf)
+    assert np.array_equal(s2, s2b) and np.array_equal(z2, z2b)
