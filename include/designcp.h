@@ -129,6 +129,28 @@ dcp_status dcp_pair_transition(const void *z, void *z_out, int64_t n_pairs, int 
                                const void *w3, const void *ln_gamma, const void *ln_beta, float ln_eps, dcp_dtype dtype,
                                void *workspace, size_t workspace_bytes, void *stream);
 
+/* A stack of non-triangular Pairformer blocks on a resident pair tensor (first step).
+ * PAPER.md:289 "The Pairformer block ... is ... an AttentionPairBias (16 heads, optional QK-norm) followed by a Transition
+ * module; both stock configurations explicitly disable the ... triangle multiplication and triangle attention paths";
+ * :293 "Two non-triangular Pairformer blocks (each 16-head AttentionPairBias + Transition) then refine (S, Z)".
+ * Block b (reading 23):   S <- S + AttentionPairBias_b(S, Z)   (dcp_pair_bias_attention, MONOLITHIC)
+ *                                   Z <- Z + Transition_b(Z)             (dcp_pair_transition, Eq. 6)
+ * and block b + 1 sees the updated (S, Z).  s [I, c_s] and z [I, I, c_z] are device tensors updated IN PLACE, stored in
+ * the storage dtype after every block.  blocks: HOST array of n_blocks entries whose pointers are device pointers
+ * (attn as in dcp_pair_bias_attention; w1, w2 [c_z, 4 c_z], w3 [4 c_z, c_z], ln_gamma, ln_beta [c_z] as in
+ * dcp_pair_transition); it is read during the call only.  DCP_BF16 with c_z = 128 and an (H, c) the fused kernel is
+ * instantiated for (DCP_ERR_UNSUPPORTED otherwise); I * I < 2^31.  workspace >= dcp_pairformer_stack_workspace_bytes,
+ * 256-byte aligned.  Enqueues 7 launches per block on `stream` and returns. */
+typedef struct {
+  dcp_weights attn;
+  const void *w1, *w2, *w3, *ln_gamma, *ln_beta;
+  float ln_eps; /* <= 0 means 1e-5 */
+} dcp_block_weights;
+dcp_status dcp_pairformer_stack_workspace_bytes(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype, size_t *bytes);
+dcp_status dcp_pairformer_stack(void *s, void *z, const dcp_block_weights *blocks, int n_blocks, int64_t I, int c_s,
+                                int H, int c, int c_z, dcp_dtype dtype, void *workspace, size_t workspace_bytes,
+                                void *stream);
+
 /* p_slice[l, j, :] = p[l, idx[l, j], :] ("The relevant slice of P is gathered at those k indices"): the
  * dense atom-pair tensor p [L, L, c_atompair] (row pitch ldp elements, 0 = L * c_atompair) -> the slice
  * [L, k, c_atompair] that dcp_sparse_atom_attention consumes; slots with idx < 0 are filled with zeros.  Device

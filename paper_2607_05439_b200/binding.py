@@ -29,6 +29,7 @@ EXPORTS = [
     "dcp_pair_bias_attention_host", "dcp_partial_states", "dcp_merge_states", "dcp_shard_range",
     "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention", "dcp_knn", "dcp_gather_pair_slice",
     "dcp_pair_transition_workspace_bytes", "dcp_pair_transition",
+    "dcp_pairformer_stack_workspace_bytes", "dcp_pairformer_stack",
     "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
     "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
 ]
@@ -43,6 +44,11 @@ class DcpError(RuntimeError):
 class dcp_weights(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in (
         "w_q", "w_k", "w_v", "w_g", "w_b", "w_o", "ln_z_gamma", "ln_z_beta", "ln_s_gamma", "ln_s_beta", "b_q")]
+    _fields_ += [("ln_eps", C.c_float)]
+
+
+class dcp_block_weights(C.Structure):
+    _fields_ = [("attn", dcp_weights)] + [(n, C.c_void_p) for n in ("w1", "w2", "w3", "ln_gamma", "ln_beta")]
     _fields_ += [("ln_eps", C.c_float)]
 
 
@@ -88,7 +94,9 @@ def _load() -> C.CDLL:
     lib.dcp_gather_pair_slice.argtypes = [vp, i64, vp, vp, i64, i32, i32, i32, vp]
     lib.dcp_pair_transition_workspace_bytes.argtypes = [i32, i32, C.POINTER(sz)]
     lib.dcp_pair_transition.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, C.c_float, i32, vp, sz, vp]
-    for n in EXPORTS[:13]:
+    lib.dcp_pairformer_stack_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, i32, C.POINTER(sz)]
+    lib.dcp_pairformer_stack.argtypes = [vp, vp, C.POINTER(dcp_block_weights), i32, i64, i32, i32, i32, i32, i32, vp, sz, vp]
+    for n in EXPORTS[:15]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -239,6 +247,31 @@ def dcp_pair_transition(z, w1, w2, w3, ln_gamma, ln_beta, eps=1e-5, out=None, wo
                                   C.c_float(eps), _dtype_code(z.dtype), _ptr(workspace), workspace.numel(), _stream_ptr(stream))
     _check(st, "dcp_pair_transition")
     return out
+
+
+def dcp_pairformer_stack(s, z, blocks, H, c, eps=1e-5, workspace=None, stream=None):
+    """n_blocks non-triangular Pairformer blocks, IN PLACE on s [I, c_s] and z [I, I, c_z]:
+    s += AttentionPairBias_b(s, z); z += Transition_b(z).  blocks: sequence of (attention weights dict, transition
+    dict with w1, w2, w3, gamma, beta)."""
+    assert s.is_cuda and z.is_cuda and s.is_contiguous() and z.is_contiguous()
+    I, c_s, c_z = s.shape[0], s.shape[1], z.shape[-1]
+    arr = (dcp_block_weights * len(blocks))()
+    for b, (wa, wt) in enumerate(blocks):
+        arr[b].attn = _weights_struct(wa, eps)
+        for dst, src in (("w1", "w1"), ("w2", "w2"), ("w3", "w3"), ("ln_gamma", "gamma"), ("ln_beta", "beta")):
+            t = wt[src]
+            assert t.is_cuda and t.is_contiguous(), src
+            setattr(arr[b], dst, t.data_ptr())
+        arr[b].ln_eps = float(eps)
+    if workspace is None:
+        n = C.c_size_t(0)
+        _check(_lib.dcp_pairformer_stack_workspace_bytes(I, c_s, H, c, c_z, _dtype_code(s.dtype), C.byref(n)),
+               "dcp_pairformer_stack_workspace_bytes")
+        workspace = _alloc_ws(int(n.value), s.device)
+    st = _lib.dcp_pairformer_stack(_ptr(s), _ptr(z), arr, len(blocks), I, c_s, H, c, c_z, _dtype_code(s.dtype), _ptr(workspace),
+                                   workspace.numel(), _stream_ptr(stream))
+    _check(st, "dcp_pairformer_stack")
+    return s, z
 
 
 def dcp_gather_pair_slice(p, idx, out=None, stream=None):

@@ -479,6 +479,67 @@ dcp_status dcp_pair_transition(const void* z, void* z_out, int64_t n_pairs, int 
   return DCP_OK;
 }
 
+// s <- bf16(s + o), eight elements per thread
+static __global__ void __launch_bounds__(256) residual_add_bf16_kernel(__nv_bfloat16* __restrict__ s, const __nv_bfloat16* __restrict__ o,
+                                                                int64_t n8) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n8) return;
+  uint4 a = reinterpret_cast<const uint4*>(s)[i];
+  const uint4 b = reinterpret_cast<const uint4*>(o)[i];
+  __nv_bfloat162* pa = reinterpret_cast<__nv_bfloat162*>(&a);
+  const __nv_bfloat162* pb = reinterpret_cast<const __nv_bfloat162*>(&b);
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const float2 x = __bfloat1622float2(pa[j]), y = __bfloat1622float2(pb[j]);
+    pa[j] = __floats2bfloat162_rn(x.x + y.x, x.y + y.y);
+  }
+  reinterpret_cast<uint4*>(s)[i] = a;
+}
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+dcp_status dcp_pairformer_stack_workspace_bytes(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype, size_t* bytes) {
+  if (!bytes) return DCP_ERR_INVALID_ARG;
+  size_t attn = 0;
+  dcp_status st = dcp_workspace_bytes(I, c_s, H, c, c_z, dtype, DCP_MONOLITHIC, nullptr, &attn);
+  if (st != DCP_OK) return st;
+  if (!pair_transition_supports(dtype, c_z)) return DCP_ERR_UNSUPPORTED;
+  *bytes = align256(attn) + align256((size_t)I * c_s * elt_size(dtype)) + align256(pair_transition_workspace_bytes());
+  return DCP_OK;
+}
+
+dcp_status dcp_pairformer_stack(void* s, void* z, const dcp_block_weights* blocks, int n_blocks, int64_t I, int c_s, int H,
+                                int c, int c_z, dcp_dtype dtype, void* workspace, size_t workspace_bytes, void* stream) {
+  g_launches = 0;
+  if (!s || !z || !blocks || !workspace || n_blocks <= 0) return DCP_ERR_INVALID_ARG;
+  size_t need = 0, attn = 0;
+  dcp_status st = dcp_pairformer_stack_workspace_bytes(I, c_s, H, c, c_z, dtype, &need);
+  if (st != DCP_OK) return st;
+  if (workspace_bytes < need) return DCP_ERR_WORKSPACE;
+  if (((uintptr_t)workspace & 255) != 0 || (((uintptr_t)s | (uintptr_t)z) & 15) != 0 || (I * c_s) % 8 != 0) return DCP_ERR_INVALID_ARG;
+  if (I * I > 0x7fffff00ll) return DCP_ERR_INVALID_ARG;
+  dcp_workspace_bytes(I, c_s, H, c, c_z, dtype, DCP_MONOLITHIC, nullptr, &attn);
+  char* ws = reinterpret_cast<char*>(workspace);
+  void* ws_attn = ws;
+  void* o = ws + align256(attn);
+  void* ws_tr = ws + align256(attn) + align256((size_t)I * c_s * elt_size(dtype));
+  int launches = 0;
+  for (int b = 0; b < n_blocks; ++b) {
+    const dcp_block_weights& w = blocks[b];
+    st = layer(s, z, 0, &w.attn, o, I, c_s, H, c, c_z, dtype, DCP_MONOLITHIC, nullptr, ws_attn, attn, stream);   // AttentionPairBias
+    if (st != DCP_OK) return st;
+    launches += g_launches;
+    const int64_t n8 = I * c_s / 8;
+    residual_add_bf16_kernel<<<(unsigned)((n8 + 255) / 256), 256, 0, (cudaStream_t)stream>>>((__nv_bfloat16*)s, (const __nv_bfloat16*)o, n8);
+    if (cudaGetLastError() != cudaSuccess) return DCP_ERR_CUDA;
+    st = dcp_pair_transition(z, z, I * I, c_z, w.w1, w.w2, w.w3, w.ln_gamma, w.ln_beta, w.ln_eps, dtype, ws_tr,
+                             pair_transition_workspace_bytes(), stream);                                       // Transition, Eq. 6
+    if (st != DCP_OK) return st;
+    launches += 1 + g_launches;
+  }
+  g_launches = launches;
+  return DCP_OK;
+}
+
 dcp_status dcp_knn(const float* x, int32_t* idx, int64_t L, int k, void* stream) {
   g_launches = 0;
   if (!x || !idx || L <= 0 || k <= 0 || k > L) return DCP_ERR_INVALID_ARG;
