@@ -48,7 +48,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4", "K4", "T2", "T3"],
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4", "K4", "T2", "T3", "P2"],
                     help="C0..C4: BASELINE.json configs (dense layer); S4: sparse k-neighbour atom attention on C4's atoms; "
                          "K4: the k-nearest-neighbour lists of C4's atoms (dcp_knn); T2 / T3: the pairwise SwiGLU transition on "
                          "C2's / C3's pair tensor (dcp_pair_transition)")
@@ -56,6 +56,7 @@ def parse():
     ap.add_argument("--decomp", default="monolithic", choices=["monolithic", "row", "grid"])
     ap.add_argument("--parts", type=int, default=0, help="row stripes / grid cells (0: 8 rows, 16 grid)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "mma"])
+    ap.add_argument("--blocks", type=int, default=2, help="P2: Pairformer blocks in the stack (PAPER.md:293: two)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-rows", type=int, default=0, help="oracle sample rows (0: sized for ~10-20 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -179,6 +180,28 @@ def run_reference(args, rank, world):
                           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                           "config": {"workload": f"K4: k-nearest-neighbour lists L={cfg.I} k={args.neighbours}", "sample": sample},
                           "cpu_baseline": {"value": value, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
+                          "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                          "gpu_launches": 0}), flush=True)
+        return
+    if args.workload == "P2":
+        cfg = syn.CONFIGS["C2"]
+        dev = "cuda:0" if torch.cuda.is_available() else "cpu"
+        blocks = stack_blocks(cfg, 1, dev)
+        s, z = syn.make_s(cfg, dev), syn.make_z(cfg, dev)
+        n_rows = args.cpu_rows or 400
+        pairs = secs = 0.0
+        threads = 1
+        for k in range(args.steps):
+            p, dt, threads, _, _, _ = stack_oracle_sample(cfg, s, z, blocks[0], n_rows, seed=k)
+            pairs += p
+            secs += dt
+        value = pairs / secs / 1e9
+        sample = f"one block on {n_rows} sampled query rows x {cfg.I} keys per step ({args.steps} steps), fp64 numpy oracle"
+        print(json.dumps({"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / max(args.steps, 1) * 1e3,
+                          "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                          "config": {"workload": f"P2: Pairformer blocks on I={cfg.I}", "sample": sample},
+                          "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
                           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
                           "gpu_launches": 0}), flush=True)
         return
@@ -443,6 +466,155 @@ def run_transition(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def stack_blocks(cfg, n_blocks, dev):
+    """Seeded weights of the P2 stack: per block the layer weights (seed offset by block) and the transition weights."""
+    import dataclasses
+    import math
+    import torch
+    import dcp_synth as syn
+    blocks = []
+    for b in range(n_blocks):
+        wa = syn.make_weights(dataclasses.replace(cfg, seed=cfg.seed + 31 * (b + 1)), dev)
+        g = torch.Generator(device="cpu").manual_seed(cfg.seed * 1000003 + 131 + b)
+        rn = lambda *sh, std=1.0: (torch.randn(*sh, generator=g) * std).to(torch.bfloat16).to(dev)
+        c_z = cfg.c_z
+        blocks.append((wa, {"w1": rn(c_z, 4 * c_z, std=1 / math.sqrt(c_z)), "w2": rn(c_z, 4 * c_z, std=1 / math.sqrt(c_z)),
+                            "w3": rn(4 * c_z, c_z, std=1 / math.sqrt(4 * c_z)),
+                            "gamma": (1 + 0.1 * torch.randn(c_z, generator=g)).to(torch.bfloat16).to(dev),
+                            "beta": (0.1 * torch.randn(c_z, generator=g)).to(torch.bfloat16).to(dev)}))
+    return blocks
+
+
+def stack_oracle_sample(cfg, s, z, block, n_rows, seed=0):
+    """The oracle's block (oracle/pairformer_stack.py) on `n_rows` sampled query rows: the attention rows and the
+    transition of those rows' I pairs each.  Returns (pairs, seconds, threads, rows, s_rows_new, z_rows_new)."""
+    import numpy as np
+    import torch
+    from oracle import pair_transition as pto
+    wa, wt = block
+    pairs, dt, threads, rows, attn = oracle_sample(cfg, s, z, wa, n_rows, seed=seed)
+    f64 = lambda t: t.detach().float().cpu().double().numpy()
+    z_rows = f64(z.index_select(0, torch.as_tensor(rows, device=z.device)))
+    t0 = time.perf_counter()
+    z_new = pto.pair_transition(z_rows, f64(wt["w1"]), f64(wt["w2"]), f64(wt["w3"]), f64(wt["gamma"]), f64(wt["beta"]))
+    dt += time.perf_counter() - t0
+    s_new = f64(s)[np.asarray(rows)] + attn
+    return pairs, dt, threads, rows, s_new, z_new
+
+
+def run_stack(args, rank, world, local_rank):
+    """--workload P2 (first step): --blocks non-triangular Pairformer blocks in
+    place on C2's resident (S, Z).  One pair = one (block, token pair): blocks * I^2 per step."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as ge
+    if rank == 0 or world == 1:
+        ge.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    import dcp_synth as syn
+    import paper_2607_05439_b200 as dcp
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    cfg = replica_config(syn.CONFIGS["C2"], rank, world)
+    nb = args.blocks
+    blocks = stack_blocks(cfg, nb, dev)
+    s0, z0 = syn.make_s(cfg, dev), syn.make_z(cfg, dev)
+    s, z = s0.clone(), z0.clone()
+    n_pairs = float(cfg.I) * cfg.I * nb
+    # every step continues from the previous state (the tracks stay finite: LayerNorm inside both updates); inputs
+    # are restored before the parity sample below
+    for _ in range(max(args.warmup, 3)):
+        dcp.dcp_pairformer_stack(s, z, blocks, cfg.H, cfg.c)
+    launches = dcp.dcp_last_launch_count()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = dcp.Event(), dcp.Event()
+    e0.record()
+    for _ in range(args.steps):
+        dcp.dcp_pairformer_stack(s, z, blocks, cfg.H, cfg.c)
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = max_over_ranks_ms(e0.elapsed_ms(e1), world, dev)
+    step_ms = total_ms / args.steps
+    value = n_pairs * args.steps * world / (total_ms * 1e-3) / 1e9
+    # the dominant kernel (pair_transition_kernel, tensor bound) timed on the same z with events of its own
+    wt = blocks[0][1]
+    k0, k1 = dcp.Event(), dcp.Event()
+    dcp.dcp_pair_transition(z, wt["w1"], wt["w2"], wt["w3"], wt["gamma"], wt["beta"], out=z)
+    k0.record()
+    for _ in range(args.steps):
+        dcp.dcp_pair_transition(z, wt["w1"], wt["w2"], wt["w3"], wt["gamma"], wt["beta"], out=z)
+    k1.record()
+    torch.cuda.synchronize()
+    kms = k0.elapsed_ms(k1) / args.steps
+    c_z = cfg.c_z
+    flops = float(cfg.I) * cfg.I * (2.0 * c_z * 4 * c_z * 2 + 2.0 * 4 * c_z * c_z)
+    with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+        pk = json.load(f)
+    peak_tf = float(pk["bf16_tflops_sustained" if kms > 2.0 else "bf16_tflops"])
+    roofline = {"bound": "tensor", "achieved": flops / (kms * 1e-3) / 1e12, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": flops / (kms * 1e-3) / 1e12 / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(("pair_transition_kernel", "T2")),
+                "kernel": "pair_transition_kernel", "kernel_ms": kms, "kernel_share_of_step": nb * kms / step_ms,
+                "peak_source": "measured (MEASURED_PEAKS.json, cuBLAS bf16 8192^3: sustained for a > 2 ms kernel, else burst)",
+                "algorithmic_flops_per_launch": flops, "launches_per_step": nb}
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        n_rows = args.cpu_rows or 400
+        pairs, dt, threads, rows, s_ref, z_ref = stack_oracle_sample(cfg, s0, z0, blocks[0], n_rows)
+        s1, z1 = s0.clone(), z0.clone()
+        dcp.dcp_pairformer_stack(s1, z1, blocks[:1], cfg.H, cfg.c)
+        idx = torch.as_tensor(rows, device=dev)
+        f64 = lambda t: t.detach().float().cpu().double().numpy()
+        gs, gz = f64(s1.index_select(0, idx)), f64(z1.index_select(0, idx))
+        cpu = {"value": pairs / dt / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"block 1 of the stack on {len(rows)} sampled query rows x {cfg.I} keys ({dt:.1f} s), fp64 numpy oracle",
+               "gpu_vs_oracle_rel_l2_s": float(np.linalg.norm(gs - s_ref) / np.linalg.norm(s_ref)),
+               "gpu_vs_oracle_rel_l2_z": float(np.linalg.norm(gz - z_ref) / np.linalg.norm(z_ref)),
+               "gpu_vs_oracle_within_tolerance": bool(np.all(np.abs(gs - s_ref) <= 2e-2 + 2.0 ** -8 * np.abs(s_ref))
+                                                      and np.all(np.abs(gz - z_ref) <= 2e-2 + 2.0 ** -8 * np.abs(z_ref)))}
+    e2e = None
+    if not args.no_e2e:
+        sh, zh = s0.cpu().pin_memory(), z0.cpu().pin_memory()
+        so = torch.empty(s0.shape, dtype=s0.dtype).pin_memory()
+        ne = max(1, args.e2e_steps)
+        a, b = dcp.Event(), dcp.Event()
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(ne):
+            s.copy_(sh, non_blocking=True)
+            z.copy_(zh, non_blocking=True)
+            dcp.dcp_pairformer_stack(s, z, blocks, cfg.H, cfg.c)
+            so.copy_(s, non_blocking=True)
+        b.record()
+        torch.cuda.synchronize()
+        ms = max_over_ranks_ms(a.elapsed_ms(b), world, dev)
+        e2e = {"value": n_pairs * ne * world / (ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": (sh.numel() + zh.numel()) * 2,
+               "d2h_bytes_per_step": so.numel() * 2, "steps": ne, "note": "PCIe host->device copy of z dominates"}
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic",
+            "config": {"workload": f"P2: {nb} non-triangular Pairformer blocks (AttentionPairBias + pair Transition) in place on "
+                                   f"I={cfg.I} c_s={cfg.c_s} c_z={c_z} H={cfg.H} c={cfg.c} bf16 (icosahedral 60 x {cfg.n_res})",
+                       "pair": "one (block, token pair)", "blocks": nb, "kernel": "pair_transition_kernel",
+                       "l2": "z (%.0f MB) larger than the 126 MB L2: no flush needed" % (z.numel() * 2 / 1e6),
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "peak_device_bytes": int(torch.cuda.max_memory_allocated())},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": launches * (args.steps + max(args.warmup, 3)), "clocks": clocks}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def run_knn(args, rank, world, local_rank):
     """--workload K4: neighbour lists of C4's 24000 synthetic atoms, k = --neighbours.
     One pair = one (query atom, candidate atom) distance: L^2 per call.  Single GPU (or independent replicas)."""
@@ -686,6 +858,9 @@ def main():
         return
     if args.workload in ("T2", "T3"):
         run_transition(args, rank, world, local_rank)
+        return
+    if args.workload == "P2":
+        run_stack(args, rank, world, local_rank)
         return
 
     import torch
