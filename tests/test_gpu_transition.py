@@ -85,3 +85,22 @@ def test_transition_error_paths():
     with pytest.raises(dcp.DcpError) as e:
         dcp.dcp_pair_transition(torch.zeros(10, C_Z, device=DEV), *[t.float() for t in w])
     assert e.value.status == 2
+
+
+def test_transition_full_size_sampled():
+    """C2's pair tensor (I = 3000, 9.0 M pairs), the launch configuration bench.py --workload T2 times: sampled pairs
+    (first / last, both sides of tile and CTA-pair boundaries, seeded random ones) against the oracle, in place."""
+    dcp = _dcp()
+    import dcp_synth as syn
+    cfg = syn.CONFIGS["C2"]
+    z = syn.make_z(cfg, DEV)
+    w = _weights(11)
+    n_pairs = cfg.I * cfg.I
+    g = torch.Generator(device="cpu").manual_seed(5)
+    idx = torch.cat([torch.tensor([0, 1, 127, 128, 129, 255, 256, 148 * 128 - 1, 148 * 128, 148 * 128 + 1, n_pairs - 129,
+                                   n_pairs - 128, n_pairs - 2, n_pairs - 1]),
+                     torch.randint(0, n_pairs, (4000,), generator=g)]).to(DEV)
+    zs = z.reshape(-1, C_Z).index_select(0, idx)
+    dcp.dcp_pair_transition(z, *w, out=z)
+    torch.cuda.synchronize()
+    _check(z.reshape(-1, C_Z).index_select(0, idx), zs, w, "transition I=3000 sampled")
