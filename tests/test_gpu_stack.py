@@ -102,3 +102,27 @@ def test_stack_error_paths():
     with pytest.raises(dcp.DcpError):                       # fp32 / c_z = 64: the transition is not instantiated
         dcp.dcp_pairformer_stack(syn.make_s(cfg32, DEV), syn.make_z(cfg32, DEV),
                                  [(syn.make_weights(cfg32, DEV), blocks[0][1])], cfg32.H, cfg32.c)
+
+
+def test_stack_full_size_block_sampled():
+    """One block at C2's full size (I = 3000: the shape bench.py --workload P2 times): sampled query rows of S and the
+    same rows of Z against the oracle's block (the attention rows oracle + the transition of those rows' pairs)."""
+    dcp = _dcp()
+    from oracle import pair_bias_attention as orc
+    from oracle import pair_transition as pto
+    cfg = syn.CONFIGS["C2"]
+    s0, z0 = syn.make_s(cfg, DEV), syn.make_z(cfg, DEV)
+    (wa, wt), = _blocks(cfg, 1)
+    rows = syn.sample_rows(cfg.I, 24, boundaries=(32, 1000, 2000), seed=3)
+    idx = torch.as_tensor(rows, device=DEV)
+    z_rows0 = util.np64(z0.index_select(0, idx))
+    s_ref = util.np64(s0)[np.asarray(rows)] + orc.pair_bias_attention_rows(
+        util.np64(s0), z_rows0, rows, {k: util.np64(v) for k, v in wa.items()}, cfg.H, cfg.c)
+    z_ref = pto.pair_transition(z_rows0, *[util.np64(wt[k]) for k in ("w1", "w2", "w3", "gamma", "beta")])
+    s, z = s0.clone(), z0
+    dcp.dcp_pairformer_stack(s, z, [(wa, wt)], cfg.H, cfg.c)
+    torch.cuda.synchronize()
+    for name, got, ref in (("s", util.np64(s.index_select(0, idx)), s_ref), ("z", util.np64(z.index_select(0, idx)), z_ref)):
+        rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+        assert rel <= 1e-2, f"{name}: rel-L2 {rel:.3e}"
+        assert np.all(np.abs(got - ref) <= 2e-2 + 2.0 ** -8 * np.abs(ref)), f"{name}: max-abs {np.abs(got - ref).max():.3e}"
