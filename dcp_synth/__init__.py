@@ -252,3 +252,25 @@ def make_p_slice(cfg: LayerConfig, idx: torch.Tensor, device="cpu", noise: float
         blk += noise * torch.randn(i1 - i0, k, cfg.c_z, generator=g, device=device, dtype=torch.float32)
         out[i0:i1] = blk.to(out.dtype)
     return out
+
+
+# ------------------------------------------------------------------ LayerNorm edge cases (per-pair affine shifts)
+def affine_pairs(z: torch.Tensor, a: float, t: float, seed: int = 0, n_const: int = 0) -> torch.Tensor:
+    """Edge-case inputs for the pair LayerNorm: every pair (leading dims of z; the last dim is the channel axis) becomes
+    a * z + t_pair * 1 with t_pair = +-|t| * U(0.5, 1) (seeded sign and magnitude), computed in fp32 and rounded once to
+    z's dtype; `n_const` seeded pairs are then overwritten by a constant across channels (variance exactly 0).
+    LayerNorm is invariant under such a map up to the epsilon term and the storage rounding ("LN axis
+    and affine"), so the layer's output barely moves while |mean| / sigma of a pair grows to |t| / (1.4 a)."""
+    g = _gen(seed * 7919 + 3, "cpu")
+    lead = z.shape[:-1]
+    n = int(torch.tensor(lead).prod()) if len(lead) else 1
+    sign = torch.where(torch.rand(n, generator=g) < 0.5, -1.0, 1.0)
+    mag = 0.5 + 0.5 * torch.rand(n, generator=g)
+    tp = (float(t) * sign * mag).reshape(*lead, 1).to(z.device)
+    out = (float(a) * z.float() + tp).to(z.dtype)
+    if n_const > 0:
+        flat = out.reshape(n, z.shape[-1])
+        pick = torch.randperm(n, generator=g)[:min(n_const, n)].to(z.device)
+        flat[pick] = flat[pick][:, :1].expand(-1, z.shape[-1]).clone()
+        out = flat.reshape(z.shape)
+    return out.contiguous()

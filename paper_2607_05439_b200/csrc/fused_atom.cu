@@ -213,8 +213,8 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
               const int m = half * 4 + i;
               // LayerNorm statistics (fp32): mu = sum/c_z, var = sum z^2 / c_z - mu^2
               const float mu = v[i][aH] * (1.f / aCz);
-              const float var = fmaxf(fmaf(zsq[m], 1.f / aCz, -mu * mu), 0.f);
-              const float rstd = rsqrtf(var + p.eps);
+              const float var = fmaf(-mu, mu, zsq[m] * (1.f / aCz));   // one rounding; == 0 exactly for a constant row
+              const float rstd = var > 0.f ? rsqrtf(var + p.eps) : 0.f;  // (fused_mma.cu has the argument)
               const float nm = -mu * rstd;
               // bias[h][query][key ^ 16 (query odd)]: the XOR makes the attention warps' 128-bit reads conflict-free
               const int ql = sub * aSubQ + 4 * m + pw;

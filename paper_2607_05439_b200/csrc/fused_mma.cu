@@ -211,10 +211,14 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           __syncwarp();
           if (lane == 0) mbar_arrive(bar_tempty + 8 * tb);    // accumulators are in registers: buffer free
           if (++tb == kNT) { tb = 0; tphase ^= 1; }
-          // LayerNorm statistics (fp32): mu = sum/c_z, var = sum z^2 / c_z - mu^2
+          // LayerNorm statistics (fp32): mu = sum / c_z, var = sum z^2 / c_z - mu^2 with ONE rounding: c_z is a power of
+          // two, so sum z^2 / c_z is exact, and the FMA subtracts the unrounded mu^2.  The sums themselves are exact
+          // whenever the row's values span few binades (bf16 x bf16 products have 16 significant bits), which is exactly
+          // when |mu| >> sigma makes the subtraction cancel; a constant row gives var == 0 exactly, and then LN(z) = beta:
+          // rstd = 0 keeps the tensor pipe's rounding residue of z.W' - mu c1 from being amplified by 1 / sqrt(eps).
           const float mu = zsum * (1.f / kCz);
-          const float var = fmaxf(fmaf(zsq, 1.f / kCz, -mu * mu), 0.f);
-          const float rstd = rsqrtf(var + p.eps);
+          const float var = fmaf(-mu, mu, zsq * (1.f / kCz));
+          const float rstd = var > 0.f ? rsqrtf(var + p.eps) : 0.f;
           const float nm = -mu * rstd;
           // ---- LN(z) W_b = rstd * (z.W' - mu * c1) + c0 ; store to bias[h][query][key] (32 lanes = 128 contiguous bytes)
           const uint32_t brow = bias_buf + ((sub * kSubQ) * kTileK + prow) * 4;

@@ -41,7 +41,7 @@ constexpr uint16_t tClusterMask = (1u << tCluster) - 1;
 constexpr int tZBytes = tM * tCz * 2;          // 32 KB, two 64-channel halves of 16 KB
 constexpr int tW12Bytes = 2 * tCz * tNC * 2;   // 64 KB: per k-block of 64: [W1 n-half 0][W1 n-half 1][W2 n-half 0][W2 n-half 1]
 constexpr int tW3Bytes = tNC * tCz * 2;        // 32 KB: per k-block of 64: [n-half 0][n-half 1]
-constexpr int tKx = 16;                        // the K extension: channels 128 (-mu), 129 (1 / rstd), 130..143 (zero)
+constexpr int tKx = 16;                        // the K extension: channels 128..133 (-mu terms), 134..136 (1 / rstd terms), zeros
 constexpr int tZxBytes = tM * tKx * 2;         // 4 KB per z buffer, K-major, 32-byte swizzle
 constexpr int tW12xBytes = 4 * 64 * tKx * 2;   // 8 KB: rows k = 128..143 of [W1'c | W2'c], four 64-n blocks of 2 KB
 constexpr size_t tSmemZ = 0;
@@ -352,13 +352,21 @@ __global__ void __cluster_dims__(tCluster, 1, 1) __launch_bounds__(tThreads, 1) 
           const uint4 w = lds_u32x4(zrow + hf * (tZBytes / 2) + ((ch ^ sw) << 4));
           stats_bf16x2(sm, sq, w.x); stats_bf16x2(sm, sq, w.y); stats_bf16x2(sm, sq, w.z); stats_bf16x2(sm, sq, w.w);
         }
+      // var with ONE rounding: sum z^2 / c_z is exact (c_z is a power of two) and the FMA subtracts the unrounded mu^2
       const float mu = sm * (1.f / tCz);
-      const float vpe = fmaxf(fmaf(sq, 1.f / tCz, -mu * mu), 0.f) + eps;
+      const float vpe = fmaxf(fmaf(-mu, mu, sq * (1.f / tCz)), 0.f) + eps;
       if (half == 0) {
+        // -mu and 1 / rstd travel through the bf16 tensor pipe as sums of bf16 terms (hi + lo + lo2, hi + lo) against the
+        // weight rows [c1h, c1l, c1l2, c1h, c1l, c1h | c0h, c0l, c0h] (transition_fold_kernel): every product of the
+        // expansion down to 2^-16 of mu c1 is there, so z.W' - mu c1 cancels to fp32 accuracy however large |mu| / sigma is.
+        const float nm = -mu, sd = sqrtf(vpe);
+        const float mh = bf16_round(nm), ml = bf16_round(nm - mh), ml2 = bf16_round((nm - mh) - ml);
+        const float rh = bf16_round(sd), rl = bf16_round(sd - rh);
         const uint32_t xrow = s_zx + zb * tZxBytes + r * 32;
         const uint32_t c0 = ((uint32_t)(r >> 2) & 1u) << 4;
-        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %2, %2};" ::"r"(xrow + c0), "r"(pack_bf16(-mu, sqrtf(vpe))), "r"(0u) : "memory");
-        asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(xrow + (c0 ^ 16u)), "r"(0u) : "memory");
+        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(xrow + c0), "r"(pack_bf16(mh, mh)), "r"(pack_bf16(mh, ml)),
+                     "r"(pack_bf16(ml, ml2)), "r"(pack_bf16(rh, rh)) : "memory");
+        asm volatile("st.shared.v4.u32 [%0], {%1, %2, %2, %2};" ::"r"(xrow + (c0 ^ 16u)), "r"(pack_bf16(rl, 0.f)), "r"(0u) : "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
         if (lane == 0) mbar_arrive(b_xfull + 8 * zb);
@@ -421,8 +429,8 @@ __global__ void __cluster_dims__(tCluster, 1, 1) __launch_bounds__(tThreads, 1) 
   }
 }
 
-// Folded weights [c_z + 16][4 c_z] for W1 and W2: rows k < c_z: bf16(gamma_k W[k][j]); row c_z: c1[j] = sum_k of those
-// rounded values; row c_z + 1: c0[j] = sum_k beta_k W[k][j]; rows c_z + 2 ..: zero (the K extension of the first GEMM)
+// Folded weights [c_z + 16][4 c_z] for W1 and W2: rows k < c_z: bf16(gamma_k W[k][j]); rows c_z ..: the K extension of the
+// first GEMM -- c1[j] = sum_k of those rounded values and c0[j] = sum_k beta_k W[k][j], each split into bf16 terms
 __global__ void __launch_bounds__(32) transition_fold_kernel(const __nv_bfloat16* __restrict__ w1, const __nv_bfloat16* __restrict__ w2,
                                                              const __nv_bfloat16* __restrict__ gamma, const __nv_bfloat16* __restrict__ beta,
                                                              __nv_bfloat16* __restrict__ w1f, __nv_bfloat16* __restrict__ w2f) {
@@ -439,9 +447,16 @@ __global__ void __launch_bounds__(32) transition_fold_kernel(const __nv_bfloat16
     c11 += to_f32(af); c12 += to_f32(cf);
     c01 = fmaf(b, a, c01); c02 = fmaf(b, c, c02);
   }
-  w1f[tCz * tHid + j] = __float2bfloat16_rn(c11); w1f[(tCz + 1) * tHid + j] = __float2bfloat16_rn(c01);
-  w2f[tCz * tHid + j] = __float2bfloat16_rn(c12); w2f[(tCz + 1) * tHid + j] = __float2bfloat16_rn(c02);
-  for (int k = tCz + 2; k < tCz + tKx; ++k) { w1f[k * tHid + j] = __float2bfloat16_rn(0.f); w2f[k * tHid + j] = __float2bfloat16_rn(0.f); }
+  // K-extension rows, matching the columns [mh, mh, mh, ml, ml, ml2 | rh, rh, rl | 0 ...] the kernel writes per pair
+  auto ext = [&](__nv_bfloat16* wf, float c1, float c0) {
+    const __nv_bfloat16 c1h = __float2bfloat16_rn(c1), c1l = __float2bfloat16_rn(c1 - to_f32(c1h)),
+                        c1l2 = __float2bfloat16_rn((c1 - to_f32(c1h)) - to_f32(c1l));
+    const __nv_bfloat16 c0h = __float2bfloat16_rn(c0), c0l = __float2bfloat16_rn(c0 - to_f32(c0h));
+    const __nv_bfloat16 rows[tKx] = {c1h, c1l, c1l2, c1h, c1l, c1h, c0h, c0l, c0h};
+    for (int k = 0; k < tKx; ++k) wf[(tCz + k) * tHid + j] = k < 9 ? rows[k] : __float2bfloat16_rn(0.f);
+  };
+  ext(w1f, c11, c01);
+  ext(w2f, c12, c02);
 }
 
 CUresult encode2d(PFN_cuTensorMapEncodeTiled enc, CUtensorMap* m, const void* base, uint64_t d0, uint64_t d1, uint32_t b0,

@@ -116,9 +116,9 @@ __global__ void __launch_bounds__(128) sparse_atom_kernel(const SparseParams p) 
           dot_bf16x2(pw, pw_[i], wf_[i]);
         }
         const float mu = sm * (1.f / sCz);
-        const float var = fmaxf(fmaf(sq, 1.f / sCz, -mu * mu), 0.f);
-        const float rstd = rsqrtf(var + p.eps);
-        s[ps] = (d0 + d1) + fmaf(rstd, pw - mu * c1, c0);
+        const float var = fmaf(-mu, mu, sq * (1.f / sCz));      // one rounding (c_z is a power of two); 0 for a constant row
+        const float rstd = var > 0.f ? rsqrtf(var + p.eps) : 0.f;
+        s[ps] = (d0 + d1) + fmaf(rstd, fmaf(-mu, c1, pw), c0);
         mx = fmaxf(mx, s[ps]);
       }
     }
@@ -202,7 +202,8 @@ __global__ void __launch_bounds__(128) sparse_atom_rows_kernel(const SparseParam
 #pragma unroll
       for (int i = 0; i < 8; ++i) { dot_bf16x2(sm, pw_[i], ones); dot_bf16x2(sq, pw_[i], pw_[i]); }
       const float mu = sm * (1.f / sCz);
-      const float rstd = rsqrtf(fmaxf(fmaf(sq, 1.f / sCz, -mu * mu), 0.f) + p.eps);
+      const float var = fmaf(-mu, mu, sq * (1.f / sCz));        // one rounding (c_z is a power of two); 0 for a constant row
+      const float rstd = var > 0.f ? rsqrtf(var + p.eps) : 0.f;
 #pragma unroll
       for (int h = 0; h < H; ++h) {
         const uint4 w0 = __ldg(reinterpret_cast<const uint4*>(p.wfold + h * sCz));
@@ -211,7 +212,7 @@ __global__ void __launch_bounds__(128) sparse_atom_rows_kernel(const SparseParam
         float pw = 0.f;
 #pragma unroll
         for (int i = 0; i < 8; ++i) dot_bf16x2(pw, pw_[i], wf_[i]);
-        s_logit[j * H + h] = fmaf(rstd, pw - mu * __ldg(p.c1 + h), __ldg(p.c0 + h));
+        s_logit[j * H + h] = fmaf(rstd, fmaf(-mu, __ldg(p.c1 + h), pw), __ldg(p.c0 + h));
       }
     } else {
 #pragma unroll

@@ -106,32 +106,78 @@ def test_c1_bf16_full():
         assert torch.equal(again, mono)
 
 
-# ------------------------------------------------------------------ full-size configs on sampled rows
-@pytest.mark.parametrize("name,decomps", [
-    ("C2", [("monolithic", 1), ("row", 8), ("grid", 16)]),   # stripes of 375, 4x4 grid of 750^2 quadrants
-    ("C3", [("monolithic", 1), ("grid", 16)]),
-    ("C4", [("monolithic", 1), ("row", 16), ("grid", 16)]),
+# ------------------------------------------------------------------ full-size configs: SURVEY.md 8(c)'s acceptance protocol
+def protocol_rows(dcp, I, tile, shard_counts, count, seed):
+    """Query rows SURVEY.md 8(c) asks for at sizes the oracle cannot cover in full: the first and last row of the tensor,
+    both sides of every stripe / row-block boundary, and every query-tile class of every shard -- first and last row of
+    its first tile, of an interior tile and of its last (possibly ragged) tile -- topped up with seeded random rows."""
+    rows = set()
+    for parts in shard_counts:
+        for p in range(parts):
+            b, n = dcp.dcp_shard_range(I, parts, p)
+            last_tile = b + (n - 1) // tile * tile
+            mid_tile = b + (n // tile // 2) * tile
+            rows |= {b - 1, b, b + 1, b + tile - 1, b + tile, mid_tile, mid_tile + tile - 1, last_tile - 1, last_tile,
+                     b + n - 2, b + n - 1}
+    rows = {r for r in rows if 0 <= r < I}
+    extra = 0
+    while len(rows) < count:                       # seeded random rows until the protocol's count is reached
+        extra += count - len(rows)
+        rows |= set(syn.sample_rows(I, extra + 2, seed=seed))
+    return sorted(rows)
+
+
+def _oracle_rows_chunked(cfg, s, z, w, rows, chunk=256):
+    return np.concatenate([util.oracle_rows(cfg, s, z, w, rows[i:i + chunk]) for i in range(0, len(rows), chunk)], axis=0)
+
+
+def test_c2_bf16_full_output():
+    """C2 (the headline config, I = 3000) over the FULL output, all three decompositions ("C1, C2 over
+    the full output"): monolithic, 8 stripes of 375, 4 x 4 grid of 750^2 quadrants."""
+    dcp = _dcp()
+    cfg = syn.CONFIGS["C2"]
+    s, z, w = util.make_problem(cfg, DEV)
+    ref = _oracle_rows_chunked(cfg, s, z, w, list(range(cfg.I)))
+    mono = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c)
+    util.check_close(mono, ref, "bf16", "C2 monolithic (full output)")
+    row = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, decomp="row", parts=8)
+    assert torch.equal(row, mono), "row(8) != monolithic bitwise"
+    grid = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, decomp="grid", parts=16)
+    util.check_close(grid, ref, "bf16", "C2 grid(4x4) (full output)")
+    assert torch.equal(grid, dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, key_split=4))
+    del z
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("name,decomps,tile", [
+    ("C3", [("monolithic", 1), ("row", 16), ("grid", 16)], 32),
+    ("C4", [("monolithic", 1), ("row", 16), ("grid", 16)], 64),
 ])
-def test_full_size_sampled_rows(name, decomps):
+def test_full_size_sampled_rows(name, decomps, tile):
+    """C3 / C4 on >= 256 sampled query rows (a row's output needs only s and z[i, :, :], so a sampled row is exact)."""
     dcp = _dcp()
     cfg = syn.CONFIGS[name]
     free, _ = torch.cuda.mem_get_info()
     if cfg.z_bytes() * 1.15 > free:
         pytest.skip(f"{name}: z needs {cfg.z_bytes() / 1e9:.1f} GB")
     s, z, w = util.make_problem(cfg, DEV)
-    bounds = []
+    shard_counts = {1}
     for _, P in decomps:
-        G = int(round(P ** 0.5)) if P > 1 else 1
-        for parts in {P, G}:
-            bounds += [dcp.dcp_shard_range(cfg.I, parts, p)[0] for p in range(parts)]
-    rows = syn.sample_rows(cfg.I, 48 if name != "C2" else 96, boundaries=bounds + [128, 256], seed=cfg.seed)
-    ref = util.oracle_rows(cfg, s, z, w, rows)
+        shard_counts |= {P, int(round(P ** 0.5))}
+    rows = protocol_rows(dcp, cfg.I, tile, sorted(shard_counts), 256, cfg.seed)
+    assert len(rows) >= 256 and rows[0] == 0 and rows[-1] == cfg.I - 1
+    ref = _oracle_rows_chunked(cfg, s, z, w, rows)
     idx = torch.as_tensor(rows, device=DEV)
     atom = name == "C4"
+    mono = None
     for decomp, P in decomps:
         out = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, decomp=decomp, parts=P, atom=atom)
         util.check_close(out.index_select(0, idx), ref, "bf16", f"{name} {decomp}({P})")
         assert torch.isfinite(out.float()).all()
+        if decomp == "monolithic":
+            mono = out
+        elif decomp == "row":
+            assert torch.equal(out, mono), f"{name} row({P}) != monolithic bitwise"
     del z
     torch.cuda.empty_cache()
 
