@@ -913,27 +913,34 @@ def main():
     if rank == 0:
         sampler.start()
     evs = [(dcp.Event(), dcp.Event()) for _ in range(args.steps)]
-    t_begin, t_end = dcp.Event(), dcp.Event()
-    step_ms = []
-    torch.cuda.synchronize()
-    if flush is None:
-        t_begin.record()
-        for k in range(args.steps):
-            step(evs[k])
-        t_end.record()
+
+    def timed(with_kernel_events):
         torch.cuda.synchronize()
-        total_ms = t_begin.elapsed_ms(t_end)
-    else:
+        if flush is None:
+            t_begin, t_end = dcp.Event(), dcp.Event()
+            t_begin.record()
+            for k in range(args.steps):
+                step(evs[k] if with_kernel_events else None)
+            t_end.record()
+            torch.cuda.synchronize()
+            return t_begin.elapsed_ms(t_end)
         # small workload: flush L2 between steps, time each step with its own event pair
-        total_ms = 0.0
+        ms = 0.0
         for k in range(args.steps):
             flush.zero_()
             a, b = dcp.Event(), dcp.Event()
             a.record()
-            step(evs[k])
+            step(evs[k] if with_kernel_events else None)
             b.record()
             torch.cuda.synchronize()
-            total_ms += a.elapsed_ms(b)
+            ms += a.elapsed_ms(b)
+        return ms
+
+    # Pass 1 (the reported value): exactly K steps, the call as a user makes it -- its four launches are chained by
+    # programmatic dependent launch.  Pass 2, the same K steps again: an event pair brackets the dominant kernel; the
+    # event records serialise the launches around that kernel, so this pass is a little slower and only times the kernel.
+    total_ms = timed(False)
+    total_ms_with_events = timed(True)
     clocks = sampler.stop() if rank == 0 else None
     fused_ms = [a.elapsed_ms(b) for a, b in evs]
     total_ms = max_over_ranks_ms(total_ms, world, dev)
@@ -952,7 +959,8 @@ def main():
             kname = "fused_mma_kernel" if cfg.H == 16 else "fused_atom_kernel"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES.get((kname, cfg.name)), "kernel": kname, "peak_source": peak_how,
-                "kernel_ms": fused_avg_ms, "kernel_share_of_step": fused_avg_ms * args.steps / total_ms,
+                "kernel_ms": fused_avg_ms, "kernel_share_of_step": fused_avg_ms * args.steps / total_ms_with_events,
+                "ms_per_step_with_kernel_events": total_ms_with_events / args.steps,
                 "algorithmic_bytes_per_launch": alg_bytes,
                 "fused_launches_per_step": 1 if args.decomp == "monolithic" else None}
 

@@ -4,6 +4,7 @@
 // strided view of z (a base-pointer offset, no copy), partial states merged left to right by one kernel.
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "kernels.h"
@@ -14,6 +15,13 @@ namespace {
 thread_local int g_launches = 0;
 
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// Programmatic dependent launch between the kernels of a call (common.cuh) is on unless DCP_PDL=0 is set in the
+// environment (a debugging / A-B timing switch, read once).
+bool pdl_enabled() {
+  static const bool on = [] { const char* e = getenv("DCP_PDL"); return !(e && e[0] == '0'); }();
+  return on;
+}
 inline int elt_size(dcp_dtype dt) { return dt == DCP_F32 ? 4 : 2; }
 
 struct Carve {
@@ -194,6 +202,7 @@ dcp_status run_prologue_mma(const Ctx& x, const void* s) {
   gp.fold_w_b = x.w->w_b; gp.fold_gamma = x.w->ln_z_gamma; gp.fold_beta = x.w->ln_z_beta;
   gp.fold_wfold = x.ws + x.cv.wfold; gp.fold_c1 = (float*)(x.ws + x.cv.c1); gp.fold_c0 = (float*)(x.ws + x.cv.c0);
   gp.fold_c_z = x.c_z; gp.fold_H = x.H; gp.fold_H_pad = 16;
+  gp.pdl = pdl_enabled();   // programmatic dependent of whatever kernel precedes the call in the stream (common.cuh)
   bool folded = false;
   DCP_CUDA(launch_gemm_mma(gp, x.st, &folded));
   if (!folded)
@@ -270,6 +279,7 @@ dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w
     mp.q_begin = 0; mp.q_end = (int)I; mp.n_qparts = plan.decomp == DCP_GRID ? plan.G : plan.parts;
     mp.k_begin = 0; mp.k_end = (int)I; mp.n_kparts = plan.key_split;
     mp.nseg = plan.nseg; mp.slot0 = 0;
+    mp.pdl = pdl_enabled() && plan.ev_begin == nullptr;   // an event record between two launches would serialise them anyway
     if (plan.ev_begin && cudaEventRecord(plan.ev_begin, x.st) != cudaSuccess) return DCP_ERR_CUDA;
     DCP_CUDA(launch_fused_mma(mp, z, ldz, x.st));
   } else {
@@ -324,11 +334,13 @@ dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w
   mp.g = x.ws + x.cv.g;
   mp.gated = x.ws + x.cv.gated;
   mp.rows = I; mp.n_slots = plan.slots; mp.H = H; mp.c = c; mp.D = x.D;
+  mp.pdl = pdl_enabled() && plan.use_mma && plan.ev_end == nullptr;
   DCP_CUDA(launch_merge(dt, mp, x.st));
   if (plan.use_mma) {
     GemmMmaParams gp{};
     gp.A = x.ws + x.cv.gated; gp.lda = x.D; gp.M = I; gp.N = c_s; gp.K = x.D; gp.nseg = 1;
     gp.W[0] = w->w_o; gp.C[0] = out; gp.mode[0] = GEMM_OUT_PLAIN; gp.ldc[0] = c_s;
+    gp.pdl = pdl_enabled();
     DCP_CUDA(launch_gemm_mma(gp, x.st));
   } else {
     DCP_CUDA(launch_gemm(dt, false, x.ws + x.cv.gated, x.D, w->w_o, nullptr, out, c_s, I, c_s, x.D, EPI_NONE, x.st));

@@ -19,6 +19,31 @@ __host__ __device__ inline void shard_range(int64_t n, int parts, int p, int64_t
   *start = (int64_t)p * base + (p < rem ? p : rem);
 }
 
+// ---- programmatic dependent launch (sm_90+): a kernel launched with launch_kernel(..., pdl = true) may start while the
+// previous kernel in the stream is still draining; everything before pdl_wait() (barrier init, tensor-memory allocation,
+// descriptor prefetch) overlaps the predecessor's tail, everything after it sees the predecessor's writes.  Every kernel
+// of the chain executes pdl_wait() in every thread before it touches global memory, so completion is transitive: when a
+// kernel's pdl_wait() returns, all earlier kernels of the stream have finished.  Both calls are no-ops in a kernel that was
+// launched without the attribute.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_kernel(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
+                                 Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 __device__ __forceinline__ float to_f32(float x) { return x; }
 __device__ __forceinline__ float to_f32(__nv_bfloat16 x) { return __bfloat162float(x); }
 template <typename T> __device__ __forceinline__ T from_f32(float x);
@@ -67,6 +92,7 @@ struct MergeParams {
   float *m_out, *l_out, *acc_out;  // merged state out (when g == nullptr)
   int64_t rows;
   int n_slots, H, c, D;
+  bool pdl;             // host only: launch as a programmatic dependent of the previous kernel in the stream
 };
 
 }  // namespace dcp

@@ -75,6 +75,7 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
 
+  pdl_trigger();
   if (threadIdx.x == 0) {
     // zempty: the tcgen05.commit of the stage's MMAs + the four epilogue warps that read the rows with LDS
     for (int s = 0; s < aNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + aNumProjWarps); }
@@ -84,6 +85,8 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), aTmemCols);
+  pdl_wait();          // the prologue's q / k / v / folded weights are final (and so is everything before it in the stream)
   // W'' = B operand of the projection MMA: 16 rows (n) x 16 channels, K-major, 32-byte swizzle by hand (16-byte chunk
   // index ^ bit 2 of the row): row n < 4 = head n of (gamma (.) W_b log2 e)^T, row 4 = ones, rows 5..15 = 0.
   if (threadIdx.x < aProjN * 2) {
@@ -94,7 +97,6 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
     *reinterpret_cast<uint4*>(smem + aSmemWt + n * 32 + ((ch ^ ((n >> 2) & 1)) << 4)) = v;
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to tcgen05
-  if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), aTmemCols);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -457,8 +459,7 @@ cudaError_t launch_fused_atom(const MmaParams& p, const void* z, int64_t ldz, cu
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (sms <= 0) sms = 148;
   const unsigned grid = (unsigned)(units < sms ? units : sms);
-  fused_atom_kernel<<<grid, aThreads, aSmemAlloc, st>>>(tm, p);
-  return cudaGetLastError();
+  return launch_kernel(fused_atom_kernel, dim3(grid), dim3(aThreads), aSmemAlloc, st, p.pdl, tm, p);
 }
 
 }  // namespace dcp

@@ -71,6 +71,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
 
+  pdl_trigger();
   if (threadIdx.x == 0) {
     // zempty / tfull are arrived on by tcgen05.commit (the MMAs that read the stage / wrote the accumulators are done)
     for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + kNumProjWarps); }
@@ -78,6 +79,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     for (int b = 0; b < kNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, kNumProjWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), kTmemCols);
+  pdl_wait();          // the prologue's q / k / v / folded weights are final (and so is everything before it in the stream)
   // W'' = B operand of the projection MMA, K-major, 128-byte swizzled by hand: row n < 16 = head n of
   // (gamma (.) W_b log2 e)^T, row 16 = ones (its accumulator column is sum_k z), rows 17..31 = 0.
   for (int e = threadIdx.x; e < kProjN * (kCz / 8); e += kThreads) {
@@ -89,7 +92,6 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     *reinterpret_cast<uint4*>(smem + kSmemWt + half * kWtHalfBytes + n * 128 + ((c ^ (n & 7)) << 4)) = v;
   }
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to TMA / tcgen05
-  if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), kTmemCols);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -424,8 +426,7 @@ cudaError_t launch_c(const CUtensorMap& tm, const MmaParams& p, int64_t units, c
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (sms <= 0) sms = 148;
   const unsigned grid = (unsigned)(units < sms ? units : sms);
-  fused_mma_kernel<C, CP><<<grid, kThreads, smem_alloc(CP), st>>>(tm, p);
-  return cudaGetLastError();
+  return launch_kernel(fused_mma_kernel<C, CP>, dim3(grid), dim3(kThreads), smem_alloc(CP), st, p.pdl, tm, p);
 }
 
 }  // namespace

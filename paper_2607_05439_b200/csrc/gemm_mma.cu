@@ -43,6 +43,8 @@ __device__ __forceinline__ void mma16816(float (&d)[4], const uint32_t (&a)[4], 
 
 template <int MI>
 __global__ void __launch_bounds__(256) gemm_mma_kernel(const GemmMmaParams p) {
+  pdl_trigger();
+  pdl_wait();
   constexpr int BM = 32 * MI;
   // pipeline buffers; after the main loop the same memory stages the C tile of the fragment-order outputs
   constexpr int kAElems = 2 * BM * LDA_S, kBElems = 2 * BK * LDB_S, kCElems = BM * LDB_S;
@@ -242,12 +244,11 @@ cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st, bool* fold_
   const int64_t nb = (int64_t)p.nseg * ((p.N + BN - 1) / BN);
   if (nb * ((p.M + 127) / 128) >= 2 * 148) {   // enough 128-row tiles for two CTAs per SM
     dim3 grid((unsigned)nb, (unsigned)((p.M + 127) / 128));
-    gemm_mma_kernel<4><<<grid, 256, 0, st>>>(p);
+    return launch_kernel(gemm_mma_kernel<4>, grid, dim3(256), 0, st, p.pdl, p);
   } else {
     dim3 grid((unsigned)nb, (unsigned)((p.M + 63) / 64));
-    gemm_mma_kernel<2><<<grid, 256, 0, st>>>(p);
+    return launch_kernel(gemm_mma_kernel<2>, grid, dim3(256), 0, st, p.pdl, p);
   }
-  return cudaGetLastError();
 }
 
 cudaError_t launch_layernorm_rows_bf16(const void* x, const void* gamma, const void* beta, void* y, int64_t rows,

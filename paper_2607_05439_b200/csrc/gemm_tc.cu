@@ -75,8 +75,10 @@ __global__ void __launch_bounds__(kTcThreads, 2) gemm_tc_kernel(const __grid_con
   const uint32_t bar_full = s_bar, bar_empty = s_bar + 8 * TST, bar_acc = s_bar + 16 * TST;
   volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + kTcSmemBar + (2 * TST + 2) * 8);
 
+  pdl_trigger();
   if (blockIdx.y == gridDim.y - 1 && p.fold_w_b != nullptr) {
     // the extra CTA row of the launch: CTA 0 folds LayerNorm(z) into the bias projection weights, the others leave
+    pdl_wait();
     if (blockIdx.x == 0 && threadIdx.x < 256)
       fold_ln_z_mma_device(p.fold_w_b, p.fold_gamma, p.fold_beta, p.fold_wfold, p.fold_c1, p.fold_c0, p.fold_c_z, p.fold_H,
                            p.fold_H_pad, threadIdx.x, 256);
@@ -99,6 +101,7 @@ __global__ void __launch_bounds__(kTcThreads, 2) gemm_tc_kernel(const __grid_con
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *s_tmem;
+  pdl_wait();                                                // the previous kernel's writes (A, the C buffers) are final
 
   if (warp == 0) {
     if (lane == 0) {
@@ -267,12 +270,11 @@ cudaError_t launch_gemm_tc(const GemmMmaParams& p, cudaStream_t st) {
   // 128-wide tiles when they give every SM two CTAs (or N does not split into 64s evenly enough to matter)
   if (p.N % 128 == 0 && (int64_t)p.nseg * (p.N / 128) * mt_tiles >= 2 * 148) {
     dim3 grid((unsigned)(p.nseg * (p.N / 128)), mt);
-    gemm_tc_kernel<128><<<grid, kTcThreads, TcCfg<128>::kSmemAlloc, st>>>(maps, p);
+    return launch_kernel(gemm_tc_kernel<128>, grid, dim3(kTcThreads), TcCfg<128>::kSmemAlloc, st, p.pdl, maps, p);
   } else {
     dim3 grid((unsigned)(p.nseg * (p.N / 64)), mt);
-    gemm_tc_kernel<64><<<grid, kTcThreads, TcCfg<64>::kSmemAlloc, st>>>(maps, p);
+    return launch_kernel(gemm_tc_kernel<64>, grid, dim3(kTcThreads), TcCfg<64>::kSmemAlloc, st, p.pdl, maps, p);
   }
-  return cudaGetLastError();
 }
 
 }  // namespace dcp

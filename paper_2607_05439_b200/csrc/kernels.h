@@ -45,6 +45,7 @@ struct GemmMmaParams {
   void* fold_wfold;
   float *fold_c1, *fold_c0;
   int fold_c_z, fold_H, fold_H_pad;
+  bool pdl;             // host only: launch as a programmatic dependent of the previous kernel in the stream (common.cuh)
 };
 cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st, bool* fold_done = nullptr);   // dispatches to launch_gemm_tc when it applies
 // tcgen05 / TMA GEMM (gemm_tc.cu): N % 128 == 0, K % 64 == 0, 16-byte aligned operands
@@ -77,6 +78,7 @@ struct MmaParams {
   int nseg, slot0;
   int H, c, c_z;
   float eps;
+  bool pdl;             // host only: launch as a programmatic dependent of the previous kernel in the stream
 };
 cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st);
 bool fused_mma_supports(dcp_dtype dt, int H, int c, int c_z);

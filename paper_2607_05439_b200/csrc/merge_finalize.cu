@@ -13,6 +13,8 @@ namespace {
 
 template <typename T>
 __global__ void __launch_bounds__(256) merge_kernel(const MergeParams p) {
+  pdl_trigger();
+  pdl_wait();
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t total = p.rows * p.D;
   if (idx >= total) return;
@@ -50,6 +52,8 @@ __global__ void __launch_bounds__(256) merge_kernel(const MergeParams p) {
 // its order and every operation are the same as in the runtime-count version: same bits).
 template <typename T, int NS>
 __global__ void __launch_bounds__(256) merge_vec4_kernel(const MergeParams p) {
+  pdl_trigger();
+  pdl_wait();
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int dq = p.D >> 2;
   if (idx >= p.rows * dq) return;
@@ -108,14 +112,22 @@ __global__ void __launch_bounds__(256) merge_vec4_kernel(const MergeParams p) {
   }
 }
 
+template <typename T, int NS>
+cudaError_t launch_vec4_n(const MergeParams& p, unsigned blocks, cudaStream_t st) {
+  return launch_kernel(merge_vec4_kernel<T, NS>, dim3(blocks), dim3(256), 0, st, p.pdl, p);
+}
 template <typename T>
-void launch_vec4(const MergeParams& p, unsigned blocks, cudaStream_t st) {
+cudaError_t launch_vec4(const MergeParams& p, unsigned blocks, cudaStream_t st) {
   switch (p.n_slots) {
-    case 1: merge_vec4_kernel<T, 1><<<blocks, 256, 0, st>>>(p); break;
-    case 2: merge_vec4_kernel<T, 2><<<blocks, 256, 0, st>>>(p); break;
-    case 3: merge_vec4_kernel<T, 3><<<blocks, 256, 0, st>>>(p); break;
-    case 4: merge_vec4_kernel<T, 4><<<blocks, 256, 0, st>>>(p); break;
-    default: merge_vec4_kernel<T, 0><<<blocks, 256, 0, st>>>(p); break;
+    case 1: return launch_vec4_n<T, 1>(p, blocks, st);
+    case 2: return launch_vec4_n<T, 2>(p, blocks, st);
+    case 3: return launch_vec4_n<T, 3>(p, blocks, st);
+    case 4: return launch_vec4_n<T, 4>(p, blocks, st);
+    case 6: return launch_vec4_n<T, 6>(p, blocks, st);
+    case 8: return launch_vec4_n<T, 8>(p, blocks, st);
+    case 12: return launch_vec4_n<T, 12>(p, blocks, st);
+    case 16: return launch_vec4_n<T, 16>(p, blocks, st);
+    default: return launch_vec4_n<T, 0>(p, blocks, st);
   }
 }
 
@@ -126,14 +138,11 @@ cudaError_t launch_merge(dcp_dtype dt, const MergeParams& p, cudaStream_t st) {
   if (total <= 0) return cudaSuccess;
   if (p.c % 4 == 0 && ((uintptr_t)p.st_acc & 15) == 0 && (p.g != nullptr || ((uintptr_t)p.acc_out & 15) == 0)) {
     const unsigned vblocks = (unsigned)((total / 4 + 255) / 256);
-    if (dt == DCP_F32) launch_vec4<float>(p, vblocks, st);
-    else launch_vec4<__nv_bfloat16>(p, vblocks, st);
-    return cudaGetLastError();
+    return dt == DCP_F32 ? launch_vec4<float>(p, vblocks, st) : launch_vec4<__nv_bfloat16>(p, vblocks, st);
   }
   unsigned blocks = (unsigned)((total + 255) / 256);
-  if (dt == DCP_F32) merge_kernel<float><<<blocks, 256, 0, st>>>(p);
-  else merge_kernel<__nv_bfloat16><<<blocks, 256, 0, st>>>(p);
-  return cudaGetLastError();
+  return dt == DCP_F32 ? launch_kernel(merge_kernel<float>, dim3(blocks), dim3(256), 0, st, p.pdl, p)
+                       : launch_kernel(merge_kernel<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, p.pdl, p);
 }
 
 }  // namespace dcp
