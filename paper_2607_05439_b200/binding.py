@@ -13,7 +13,8 @@ from typing import Dict, Optional
 import torch
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_PKG, "libdesigncp.so")
+# DCP_LIB names another build of the same library (A/B timing of two builds in one process each); default: in-tree
+LIB_PATH = os.environ.get("DCP_LIB") or os.path.join(_PKG, "libdesigncp.so")
 
 DCP_OK = 0
 DCP_ERR_INVALID_ARG, DCP_ERR_UNSUPPORTED, DCP_ERR_WORKSPACE, DCP_ERR_CUDA = 1, 2, 3, 4
@@ -54,6 +55,7 @@ class dcp_block_weights(C.Structure):
 
 class dcp_plan(C.Structure):
     _fields_ = [("parts", C.c_int), ("key_split", C.c_int), ("kernel", C.c_int),
+                ("tile_q", C.c_int), ("tile_k", C.c_int), ("key_segments", C.c_int),
                 ("ev_fused_begin", C.c_void_p), ("ev_fused_end", C.c_void_p)]
 
 
@@ -147,10 +149,10 @@ def _weights_struct(w: Dict[str, torch.Tensor], eps: float) -> dcp_weights:
     return ws
 
 
-def _plan(parts: int, key_split: int, kernel, events=None) -> dcp_plan:
+def _plan(parts: int, key_split: int, kernel, events=None, tile=(0, 0), key_segments: int = 0) -> dcp_plan:
     k = KERNEL[kernel] if isinstance(kernel, str) else int(kernel)
     e0, e1 = (events if events is not None else (None, None))
-    return dcp_plan(int(parts), int(key_split), k, e0, e1)
+    return dcp_plan(int(parts), int(key_split), k, int(tile[0]), int(tile[1]), int(key_segments), e0, e1)
 
 
 class Event:
@@ -184,9 +186,9 @@ def dcp_shard_range(n: int, parts: int, p: int):
 
 
 def dcp_workspace_bytes(I, c_s, H, c, c_z, dtype: torch.dtype, decomp="monolithic", parts=1, key_split=1,
-                        kernel="auto") -> int:
+                        kernel="auto", tile=(0, 0), key_segments=0) -> int:
     out = C.c_size_t()
-    pl = _plan(parts, key_split, kernel)
+    pl = _plan(parts, key_split, kernel, None, tile, key_segments)
     _check(_lib.dcp_workspace_bytes(I, c_s, H, c, c_z, _dtype_code(dtype), DECOMP[decomp], C.byref(pl),
                                     C.byref(out)), "dcp_workspace_bytes")
     return int(out.value)
@@ -206,7 +208,8 @@ def _alloc_ws(nbytes: int, device) -> torch.Tensor:
 
 
 def dcp_pair_bias_attention(s, z, w, H, c, decomp="monolithic", parts=1, key_split=1, kernel="auto", eps=1e-5,
-                            out=None, workspace=None, stream=None, atom=False, ldz=0, fused_events=None):
+                            out=None, workspace=None, stream=None, atom=False, ldz=0, fused_events=None, tile=(0, 0),
+                            key_segments=0):
     """out[I, c_s] = W_o (sigmoid(s W_g) (.) softmax(Q K^T/sqrt(c) + LN(z) W_b) V)  on the current CUDA device."""
     assert s.is_cuda and z.is_cuda and s.is_contiguous()
     I, c_s = s.shape
@@ -216,9 +219,10 @@ def dcp_pair_bias_attention(s, z, w, H, c, decomp="monolithic", parts=1, key_spl
     if out is None:
         out = torch.empty(I, c_s, dtype=s.dtype, device=s.device)
     pl = _plan(parts, key_split, kernel,
-               None if fused_events is None else (fused_events[0].handle, fused_events[1].handle))
+               None if fused_events is None else (fused_events[0].handle, fused_events[1].handle), tile, key_segments)
     if workspace is None:
-        workspace = _alloc_ws(dcp_workspace_bytes(I, c_s, H, c, c_z, s.dtype, decomp, parts, key_split, kernel), s.device)
+        workspace = _alloc_ws(dcp_workspace_bytes(I, c_s, H, c, c_z, s.dtype, decomp, parts, key_split, kernel, tile,
+                                                  key_segments), s.device)
     ws = _weights_struct(w, eps)
     fn = _lib.dcp_atom_pair_bias_attention if atom else _lib.dcp_pair_bias_attention
     st = fn(_ptr(s), _ptr(z), int(ldz), C.byref(ws), _ptr(out), I, c_s, H, c, c_z, dt, DECOMP[decomp], C.byref(pl),

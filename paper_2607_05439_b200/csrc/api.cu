@@ -98,7 +98,16 @@ dcp_status make_plan(int64_t I, int H, int c, int c_z, dcp_dtype dt, dcp_decomp 
   if (p.kernel == DCP_KERNEL_MMA && !mma_ok) return DCP_ERR_UNSUPPORTED;
   if (p.kernel == DCP_KERNEL_GENERIC && !fused_generic_supports(dt, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
   p.use_mma = mma_ok && p.kernel != DCP_KERNEL_GENERIC;
+  if (in && (in->tile_q < 0 || in->tile_k < 0 || in->key_segments < 0 || in->key_segments > 64)) return DCP_ERR_INVALID_ARG;
+  if (in && (in->tile_q || in->tile_k)) {
+    // one tiling per kernel: a non-zero request must name it (include/designcp.h)
+    int tq, tk;
+    if (p.use_mma) { tq = H == 16 ? 32 : fused_atom_tile_q(); tk = H == 16 ? 16 : 32; }
+    else { tq = 8; tk = 32; }
+    if ((in->tile_q && in->tile_q != tq) || (in->tile_k && in->tile_k != tk)) return DCP_ERR_UNSUPPORTED;
+  }
   p.nseg = p.use_mma ? mma_num_segments(I, H, p.key_split) : 1;
+  if (p.use_mma && in && in->key_segments > 0) p.nseg = std::min<int64_t>(in->key_segments, std::max<int64_t>(1, I / p.key_split));
   p.slots = p.key_split * p.nseg;
   *out = p;
   return DCP_OK;
@@ -686,6 +695,6 @@ const char* dcp_status_string(dcp_status st) {
   }
 }
 
-int dcp_version(void) { return 100; }
+int dcp_version(void) { return 200; }
 
 }  // extern "C"

@@ -38,6 +38,7 @@ constexpr int kBiasHeadPitch = kTileQ * kTileK + 4;     // floats; +4: conflict-
 constexpr int kBiasBufFloats = kH * kBiasHeadPitch;
 constexpr int kThreads = 512;
 constexpr int kProjWarp0 = 4, kNumProjWarps = 4, kAttnWarp0 = 8, kNumAttnWarps = 8;
+constexpr int kNumIssuers = 3;      // tcgen05 issuing threads (lane 0 of warps 1..3)
 
 constexpr size_t kSmemZ = 0;
 constexpr size_t kSmemBias = kSmemZ + (size_t)kNZ * kStageBytes;
@@ -123,14 +124,19 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           }
         }
       }
-    } else if (warp == 1 && lane == 0) {
-      // ============================================================= tcgen05 issuer (one thread)
+    } else if (warp >= 1 && warp <= kNumIssuers && lane == 0) {
+      // ============================================================= tcgen05 issuers (one thread each, warps 1..3)
+      // A K = 16 projection MMA costs its issuing thread ~130 cycles whatever N is (the 4 KB A-operand fetch), eight of
+      // them per 32 KB stage: one thread alone needs ~1050 of the ~1450 cycles a stage may take at the HBM bound, and
+      // with the attention warps competing for issue slots it became the kernel's pacemaker (what-if: half the MMAs
+      // -> -9.5 % kernel time).  Several threads' MMAs overlap in the tensor pipe, so stage n goes to issuer n % 3.
       // Per z stage (128 pair rows = 8 queries x 16 keys, K-major, exactly as TMA wrote it) two accumulator chains
       // over the 8 K = 16 steps:   P[128 x 32]  = z . W''^T   (a3: 16 heads; column 16 = sum_k z)
       //                            G[128 x 128] = z . z^T     (a2: its diagonal is sum_k z^2)
       // into TMEM buffer tb; tcgen05.commit then releases the smem stage and publishes the accumulators.
       constexpr uint32_t idesc_p = umma_idesc_bf16(128, kProjN);
-      int stage = 0, tb = 0;
+      const int me = warp - 1;
+      int stage = 0, tb = 0, turn = 0;
       uint32_t phase = 0, tphase = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
         const Unit un = decode_unit<kTileQ>(p, u);
@@ -138,6 +144,13 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
         const int nsub = (rows + kSubQ - 1) / kSubQ;
         for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
           for (int sub = 0; sub < nsub; ++sub) {
+            const bool mine = turn == me;
+            if (++turn == kNumIssuers) turn = 0;
+            if (!mine) {
+              if (++stage == kNZ) { stage = 0; phase ^= 1; }
+              if (++tb == kNT) { tb = 0; tphase ^= 1; }
+              continue;
+            }
             mbar_wait(bar_tempty + 8 * tb, tphase ^ 1);
             mbar_wait(bar_zfull + 8 * stage, phase);
             tc_fence_after();
