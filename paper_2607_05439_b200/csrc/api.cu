@@ -107,7 +107,11 @@ dcp_status make_plan(int64_t I, int H, int c, int c_z, dcp_dtype dt, dcp_decomp 
     if ((in->tile_q && in->tile_q != tq) || (in->tile_k && in->tile_k != tk)) return DCP_ERR_UNSUPPORTED;
   }
   p.nseg = p.use_mma ? mma_num_segments(I, H, p.key_split) : 1;
-  if (p.use_mma && in && in->key_segments > 0) p.nseg = std::min<int64_t>(in->key_segments, std::max<int64_t>(1, I / p.key_split));
+  if (p.use_mma && in && in->key_segments > 0) {
+    // never more segments than whole key tiles in the smallest chunk: every segment keeps at least one key
+    const int64_t tile_k = H == 16 ? 16 : 32;
+    p.nseg = (int)std::min<int64_t>(in->key_segments, std::max<int64_t>(1, (I / p.key_split) / tile_k));
+  }
   p.slots = p.key_split * p.nseg;
   *out = p;
   return DCP_OK;

@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
       int stage = 0;
       uint32_t phase = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const Unit un = decode_unit<aTileQ>(p, u);
+        const Unit un = decode_unit<aTileQ, aTileK>(p, u);
         const int rows = (un.q_end - un.q0) < aTileQ ? (un.q_end - un.q0) : aTileQ;
         const int nsub = (rows + aSubQ - 1) / aSubQ;
         for (int j0 = un.ks & ~(aTileK - 1); j0 < un.ke; j0 += aTileK) {
@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
       int stage = 0, tb = 0;
       uint32_t phase = 0, tphase = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const Unit un = decode_unit<aTileQ>(p, u);
+        const Unit un = decode_unit<aTileQ, aTileK>(p, u);
         const int rows = (un.q_end - un.q0) < aTileQ ? (un.q_end - un.q0) : aTileQ;
         const int nsub = (rows + aSubQ - 1) / aSubQ;
         for (int j0 = un.ks & ~(aTileK - 1); j0 < un.ke; j0 += aTileK) {
@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
     int tb = 0, bbuf = 0, stage = 0;
     uint32_t tphase = 0, bphase = 0, zphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const Unit un = decode_unit<aTileQ>(p, u);
+      const Unit un = decode_unit<aTileQ, aTileK>(p, u);
       const int rows = (un.q_end - un.q0) < aTileQ ? (un.q_end - un.q0) : aTileQ;
       const int nsub = (rows + aSubQ - 1) / aSubQ;
       for (int j0 = un.ks & ~(aTileK - 1); j0 < un.ke; j0 += aTileK) {
@@ -249,7 +249,7 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
     int bbuf = 0;
     uint32_t bphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const Unit un = decode_unit<aTileQ>(p, u);
+      const Unit un = decode_unit<aTileQ, aTileK>(p, u);
       // Q fragments (registers): [m-block][k-step] -> (a0, a2) of row g and (a1, a3) of row g + 8
       uint2 qa[2][KK], qb[2][KK];
 #pragma unroll

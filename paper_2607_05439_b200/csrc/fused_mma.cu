@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
       int stage = 0;
       uint32_t phase = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const Unit un = decode_unit<kTileQ>(p, u);
+        const Unit un = decode_unit<kTileQ, kTileK>(p, u);
         const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
         const int nsub = (rows + kSubQ - 1) / kSubQ;
         for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
       int stage = 0, tb = 0, turn = 0;
       uint32_t phase = 0, tphase = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const Unit un = decode_unit<kTileQ>(p, u);
+        const Unit un = decode_unit<kTileQ, kTileK>(p, u);
         const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
         const int nsub = (rows + kSubQ - 1) / kSubQ;
         for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
@@ -187,7 +187,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     int tb = 0, bbuf = 0, stage = 0;
     uint32_t tphase = 0, bphase = 0, zphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const Unit un = decode_unit<kTileQ>(p, u);
+      const Unit un = decode_unit<kTileQ, kTileK>(p, u);
       const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
       const int nsub = (rows + kSubQ - 1) / kSubQ;
       for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
@@ -259,17 +259,31 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     int bbuf = 0;
     uint32_t bphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const Unit un = decode_unit<kTileQ>(p, u);
+      const Unit un = decode_unit<kTileQ, kTileK>(p, u);
       // Q tile -> shared memory (rows of the tile, all heads), shared by the 8 attention warps; row pitch padded so the
       // per-thread 64-bit fragment loads are conflict-free.  Named barrier 1 = the 256 attention threads.
       constexpr int kQP = q_pitch(CP);
       constexpr int kQRowChunks = kH * CP * 2 / 16;
-      asm volatile("bar.sync 1, 256;" ::: "memory");          // every warp is done with the previous unit's Q
-      for (int e = threadIdx.x - kAttnWarp0 * 32; e < kTileQ * kQRowChunks; e += kNumAttnWarps * 32) {
-        const int r = e / kQRowChunks, ch = e - r * kQRowChunks;
-        const int64_t row = (un.q0 + r) < p.I ? (un.q0 + r) : p.I - 1;
-        const uint4 v = __ldg(reinterpret_cast<const uint4*>(qp + row * (kH * CP)) + ch);
-        *reinterpret_cast<uint4*>(smem + kSmemQ + r * kQP + ch * 16) = v;
+      // All of a thread's chunks are requested before the barrier and stored after it: the unit change costs one L2 round
+      // trip, not one per chunk (kTileQ * kQRowChunks is a multiple of the 256 attention threads for every CP).
+      {
+        constexpr int kQIter = kTileQ * kQRowChunks / (kNumAttnWarps * 32);
+        static_assert(kQIter * kNumAttnWarps * 32 == kTileQ * kQRowChunks, "Q tile chunks per thread");
+        uint4 qv[kQIter];
+#pragma unroll
+        for (int i = 0; i < kQIter; ++i) {
+          const int e = threadIdx.x - kAttnWarp0 * 32 + i * (kNumAttnWarps * 32);
+          const int r = e / kQRowChunks, ch = e - r * kQRowChunks;
+          const int64_t row = (un.q0 + r) < p.I ? (un.q0 + r) : p.I - 1;
+          qv[i] = __ldg(reinterpret_cast<const uint4*>(qp + row * (kH * CP)) + ch);
+        }
+        asm volatile("bar.sync 1, 256;" ::: "memory");        // every warp is done with the previous unit's Q
+#pragma unroll
+        for (int i = 0; i < kQIter; ++i) {
+          const int e = threadIdx.x - kAttnWarp0 * 32 + i * (kNumAttnWarps * 32);
+          const int r = e / kQRowChunks, ch = e - r * kQRowChunks;
+          *reinterpret_cast<uint4*>(smem + kSmemQ + r * kQP + ch * 16) = qv[i];
+        }
       }
       asm volatile("bar.sync 1, 256;" ::: "memory");
       // fragment address of (row g, head 2aw, k-step 0): + mb*16*kQP (+8 rows: +8*kQP), + hh*CP*2, + kk*32

@@ -183,7 +183,10 @@ __host__ __device__ inline int64_t mma_num_units(int n, int n_qparts, int n_kpar
   return ((int64_t)rem * t_big + (int64_t)(n_qparts - rem) * t_small) * n_kparts * nseg;
 }
 
-template <int kTileQ>
+// Key chunk cb (Eq. 5 over the keys: the decomposition contract's chunks) is cut into nseg segments along the kTileK-key
+// tiles that overlap it (Eq. 5 over those tiles), so that only chunk boundaries -- never segment boundaries -- fall
+// inside a tile: a boundary tile would be streamed and projected twice.  A pure function of (I, chunks, segments).
+template <int kTileQ, int kTileK>
 __device__ __forceinline__ Unit decode_unit(const MmaParams& p, int u) {
   const int n = p.q_end - p.q_begin;
   const int base = n / p.n_qparts, rem = n % p.n_qparts;
@@ -200,11 +203,14 @@ __device__ __forceinline__ Unit decode_unit(const MmaParams& p, int u) {
   un.q0 = p.q_begin + ps + tq * kTileQ;
   un.q_end = p.q_begin + ps + pl;
   const int cb = r / p.nseg, sg = r - cb * p.nseg;
-  int cs, cl, ss, sl;
+  int cs, cl, ts, tl;
   shard32(p.k_end - p.k_begin, p.n_kparts, cb, &cs, &cl);
-  shard32(cl, p.nseg, sg, &ss, &sl);
-  un.ks = p.k_begin + cs + ss;
-  un.ke = un.ks + sl;
+  cs += p.k_begin;
+  const int t0 = cs / kTileK, t1 = (cs + cl + kTileK - 1) / kTileK;     // tiles [t0, t1) overlap the chunk
+  shard32(t1 - t0, p.nseg, sg, &ts, &tl);
+  const int a = (t0 + ts) * kTileK, b = (t0 + ts + tl) * kTileK;
+  un.ks = a > cs ? a : cs;
+  un.ke = b < cs + cl ? b : cs + cl;
   un.slot = p.slot0 + r;
   return un;
 }
