@@ -36,7 +36,8 @@ typedef enum {
   DCP_OK = 0,
   DCP_ERR_INVALID_ARG = 1, /* null pointer, non-positive size, parts > I, GRID with non-square parts,
                               misaligned pointer / pitch (16 B), c_z*sizeof(elt) % 16 != 0                         */
-  DCP_ERR_UNSUPPORTED = 2, /* a (dtype, H, c, c_z) the kernels are not instantiated for                           */
+  DCP_ERR_UNSUPPORTED = 2, /* a (dtype, H, c, c_z) the kernels are not instantiated for; a tensor-core shape with
+                              c_s % 8 != 0 (its GEMMs move 16-byte row pieces); a tile the kernel does not have   */
   DCP_ERR_WORKSPACE = 3,   /* workspace too small (see dcp_workspace_bytes)                                       */
   DCP_ERR_CUDA = 4         /* a CUDA runtime / driver call failed at launch time                                  */
 } dcp_status;
@@ -45,9 +46,11 @@ typedef enum { DCP_F32 = 0, DCP_BF16 = 1 } dcp_dtype;
 
 /* How the layer is cut (the on-device emulation of Design-CP's schemes):
  *   MONOLITHIC  one problem; keys processed as `key_split` Eq.-5 chunks merged left to right
- *   ROW         PAPER.md:72-86: `parts` query stripes (Eq. 5), each against ALL keys, one launch per stripe
- *   GRID        PAPER.md:90: G x G quadrants, G = sqrt(parts) (parts must be a perfect square), one launch per
- *               quadrant producing a partial (m, l, acc); the G key blocks of a row are merged left to right  */
+ *   ROW         PAPER.md:72-86: `parts` query stripes (Eq. 5), each against ALL keys
+ *   GRID        PAPER.md:90: G x G quadrants, G = sqrt(parts) (parts must be a perfect square), each producing a
+ *               partial (m, l, acc) from its own block of z; the G key blocks of a row are merged left to right
+ * On the tensor-core kernels all stripes / quadrants of a call are work units of ONE persistent launch (each unit
+ * reads only its own block of z, through a strided view); the generic kernel launches once per stripe / quadrant. */
 typedef enum { DCP_MONOLITHIC = 0, DCP_ROW = 1, DCP_GRID = 2 } dcp_decomp;
 
 /* Which fused kernel runs the (query-tile, key-tile) loop. */
@@ -116,7 +119,7 @@ dcp_status dcp_atom_pair_bias_attention(const void *a, const void *p, int64_t ld
  * softmax over the VALID slots, out_l = (sigmoid(a_l W_g) (.) sum_j a_j v_m) W_o.
  *   a [L, c_atom], p_slice [L, k, c_atompair], out [L, c_atom]: device, storage dtype, row-major, 16-byte aligned;
  *   idx [L, k]: device int32; idx < 0 marks an unused slot (an atom without valid slots gets out = 0); a neighbour
- *   listed twice counts twice; indices >= L are undefined behaviour.
+ *   listed twice counts twice; an index >= L is treated like a negative one (unused slot).
  * Instantiated for DCP_BF16, c = 32, c_atompair = 16, H <= 16, k <= 512, c_atom % 8 == 0 (DCP_ERR_UNSUPPORTED
  * otherwise).  workspace >= dcp_sparse_atom_workspace_bytes(...), 256-byte aligned.  Enqueues on `stream`.
  * `plan` may be NULL; only its ev_fused_begin / ev_fused_end (recorded around the gather kernel) are used. */
@@ -163,7 +166,8 @@ dcp_status dcp_pairformer_stack(void *s, void *z, const dcp_block_weights *block
 /* p_slice[l, j, :] = p[l, idx[l, j], :] ("The relevant slice of P is gathered at those k indices"): the
  * dense atom-pair tensor p [L, L, c_atompair] (row pitch ldp elements, 0 = L * c_atompair) -> the slice
  * [L, k, c_atompair] that dcp_sparse_atom_attention consumes; slots with idx < 0 are filled with zeros.  Device
- * pointers, c_atompair * element size a multiple of 16 bytes, 16-byte aligned (DCP_ERR_INVALID_ARG otherwise). */
+ * pointers, dtype DCP_F32 or DCP_BF16, c_atompair * element size a multiple of 16 bytes, 16-byte aligned
+ * (DCP_ERR_INVALID_ARG otherwise); an index >= L is treated like a negative one. */
 dcp_status dcp_gather_pair_slice(const void *p, int64_t ldp, const int32_t *idx, void *p_slice, int64_t L, int k,
                                  int c_atompair, dcp_dtype dtype, void *stream);
 
@@ -187,7 +191,13 @@ dcp_status dcp_pair_bias_attention_host(const void *s_host, const void *z_host, 
                                         void *workspace, size_t workspace_bytes, void *stream);
 
 /* Diagnostic: the partial online-softmax state of query rows [q0,q1) against keys [k0,k1) only:
- * m [q1-q0, H] = max_j logit, l [q1-q0, H] = sum_j e^{logit-m}, acc [q1-q0, H*c] = sum_j e^{logit-m} v_j (fp32). */
+ * m [q1-q0, H] = the state's reference, l [q1-q0, H] = sum_j e^{logit-m}, acc [q1-q0, H*c] = sum_j e^{logit-m} v_j
+ * (fp32, natural-log units).  A state is defined up to its reference: (m, l, acc) and (m', l e^{m-m'}, acc e^{m-m'})
+ * are the same state, and dcp_merge_states treats them alike.  DCP_KERNEL_GENERIC returns m = max_j logit; the
+ * tensor-core kernels move a row's reference lazily (only when a key tile's maximum exceeds it by more than 8 in
+ * log2 units), so their m satisfies  max_j logit - 8 ln 2 <= m <= max_j logit  (reading 19).
+ * Pointers, ldz and the workspace obey the same alignment rules as dcp_pair_bias_attention (16 bytes; workspace
+ * 256; >= dcp_workspace_bytes of the MONOLITHIC plan); m, l, acc 16-byte aligned. */
 dcp_status dcp_partial_states(const void *s, const void *z, int64_t ldz, const dcp_weights *w,
                               int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype, int kernel,
                               int64_t q0, int64_t q1, int64_t k0, int64_t k1,
@@ -196,7 +206,8 @@ dcp_status dcp_partial_states(const void *s, const void *z, int64_t ldz, const d
 
 /* The merge kernel alone: left fold over `n_parts` partial states of `rows` rows:
  * m' = max(m_a, m_b), l' = l_a e^{m_a-m'} + l_b e^{m_b-m'}, acc' likewise.  m, l: [n_parts, rows, H];
- * acc: [n_parts, rows, H*c]; outputs m_out, l_out [rows, H], acc_out [rows, H*c].  All fp32, device. */
+ * acc: [n_parts, rows, H*c]; outputs m_out, l_out [rows, H], acc_out [rows, H*c].  All fp32, device.  An empty
+ * state (m = -inf, l = 0, acc = 0) is the identity of the fold, also when both operands are empty. */
 dcp_status dcp_merge_states(int n_parts, int64_t rows, int H, int c, const float *m, const float *l,
                             const float *acc, float *m_out, float *l_out, float *acc_out, void *stream);
 

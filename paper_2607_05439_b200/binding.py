@@ -136,14 +136,16 @@ def _stream_ptr(stream=None):
     return C.c_void_p(s.cuda_stream)
 
 
-def _weights_struct(w: Dict[str, torch.Tensor], eps: float) -> dcp_weights:
+def _weights_struct(w: Dict[str, torch.Tensor], eps: float, dtype: Optional[torch.dtype] = None) -> dcp_weights:
     ws = dcp_weights()
     for name in ("w_q", "w_k", "w_v", "w_g", "w_b", "w_o", "ln_z_gamma", "ln_z_beta"):
         t = w[name]
         assert t.is_cuda and t.is_contiguous(), name
+        assert dtype is None or t.dtype == dtype, f"{name}: {t.dtype}, the activations are {dtype}"
         setattr(ws, name, t.data_ptr())
     for name in ("ln_s_gamma", "ln_s_beta", "b_q"):
         t = w.get(name)
+        assert t is None or (t.is_cuda and t.is_contiguous() and (dtype is None or t.dtype == dtype)), name
         setattr(ws, name, None if t is None else t.data_ptr())
     ws.ln_eps = float(eps)
     return ws
@@ -203,8 +205,13 @@ def dcp_last_launch_count() -> int:
     return int(_lib.dcp_last_launch_count())
 
 
-def _alloc_ws(nbytes: int, device) -> torch.Tensor:
-    return torch.empty(max(nbytes, 256), dtype=torch.uint8, device=device)
+def _alloc_ws(nbytes: int, device, stream=None) -> torch.Tensor:
+    """A temporary the kernels of `stream` use after the call returned: told to the caching allocator, so the block is
+    not handed to another tensor while those kernels run."""
+    t = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=device)
+    if stream is not None:
+        t.record_stream(stream)
+    return t
 
 
 def dcp_pair_bias_attention(s, z, w, H, c, decomp="monolithic", parts=1, key_split=1, kernel="auto", eps=1e-5,
@@ -216,14 +223,16 @@ def dcp_pair_bias_attention(s, z, w, H, c, decomp="monolithic", parts=1, key_spl
     c_z = z.shape[-1]
     dt = _dtype_code(s.dtype)
     assert z.dtype == s.dtype
+    # z may be a view with a row pitch (ldz), but keys and channels are dense
+    assert z.stride(-1) == 1 and z.stride(1) == c_z and (ldz or z.stride(0) == I * c_z), "z: inner dimensions not contiguous"
     if out is None:
         out = torch.empty(I, c_s, dtype=s.dtype, device=s.device)
     pl = _plan(parts, key_split, kernel,
                None if fused_events is None else (fused_events[0].handle, fused_events[1].handle), tile, key_segments)
     if workspace is None:
         workspace = _alloc_ws(dcp_workspace_bytes(I, c_s, H, c, c_z, s.dtype, decomp, parts, key_split, kernel, tile,
-                                                  key_segments), s.device)
-    ws = _weights_struct(w, eps)
+                                                  key_segments), s.device, stream)
+    ws = _weights_struct(w, eps, s.dtype)
     fn = _lib.dcp_atom_pair_bias_attention if atom else _lib.dcp_pair_bias_attention
     st = fn(_ptr(s), _ptr(z), int(ldz), C.byref(ws), _ptr(out), I, c_s, H, c, c_z, dt, DECOMP[decomp], C.byref(pl),
             _ptr(workspace), workspace.numel(), _stream_ptr(stream))
@@ -246,7 +255,7 @@ def dcp_pair_transition(z, w1, w2, w3, ln_gamma, ln_beta, eps=1e-5, out=None, wo
     if workspace is None:
         n = C.c_size_t(0)
         _check(_lib.dcp_pair_transition_workspace_bytes(c_z, _dtype_code(z.dtype), C.byref(n)), "dcp_pair_transition_workspace_bytes")
-        workspace = _alloc_ws(int(n.value), z.device)
+        workspace = _alloc_ws(int(n.value), z.device, stream)
     st = _lib.dcp_pair_transition(_ptr(z), _ptr(out), n_pairs, c_z, _ptr(w1), _ptr(w2), _ptr(w3), _ptr(ln_gamma), _ptr(ln_beta),
                                   C.c_float(eps), _dtype_code(z.dtype), _ptr(workspace), workspace.numel(), _stream_ptr(stream))
     _check(st, "dcp_pair_transition")
@@ -261,7 +270,7 @@ def dcp_pairformer_stack(s, z, blocks, H, c, eps=1e-5, workspace=None, stream=No
     I, c_s, c_z = s.shape[0], s.shape[1], z.shape[-1]
     arr = (dcp_block_weights * len(blocks))()
     for b, (wa, wt) in enumerate(blocks):
-        arr[b].attn = _weights_struct(wa, eps)
+        arr[b].attn = _weights_struct(wa, eps, s.dtype)
         for dst, src in (("w1", "w1"), ("w2", "w2"), ("w3", "w3"), ("ln_gamma", "gamma"), ("ln_beta", "beta")):
             t = wt[src]
             assert t.is_cuda and t.is_contiguous(), src
@@ -271,7 +280,7 @@ def dcp_pairformer_stack(s, z, blocks, H, c, eps=1e-5, workspace=None, stream=No
         n = C.c_size_t(0)
         _check(_lib.dcp_pairformer_stack_workspace_bytes(I, c_s, H, c, c_z, _dtype_code(s.dtype), C.byref(n)),
                "dcp_pairformer_stack_workspace_bytes")
-        workspace = _alloc_ws(int(n.value), s.device)
+        workspace = _alloc_ws(int(n.value), s.device, stream)
     st = _lib.dcp_pairformer_stack(_ptr(s), _ptr(z), arr, len(blocks), I, c_s, H, c, c_z, _dtype_code(s.dtype), _ptr(workspace),
                                    workspace.numel(), _stream_ptr(stream))
     _check(st, "dcp_pairformer_stack")
@@ -318,8 +327,8 @@ def dcp_sparse_atom_attention(a, p_slice, idx, w, H, c, eps=1e-5, out=None, work
     if out is None:
         out = torch.empty(L, c_atom, dtype=a.dtype, device=a.device)
     if workspace is None:
-        workspace = _alloc_ws(dcp_sparse_atom_workspace_bytes(L, c_atom, H, c, a.dtype), a.device)
-    ws = _weights_struct(w, eps)
+        workspace = _alloc_ws(dcp_sparse_atom_workspace_bytes(L, c_atom, H, c, a.dtype), a.device, stream)
+    ws = _weights_struct(w, eps, a.dtype)
     pl = _plan(1, 1, "auto", None if fused_events is None else (fused_events[0].handle, fused_events[1].handle))
     st = _lib.dcp_sparse_atom_attention(_ptr(a), _ptr(p_slice), _ptr(idx), C.byref(ws), _ptr(out), L, k, c_atom, H, c, c_p,
                                         _dtype_code(a.dtype), C.byref(pl), _ptr(workspace), workspace.numel(),
@@ -352,8 +361,8 @@ def dcp_partial_states(s, z, w, H, c, q0, q1, k0, k1, kernel="auto", eps=1e-5, s
     m = torch.empty(max(R, 0), H, dtype=torch.float32, device=s.device)
     l = torch.empty_like(m)
     acc = torch.empty(max(R, 0), D, dtype=torch.float32, device=s.device)
-    workspace = _alloc_ws(dcp_workspace_bytes(I, c_s, H, c, c_z, s.dtype), s.device)
-    ws = _weights_struct(w, eps)
+    workspace = _alloc_ws(dcp_workspace_bytes(I, c_s, H, c, c_z, s.dtype), s.device, stream)
+    ws = _weights_struct(w, eps, s.dtype)
     k = KERNEL[kernel] if isinstance(kernel, str) else int(kernel)
     st = _lib.dcp_partial_states(_ptr(s), _ptr(z), 0, C.byref(ws), I, c_s, H, c, c_z, _dtype_code(s.dtype), k,
                                  q0, q1, k0, k1, _ptr(m), _ptr(l), _ptr(acc), _ptr(workspace), workspace.numel(),
@@ -368,8 +377,12 @@ def dcp_merge_states(m, l, acc, H, c, stream=None):
     m_out = torch.empty(rows, H, dtype=torch.float32, device=m.device)
     l_out = torch.empty_like(m_out)
     acc_out = torch.empty(rows, H * c, dtype=torch.float32, device=m.device)
-    st = _lib.dcp_merge_states(n, rows, H, c, _ptr(m.contiguous()), _ptr(l.contiguous()), _ptr(acc.contiguous()),
-                               _ptr(m_out), _ptr(l_out), _ptr(acc_out), _stream_ptr(stream))
+    m, l, acc = m.contiguous(), l.contiguous(), acc.contiguous()
+    if stream is not None:
+        for t in (m, l, acc):
+            t.record_stream(stream)
+    st = _lib.dcp_merge_states(n, rows, H, c, _ptr(m), _ptr(l), _ptr(acc), _ptr(m_out), _ptr(l_out), _ptr(acc_out),
+                               _stream_ptr(stream))
     _check(st, "dcp_merge_states")
     return m_out, l_out, acc_out
 

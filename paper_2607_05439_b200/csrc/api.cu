@@ -123,6 +123,8 @@ dcp_status check_shape(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dt) 
   if (I > (int64_t)1 << 30) return DCP_ERR_INVALID_ARG;
   if ((c_z * elt_size(dt)) % 16 != 0) return DCP_ERR_INVALID_ARG;
   if (!fused_generic_supports(dt, H, c, c_z) && !fused_mma_supports(dt, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
+  // the tensor-core path's GEMMs move 16-byte row pieces of s, the projections and out
+  if (fused_mma_supports(dt, H, c, c_z) && c_s % 8 != 0) return DCP_ERR_UNSUPPORTED;
   return DCP_OK;
 }
 
@@ -471,7 +473,8 @@ dcp_status dcp_sparse_atom_attention(const void* a, const void* p_slice, const i
 dcp_status dcp_gather_pair_slice(const void* p, int64_t ldp, const int32_t* idx, void* p_slice, int64_t L, int k,
                                  int c_atompair, dcp_dtype dtype, void* stream) {
   g_launches = 0;
-  if (!p || !idx || !p_slice || L <= 0 || k <= 0 || c_atompair <= 0) return DCP_ERR_INVALID_ARG;
+  if (!p || !idx || !p_slice || L <= 0 || k <= 0 || c_atompair <= 0 || L > 0x7fffffff) return DCP_ERR_INVALID_ARG;
+  if (dtype != DCP_F32 && dtype != DCP_BF16) return DCP_ERR_INVALID_ARG;
   const int64_t e = elt_size(dtype);
   if (ldp == 0) ldp = L * (int64_t)c_atompair;
   if ((c_atompair * e) % 16 != 0 || (ldp * e) % 16 != 0 || (((uintptr_t)p | (uintptr_t)p_slice) & 15) != 0)
@@ -608,7 +611,9 @@ dcp_status dcp_partial_states(const void* s, const void* z, int64_t ldz, const d
   if (kernel == DCP_KERNEL_GENERIC && !fused_generic_supports(dtype, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
   const bool use_mma = mma_ok && kernel != DCP_KERNEL_GENERIC;
   if (ldz == 0) ldz = I * (int64_t)c_z;
-  if (misaligned(s) || misaligned(z) || misaligned(workspace, 256)) return DCP_ERR_INVALID_ARG;
+  if (ldz < I * (int64_t)c_z || (ldz * elt_size(dtype)) % 16 != 0) return DCP_ERR_INVALID_ARG;
+  if (misaligned(s) || misaligned(z) || misaligned(workspace, 256) || misaligned(m) || misaligned(l) || misaligned(acc))
+    return DCP_ERR_INVALID_ARG;
   Ctx x{};
   x.I = I; x.c_s = c_s; x.H = H; x.c = c; x.c_z = c_z; x.D = H * c; x.dt = dtype; x.w = w;
   x.eps = w->ln_eps > 0.f ? w->ln_eps : 1e-5f;

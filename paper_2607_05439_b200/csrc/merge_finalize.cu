@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(256) merge_kernel(const MergeParams p) {
     const float lb = p.st_l[srow * p.H + h];
     const float ab = p.st_acc[srow * p.D + e];
     const float mn = fmaxf(m, mb);
-    const float fa = expf(m - mn), fb = expf(mb - mn);
+    const float fa = mn == -INFINITY ? 0.f : expf(m - mn), fb = mn == -INFINITY ? 0.f : expf(mb - mn);   // empty (+) empty
     l = l * fa + lb * fb;
     a = a * fa + ab * fb;
     m = mn;
@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(256) merge_vec4_kernel(const MergeParams p) {
 #pragma unroll
     for (int s = 1; s < NS; ++s) {
       const float mn = fmaxf(m, ms[s]);
-      const float fa = expf(m - mn), fb = expf(ms[s] - mn);
+      const float fa = mn == -INFINITY ? 0.f : expf(m - mn), fb = mn == -INFINITY ? 0.f : expf(ms[s] - mn);
       l = l * fa + ls[s] * fb;
       a.x = a.x * fa + as[s].x * fb; a.y = a.y * fa + as[s].y * fb;
       a.z = a.z * fa + as[s].z * fb; a.w = a.w * fa + as[s].w * fb;
@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(256) merge_vec4_kernel(const MergeParams p) {
       const float lb = p.st_l[srow * p.H + h];
       const float4 ab = *reinterpret_cast<const float4*>(p.st_acc + srow * p.D + e);
       const float mn = fmaxf(m, mb);
-      const float fa = expf(m - mn), fb = expf(mb - mn);
+      const float fa = mn == -INFINITY ? 0.f : expf(m - mn), fb = mn == -INFINITY ? 0.f : expf(mb - mn);
       l = l * fa + lb * fb;
       a.x = a.x * fa + ab.x * fb; a.y = a.y * fa + ab.y * fb;
       a.z = a.z * fa + ab.z * fb; a.w = a.w * fa + ab.w * fb;

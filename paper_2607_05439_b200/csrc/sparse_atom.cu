@@ -93,7 +93,8 @@ __global__ void __launch_bounds__(128) sparse_atom_kernel(const SparseParams p) 
     nb[ps] = -1;
     if (ps < npass) {
       const int j = ps * 32 + lane;
-      const int m = j < p.kn ? __ldg(p.idx + l * p.kn + j) : -1;
+      int m = j < p.kn ? __ldg(p.idx + l * p.kn + j) : -1;
+      if ((unsigned)m >= (unsigned)p.L) m = -1;          // negative or >= L: unused slot
       nb[ps] = m;
       if (m >= 0) {
         const uint4* kr = reinterpret_cast<const uint4*>(p.k + (int64_t)m * D + h * sC);
@@ -192,7 +193,8 @@ __global__ void __launch_bounds__(128) sparse_atom_rows_kernel(const SparseParam
   // ---- (A) lane = slot: neighbour index, LayerNorm statistics of the p row, bias of every head
   for (int j0 = 0; j0 < kpad; j0 += 32) {
     const int j = j0 + lane;
-    const int m = j < p.kn ? __ldg(p.idx + l * p.kn + j) : -1;
+    int m = j < p.kn ? __ldg(p.idx + l * p.kn + j) : -1;
+    if ((unsigned)m >= (unsigned)p.L) m = -1;            // negative or >= L: unused slot
     s_idx[j] = m;
     if (m >= 0) {
       const uint4* pr = reinterpret_cast<const uint4*>(p.p + (l * p.kn + j) * sCz);
@@ -326,7 +328,7 @@ __global__ void __launch_bounds__(256) gather_pair_slice_kernel(const uint4* __r
   const int64_t slot = e / chunks;
   const int64_t l = slot / kn;
   const int m = __ldg(idx + slot);
-  out[e] = m >= 0 ? __ldg(P + l * ldp16 + (int64_t)m * chunks + ch) : make_uint4(0u, 0u, 0u, 0u);
+  out[e] = (unsigned)m < (unsigned)L ? __ldg(P + l * ldp16 + (int64_t)m * chunks + ch) : make_uint4(0u, 0u, 0u, 0u);
 }
 
 }  // namespace

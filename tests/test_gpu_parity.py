@@ -296,3 +296,86 @@ def test_error_paths():
     # still healthy afterwards
     out = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c)
     assert torch.isfinite(out).all() and dcp.dcp_last_launch_count() > 0
+
+
+# ------------------------------------------------------------------ the ring's visiting order (SURVEY.md 8c reading 13)
+@pytest.mark.parametrize("dtype,c_z,H,c,kern", [("f32", 32, 4, 24, "generic"), ("bf16", 128, 16, 48, "mma")])
+def test_merge_in_rotated_ring_order(dtype, c_z, H, c, kern):
+    """Row block r of a G x G grid merged in the order a ring visits its key blocks -- starting at block c = r
+    ("bundles the K/V/B shift") -- instead of ascending c: the device merge of the device's own
+    quadrant states, fed in rotated order, agrees with the oracle's rotated-order grid and with the canonical order
+    within tolerance (not bitwise: the fold is not associative)."""
+    from oracle import decompositions as dec
+    dcp = _dcp()
+    G = 3
+    cfg = syn.small_config("ring", I=150, c_s=64, c_z=c_z, H=H, c=c, dtype=dtype, seed=41)
+    s, z, w = util.make_problem(cfg, DEV)
+    ref_rot = dec.grid_decomposition(util.np64(s), util.np32(z), util.weights_np(w), cfg.H, cfg.c, G * G, first_block_offset=True)
+    ref = util.oracle_rows(cfg, s, z, w, range(cfg.I))
+    assert np.max(np.abs(ref_rot - ref)) <= 1e-10
+    wn = util.weights_np(w)
+    g = 1.0 / (1.0 + np.exp(-(util.np64(s) @ wn["w_g"])))
+    out_rot, out_can = np.zeros_like(ref), np.zeros_like(ref)
+    for r in range(G):
+        q0, ql = dcp.dcp_shard_range(cfg.I, G, r)
+        st = []
+        for cb in range(G):
+            k0, kl = dcp.dcp_shard_range(cfg.I, G, cb)
+            st.append(dcp.dcp_partial_states(s, z, w, cfg.H, cfg.c, q0, q0 + ql, k0, k0 + kl, kernel=kern))
+        for order, dst in (([(r + t) % G for t in range(G)], out_rot), (list(range(G)), out_can)):
+            M = torch.stack([st[cb][0] for cb in order]); L = torch.stack([st[cb][1] for cb in order])
+            A = torch.stack([st[cb][2] for cb in order])
+            _, ll, aa = dcp.dcp_merge_states(M, L, A, cfg.H, cfg.c)
+            o = util.np64(aa).reshape(ql, cfg.H, cfg.c) / util.np64(ll)[..., None]
+            dst[q0:q0 + ql] = (g[q0:q0 + ql] * o.reshape(ql, -1)) @ wn["w_o"]
+    tol = 1e-5 if dtype == "f32" else util.TOL_BF16_MAXABS
+    assert np.max(np.abs(out_rot - ref)) <= tol and np.max(np.abs(out_can - ref)) <= tol
+    assert np.max(np.abs(out_rot - out_can)) <= (1e-6 if dtype == "f32" else 1e-4) * max(1.0, np.max(np.abs(ref)))
+
+
+def test_merge_of_empty_states_is_the_identity():
+    dcp = _dcp()
+    rows, H, c = 4, 2, 4
+    g = torch.Generator(device="cpu").manual_seed(8)
+    m = torch.randn(3, rows, H, generator=g); l = torch.rand(3, rows, H, generator=g) + 0.5
+    acc = torch.randn(3, rows, H * c, generator=g)
+    for empty in ((0, 1), (1, 2), (0, 1, 2)):
+        mm, ll, aa = m.clone(), l.clone(), acc.clone()
+        for e in empty:
+            mm[e] = -float("inf"); ll[e] = 0.0; aa[e] = 0.0
+        mo, lo, ao = dcp.dcp_merge_states(mm.to(DEV), ll.to(DEV), aa.to(DEV), H, c)
+        assert not torch.isnan(mo).any() and not torch.isnan(lo).any() and not torch.isnan(ao).any()
+        keep = [i for i in range(3) if i not in empty]
+        if len(keep) == 1:
+            assert torch.equal(mo.cpu(), m[keep[0]]) and torch.equal(lo.cpu(), l[keep[0]]) and torch.equal(ao.cpu(), acc[keep[0]])
+        else:
+            assert torch.isinf(mo).all() and (lo == 0).all() and (ao == 0).all()
+
+
+# ------------------------------------------------------------------ dcp_plan: tile and key_segments
+def test_plan_tile_and_key_segments():
+    dcp = _dcp()
+    cfg = syn.small_config("plan", I=300, c_s=64, c_z=128, H=16, c=48, dtype="bf16", seed=17)
+    s, z, w = util.make_problem(cfg, DEV)
+    ref = util.oracle_rows(cfg, s, z, w, range(cfg.I))
+    base = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c)
+    assert torch.equal(dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, tile=(32, 16)), base)     # the kernel's own tiling
+    for bad in ((64, 16), (32, 32), (128, 0)):
+        with pytest.raises(dcp.DcpError) as e:
+            dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, tile=bad)
+        assert e.value.status == 2
+    with pytest.raises(dcp.DcpError) as e:
+        dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, key_segments=65)
+    assert e.value.status == 1
+    for ks in (1, 2, 5, 64):           # 64 is clamped to the whole key tiles of a chunk
+        mono = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, key_segments=ks)
+        util.check_close(mono, ref, "bf16", f"key_segments={ks}")
+        row = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, decomp="row", parts=7, key_segments=ks)
+        assert torch.equal(row, mono), f"row(7) != monolithic bitwise at key_segments={ks}"
+        grid = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, decomp="grid", parts=9, key_segments=ks)
+        assert torch.equal(grid, dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, key_split=3, key_segments=ks))
+        util.check_close(grid, ref, "bf16", f"grid(9) key_segments={ks}")
+    cfg0 = syn.CONFIGS["C0"]
+    s0, z0, w0 = util.make_problem(cfg0, DEV)
+    assert torch.equal(dcp.dcp_pair_bias_attention(s0, z0, w0, cfg0.H, cfg0.c, tile=(8, 32)),
+                       dcp.dcp_pair_bias_attention(s0, z0, w0, cfg0.H, cfg0.c))

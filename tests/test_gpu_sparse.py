@@ -65,6 +65,26 @@ def test_sparse_masked_slots_and_empty_rows():
     assert torch.all(out[5] == 0)
 
 
+def test_sparse_out_of_range_indices_are_unused_slots():
+    """An index >= L is treated like a negative one (include/designcp.h): same output as with -1 there, for both
+    kernels (rows kernel H = 4, slot-per-lane kernel H = 16) and for the gather."""
+    dcp = _dcp()
+    for H in (4, 16):
+        cfg, a, p, idx, w = _problem(80, 48, H=H, seed=23)
+        g = torch.Generator(device="cpu").manual_seed(6)
+        mask = (torch.rand(idx.shape, generator=g) < 0.25).to(DEV)
+        big = torch.where(mask, torch.full_like(idx, cfg.I + 1000), idx).contiguous()
+        big[3, 0] = 2 ** 31 - 1
+        neg = torch.where(big >= cfg.I, torch.full_like(idx, -1), big).contiguous()
+        assert torch.equal(dcp.dcp_sparse_atom_attention(a, p, big, w, cfg.H, cfg.c),
+                           dcp.dcp_sparse_atom_attention(a, p, neg, w, cfg.H, cfg.c))
+    P = syn.make_z(cfg, DEV)
+    assert torch.equal(dcp.dcp_gather_pair_slice(P, big), dcp.dcp_gather_pair_slice(P, neg))
+    from paper_2607_05439_b200 import binding
+    st = binding.raw().dcp_gather_pair_slice(P.data_ptr(), 0, big.data_ptr(), p.data_ptr(), cfg.I, big.shape[1], 16, 7, None)
+    assert st == 1                                         # unknown dtype code
+
+
 def test_sparse_full_budget_matches_dense_layer():
     """k = L with every atom listed once: the sparse kernel and the dense atom-level kernel compute the same layer."""
     dcp = _dcp()
