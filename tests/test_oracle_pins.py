@@ -552,3 +552,53 @@ def test_stack_round_store_is_applied_once_per_block():
     s1, z1 = pso.pairformer_block(bf(s), bf(z), *blocks[0], H, c, round_store=bf)
     s2b, z2b = pso.pairformer_block(s1, z1, *blocks[1], H, c, round_store=bf)
     assert np.array_equal(s2, s2b) and np.array_equal(z2, z2b)
+
+
+# ------------------------------------------------------------------ attention stack on a read-only pair tensor
+def _attn_stack_problem(rng, I=5, c_s=6, c_z=4, H=2, c=3, n_blocks=3):
+    s, z, _ = rand_problem(rng, I, c_s, c_z, H, c)
+    return s, z, [rand_problem(rng, I, c_s, c_z, H, c)[2] for _ in range(n_blocks)]
+
+
+def test_attention_stack_identity_and_single_block():
+    from oracle import attention_stack as aso
+    from oracle import pair_bias_attention as orc
+    H, c = 2, 3
+    a, z, blocks = _attn_stack_problem(np.random.default_rng(81))
+    z0 = z.copy()
+    one = aso.attention_stack(a, z, blocks[:1], H, c)
+    assert np.array_equal(one, a + orc.pair_bias_attention(a, z, blocks[0], H, c))
+    assert np.array_equal(z, z0)                                        # Z is read-only
+    dead = [dict(w, w_o=np.zeros_like(w["w_o"])) for w in blocks]
+    assert np.array_equal(aso.attention_stack(a, z, dead, H, c), a)     # W_o = 0: identity at any depth
+
+
+def test_attention_stack_order_against_brute_force():
+    """Block b reads the latent block b - 1 wrote, its OWN weights, and the original Z."""
+    from oracle import attention_stack as aso
+    H, c = 2, 3
+    a, z, blocks = _attn_stack_problem(np.random.default_rng(82))
+    a1 = aso.attention_stack(a, z, blocks[:1], H, c)
+    a2 = aso.attention_stack(a, z, blocks[:2], H, c)
+    a3 = aso.attention_stack(a, z, blocks, H, c)
+    assert np.max(np.abs(a1 - (a + _brute_attention(a, z, blocks[0], H, c)))) <= 1e-12
+    assert np.max(np.abs(a2 - (a1 + _brute_attention(a1, z, blocks[1], H, c)))) <= 1e-12
+    assert np.max(np.abs(a3 - (a2 + _brute_attention(a2, z, blocks[2], H, c)))) <= 1e-12
+    # the plausible mistakes move the result by far more than rounding
+    assert np.max(np.abs(a2 - (a1 + _brute_attention(a, z, blocks[1], H, c)))) > 1e-3      # stale latent
+    assert np.max(np.abs(a2 - (a1 + _brute_attention(a1, z, blocks[0], H, c)))) > 1e-3     # another block's weights
+    assert np.max(np.abs(a2 - (a + _brute_attention(a1, z, blocks[1], H, c)))) > 1e-3      # residual onto the wrong latent
+
+
+def test_attention_stack_round_store_once_per_block():
+    from oracle import attention_stack as aso
+    H, c = 2, 3
+    a, z, blocks = _attn_stack_problem(np.random.default_rng(83))
+    bf = lambda x: torch.from_numpy(np.asarray(x)).to(torch.bfloat16).double().numpy()
+    a3 = aso.attention_stack(bf(a), bf(z), blocks, H, c, round_store=bf)
+    assert np.array_equal(bf(a3), a3)
+    step = bf(a)
+    for w in blocks:
+        step = aso.attention_stack(step, bf(z), [w], H, c, round_store=bf)
+    assert np.array_equal(a3, step)
+    assert np.max(np.abs(a3 - aso.attention_stack(bf(a), bf(z), blocks, H, c))) > 0          # the rounding is really there
