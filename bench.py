@@ -48,7 +48,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4", "K4", "T2", "T3", "P2"],
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4", "K4", "T2", "T3", "P2", "D2", "D3"],
                     help="C0..C4: BASELINE.json configs (dense layer); S4: sparse k-neighbour atom attention on C4's atoms; "
                          "K4: the k-nearest-neighbour lists of C4's atoms (dcp_knn); T2 / T3: the pairwise SwiGLU transition on "
                          "C2's / C3's pair tensor (dcp_pair_transition)")
@@ -56,7 +56,7 @@ def parse():
     ap.add_argument("--decomp", default="monolithic", choices=["monolithic", "row", "grid"])
     ap.add_argument("--parts", type=int, default=0, help="row stripes / grid cells (0: 8 rows, 16 grid)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "mma"])
-    ap.add_argument("--blocks", type=int, default=2, help="P2: Pairformer blocks in the stack (PAPER.md:293: two)")
+    ap.add_argument("--blocks", type=int, default=2, help="P2: Pairformer blocks in the stack (PAPER.md:293: two); D2 | D3: attention blocks (default there: 18, PAPER.md:294)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-rows", type=int, default=0, help="oracle sample rows (0: sized for ~10-20 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -615,6 +615,127 @@ def run_stack(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_attention_stack(args, rank, world, local_rank):
+    """--workload D2 | D3: --blocks (default 18) sequential AttentionPairBias blocks with
+    residual on the c_token = 768 latent against the READ-ONLY pair tensor of C2 (I = 3000) / C3 (I = 12000), one call.
+    One pair = one (block, token pair): blocks * I^2 per step.  Every block re-streams z: algorithmic bytes per block =
+    I^2 * c_z * 2, roofline = HBM."""
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import __graft_entry__ as ge
+    if rank == 0 or world == 1:
+        ge.build()
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+        dist.barrier()
+    import dcp_synth as syn
+    import paper_2607_05439_b200 as dcp
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    base = syn.CONFIGS["C2" if args.workload == "D2" else "C3"]
+    cfg = replica_config(syn.small_config(args.workload, I=base.I, c_s=768, c_z=base.c_z, H=base.H, c=base.c, dtype="bf16",
+                                          seed=base.seed, structured=True), rank, world)
+    nb = args.blocks if args.blocks != 2 else 18
+    # every block normalises the latent it reads (the paper's blocks all have a layer-norm path, PAPER.md:289): keeps the
+    # residual stream of random-weight blocks finite over many steps
+    blocks = [syn.make_weights(syn.small_config("blk", I=cfg.I, c_s=cfg.c_s, c_z=cfg.c_z, H=cfg.H, c=cfg.c, dtype="bf16",
+                                                seed=cfg.seed + 101 * (b + 1)), dev, with_ln_s=True) for b in range(nb)]
+    a0, z = syn.make_s(cfg, dev), syn.make_z(cfg, dev)
+    a = a0.clone()
+    ws = torch.empty(dcp.dcp_attention_stack_workspace_bytes(cfg.I, cfg.c_s, cfg.H, cfg.c, cfg.c_z, a.dtype), dtype=torch.uint8, device=dev)
+    n_pairs = float(cfg.I) * cfg.I * nb
+    for _ in range(max(args.warmup, 3)):
+        dcp.dcp_attention_stack(a, z, blocks, cfg.H, cfg.c, workspace=ws)
+    launches = dcp.dcp_last_launch_count()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = dcp.Event(), dcp.Event()
+    e0.record()
+    for _ in range(args.steps):
+        dcp.dcp_attention_stack(a, z, blocks, cfg.H, cfg.c, workspace=ws)
+    e1.record()
+    torch.cuda.synchronize()
+    total_ms = max_over_ranks_ms(e0.elapsed_ms(e1), world, dev)
+    step_ms = total_ms / args.steps
+    value = n_pairs * args.steps * world / (total_ms * 1e-3) / 1e9
+    # the dominant kernel (fused_mma_kernel), timed on the same shapes with an event pair around it: one layer call per step
+    lw = torch.empty(dcp.dcp_workspace_bytes(cfg.I, cfg.c_s, cfg.H, cfg.c, cfg.c_z, a.dtype), dtype=torch.uint8, device=dev)
+    out = torch.empty_like(a)
+    evs = [(dcp.Event(), dcp.Event()) for _ in range(args.steps)]
+    for k in range(args.steps):
+        dcp.dcp_pair_bias_attention(a0, z, blocks[k % nb], cfg.H, cfg.c, out=out, workspace=lw, fused_events=evs[k])
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if rank == 0 else None
+    kms = sum(x.elapsed_ms(y) for x, y in evs) / len(evs)
+    peak, peak_how = measured_peaks()
+    zb = float(cfg.I) * cfg.I * cfg.c_z * 2
+    roofline = {"bound": "hbm", "achieved": zb / (kms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                "frac": zb / (kms * 1e-3) / 1e9 / peak, "traffic": None, "kernel": "fused_mma_kernel", "peak_source": peak_how,
+                "kernel_ms": kms, "kernel_share_of_step": nb * kms / step_ms, "algorithmic_bytes_per_launch": zb,
+                "launches_per_step": nb, "call_achieved": nb * zb / (step_ms * 1e-3) / 1e9,
+                "call_frac": nb * zb / (step_ms * 1e-3) / 1e9 / peak,
+                "note": "kernel_ms: fused kernel of single layer calls on the same shapes (event pair around it); "
+                        "call_frac: blocks x z bytes over the whole stack call"}
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        n_rows = args.cpu_rows or max(2, min(cfg.I, int(3.0e6 / cfg.I)))
+        oracle_sample(cfg, a0, z, blocks[0], 2)
+        pairs, dt, threads, rows, ref = oracle_sample(cfg, a0, z, blocks[0], n_rows)
+        a1 = a0.clone()
+        dcp.dcp_attention_stack(a1, z, blocks[:1], cfg.H, cfg.c, workspace=ws)
+        idx = torch.as_tensor(rows, device=dev)
+        f64 = lambda t: t.detach().float().cpu().double().numpy()
+        upd = f64(a1.index_select(0, idx)) - f64(a0.index_select(0, idx))
+        cpu = {"value": pairs / dt / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"block 1 of the stack on {len(rows)} sampled query rows x {cfg.I} keys ({dt:.1f} s), fp64 numpy oracle",
+               "gpu_vs_oracle_update_rel_l2_on_sample": float(np.linalg.norm(upd - ref) / np.linalg.norm(ref))}
+    e2e = None
+    if not args.no_e2e:
+        try:
+            ah, zh = a0.cpu().pin_memory(), z.cpu().pin_memory()
+            ao = torch.empty(a0.shape, dtype=a0.dtype).pin_memory()
+            ne = max(1, args.e2e_steps)
+            x, y = dcp.Event(), dcp.Event()
+            torch.cuda.synchronize()
+            x.record()
+            for _ in range(ne):
+                a.copy_(ah, non_blocking=True)
+                z.copy_(zh, non_blocking=True)
+                dcp.dcp_attention_stack(a, z, blocks, cfg.H, cfg.c, workspace=ws)
+                ao.copy_(a, non_blocking=True)
+            y.record()
+            torch.cuda.synchronize()
+            ms = max_over_ranks_ms(x.elapsed_ms(y), world, dev)
+            e2e = {"value": n_pairs * ne * world / (ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": (ah.numel() + zh.numel()) * 2,
+                   "d2h_bytes_per_step": ao.numel() * 2, "steps": ne, "note": "host latent and pair tensor copied in every step"}
+        except Exception as exc:
+            e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": None, "d2h_bytes_per_step": None, "error": repr(exc)[:200]}
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic",
+            "config": {"workload": f"{args.workload}: {nb} sequential AttentionPairBias blocks with residual on the c_token={cfg.c_s} "
+                                   f"latent, read-only pair tensor I={cfg.I} c_z={cfg.c_z} H={cfg.H} c={cfg.c} bf16 "
+                                   f"(icosahedral 60 x {cfg.n_res}; PAPER.md:294)",
+                       "pair": "one (block, token pair)", "blocks": nb, "kernel": "fused_mma_kernel",
+                       "ms_per_block": step_ms / nb,
+                       "l2": "z (%.0f MB) larger than the 126 MB L2: no flush needed" % (z.numel() * 2 / 1e6),
+                       "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "peak_device_bytes": int(torch.cuda.max_memory_allocated())},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": launches * args.steps, "clocks": clocks,
+            "hbm_roofline_gpair_per_s": peak * 1e9 / (cfg.c_z * 2) / 1e9}), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
 def run_knn(args, rank, world, local_rank):
     """--workload K4: neighbour lists of C4's 24000 synthetic atoms, k = --neighbours.
     One pair = one (query atom, candidate atom) distance: L^2 per call.  Single GPU (or independent replicas)."""
@@ -861,6 +982,9 @@ def main():
         return
     if args.workload == "P2":
         run_stack(args, rank, world, local_rank)
+        return
+    if args.workload in ("D2", "D3"):
+        run_attention_stack(args, rank, world, local_rank)
         return
 
     import torch

@@ -163,6 +163,24 @@ dcp_status dcp_pairformer_stack(void *s, void *z, const dcp_block_weights *block
                                 int H, int c, int c_z, dcp_dtype dtype, void *workspace, size_t workspace_bytes,
                                 void *stream);
 
+/* The diffusion transformer's attention stack on a resident, READ-ONLY pair tensor.
+ * PAPER.md:294 "Eighteen sequential AttentionPairBiasDiffusion + ConditionedTransitionBlock blocks (16 heads each ...)
+ * update the token-level latent A_I in R^{B x I x c_token} using the local pair bias derived from Z.  This is the stage
+ * that dominates per-step compute"; :285 c_token = 768.  Block b = 0 .. n_blocks-1 (reading 25):
+ *       A <- A + AttentionPairBias_b(A, Z)        (the layer of dcp_pair_bias_attention with blocks[b], MONOLITHIC)
+ * a [I, c_s] (c_s = c_token) is updated IN PLACE and stored in the storage dtype once per block (the residual is added
+ * in fp32 inside the output projection); z [I, I, c_z] (row pitch ldz elements, 0 = I * c_z) is only read: every block
+ * re-streams it and derives its own bias LN_b(z) W_b^b.  The conditional (AdaLN) normalisation and the
+ * ConditionedTransitionBlock have no formulas in the paper and are not part of the call.
+ * blocks: HOST array of n_blocks dcp_weights whose pointers are device pointers, read during the call only.
+ * DCP_BF16 and a (H, c, c_z) the tensor-core kernel is instantiated for (DCP_ERR_UNSUPPORTED otherwise).
+ * workspace >= dcp_attention_stack_workspace_bytes, 256-byte aligned.  Enqueues 4 launches per block on `stream`
+ * (chained by programmatic dependent launch), no host synchronisation: capturable into a CUDA graph. */
+dcp_status dcp_attention_stack_workspace_bytes(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype, size_t *bytes);
+dcp_status dcp_attention_stack(void *a, const void *z, int64_t ldz, const dcp_weights *blocks, int n_blocks, int64_t I,
+                               int c_s, int H, int c, int c_z, dcp_dtype dtype, void *workspace, size_t workspace_bytes,
+                               void *stream);
+
 /* p_slice[l, j, :] = p[l, idx[l, j], :] ("The relevant slice of P is gathered at those k indices"): the
  * dense atom-pair tensor p [L, L, c_atompair] (row pitch ldp elements, 0 = L * c_atompair) -> the slice
  * [L, k, c_atompair] that dcp_sparse_atom_attention consumes; slots with idx < 0 are filled with zeros.  Device

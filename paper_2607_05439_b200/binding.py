@@ -31,6 +31,7 @@ EXPORTS = [
     "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention", "dcp_knn", "dcp_gather_pair_slice",
     "dcp_pair_transition_workspace_bytes", "dcp_pair_transition",
     "dcp_pairformer_stack_workspace_bytes", "dcp_pairformer_stack",
+    "dcp_attention_stack_workspace_bytes", "dcp_attention_stack",
     "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
     "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
 ]
@@ -98,7 +99,9 @@ def _load() -> C.CDLL:
     lib.dcp_pair_transition.argtypes = [vp, vp, i64, i32, vp, vp, vp, vp, vp, C.c_float, i32, vp, sz, vp]
     lib.dcp_pairformer_stack_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, i32, C.POINTER(sz)]
     lib.dcp_pairformer_stack.argtypes = [vp, vp, C.POINTER(dcp_block_weights), i32, i64, i32, i32, i32, i32, i32, vp, sz, vp]
-    for n in EXPORTS[:15]:
+    lib.dcp_attention_stack_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, i32, C.POINTER(sz)]
+    lib.dcp_attention_stack.argtypes = [vp, vp, i64, C.POINTER(dcp_weights), i32, i64, i32, i32, i32, i32, i32, vp, sz, vp]
+    for n in EXPORTS[:17]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -285,6 +288,33 @@ def dcp_pairformer_stack(s, z, blocks, H, c, eps=1e-5, workspace=None, stream=No
                                    workspace.numel(), _stream_ptr(stream))
     _check(st, "dcp_pairformer_stack")
     return s, z
+
+
+def dcp_attention_stack(a, z, blocks, H, c, eps=1e-5, workspace=None, stream=None, ldz=0):
+    """n sequential AttentionPairBias blocks with residual, IN PLACE on the latent a [I, c_token], against the read-only
+    pair tensor z [I, I, c_z].  blocks: sequence of attention weight dicts (one per block)."""
+    assert a.is_cuda and z.is_cuda and a.is_contiguous() and z.dtype == a.dtype
+    I, c_s, c_z = a.shape[0], a.shape[1], z.shape[-1]
+    assert z.stride(-1) == 1 and z.stride(1) == c_z and (ldz or z.stride(0) == I * c_z), "z: inner dimensions not contiguous"
+    arr = (dcp_weights * len(blocks))()
+    for b, w in enumerate(blocks):
+        arr[b] = _weights_struct(w, eps, a.dtype)
+    if workspace is None:
+        n = C.c_size_t(0)
+        _check(_lib.dcp_attention_stack_workspace_bytes(I, c_s, H, c, c_z, _dtype_code(a.dtype), C.byref(n)),
+               "dcp_attention_stack_workspace_bytes")
+        workspace = _alloc_ws(int(n.value), a.device, stream)
+    st = _lib.dcp_attention_stack(_ptr(a), _ptr(z), int(ldz), arr, len(blocks), I, c_s, H, c, c_z, _dtype_code(a.dtype),
+                                  _ptr(workspace), workspace.numel(), _stream_ptr(stream))
+    _check(st, "dcp_attention_stack")
+    return a
+
+
+def dcp_attention_stack_workspace_bytes(I, c_s, H, c, c_z, dtype: torch.dtype) -> int:
+    n = C.c_size_t(0)
+    _check(_lib.dcp_attention_stack_workspace_bytes(int(I), int(c_s), int(H), int(c), int(c_z), _dtype_code(dtype), C.byref(n)),
+           "dcp_attention_stack_workspace_bytes")
+    return int(n.value)
 
 
 def dcp_gather_pair_slice(p, idx, out=None, stream=None):

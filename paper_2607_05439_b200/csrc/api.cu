@@ -256,7 +256,9 @@ dcp_status validate_weights(const dcp_weights* w) {
 
 dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w, void* out, int64_t I, int c_s, int H,
                  int c, int c_z, dcp_dtype dt, dcp_decomp decomp, const dcp_plan* plan_in, void* workspace,
-                 size_t workspace_bytes, void* stream) {
+                 size_t workspace_bytes, void* stream, const void* residual = nullptr) {
+  // residual != nullptr: out = storage(residual + layer output), added in fp32 inside the W_o GEMM's epilogue (tensor-core
+  // path with a tcgen05-shaped W_o only: DCP_ERR_UNSUPPORTED otherwise); residual may be `out`
   g_launches = 0;
   if (!s || !z || !out || !workspace) return DCP_ERR_INVALID_ARG;
   dcp_status st = validate_weights(w);
@@ -356,8 +358,13 @@ dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w
     gp.A = x.ws + x.cv.gated; gp.lda = x.D; gp.M = I; gp.N = c_s; gp.K = x.D; gp.nseg = 1;
     gp.W[0] = w->w_o; gp.C[0] = out; gp.mode[0] = GEMM_OUT_PLAIN; gp.ldc[0] = c_s;
     gp.pdl = pdl_enabled();
+    if (residual != nullptr) {
+      gp.residual = residual; gp.ldr = c_s;
+      if (!gemm_tc_supports(gp)) return DCP_ERR_UNSUPPORTED;
+    }
     DCP_CUDA(launch_gemm_mma(gp, x.st));
   } else {
+    if (residual != nullptr) return DCP_ERR_UNSUPPORTED;
     DCP_CUDA(launch_gemm(dt, false, x.ws + x.cv.gated, x.D, w->w_o, nullptr, out, c_s, I, c_s, x.D, EPI_NONE, x.st));
   }
   return DCP_OK;
@@ -563,6 +570,49 @@ dcp_status dcp_pairformer_stack(void* s, void* z, const dcp_block_weights* block
                              pair_transition_workspace_bytes(), stream);                                       // Transition, Eq. 6
     if (st != DCP_OK) return st;
     launches += 1 + g_launches;
+  }
+  g_launches = launches;
+  return DCP_OK;
+}
+
+// ---- attention stack on a read-only pair tensor (reading 25)
+dcp_status dcp_attention_stack_workspace_bytes(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype, size_t* bytes) {
+  if (!bytes) return DCP_ERR_INVALID_ARG;
+  size_t attn = 0;
+  dcp_status st = dcp_workspace_bytes(I, c_s, H, c, c_z, dtype, DCP_MONOLITHIC, nullptr, &attn);
+  if (st != DCP_OK) return st;
+  if (dtype != DCP_BF16 || !fused_mma_supports(dtype, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
+  *bytes = align256(attn) + align256((size_t)I * c_s * elt_size(dtype));
+  return DCP_OK;
+}
+
+dcp_status dcp_attention_stack(void* a, const void* z, int64_t ldz, const dcp_weights* blocks, int n_blocks, int64_t I,
+                               int c_s, int H, int c, int c_z, dcp_dtype dtype, void* workspace, size_t workspace_bytes,
+                               void* stream) {
+  g_launches = 0;
+  if (!a || !z || !blocks || !workspace || n_blocks <= 0) return DCP_ERR_INVALID_ARG;
+  size_t need = 0, attn = 0;
+  dcp_status st = dcp_attention_stack_workspace_bytes(I, c_s, H, c, c_z, dtype, &need);
+  if (st != DCP_OK) return st;
+  if (workspace_bytes < need) return DCP_ERR_WORKSPACE;
+  if (((uintptr_t)workspace & 255) != 0 || (I * c_s) % 8 != 0) return DCP_ERR_INVALID_ARG;
+  dcp_workspace_bytes(I, c_s, H, c, c_z, dtype, DCP_MONOLITHIC, nullptr, &attn);
+  char* ws = reinterpret_cast<char*>(workspace);
+  void* o = ws + align256(attn);
+  int launches = 0;
+  for (int b = 0; b < n_blocks; ++b) {
+    // A <- A + AttentionPairBias_b(A, Z): the residual rides in the output GEMM's epilogue (one rounding per block)
+    st = layer(a, z, ldz, &blocks[b], a, I, c_s, H, c, c_z, dtype, DCP_MONOLITHIC, nullptr, ws, attn, stream, a);
+    if (st == DCP_ERR_UNSUPPORTED) {   // W_o not tcgen05-shaped: layer output to scratch, then the residual kernel
+      st = layer(a, z, ldz, &blocks[b], o, I, c_s, H, c, c_z, dtype, DCP_MONOLITHIC, nullptr, ws, attn, stream);
+      if (st != DCP_OK) return st;
+      const int64_t n8 = I * c_s / 8;
+      residual_add_bf16_kernel<<<(unsigned)((n8 + 255) / 256), 256, 0, (cudaStream_t)stream>>>((__nv_bfloat16*)a, (const __nv_bfloat16*)o, n8);
+      if (cudaGetLastError() != cudaSuccess) return DCP_ERR_CUDA;
+      ++launches;
+    }
+    if (st != DCP_OK) return st;
+    launches += g_launches;
   }
   g_launches = launches;
   return DCP_OK;

@@ -240,7 +240,7 @@ cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st, bool* fold_
     if (fold_done) *fold_done = p.fold_w_b != nullptr;
     return launch_gemm_tc(p, st);
   }
-  if (p.K % 8 != 0 || p.N % 8 != 0 || p.lda % 8 != 0) return cudaErrorInvalidValue;
+  if (p.K % 8 != 0 || p.N % 8 != 0 || p.lda % 8 != 0 || p.residual != nullptr) return cudaErrorInvalidValue;   // residual: tcgen05 GEMM only
   const int64_t nb = (int64_t)p.nseg * ((p.N + BN - 1) / BN);
   if (nb * ((p.M + 127) / 128) >= 2 * 148) {   // enough 128-row tiles for two CTAs per SM
     dim3 grid((unsigned)nb, (unsigned)((p.M + 127) / 128));

@@ -162,6 +162,20 @@ __global__ void __launch_bounds__(kTcThreads, 2) gemm_tc_kernel(const __grid_con
 #pragma unroll
         for (int i = 0; i < 32; ++i) v[i] = 1.f / (1.f + expf(-v[i]));
       }
+      if (mode == GEMM_OUT_PLAIN && p.residual != nullptr && m0 + row < p.M) {
+        const uint4* rp = reinterpret_cast<const uint4*>(reinterpret_cast<const __nv_bfloat16*>(p.residual) +
+                                                         (int64_t)(m0 + row) * p.ldr + n0 + ch * 32);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const uint4 r = rp[i];                              // plain load: the buffer may be this kernel's own output
+          const uint32_t rw[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            v[8 * i + 2 * j] += __uint_as_float(rw[j] << 16);
+            v[8 * i + 2 * j + 1] += __uint_as_float(rw[j] & 0xffff0000u);
+          }
+        }
+      }
       uint4* dst = reinterpret_cast<uint4*>(Cs + row * kCsPitch + ch * 32);
 #pragma unroll
       for (int i = 0; i < 4; ++i)
@@ -232,6 +246,7 @@ bool gemm_tc_supports(const GemmMmaParams& p) {
     if ((p.mode[s] == GEMM_OUT_PLAIN || p.mode[s] == GEMM_OUT_SIGMOID) && p.ldc[s] % 8 != 0) return false;
     if (p.mode[s] == GEMM_OUT_TRANSPOSED) return false;
   }
+  if (p.residual != nullptr && (p.ldr % 8 != 0 || ((uintptr_t)p.residual & 15) != 0)) return false;
   return get_encode_fn() != nullptr;
 }
 

@@ -45,6 +45,10 @@ struct GemmMmaParams {
   void* fold_wfold;
   float *fold_c1, *fold_c0;
   int fold_c_z, fold_H, fold_H_pad;
+  // optional, GEMM_OUT_PLAIN segments of the tcgen05 GEMM only: C = bf16(acc + residual[row][col]) (fp32 add, one rounding);
+  // residual may be C itself (in place: a CTA reads its tile's residual before the barrier that precedes its stores)
+  const void* residual;
+  int64_t ldr;
   bool pdl;             // host only: launch as a programmatic dependent of the previous kernel in the stream (common.cuh)
 };
 cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st, bool* fold_done = nullptr);   // dispatches to launch_gemm_tc when it applies
