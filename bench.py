@@ -33,13 +33,29 @@ METRIC = "pair_bias_attention_gpair_per_s"
 UNIT = "Gpair/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/, named per round); None = not captured for that kernel / workload.
+# These are values of a PAST capture, not of this run: `traffic_source` in the JSON line names the capture file and the
+# commit it was taken at; the kernels stream their pair tensor exactly once in every version since.
 NCU_TRAFFIC_BYTES = {
-    # (kernel, workload): bytes   -- profiles/r01_fused_c2_ncu_full.txt, profiles/r01_fused_atom_c4_ncu_full.txt
-    ("fused_mma_kernel", "C2"): 2330531000 + 7912448,
-    ("fused_atom_kernel", "C4"): 18746721000 + 124210176,
-    # profiles/r01_pair_transition_t2_ncu_full.txt (z read once, written once)
-    ("pair_transition_kernel", "T2"): 2305023000 + 2259754000,
+    # (kernel, workload): (bytes, capture)
+    ("fused_mma_kernel", "C2"): (2330531000 + 7912448, "profiles/r01_fused_c2_ncu_full.txt (commit 8f4dd16, round 1)"),
+    ("fused_atom_kernel", "C4"): (18746721000 + 124210176, "profiles/r01_fused_atom_c4_ncu_full.txt (round 1)"),
+    ("pair_transition_kernel", "T2"): (2305023000 + 2259754000, "profiles/r01_pair_transition_t2_ncu_full.txt (round 1)"),
 }
+
+
+def ncu_traffic(kernel, workload):
+    b, src = NCU_TRAFFIC_BYTES.get((kernel, workload), (None, None))
+    return {"traffic": b, "traffic_source": src}
+
+
+def tensor_peaks():
+    """(burst, sustained) cuBLAS bf16 TFLOP/s of MEASURED_PEAKS.json (fallback: B200_PROFILING.md 1590 / 1400)."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return float(d["bf16_tflops"]), float(d["bf16_tflops_sustained"]), "measured (MEASURED_PEAKS.json, cuBLAS bf16 8192^3)"
+    return 1590.0, 1400.0, "fallback (B200_PROFILING.md)"
 
 
 def parse():
@@ -246,7 +262,8 @@ def run_ceiling(args):
     import dcp_synth as syn
     import paper_2607_05439_b200 as dcp
     dev = "cuda:0"
-    base = syn.CONFIGS["C3"]
+    atom = args.workload == "C4"          # --workload C4 --ceiling: the atom-level variant's L_max (north_star: "largest I and L")
+    base = syn.CONFIGS["C4" if atom else "C3"]
     free0, total = torch.cuda.mem_get_info()
 
     def try_alloc(I):
@@ -261,7 +278,8 @@ def run_ceiling(args):
         except torch.OutOfMemoryError:
             return None
 
-    lo, hi = base.I // 60, 32000 // 60          # lo fits (C3 itself), hi cannot (245 GB of z)
+    # lo fits (the config itself), hi cannot (C3 widths: 245 GB of z at 32000; C4 widths: 259 GB of p at 90000)
+    lo, hi = base.I // 60, (90000 if atom else 32000) // 60
     while hi - lo > 1:
         mid = (lo + hi) // 2
         got = try_alloc(60 * mid)
@@ -279,7 +297,7 @@ def run_ceiling(args):
     e0, e1 = dcp.Event(), dcp.Event()
     for k in range(2):
         e0.record()
-        dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, out=out, workspace=ws)
+        dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, out=out, workspace=ws, atom=atom)
         e1.record()
         torch.cuda.synchronize()
     ms = e0.elapsed_ms(e1)
@@ -290,13 +308,15 @@ def run_ceiling(args):
     rel = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
     mab = float(np.abs(got - ref).max())
     line = {"metric": METRIC, "unit": UNIT, "n_gpus": 1, "data": "synthetic", "dtype": "bf16",
-            "ceiling": {"I_max": I, "step": 60, "z_bytes": int(z.numel() * 2), "workspace_bytes": int(ws.numel()),
+            "config": {"workload": ("atom-level widths of C4 (c_atom=128 c_atompair=16 H=4 c=32): L_max" if atom else
+                                    "token-level widths of C3 (c_s=384 c_z=128 H=16 c=48): I_max")},
+            "ceiling": {("L_max" if atom else "I_max"): I, "step": 60, "z_bytes": int(z.numel() * 2), "workspace_bytes": int(ws.numel()),
                         "peak_device_bytes": peak_bytes, "device_total_bytes": int(total), "device_free_bytes_at_start": int(free0),
                         "ms": ms, "value": I * float(I) / (ms * 1e-3) / 1e9,
                         "hbm_frac": I * float(I) * cfg.c_z * 2 / (ms * 1e-3) / 1e9 / measured_peaks()[0],
                         "sampled_rows": len(rows), "rel_l2_vs_oracle": rel, "max_abs_vs_oracle": mab,
                         "parity_ok": bool(rel <= 1e-2 and mab <= 2e-2),
-                        "next_I_fails": 60 * hi}}
+                        ("next_L_fails" if atom else "next_I_fails"): 60 * hi}}
     print(json.dumps(line), flush=True)
 
 
@@ -408,12 +428,13 @@ def run_transition(args, rank, world, local_rank):
     kms = total_ms / args.steps
     value = n_pairs * args.steps * world / (total_ms * 1e-3) / 1e9
     flops = n_pairs * (2.0 * c_z * 4 * c_z * 2 + 2.0 * 4 * c_z * c_z)       # 393216 per pair
-    with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-        pk = json.load(f)
-    peak_tf = float(pk["bf16_tflops_sustained" if kms > 2.0 else "bf16_tflops"])
-    roofline = {"bound": "tensor", "achieved": flops / (kms * 1e-3) / 1e12, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": flops / (kms * 1e-3) / 1e12 / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(("pair_transition_kernel", args.workload)), "kernel": "pair_transition_kernel",
-                "peak_source": "measured (MEASURED_PEAKS.json, cuBLAS bf16 8192^3: sustained for a > 2 ms kernel, else burst)",
+    burst_tf, sust_tf, peak_how = tensor_peaks()
+    ach = flops / (kms * 1e-3) / 1e12
+    roofline = {"bound": "tensor", "achieved": ach, "peak": burst_tf, "unit": "TFLOP/s", "frac": ach / burst_tf,
+                "frac_burst": ach / burst_tf, "frac_sustained": ach / sust_tf, "peak_sustained": sust_tf,
+                **ncu_traffic("pair_transition_kernel", args.workload), "kernel": "pair_transition_kernel",
+                "peak_source": peak_how + ": `frac` is against the burst rate (a kernel timed alone in a short loop); the "
+                               "seconds-long sustained rate is printed beside it",
                 "kernel_ms": kms, "kernel_share_of_step": 1.0, "algorithmic_flops_per_launch": flops,
                 "hbm_bytes_per_launch": n_pairs * c_z * 2 * 2, "hbm_gbs": n_pairs * c_z * 4 / (kms * 1e-3) / 1e9}
     cpu = None
@@ -557,13 +578,13 @@ def run_stack(args, rank, world, local_rank):
     kms = k0.elapsed_ms(k1) / args.steps
     c_z = cfg.c_z
     flops = float(cfg.I) * cfg.I * (2.0 * c_z * 4 * c_z * 2 + 2.0 * 4 * c_z * c_z)
-    with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-        pk = json.load(f)
-    peak_tf = float(pk["bf16_tflops_sustained" if kms > 2.0 else "bf16_tflops"])
-    roofline = {"bound": "tensor", "achieved": flops / (kms * 1e-3) / 1e12, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": flops / (kms * 1e-3) / 1e12 / peak_tf, "traffic": NCU_TRAFFIC_BYTES.get(("pair_transition_kernel", "T2")),
+    burst_tf, sust_tf, peak_how = tensor_peaks()
+    ach = flops / (kms * 1e-3) / 1e12
+    roofline = {"bound": "tensor", "achieved": ach, "peak": burst_tf, "unit": "TFLOP/s", "frac": ach / burst_tf,
+                "frac_burst": ach / burst_tf, "frac_sustained": ach / sust_tf, "peak_sustained": sust_tf,
+                **ncu_traffic("pair_transition_kernel", "T2"),
                 "kernel": "pair_transition_kernel", "kernel_ms": kms, "kernel_share_of_step": nb * kms / step_ms,
-                "peak_source": "measured (MEASURED_PEAKS.json, cuBLAS bf16 8192^3: sustained for a > 2 ms kernel, else burst)",
+                "peak_source": peak_how + ": `frac` is against the burst rate; the sustained rate is printed beside it",
                 "algorithmic_flops_per_launch": flops, "launches_per_step": nb}
     cpu = None
     if rank == 0 and not args.no_cpu_baseline:
@@ -887,18 +908,23 @@ def run_sparse(args, rank, world, local_rank):
     pairs = float(L) * k
     value = pairs * args.steps * world / (total_ms * 1e-3) / 1e9
     kms = sum(fused_ms) / len(fused_ms)
-    # the gather kernel's bytes: every slot reads a 64-byte K slice and a 64-byte V slice per head (from L2: K and V
-    # are 12 MB), its 32-byte p row and its index; bound = L2 -> SM gather, reported against the HBM copy peak
+    # The gather kernel's bytes: every slot reads a 64-byte K slice and a 64-byte V slice per head out of L2 (K and V are
+    # 12 MB, resident), its 32-byte p row and its index.  Every query has its own key set, so this is a gather, not a
+    # stream: the bound is the L2 -> SM path, not HBM (the compulsory HBM bytes -- p_slice, idx, q, k, v, g, gated -- are
+    # 15 % of the copy bandwidth at this speed and are printed beside it).  The L2 ceiling is DERIVED, not measured on this
+    # pool: ~6300 B / cycle chip-wide (B300_MICROARCH.md "LTS throughput cap", same L2 slice count) x the SM clock.
     peak, peak_how = measured_peaks()
     gather_bytes = pairs * (2 * cfg.H * cfg.c * 2 + cfg.c_z * 2 + 4)
     hbm_bytes = pairs * (cfg.c_z * 2 + 4) + 5 * L * cfg.D * 2
-    roofline = {"bound": "hbm", "achieved": hbm_bytes / (kms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
-                "frac": hbm_bytes / (kms * 1e-3) / 1e9 / peak, "traffic": None, "kernel": "sparse_atom_kernel",
-                "peak_source": peak_how, "kernel_ms": kms, "kernel_share_of_step": kms * args.steps / total_ms,
-                "algorithmic_bytes_per_launch": hbm_bytes,
-                "l2_gather_bytes_per_launch": gather_bytes, "l2_gather_gbs": gather_bytes / (kms * 1e-3) / 1e9,
-                "note": "K / V rows are gathered from L2 (12 MB resident): the compulsory HBM bytes are p_slice + idx + "
-                        "q, k, v, g, gated; the kernel is L2-gather / issue bound, see DESIGN.md"}
+    l2_peak = 6300.0 * 1.965
+    roofline = {"bound": "l2", "achieved": gather_bytes / (kms * 1e-3) / 1e9, "peak": l2_peak, "unit": "GB/s",
+                "frac": gather_bytes / (kms * 1e-3) / 1e9 / l2_peak, "traffic": None, "kernel": "sparse_atom_rows_kernel",
+                "peak_source": "derived: 6300 B/cycle L2 throughput cap (B300_MICROARCH.md) x 1.965 GHz; not measured on this pool",
+                "kernel_ms": kms, "kernel_share_of_step": kms * args.steps / total_ms,
+                "algorithmic_bytes_per_launch": gather_bytes,
+                "hbm_bytes_per_launch": hbm_bytes, "hbm_gbs": hbm_bytes / (kms * 1e-3) / 1e9,
+                "hbm_frac": hbm_bytes / (kms * 1e-3) / 1e9 / peak, "hbm_peak_source": peak_how,
+                "note": "gather-bound: achieved = bytes the warps pull from L2 (K / V rows of the listed neighbours + p rows)"}
     cpu = None
     if rank == 0 and not args.no_cpu_baseline:
         rows = syn.sample_rows(L, args.cpu_rows or L, seed=0)     # every atom: ~2 s of oracle time
@@ -1082,7 +1108,7 @@ def main():
         if dcp.dcp_kernel_supported("mma", tdt, cfg.H, cfg.c, cfg.c_z):
             kname = "fused_mma_kernel" if cfg.H == 16 else "fused_atom_kernel"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get((kname, cfg.name)), "kernel": kname, "peak_source": peak_how,
+                **ncu_traffic(kname, cfg.name), "kernel": kname, "peak_source": peak_how,
                 "kernel_ms": fused_avg_ms, "kernel_share_of_step": fused_avg_ms * args.steps / total_ms_with_events,
                 "ms_per_step_with_kernel_events": total_ms_with_events / args.steps,
                 "algorithmic_bytes_per_launch": alg_bytes,
