@@ -602,3 +602,131 @@ def test_attention_stack_round_store_once_per_block():
         step = aso.attention_stack(step, bf(z), [w], H, c, round_store=bf)
     assert np.array_equal(a3, step)
     assert np.max(np.abs(a3 - aso.attention_stack(bf(a), bf(z), blocks, H, c))) > 0          # the rounding is really there
+
+
+# ------------------------------------------------------------------ structured neighbour budget
+def _four_chain_lattice(n_per_chain=(60, 60, 60, 60), gap=100.0):
+    """Chains = parallel lines of unit-spaced atoms along x, chain c at y = gap * c; residue = 4 consecutive atoms."""
+    xs, rid, cid = [], [], []
+    for ch, n in enumerate(n_per_chain):
+        for a in range(n):
+            xs.append((float(a), gap * ch, 0.0)); rid.append(a // 4); cid.append(ch)
+    return np.array(xs, dtype=np.float32), np.array(rid), np.array(cid)
+
+
+def test_knn_budget_reduces_to_plain_knn():
+    from oracle import knn as ko
+    from oracle import knn_budget as kb
+    rng = np.random.default_rng(91)
+    x = rng.normal(size=(70, 3)).astype(np.float32) * 3
+    rid, cid = np.arange(70) // 5, np.arange(70) // 30          # three chains: no quota
+    assert np.array_equal(kb.knn_budget(x, rid, cid, 16, n_seq=0), ko.knn(x, 16))
+    assert np.array_equal(kb.knn_budget(x, rid, np.zeros(70, int), 70, n_seq=2), ko.knn(x, 70))   # k = L: everything
+
+
+def test_knn_budget_quotas_bind_on_a_four_chain_lattice():
+    from oracle import knn_budget as kb
+    k = 48                                                       # q_out = max(32, 12) = 32, the own chain gets 16
+    x, rid, cid = _four_chain_lattice()
+    l = 30                                                       # middle of chain 0, residue 7 (atoms 28..31)
+    row = kb.knn_budget_rows(x, rid, cid, k, [l], n_seq=2)[0]
+    intra = [m for m in row if cid[m] == 0]
+    inter = [m for m in row if cid[m] != 0]
+    assert len(intra) == 16 and len(inter) == 32                 # both quotas bind (pure kNN would stay in chain 0)
+    # intra: S = residues 6..8 = atoms 24..35 (12 atoms), then the closest others: 23, 36 (d = 7, 6) -> 36 first, 23, 37, 22
+    assert sorted(intra) == [22, 23] + list(range(24, 36)) + [36, 37]
+    # inter: chain 1 is the closest foreign chain (y = 100): its 32 atoms nearest x = 30, ties by the smaller index
+    assert sorted(inter) == [60 + a for a in range(14, 46)]     # |a - 30| <= 15, and a = 14 (idx 74) wins the tie with 46
+    assert row[0] == l and len(set(row.tolist())) == k
+    d2 = ((x[row] - x[l]) ** 2).sum(1)
+    assert np.all(np.diff(d2) >= 0)                              # output ordered by distance
+    # three chains only: no split, the list is S + the closest atoms, all in chain 0
+    keep = cid < 3
+    row3 = kb.knn_budget_rows(x[keep], rid[keep], cid[keep], k, [l], n_seq=2)[0]
+    assert all(cid[m] == 0 for m in row3) and sorted(row3.tolist()) == list(range(6, 54)) or sorted(row3.tolist()) == list(range(7, 55))
+
+
+def test_knn_budget_short_chain_and_few_foreign_atoms():
+    from oracle import knn_budget as kb
+    k = 48
+    x, rid, cid = _four_chain_lattice((10, 60, 60, 60))          # own chain has 10 < q_in atoms: the others fill
+    row = kb.knn_budget_rows(x, rid, cid, k, [3], n_seq=2)[0]
+    assert sum(cid[m] == 0 for m in row) == 10 and sum(cid[m] != 0 for m in row) == 38
+    x, rid, cid = _four_chain_lattice((60, 5, 5, 5))             # 15 foreign atoms < q_out: the own chain fills
+    row = kb.knn_budget_rows(x, rid, cid, k, [30], n_seq=2)[0]
+    assert sum(cid[m] != 0 for m in row) == 15 and sum(cid[m] == 0 for m in row) == 33
+    x, rid, cid = _four_chain_lattice((20, 4, 4, 4))             # k = L
+    assert sorted(kb.knn_budget_rows(x, rid, cid, 32, [0], n_seq=2)[0].tolist()) == list(range(32))
+
+
+def test_knn_budget_sequence_local_atoms_come_first():
+    from oracle import knn_budget as kb
+    rng = np.random.default_rng(92)
+    L, k = 80, 8
+    x = rng.normal(size=(L, 3)).astype(np.float32)
+    rid, cid = np.arange(L) // 4, np.zeros(L, int)
+    x[36:40] += 1000.0                                           # residue 9, flanking residue 8 of atom 33, moved far away
+    row2 = kb.knn_budget_rows(x, rid, cid, k, [33], n_seq=2)[0]
+    assert set(range(28, 40)) >= set(row2.tolist()) and len(row2) == k     # S = residues 7..9 = 12 atoms >= k: its 8 closest
+    row1 = kb.knn_budget_rows(x, rid, cid, 16, [33], n_seq=2)[0]
+    assert set(range(28, 40)) <= set(row1.tolist())              # all of S, the far residue included, + 4 spatial ones
+    row0 = kb.knn_budget_rows(x, rid, cid, 16, [33], n_seq=1)[0]
+    assert set(range(32, 36)) <= set(row0.tolist()) and not (set(range(36, 40)) & set(row0.tolist()))
+    cid2 = cid.copy(); cid2[36:40] = 1                           # the flanking residue belongs to another chain: not local
+    assert not (set(range(36, 40)) & set(kb.knn_budget_rows(x, rid, cid2, 16, [33], n_seq=2)[0].tolist()))
+
+
+def test_knn_budget_brute_force_binary32():
+    """A second implementation: struct-rounded binary32 distances, selection by repeated extraction of the minimum."""
+    import struct
+    from oracle import knn_budget as kb
+    f32 = lambda v: struct.unpack("f", struct.pack("f", v))[0]
+    rng = np.random.default_rng(93)
+    for L, k, n_chains, n_seq in ((90, 40, 5, 2), (64, 36, 4, 1), (50, 12, 2, 2), (77, 33, 6, 0)):
+        x = (rng.integers(-6, 7, size=(L, 3)) * 0.37).astype(np.float32)      # many exact ties
+        cid = np.sort(rng.integers(0, n_chains, size=L)); rid = np.arange(L) // 3
+        got = kb.knn_budget(x, rid, cid, k, n_seq=n_seq)
+        split = len(set(cid.tolist())) > 3
+        q_out = min(max(32, k // 4), k - 1)
+        for l in range(L):
+            d2 = []
+            for m in range(L):
+                t = [f32(float(x[m, a]) - float(x[l, a])) for a in range(3)]
+                d2.append(f32(f32(f32(t[0] * t[0]) + f32(t[1] * t[1])) + f32(t[2] * t[2])))
+            pool = set(range(L))
+            def take(pred, n):
+                got_ = []
+                while len(got_) < n:
+                    cand = [m for m in pool if pred(m)]
+                    if not cand:
+                        break
+                    b = min(cand, key=lambda m: (d2[m], m)); pool.discard(b); got_.append(b)
+                return got_
+            local = lambda m: n_seq >= 1 and cid[m] == cid[l] and abs(rid[m] - rid[l]) <= n_seq - 1
+            if not split:
+                sel = take(local, k)
+                sel += take(lambda m: True, k - len(sel))
+            else:
+                out_ = take(lambda m: cid[m] != cid[l], q_out)         # the foreign quota is served first ...
+                sel = take(local, k - len(out_))                       # ... then the own chain, sequence-local atoms first
+                sel += take(lambda m: cid[m] == cid[l], k - len(out_) - len(sel))
+                sel += out_
+                sel += take(lambda m: True, k - len(sel))              # a small own chain: the others fill
+            want = sorted(sel, key=lambda m: (d2[m], m))
+            assert got[l].tolist() == want, (L, k, l)
+
+
+def test_knn_budget_invariances():
+    from oracle import knn_budget as kb
+    rng = np.random.default_rng(94)
+    L, k = 120, 40
+    x = rng.normal(size=(L, 3)).astype(np.float32) * 4
+    rid, cid = np.arange(L) // 6, np.arange(L) // 24             # five chains
+    base = kb.knn_budget(x, rid, cid, k)
+    assert np.array_equal(kb.knn_budget(x, rid, (cid * 7 + 3) % 11, k), base)          # chain labels are only labels
+    assert np.array_equal(kb.knn_budget(x, rid + 1000, cid, k), base)                  # so are residue offsets
+    xi = np.round(x * 8) / 8                                                           # exactly representable grid
+    assert np.array_equal(kb.knn_budget(xi + np.float32(16.0), rid, cid, k), kb.knn_budget(xi, rid, cid, k))
+    for l in range(L):
+        assert base[l, 0] == l and len(set(base[l].tolist())) == k
+        assert sum(cid[m] != cid[l] for m in base[l]) >= 32                            # PAPER.md:303 "at least 32"
