@@ -64,7 +64,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="native", choices=["native", "reference"])
-    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4", "K4", "T2", "T3", "P2", "D2", "D3"],
+    ap.add_argument("--workload", default="C2", choices=["C0", "C1", "C2", "C3", "C4", "S4", "K4", "B4", "T2", "T3", "P2", "D2", "D3"],
                     help="C0..C4: BASELINE.json configs (dense layer); S4: sparse k-neighbour atom attention on C4's atoms; "
                          "K4: the k-nearest-neighbour lists of C4's atoms (dcp_knn); T2 / T3: the pairwise SwiGLU transition on "
                          "C2's / C3's pair tensor (dcp_pair_transition)")
@@ -354,16 +354,22 @@ def run_reference_sparse(args):
     k = args.neighbours
     w = syn.make_weights(cfg, dev)
     a = syn.make_s(cfg, dev)
-    idx = syn.make_knn_idx(cfg, k, dev)
-    p = syn.make_p_slice(cfg, idx, dev)
+    # the reference arm runs no product code: the neighbour lists of the sampled atoms come from the oracle's own
+    # structured budget (oracle/knn_budget.py, untimed input preparation), the pair rows from the shared generator
+    from oracle import knn_budget as kbo
+    rid_, cid_, _ = syn.make_atom_topology(cfg, "cpu")
+    x_ = syn.make_atom_coords(cfg, "cpu").numpy()
     f64 = lambda t: t.detach().float().cpu().double().numpy()
     a64, w64 = f64(a), {kk: f64(v) for kk, v in w.items()}
-    n_rows = args.cpu_rows or cfg.I
+    n_rows = args.cpu_rows or 2000
     pairs = secs = 0.0
     for step in range(args.steps + min(args.warmup, 1)):
         rows = syn.sample_rows(cfg.I, n_rows, seed=step)
-        r = torch.as_tensor(rows, device=dev)
-        p_rows, i_rows = p.index_select(0, r).float().cpu().numpy(), idx.index_select(0, r).cpu().numpy()
+        idx = torch.full((cfg.I, k), -1, dtype=torch.int32)
+        idx[torch.as_tensor(rows)] = torch.from_numpy(kbo.knn_budget_rows(x_, rid_.numpy(), cid_.numpy(), k, rows))
+        p = syn.make_p_slice(cfg, idx, "cpu")
+        r = torch.as_tensor(rows)
+        p_rows, i_rows = p.index_select(0, r).float().numpy(), idx.index_select(0, r).numpy()
         t0 = time.perf_counter()
         spo.sparse_atom_attention_rows(a64, p_rows, i_rows, rows, w64, cfg.H, cfg.c)
         if step >= min(args.warmup, 1):
@@ -778,8 +784,14 @@ def run_knn(args, rank, world, local_rank):
     k, L = args.neighbours, syn.CONFIGS["C4"].I
     x = syn.make_atom_coords(cfg, dev)
     out = torch.empty(L, k, dtype=torch.int32, device=dev)
+    # --workload B4: the structured budget of PAPER.md:303 (sequence-local atoms first, inter-chain quota: 60 chains)
+    budget = args.workload == "B4"
+    from oracle import knn_budget as kbo
+    rid, cid, n_chains = syn.make_atom_topology(cfg, dev)
+    knn_call = ((lambda xx, oo: dcp.dcp_knn_budget(xx, rid, cid, k, n_chains, out=oo)) if budget
+                else (lambda xx, oo: dcp.dcp_knn(xx, k, out=oo)))
     for _ in range(max(args.warmup, 3)):
-        dcp.dcp_knn(x, k, out=out)
+        knn_call(x, out)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -789,7 +801,7 @@ def run_knn(args, rank, world, local_rank):
     e0, e1 = dcp.Event(), dcp.Event()
     e0.record()
     for _ in range(args.steps):
-        dcp.dcp_knn(x, k, out=out)
+        knn_call(x, out)
     e1.record()
     torch.cuda.synchronize()
     clocks = sampler.stop() if rank == 0 else None
@@ -803,7 +815,7 @@ def run_knn(args, rank, world, local_rank):
     peak = 148 * 128 * sm_clock_ghz / 12.0
     roofline = {"bound": "alu", "achieved": pairs / (kms * 1e-3) / 1e9, "peak": peak, "unit": "Gpair/s",
                 "frac": pairs / (kms * 1e-3) / 1e9 / peak, "traffic": None,
-                "kernel": "knn_select_kernel" if k <= 256 else "knn_kernel",
+                "kernel": "knn_budget_kernel" if budget else "knn_select_kernel" if k <= 256 else "knn_kernel",
                 "peak_source": "derived: 148 SMs x 128 FP32 lanes x 1.965 GHz / 12 instructions per candidate",
                 "kernel_ms": kms, "kernel_share_of_step": 1.0}
     cpu = None
@@ -811,7 +823,8 @@ def run_knn(args, rank, world, local_rank):
         rows = syn.sample_rows(L, args.cpu_rows or 3000, seed=0)
         xh = x.cpu().numpy()
         t0 = time.perf_counter()
-        ref = ko.knn_rows(xh, k, rows)
+        ref = (kbo.knn_budget_rows(xh, rid.cpu().numpy(), cid.cpu().numpy(), k, rows) if budget
+               else ko.knn_rows(xh, k, rows))
         dt = time.perf_counter() - t0
         got = out.index_select(0, torch.as_tensor(rows, device=dev)).cpu().numpy()
         cpu = {"value": len(rows) * float(L) / dt / 1e9, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
@@ -827,7 +840,7 @@ def run_knn(args, rank, world, local_rank):
         a.record()
         for _ in range(ne):
             xd.copy_(xh, non_blocking=True)
-            dcp.dcp_knn(xd, k, out=out)
+            knn_call(xd, out)
             oh.copy_(out, non_blocking=True)
         b.record()
         torch.cuda.synchronize()
@@ -839,9 +852,10 @@ def run_knn(args, rank, world, local_rank):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": kms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
-            "config": {"workload": f"K4: k-nearest-neighbour lists L={L} k={k} (icosahedral 60 x {cfg.n_res} synthetic atoms)",
+            "config": {"workload": (f"B4: structured neighbour budget (n_seq=2, inter-chain quota) L={L} k={k} (60 chains x {cfg.n_res} synthetic atoms)"
+                                    if budget else f"K4: k-nearest-neighbour lists L={L} k={k} (icosahedral 60 x {cfg.n_res} synthetic atoms)"),
                        "pair": "one (query atom, candidate atom) distance",
-                       "kernel": "knn_select_kernel" if k <= 256 else "knn_kernel",
+                       "kernel": "knn_budget_kernel" if budget else "knn_select_kernel" if k <= 256 else "knn_kernel",
                        "l2": "inputs (288 KB) are cache resident by nature; nothing to flush",
                        "parallelism": "replicas only" if world > 1 else "single GPU",
                        "peak_device_bytes": int(torch.cuda.max_memory_allocated())},
@@ -872,7 +886,8 @@ def run_sparse(args, rank, world, local_rank):
     k = args.neighbours
     w = syn.make_weights(cfg, dev)
     a = syn.make_s(cfg, dev)
-    idx = syn.make_knn_idx(cfg, k, dev)
+    rid_, cid_, nch_ = syn.make_atom_topology(cfg, dev)
+    idx = dcp.dcp_knn_budget(syn.make_atom_coords(cfg, dev), rid_, cid_, min(k, cfg.I), nch_)   # the structured budget
     p = syn.make_p_slice(cfg, idx, dev)
     L = cfg.I
     ws = torch.empty(dcp.dcp_sparse_atom_workspace_bytes(L, cfg.c_s, cfg.H, cfg.c, a.dtype), dtype=torch.uint8, device=dev)
@@ -1000,7 +1015,7 @@ def main():
     if args.workload == "S4":
         run_sparse(args, rank, world, local_rank)
         return
-    if args.workload == "K4":
+    if args.workload in ("K4", "B4"):
         run_knn(args, rank, world, local_rank)
         return
     if args.workload in ("T2", "T3"):

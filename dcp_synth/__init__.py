@@ -218,18 +218,16 @@ def make_atom_coords(cfg: LayerConfig, device="cpu") -> torch.Tensor:
     return torch.cat(out, dim=0).to(device).contiguous()
 
 
-def make_knn_idx(cfg: LayerConfig, k: int, device="cpu", chunk: int = 2048) -> torch.Tensor:
-    """Neighbour lists idx [L, k] int32: the k spatially closest atoms of each query atom (itself included), from
-    make_atom_coords by a chunked distance matrix + top-k.  Stands in for the paper's budget of sequence-local plus
-    spatially closest atoms; k = min(k, L)."""
-    x = make_atom_coords(cfg, device)
-    L = x.shape[0]
-    k = min(k, L)
-    idx = torch.empty(L, k, dtype=torch.int32, device=device)
-    for i0 in range(0, L, chunk):
-        d = torch.cdist(x[i0:i0 + chunk], x)
-        idx[i0:i0 + chunk] = torch.topk(d, k, dim=1, largest=False).indices.to(torch.int32)
-    return idx.contiguous()
+def make_atom_topology(cfg: LayerConfig, device="cpu", atoms_per_residue: int = 8):
+    """(residue_id, chain_id, n_chains): the [L] int32 token and chain assignments of the synthetic assembly (the inputs
+    PAPER.md:454 names) -- every ASU copy is one chain, `atoms_per_residue` consecutive atoms form a residue, residue ids
+    run on across chains (global token index).  Unstructured configs: one chain."""
+    L = cfg.I
+    a = torch.arange(L, dtype=torch.int32)
+    n = cfg.n_res if cfg.structured else L
+    residue_id = (a // atoms_per_residue).to(torch.int32)
+    chain_id = (a // n).to(torch.int32) if cfg.structured else torch.zeros(L, dtype=torch.int32)
+    return residue_id.to(device).contiguous(), chain_id.to(device).contiguous(), (cfg.copies if cfg.structured else 1)
 
 
 def make_p_slice(cfg: LayerConfig, idx: torch.Tensor, device="cpu", noise: float = 0.1, chunk: int = 4096) -> torch.Tensor:

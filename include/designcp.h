@@ -194,9 +194,24 @@ dcp_status dcp_gather_pair_slice(const void *p, int64_t ldp, const int32_t *idx,
  * without the [L, L] matrix).  x [L, 3] fp32 device; idx [L, k] int32 device: the k atoms with the smallest squared
  * Euclidean distance to atom l (itself included), ordered by (distance, atom index) ascending -- unique, and
  * bit-exact against the oracle: distances in binary32, t = x_m - x_l, d2 = (t0 t0 + t1 t1) + t2 t2, no FMA.
- * 1 <= k <= min(L, 512) (DCP_ERR_INVALID_ARG / DCP_ERR_UNSUPPORTED otherwise).  The paper's sequence-local and
- * inter-chain quotas are not part of this call. */
+ * 1 <= k <= min(L, 512) (DCP_ERR_INVALID_ARG / DCP_ERR_UNSUPPORTED otherwise).  Pure spatial top-k: the paper's
+ * sequence-local and inter-chain quotas are dcp_knn_budget below. */
 dcp_status dcp_knn(const float *x, int32_t *idx, int64_t L, int k, void *stream);
+
+/* The STRUCTURED neighbour budget: "a fixed number n_seq of per-residue sequence-local neighbours
+ * (default n_seq = 2, namely the query atom plus its immediate flanking residues' atoms), and the spatially closest
+ * atoms beyond those, until the per-query budget k ... is filled ... When the input is a multi-chain assembly with more
+ * than three chains, the budget is split into an intra-chain quota of k - max(32, k/4) neighbours and an inter-chain
+ * quota of at least 32 neighbours".  Inputs as PAPER.md:454 names them: x [L, 3] fp32, residue_id [L] and chain_id [L]
+ * int32 (device).  Readings (#26): closest = smallest (binary32 squared distance as in dcp_knn, atom index);
+ * sequence-local = same chain and |residue_id difference| <= n_seq - 1 (n_seq = 0: none), taken first; with
+ * n_chains > 3 the min(max(32, k/4), k - 1) closest atoms of OTHER chains are served first, the own chain gets the
+ * rest (sequence-local atoms first), and whatever one side cannot fill goes to the other.  n_chains = the number of
+ * distinct values in chain_id (the caller knows it; only "> 3" matters).  idx [L, k]: the selected atoms by
+ * (distance, index) ascending, the query itself included; bit-exact against oracle/knn_budget.py.
+ * 1 <= k <= min(L, 512), n_seq >= 0 (DCP_ERR_INVALID_ARG / DCP_ERR_UNSUPPORTED otherwise). */
+dcp_status dcp_knn_budget(const float *x, const int32_t *residue_id, const int32_t *chain_id, int32_t *idx, int64_t L,
+                          int k, int n_seq, int n_chains, void *stream);
 
 /* End-to-end entry with HOST inputs/outputs: s_host, z_host, out_host are HOST pointers (pinned memory gives
  * full PCIe rate); weights stay device-resident (they are parameters, not per-step inputs).  Copies s and z

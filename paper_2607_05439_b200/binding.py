@@ -28,7 +28,7 @@ KERNEL = {"auto": DCP_KERNEL_AUTO, "generic": DCP_KERNEL_GENERIC, "mma": DCP_KER
 EXPORTS = [
     "dcp_workspace_bytes", "dcp_pair_bias_attention", "dcp_atom_pair_bias_attention",
     "dcp_pair_bias_attention_host", "dcp_partial_states", "dcp_merge_states", "dcp_shard_range",
-    "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention", "dcp_knn", "dcp_gather_pair_slice",
+    "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention", "dcp_knn", "dcp_knn_budget", "dcp_gather_pair_slice",
     "dcp_pair_transition_workspace_bytes", "dcp_pair_transition",
     "dcp_pairformer_stack_workspace_bytes", "dcp_pairformer_stack",
     "dcp_attention_stack_workspace_bytes", "dcp_attention_stack",
@@ -101,7 +101,8 @@ def _load() -> C.CDLL:
     lib.dcp_pairformer_stack.argtypes = [vp, vp, C.POINTER(dcp_block_weights), i32, i64, i32, i32, i32, i32, i32, vp, sz, vp]
     lib.dcp_attention_stack_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, i32, C.POINTER(sz)]
     lib.dcp_attention_stack.argtypes = [vp, vp, i64, C.POINTER(dcp_weights), i32, i64, i32, i32, i32, i32, i32, vp, sz, vp]
-    for n in EXPORTS[:17]:
+    lib.dcp_knn_budget.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, vp]
+    for n in EXPORTS[:18]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -335,6 +336,20 @@ def dcp_knn(x, k, out=None, stream=None):
     if out is None:
         out = torch.empty(L, k, dtype=torch.int32, device=x.device)
     _check(_lib.dcp_knn(_ptr(x), _ptr(out), L, int(k), _stream_ptr(stream)), "dcp_knn")
+    return out
+
+
+def dcp_knn_budget(x, residue_id, chain_id, k, n_chains, n_seq=2, out=None, stream=None):
+    """idx [L, k] int32: the structured neighbour budget of PAPER.md:303 (sequence-local atoms first, spatial fill,
+    inter-chain quota when n_chains > 3).  residue_id, chain_id: [L] int32 device; n_chains: distinct chain ids."""
+    assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous() and x.shape[1] == 3
+    for t in (residue_id, chain_id):
+        assert t.is_cuda and t.dtype == torch.int32 and t.is_contiguous() and t.shape[0] == x.shape[0]
+    L = x.shape[0]
+    if out is None:
+        out = torch.empty(L, k, dtype=torch.int32, device=x.device)
+    _check(_lib.dcp_knn_budget(_ptr(x), _ptr(residue_id), _ptr(chain_id), _ptr(out), L, int(k), int(n_seq), int(n_chains),
+                               _stream_ptr(stream)), "dcp_knn_budget")
     return out
 
 

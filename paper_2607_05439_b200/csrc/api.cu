@@ -626,6 +626,15 @@ dcp_status dcp_knn(const float* x, int32_t* idx, int64_t L, int k, void* stream)
   return DCP_OK;
 }
 
+dcp_status dcp_knn_budget(const float* x, const int32_t* residue_id, const int32_t* chain_id, int32_t* idx, int64_t L, int k,
+                          int n_seq, int n_chains, void* stream) {
+  g_launches = 0;
+  if (!x || !residue_id || !chain_id || !idx || L <= 0 || k <= 0 || k > L || n_seq < 0 || n_chains < 1) return DCP_ERR_INVALID_ARG;
+  if (!knn_supports(L, k)) return DCP_ERR_UNSUPPORTED;
+  DCP_CUDA(launch_knn_budget(x, residue_id, chain_id, idx, L, k, n_seq, n_chains, (cudaStream_t)stream));
+  return DCP_OK;
+}
+
 dcp_status dcp_pair_bias_attention_host(const void* s_host, const void* z_host, const dcp_weights* w, void* out_host,
                                         void* s_dev, void* z_dev, void* out_dev, int64_t I, int c_s, int H, int c,
                                         int c_z, dcp_dtype dtype, dcp_decomp decomp, const dcp_plan* plan,

@@ -108,6 +108,9 @@ cudaError_t launch_gather_pair_slice(const void* P, int64_t ldp_bytes, const int
 // k nearest neighbours of every atom (knn.cu): x [L][3] fp32 -> idx [L][k], ordered by (d2, index)
 bool knn_supports(int64_t L, int k);
 cudaError_t launch_knn(const float* x, int32_t* idx, int64_t L, int k, cudaStream_t st);
+// the structured budget: sequence-local atoms first, inter-chain quota when n_chains > 3
+cudaError_t launch_knn_budget(const float* x, const int32_t* residue_id, const int32_t* chain_id, int32_t* idx, int64_t L, int k,
+                              int n_seq, int n_chains, cudaStream_t st);
 
 // Pairwise SwiGLU transition z <- z + W3 (SiLU(W1 LN z) (.) W2 LN z) (pair_transition.cu)
 bool pair_transition_supports(dcp_dtype dt, int c_z);

@@ -309,7 +309,179 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
   for (int j = lane; j < k; j += 32) idx[(int64_t)l * k + j] = bi[j];
 }
 
+// ---- structured neighbour budget (reading 26; oracle/knn_budget.py)
+// One warp per query, the insertion scan of knn_kernel with TWO sorted register lists: the own chain (class A; with at
+// most three chains: every atom) ordered by (not sequence-local, d2, index) -- the flag rides in bit 31 of the
+// non-negative distance's bit pattern, so sequence-local atoms come first -- and the other chains (class B) ordered by
+// (d2, index).  After the scan the quotas are arithmetic on the class sizes; the chosen prefixes of the two lists are
+// sorted together by (d2, index) in shared memory (bitonic) and written out.
+template <int NR>
+struct TopList {
+  unsigned key[NR];
+  int li[NR];
+  unsigned tau;
+  int tau_i;
+  int last_lane, last_r;
+  __device__ __forceinline__ void init(int cap) {
+#pragma unroll
+    for (int r = 0; r < NR; ++r) { key[r] = 0xffffffffu; li[r] = 0x7fffffff; }
+    tau = 0xffffffffu; tau_i = 0x7fffffff;
+    last_lane = (cap - 1) / NR; last_r = (cap - 1) % NR;
+  }
+  __device__ __forceinline__ bool beats(unsigned kk, int m) const { return kk < tau || (kk == tau && m < tau_i); }
+  // insert the candidates of `mask` (lane b holds key kk of atom c0 + b), in increasing index
+  __device__ __forceinline__ void insert_chunk(int c0, unsigned kk, unsigned mask, int lane) {
+    while (mask) {
+      const int b = __ffs(mask) - 1;
+      mask &= mask - 1;
+      const unsigned kn = __shfl_sync(0xffffffffu, kk, b);
+      const int mn = c0 + b;
+      if (!beats(kn, mn)) continue;                            // the last entry moved meanwhile (warp-uniform)
+      int pos = 0;
+#pragma unroll
+      for (int r = 0; r < NR; ++r) pos += __popc(__ballot_sync(0xffffffffu, key[r] < kn || (key[r] == kn && li[r] < mn)));
+      const int pl = pos / NR, pr = pos % NR;
+      const unsigned up_k = __shfl_up_sync(0xffffffffu, key[NR - 1], 1);
+      const int up_i = __shfl_up_sync(0xffffffffu, li[NR - 1], 1);
+      if (lane > pl) {
+#pragma unroll
+        for (int r = NR - 1; r > 0; --r) { key[r] = key[r - 1]; li[r] = li[r - 1]; }
+        key[0] = up_k; li[0] = up_i;
+      } else if (lane == pl) {
+#pragma unroll
+        for (int r = NR - 1; r > 0; --r)
+          if (r > pr) { key[r] = key[r - 1]; li[r] = li[r - 1]; }
+#pragma unroll
+        for (int r = 0; r < NR; ++r)
+          if (r == pr) { key[r] = kn; li[r] = mn; }
+      }
+      unsigned tk = key[0];
+      int ti = li[0];
+#pragma unroll
+      for (int r = 1; r < NR; ++r) { tk = r == last_r ? key[r] : tk; ti = r == last_r ? li[r] : ti; }
+      tau = __shfl_sync(0xffffffffu, tk, last_lane);
+      tau_i = __shfl_sync(0xffffffffu, ti, last_lane);
+    }
+  }
+};
+
+template <int NR>
+__global__ void __launch_bounds__(256) knn_budget_kernel(const float* __restrict__ x, const int32_t* __restrict__ rid,
+                                                         const int32_t* __restrict__ cid, int32_t* __restrict__ idx, int L, int k,
+                                                         int n_seq, int split, int q_out) {
+  extern __shared__ float smem_knn[];
+  float* sx = smem_knn;
+  float* sy = sx + kTile;
+  float* sz = sy + kTile;
+  int* sr = reinterpret_cast<int*>(sz + kTile);
+  int* sc = sr + kTile;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  unsigned* bk = reinterpret_cast<unsigned*>(sc + kTile) + wib * (2 * 512);   // per-warp sort buffer: 512 keys, 512 indices
+  int* bi = reinterpret_cast<int*>(bk + 512);
+  const int lq = blockIdx.x * 8 + wib;
+  const bool active = lq < L;
+  const int l = active ? lq : L - 1;
+  const float q0 = __ldg(x + 3 * (int64_t)l), q1 = __ldg(x + 3 * (int64_t)l + 1), q2 = __ldg(x + 3 * (int64_t)l + 2);
+  const int qr = __ldg(rid + l), qc = __ldg(cid + l), win = n_seq - 1;
+  TopList<NR> la, lb;
+  la.init(k);
+  lb.init(k);
+  int cnt_a = 0, cnt_b = 0;
+  const int n_tiles = (L + kTile - 1) / kTile;
+  const int own = (blockIdx.x * 8) / kTile;
+  for (int tt = 0; tt < n_tiles; ++tt) {
+    const int tile = tt == 0 ? own : (tt <= own ? tt - 1 : tt);
+    const int t0 = tile * kTile;
+    __syncthreads();
+    for (int e = threadIdx.x; e < kTile; e += blockDim.x) {
+      const int m = t0 + e;
+      sx[e] = m < L ? __ldg(x + 3 * (int64_t)m) : 0.f;
+      sy[e] = m < L ? __ldg(x + 3 * (int64_t)m + 1) : 0.f;
+      sz[e] = m < L ? __ldg(x + 3 * (int64_t)m + 2) : 0.f;
+      sr[e] = m < L ? __ldg(rid + m) : 0;
+      sc[e] = m < L ? __ldg(cid + m) : -1;
+    }
+    __syncthreads();
+    if (!active) continue;
+    const int n_here = (L - t0 < kTile ? L - t0 : kTile);
+    for (int c0 = 0; c0 < n_here; c0 += 32) {
+      const int e = c0 + lane;
+      const bool valid = e < n_here;
+      const float a0 = __fsub_rn(sx[e & (kTile - 1)], q0), a1 = __fsub_rn(sy[e & (kTile - 1)], q1), a2 = __fsub_rn(sz[e & (kTile - 1)], q2);
+      const unsigned db = __float_as_uint(__fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2)));
+      const bool same = sc[e & (kTile - 1)] == qc;
+      int dr = sr[e & (kTile - 1)] - qr;
+      dr = dr < 0 ? -dr : dr;
+      const bool local = same && dr <= win;
+      const bool in_a = valid && (same || !split);
+      const bool in_b = valid && !same && split;
+      const unsigned ka = db | (local ? 0u : 0x80000000u);
+      const int m = t0 + e;
+      cnt_a += __popc(__ballot_sync(0xffffffffu, in_a));
+      cnt_b += __popc(__ballot_sync(0xffffffffu, in_b));
+      const unsigned mka = __ballot_sync(0xffffffffu, in_a && la.beats(ka, m));
+      const unsigned mkb = __ballot_sync(0xffffffffu, in_b && lb.beats(db, m));
+      if (mka) la.insert_chunk(t0 + c0, ka, mka, lane);
+      if (mkb) lb.insert_chunk(t0 + c0, db, mkb, lane);
+    }
+  }
+  if (!active) return;
+  // quotas (oracle/knn_budget.py): the foreign quota first, the own chain gets the rest, leftovers go back
+  int n_out = cnt_b < q_out ? cnt_b : q_out;
+  const int n_in = cnt_a < k - n_out ? cnt_a : k - n_out;
+  n_out = cnt_b < k - n_in ? cnt_b : k - n_in;
+  int P = 32;
+  while (P < k) P <<= 1;
+  for (int e = lane; e < P; e += 32) { bk[e] = 0xffffffffu; bi[e] = 0x7fffffff; }
+  __syncwarp();
+#pragma unroll
+  for (int r = 0; r < NR; ++r) {
+    const int pos = lane * NR + r;
+    if (pos < n_in) { bk[pos] = la.key[r] & 0x7fffffffu; bi[pos] = la.li[r]; }
+    if (pos < n_out) { bk[n_in + pos] = lb.key[r]; bi[n_in + pos] = lb.li[r]; }
+  }
+  __syncwarp();
+  for (int size = 2; size <= P; size <<= 1) {
+    for (int stride = size >> 1; stride > 0; stride >>= 1) {
+      for (int i = lane; i < (P >> 1); i += 32) {
+        const int pos = 2 * i - (i & (stride - 1));
+        const int par = pos + stride;
+        const bool asc = (pos & size) == 0;
+        const unsigned da = bk[pos], dbb = bk[par];
+        const int ia = bi[pos], ib = bi[par];
+        const bool a_after_b = da > dbb || (da == dbb && ia > ib);
+        if (a_after_b == asc) { bk[pos] = dbb; bk[par] = da; bi[pos] = ib; bi[par] = ia; }
+      }
+      __syncwarp();
+    }
+  }
+  for (int j = lane; j < k; j += 32) idx[(int64_t)l * k + j] = bi[j];
+}
+
+template <int NR>
+cudaError_t launch_budget(const float* x, const int32_t* rid, const int32_t* cid, int32_t* idx, int L, int k, int n_seq, int split,
+                          int q_out, cudaStream_t st) {
+  const size_t smem = (size_t)(5 * kTile + 8 * 2 * 512) * 4;
+  cudaError_t e = cudaFuncSetAttribute(knn_budget_kernel<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  knn_budget_kernel<NR><<<(unsigned)((L + 7) / 8), 256, smem, st>>>(x, rid, cid, idx, L, k, n_seq, split, q_out);
+  return cudaGetLastError();
+}
+
 }  // namespace
+
+cudaError_t launch_knn_budget(const float* x, const int32_t* rid, const int32_t* cid, int32_t* idx, int64_t L, int k, int n_seq,
+                              int n_chains, cudaStream_t st) {
+  const int split = n_chains > 3 ? 1 : 0;
+  int q_out = k / 4 > 32 ? k / 4 : 32;
+  if (q_out > k - 1) q_out = k - 1;
+  const int nr = (k + 31) / 32;
+  if (nr <= 1) return launch_budget<1>(x, rid, cid, idx, (int)L, k, n_seq, split, q_out, st);
+  if (nr <= 2) return launch_budget<2>(x, rid, cid, idx, (int)L, k, n_seq, split, q_out, st);
+  if (nr <= 4) return launch_budget<4>(x, rid, cid, idx, (int)L, k, n_seq, split, q_out, st);
+  if (nr <= 8) return launch_budget<8>(x, rid, cid, idx, (int)L, k, n_seq, split, q_out, st);
+  return launch_budget<16>(x, rid, cid, idx, (int)L, k, n_seq, split, q_out, st);
+}
 
 bool knn_supports(int64_t L, int k) { return L >= 1 && L <= 0x7fffffff && k >= 1 && k <= 512 && k <= L; }
 

@@ -1,10 +1,12 @@
-"""GPU parity of dcp_knn against the oracle: index work, so BIT-EXACT."""
+"""GPU parity of dcp_knn and dcp_knn_budget against their oracles: index
+work, so BIT-EXACT."""
 import numpy as np
 import pytest
 import torch
 
 import dcp_synth as syn
 from oracle import knn as ko
+from oracle import knn_budget as kbo
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda:0"
@@ -46,8 +48,7 @@ def test_knn_dense_cluster_takes_the_exact_fallback():
 
 
 def test_knn_structured_atoms_sampled_rows():
-    """C4's synthetic assembly (L = 24000), k = 128: sampled queries against the oracle, and against the torch
-    cdist + topk lists the input generator builds (same sets wherever no near-tie decides)."""
+    """C4's synthetic assembly (L = 24000), k = 128: sampled queries against the oracle."""
     dcp = _dcp()
     cfg = syn.CONFIGS["C4"]
     x = syn.make_atom_coords(cfg, DEV)
@@ -71,3 +72,83 @@ def test_knn_error_paths():
     with pytest.raises(dcp.DcpError) as e:
         dcp.dcp_knn(xl, 513)
     assert e.value.status == 2
+
+
+# ------------------------------------------------------------------ the structured budget
+def _topology(L, n_chains, atoms_per_residue, seed):
+    g = torch.Generator(device="cpu").manual_seed(seed)
+    cid = torch.sort(torch.randint(0, n_chains, (L,), generator=g)).values.to(torch.int32)
+    rid = (torch.arange(L) // atoms_per_residue).to(torch.int32)
+    return rid, cid, int(torch.unique(cid).numel())
+
+
+@pytest.mark.parametrize("L,k,n_chains,apr,n_seq", [
+    (300, 128, 6, 8, 2),      # the paper's defaults: k = 128, n_seq = 2, more than three chains: both quotas live
+    (300, 128, 3, 8, 2),      # three chains: no split
+    (200, 48, 5, 4, 2),       # q_out = 32 of 48
+    (150, 33, 4, 5, 1),       # own residue only
+    (257, 40, 7, 3, 0),       # no sequence-local atoms
+    (90, 8, 5, 6, 2),         # the sequence-local set alone exceeds k; q_out = k - 1
+    (64, 64, 4, 4, 2),        # k = L
+    (700, 300, 9, 10, 2),     # NR = 16 lists
+    (1000, 512, 5, 8, 2),     # the largest budget
+    (40, 1, 4, 4, 2),         # k = 1: the query itself
+])
+def test_knn_budget_bit_exact(L, k, n_chains, apr, n_seq):
+    dcp = _dcp()
+    g = torch.Generator(device="cpu").manual_seed(2000 + L + k)
+    x = (torch.randn(L, 3, generator=g) * 6)
+    rid, cid, nch = _topology(L, n_chains, apr, L + k)
+    got = dcp.dcp_knn_budget(x.to(DEV), rid.to(DEV), cid.to(DEV), k, nch, n_seq=n_seq).cpu().numpy()
+    ref = kbo.knn_budget(x.numpy(), rid.numpy(), cid.numpy(), k, n_seq=n_seq)
+    assert np.array_equal(got, ref)
+
+
+def test_knn_budget_ties_and_short_chains():
+    """Integer lattice (exact ties everywhere), one chain of 5 atoms and one of 2 among six: order = (distance, index)."""
+    dcp = _dcp()
+    g = torch.Generator(device="cpu").manual_seed(9)
+    L = 400
+    x = torch.randint(0, 4, (L, 3), generator=g).float()
+    cid = torch.cat([torch.full((5,), 0), torch.full((2,), 1), torch.full((150,), 2), torch.full((100,), 3),
+                     torch.full((100,), 4), torch.full((43,), 5)]).to(torch.int32)
+    rid = (torch.arange(L) // 7).to(torch.int32)
+    for k, n_seq in ((96, 2), (40, 1), (400, 2)):
+        got = dcp.dcp_knn_budget(x.to(DEV), rid.to(DEV), cid.to(DEV), k, 6, n_seq=n_seq).cpu().numpy()
+        assert np.array_equal(got, kbo.knn_budget(x.numpy(), rid.numpy(), cid.numpy(), k, n_seq=n_seq))
+
+
+def test_knn_budget_reduces_to_plain_knn_on_the_device():
+    dcp = _dcp()
+    g = torch.Generator(device="cpu").manual_seed(4)
+    x = (torch.randn(500, 3, generator=g) * 5).to(DEV)
+    rid = (torch.arange(500) // 8).to(torch.int32).to(DEV)
+    cid = (torch.arange(500) // 200).to(torch.int32).to(DEV)          # three chains
+    assert torch.equal(dcp.dcp_knn_budget(x, rid, cid, 100, 3, n_seq=0), dcp.dcp_knn(x, 100))
+
+
+def test_knn_budget_structured_atoms_sampled_rows():
+    """C4's synthetic assembly (L = 24000: 60 chains of 400 atoms, 8 atoms per residue), the paper's k = 128, n_seq = 2:
+    sampled queries bit-exact against the oracle; every list keeps >= 32 atoms of other chains."""
+    dcp = _dcp()
+    cfg = syn.CONFIGS["C4"]
+    x = syn.make_atom_coords(cfg, DEV)
+    rid, cid, nch = syn.make_atom_topology(cfg, DEV)
+    got = dcp.dcp_knn_budget(x, rid, cid, 128, nch)
+    rows = syn.sample_rows(cfg.I, 300, boundaries=[400, 12000], seed=2)
+    ref = kbo.knn_budget_rows(x.cpu().numpy(), rid.cpu().numpy(), cid.cpu().numpy(), 128, rows)
+    assert np.array_equal(got[torch.as_tensor(rows, device=DEV)].cpu().numpy(), ref)
+    foreign = (cid[got.long()] != cid[:, None]).sum(dim=1)
+    assert int(foreign.min()) >= 32
+    assert torch.equal(got[:, 0].cpu(), torch.arange(cfg.I, dtype=torch.int32))
+    assert torch.equal(got, dcp.dcp_knn_budget(x, rid, cid, 128, nch))
+
+
+def test_knn_budget_error_paths():
+    dcp = _dcp()
+    x = torch.zeros(10, 3, device=DEV)
+    z = torch.zeros(10, dtype=torch.int32, device=DEV)
+    for k, n_seq, nch in ((0, 2, 1), (11, 2, 1), (4, -1, 1), (4, 2, 0)):
+        with pytest.raises(dcp.DcpError) as e:
+            dcp.dcp_knn_budget(x, z, z, k, nch, n_seq=n_seq)
+        assert e.value.status == 1

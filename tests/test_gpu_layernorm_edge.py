@@ -69,7 +69,7 @@ def test_sparse_affine_shifted_pairs(H, a, t):
     L, k = 200, 96
     cfg = syn.small_config("lnsp", I=L, c_s=64, c_z=16, H=H, c=32, dtype="bf16", seed=int(a * 10 + t))
     w, x = syn.make_weights(cfg, DEV), syn.make_s(cfg, DEV)
-    idx = syn.make_knn_idx(cfg, k, DEV)
+    idx = util.neighbour_lists(cfg, k, DEV)
     p = syn.affine_pairs(syn.make_p_slice(cfg, idx, DEV), a, t, seed=int(t) + 1, n_const=60)
     ref = spo.sparse_atom_attention_rows(util.np64(x), util.np32(p), idx.cpu().numpy(), list(range(L)), util.weights_np(w),
                                          cfg.H, cfg.c)

@@ -22,7 +22,7 @@ def _problem(L, k, H=4, c_atom=128, seed=11, structured=False, copies=60, ln_s=F
                            copies=copies)
     w = syn.make_weights(cfg, DEV, with_ln_s=ln_s, with_b_q=b_q)
     a = syn.make_s(cfg, DEV)
-    idx = syn.make_knn_idx(cfg, k, DEV)
+    idx = util.neighbour_lists(cfg, k, DEV)
     p = syn.make_p_slice(cfg, idx, DEV)
     return cfg, a, p, idx, w
 
@@ -130,7 +130,7 @@ def test_sparse_c4_sampled_rows():
     cfg = syn.CONFIGS["C4"]
     w = syn.make_weights(cfg, DEV)
     a = syn.make_s(cfg, DEV)
-    idx = syn.make_knn_idx(cfg, 128, DEV)
+    idx = util.neighbour_lists(cfg, 128, DEV)
     p = syn.make_p_slice(cfg, idx, DEV)
     out = dcp.dcp_sparse_atom_attention(a, p, idx, w, cfg.H, cfg.c)
     rows = syn.sample_rows(cfg.I, 200, boundaries=[400, 12000], seed=1)

@@ -50,3 +50,13 @@ def check_close(out: torch.Tensor, ref: np.ndarray, dtype: str, what: str = ""):
         assert rel <= TOL_BF16_RELL2, f"{what}: rel-L2 {rel:.3e} > {TOL_BF16_RELL2}"
         assert maxabs <= TOL_BF16_MAXABS, f"{what}: max-abs {maxabs:.3e} > {TOL_BF16_MAXABS}"
     return maxabs, rel
+
+
+def neighbour_lists(cfg, k, device):
+    """Neighbour lists [L, k] int32 for the sparse-attention tests: the structured budget of the synthetic
+    assembly's coordinates, built by the library's own dcp_knn_budget (itself bit-exact against oracle/knn_budget.py,
+    tests/test_gpu_knn.py).  They are INPUTS of the attention under test: its oracle receives the same lists."""
+    import paper_2607_05439_b200 as dcp
+    x = syn.make_atom_coords(cfg, device)
+    rid, cid, n_chains = syn.make_atom_topology(cfg, device)
+    return dcp.dcp_knn_budget(x, rid, cid, min(k, cfg.I), n_chains)
