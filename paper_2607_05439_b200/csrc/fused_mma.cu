@@ -258,8 +258,33 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     const uint4* vfr = reinterpret_cast<const uint4*>(p.vfr);
     int bbuf = 0;
     uint32_t bphase = 0;
+    // K / V fragments of (key tile j, head h) are read from L2 into the registers the previous block just released:
+    // K right after the last QK^T MMA that used it, V right after the last PV MMA (software pipelining, no extra
+    // registers).  Both live in MMA B-fragment order (gemm_mma.cu), so every load is one coalesced 128-bit access per
+    // lane: K k-step kk -> (n-block A, n-block B) fragments, V n-block pair ndp -> fragments of nd = 2 ndp, 2 ndp + 1.
+    // key of S column: n-block A col c <-> j + 4*(c/2) + c%2, n-block B col c <-> that + 2
+    constexpr int NDP = CP / 16;
+    uint4 kq[KK], vq[NDP];
+    auto load_k = [&](int j, int h) {
+      const uint4* src = kfr + ((int64_t)((j >> 4) * kH + h) * KK) * 32 + lane;
+#pragma unroll
+      for (int kk = 0; kk < KK; ++kk) kq[kk] = __ldg(src + kk * 32);
+    };
+    auto load_v = [&](int j, int h) {
+      const uint4* src = vfr + ((int64_t)((j >> 4) * kH + h) * NDP) * 32 + lane;
+#pragma unroll
+      for (int ndp = 0; ndp < NDP; ++ndp) vq[ndp] = __ldg(src + ndp * 32);
+    };
+    // The first K / V tile of a unit is requested during the last tile of the previous one (the slot that would re-read
+    // the tile itself), so a unit change costs one L2 round trip (the Q tile) instead of two.
+    if ((int)blockIdx.x < n_units) {
+      const Unit u0 = decode_unit<kTileQ, kTileK>(p, blockIdx.x);
+      load_k(u0.ks & ~(kTileK - 1), 2 * aw);
+      load_v(u0.ks & ~(kTileK - 1), 2 * aw);
+    }
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
       const Unit un = decode_unit<kTileQ, kTileK>(p, u);
+      const int next_first = u + (int)gridDim.x < n_units ? (decode_unit<kTileQ, kTileK>(p, u + gridDim.x).ks & ~(kTileK - 1)) : -1;
       // Q tile -> shared memory (rows of the tile, all heads), shared by the 8 attention warps; row pitch padded so the
       // per-thread 64-bit fragment loads are conflict-free.  Named barrier 1 = the 256 attention threads.
       constexpr int kQP = q_pitch(CP);
@@ -302,29 +327,11 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             for (int x = 0; x < 4; ++x) o[hh][mb][nd][x] = 0.f;
         }
 
-      // K / V fragments of (key tile j, head h) are read from L2 into the registers the previous block just released:
-      // K right after the last QK^T MMA that used it, V right after the last PV MMA (software pipelining, no extra
-      // registers).  Both live in MMA B-fragment order (gemm_mma.cu), so every load is one coalesced 128-bit access per
-      // lane: K k-step kk -> (n-block A, n-block B) fragments, V n-block pair ndp -> fragments of nd = 2 ndp, 2 ndp + 1.
-      // key of S column: n-block A col c <-> j + 4*(c/2) + c%2, n-block B col c <-> that + 2
-      constexpr int NDP = CP / 16;
-      uint4 kq[KK], vq[NDP];
-      auto load_k = [&](int j, int h) {
-        const uint4* src = kfr + ((int64_t)((j >> 4) * kH + h) * KK) * 32 + lane;
-#pragma unroll
-        for (int kk = 0; kk < KK; ++kk) kq[kk] = __ldg(src + kk * 32);
-      };
-      auto load_v = [&](int j, int h) {
-        const uint4* src = vfr + ((int64_t)((j >> 4) * kH + h) * NDP) * 32 + lane;
-#pragma unroll
-        for (int ndp = 0; ndp < NDP; ++ndp) vq[ndp] = __ldg(src + ndp * 32);
-      };
-      load_k(un.ks & ~(kTileK - 1), 2 * aw);
-      load_v(un.ks & ~(kTileK - 1), 2 * aw);
 
       for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
         const bool partial = (j0 < un.ks) || (j0 + kTileK > un.ke);
-        const int jn = j0 + kTileK < un.ke ? j0 + kTileK : j0;     // next tile (the last one re-reads itself: harmless)
+        // next tile; the unit's last tile fetches the next unit's first one (or re-reads itself at the very end: harmless)
+        const int jn = j0 + kTileK < un.ke ? j0 + kTileK : (next_first >= 0 ? next_first : j0);
         mbar_wait(bar_bfull + 8 * bbuf, bphase);
         const uint32_t bias_buf = smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4) + (g * kTileK + 4 * t) * 4;
 #pragma unroll

@@ -12,6 +12,8 @@
 //             the output modes)
 // The launcher falls back to the mma.sync kernel (gemm_mma.cu) for shapes this tiling does not cover
 // (N % 64, K % 64, unaligned pitches).  Every output element is accumulated over k in one fixed order.
+#include <cstdlib>
+
 #include "fold.cuh"
 #include "kernels.h"
 #include "mma_ptx.cuh"
@@ -283,7 +285,8 @@ cudaError_t launch_gemm_tc(const GemmMmaParams& p, cudaStream_t st) {
   const unsigned mt_tiles = (unsigned)((p.M + TBM - 1) / TBM);
   const unsigned mt = mt_tiles + (p.fold_w_b != nullptr ? 1u : 0u);     // + the row that carries the LayerNorm(z) fold
   // 128-wide tiles when they give every SM two CTAs (or N does not split into 64s evenly enough to matter)
-  if (p.N % 128 == 0 && (int64_t)p.nseg * (p.N / 128) * mt_tiles >= 2 * 148) {
+  static const int force = [] { const char* e = getenv("DCP_GEMM_TBN"); return e ? atoi(e) : 0; }();
+  if (force != 64 && p.N % 128 == 0 && (force == 128 || (int64_t)p.nseg * (p.N / 128) * mt_tiles >= 2 * 148)) {
     dim3 grid((unsigned)(p.nseg * (p.N / 128)), mt);
     return launch_kernel(gemm_tc_kernel<128>, grid, dim3(kTcThreads), TcCfg<128>::kSmemAlloc, st, p.pdl, maps, p);
   } else {
