@@ -414,29 +414,48 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
         if (bbuf == 0) bphase ^= 1;
       }
 
-      // ---- a7: partial state of (rows, key segment) -> slot   (m back in natural-log units)
+      // ---- a7: partial state of (rows, key segment) -> slot   (m back in natural-log units).
+      // acc goes through shared memory: in the MMA fragment layout a store instruction touches 8 rows (8 lines of 32
+      // useful bytes; the unit's 96 KB cost ~7 us of LSU wavefronts, a what-if without them showed); staged per
+      // (head, 16-row block) in the warp's slab of the Q tile's buffer -- free once every warp has finished the unit's
+      // last QK^T -- and written back as 128-bit row pieces, a row's C floats contiguous.
       constexpr float kLn2 = 0.6931471805599453f;
+      constexpr int kOPitch = C == 24 ? 40 : C + 8;            // floats; conflict-free 64-bit fragment writes
+      static_assert(8 * 16 * kOPitch * 4 <= kTileQ * q_pitch(CP), "O staging fits the Q tile buffer");
+      const uint32_t slab = s_q + aw * (16 * kOPitch * 4);
+      asm volatile("bar.sync 1, 256;" ::: "memory");          // nobody reads this unit's Q tile any more
 #pragma unroll
       for (int hh = 0; hh < 2; ++hh)
 #pragma unroll
-        for (int mb = 0; mb < 2; ++mb)
+        for (int mb = 0; mb < 2; ++mb) {
+          const int h = 2 * aw + hh;
 #pragma unroll
           for (int x = 0; x < 2; ++x) {
             const float l = quad_sum(l_run[hh][mb][x]);
             const int row = un.q0 + mb * 16 + g + 8 * x;
-            if (row < un.q_end) {
-              const int h = 2 * aw + hh;
+            if (row < un.q_end && t == 0) {
               const int64_t srow = (int64_t)un.slot * p.state_rows + (row - p.state_row0);
-              if (t == 0) {
-                p.st_m[srow * kH + h] = m_run[hh][mb][x] * kLn2;
-                p.st_l[srow * kH + h] = l;
-              }
-              float* dst = p.st_acc + srow * (kH * C) + h * C + 2 * t;
+              p.st_m[srow * kH + h] = m_run[hh][mb][x] * kLn2;
+              p.st_l[srow * kH + h] = l;
+            }
 #pragma unroll
-              for (int nd = 0; nd < ND; ++nd)
-                *reinterpret_cast<float2*>(dst + nd * 8) = make_float2(o[hh][mb][nd][2 * x], o[hh][mb][nd][2 * x + 1]);
+            for (int nd = 0; nd < ND; ++nd)
+              asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(slab + ((g + 8 * x) * kOPitch + nd * 8 + 2 * t) * 4),
+                           "f"(o[hh][mb][nd][2 * x]), "f"(o[hh][mb][nd][2 * x + 1]) : "memory");
+          }
+          __syncwarp();
+#pragma unroll
+          for (int i = 0; i < 16 * (C / 4) / 32; ++i) {
+            const int e = i * 32 + lane, r = e / (C / 4), c4 = e - r * (C / 4);
+            const int row = un.q0 + mb * 16 + r;
+            const float4 v = lds_f32x4(slab + (r * kOPitch + c4 * 4) * 4);
+            if (row < un.q_end) {
+              const int64_t srow = (int64_t)un.slot * p.state_rows + (row - p.state_row0);
+              *reinterpret_cast<float4*>(p.st_acc + srow * (kH * C) + h * C + c4 * 4) = v;
             }
           }
+          __syncwarp();
+        }
     }
   }
   // teardown: every role is done with tensor memory before the allocating warp frees it
