@@ -2,23 +2,26 @@
 //   per pair (i, j):  LayerNorm(z_ij) -> bias_h = zhat . W_b[:,h]          ("learned projection of Z")
 //   logit_h = q_i^h . k_j^h / sqrt(c) + bias_h                             (PAPER.md:83 Eq. 2; i = row of z, :81)
 //   online softmax over keys with running (m, l, acc)
-// z is streamed from HBM exactly once by TMA (cp.async.bulk.tensor, 128-byte swizzle) through a 4-stage
+// z is streamed from HBM exactly once by TMA (cp.async.bulk.tensor, 128-byte swizzle, evict_first) through a 3-stage
 // mbarrier ring; the I*I*H logits and the LayerNorm output never leave the SM.
 //
-// One persistent CTA per SM, 16 warps, warp-specialised (register budgets moved with setmaxnreg):
+// One persistent CTA per SM, 16 warps, warp-specialised (register budgets moved with setmaxnreg 24 / 104 / 192):
 //   warp 0        TMA producer: z boxes of (64 ch, 16 keys, 8 queries) x 2 channel halves = 32 KB per stage
-//   warps 4-7     bias projection: per (query, 16 keys) one m16 block; A = raw z tile (ldmatrix from the swizzled
-//                 stage), B = (gamma (.) W_b log2 e)^T bf16, fp32 accumulate; LayerNorm statistics (two-pass, fp32)
-//                 come from the same A fragments; bias = rstd*(z.W' - mu*c1) + c0 goes to a double-buffered
-//                 shared-memory tile bias[h][32 queries][16 keys] fp32  (the layout change projection -> logits)
-//   warps 8-15    attention: warp w owns heads 2w, 2w+1 for the tile's 32 queries (two m16 blocks): the MMA
-//                 accumulator is initialised with the bias, S += Q K^T, online softmax in the exp2 domain
-//                 (q is pre-scaled by log2 e / sqrt(c)), P (bf16) feeds PV straight from registers,
-//                 K / V^T fragments are read from L2 with 64-bit loads (a per-16 key permutation makes each
-//                 thread's fragment contiguous), O stays in registers (96 per thread).
-// Work unit = (32-query tile) x (key segment); key tiles are aligned to absolute multiples of 16 and a row's
-// arithmetic depends only on its key segments, so row(P) == monolithic and grid(GxG) == monolithic(key_split=G)
-// bitwise.  No atomics.
+//   warps 1-3     tcgen05 issuers (one lane each, stage n -> issuer n % 3): per stage 8 x tcgen05.mma kind::f16
+//                 (M = 128 pair rows exactly as TMA wrote them, N = 32, K = 16) against W'' = [(gamma (.) W_b log2 e)^T ;
+//                 ones ; 0] -> z.W' for 16 heads and sum_k z, accumulated in tensor memory (4 buffers of 32 columns)
+//   warps 4-7     LayerNorm statistics + bias epilogue, thread = pair: sum_k z^2 from the thread's own 256-byte row of
+//                 the swizzled stage (exact bf16 x bf16 products, fp32 sums: fma.rn.f32.bf16), z.W' and sum z by
+//                 tcgen05.ld; bias = rstd (z.W' - mu c1) + c0 -> double-buffered shared tile bias[h][32 queries][16 keys]
+//                 fp32 (the layout change "row = pair" -> "row = query")
+//   warps 8-15    attention: warp w owns heads 2w, 2w+1 for the tile's 32 queries (two m16 blocks): the mma.sync
+//                 accumulator is initialised with the bias, S += Q K^T (Q fragments by conflict-free LDS.64 from a padded
+//                 shared Q tile), online softmax in the exp2 domain with a lazily moving reference (q is pre-scaled by
+//                 log2 e / sqrt(c)), P (bf16) feeds PV straight from registers, K / V fragments are single coalesced
+//                 128-bit loads from L2 (MMA B-fragment order, written by the prologue GEMM), O stays in registers
+//                 (96 per thread) and leaves as a partial state through a shared-memory slab.
+// Why QK^T / PV stay on mma.sync: what-if builds (profiles/r02_fused_c2_ncu_full.txt) show that removing every
+// attention MMA changes the kernel time by 1-2 %; what paced the kernel was the issue rate of the projection MMAs.
 #include "kernels.h"
 #include "mma_ptx.cuh"
 
