@@ -76,10 +76,11 @@ typedef struct {
   int key_split; /* MONOLITHIC / ROW: key chunks (Eq. 5) merged left to right; <= 0 means 1.  GRID: ignored
                     (the key axis is cut into sqrt(parts) blocks).                                       */
   int kernel;    /* a dcp_kernel                                                                         */
-  int tile_q, tile_k; /* query / key tile of the fused kernel (north_star's `tile`): 0 = the kernel's own tiling.
-                    The kernels are instantiated for ONE tiling each (fused_mma 32 x 16, fused_atom 64 x 32,
-                    fused_generic 8 x 32); any other non-zero value is
-                    DCP_ERR_UNSUPPORTED.  Results do not depend on the tiling beyond rounding.             */
+  int tile_q, tile_k; /* query / key tile of the fused kernel (north_star's `tile`): 0 = automatic.  fused_mma_kernel
+                    (tokens) takes any query-tile height 25..32 (its last TMA box is trimmed to the tile) and picks
+                    the one whose unit count fills whole waves of SMs; key tile 16.  fused_atom_kernel: 64 x 32,
+                    fused_generic_kernel: 8 x 32, fixed.  Any other non-zero value is DCP_ERR_UNSUPPORTED.  The
+                    tiling changes no row's arithmetic: results are bitwise independent of tile_q.           */
   int key_segments; /* tensor-core kernels: Eq.-5 segments each key chunk is cut into (the units that fill the 148
                     SMs; one partial state per segment, merged left to right like the chunks).  0 = automatic, a
                     pure function of (I, number of chunks), so that every decomposition cuts a row's keys alike

@@ -63,6 +63,7 @@ struct Plan {
   int parts, key_split, slots, G, kernel;
   bool use_mma;   // bf16 tensor-core path (fused_mma.cu) instead of the generic fp32 CUDA-core kernel
   int nseg;       // tensor-core path: Eq.-5 segments per key chunk (a pure function of I and the chunk count)
+  int tile_h;     // tensor-core path: query rows per work unit
   cudaEvent_t ev_begin, ev_end;
 };
 
@@ -104,13 +105,21 @@ dcp_status make_plan(int64_t I, int H, int c, int c_z, dcp_dtype dt, dcp_decomp 
     int tq, tk;
     if (p.use_mma) { tq = H == 16 ? 32 : fused_atom_tile_q(); tk = H == 16 ? 16 : 32; }
     else { tq = 8; tk = 32; }
-    if ((in->tile_q && in->tile_q != tq) || (in->tile_k && in->tile_k != tk)) return DCP_ERR_UNSUPPORTED;
+    // fused_mma_kernel takes any query-tile height 25..32 (a trimmed last TMA box); the others have one tiling
+    const bool tq_ok = in->tile_q == 0 || in->tile_q == tq || (p.use_mma && H == 16 && in->tile_q >= 25 && in->tile_q <= 32);
+    if (!tq_ok || (in->tile_k && in->tile_k != tk)) return DCP_ERR_UNSUPPORTED;
   }
-  p.nseg = p.use_mma ? mma_num_segments(I, H, p.key_split) : 1;
-  if (p.use_mma && in && in->key_segments > 0) {
-    // never more segments than whole key tiles in the smallest chunk: every segment keeps at least one key
-    const int64_t tile_k = H == 16 ? 16 : 32;
-    p.nseg = (int)std::min<int64_t>(in->key_segments, std::max<int64_t>(1, (I / p.key_split) / tile_k));
+  p.nseg = 1;
+  p.tile_h = 0;
+  if (p.use_mma) {
+    int force_s = 0;
+    if (in && in->key_segments > 0) {
+      // never more segments than whole key tiles in the smallest chunk: every segment keeps at least one key
+      const int64_t tile_k = H == 16 ? 16 : 32;
+      force_s = (int)std::min<int64_t>(in->key_segments, std::max<int64_t>(1, (I / p.key_split) / tile_k));
+    }
+    const int n_qparts = decomp == DCP_GRID ? p.G : p.parts;
+    mma_pick_units(I, H, n_qparts, p.key_split, force_s, (in && H == 16) ? in->tile_q : 0, &p.nseg, &p.tile_h);
   }
   p.slots = p.key_split * p.nseg;
   *out = p;
@@ -295,7 +304,7 @@ dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w
     mp.state_rows = I; mp.state_row0 = 0;
     mp.q_begin = 0; mp.q_end = (int)I; mp.n_qparts = plan.decomp == DCP_GRID ? plan.G : plan.parts;
     mp.k_begin = 0; mp.k_end = (int)I; mp.n_kparts = plan.key_split;
-    mp.nseg = plan.nseg; mp.slot0 = 0;
+    mp.nseg = plan.nseg; mp.slot0 = 0; mp.tile_h = plan.tile_h;
     mp.pdl = pdl_enabled() && plan.ev_begin == nullptr;   // an event record between two launches would serialise them anyway
     if (plan.ev_begin && cudaEventRecord(plan.ev_begin, x.st) != cudaSuccess) return DCP_ERR_CUDA;
     DCP_CUDA(launch_fused_mma(mp, z, ldz, x.st));
@@ -688,7 +697,7 @@ dcp_status dcp_partial_states(const void* s, const void* z, int64_t ldz, const d
     mp.state_rows = q1 - q0; mp.state_row0 = q0;
     mp.q_begin = (int)q0; mp.q_end = (int)q1; mp.n_qparts = 1;
     mp.k_begin = (int)k0; mp.k_end = (int)k1; mp.n_kparts = 1;
-    mp.nseg = 1; mp.slot0 = 0;
+    mp.nseg = 1; mp.slot0 = 0; mp.tile_h = 32;
     DCP_CUDA(launch_fused_mma(mp, z, ldz, x.st));
     return DCP_OK;
   }

@@ -60,7 +60,7 @@ __host__ __device__ constexpr size_t smem_alloc(int CP) { return kSmemQ + (size_
 // C = head dim, CP = C rounded up to a multiple of 16 (q/k rows are zero-padded to CP by the prologue)
 template <int C, int CP>
 __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_constant__ CUtensorMap tmap_z,
-                                                                const MmaParams p) {
+                                                                const __grid_constant__ CUtensorMap tmap_tail, const MmaParams p) {
   extern __shared__ unsigned char smem_dyn[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
   const uint32_t s_z = smem_u32(smem + kSmemZ);
@@ -101,7 +101,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   tc_fence_after();
   const uint32_t tmem_base = *s_tmem;
 
-  const int n_units = (int)mma_num_units<kTileQ>(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
+  const int n_units = (int)mma_num_units<0>(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg, p.tile_h);
 
   if (warp < kProjWarp0) {
     // =============================================================== TMA producer (warp 0, one lane)
@@ -111,18 +111,24 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
       asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
       int stage = 0;
       uint32_t phase = 0;
+      const int tail_rows = p.tile_h % kSubQ;               // 0: every stage is a full box
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const Unit un = decode_unit<kTileQ, kTileK>(p, u);
-        const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
+        const Unit un = decode_unit<0, kTileK>(p, u);
+        const int rows = (un.q_end - un.q0) < p.tile_h ? (un.q_end - un.q0) : p.tile_h;
         const int nsub = (rows + kSubQ - 1) / kSubQ;
         for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
           for (int sub = 0; sub < nsub; ++sub) {
             mbar_wait(bar_zempty + 8 * stage, phase ^ 1);
-            mbar_expect_tx(bar_zfull + 8 * stage, kStageBytes);
+            // the last stage of a tile whose height is not a multiple of 8 fetches only the tile's own rows (box of
+            // tail_rows queries; the stage's remaining pair rows keep stale data, their results are never stored)
+            const bool tail = sub == nsub - 1 && rows - sub * kSubQ == tail_rows;
+            const CUtensorMap* tm = tail ? &tmap_tail : &tmap_z;
+            const uint32_t half_bytes = tail ? tail_rows * (kHalfBytes / kSubQ) : kHalfBytes;
+            mbar_expect_tx(bar_zfull + 8 * stage, 2 * half_bytes);
             const uint32_t dst = s_z + stage * kStageBytes;
             const int qrow = un.q0 + sub * kSubQ;
-            tma_load_3d(dst, &tmap_z, 0, j0, qrow, bar_zfull + 8 * stage, policy);
-            tma_load_3d(dst + kHalfBytes, &tmap_z, 64, j0, qrow, bar_zfull + 8 * stage, policy);
+            tma_load_3d(dst, tm, 0, j0, qrow, bar_zfull + 8 * stage, policy);
+            tma_load_3d(dst + kHalfBytes, tm, 64, j0, qrow, bar_zfull + 8 * stage, policy);
             if (++stage == kNZ) { stage = 0; phase ^= 1; }
           }
         }
@@ -142,8 +148,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
       int stage = 0, tb = 0, turn = 0;
       uint32_t phase = 0, tphase = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const Unit un = decode_unit<kTileQ, kTileK>(p, u);
-        const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
+        const Unit un = decode_unit<0, kTileK>(p, u);
+        const int rows = (un.q_end - un.q0) < p.tile_h ? (un.q_end - un.q0) : p.tile_h;
         const int nsub = (rows + kSubQ - 1) / kSubQ;
         for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
           for (int sub = 0; sub < nsub; ++sub) {
@@ -190,8 +196,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     int tb = 0, bbuf = 0, stage = 0;
     uint32_t tphase = 0, bphase = 0, zphase = 0;
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const Unit un = decode_unit<kTileQ, kTileK>(p, u);
-      const int rows = (un.q_end - un.q0) < kTileQ ? (un.q_end - un.q0) : kTileQ;
+      const Unit un = decode_unit<0, kTileK>(p, u);
+      const int rows = (un.q_end - un.q0) < p.tile_h ? (un.q_end - un.q0) : p.tile_h;
       const int nsub = (rows + kSubQ - 1) / kSubQ;
       for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
         mbar_wait(bar_bempty + 8 * bbuf, bphase ^ 1);
@@ -281,13 +287,13 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     // The first K / V tile of a unit is requested during the last tile of the previous one (the slot that would re-read
     // the tile itself), so a unit change costs one L2 round trip (the Q tile) instead of two.
     if ((int)blockIdx.x < n_units) {
-      const Unit u0 = decode_unit<kTileQ, kTileK>(p, blockIdx.x);
+      const Unit u0 = decode_unit<0, kTileK>(p, blockIdx.x);
       load_k(u0.ks & ~(kTileK - 1), 2 * aw);
       load_v(u0.ks & ~(kTileK - 1), 2 * aw);
     }
     for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-      const Unit un = decode_unit<kTileQ, kTileK>(p, u);
-      const int next_first = u + (int)gridDim.x < n_units ? (decode_unit<kTileQ, kTileK>(p, u + gridDim.x).ks & ~(kTileK - 1)) : -1;
+      const Unit un = decode_unit<0, kTileK>(p, u);
+      const int next_first = u + (int)gridDim.x < n_units ? (decode_unit<0, kTileK>(p, u + gridDim.x).ks & ~(kTileK - 1)) : -1;
       // Q tile -> shared memory (rows of the tile, all heads), shared by the 8 attention warps; row pitch padded so the
       // per-thread 64-bit fragment loads are conflict-free.  Named barrier 1 = the 256 attention threads.
       constexpr int kQP = q_pitch(CP);
@@ -472,7 +478,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
 
 // ------------------------------------------------------------------ host side
 template <int C, int CP>
-cudaError_t launch_c(const CUtensorMap& tm, const MmaParams& p, int64_t units, cudaStream_t st) {
+cudaError_t launch_c(const CUtensorMap& tm, const CUtensorMap& tm_tail, const MmaParams& p, int64_t units, cudaStream_t st) {
   {   // per-device function attribute: set on every launch (cheap), so a process may use several GPUs
     cudaError_t e = cudaFuncSetAttribute(fused_mma_kernel<C, CP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_alloc(CP));
     if (e != cudaSuccess) return e;
@@ -482,7 +488,7 @@ cudaError_t launch_c(const CUtensorMap& tm, const MmaParams& p, int64_t units, c
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (sms <= 0) sms = 148;
   const unsigned grid = (unsigned)(units < sms ? units : sms);
-  return launch_kernel(fused_mma_kernel<C, CP>, dim3(grid), dim3(kThreads), smem_alloc(CP), st, p.pdl, tm, p);
+  return launch_kernel(fused_mma_kernel<C, CP>, dim3(grid), dim3(kThreads), smem_alloc(CP), st, p.pdl, tm, tm_tail, p);
 }
 
 }  // namespace
@@ -495,25 +501,55 @@ int mma_head_pad(int c) { return (c + 15) / 16 * 16; }
 // keys rounded up to 32: the atom kernel reads K / V two 16-key blocks at a time
 int64_t mma_frag_elems(int64_t I, int H, int c) { return (I + 31) / 32 * 2 * H * (mma_head_pad(c) / 16) * 256; }
 
-// Segments per key chunk: a pure function of (I, n_kparts) so every decomposition cuts a row's keys alike.
-// Picks the count that best fills 148 SMs with (32-query tile) x (segment) units, charging the partial-state
-// round trip (~25 * segments / I of the z bytes) and keeping segments >= 64 keys.
-int mma_num_segments(int64_t I, int H, int n_kparts) {
-  const int tile_q = H == kH ? kTileQ : fused_atom_tile_q();
-  const int64_t qtiles = (I + tile_q - 1) / tile_q;
+// Work units of the tensor-core kernels.  Cost model (in key tiles of one SM): waves x (tile height / 32) x (key tiles of
+// a unit + kUnitOverhead) x (1 + the partial-state round trip, ~25 * slots / I of the z bytes), waves = ceil(units / 148).
+// nseg is picked for the MONOLITHIC row count, so that it depends on (I, n_kparts) only -- every decomposition then cuts
+// a row's keys alike (bitwise contract); the tile height (fused_mma_kernel only: a trimmed last TMA box makes a tile of
+// h rows cost h / 32 of a full one) is picked afterwards for the actual row partition and changes no row's arithmetic.
+namespace {
+constexpr double kUnitOverhead = 1.5;    // key tiles: state write + Q reload + pipeline restart, measured ~5 us at C2
+int64_t count_tiles(int64_t n, int parts, int h) {
+  const int64_t base = n / parts, rem = n % parts;
+  return rem * ((base + 1 + h - 1) / h) + (parts - rem) * ((base + h - 1) / h);
+}
+double unit_cost(int64_t I, int n_qparts, int n_kparts, int s, int h, int h_full, int tile_k) {
+  const int64_t units = count_tiles(I, n_qparts, h) * n_kparts * s;
+  const int64_t waves = (units + 147) / 148;
+  const double key_tiles = (double)I / n_kparts / s / tile_k;
+  // a lower tile streams fewer bytes but repeats the tile's fixed work (K / V fragments, attention MMAs over all 32 rows)
+  const double fixed = 1.0 + 0.1 * (h_full - h) / 8.0;
+  return (double)waves * ((double)h / h_full) * fixed * (key_tiles + kUnitOverhead) * (1.0 + 25.0 * s * n_kparts / (double)I);
+}
+}  // namespace
+
+void mma_pick_units(int64_t I, int H, int n_qparts, int n_kparts, int force_nseg, int force_tile_h, int* nseg, int* tile_h) {
+  const bool token = H == kH;
+  const int h_full = token ? kTileQ : fused_atom_tile_q(), tile_k = token ? kTileK : 32;
+  const int h_min = token ? 25 : h_full;
   const int64_t chunk = I / n_kparts;
-  int best = 1;
-  double best_score = -1.0;
-  for (int s = 1; s <= 16; ++s) {
-    if (s > 1 && chunk / s < 64) break;
-    const int64_t units = qtiles * n_kparts * s;
-    const int64_t waves = (units + 147) / 148;
-    const double fill = (double)units / (double)(waves * 148);
-    const double extra = 25.0 * s * n_kparts / (double)I;
-    const double score = fill / (1.0 + extra);
-    if (score > best_score + 1e-9) { best_score = score; best = s; }
+  int best_s = 1;
+  if (force_nseg > 0) best_s = force_nseg;
+  else {
+    double best = 1e300;
+    for (int s = 1; s <= 16; ++s) {
+      if (s > 1 && chunk / s < 64) break;
+      for (int h = h_full; h >= h_min; --h) {
+        const double c = unit_cost(I, 1, n_kparts, s, h, h_full, tile_k);
+        if (c < best * (1.0 - 1e-9)) { best = c; best_s = s; }
+      }
+    }
   }
-  return best;
+  int best_h = h_full;
+  if (force_tile_h > 0) best_h = force_tile_h;
+  else {
+    double best = 1e300;
+    for (int h = h_full; h >= h_min; --h) {
+      const double c = unit_cost(I, n_qparts, n_kparts, best_s, h, h_full, tile_k);
+      if (c < best * (1.0 - 1e-9)) { best = c; best_h = h; }
+    }
+  }
+  *nseg = best_s;
+  *tile_h = best_h;
 }
 
 cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st) {
@@ -530,12 +566,21 @@ cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cud
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
-  const int64_t units = mma_num_units<kTileQ>(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
+  if (p.tile_h < 1 || p.tile_h > kTileQ) return cudaErrorInvalidValue;
+  CUtensorMap tm_tail = tm;                                  // tile heights that are not a multiple of 8: the tile's last box
+  if (p.tile_h % kSubQ != 0) {
+    const cuuint32_t box_t[3] = {64, kTileK, (cuuint32_t)(p.tile_h % kSubQ)};
+    r = enc(&tm_tail, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(z), gdim, gstr, box_t, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  }
+  const int64_t units = mma_num_units<0>(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg, p.tile_h);
   if (units > 0x7fffffff) return cudaErrorInvalidValue;
   switch (p.c) {
-    case 24: return launch_c<24, 32>(tm, p, units, st);
-    case 32: return launch_c<32, 32>(tm, p, units, st);
-    case 48: return launch_c<48, 48>(tm, p, units, st);
+    case 24: return launch_c<24, 32>(tm, tm_tail, p, units, st);
+    case 32: return launch_c<32, 32>(tm, tm_tail, p, units, st);
+    case 48: return launch_c<48, 48>(tm, tm_tail, p, units, st);
     default: return cudaErrorInvalidValue;
   }
 }

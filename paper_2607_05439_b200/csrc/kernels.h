@@ -80,6 +80,7 @@ struct MmaParams {
   int q_begin, q_end, n_qparts;
   int k_begin, k_end, n_kparts;
   int nseg, slot0;
+  int tile_h;           // fused_mma_kernel: query rows per work unit (25..32; the atom kernel's tile is fixed)
   int H, c, c_z;
   float eps;
   bool pdl;             // host only: launch as a programmatic dependent of the previous kernel in the stream
@@ -88,7 +89,10 @@ cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cud
 bool fused_mma_supports(dcp_dtype dt, int H, int c, int c_z);
 int mma_head_pad(int c);
 int64_t mma_frag_elems(int64_t I, int H, int c);   // bf16 elements of kfr (= of vfr)
-int mma_num_segments(int64_t I, int H, int n_kparts);
+// Units of the tensor-core kernels: *nseg = Eq.-5 segments per key chunk, *tile_h = query rows per unit (fused_mma_kernel:
+// 25..32, chosen so that the unit count fills whole waves of 148 SMs; fused_atom_kernel: fixed).  Pure functions of
+// (I, H, n_qparts, n_kparts): every call with the same decomposition cuts its rows and keys alike.
+void mma_pick_units(int64_t I, int H, int n_qparts, int n_kparts, int force_nseg, int force_tile_h, int* nseg, int* tile_h);
 // atom-level shape (c_atompair = 16, H = 4, c = 32): fused_atom.cu, dispatched to by launch_fused_mma
 cudaError_t launch_fused_atom(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st);
 bool fused_atom_supports(dcp_dtype dt, int H, int c, int c_z);

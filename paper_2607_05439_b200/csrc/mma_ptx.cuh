@@ -163,7 +163,7 @@ inline PFN_cuTensorMapEncodeTiled get_encode_fn() {
 // ------------------------------------------------------------------ work units
 struct Unit {
   int q0;      // first query row of the TQ-row tile
-  int q_end;   // end of the query part the tile belongs to (rows >= q_end are not computed / stored)
+  int q_end;   // end of the tile's own rows (rows >= q_end are not stored)
   int ks, ke;  // key segment
   int slot;    // partial-state slot
 };
@@ -175,11 +175,13 @@ __device__ __forceinline__ void shard32(int n, int parts, int p, int* start, int
   *start = p * base + (p < rem ? p : rem);
 }
 
+// kTileQ > 0: compile-time tile height; kTileQ == 0: run-time height `tq_rt` (fused_mma_kernel: MmaParams.tile_h)
 template <int kTileQ>
-__host__ __device__ inline int64_t mma_num_units(int n, int n_qparts, int n_kparts, int nseg) {
+__host__ __device__ inline int64_t mma_num_units(int n, int n_qparts, int n_kparts, int nseg, int tq_rt = 0) {
+  const int tq = kTileQ > 0 ? kTileQ : tq_rt;
   // query parts have sizes floor(n/P) or floor(n/P)+1 (Eq. 5): count their TQ-row tiles in closed form
   const int base = n / n_qparts, rem = n % n_qparts;
-  const int t_big = (base + 1 + kTileQ - 1) / kTileQ, t_small = (base + kTileQ - 1) / kTileQ;
+  const int t_big = (base + 1 + tq - 1) / tq, t_small = (base + tq - 1) / tq;
   return ((int64_t)rem * t_big + (int64_t)(n_qparts - rem) * t_small) * n_kparts * nseg;
 }
 
@@ -188,20 +190,22 @@ __host__ __device__ inline int64_t mma_num_units(int n, int n_qparts, int n_kpar
 // inside a tile: a boundary tile would be streamed and projected twice.  A pure function of (I, chunks, segments).
 template <int kTileQ, int kTileK>
 __device__ __forceinline__ Unit decode_unit(const MmaParams& p, int u) {
+  const int tq = kTileQ > 0 ? kTileQ : p.tile_h;
   const int n = p.q_end - p.q_begin;
   const int base = n / p.n_qparts, rem = n % p.n_qparts;
-  const int t_big = (base + 1 + kTileQ - 1) / kTileQ, t_small = (base + kTileQ - 1) / kTileQ;
+  const int t_big = (base + 1 + tq - 1) / tq, t_small = (base + tq - 1) / tq;
   const int per_tile = p.n_kparts * p.nseg;
   int tile = u / per_tile;
   const int r = u - tile * per_tile;
-  int part, tq;
-  if (tile < rem * t_big) { part = tile / t_big; tq = tile - part * t_big; }
-  else { tile -= rem * t_big; part = tile / t_small; tq = tile - part * t_small; part += rem; }
+  int part, tile_i;
+  if (tile < rem * t_big) { part = tile / t_big; tile_i = tile - part * t_big; }
+  else { tile -= rem * t_big; part = tile / t_small; tile_i = tile - part * t_small; part += rem; }
   int ps, pl;
   shard32(n, p.n_qparts, part, &ps, &pl);
   Unit un;
-  un.q0 = p.q_begin + ps + tq * kTileQ;
-  un.q_end = p.q_begin + ps + pl;
+  un.q0 = p.q_begin + ps + tile_i * tq;
+  un.q_end = p.q_begin + ps + pl;                             // end of the part ...
+  if (un.q_end > un.q0 + tq) un.q_end = un.q0 + tq;           // ... or of the tile (tile heights below the kernel's 32 / 64 rows)
   const int cb = r / p.nseg, sg = r - cb * p.nseg;
   int cs, cl, ts, tl;
   shard32(p.k_end - p.k_begin, p.n_kparts, cb, &cs, &cl);

@@ -359,8 +359,11 @@ def test_plan_tile_and_key_segments():
     s, z, w = util.make_problem(cfg, DEV)
     ref = util.oracle_rows(cfg, s, z, w, range(cfg.I))
     base = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c)
-    assert torch.equal(dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, tile=(32, 16)), base)     # the kernel's own tiling
-    for bad in ((64, 16), (32, 32), (128, 0)):
+    for tq in (32, 31, 28, 25):        # any query-tile height 25..32: the tiling changes no row's arithmetic
+        assert torch.equal(dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, tile=(tq, 16)), base), tq
+        assert torch.equal(dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, tile=(tq, 0), decomp="grid", parts=9),
+                           dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, decomp="grid", parts=9)), tq
+    for bad in ((64, 16), (32, 32), (128, 0), (24, 16), (33, 0)):
         with pytest.raises(dcp.DcpError) as e:
             dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, tile=bad)
         assert e.value.status == 2
