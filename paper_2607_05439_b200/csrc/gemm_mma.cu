@@ -208,6 +208,8 @@ __global__ void layernorm_rows_bf16_kernel(const __nv_bfloat16* __restrict__ x, 
                                            const __nv_bfloat16* __restrict__ beta, __nv_bfloat16* __restrict__ y,
                                            int64_t rows, int width, float eps) {
   // one warp per row; two-pass, population variance (reading #2 in DESIGN.md); output rounded to bf16
+  pdl_trigger();
+  pdl_wait();
   int64_t row = (int64_t)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;
   int lane = threadIdx.x % 32;
   if (row >= rows) return;
@@ -223,6 +225,58 @@ __global__ void layernorm_rows_bf16_kernel(const __nv_bfloat16* __restrict__ x, 
   float rstd = rsqrtf(warp_sum(v) / (float)width + eps);
   for (int k = lane; k < width; k += 32)
     y[row * width + k] = __float2bfloat16_rn((to_f32(xr[k]) - mu) * rstd * to_f32(gamma[k]) + to_f32(beta[k]));
+}
+
+// The same for widths that are a multiple of 8 up to 1024 with 16-byte aligned rows: the row lives in registers (up to four
+// 128-bit loads per lane), read once
+__global__ void __launch_bounds__(256) layernorm_rows_bf16_vec_kernel(const __nv_bfloat16* __restrict__ x, const __nv_bfloat16* __restrict__ gamma,
+                                                                      const __nv_bfloat16* __restrict__ beta, __nv_bfloat16* __restrict__ y,
+                                                                      int64_t rows, int width, float eps) {
+  pdl_trigger();
+  pdl_wait();
+  const int64_t row = (int64_t)blockIdx.x * 8 + threadIdx.x / 32;
+  const int lane = threadIdx.x % 32, nv = width >> 3;
+  if (row >= rows) return;
+  const uint4* xr = reinterpret_cast<const uint4*>(x + row * width);
+  float f[4][8];
+  float s = 0.f;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int vi = lane + 32 * i;
+    const uint4 u = vi < nv ? xr[vi] : make_uint4(0u, 0u, 0u, 0u);
+    const uint32_t w[4] = {u.x, u.y, u.z, u.w};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      f[i][2 * j] = __uint_as_float(w[j] << 16);
+      f[i][2 * j + 1] = __uint_as_float(w[j] & 0xffff0000u);
+      s += f[i][2 * j] + f[i][2 * j + 1];
+    }
+  }
+  const float mu = warp_sum(s) / (float)width;
+  float v = 0.f;
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+    if (lane + 32 * i < nv) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) { const float d = f[i][j] - mu; v = fmaf(d, d, v); }
+    }
+  const float rstd = rsqrtf(warp_sum(v) / (float)width + eps);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int vi = lane + 32 * i;
+    if (vi < nv) {
+      const uint4 g4 = __ldg(reinterpret_cast<const uint4*>(gamma) + vi), b4 = __ldg(reinterpret_cast<const uint4*>(beta) + vi);
+      const uint32_t gw[4] = {g4.x, g4.y, g4.z, g4.w}, bw[4] = {b4.x, b4.y, b4.z, b4.w};
+      uint32_t o[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const float y0 = (f[i][2 * j] - mu) * rstd * __uint_as_float(gw[j] << 16) + __uint_as_float(bw[j] << 16);
+        const float y1 = (f[i][2 * j + 1] - mu) * rstd * __uint_as_float(gw[j] & 0xffff0000u) + __uint_as_float(bw[j] & 0xffff0000u);
+        o[j] = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(y0)) | ((uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(y1)) << 16);
+      }
+      reinterpret_cast<uint4*>(y + row * width)[vi] = make_uint4(o[0], o[1], o[2], o[3]);
+    }
+  }
 }
 
 __global__ void fold_ln_z_mma_kernel(const __nv_bfloat16* __restrict__ w_b, const __nv_bfloat16* __restrict__ gamma,
@@ -254,9 +308,11 @@ cudaError_t launch_gemm_mma(const GemmMmaParams& p, cudaStream_t st, bool* fold_
 cudaError_t launch_layernorm_rows_bf16(const void* x, const void* gamma, const void* beta, void* y, int64_t rows,
                                        int width, float eps, cudaStream_t st) {
   unsigned blocks = (unsigned)((rows + 7) / 8);
-  layernorm_rows_bf16_kernel<<<blocks, 256, 0, st>>>((const __nv_bfloat16*)x, (const __nv_bfloat16*)gamma,
-                                                     (const __nv_bfloat16*)beta, (__nv_bfloat16*)y, rows, width, eps);
-  return cudaGetLastError();
+  const bool vec = width % 8 == 0 && width <= 1024 &&
+                   (((uintptr_t)x | (uintptr_t)y | (uintptr_t)gamma | (uintptr_t)beta) & 15) == 0;
+  // a programmatic dependent of the previous kernel in the stream (in a stack: the previous block's output GEMM)
+  return launch_kernel(vec ? layernorm_rows_bf16_vec_kernel : layernorm_rows_bf16_kernel, dim3(blocks), dim3(256), 0, st, true,
+                       (const __nv_bfloat16*)x, (const __nv_bfloat16*)gamma, (const __nv_bfloat16*)beta, (__nv_bfloat16*)y, rows, width, eps);
 }
 
 cudaError_t launch_fold_ln_z_mma(const void* w_b, const void* gamma, const void* beta, void* wfold, float* c1, float* c0,
