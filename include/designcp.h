@@ -248,6 +248,13 @@ dcp_status dcp_merge_states(int n_parts, int64_t rows, int H, int c, const float
 /* Eq. 5, host only: shard p of n items over `parts` shards. */
 dcp_status dcp_shard_range(int64_t n, int parts, int p, int64_t *start, int64_t *len);
 
+/* Host only: how a call with this plan is cut into work units on the tensor-core kernels -- key_segments (Eq.-5 segments
+ * per key chunk), tile_q (query rows per unit) and slots (partial states per row = key chunks x segments); 1 / 0 / chunks
+ * for the generic kernel.  key_segments depends on (I, key chunks) only, never on the row partition: that is what makes
+ * row(P) == monolithic and grid(G x G) == monolithic(key_split = G) bitwise.  `plan` may be NULL. */
+dcp_status dcp_plan_units(int64_t I, int H, int c, int c_z, dcp_dtype dtype, dcp_decomp decomp, const dcp_plan *plan,
+                          int *key_segments, int *tile_q, int *slots);
+
 /* 1 if fused kernel `kernel` (a dcp_kernel, not AUTO) is instantiated for this (dtype, H, c, c_z), else 0. Host only. */
 int dcp_kernel_supported(int kernel, dcp_dtype dtype, int H, int c, int c_z);
 

@@ -31,7 +31,7 @@ EXPORTS = [
     "dcp_sparse_atom_workspace_bytes", "dcp_sparse_atom_attention", "dcp_knn", "dcp_knn_budget", "dcp_gather_pair_slice",
     "dcp_pair_transition_workspace_bytes", "dcp_pair_transition",
     "dcp_pairformer_stack_workspace_bytes", "dcp_pairformer_stack",
-    "dcp_attention_stack_workspace_bytes", "dcp_attention_stack",
+    "dcp_attention_stack_workspace_bytes", "dcp_attention_stack", "dcp_plan_units",
     "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
     "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
 ]
@@ -102,7 +102,8 @@ def _load() -> C.CDLL:
     lib.dcp_attention_stack_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, i32, C.POINTER(sz)]
     lib.dcp_attention_stack.argtypes = [vp, vp, i64, C.POINTER(dcp_weights), i32, i64, i32, i32, i32, i32, i32, vp, sz, vp]
     lib.dcp_knn_budget.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, vp]
-    for n in EXPORTS[:18]:
+    lib.dcp_plan_units.argtypes = [i64, i32, i32, i32, i32, i32, C.POINTER(dcp_plan), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
+    for n in EXPORTS[:19]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -198,6 +199,16 @@ def dcp_workspace_bytes(I, c_s, H, c, c_z, dtype: torch.dtype, decomp="monolithi
     _check(_lib.dcp_workspace_bytes(I, c_s, H, c, c_z, _dtype_code(dtype), DECOMP[decomp], C.byref(pl),
                                     C.byref(out)), "dcp_workspace_bytes")
     return int(out.value)
+
+
+def dcp_plan_units(I, H, c, c_z, dtype: torch.dtype, decomp="monolithic", parts=1, key_split=1, kernel="auto", tile=(0, 0),
+                   key_segments=0):
+    """(key_segments, tile_q, slots) a call with this plan uses (host only; no device needed)."""
+    pl = _plan(parts, key_split, kernel, None, tile, key_segments)
+    a, b, cc = C.c_int(), C.c_int(), C.c_int()
+    _check(_lib.dcp_plan_units(int(I), H, c, c_z, _dtype_code(dtype), DECOMP[decomp], C.byref(pl), C.byref(a), C.byref(b),
+                               C.byref(cc)), "dcp_plan_units")
+    return a.value, b.value, cc.value
 
 
 def dcp_kernel_supported(kernel, dtype: torch.dtype, H: int, c: int, c_z: int) -> bool:

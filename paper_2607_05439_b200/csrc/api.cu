@@ -732,6 +732,19 @@ dcp_status dcp_shard_range(int64_t n, int parts, int p, int64_t* start, int64_t*
   return DCP_OK;
 }
 
+dcp_status dcp_plan_units(int64_t I, int H, int c, int c_z, dcp_dtype dtype, dcp_decomp decomp, const dcp_plan* plan_in,
+                          int* key_segments, int* tile_q, int* slots) {
+  if (!key_segments || !tile_q || !slots || I <= 0) return DCP_ERR_INVALID_ARG;
+  if (!fused_generic_supports(dtype, H, c, c_z) && !fused_mma_supports(dtype, H, c, c_z)) return DCP_ERR_UNSUPPORTED;
+  Plan plan;
+  dcp_status st = make_plan(I, H, c, c_z, dtype, decomp, plan_in, &plan);
+  if (st != DCP_OK) return st;
+  *key_segments = plan.nseg;
+  *tile_q = plan.tile_h;
+  *slots = plan.slots;
+  return DCP_OK;
+}
+
 int dcp_kernel_supported(int kernel, dcp_dtype dtype, int H, int c, int c_z) {
   if (kernel == DCP_KERNEL_GENERIC) return fused_generic_supports(dtype, H, c, c_z) ? 1 : 0;
   if (kernel == DCP_KERNEL_MMA) return fused_mma_supports(dtype, H, c, c_z) ? 1 : 0;

@@ -51,7 +51,9 @@ def test_workspace_bytes_and_validation_without_gpu():
     b4 = dcp.dcp_workspace_bytes(3000, 384, 16, 48, 128, torch.bfloat16, "grid", 16)
     assert b4 > b1 > 5 * 3000 * 768 * 2
     # states: [slots][I][H] x2 + [slots][I][D] fp32
-    assert b4 - b1 >= 3 * 3000 * (2 * 16 + 768) * 4
+    s1 = dcp.dcp_plan_units(3000, 16, 48, 128, torch.bfloat16)[2]
+    s4 = dcp.dcp_plan_units(3000, 16, 48, 128, torch.bfloat16, "grid", 16)[2]
+    assert s4 > s1 and b4 - b1 >= (s4 - s1) * 3000 * (2 * 16 + 768) * 4
     for bad in (dict(decomp="grid", parts=8), dict(decomp="row", parts=3001), dict(decomp="grid", parts=0)):
         with pytest.raises(dcp.DcpError) as e:
             dcp.dcp_workspace_bytes(3000, 384, 16, 48, 128, torch.bfloat16, **bad)
@@ -64,6 +66,37 @@ def test_workspace_bytes_and_validation_without_gpu():
     assert e.value.status == 2
     assert dcp.status_string(0) == "DCP_OK" and dcp.version() >= 100
     assert dcp.dcp_kernel_supported("generic", torch.float32, 4, 32, 64)
+
+
+def test_plan_units_are_a_pure_function_of_the_key_cut():
+    """Host logic behind the bitwise decomposition contract: the segments a key chunk is cut into
+    depend on (I, number of chunks) only -- never on the row partition -- so row(P) and the G x G grid cut a row's keys
+    exactly like monolithic(key_split = 1 resp. G); the tile height may differ (it changes no row's arithmetic)."""
+    _ensure_built()
+    import paper_2607_05439_b200 as dcp
+    bf = torch.bfloat16
+    for I in (131, 600, 3000, 12000, 27180):
+        seg1, tq1, slots1 = dcp.dcp_plan_units(I, 16, 48, 128, bf)
+        assert slots1 == seg1 and 25 <= tq1 <= 32 and 1 <= seg1 <= 16
+        for P in (2, 7, 8, 16):
+            if P > I:
+                continue
+            seg, tq, slots = dcp.dcp_plan_units(I, 16, 48, 128, bf, "row", P)
+            assert (seg, slots) == (seg1, slots1) and 25 <= tq <= 32
+        for G in (2, 4):
+            segk, _, slotsk = dcp.dcp_plan_units(I, 16, 48, 128, bf, key_split=G)
+            segg, _, slotsg = dcp.dcp_plan_units(I, 16, 48, 128, bf, "grid", G * G)
+            assert (segg, slotsg) == (segk, slotsk) and slotsg == G * segg
+    # the headline config: 3 segments x 97 tiles of 31 rows = 291 units for 148 SMs (two waves)
+    assert dcp.dcp_plan_units(3000, 16, 48, 128, bf) == (3, 31, 3)
+    # forced values are honoured, clamped to whole key tiles; the atom and generic kernels have one tiling
+    assert dcp.dcp_plan_units(3000, 16, 48, 128, bf, key_segments=5, tile=(28, 16))[:2] == (5, 28)
+    assert dcp.dcp_plan_units(300, 16, 48, 128, bf, key_segments=64)[0] == 300 // 16
+    assert dcp.dcp_plan_units(24000, 4, 32, 16, bf)[1] == 64
+    assert dcp.dcp_plan_units(64, 4, 32, 64, torch.float32, key_split=2) == (1, 0, 2)
+    with pytest.raises(dcp.DcpError) as e:
+        dcp.dcp_plan_units(3000, 16, 48, 128, bf, tile=(24, 16))
+    assert e.value.status == 2
 
 
 def test_product_does_not_import_oracle():
