@@ -382,3 +382,35 @@ def test_plan_tile_and_key_segments():
     s0, z0, w0 = util.make_problem(cfg0, DEV)
     assert torch.equal(dcp.dcp_pair_bias_attention(s0, z0, w0, cfg0.H, cfg0.c, tile=(8, 32)),
                        dcp.dcp_pair_bias_attention(s0, z0, w0, cfg0.H, cfg0.c))
+
+
+# ------------------------------------------------------------------ seeded fuzz over shapes, decompositions and unit plans
+def test_fuzz_decompositions_and_unit_plans():
+    """Forty seeded random problems on the tensor-core kernels (token shape, every fourth the atom shape; ragged I from 1
+    to 420, every instantiated head size, random stripes / grids / key splits / forced segments / tile heights): each result against the oracle, and the
+    bitwise contract row(P) == monolithic, grid(G x G) == monolithic(key_split = G) for equal key segments."""
+    dcp = _dcp()
+    rng = np.random.default_rng(2025)
+    for case in range(40):
+        I = int(rng.integers(1, 421))
+        atom = case % 4 == 3                       # every fourth case: the atom-level kernel's shape
+        c = 32 if atom else int(rng.choice([24, 32, 48]))
+        c_s = int(rng.choice([32, 64, 96]))
+        cfg = syn.small_config("fuzz", I=I, c_s=c_s, c_z=16 if atom else 128, H=4 if atom else 16, c=c, dtype="bf16",
+                               seed=1000 + case)
+        s, z, w = util.make_problem(cfg, DEV, with_ln_s=bool(rng.integers(0, 2)), with_b_q=bool(rng.integers(0, 2)))
+        ref = util.oracle_rows(cfg, s, z, w, range(I))
+        ks = int(rng.choice([0, 0, 1, 2, 3, 7]))
+        tq = 0 if atom else int(rng.choice([0, 0, 25, 27, 30, 31, 32]))
+        kw = dict(key_segments=ks, tile=(tq, 0))
+        mono = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, **kw)
+        util.check_close(mono, ref, "bf16", f"fuzz {case}: I={I} c={c} ks={ks} tq={tq}")
+        P = int(rng.integers(1, min(I, 9) + 1))
+        row = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, decomp="row", parts=P, key_segments=ks,
+                                          tile=(0 if atom else int(rng.choice([0, 26, 32])), 0))
+        assert torch.equal(row, mono), f"fuzz {case}: row({P}) != monolithic (I={I}, ks={ks})"
+        G = int(rng.integers(1, min(I, 4) + 1))
+        grid = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, decomp="grid", parts=G * G, **kw)
+        mk = dcp.dcp_pair_bias_attention(s, z, w, cfg.H, cfg.c, key_split=G, key_segments=ks)
+        assert torch.equal(grid, mk), f"fuzz {case}: grid({G * G}) != monolithic(key_split={G}) (I={I}, ks={ks})"
+        util.check_close(grid, ref, "bf16", f"fuzz {case}: grid({G * G})")
