@@ -17,6 +17,8 @@
 //                 K / V fragments (MMA B-fragment order, gemm_mma.cu) are 128-bit L2 / L1 loads
 // Work unit = (64-query tile) x (key segment); key tiles are aligned to absolute multiples of 32 and a row's arithmetic
 // depends only on its key segments.  No atomics.
+#include <cstdlib>
+
 #include "kernels.h"
 #include "mma_ptx.cuh"
 
@@ -60,6 +62,13 @@ __device__ __forceinline__ void tmem_ld_x8(uint32_t taddr, float (&v)[8]) {
   for (int i = 0; i < 8; ++i) v[i] = __uint_as_float(r[i]);
 }
 
+// kWide (L % 4 == 0): p is viewed as [L queries][L / 4 key groups][4 keys x 16 ch = 128 bytes] and fetched with 128-byte
+// TMA rows (128-byte swizzle): a 32 KB stage is 256 TMA rows instead of 1024 -- with 32-byte rows the TMA engine, not HBM,
+// capped the stream at 5.8 TB/s.  Stage row = 8 q + key group; MMA (b, s), b = 128-row block, s = key
+// inside the group, reads the 32 bytes at offset 32 s of every row (the K = 16 slice of the swizzle atom): its TMEM lane r
+// is the pair (query 16 b + r / 8, key 4 (r % 8) + s) of the stage.  Otherwise (any L): 32-byte rows, stage row = 32 q +
+// key, MMA m covers queries 4 m .. 4 m + 3.
+template <bool kWide>
 __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_constant__ CUtensorMap tmap_z,
                                                                  const MmaParams p) {
   extern __shared__ unsigned char smem_dyn[];
@@ -120,7 +129,7 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
           for (int sub = 0; sub < nsub; ++sub) {
             mbar_wait(bar_zempty + 8 * stage, phase ^ 1);
             mbar_expect_tx(bar_zfull + 8 * stage, aStageBytes);
-            tma_load_3d(s_z + stage * aStageBytes, &tmap_z, 0, j0, un.q0 + sub * aSubQ, bar_zfull + 8 * stage, policy);
+            tma_load_3d(s_z + stage * aStageBytes, &tmap_z, 0, kWide ? j0 >> 2 : j0, un.q0 + sub * aSubQ, bar_zfull + 8 * stage, policy);
             if (++stage == aNZ) { stage = 0; phase ^= 1; }
           }
         }
@@ -144,7 +153,8 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
             const uint32_t zs = s_z + stage * aStageBytes;
 #pragma unroll
             for (int m = 0; m < aMmaPerStage; ++m)
-              umma_bf16(tmem_base + tb * aTmemBufCols + m * aProjN, umma_desc_sw32(zs + m * 4096), bdesc, idesc, 0);
+              umma_bf16(tmem_base + tb * aTmemBufCols + m * aProjN,
+                        kWide ? umma_desc_sw128(zs + (m >> 2) * 16384 + (m & 3) * 32) : umma_desc_sw32(zs + m * 4096), bdesc, idesc, 0);
             umma_commit(bar_zempty + 8 * stage);
             umma_commit(bar_tfull + 8 * tb);
             if (++stage == aNZ) { stage = 0; phase ^= 1; }
@@ -180,6 +190,27 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
           // ---- a2: sum_k z^2 of the thread's 8 pairs straight from the TMA stage
           mbar_wait(bar_zfull + 8 * stage, zphase);
           float zsq[aMmaPerStage];
+          if constexpr (kWide) {
+            // the thread's two 128-byte rows (one per block b): key s of the group = 16-byte chunks 2 s, 2 s + 1, each at
+            // (chunk ^ row % 8): eight conflict-free LDS.128 per row
+            const uint32_t rp = pw * 32 + lane, sw = rp & 7;
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {
+              const uint32_t base = s_z + stage * aStageBytes + (128 * b + rp) * 128;
+              uint4 w[8];
+#pragma unroll
+              for (int c = 0; c < 8; ++c) w[c] = lds_u32x4(base + ((c ^ sw) << 4));
+#pragma unroll
+              for (int sk = 0; sk < 4; ++sk) {
+                float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+                fma_sq_bf16x2(s0, s1, w[2 * sk].x); fma_sq_bf16x2(s2, s3, w[2 * sk].y);
+                fma_sq_bf16x2(s0, s1, w[2 * sk].z); fma_sq_bf16x2(s2, s3, w[2 * sk].w);
+                fma_sq_bf16x2(s0, s1, w[2 * sk + 1].x); fma_sq_bf16x2(s2, s3, w[2 * sk + 1].y);
+                fma_sq_bf16x2(s0, s1, w[2 * sk + 1].z); fma_sq_bf16x2(s2, s3, w[2 * sk + 1].w);
+                zsq[4 * b + sk] = (s0 + s1) + (s2 + s3);
+              }
+            }
+          } else {
 #pragma unroll
           for (int m = 0; m < aMmaPerStage; ++m) {
             const uint4 w0 = lds_u32x4(zrow + stage * aStageBytes + m * 4096);
@@ -190,6 +221,7 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
             fma_sq_bf16x2(s0, s1, w1.x); fma_sq_bf16x2(s2, s3, w1.y);
             fma_sq_bf16x2(s0, s1, w1.z); fma_sq_bf16x2(s2, s3, w1.w);
             zsq[m] = (s0 + s1) + (s2 + s3);
+          }
           }
 #pragma unroll
           for (int m = 0; m < aMmaPerStage; ++m) asm volatile("" : "+f"(zsq[m]));   // rows consumed before the release
@@ -210,6 +242,25 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
               __syncwarp();
               if (lane == 0) mbar_arrive(bar_tempty + 8 * tb);    // accumulators are in registers: buffer free
             }
+            if constexpr (kWide) {
+              // the four MMAs of this block are the four keys of the thread's group: one 128-bit store per head
+              float bv[aH][4];
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                const float mu = v[i][aH] * (1.f / aCz);
+                const float var = fmaf(-mu, mu, zsq[half * 4 + i] * (1.f / aCz));
+                const float rstd = var > 0.f ? rsqrtf(var + p.eps) : 0.f;
+                const float nm = -mu * rstd;
+#pragma unroll
+                for (int h = 0; h < aH; ++h) bv[h][i] = fmaf(v[i][h], rstd, fmaf(nm, c1h[h], c0h[h]));
+              }
+              const int ql = sub * aSubQ + 16 * half + 4 * pw + (lane >> 3);
+              const uint32_t brow = bias_buf + (ql * aTileK + ((4 * (lane & 7)) ^ ((ql & 1) << 4))) * 4;
+#pragma unroll
+              for (int h = 0; h < aH; ++h)
+                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(brow + h * (aTileQ * aTileK * 4)), "f"(bv[h][0]),
+                             "f"(bv[h][1]), "f"(bv[h][2]), "f"(bv[h][3]) : "memory");
+            } else {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               const int m = half * 4 + i;
@@ -224,6 +275,7 @@ __global__ void __launch_bounds__(aThreads, 1) fused_atom_kernel(const __grid_co
 #pragma unroll
               for (int h = 0; h < aH; ++h)
                 sts_f32(brow + h * (aTileQ * aTileK * 4), fmaf(v[i][h], rstd, fmaf(nm, c1h[h], c0h[h])));
+            }
             }
           }
           tb ^= 1;
@@ -440,18 +492,32 @@ cudaError_t launch_fused_atom(const MmaParams& p, const void* z, int64_t ldz, cu
   PFN_cuTensorMapEncodeTiled enc = get_encode_fn();
   if (!enc) return cudaErrorNotSupported;
   CUtensorMap tm;
-  const cuuint64_t gdim[3] = {(cuuint64_t)aCz, (cuuint64_t)p.I, (cuuint64_t)p.I};
-  const cuuint64_t gstr[2] = {(cuuint64_t)aCz * 2, (cuuint64_t)ldz * 2};
-  const cuuint32_t box[3] = {aCz, aTileK, aSubQ};
+  static const bool narrow_only = [] { const char* e = getenv("DCP_ATOM_NARROW"); return e && e[0] == '1'; }();   // A-B timing switch
+  const bool wide = p.I % 4 == 0 && !narrow_only;          // whole key groups of 4: 128-byte TMA rows
   const cuuint32_t estr[3] = {1, 1, 1};
-  CUresult r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(z), gdim, gstr, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  CUresult r;
+  if (wide) {
+    const cuuint64_t gdim[3] = {(cuuint64_t)4 * aCz, (cuuint64_t)p.I / 4, (cuuint64_t)p.I};
+    const cuuint64_t gstr[2] = {(cuuint64_t)4 * aCz * 2, (cuuint64_t)ldz * 2};
+    const cuuint32_t box[3] = {4 * aCz, aTileK / 4, aSubQ};
+    r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(z), gdim, gstr, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  } else {
+    const cuuint64_t gdim[3] = {(cuuint64_t)aCz, (cuuint64_t)p.I, (cuuint64_t)p.I};
+    const cuuint64_t gstr[2] = {(cuuint64_t)aCz * 2, (cuuint64_t)ldz * 2};
+    const cuuint32_t box[3] = {aCz, aTileK, aSubQ};
+    r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(z), gdim, gstr, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_32B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  }
   if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
   const int64_t units = mma_num_units<aTileQ>(p.q_end - p.q_begin, p.n_qparts, p.n_kparts, p.nseg);
   if (units > 0x7fffffff) return cudaErrorInvalidValue;
   {   // per-device function attribute: set on every launch (cheap), so a process may use several GPUs
-    cudaError_t e = cudaFuncSetAttribute(fused_atom_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aSmemAlloc);
+    cudaError_t e = cudaFuncSetAttribute(fused_atom_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aSmemAlloc);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(fused_atom_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)aSmemAlloc);
     if (e != cudaSuccess) return e;
   }
   int dev = 0, sms = 0;
@@ -459,7 +525,8 @@ cudaError_t launch_fused_atom(const MmaParams& p, const void* z, int64_t ldz, cu
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   if (sms <= 0) sms = 148;
   const unsigned grid = (unsigned)(units < sms ? units : sms);
-  return launch_kernel(fused_atom_kernel, dim3(grid), dim3(aThreads), aSmemAlloc, st, p.pdl, tm, p);
+  return wide ? launch_kernel(fused_atom_kernel<true>, dim3(grid), dim3(aThreads), aSmemAlloc, st, p.pdl, tm, p)
+              : launch_kernel(fused_atom_kernel<false>, dim3(grid), dim3(aThreads), aSmemAlloc, st, p.pdl, tm, p);
 }
 
 }  // namespace dcp
