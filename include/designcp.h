@@ -258,6 +258,18 @@ dcp_status dcp_plan_units(int64_t I, int H, int c, int c_z, dcp_dtype dtype, dcp
 /* 1 if fused kernel `kernel` (a dcp_kernel, not AUTO) is instantiated for this (dtype, H, c, c_z), else 0. Host only. */
 int dcp_kernel_supported(int kernel, dcp_dtype dtype, int H, int c, int c_z);
 
+/* Measurement probes (bench.py): kernels that compute nothing the method needs and exist to MEASURE the ceilings of the
+ * two rows whose bound is neither HBM nor the tensor pipe.  dcp_probe_l2_gather: n_warps warps each make
+ * gathers_per_warp (a multiple of 8) warp-level 128-bit loads covering two random 256-byte rows of `table`
+ * [n_rows][256 bytes] (device, 16-byte aligned; keep it L2-resident): bytes moved = n_warps * gathers_per_warp * 512 --
+ * the access pattern of the sparse atom attention's K / V gather.  dcp_probe_scan: one warp per query atom of x [L, 3]
+ * scans all L candidates exactly like dcp_knn (binary32 distance in the pinned order, one compare + ballot per 32
+ * candidates from shared-memory tiles) without selecting anything: L * L distance pairs.  `sink`: one device word,
+ * never written in practice.  Both enqueue on `stream`. */
+dcp_status dcp_probe_l2_gather(const void *table, int64_t n_rows, int64_t n_warps, int gathers_per_warp, uint32_t *sink,
+                               void *stream);
+dcp_status dcp_probe_scan(const float *x, int64_t L, uint32_t *sink, void *stream);
+
 /* CUDA-event helpers for callers without a CUDA runtime binding (bench.py): timing-enabled events. */
 dcp_status dcp_event_create(void **ev);
 dcp_status dcp_event_record(void *ev, void *stream);

@@ -32,6 +32,7 @@ EXPORTS = [
     "dcp_pair_transition_workspace_bytes", "dcp_pair_transition",
     "dcp_pairformer_stack_workspace_bytes", "dcp_pairformer_stack",
     "dcp_attention_stack_workspace_bytes", "dcp_attention_stack", "dcp_plan_units",
+    "dcp_probe_l2_gather", "dcp_probe_scan",
     "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
     "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
 ]
@@ -103,7 +104,9 @@ def _load() -> C.CDLL:
     lib.dcp_attention_stack.argtypes = [vp, vp, i64, C.POINTER(dcp_weights), i32, i64, i32, i32, i32, i32, i32, vp, sz, vp]
     lib.dcp_knn_budget.argtypes = [vp, vp, vp, vp, i64, i32, i32, i32, vp]
     lib.dcp_plan_units.argtypes = [i64, i32, i32, i32, i32, i32, C.POINTER(dcp_plan), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
-    for n in EXPORTS[:19]:
+    lib.dcp_probe_l2_gather.argtypes = [vp, i64, i64, i32, vp, vp]
+    lib.dcp_probe_scan.argtypes = [vp, i64, vp, vp]
+    for n in EXPORTS[:21]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -209,6 +212,23 @@ def dcp_plan_units(I, H, c, c_z, dtype: torch.dtype, decomp="monolithic", parts=
     _check(_lib.dcp_plan_units(int(I), H, c, c_z, _dtype_code(dtype), DECOMP[decomp], C.byref(pl), C.byref(a), C.byref(b),
                                C.byref(cc)), "dcp_plan_units")
     return a.value, b.value, cc.value
+
+
+def dcp_probe_l2_gather(table, n_warps, gathers_per_warp, stream=None):
+    """Measurement probe: random 256-byte-row gathers from `table` (uint8 [n_rows * 256], device).  Returns bytes moved."""
+    assert table.is_cuda and table.dtype == torch.uint8 and table.numel() % 256 == 0
+    sink = torch.zeros(1, dtype=torch.int32, device=table.device)
+    _check(_lib.dcp_probe_l2_gather(_ptr(table), table.numel() // 256, int(n_warps), int(gathers_per_warp), _ptr(sink),
+                                    _stream_ptr(stream)), "dcp_probe_l2_gather")
+    return int(n_warps) * int(gathers_per_warp) * 512
+
+
+def dcp_probe_scan(x, stream=None):
+    """Measurement probe: the kNN candidate scan without selection over x [L, 3] fp32.  Returns L * L."""
+    assert x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()
+    sink = torch.zeros(1, dtype=torch.int32, device=x.device)
+    _check(_lib.dcp_probe_scan(_ptr(x), x.shape[0], _ptr(sink), _stream_ptr(stream)), "dcp_probe_scan")
+    return x.shape[0] * x.shape[0]
 
 
 def dcp_kernel_supported(kernel, dtype: torch.dtype, H: int, c: int, c_z: int) -> bool:
