@@ -182,6 +182,20 @@ dcp_status dcp_attention_stack(void *a, const void *z, int64_t ldz, const dcp_we
                                int c_s, int H, int c, int c_z, dcp_dtype dtype, void *workspace, size_t workspace_bytes,
                                void *stream);
 
+/* The same stack with a BIAS CACHE: every block derives its bias LN_b(z) W_b^b from the same read-only
+ * pair tensor, so one pass over z per 15 blocks computes the LayerNorm statistics once per pair and writes every block's
+ * bias as fp16 tiles (H * 2 = 32 bytes per pair and block; PAPER.md:81 materialises B in R^{I x I x H} per block too);
+ * each block then streams its 32 bytes per pair instead of the 256 bytes of z.  Same result as dcp_attention_stack up
+ * to the fp16 rounding of the bias (2^-11 relative, below the bf16 rounding of P that follows).
+ * bias_cache: device, 16-byte aligned, >= dcp_attention_stack_cache_bytes(I, n_blocks) (I = 3000, 18 blocks: 5.2 GB);
+ * it is scratch, valid only during the call.  H = 16, c_z = 128, DCP_BF16, all blocks with the same ln_eps
+ * (DCP_ERR_UNSUPPORTED otherwise).  workspace >= dcp_attention_stack_cached_workspace_bytes. */
+dcp_status dcp_attention_stack_cache_bytes(int64_t I, int n_blocks, size_t *bytes);
+dcp_status dcp_attention_stack_cached_workspace_bytes(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype, size_t *bytes);
+dcp_status dcp_attention_stack_cached(void *a, const void *z, int64_t ldz, const dcp_weights *blocks, int n_blocks, int64_t I,
+                                      int c_s, int H, int c, int c_z, dcp_dtype dtype, void *bias_cache,
+                                      size_t bias_cache_bytes, void *workspace, size_t workspace_bytes, void *stream);
+
 /* p_slice[l, j, :] = p[l, idx[l, j], :] ("The relevant slice of P is gathered at those k indices"): the
  * dense atom-pair tensor p [L, L, c_atompair] (row pitch ldp elements, 0 = L * c_atompair) -> the slice
  * [L, k, c_atompair] that dcp_sparse_atom_attention consumes; slots with idx < 0 are filled with zeros.  Device

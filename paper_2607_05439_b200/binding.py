@@ -33,6 +33,7 @@ EXPORTS = [
     "dcp_pairformer_stack_workspace_bytes", "dcp_pairformer_stack",
     "dcp_attention_stack_workspace_bytes", "dcp_attention_stack", "dcp_plan_units",
     "dcp_probe_l2_gather", "dcp_probe_scan",
+    "dcp_attention_stack_cache_bytes", "dcp_attention_stack_cached_workspace_bytes", "dcp_attention_stack_cached",
     "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
     "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
 ]
@@ -106,7 +107,10 @@ def _load() -> C.CDLL:
     lib.dcp_plan_units.argtypes = [i64, i32, i32, i32, i32, i32, C.POINTER(dcp_plan), C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
     lib.dcp_probe_l2_gather.argtypes = [vp, i64, i64, i32, vp, vp]
     lib.dcp_probe_scan.argtypes = [vp, i64, vp, vp]
-    for n in EXPORTS[:21]:
+    lib.dcp_attention_stack_cache_bytes.argtypes = [i64, i32, C.POINTER(sz)]
+    lib.dcp_attention_stack_cached_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, i32, C.POINTER(sz)]
+    lib.dcp_attention_stack_cached.argtypes = [vp, vp, i64, C.POINTER(dcp_weights), i32, i64, i32, i32, i32, i32, i32, vp, sz, vp, sz, vp]
+    for n in EXPORTS[:24]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -339,6 +343,35 @@ def dcp_attention_stack(a, z, blocks, H, c, eps=1e-5, workspace=None, stream=Non
     st = _lib.dcp_attention_stack(_ptr(a), _ptr(z), int(ldz), arr, len(blocks), I, c_s, H, c, c_z, _dtype_code(a.dtype),
                                   _ptr(workspace), workspace.numel(), _stream_ptr(stream))
     _check(st, "dcp_attention_stack")
+    return a
+
+
+def dcp_attention_stack_cache_bytes(I, n_blocks) -> int:
+    n = C.c_size_t(0)
+    _check(_lib.dcp_attention_stack_cache_bytes(int(I), int(n_blocks), C.byref(n)), "dcp_attention_stack_cache_bytes")
+    return int(n.value)
+
+
+def dcp_attention_stack_cached(a, z, blocks, H, c, eps=1e-5, bias_cache=None, workspace=None, stream=None, ldz=0):
+    """dcp_attention_stack with a bias cache: one pass over z writes every block's bias tiles (fp16), the blocks then
+    stream 32 bytes per pair each.  bias_cache: device uint8 scratch of dcp_attention_stack_cache_bytes(I, n) bytes."""
+    assert a.is_cuda and z.is_cuda and a.is_contiguous() and z.dtype == a.dtype
+    I, c_s, c_z = a.shape[0], a.shape[1], z.shape[-1]
+    assert z.stride(-1) == 1 and z.stride(1) == c_z and (ldz or z.stride(0) == I * c_z), "z: inner dimensions not contiguous"
+    arr = (dcp_weights * len(blocks))()
+    for b, w in enumerate(blocks):
+        arr[b] = _weights_struct(w, eps, a.dtype)
+    if bias_cache is None:
+        bias_cache = _alloc_ws(dcp_attention_stack_cache_bytes(I, len(blocks)), a.device, stream)
+    if workspace is None:
+        n = C.c_size_t(0)
+        _check(_lib.dcp_attention_stack_cached_workspace_bytes(I, c_s, H, c, c_z, _dtype_code(a.dtype), C.byref(n)),
+               "dcp_attention_stack_cached_workspace_bytes")
+        workspace = _alloc_ws(int(n.value), a.device, stream)
+    st = _lib.dcp_attention_stack_cached(_ptr(a), _ptr(z), int(ldz), arr, len(blocks), I, c_s, H, c, c_z, _dtype_code(a.dtype),
+                                         _ptr(bias_cache), bias_cache.numel(), _ptr(workspace), workspace.numel(),
+                                         _stream_ptr(stream))
+    _check(st, "dcp_attention_stack_cached")
     return a
 
 

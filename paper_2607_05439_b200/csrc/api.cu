@@ -265,7 +265,9 @@ dcp_status validate_weights(const dcp_weights* w) {
 
 dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w, void* out, int64_t I, int c_s, int H,
                  int c, int c_z, dcp_dtype dt, dcp_decomp decomp, const dcp_plan* plan_in, void* workspace,
-                 size_t workspace_bytes, void* stream, const void* residual = nullptr) {
+                 size_t workspace_bytes, void* stream, const void* residual = nullptr, const uint32_t* bias_cache = nullptr) {
+  // bias_cache != nullptr: this block's bias tiles (bias_tiles.cu) replace the LayerNorm + projection of z (token kernel,
+  // MONOLITHIC, 32-row tiles)
   // residual != nullptr: out = storage(residual + layer output), added in fp32 inside the W_o GEMM's epilogue (tensor-core
   // path with a tcgen05-shaped W_o only: DCP_ERR_UNSUPPORTED otherwise); residual may be `out`
   g_launches = 0;
@@ -305,10 +307,12 @@ dcp_status layer(const void* s, const void* z, int64_t ldz, const dcp_weights* w
     mp.q_begin = 0; mp.q_end = (int)I; mp.n_qparts = plan.decomp == DCP_GRID ? plan.G : plan.parts;
     mp.k_begin = 0; mp.k_end = (int)I; mp.n_kparts = plan.key_split;
     mp.nseg = plan.nseg; mp.slot0 = 0; mp.tile_h = plan.tile_h;
+    mp.bias_cache = bias_cache;
     mp.pdl = pdl_enabled() && plan.ev_begin == nullptr;   // an event record between two launches would serialise them anyway
     if (plan.ev_begin && cudaEventRecord(plan.ev_begin, x.st) != cudaSuccess) return DCP_ERR_CUDA;
     DCP_CUDA(launch_fused_mma(mp, z, ldz, x.st));
   } else {
+  if (bias_cache != nullptr) return DCP_ERR_UNSUPPORTED;
   st = run_prologue(x, s);
   if (st != DCP_OK) return st;
 
@@ -620,6 +624,68 @@ dcp_status dcp_attention_stack(void* a, const void* z, int64_t ldz, const dcp_we
       if (cudaGetLastError() != cudaSuccess) return DCP_ERR_CUDA;
       ++launches;
     }
+    if (st != DCP_OK) return st;
+    launches += g_launches;
+  }
+  g_launches = launches;
+  return DCP_OK;
+}
+
+// ---- the same stack with a bias cache: one pass over z per 15 blocks writes every block's bias tiles, then each block
+// streams 32 bytes per pair instead of 256
+dcp_status dcp_attention_stack_cache_bytes(int64_t I, int n_blocks, size_t* bytes) {
+  if (!bytes || I <= 0 || n_blocks <= 0) return DCP_ERR_INVALID_ARG;
+  *bytes = (size_t)n_blocks * (size_t)bias_tiles_block_words(I) * 4;
+  return DCP_OK;
+}
+
+dcp_status dcp_attention_stack_cached_workspace_bytes(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype, size_t* bytes) {
+  size_t base = 0;
+  dcp_status st = dcp_attention_stack_workspace_bytes(I, c_s, H, c, c_z, dtype, &base);
+  if (st != DCP_OK) return st;
+  if (H != 16 || c_z != 128) return DCP_ERR_UNSUPPORTED;
+  *bytes = base + align256(bias_tiles_fold_bytes(bias_tiles_max_blocks()));
+  return DCP_OK;
+}
+
+dcp_status dcp_attention_stack_cached(void* a, const void* z, int64_t ldz, const dcp_weights* blocks, int n_blocks, int64_t I,
+                                      int c_s, int H, int c, int c_z, dcp_dtype dtype, void* bias_cache, size_t bias_cache_bytes,
+                                      void* workspace, size_t workspace_bytes, void* stream) {
+  g_launches = 0;
+  if (!a || !z || !blocks || !workspace || !bias_cache || n_blocks <= 0) return DCP_ERR_INVALID_ARG;
+  size_t need = 0, base = 0, attn = 0, cache_need = 0;
+  dcp_status st = dcp_attention_stack_cached_workspace_bytes(I, c_s, H, c, c_z, dtype, &need);
+  if (st != DCP_OK) return st;
+  dcp_attention_stack_cache_bytes(I, n_blocks, &cache_need);
+  if (workspace_bytes < need || bias_cache_bytes < cache_need) return DCP_ERR_WORKSPACE;
+  if (((uintptr_t)workspace & 255) != 0 || ((uintptr_t)bias_cache & 15) != 0 || ((uintptr_t)z & 15) != 0 || (I * c_s) % 8 != 0)
+    return DCP_ERR_INVALID_ARG;
+  if (ldz == 0) ldz = I * (int64_t)c_z;
+  if (ldz < I * (int64_t)c_z || (ldz * 2) % 16 != 0) return DCP_ERR_INVALID_ARG;
+  for (int b = 0; b < n_blocks; ++b) {
+    if (validate_weights(&blocks[b]) != DCP_OK) return DCP_ERR_INVALID_ARG;
+    if ((blocks[b].ln_eps > 0.f ? blocks[b].ln_eps : 1e-5f) != (blocks[0].ln_eps > 0.f ? blocks[0].ln_eps : 1e-5f))
+      return DCP_ERR_UNSUPPORTED;                            // one set of LayerNorm statistics serves every block of a pass
+  }
+  dcp_attention_stack_workspace_bytes(I, c_s, H, c, c_z, dtype, &base);
+  dcp_workspace_bytes(I, c_s, H, c, c_z, dtype, DCP_MONOLITHIC, nullptr, &attn);
+  char* ws = reinterpret_cast<char*>(workspace);
+  void* fold_ws = ws + base;
+  const float eps = blocks[0].ln_eps > 0.f ? blocks[0].ln_eps : 1e-5f;
+  const int64_t bw = bias_tiles_block_words(I);
+  int launches = 0;
+  for (int b0 = 0; b0 < n_blocks; b0 += bias_tiles_max_blocks()) {
+    const int nb = std::min(n_blocks - b0, bias_tiles_max_blocks());
+    if (launch_bias_tiles(z, ldz, I, blocks + b0, nb, eps, fold_ws, reinterpret_cast<uint32_t*>(bias_cache) + (int64_t)b0 * bw,
+                          (cudaStream_t)stream) != cudaSuccess)
+      return DCP_ERR_CUDA;
+    launches += 2;
+  }
+  dcp_plan plan{};
+  plan.parts = 1; plan.key_split = 1; plan.kernel = DCP_KERNEL_MMA; plan.tile_q = 32;   // tiles aligned with the cache's
+  for (int b = 0; b < n_blocks; ++b) {
+    st = layer(a, z, ldz, &blocks[b], a, I, c_s, H, c, c_z, dtype, DCP_MONOLITHIC, &plan, ws, attn, stream, a,
+               reinterpret_cast<const uint32_t*>(bias_cache) + (int64_t)b * bw);
     if (st != DCP_OK) return st;
     launches += g_launches;
   }

@@ -1,0 +1,245 @@
+// Bias cache for the attention stack on a read-only pair tensor ("cached" mode).
+// Every block b of the stack derives its own bias  LN_b(z_ij) W_b^b  from the SAME pair tensor; one pass over z computes
+// the biases of up to 15 blocks at once -- LayerNorm statistics once per pair, one tcgen05 projection with
+// N = 16 heads x n_blocks + the ones column -- and writes them as fp16 tiles in exactly the layout the attention kernel
+// consumes ([query tile of 32][key tile of 16][head pair][32 queries][16 keys] half2, 16 KB per tile), so that each block
+// afterwards streams 32 bytes per pair instead of the 256 bytes of z (the paper's own stack materialises
+// B in R^{I x I x H} per block).  Values are in the exp2 domain (W' carries log2 e), like the fused kernel's.
+//
+// One persistent CTA per SM, 8 warps: warp 0 TMA producer (z boxes as in fused_mma.cu), warps 1-2 tcgen05 issuers
+// (stage n -> issuer n % 2), warps 4-7 statistics + epilogue (thread = pair).
+#include "fold.cuh"
+#include "kernels.h"
+#include "mma_ptx.cuh"
+
+namespace dcp {
+
+namespace {
+
+constexpr int bCz = 128, bH = 16, bTileQ = 32, bTileK = 16, bSubQ = 8, bNZ = 3, bNT = 2;
+constexpr int bStageBytes = bSubQ * bTileK * bCz * 2;      // 32 KB
+constexpr int bHalfBytes = bStageBytes / 2;
+constexpr int bMaxBlocks = 15;                              // 16 * 15 + 16 = 256 projection columns
+constexpr int bMaxN = 256;
+constexpr int bThreads = 256;
+constexpr size_t bSmemZ = 0;
+constexpr size_t bSmemWt = bSmemZ + (size_t)bNZ * bStageBytes;            // 2 halves x 256 rows x 128 B = 64 KB
+constexpr size_t bSmemC = bSmemWt + 2 * (size_t)bMaxN * 128;              // c1, c0: [15][16] floats each
+constexpr size_t bSmemBar = bSmemC + 2 * bMaxBlocks * bH * 4;
+constexpr size_t bSmemAlloc = bSmemBar + (2 * bNZ + 2 * bNT) * 8 + 16 + 1024;
+
+struct BiasTilesParams {
+  const void* wfold;       // [n_blocks][16][128] bf16
+  const float* c1;         // [n_blocks][16]
+  const float* c0;         // [n_blocks][16]
+  uint32_t* cache;         // block b: cache + b * block_words; tile (qt, kt): + ((qt * KT + kt) * 8 + hp) * 512 + q * 16 + key
+  int64_t block_words;
+  int I, n_blocks, KT, n_tiles;
+  float eps;
+};
+
+__global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_constant__ CUtensorMap tmap_z, const BiasTilesParams p) {
+  extern __shared__ unsigned char smem_dyn[];
+  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
+  const uint32_t s_z = smem_u32(smem + bSmemZ), s_wt = smem_u32(smem + bSmemWt), s_bar = smem_u32(smem + bSmemBar);
+  float* s_c1 = reinterpret_cast<float*>(smem + bSmemC);
+  float* s_c0 = s_c1 + bMaxBlocks * bH;
+  const uint32_t bar_zfull = s_bar, bar_zempty = s_bar + 8 * bNZ, bar_tfull = s_bar + 16 * bNZ, bar_tempty = bar_tfull + 8 * bNT;
+  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + bSmemBar + (2 * bNZ + 2 * bNT) * 8);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int NP = 16 * p.n_blocks + 16;                       // projection columns: heads of every block, ones, zero rows
+
+  pdl_trigger();
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < bNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + 4); }
+    for (int b = 0; b < bNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), 512);
+  pdl_wait();
+  // W'': row n < 16 nb = head n % 16 of block n / 16, row 16 nb = ones, others 0; K-major, 128-byte swizzle by hand
+  for (int e = threadIdx.x; e < NP * (bCz / 8); e += bThreads) {
+    const int n = e / (bCz / 8), ch16 = e % (bCz / 8);
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (n < 16 * p.n_blocks) v = __ldg(reinterpret_cast<const uint4*>(p.wfold) + n * (bCz / 8) + ch16);
+    else if (n == 16 * p.n_blocks) v = make_uint4(0x3f803f80u, 0x3f803f80u, 0x3f803f80u, 0x3f803f80u);
+    const int half = ch16 >> 3, c = ch16 & 7;
+    *reinterpret_cast<uint4*>(smem + bSmemWt + half * (bMaxN * 128) + n * 128 + ((c ^ (n & 7)) << 4)) = v;
+  }
+  for (int e = threadIdx.x; e < p.n_blocks * bH; e += bThreads) { s_c1[e] = __ldg(p.c1 + e); s_c0[e] = __ldg(p.c0 + e); }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *s_tmem;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      // =============================================================== TMA producer
+      uint64_t policy;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+      uint32_t it = 0;
+      for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
+        const int q0 = (tile / p.KT) * bTileQ, j0 = (tile % p.KT) * bTileK;
+        for (int sub = 0; sub < bTileQ / bSubQ; ++sub, ++it) {
+          const int stage = it % bNZ;
+          mbar_wait(bar_zempty + 8 * stage, ((it / bNZ) & 1) ^ 1);
+          mbar_expect_tx(bar_zfull + 8 * stage, bStageBytes);
+          const uint32_t dst = s_z + stage * bStageBytes;
+          tma_load_3d(dst, &tmap_z, 0, j0, q0 + sub * bSubQ, bar_zfull + 8 * stage, policy);
+          tma_load_3d(dst + bHalfBytes, &tmap_z, 64, j0, q0 + sub * bSubQ, bar_zfull + 8 * stage, policy);
+        }
+      }
+    }
+  } else if (warp <= 3) {
+    if (warp <= 2 && lane == 0) {
+      // =============================================================== tcgen05 issuers (stage n -> issuer n % 2: with two
+      // accumulator buffers a buffer's consecutive users are then the same thread, so its parity waits cannot alias)
+      const uint32_t idesc = umma_idesc_bf16(128, NP);
+      const uint32_t me = warp - 1;
+      uint32_t it = 0;
+      for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
+        for (int sub = 0; sub < bTileQ / bSubQ; ++sub, ++it) {
+          if (it % 2 != me) continue;
+          const int stage = it % bNZ, tb = it % bNT;
+          mbar_wait(bar_tempty + 8 * tb, ((it / bNT) & 1) ^ 1);
+          mbar_wait(bar_zfull + 8 * stage, (it / bNZ) & 1);
+          tc_fence_after();
+          const uint32_t zs = s_z + stage * bStageBytes;
+#pragma unroll
+          for (int ks = 0; ks < 8; ++ks)
+            umma_bf16(tmem_base + tb * bMaxN, umma_desc_sw128(zs + (ks >> 2) * bHalfBytes + (ks & 3) * 32),
+                      umma_desc_sw128(s_wt + (ks >> 2) * (bMaxN * 128) + (ks & 3) * 32), idesc, ks > 0);
+          umma_commit(bar_zempty + 8 * stage);
+          umma_commit(bar_tfull + 8 * tb);
+        }
+      }
+    }
+  } else {
+    // =============================================================== LayerNorm statistics + epilogue, thread = pair
+    const int pw = warp - 4;
+    const uint32_t t_lane = tmem_base + ((uint32_t)(pw * 32) << 16);
+    const int prow = pw * 32 + lane;
+    const uint32_t zrow = s_z + prow * 128, zsw = (uint32_t)(prow & 7);
+    uint32_t it = 0;
+    for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
+      for (int sub = 0; sub < bTileQ / bSubQ; ++sub, ++it) {
+        const int stage = it % bNZ, tb = it % bNT;
+        mbar_wait(bar_zfull + 8 * stage, (it / bNZ) & 1);
+        float sq0 = 0.f, sq1 = 0.f, sq2 = 0.f, sq3 = 0.f;
+        const uint32_t zr = zrow + stage * bStageBytes;
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+          uint4 w[8];
+#pragma unroll
+          for (int c = 0; c < 8; ++c) w[c] = lds_u32x4(zr + half * bHalfBytes + ((c ^ zsw) << 4));
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            fma_sq_bf16x2(sq0, sq1, w[c].x); fma_sq_bf16x2(sq2, sq3, w[c].y);
+            fma_sq_bf16x2(sq0, sq1, w[c].z); fma_sq_bf16x2(sq2, sq3, w[c].w);
+          }
+        }
+        float zsq = (sq0 + sq1) + (sq2 + sq3);
+        asm volatile("" : "+f"(zsq));
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_zempty + 8 * stage);
+        mbar_wait(bar_tfull + 8 * tb, (it / bNT) & 1);
+        tc_fence_after();
+        const uint32_t t_p = t_lane + tb * bMaxN;
+        const float zsum = tmem_ld_x1(t_p + 16 * p.n_blocks);
+        tmem_ld_wait();
+        const float mu = zsum * (1.f / bCz);
+        const float var = fmaf(-mu, mu, zsq * (1.f / bCz));      // one rounding; exactly 0 for a constant row (fused_mma.cu)
+        const float rstd = var > 0.f ? rsqrtf(var + p.eps) : 0.f;
+        const float nm = -mu * rstd;
+        uint32_t* dst = p.cache + (int64_t)tile * (8 * 512) + sub * (bSubQ * bTileK) + prow;
+        for (int b = 0; b < p.n_blocks; ++b) {
+          float acc[16];
+          tmem_ld_x16(t_p + 16 * b, acc);
+          tmem_ld_wait();
+          const float* c1 = s_c1 + b * bH;
+          const float* c0 = s_c0 + b * bH;
+#pragma unroll
+          for (int hp = 0; hp < 8; ++hp)
+            dst[(int64_t)b * p.block_words + hp * 512] =
+                pack_f16(fmaf(acc[2 * hp], rstd, fmaf(nm, c1[2 * hp], c0[2 * hp])),
+                         fmaf(acc[2 * hp + 1], rstd, fmaf(nm, c1[2 * hp + 1], c0[2 * hp + 1])));
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_tempty + 8 * tb);
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    __syncwarp();
+    tmem_dealloc(tmem_base, 512);
+  }
+}
+
+struct FoldAllParams {
+  const void* w_b[bMaxBlocks];
+  const void* gamma[bMaxBlocks];
+  const void* beta[bMaxBlocks];
+  void* wfold;
+  float *c1, *c0;
+};
+__global__ void __launch_bounds__(256) fold_all_kernel(const FoldAllParams f) {
+  pdl_trigger();
+  pdl_wait();
+  const int b = blockIdx.x;
+  fold_ln_z_mma_device(f.w_b[b], f.gamma[b], f.beta[b], reinterpret_cast<__nv_bfloat16*>(f.wfold) + (size_t)b * bH * bCz,
+                       f.c1 + b * bH, f.c0 + b * bH, bCz, bH, bH, threadIdx.x, 256);
+}
+
+}  // namespace
+
+int bias_tiles_max_blocks() { return bMaxBlocks; }
+int64_t bias_tiles_block_words(int64_t I) { return ((I + bTileQ - 1) / bTileQ) * ((I + bTileK - 1) / bTileK) * 8 * 512; }
+size_t bias_tiles_fold_bytes(int n_blocks) { return (size_t)n_blocks * (bH * bCz * 2 + 2 * bH * 4) + 512; }
+
+// Biases of blocks [0, n_blocks) (n_blocks <= 15) of one pass: fold (one small launch) + the streaming kernel.
+cudaError_t launch_bias_tiles(const void* z, int64_t ldz, int64_t I, const dcp_weights* blocks, int n_blocks, float eps,
+                              void* fold_ws, void* cache, cudaStream_t st) {
+  if (n_blocks < 1 || n_blocks > bMaxBlocks) return cudaErrorInvalidValue;
+  PFN_cuTensorMapEncodeTiled enc = get_encode_fn();
+  if (!enc) return cudaErrorNotSupported;
+  FoldAllParams f{};
+  for (int b = 0; b < n_blocks; ++b) { f.w_b[b] = blocks[b].w_b; f.gamma[b] = blocks[b].ln_z_gamma; f.beta[b] = blocks[b].ln_z_beta; }
+  char* ws = reinterpret_cast<char*>(fold_ws);
+  f.wfold = ws;
+  f.c1 = reinterpret_cast<float*>(ws + ((size_t)n_blocks * bH * bCz * 2 + 255) / 256 * 256);
+  f.c0 = f.c1 + n_blocks * bH;
+  cudaError_t e = launch_kernel(fold_all_kernel, dim3(n_blocks), dim3(256), 0, st, true, f);
+  if (e != cudaSuccess) return e;
+  CUtensorMap tm;
+  const cuuint64_t gdim[3] = {(cuuint64_t)bCz, (cuuint64_t)I, (cuuint64_t)I};
+  const cuuint64_t gstr[2] = {(cuuint64_t)bCz * 2, (cuuint64_t)ldz * 2};
+  const cuuint32_t box[3] = {64, bTileK, bSubQ};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  if (enc(&tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(z), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+    return cudaErrorInvalidValue;
+  BiasTilesParams p{};
+  p.wfold = f.wfold; p.c1 = f.c1; p.c0 = f.c0;
+  p.cache = reinterpret_cast<uint32_t*>(cache);
+  p.block_words = bias_tiles_block_words(I);
+  p.I = (int)I; p.n_blocks = n_blocks;
+  p.KT = (int)((I + bTileK - 1) / bTileK);
+  const int64_t n_tiles = ((I + bTileQ - 1) / bTileQ) * p.KT;
+  if (n_tiles > 0x7fffffff) return cudaErrorInvalidValue;
+  p.n_tiles = (int)n_tiles;
+  p.eps = eps;
+  e = cudaFuncSetAttribute(bias_tiles_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bSmemAlloc);
+  if (e != cudaSuccess) return e;
+  int dev = 0, sms = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (sms <= 0) sms = 148;
+  const unsigned grid = (unsigned)(n_tiles < sms ? n_tiles : sms);
+  return launch_kernel(bias_tiles_kernel, dim3(grid), dim3(bThreads), bSmemAlloc, st, true, tm, p);
+}
+
+}  // namespace dcp

@@ -74,12 +74,14 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
+  const bool cached = p.bias_cache != nullptr;               // bias tiles come from the cache (bias_tiles.cu), z is not read
 
   pdl_trigger();
   if (threadIdx.x == 0) {
     // zempty / tfull are arrived on by tcgen05.commit (the MMAs that read the stage / wrote the accumulators are done)
     for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + kNumProjWarps); }
-    for (int b = 0; b < 2; ++b) { mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps); }
+    // bfull: the four epilogue warps -- or, with a bias cache, the producer's expect_tx arrival + the bulk copy's bytes
+    for (int b = 0; b < 2; ++b) { mbar_init(bar_bfull + 8 * b, cached ? 1 : kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps); }
     for (int b = 0; b < kNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, kNumProjWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -87,7 +89,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   pdl_wait();          // the prologue's q / k / v / folded weights are final (and so is everything before it in the stream)
   // W'' = B operand of the projection MMA, K-major, 128-byte swizzled by hand: row n < 16 = head n of
   // (gamma (.) W_b log2 e)^T, row 16 = ones (its accumulator column is sum_k z), rows 17..31 = 0.
-  for (int e = threadIdx.x; e < kProjN * (kCz / 8); e += kThreads) {
+  for (int e = threadIdx.x; e < (cached ? 0 : kProjN * (kCz / 8)); e += kThreads) {
     const int n = e / (kCz / 8), ch16 = e % (kCz / 8);          // 16-byte chunk = 8 channels
     uint4 v = make_uint4(0u, 0u, 0u, 0u);
     if (n < kH) v = __ldg(reinterpret_cast<const uint4*>(p.wfold) + n * (kCz / 8) + ch16);
@@ -106,7 +108,25 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   if (warp < kProjWarp0) {
     // =============================================================== TMA producer (warp 0, one lane)
     reg_dec<24>();
-    if (warp == 0 && lane == 0) {
+    if (warp == 0 && lane == 0 && cached) {
+      // bias cache: one 16 KB tile [head pair][32 queries][16 keys] half2 per (query tile, key tile), by one bulk copy
+      const int KT = (p.I + kTileK - 1) / kTileK;
+      int bbuf = 0;
+      uint32_t bphase = 0;
+      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+        const Unit un = decode_unit<0, kTileK>(p, u);
+        for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
+          mbar_wait(bar_bempty + 8 * bbuf, bphase ^ 1);
+          mbar_expect_tx(bar_bfull + 8 * bbuf, (kH / 2) * kTileQ * kTileK * 4);
+          const uint32_t* src = p.bias_cache + ((int64_t)(un.q0 / kTileQ) * KT + (j0 / kTileK)) * ((kH / 2) * kTileQ * kTileK);
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                       ::"r"(smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4)), "l"(src), "r"((kH / 2) * kTileQ * kTileK * 4),
+                         "r"(bar_bfull + 8 * bbuf) : "memory");
+          bbuf ^= 1;
+          if (bbuf == 0) bphase ^= 1;
+        }
+      }
+    } else if (warp == 0 && lane == 0) {
       uint64_t policy;
       asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
       int stage = 0;
@@ -133,7 +153,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           }
         }
       }
-    } else if (warp >= 1 && warp <= kNumIssuers && lane == 0) {
+    } else if (warp >= 1 && warp <= kNumIssuers && lane == 0 && !cached) {
       // ============================================================= tcgen05 issuers (one thread each, warps 1..3)
       // A K = 16 projection MMA costs its issuing thread ~130 cycles whatever N is (the 4 KB A-operand fetch), eight of
       // them per 32 KB stage: one thread alone needs ~1050 of the ~1450 cycles a stage may take at the HBM bound, and
@@ -195,7 +215,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     const uint32_t zsw = (uint32_t)(prow & 7);
     int tb = 0, bbuf = 0, stage = 0;
     uint32_t tphase = 0, bphase = 0, zphase = 0;
-    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
+    for (int u = blockIdx.x; u < (cached ? 0 : n_units); u += gridDim.x) {
       const Unit un = decode_unit<0, kTileK>(p, u);
       const int rows = (un.q_end - un.q0) < p.tile_h ? (un.q_end - un.q0) : p.tile_h;
       const int nsub = (rows + kSubQ - 1) / kSubQ;
@@ -343,6 +363,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
         const int jn = j0 + kTileK < un.ke ? j0 + kTileK : (next_first >= 0 ? next_first : j0);
         mbar_wait(bar_bfull + 8 * bbuf, bphase);
         const uint32_t bias_buf = smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4) + (g * kTileK + 4 * t) * 4;
+        const uint32_t bias_c = bias_buf + aw * (kTileQ * kTileK * 4);       // cached: this warp's head pair plane
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
           const int h = 2 * aw + hh;
@@ -350,10 +371,18 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           float sA[2][4], sB[2][4];
 #pragma unroll
           for (int mb = 0; mb < 2; ++mb) {
-            const float4 b0 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + mb * 16 * kTileK) * 4);
-            const float4 b1 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + (mb * 16 + 8) * kTileK) * 4);
-            sA[mb][0] = b0.x; sA[mb][1] = b0.y; sA[mb][2] = b1.x; sA[mb][3] = b1.y;
-            sB[mb][0] = b0.z; sB[mb][1] = b0.w; sB[mb][2] = b1.z; sB[mb][3] = b1.w;
+            if (cached) {
+              // word j of the 16 bytes = (head 2 aw, head 2 aw + 1) of key 4 t + j, fp16
+              const uint4 b0 = lds_u32x4(bias_c + (mb * 16 * kTileK) * 4);
+              const uint4 b1 = lds_u32x4(bias_c + ((mb * 16 + 8) * kTileK) * 4);
+              sA[mb][0] = f16_half(b0.x, hh); sA[mb][1] = f16_half(b0.y, hh); sA[mb][2] = f16_half(b1.x, hh); sA[mb][3] = f16_half(b1.y, hh);
+              sB[mb][0] = f16_half(b0.z, hh); sB[mb][1] = f16_half(b0.w, hh); sB[mb][2] = f16_half(b1.z, hh); sB[mb][3] = f16_half(b1.w, hh);
+            } else {
+              const float4 b0 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + mb * 16 * kTileK) * 4);
+              const float4 b1 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + (mb * 16 + 8) * kTileK) * 4);
+              sA[mb][0] = b0.x; sA[mb][1] = b0.y; sA[mb][2] = b1.x; sA[mb][3] = b1.y;
+              sB[mb][0] = b0.z; sB[mb][1] = b0.w; sB[mb][2] = b1.z; sB[mb][3] = b1.w;
+            }
           }
 #pragma unroll
           for (int kk = 0; kk < KK; ++kk)
@@ -553,8 +582,9 @@ void mma_pick_units(int64_t I, int H, int n_qparts, int n_kparts, int force_nseg
 }
 
 cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st) {
-  if (p.H != kH) return launch_fused_atom(p, z, ldz, st);
+  if (p.H != kH) return p.bias_cache ? cudaErrorInvalidValue : launch_fused_atom(p, z, ldz, st);
   if (p.q_end <= p.q_begin || p.k_end <= p.k_begin) return cudaSuccess;
+  if (p.bias_cache && (p.q_begin != 0 || p.n_qparts != 1 || p.tile_h != kTileQ)) return cudaErrorInvalidValue;
   PFN_cuTensorMapEncodeTiled enc = get_encode_fn();
   if (!enc) return cudaErrorNotSupported;
   CUtensorMap tm;

@@ -83,6 +83,10 @@ struct MmaParams {
   int tile_h;           // fused_mma_kernel: query rows per work unit (25..32; the atom kernel's tile is fixed)
   int H, c, c_z;
   float eps;
+  // fused_mma_kernel only, optional: the bias of this call comes from a cache (bias_tiles.cu) instead of z -- the TMA
+  // producer copies one 16 KB fp16 tile per (32-query tile, 16-key tile) into the bias buffer; z is not touched.
+  // Needs q_begin == 0, n_qparts == 1, tile_h == 32 (tiles aligned with the cache's).
+  const uint32_t* bias_cache;
   bool pdl;             // host only: launch as a programmatic dependent of the previous kernel in the stream
 };
 cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st);
@@ -122,6 +126,14 @@ size_t pair_transition_workspace_bytes();
 cudaError_t launch_pair_transition(const void* z_in, void* z_out, int64_t n_pairs, const void* w1, const void* w2,
                                    const void* w3, const void* gamma, const void* beta, float eps, void* workspace,
                                    cudaStream_t st);
+
+// Bias cache of the attention stack (bias_tiles.cu): the biases LN_b(z) W_b^b of up to bias_tiles_max_blocks() blocks in one
+// pass over z, as fp16 tiles in the layout fused_mma_kernel consumes when MmaParams.bias_cache is set
+int bias_tiles_max_blocks();
+int64_t bias_tiles_block_words(int64_t I);          // 32-bit words of one block's cache
+size_t bias_tiles_fold_bytes(int n_blocks);         // scratch for the folded weights of a pass
+cudaError_t launch_bias_tiles(const void* z, int64_t ldz, int64_t I, const dcp_weights* blocks, int n_blocks, float eps,
+                              void* fold_ws, void* cache, cudaStream_t st);
 
 // Merge (step a8) + normalise + gate (first half of a9); or raw merged state out.
 cudaError_t launch_merge(dcp_dtype dt, const MergeParams& p, cudaStream_t st);

@@ -145,3 +145,66 @@ def test_attention_stack_error_paths():
     assert e.value.status == 2
     out = dcp.dcp_attention_stack(a, z, blocks, cfg.H, cfg.c)
     assert torch.isfinite(out.float()).all()
+
+
+# ------------------------------------------------------------------ the same stack with a bias cache
+@pytest.mark.parametrize("I,copies,c,n_blocks", [
+    (96, 12, 48, 1),
+    (75, 15, 48, 3),       # ragged I: the last query / key tiles of the cache are partly out of range
+    (131, 1, 24, 4),
+    (60, 60, 48, 18),      # two passes over z (15 + 3 blocks)
+    (300, 60, 32, 16),
+])
+def test_attention_stack_cached_matches_oracle_and_streaming(I, copies, c, n_blocks):
+    """One pass over z writes every block's bias tiles (fp16), the blocks then read those: per block from the oracle's
+    latent at the same bounds as the streaming stack, and the chain close to the streaming call (they differ by the
+    fp16 rounding of the bias only)."""
+    dcp = _dcp()
+    c_s = 768 if c == 48 else 384
+    cfg = syn.small_config("cstack", I=I, c_s=c_s, c_z=128, H=16, c=c, dtype="bf16", seed=31 + I, structured=copies > 1,
+                           copies=copies)
+    a0, z = syn.make_s(cfg, DEV), syn.make_z(cfg, DEV)
+    z_before = z.clone()
+    blocks = _blocks(cfg, n_blocks, "all")
+    ob = [util.weights_np(w) for w in blocks]
+    zn = util.np64(z)
+    a_ref = util.np64(a0)
+    for b in range(n_blocks):
+        a_in = a_ref
+        a_ref = aso.attention_stack(a_in, zn, ob[b:b + 1], cfg.H, cfg.c, round_store=_bf)
+        a1 = torch.from_numpy(a_in).to(torch.bfloat16).to(DEV)
+        dcp.dcp_attention_stack_cached(a1, z, blocks[b:b + 1], cfg.H, cfg.c)
+        got = util.np64(a1)
+        upd_ref = a_ref - a_in
+        rel = np.linalg.norm((got - a_in) - upd_ref) / np.linalg.norm(upd_ref)
+        assert rel <= 2e-2, f"block {b}: update rel-L2 {rel:.3e}"
+        rms = max(1.0, float(np.sqrt(np.mean(upd_ref ** 2))))
+        bad = np.abs(got - a_ref) > util.TOL_BF16_MAXABS * rms + 2.0 ** -7 * np.abs(a_ref)
+        assert not bad.any(), f"block {b}: {bad.sum()} elements out of tolerance, max-abs {np.abs(got - a_ref).max():.3e}"
+    a_c, a_s = a0.clone(), a0.clone()
+    dcp.dcp_attention_stack_cached(a_c, z, blocks, cfg.H, cfg.c)
+    dcp.dcp_attention_stack(a_s, z, blocks, cfg.H, cfg.c)
+    torch.cuda.synchronize()
+    assert torch.equal(z, z_before)
+    gc, gs = util.np64(a_c), util.np64(a_s)
+    assert np.all(np.isfinite(gc))
+    assert np.linalg.norm(gc - a_ref) / np.linalg.norm(a_ref) <= n_blocks * util.TOL_BF16_RELL2
+    assert np.linalg.norm(gc - gs) / np.linalg.norm(gs) <= n_blocks * 2e-3, "cached and streaming stacks drift apart"
+    again = a0.clone()
+    dcp.dcp_attention_stack_cached(again, z, blocks, cfg.H, cfg.c)
+    assert torch.equal(again, a_c)
+
+
+def test_attention_stack_cached_error_paths():
+    dcp = _dcp()
+    cfg = syn.small_config("cserr", I=64, c_s=768, c_z=128, H=16, c=48, dtype="bf16", seed=5)
+    a, z = syn.make_s(cfg, DEV), syn.make_z(cfg, DEV)
+    blocks = _blocks(cfg, 2)
+    with pytest.raises(dcp.DcpError) as e:                 # cache too small
+        dcp.dcp_attention_stack_cached(a, z, blocks, cfg.H, cfg.c, bias_cache=torch.empty(1024, dtype=torch.uint8, device=DEV))
+    assert e.value.status == 3
+    cfg4 = syn.small_config("cserr4", I=64, c_s=128, c_z=16, H=4, c=32, dtype="bf16", seed=5)
+    with pytest.raises(dcp.DcpError) as e:                 # the atom shape has no bias cache
+        dcp.dcp_attention_stack_cached(syn.make_s(cfg4, DEV), syn.make_z(cfg4, DEV), [syn.make_weights(cfg4, DEV)], cfg4.H, cfg4.c)
+    assert e.value.status == 2
+    assert dcp.dcp_attention_stack_cache_bytes(3000, 18) == 18 * 94 * 188 * 8 * 512 * 4
