@@ -375,6 +375,13 @@ def dcp_attention_stack_cached(a, z, blocks, H, c, eps=1e-5, bias_cache=None, wo
     return a
 
 
+def dcp_attention_stack_cached_workspace_bytes(I, c_s, H, c, c_z, dtype: torch.dtype) -> int:
+    n = C.c_size_t(0)
+    _check(_lib.dcp_attention_stack_cached_workspace_bytes(int(I), int(c_s), int(H), int(c), int(c_z), _dtype_code(dtype),
+                                                           C.byref(n)), "dcp_attention_stack_cached_workspace_bytes")
+    return int(n.value)
+
+
 def dcp_attention_stack_workspace_bytes(I, c_s, H, c, c_z, dtype: torch.dtype) -> int:
     n = C.c_size_t(0)
     _check(_lib.dcp_attention_stack_workspace_bytes(int(I), int(c_s), int(H), int(c), int(c_z), _dtype_code(dtype), C.byref(n)),

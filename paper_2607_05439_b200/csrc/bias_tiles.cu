@@ -32,7 +32,7 @@ struct BiasTilesParams {
   const void* wfold;       // [n_blocks][16][128] bf16
   const float* c1;         // [n_blocks][16]
   const float* c0;         // [n_blocks][16]
-  uint32_t* cache;         // block b: cache + b * block_words; tile (qt, kt): + ((qt * KT + kt) * 8 + hp) * 512 + q * 16 + key
+  uint32_t* cache;         // block b: cache + b * block_words; tile (qt, kt): + (qt * KT + kt) * 4096 + ((q / 8) * 8 + hp) * 128 + (q % 8) * 16 + key
   int64_t block_words;
   int I, n_blocks, KT, n_tiles;
   float eps;
@@ -146,24 +146,39 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
         mbar_wait(bar_tfull + 8 * tb, (it / bNT) & 1);
         tc_fence_after();
         const uint32_t t_p = t_lane + tb * bMaxN;
+        float accA[16], accB[16];
         const float zsum = tmem_ld_x1(t_p + 16 * p.n_blocks);
+        tmem_ld_x16(t_p, accA);
         tmem_ld_wait();
         const float mu = zsum * (1.f / bCz);
         const float var = fmaf(-mu, mu, zsq * (1.f / bCz));      // one rounding; exactly 0 for a constant row (fused_mma.cu)
         const float rstd = var > 0.f ? rsqrtf(var + p.eps) : 0.f;
         const float nm = -mu * rstd;
-        uint32_t* dst = p.cache + (int64_t)tile * (8 * 512) + sub * (bSubQ * bTileK) + prow;
-        for (int b = 0; b < p.n_blocks; ++b) {
-          float acc[16];
-          tmem_ld_x16(t_p + 16 * b, acc);
-          tmem_ld_wait();
-          const float* c1 = s_c1 + b * bH;
-          const float* c0 = s_c0 + b * bH;
+        // tile layout [sub 4][head pair 8][8 queries][16 keys] words: a stage writes one contiguous 4 KB piece per block
+        uint32_t* dst = p.cache + (int64_t)tile * (8 * 512) + sub * (8 * bSubQ * bTileK) + prow;
+        // block b's 16 columns are processed while block b + 1's are in flight (one tcgen05.ld ahead)
+        auto emit = [&](float (&acc)[16], int b) {
 #pragma unroll
-          for (int hp = 0; hp < 8; ++hp)
-            dst[(int64_t)b * p.block_words + hp * 512] =
-                pack_f16(fmaf(acc[2 * hp], rstd, fmaf(nm, c1[2 * hp], c0[2 * hp])),
-                         fmaf(acc[2 * hp + 1], rstd, fmaf(nm, c1[2 * hp + 1], c0[2 * hp + 1])));
+          for (int i = 0; i < 16; ++i) asm volatile("" : "+f"(acc[i]));        // not before the wait that completes the load
+          const float4* c1 = reinterpret_cast<const float4*>(s_c1 + b * bH);
+          const float4* c0 = reinterpret_cast<const float4*>(s_c0 + b * bH);
+          uint32_t* d = dst + (int64_t)b * p.block_words;
+#pragma unroll
+          for (int h4 = 0; h4 < 4; ++h4) {
+            const float4 a1 = c1[h4], a0 = c0[h4];
+            d[(2 * h4) * 128] = pack_f16(fmaf(acc[4 * h4], rstd, fmaf(nm, a1.x, a0.x)), fmaf(acc[4 * h4 + 1], rstd, fmaf(nm, a1.y, a0.y)));
+            d[(2 * h4 + 1) * 128] = pack_f16(fmaf(acc[4 * h4 + 2], rstd, fmaf(nm, a1.z, a0.z)), fmaf(acc[4 * h4 + 3], rstd, fmaf(nm, a1.w, a0.w)));
+          }
+        };
+        for (int b = 0; b < p.n_blocks; b += 2) {
+          tmem_ld_wait();
+          if (b + 1 < p.n_blocks) tmem_ld_x16(t_p + 16 * (b + 1), accB);
+          emit(accA, b);
+          if (b + 1 < p.n_blocks) {
+            tmem_ld_wait();
+            if (b + 2 < p.n_blocks) tmem_ld_x16(t_p + 16 * (b + 2), accA);
+            emit(accB, b + 1);
+          }
         }
         tc_fence_before();
         __syncwarp();

@@ -42,6 +42,10 @@ constexpr int kBiasBufFloats = kH * kBiasHeadPitch;
 constexpr int kThreads = 512;
 constexpr int kProjWarp0 = 4, kNumProjWarps = 4, kAttnWarp0 = 8, kNumAttnWarps = 8;
 constexpr int kNumIssuers = 3;      // tcgen05 issuing threads (lane 0 of warps 1..3)
+// bias-cache mode: the z stages, bias tiles and W'' (unused then) hold a ring of per-key-tile packages
+// {bias tile 16 KB, K fragments, V fragments of all heads}, each fetched by three bulk copies
+constexpr int kCacheTileBytes = (kH / 2) * kTileQ * kTileK * 4;
+__host__ __device__ constexpr int pkg_bytes(int CP) { return kCacheTileBytes + 2 * kH * (CP / 16) * 512; }
 
 constexpr size_t kSmemZ = 0;
 constexpr size_t kSmemBias = kSmemZ + (size_t)kNZ * kStageBytes;
@@ -52,6 +56,7 @@ constexpr int kTmemBufCols = 32;                         // projection columns p
 constexpr int kTmemCols = kNT * kTmemBufCols;            // 128 (a power of two >= 32)
 constexpr size_t kSmemWt = (kSmemBias + 2 * (size_t)kBiasBufFloats * 4 + 1023) / 1024 * 1024;   // 1024-aligned (swizzle)
 constexpr size_t kSmemBar = kSmemWt + 2 * (size_t)kWtHalfBytes;
+__host__ __device__ constexpr int pkg_count(int CP) { return (int)(kSmemBar / pkg_bytes(CP)) < 3 ? (int)(kSmemBar / pkg_bytes(CP)) : 3; }
 constexpr size_t kSmemQ = (kSmemBar + (2 * kNZ + 4 + 2 * kNT) * 8 + 16 + 15) / 16 * 16;   // Q tile [32 rows][H][CP] bf16, padded rows
 __host__ __device__ constexpr int q_pitch(int CP) { return kH * CP * 2 + 32; }      // bytes; +32: conflict-free 64-bit loads
 __host__ __device__ constexpr size_t smem_alloc(int CP) { return kSmemQ + (size_t)kTileQ * q_pitch(CP) + 1024; }  // + alignment slack
@@ -75,14 +80,21 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
   const bool cached = p.bias_cache != nullptr;               // bias tiles come from the cache (bias_tiles.cu), z is not read
+  constexpr int kNC = pkg_count(CP), kPkg = pkg_bytes(CP), kFragBytes = kH * (CP / 16) * 512;
+  static_assert(kNC >= 2, "bias-cache mode needs two packages in shared memory");
 
   pdl_trigger();
   if (threadIdx.x == 0) {
     // zempty / tfull are arrived on by tcgen05.commit (the MMAs that read the stage / wrote the accumulators are done)
-    for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + kNumProjWarps); }
-    // bfull: the four epilogue warps -- or, with a bias cache, the producer's expect_tx arrival + the bulk copy's bytes
-    for (int b = 0; b < 2; ++b) { mbar_init(bar_bfull + 8 * b, cached ? 1 : kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps); }
-    for (int b = 0; b < kNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, kNumProjWarps); }
+    if (cached) {
+      // bias-cache mode: the barrier block is a ring of kNC (full, empty) pairs -- full: the producer's expect_tx arrival +
+      // the bulk copy's bytes; empty: the eight attention warps
+      for (int b = 0; b < kNC; ++b) { mbar_init(s_bar + 8 * b, 1); mbar_init(s_bar + 8 * (kNC + b), kNumAttnWarps); }
+    } else {
+      for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + kNumProjWarps); }
+      for (int b = 0; b < 2; ++b) { mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps); }
+      for (int b = 0; b < kNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, kNumProjWarps); }
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), kTmemCols);
@@ -109,21 +121,24 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     // =============================================================== TMA producer (warp 0, one lane)
     reg_dec<24>();
     if (warp == 0 && lane == 0 && cached) {
-      // bias cache: one 16 KB tile [head pair][32 queries][16 keys] half2 per (query tile, key tile), by one bulk copy
+      // bias cache: per (query tile, key tile) one package = the 16 KB bias tile [8-query block][head pair][8 queries]
+      // [16 keys] half2 + the key tile's K and V fragments of all heads (contiguous in the prologue's fragment arrays),
+      // three bulk copies on one barrier; the attention warps then never wait on an L2 round trip
       const int KT = (p.I + kTileK - 1) / kTileK;
-      int bbuf = 0;
-      uint32_t bphase = 0;
+      int cb = 0;
+      uint32_t cphase = 0;
       for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
         const Unit un = decode_unit<0, kTileK>(p, u);
         for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
-          mbar_wait(bar_bempty + 8 * bbuf, bphase ^ 1);
-          mbar_expect_tx(bar_bfull + 8 * bbuf, (kH / 2) * kTileQ * kTileK * 4);
-          const uint32_t* src = p.bias_cache + ((int64_t)(un.q0 / kTileQ) * KT + (j0 / kTileK)) * ((kH / 2) * kTileQ * kTileK);
-          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                       ::"r"(smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4)), "l"(src), "r"((kH / 2) * kTileQ * kTileK * 4),
-                         "r"(bar_bfull + 8 * bbuf) : "memory");
-          bbuf ^= 1;
-          if (bbuf == 0) bphase ^= 1;
+          mbar_wait(s_bar + 8 * (kNC + cb), cphase ^ 1);
+          mbar_expect_tx(s_bar + 8 * cb, kPkg);
+          const uint32_t dst = s_z + cb * kPkg;
+          const int kt = j0 / kTileK;
+          bulk_copy_g2s(dst, p.bias_cache + ((int64_t)(un.q0 / kTileQ) * KT + kt) * (kCacheTileBytes / 4), kCacheTileBytes, s_bar + 8 * cb);
+          bulk_copy_g2s(dst + kCacheTileBytes, reinterpret_cast<const char*>(p.kfr) + (int64_t)kt * kFragBytes, kFragBytes, s_bar + 8 * cb);
+          bulk_copy_g2s(dst + kCacheTileBytes + kFragBytes, reinterpret_cast<const char*>(p.vfr) + (int64_t)kt * kFragBytes, kFragBytes,
+                        s_bar + 8 * cb);
+          if (++cb == kNC) { cb = 0; cphase ^= 1; }
         }
       }
     } else if (warp == 0 && lane == 0) {
@@ -285,6 +300,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     const __nv_bfloat16* qp = reinterpret_cast<const __nv_bfloat16*>(p.qp);
     const uint4* kfr = reinterpret_cast<const uint4*>(p.kfr);
     const uint4* vfr = reinterpret_cast<const uint4*>(p.vfr);
+    const int nbuf = cached ? kNC : 2;
     int bbuf = 0;
     uint32_t bphase = 0;
     // K / V fragments of (key tile j, head h) are read from L2 into the registers the previous block just released:
@@ -294,19 +310,30 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     // key of S column: n-block A col c <-> j + 4*(c/2) + c%2, n-block B col c <-> that + 2
     constexpr int NDP = CP / 16;
     uint4 kq[KK], vq[NDP];
+    uint32_t pkg = s_z;               // bias-cache mode: the current key tile's package; fragments come from there
     auto load_k = [&](int j, int h) {
+      if (cached) {
+#pragma unroll
+        for (int kk = 0; kk < KK; ++kk) kq[kk] = lds_u32x4(pkg + kCacheTileBytes + ((h * KK + kk) * 32 + lane) * 16);
+        return;
+      }
       const uint4* src = kfr + ((int64_t)((j >> 4) * kH + h) * KK) * 32 + lane;
 #pragma unroll
       for (int kk = 0; kk < KK; ++kk) kq[kk] = __ldg(src + kk * 32);
     };
     auto load_v = [&](int j, int h) {
+      if (cached) {
+#pragma unroll
+        for (int ndp = 0; ndp < NDP; ++ndp) vq[ndp] = lds_u32x4(pkg + kCacheTileBytes + kFragBytes + ((h * NDP + ndp) * 32 + lane) * 16);
+        return;
+      }
       const uint4* src = vfr + ((int64_t)((j >> 4) * kH + h) * NDP) * 32 + lane;
 #pragma unroll
       for (int ndp = 0; ndp < NDP; ++ndp) vq[ndp] = __ldg(src + ndp * 32);
     };
     // The first K / V tile of a unit is requested during the last tile of the previous one (the slot that would re-read
     // the tile itself), so a unit change costs one L2 round trip (the Q tile) instead of two.
-    if ((int)blockIdx.x < n_units) {
+    if ((int)blockIdx.x < n_units && !cached) {
       const Unit u0 = decode_unit<0, kTileK>(p, blockIdx.x);
       load_k(u0.ks & ~(kTileK - 1), 2 * aw);
       load_v(u0.ks & ~(kTileK - 1), 2 * aw);
@@ -361,9 +388,15 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
         const bool partial = (j0 < un.ks) || (j0 + kTileK > un.ke);
         // next tile; the unit's last tile fetches the next unit's first one (or re-reads itself at the very end: harmless)
         const int jn = j0 + kTileK < un.ke ? j0 + kTileK : (next_first >= 0 ? next_first : j0);
-        mbar_wait(bar_bfull + 8 * bbuf, bphase);
+        mbar_wait(cached ? s_bar + 8 * bbuf : bar_bfull + 8 * bbuf, bphase);
         const uint32_t bias_buf = smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4) + (g * kTileK + 4 * t) * 4;
-        const uint32_t bias_c = bias_buf + aw * (kTileQ * kTileK * 4);       // cached: this warp's head pair plane
+        // cached: this warp's head pair plane of the ring tile; rows g + 8 s of the tile are 8-query block s
+        const uint32_t bias_c = s_z + bbuf * kPkg + (aw * (kSubQ * kTileK) + g * kTileK + 4 * t) * 4;
+        if (cached) {                 // the tile's first head: fragments straight from the package that has just landed
+          pkg = s_z + bbuf * kPkg;
+          load_k(j0, 2 * aw);
+          load_v(j0, 2 * aw);
+        }
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
           const int h = 2 * aw + hh;
@@ -373,8 +406,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           for (int mb = 0; mb < 2; ++mb) {
             if (cached) {
               // word j of the 16 bytes = (head 2 aw, head 2 aw + 1) of key 4 t + j, fp16
-              const uint4 b0 = lds_u32x4(bias_c + (mb * 16 * kTileK) * 4);
-              const uint4 b1 = lds_u32x4(bias_c + ((mb * 16 + 8) * kTileK) * 4);
+              const uint4 b0 = lds_u32x4(bias_c + (2 * mb) * (kCacheTileBytes / 4));
+              const uint4 b1 = lds_u32x4(bias_c + (2 * mb + 1) * (kCacheTileBytes / 4));
               sA[mb][0] = f16_half(b0.x, hh); sA[mb][1] = f16_half(b0.y, hh); sA[mb][2] = f16_half(b1.x, hh); sA[mb][3] = f16_half(b1.y, hh);
               sB[mb][0] = f16_half(b0.z, hh); sB[mb][1] = f16_half(b0.w, hh); sB[mb][2] = f16_half(b1.z, hh); sB[mb][3] = f16_half(b1.w, hh);
             } else {
@@ -393,7 +426,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
               mma_bf16(sA[mb], qa.x, qb.x, qa.y, qb.y, kq[kk].x, kq[kk].y);
               mma_bf16(sB[mb], qa.x, qb.x, qa.y, qb.y, kq[kk].z, kq[kk].w);
             }
-          if (hh == 0) load_k(j0, h + 1); else load_k(jn, h - 1);
+          if (hh == 0) load_k(j0, h + 1); else if (!cached) load_k(jn, h - 1);
           uint32_t pf[2][4];
 #pragma unroll
           for (int mb = 0; mb < 2; ++mb) {
@@ -444,12 +477,11 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             for (int mb = 0; mb < 2; ++mb)
               mma_bf16(o[hh][mb][nd], pf[mb][0], pf[mb][1], pf[mb][2], pf[mb][3],
                        (nd & 1) ? vq[nd >> 1].z : vq[nd >> 1].x, (nd & 1) ? vq[nd >> 1].w : vq[nd >> 1].y);
-          if (hh == 0) load_v(j0, h + 1); else load_v(jn, h - 1);
+          if (hh == 0) load_v(j0, h + 1); else if (!cached) load_v(jn, h - 1);
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar_bempty + 8 * bbuf);
-        bbuf ^= 1;
-        if (bbuf == 0) bphase ^= 1;
+        if (lane == 0) mbar_arrive(cached ? s_bar + 8 * (kNC + bbuf) : bar_bempty + 8 * bbuf);
+        if (++bbuf == nbuf) { bbuf = 0; bphase ^= 1; }
       }
 
       // ---- a7: partial state of (rows, key segment) -> slot   (m back in natural-log units).
