@@ -43,6 +43,7 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~(uintptr_t)1023);
   const uint32_t s_z = smem_u32(smem + bSmemZ), s_wt = smem_u32(smem + bSmemWt), s_bar = smem_u32(smem + bSmemBar);
   float* s_c1 = reinterpret_cast<float*>(smem + bSmemC);
+  const uint32_t s_c = smem_u32(smem + bSmemC);
   float* s_c0 = s_c1 + bMaxBlocks * bH;
   const uint32_t bar_zfull = s_bar, bar_zempty = s_bar + 8 * bNZ, bar_tfull = s_bar + 16 * bNZ, bar_tempty = bar_tfull + 8 * bNT;
   volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + bSmemBar + (2 * bNZ + 2 * bNT) * 8);
@@ -160,12 +161,12 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
         auto emit = [&](float (&acc)[16], int b) {
 #pragma unroll
           for (int i = 0; i < 16; ++i) asm volatile("" : "+f"(acc[i]));        // not before the wait that completes the load
-          const float4* c1 = reinterpret_cast<const float4*>(s_c1 + b * bH);
-          const float4* c0 = reinterpret_cast<const float4*>(s_c0 + b * bH);
+          // explicit ld.shared (generic-pointer loads compiled to LD.E: 16 of them per pair row paced this epilogue)
+          const uint32_t c1 = s_c + b * (bH * 4), c0 = c1 + bMaxBlocks * bH * 4;
           uint32_t* d = dst + (int64_t)b * p.block_words;
 #pragma unroll
           for (int h4 = 0; h4 < 4; ++h4) {
-            const float4 a1 = c1[h4], a0 = c0[h4];
+            const float4 a1 = lds_f32x4(c1 + 16 * h4), a0 = lds_f32x4(c0 + 16 * h4);
             d[(2 * h4) * 128] = pack_f16(fmaf(acc[4 * h4], rstd, fmaf(nm, a1.x, a0.x)), fmaf(acc[4 * h4 + 1], rstd, fmaf(nm, a1.y, a0.y)));
             d[(2 * h4 + 1) * 128] = pack_f16(fmaf(acc[4 * h4 + 2], rstd, fmaf(nm, a1.z, a0.z)), fmaf(acc[4 * h4 + 3], rstd, fmaf(nm, a1.w, a0.w)));
           }
