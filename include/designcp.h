@@ -39,7 +39,9 @@ typedef enum {
   DCP_ERR_UNSUPPORTED = 2, /* a (dtype, H, c, c_z) the kernels are not instantiated for; a tensor-core shape with
                               c_s % 8 != 0 (its GEMMs move 16-byte row pieces); a tile the kernel does not have   */
   DCP_ERR_WORKSPACE = 3,   /* workspace too small (see dcp_workspace_bytes)                                       */
-  DCP_ERR_CUDA = 4         /* a CUDA runtime / driver call failed at launch time                                  */
+  DCP_ERR_CUDA = 4,        /* a CUDA runtime / driver call failed at launch time                                  */
+  DCP_ERR_SCRATCH_LIMIT = 5 /* dcp_pair_bias_attention_no_alloc: the problem needs more workspace than the library's
+                              static scratch array holds (dcp_no_alloc_scratch_bytes); use the caller-workspace entry */
 } dcp_status;
 
 typedef enum { DCP_F32 = 0, DCP_BF16 = 1 } dcp_dtype;
@@ -227,6 +229,22 @@ dcp_status dcp_knn(const float *x, int32_t *idx, int64_t L, int k, void *stream)
  * 1 <= k <= min(L, 512), n_seq >= 0 (DCP_ERR_INVALID_ARG / DCP_ERR_UNSUPPORTED otherwise). */
 dcp_status dcp_knn_budget(const float *x, const int32_t *residue_id, const int32_t *chain_id, int32_t *idx, int64_t L,
                           int k, int n_seq, int n_chains, void *stream);
+
+/* The layer for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): dcp_pair_bias_attention (PAPER.md:58, :83 Eq. 2, :90) with its workspace in a
+ * static device array of DCP_NO_ALLOC_SCRATCH_BYTES inside the library, which every GPU that loads the library holds
+ * until exit.  Arguments, layouts, result and errors as dcp_pair_bias_attention (s, z, w, out: device, caller-owned);
+ * the call and everything under it calls no cudaMalloc, cudaFree or allocating library routine.
+ * Limit: dcp_workspace_bytes(...) for the problem and plan must be <= dcp_no_alloc_scratch_bytes() (32 MiB: the
+ * monolithic token-level layer up to I = 2048 at c_s = 384, H = 16, c = 48), else DCP_ERR_SCRATCH_LIMIT and nothing is
+ * launched.  All calls on a device share the one array, which keeps the previous call's contents (the layer writes
+ * every region before reading it, nothing needs clearing): calls ordered on one stream are safe, calls that overlap on
+ * the GPU (other streams, other host threads on the same device) RACE -- serialise them or use the workspace entry. */
+#define DCP_NO_ALLOC_SCRATCH_BYTES ((size_t)32 << 20)
+size_t dcp_no_alloc_scratch_bytes(void);
+dcp_status dcp_pair_bias_attention_no_alloc(const void *s, const void *z, int64_t ldz, const dcp_weights *w, void *out,
+                                            int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype,
+                                            dcp_decomp decomp, const dcp_plan *plan, void *stream);
 
 /* End-to-end entry with HOST inputs/outputs: s_host, z_host, out_host are HOST pointers (pinned memory gives
  * full PCIe rate); weights stay device-resident (they are parameters, not per-step inputs).  Copies s and z

@@ -34,8 +34,10 @@ EXPORTS = [
     "dcp_attention_stack_workspace_bytes", "dcp_attention_stack", "dcp_plan_units",
     "dcp_probe_l2_gather", "dcp_probe_scan",
     "dcp_attention_stack_cache_bytes", "dcp_attention_stack_cached_workspace_bytes", "dcp_attention_stack_cached",
+    "dcp_pair_bias_attention_no_alloc",
     "dcp_event_create", "dcp_event_record", "dcp_event_elapsed_ms", "dcp_event_destroy",
     "dcp_kernel_supported", "dcp_last_launch_count", "dcp_status_string", "dcp_version",
+    "dcp_no_alloc_scratch_bytes",
 ]
 
 
@@ -89,6 +91,10 @@ def _load() -> C.CDLL:
     lib.dcp_kernel_supported.argtypes = [i32, i32, i32, i32, i32]
     lib.dcp_kernel_supported.restype = i32
     lib.dcp_last_launch_count.restype = i32
+    lib.dcp_pair_bias_attention_no_alloc.argtypes = [vp, vp, i64, C.POINTER(dcp_weights), vp, i64, i32, i32, i32, i32, i32, i32,
+                                                     C.POINTER(dcp_plan), vp]
+    lib.dcp_no_alloc_scratch_bytes.argtypes = []
+    lib.dcp_no_alloc_scratch_bytes.restype = sz
     lib.dcp_status_string.argtypes = [i32]
     lib.dcp_status_string.restype = C.c_char_p
     lib.dcp_version.restype = i32
@@ -110,7 +116,7 @@ def _load() -> C.CDLL:
     lib.dcp_attention_stack_cache_bytes.argtypes = [i64, i32, C.POINTER(sz)]
     lib.dcp_attention_stack_cached_workspace_bytes.argtypes = [i64, i32, i32, i32, i32, i32, C.POINTER(sz)]
     lib.dcp_attention_stack_cached.argtypes = [vp, vp, i64, C.POINTER(dcp_weights), i32, i64, i32, i32, i32, i32, i32, vp, sz, vp, sz, vp]
-    for n in EXPORTS[:24]:
+    for n in EXPORTS[:25]:
         getattr(lib, n).restype = i32
     return lib
 
@@ -276,6 +282,28 @@ def dcp_pair_bias_attention(s, z, w, H, c, decomp="monolithic", parts=1, key_spl
     st = fn(_ptr(s), _ptr(z), int(ldz), C.byref(ws), _ptr(out), I, c_s, H, c, c_z, dt, DECOMP[decomp], C.byref(pl),
             _ptr(workspace), workspace.numel(), _stream_ptr(stream))
     _check(st, "dcp_atom_pair_bias_attention" if atom else "dcp_pair_bias_attention")
+    return out
+
+
+def dcp_no_alloc_scratch_bytes() -> int:
+    return int(_lib.dcp_no_alloc_scratch_bytes())
+
+
+def dcp_pair_bias_attention_no_alloc(s, z, w, H, c, out, decomp="monolithic", parts=1, key_split=1, kernel="auto", eps=1e-5,
+                                     stream=None, ldz=0):
+    """dcp_pair_bias_attention with the workspace in the library's static device array: no allocation anywhere (the
+    caller passes out); DcpError(DCP_ERR_SCRATCH_LIMIT) beyond dcp_no_alloc_scratch_bytes().  Calls that overlap on the
+    GPU race on the shared array."""
+    assert s.is_cuda and z.is_cuda and out.is_cuda and s.is_contiguous() and out.is_contiguous() and z.dtype == s.dtype
+    I, c_s = s.shape
+    c_z = z.shape[-1]
+    assert z.stride(-1) == 1 and z.stride(1) == c_z and (ldz or z.stride(0) == I * c_z), "z: inner dimensions not contiguous"
+    assert out.shape == s.shape and out.dtype == s.dtype
+    pl = _plan(parts, key_split, kernel)
+    ws = _weights_struct(w, eps, s.dtype)
+    st = _lib.dcp_pair_bias_attention_no_alloc(_ptr(s), _ptr(z), int(ldz), C.byref(ws), _ptr(out), I, c_s, H, c, c_z,
+                                               _dtype_code(s.dtype), DECOMP[decomp], C.byref(pl), _stream_ptr(stream))
+    _check(st, "dcp_pair_bias_attention_no_alloc")
     return out
 
 

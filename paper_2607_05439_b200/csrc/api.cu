@@ -847,6 +847,7 @@ const char* dcp_status_string(dcp_status st) {
     case DCP_ERR_UNSUPPORTED: return "DCP_ERR_UNSUPPORTED";
     case DCP_ERR_WORKSPACE: return "DCP_ERR_WORKSPACE";
     case DCP_ERR_CUDA: return "DCP_ERR_CUDA";
+    case DCP_ERR_SCRATCH_LIMIT: return "DCP_ERR_SCRATCH_LIMIT (needs more than dcp_no_alloc_scratch_bytes() of workspace)";
     default: return "DCP_ERR_UNKNOWN";
   }
 }
