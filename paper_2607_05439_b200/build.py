@@ -13,7 +13,7 @@ import sys
 PKG = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libdesigncp.so")
-SOURCES = ["api.cu", "prologue.cu", "fused_generic.cu", "merge_finalize.cu", "fused_mma.cu", "fused_atom.cu", "gemm_mma.cu", "gemm_tc.cu", "sparse_atom.cu", "knn.cu", "pair_transition.cu", "probes.cu", "bias_tiles.cu", "no_alloc.cu"]
+SOURCES = ["api.cu", "prologue.cu", "fused_generic.cu", "merge_finalize.cu", "fused_mma.cu", "fused_atom.cu", "gemm_mma.cu", "gemm_tc.cu", "sparse_atom.cu", "knn.cu", "pair_transition.cu", "probes.cu", "bias_tiles.cu", "no_alloc.cu", "cached_attn.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "--expt-relaxed-constexpr", "-Xcompiler", "-fPIC",

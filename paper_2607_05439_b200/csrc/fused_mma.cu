@@ -22,6 +22,8 @@
 //                 (96 per thread) and leaves as a partial state through a shared-memory slab.
 // Why QK^T / PV stay on mma.sync: what-if builds (profiles/r02_fused_c2_ncu_full.txt) show that removing every
 // attention MMA changes the kernel time by 1-2 %; what paced the kernel was the issue rate of the projection MMAs.
+#include <cstdlib>
+
 #include "kernels.h"
 #include "mma_ptx.cuh"
 
@@ -616,6 +618,7 @@ void mma_pick_units(int64_t I, int H, int n_qparts, int n_kparts, int force_nseg
 cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st) {
   if (p.H != kH) return p.bias_cache ? cudaErrorInvalidValue : launch_fused_atom(p, z, ldz, st);
   if (p.q_end <= p.q_begin || p.k_end <= p.k_begin) return cudaSuccess;
+  if (p.bias_cache && getenv("DCP_CACHED_OLD") == nullptr) return launch_cached_attn(p, st);      // cached_attn.cu: no z side
   if (p.bias_cache && (p.q_begin != 0 || p.n_qparts != 1 || p.tile_h != kTileQ)) return cudaErrorInvalidValue;
   PFN_cuTensorMapEncodeTiled enc = get_encode_fn();
   if (!enc) return cudaErrorNotSupported;

@@ -90,6 +90,8 @@ struct MmaParams {
   bool pdl;             // host only: launch as a programmatic dependent of the previous kernel in the stream
 };
 cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st);
+// attention of one block over a bias cache (cached_attn.cu): p as for launch_fused_mma with p.bias_cache set
+cudaError_t launch_cached_attn(const MmaParams& p, cudaStream_t st);
 bool fused_mma_supports(dcp_dtype dt, int H, int c, int c_z);
 int mma_head_pad(int c);
 int64_t mma_frag_elems(int64_t I, int H, int c);   // bf16 elements of kfr (= of vfr)
