@@ -16,6 +16,8 @@
 //                load delivers the four MMA operand registers in place
 // Work units, key segments and the partial-state slots are those of fused_mma_kernel (mma_ptx.cuh decode_unit), so the
 // merge kernel and the bitwise decomposition contract are unchanged.
+#include <type_traits>
+
 #include "kernels.h"
 #include "mma_ptx.cuh"
 
@@ -115,10 +117,13 @@ __global__ void __launch_bounds__(cThreads, 1) cached_attn_kernel(const MmaParam
   // this head's half of the bias words of rows g + 8 s, keys 4 t .. 4 t + 3: + s * (cBiasBytes / 4)
   const uint32_t bias_off = ((h >> 1) * (cSubQ * cTileK) + g * cTileK + 4 * t) * 4;
   const uint32_t k_off = cBiasBytes + ((h * KK) * 32 + lane) * 16, v_off = cBiasBytes + kFragBytes + ((h * NDP) * 32 + lane) * 16;
-  const int hi = h & 1;
   int bbuf = 0;
   uint32_t bphase = 0;
 
+  // The loop is compiled once per head parity (which half of a bias word the warp reads): a scheduler's four warps have
+  // the same parity, so each runs one copy, with half the conversions of a run-time select.
+  auto run = [&](auto HI) {
+  constexpr int kHi = decltype(HI)::value;
   for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
     const Unit un = decode_unit<0, cTileK>(p, u);
     {
@@ -172,13 +177,8 @@ __global__ void __launch_bounds__(cThreads, 1) cached_attn_kernel(const MmaParam
         // word j of the 16 bytes = heads (2 (h / 2), 2 (h / 2) + 1) of key 4 t + j, fp16
         const uint4 b0 = lds_u32x4(pkg + bias_off + (2 * mb) * (cBiasBytes / 4));
         const uint4 b1 = lds_u32x4(pkg + bias_off + (2 * mb + 1) * (cBiasBytes / 4));
-        if (hi) {        // warp-uniform: a branch, not sixteen selects
-          sA[mb][0] = f16_half(b0.x, 1); sA[mb][1] = f16_half(b0.y, 1); sA[mb][2] = f16_half(b1.x, 1); sA[mb][3] = f16_half(b1.y, 1);
-          sB[mb][0] = f16_half(b0.z, 1); sB[mb][1] = f16_half(b0.w, 1); sB[mb][2] = f16_half(b1.z, 1); sB[mb][3] = f16_half(b1.w, 1);
-        } else {
-          sA[mb][0] = f16_half(b0.x, 0); sA[mb][1] = f16_half(b0.y, 0); sA[mb][2] = f16_half(b1.x, 0); sA[mb][3] = f16_half(b1.y, 0);
-          sB[mb][0] = f16_half(b0.z, 0); sB[mb][1] = f16_half(b0.w, 0); sB[mb][2] = f16_half(b1.z, 0); sB[mb][3] = f16_half(b1.w, 0);
-        }
+        sA[mb][0] = f16_half(b0.x, kHi); sA[mb][1] = f16_half(b0.y, kHi); sA[mb][2] = f16_half(b1.x, kHi); sA[mb][3] = f16_half(b1.y, kHi);
+        sB[mb][0] = f16_half(b0.z, kHi); sB[mb][1] = f16_half(b0.w, kHi); sB[mb][2] = f16_half(b1.z, kHi); sB[mb][3] = f16_half(b1.w, kHi);
       }
 #pragma unroll
       for (int kk = 0; kk < KK; ++kk) {
@@ -290,6 +290,8 @@ __global__ void __launch_bounds__(cThreads, 1) cached_attn_kernel(const MmaParam
       __syncwarp();
     }
   }
+  };
+  if (h & 1) run(std::integral_constant<int, 1>{}); else run(std::integral_constant<int, 0>{});
 }
 
 template <int C, int CP>
