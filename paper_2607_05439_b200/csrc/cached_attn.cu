@@ -165,8 +165,10 @@ __global__ void __launch_bounds__(cThreads, 1) cached_attn_kernel(const MmaParam
         for (int x = 0; x < 4; ++x) o[mb][nd][x] = 0.f;
     }
 
-    for (int j0 = un.ks & ~(cTileK - 1); j0 < un.ke; j0 += cTileK) {
-      const bool partial = (j0 < un.ks) || (j0 + cTileK > un.ke);
+    // one key tile; compiled twice: tiles cut by the segment's ends (at most the first and the last of a unit) mask
+    // their foreign keys, the others carry no select at all
+    auto tile = [&](const int j0, auto PART) {
+      constexpr bool partial = decltype(PART)::value;
       mbar_wait(s_bar + 8 * bbuf, bphase);
       const uint32_t pkg = s_pkg + bbuf * kPkg;
       // ---- a4: S = bias + Q K^T for both 16-row blocks (four independent accumulator chains).  Column c of n-block A is
@@ -251,6 +253,10 @@ __global__ void __launch_bounds__(cThreads, 1) cached_attn_kernel(const MmaParam
       }
       it_next(nx);
       if (++bbuf == kNC) { bbuf = 0; bphase ^= 1; }
+    };
+    for (int j0 = un.ks & ~(cTileK - 1); j0 < un.ke; j0 += cTileK) {
+      if ((j0 < un.ks) || (j0 + cTileK > un.ke)) tile(j0, std::true_type{});
+      else tile(j0, std::false_type{});
     }
 
     // ---- a7: partial state of (rows, key segment) -> slot (m back in natural-log units).  acc is staged per 16-row block
