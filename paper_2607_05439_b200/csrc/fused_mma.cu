@@ -22,8 +22,6 @@
 //                 (96 per thread) and leaves as a partial state through a shared-memory slab.
 // Why QK^T / PV stay on mma.sync: what-if builds (profiles/r02_fused_c2_ncu_full.txt) show that removing every
 // attention MMA changes the kernel time by 1-2 %; what paced the kernel was the issue rate of the projection MMAs.
-#include <cstdlib>
-
 #include "kernels.h"
 #include "mma_ptx.cuh"
 
@@ -44,10 +42,6 @@ constexpr int kBiasBufFloats = kH * kBiasHeadPitch;
 constexpr int kThreads = 512;
 constexpr int kProjWarp0 = 4, kNumProjWarps = 4, kAttnWarp0 = 8, kNumAttnWarps = 8;
 constexpr int kNumIssuers = 3;      // tcgen05 issuing threads (lane 0 of warps 1..3)
-// bias-cache mode: the z stages, bias tiles and W'' (unused then) hold a ring of per-key-tile packages
-// {bias tile 16 KB, K fragments, V fragments of all heads}, each fetched by three bulk copies
-constexpr int kCacheTileBytes = (kH / 2) * kTileQ * kTileK * 4;
-__host__ __device__ constexpr int pkg_bytes(int CP) { return kCacheTileBytes + 2 * kH * (CP / 16) * 512; }
 
 constexpr size_t kSmemZ = 0;
 constexpr size_t kSmemBias = kSmemZ + (size_t)kNZ * kStageBytes;
@@ -58,7 +52,6 @@ constexpr int kTmemBufCols = 32;                         // projection columns p
 constexpr int kTmemCols = kNT * kTmemBufCols;            // 128 (a power of two >= 32)
 constexpr size_t kSmemWt = (kSmemBias + 2 * (size_t)kBiasBufFloats * 4 + 1023) / 1024 * 1024;   // 1024-aligned (swizzle)
 constexpr size_t kSmemBar = kSmemWt + 2 * (size_t)kWtHalfBytes;
-__host__ __device__ constexpr int pkg_count(int CP) { return (int)(kSmemBar / pkg_bytes(CP)) < 3 ? (int)(kSmemBar / pkg_bytes(CP)) : 3; }
 constexpr size_t kSmemQ = (kSmemBar + (2 * kNZ + 4 + 2 * kNT) * 8 + 16 + 15) / 16 * 16;   // Q tile [32 rows][H][CP] bf16, padded rows
 __host__ __device__ constexpr int q_pitch(int CP) { return kH * CP * 2 + 32; }      // bytes; +32: conflict-free 64-bit loads
 __host__ __device__ constexpr size_t smem_alloc(int CP) { return kSmemQ + (size_t)kTileQ * q_pitch(CP) + 1024; }  // + alignment slack
@@ -81,29 +74,20 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int g = lane >> 2, t = lane & 3;
-  const bool cached = p.bias_cache != nullptr;               // bias tiles come from the cache (bias_tiles.cu), z is not read
-  constexpr int kNC = pkg_count(CP), kPkg = pkg_bytes(CP), kFragBytes = kH * (CP / 16) * 512;
-  static_assert(kNC >= 2, "bias-cache mode needs two packages in shared memory");
 
   pdl_trigger();
   if (threadIdx.x == 0) {
     // zempty / tfull are arrived on by tcgen05.commit (the MMAs that read the stage / wrote the accumulators are done)
-    if (cached) {
-      // bias-cache mode: the barrier block is a ring of kNC (full, empty) pairs -- full: the producer's expect_tx arrival +
-      // the bulk copy's bytes; empty: the eight attention warps
-      for (int b = 0; b < kNC; ++b) { mbar_init(s_bar + 8 * b, 1); mbar_init(s_bar + 8 * (kNC + b), kNumAttnWarps); }
-    } else {
-      for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + kNumProjWarps); }
-      for (int b = 0; b < 2; ++b) { mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps); }
-      for (int b = 0; b < kNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, kNumProjWarps); }
-    }
+    for (int s = 0; s < kNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + kNumProjWarps); }
+    for (int b = 0; b < 2; ++b) { mbar_init(bar_bfull + 8 * b, kNumProjWarps); mbar_init(bar_bempty + 8 * b, kNumAttnWarps); }
+    for (int b = 0; b < kNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, kNumProjWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), kTmemCols);
   pdl_wait();          // the prologue's q / k / v / folded weights are final (and so is everything before it in the stream)
   // W'' = B operand of the projection MMA, K-major, 128-byte swizzled by hand: row n < 16 = head n of
   // (gamma (.) W_b log2 e)^T, row 16 = ones (its accumulator column is sum_k z), rows 17..31 = 0.
-  for (int e = threadIdx.x; e < (cached ? 0 : kProjN * (kCz / 8)); e += kThreads) {
+  for (int e = threadIdx.x; e < kProjN * (kCz / 8); e += kThreads) {
     const int n = e / (kCz / 8), ch16 = e % (kCz / 8);          // 16-byte chunk = 8 channels
     uint4 v = make_uint4(0u, 0u, 0u, 0u);
     if (n < kH) v = __ldg(reinterpret_cast<const uint4*>(p.wfold) + n * (kCz / 8) + ch16);
@@ -122,28 +106,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
   if (warp < kProjWarp0) {
     // =============================================================== TMA producer (warp 0, one lane)
     reg_dec<24>();
-    if (warp == 0 && lane == 0 && cached) {
-      // bias cache: per (query tile, key tile) one package = the 16 KB bias tile [8-query block][head pair][8 queries]
-      // [16 keys] half2 + the key tile's K and V fragments of all heads (contiguous in the prologue's fragment arrays),
-      // three bulk copies on one barrier; the attention warps then never wait on an L2 round trip
-      const int KT = (p.I + kTileK - 1) / kTileK;
-      int cb = 0;
-      uint32_t cphase = 0;
-      for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
-        const Unit un = decode_unit<0, kTileK>(p, u);
-        for (int j0 = un.ks & ~(kTileK - 1); j0 < un.ke; j0 += kTileK) {
-          mbar_wait(s_bar + 8 * (kNC + cb), cphase ^ 1);
-          mbar_expect_tx(s_bar + 8 * cb, kPkg);
-          const uint32_t dst = s_z + cb * kPkg;
-          const int kt = j0 / kTileK;
-          bulk_copy_g2s(dst, p.bias_cache + ((int64_t)(un.q0 / kTileQ) * KT + kt) * (kCacheTileBytes / 4), kCacheTileBytes, s_bar + 8 * cb);
-          bulk_copy_g2s(dst + kCacheTileBytes, reinterpret_cast<const char*>(p.kfr) + (int64_t)kt * kFragBytes, kFragBytes, s_bar + 8 * cb);
-          bulk_copy_g2s(dst + kCacheTileBytes + kFragBytes, reinterpret_cast<const char*>(p.vfr) + (int64_t)kt * kFragBytes, kFragBytes,
-                        s_bar + 8 * cb);
-          if (++cb == kNC) { cb = 0; cphase ^= 1; }
-        }
-      }
-    } else if (warp == 0 && lane == 0) {
+    if (warp == 0 && lane == 0) {
       uint64_t policy;
       asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
       int stage = 0;
@@ -170,7 +133,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           }
         }
       }
-    } else if (warp >= 1 && warp <= kNumIssuers && lane == 0 && !cached) {
+    } else if (warp >= 1 && warp <= kNumIssuers && lane == 0) {
       // ============================================================= tcgen05 issuers (one thread each, warps 1..3)
       // A K = 16 projection MMA costs its issuing thread ~130 cycles whatever N is (the 4 KB A-operand fetch), eight of
       // them per 32 KB stage: one thread alone needs ~1050 of the ~1450 cycles a stage may take at the HBM bound, and
@@ -232,7 +195,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     const uint32_t zsw = (uint32_t)(prow & 7);
     int tb = 0, bbuf = 0, stage = 0;
     uint32_t tphase = 0, bphase = 0, zphase = 0;
-    for (int u = blockIdx.x; u < (cached ? 0 : n_units); u += gridDim.x) {
+    for (int u = blockIdx.x; u < n_units; u += gridDim.x) {
       const Unit un = decode_unit<0, kTileK>(p, u);
       const int rows = (un.q_end - un.q0) < p.tile_h ? (un.q_end - un.q0) : p.tile_h;
       const int nsub = (rows + kSubQ - 1) / kSubQ;
@@ -302,7 +265,6 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     const __nv_bfloat16* qp = reinterpret_cast<const __nv_bfloat16*>(p.qp);
     const uint4* kfr = reinterpret_cast<const uint4*>(p.kfr);
     const uint4* vfr = reinterpret_cast<const uint4*>(p.vfr);
-    const int nbuf = cached ? kNC : 2;
     int bbuf = 0;
     uint32_t bphase = 0;
     // K / V fragments of (key tile j, head h) are read from L2 into the registers the previous block just released:
@@ -312,30 +274,19 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
     // key of S column: n-block A col c <-> j + 4*(c/2) + c%2, n-block B col c <-> that + 2
     constexpr int NDP = CP / 16;
     uint4 kq[KK], vq[NDP];
-    uint32_t pkg = s_z;               // bias-cache mode: the current key tile's package; fragments come from there
     auto load_k = [&](int j, int h) {
-      if (cached) {
-#pragma unroll
-        for (int kk = 0; kk < KK; ++kk) kq[kk] = lds_u32x4(pkg + kCacheTileBytes + ((h * KK + kk) * 32 + lane) * 16);
-        return;
-      }
       const uint4* src = kfr + ((int64_t)((j >> 4) * kH + h) * KK) * 32 + lane;
 #pragma unroll
       for (int kk = 0; kk < KK; ++kk) kq[kk] = __ldg(src + kk * 32);
     };
     auto load_v = [&](int j, int h) {
-      if (cached) {
-#pragma unroll
-        for (int ndp = 0; ndp < NDP; ++ndp) vq[ndp] = lds_u32x4(pkg + kCacheTileBytes + kFragBytes + ((h * NDP + ndp) * 32 + lane) * 16);
-        return;
-      }
       const uint4* src = vfr + ((int64_t)((j >> 4) * kH + h) * NDP) * 32 + lane;
 #pragma unroll
       for (int ndp = 0; ndp < NDP; ++ndp) vq[ndp] = __ldg(src + ndp * 32);
     };
     // The first K / V tile of a unit is requested during the last tile of the previous one (the slot that would re-read
     // the tile itself), so a unit change costs one L2 round trip (the Q tile) instead of two.
-    if ((int)blockIdx.x < n_units && !cached) {
+    if ((int)blockIdx.x < n_units) {
       const Unit u0 = decode_unit<0, kTileK>(p, blockIdx.x);
       load_k(u0.ks & ~(kTileK - 1), 2 * aw);
       load_v(u0.ks & ~(kTileK - 1), 2 * aw);
@@ -390,15 +341,8 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
         const bool partial = (j0 < un.ks) || (j0 + kTileK > un.ke);
         // next tile; the unit's last tile fetches the next unit's first one (or re-reads itself at the very end: harmless)
         const int jn = j0 + kTileK < un.ke ? j0 + kTileK : (next_first >= 0 ? next_first : j0);
-        mbar_wait(cached ? s_bar + 8 * bbuf : bar_bfull + 8 * bbuf, bphase);
+        mbar_wait(bar_bfull + 8 * bbuf, bphase);
         const uint32_t bias_buf = smem_u32(s_bias) + bbuf * (kBiasBufFloats * 4) + (g * kTileK + 4 * t) * 4;
-        // cached: this warp's head pair plane of the ring tile; rows g + 8 s of the tile are 8-query block s
-        const uint32_t bias_c = s_z + bbuf * kPkg + (aw * (kSubQ * kTileK) + g * kTileK + 4 * t) * 4;
-        if (cached) {                 // the tile's first head: fragments straight from the package that has just landed
-          pkg = s_z + bbuf * kPkg;
-          load_k(j0, 2 * aw);
-          load_v(j0, 2 * aw);
-        }
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
           const int h = 2 * aw + hh;
@@ -406,18 +350,10 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
           float sA[2][4], sB[2][4];
 #pragma unroll
           for (int mb = 0; mb < 2; ++mb) {
-            if (cached) {
-              // word j of the 16 bytes = (head 2 aw, head 2 aw + 1) of key 4 t + j, fp16
-              const uint4 b0 = lds_u32x4(bias_c + (2 * mb) * (kCacheTileBytes / 4));
-              const uint4 b1 = lds_u32x4(bias_c + (2 * mb + 1) * (kCacheTileBytes / 4));
-              sA[mb][0] = f16_half(b0.x, hh); sA[mb][1] = f16_half(b0.y, hh); sA[mb][2] = f16_half(b1.x, hh); sA[mb][3] = f16_half(b1.y, hh);
-              sB[mb][0] = f16_half(b0.z, hh); sB[mb][1] = f16_half(b0.w, hh); sB[mb][2] = f16_half(b1.z, hh); sB[mb][3] = f16_half(b1.w, hh);
-            } else {
-              const float4 b0 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + mb * 16 * kTileK) * 4);
-              const float4 b1 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + (mb * 16 + 8) * kTileK) * 4);
-              sA[mb][0] = b0.x; sA[mb][1] = b0.y; sA[mb][2] = b1.x; sA[mb][3] = b1.y;
-              sB[mb][0] = b0.z; sB[mb][1] = b0.w; sB[mb][2] = b1.z; sB[mb][3] = b1.w;
-            }
+            const float4 b0 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + mb * 16 * kTileK) * 4);
+            const float4 b1 = lds_f32x4(bias_buf + (h * kBiasHeadPitch + (mb * 16 + 8) * kTileK) * 4);
+            sA[mb][0] = b0.x; sA[mb][1] = b0.y; sA[mb][2] = b1.x; sA[mb][3] = b1.y;
+            sB[mb][0] = b0.z; sB[mb][1] = b0.w; sB[mb][2] = b1.z; sB[mb][3] = b1.w;
           }
 #pragma unroll
           for (int kk = 0; kk < KK; ++kk)
@@ -428,7 +364,7 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
               mma_bf16(sA[mb], qa.x, qb.x, qa.y, qb.y, kq[kk].x, kq[kk].y);
               mma_bf16(sB[mb], qa.x, qb.x, qa.y, qb.y, kq[kk].z, kq[kk].w);
             }
-          if (hh == 0) load_k(j0, h + 1); else if (!cached) load_k(jn, h - 1);
+          if (hh == 0) load_k(j0, h + 1); else load_k(jn, h - 1);
           uint32_t pf[2][4];
 #pragma unroll
           for (int mb = 0; mb < 2; ++mb) {
@@ -479,11 +415,12 @@ __global__ void __launch_bounds__(kThreads, 1) fused_mma_kernel(const __grid_con
             for (int mb = 0; mb < 2; ++mb)
               mma_bf16(o[hh][mb][nd], pf[mb][0], pf[mb][1], pf[mb][2], pf[mb][3],
                        (nd & 1) ? vq[nd >> 1].z : vq[nd >> 1].x, (nd & 1) ? vq[nd >> 1].w : vq[nd >> 1].y);
-          if (hh == 0) load_v(j0, h + 1); else if (!cached) load_v(jn, h - 1);
+          if (hh == 0) load_v(j0, h + 1); else load_v(jn, h - 1);
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(cached ? s_bar + 8 * (kNC + bbuf) : bar_bempty + 8 * bbuf);
-        if (++bbuf == nbuf) { bbuf = 0; bphase ^= 1; }
+        if (lane == 0) mbar_arrive(bar_bempty + 8 * bbuf);
+        bbuf ^= 1;
+        if (bbuf == 0) bphase ^= 1;
       }
 
       // ---- a7: partial state of (rows, key segment) -> slot   (m back in natural-log units).
@@ -616,10 +553,9 @@ void mma_pick_units(int64_t I, int H, int n_qparts, int n_kparts, int force_nseg
 }
 
 cudaError_t launch_fused_mma(const MmaParams& p, const void* z, int64_t ldz, cudaStream_t st) {
-  if (p.H != kH) return p.bias_cache ? cudaErrorInvalidValue : launch_fused_atom(p, z, ldz, st);
+  if (p.H != kH) return launch_fused_atom(p, z, ldz, st);
+  if (p.bias_cache) return launch_cached_attn(p, st);      // cached_attn.cu: the bias comes from a cache, z is not read
   if (p.q_end <= p.q_begin || p.k_end <= p.k_begin) return cudaSuccess;
-  if (p.bias_cache && getenv("DCP_CACHED_OLD") == nullptr) return launch_cached_attn(p, st);      // cached_attn.cu: no z side
-  if (p.bias_cache && (p.q_begin != 0 || p.n_qparts != 1 || p.tile_h != kTileQ)) return cudaErrorInvalidValue;
   PFN_cuTensorMapEncodeTiled enc = get_encode_fn();
   if (!enc) return cudaErrorNotSupported;
   CUtensorMap tm;
