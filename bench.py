@@ -738,13 +738,14 @@ def run_attention_stack(args, rank, world, local_rank):
         cb = passes * zb + 2.0 * nb * tiles * cfg.H * 2
         roofline = {"bound": "hbm", "achieved": cb / (step_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                     "frac": cb / (step_ms * 1e-3) / 1e9 / peak, "traffic": None,
-                    "kernel": "whole call: bias_tiles_kernel x %d passes + fused_mma_kernel (bias-cache input) x %d" % (passes, nb),
+                    "kernel": "whole call: bias_tiles_kernel x %d passes + cached_attn_kernel x %d" % (passes, nb),
                     "peak_source": peak_how, "algorithmic_bytes_per_call": cb, "passes": passes,
                     "streaming_call_ms": stream_ms, "speedup_vs_streaming_call": stream_ms / step_ms,
                     "streaming_bytes_equivalent_frac": nb * zb / (step_ms * 1e-3) / 1e9 / peak,
                     "streaming_single_layer_kernel_ms": kms,
                     "note": "frac: this mode's bytes (passes x z + cache written and read once) over the whole call; the "
-                            "cached blocks are bound by the attention warps (mma.sync + softmax), not by HBM; "
+                            "bias_tiles_kernel runs at the HBM rate (z read + cache write), cached_attn_kernel is bound by its attention "
+                            "warps (mma.sync + softmax), profiles/r02_cached_stack.md; "
                             "streaming_bytes_equivalent_frac: what the streaming stack would need to reach to match this time"}
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -788,7 +789,8 @@ def run_attention_stack(args, rank, world, local_rank):
             "config": {"workload": f"{args.workload}: {nb} sequential AttentionPairBias blocks with residual on the c_token={cfg.c_s} "
                                    f"latent, read-only pair tensor I={cfg.I} c_z={cfg.c_z} H={cfg.H} c={cfg.c} bf16 "
                                    f"(icosahedral 60 x {cfg.n_res}; PAPER.md:294)",
-                       "pair": "one (block, token pair)", "blocks": nb, "kernel": "fused_mma_kernel",
+                       "pair": "one (block, token pair)", "blocks": nb,
+                       "kernel": "bias_tiles_kernel + cached_attn_kernel" if args.cached else "fused_mma_kernel",
                        "mode": "bias cache (dcp_attention_stack_cached)" if args.cached else "streaming (dcp_attention_stack)",
                        "ms_per_block": step_ms / nb,
                        "l2": "z (%.0f MB) larger than the 126 MB L2: no flush needed" % (z.numel() * 2 / 1e6),
