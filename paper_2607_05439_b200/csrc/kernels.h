@@ -83,9 +83,8 @@ struct MmaParams {
   int tile_h;           // fused_mma_kernel: query rows per work unit (25..32; the atom kernel's tile is fixed)
   int H, c, c_z;
   float eps;
-  // fused_mma_kernel only, optional: the bias of this call comes from a cache (bias_tiles.cu) instead of z -- the TMA
-  // producer copies one 16 KB fp16 tile per (32-query tile, 16-key tile) into the bias buffer; z is not touched.
-  // Needs q_begin == 0, n_qparts == 1, tile_h == 32 (tiles aligned with the cache's).
+  // optional: the bias of this call comes from a cache (bias_tiles.cu) instead of z; launch_fused_mma then forwards to
+  // cached_attn_kernel (cached_attn.cu), which reads no z at all.  Whole-tensor rows, one row part, tile height 32.
   const uint32_t* bias_cache;
   bool pdl;             // host only: launch as a programmatic dependent of the previous kernel in the stream
 };
@@ -130,7 +129,7 @@ cudaError_t launch_pair_transition(const void* z_in, void* z_out, int64_t n_pair
                                    cudaStream_t st);
 
 // Bias cache of the attention stack (bias_tiles.cu): the biases LN_b(z) W_b^b of up to bias_tiles_max_blocks() blocks in one
-// pass over z, as fp16 tiles in the layout fused_mma_kernel consumes when MmaParams.bias_cache is set
+// pass over z, as fp16 tiles in the layout cached_attn_kernel consumes (MmaParams.bias_cache)
 int bias_tiles_max_blocks();
 int64_t bias_tiles_block_words(int64_t I);          // 32-bit words of one block's cache
 size_t bias_tiles_fold_bytes(int n_blocks);         // scratch for the folded weights of a pass
