@@ -128,14 +128,19 @@ __global__ void __launch_bounds__(256) knn_kernel(const float* __restrict__ x, i
 }
 
 // ---- threshold-select variant (k <= 256): no sorted list is maintained while scanning.
-//   1. the warp computes the distances to the 2048 atoms of the block's own tile (64 registers per lane) and bisects
-//      the binary32 bit pattern (non-negative floats order like unsigned integers) for a threshold T with at least k
-//      of those distances <= T: an upper bound of the final k-th distance, a few percent above the tile's own k-th;
-//   2. one scan over all L candidates appends every (d2, index) with d2 <= T to a per-warp shared-memory buffer
-//      (one ballot + one prefix popcount per 32 candidates; typically 1.5 k .. 2 k entries);
-//   3. the buffer is sorted by (d2, index) with a bitonic network and its first k entries are the answer.
+//   1. own tile (2048 atoms): each lane keeps the r = ceil(k / 32) smallest of its 64 distances while they stream past
+//      (nothing else stays in registers); the largest of the lanes' r-th smallest is a bound T1 with at least k of the
+//      tile's distances <= T1.  A second pass appends the tile's entries <= T1 to the per-warp shared-memory buffer,
+//      a bisection of the binary32 bit pattern over the BUFFER (16 values per lane, counted with ballots) tightens the
+//      bound to a threshold T a few percent above the tile's own k-th distance, and the buffer is compacted to <= T;
+//   2. one scan over the other tiles appends every (d2, index) with d2 <= T (one ballot + one prefix popcount per 32
+//      candidates; typically 1.5 k .. 2 k entries in the end);
+//   3. a full bisection over the buffer finds the exact k-th distance D, the entries <= D (k of them unless distances
+//      tie) are compacted and sorted by (d2, index) with a bitonic network: the first k are the answer.
 // Same distances, same (d2, index) order as knn_kernel: the result is identical.  A query whose buffer overflows
-// (more than kCap candidates within T: a very dense neighbourhood) falls back to the insertion scan over global memory.
+// (more than kCap candidates within the bound: a very dense neighbourhood) falls back to the insertion scan over global
+// memory.  Round 1's version held the own tile's 64 distances per lane in registers (128 registers, 16 warps per SM) and
+// sorted the whole buffer.
 
 template <int NR>
 __device__ __noinline__ void knn_insert_global(const float* __restrict__ x, int32_t* __restrict__ idx, int L, int k, int l,
@@ -204,17 +209,79 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
   float* sy = sx + kTile;
   float* sz = sy + kTile;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  float* bd = sz + kTile + wib * (2 * kCap);                   // per-warp buffer: kCap distances, kCap indices
-  int* bi = reinterpret_cast<int*>(bd + kCap);
+  unsigned* bd = reinterpret_cast<unsigned*>(sz + kTile) + wib * (2 * kCap);   // per-warp buffer: kCap distances (bit patterns),
+  int* bi = reinterpret_cast<int*>(bd + kCap);                                 // kCap indices
+  constexpr int kPer = kCap / 32;                              // buffer entries per lane
+  constexpr unsigned kInfBits = 0x7f800000u;
   const int lq = blockIdx.x * 8 + wib;
   const bool active = lq < L;
   const int l = active ? lq : L - 1;
   const float q0 = __ldg(x + 3 * (int64_t)l), q1 = __ldg(x + 3 * (int64_t)l + 1), q2 = __ldg(x + 3 * (int64_t)l + 2);
   const int n_tiles = (L + kTile - 1) / kTile;
   const int own = (blockIdx.x * 8) / kTile;
-  unsigned thr = 0x7f800000u;                                  // bit pattern of the threshold T
+  unsigned thr = kInfBits;                                     // bit pattern of the threshold T
   int cnt = 0;
   const unsigned lt_mask = (1u << lane) - 1u;
+  auto dist_bits = [&](int e) {
+    const float a0 = __fsub_rn(sx[e], q0), a1 = __fsub_rn(sy[e], q1), a2 = __fsub_rn(sz[e], q2);
+    return __float_as_uint(__fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2)));
+  };
+  // smallest pattern T in [0, hi0] with #{buffer entries <= T} >= need, to `iters` bisection steps (hi stays a valid bound)
+  auto bisect = [&](const unsigned (&bv)[kPer], unsigned hi0, int need, int iters) {
+    unsigned lo = 0u, hi = hi0;
+    for (int it = 0; it < iters && lo < hi; ++it) {
+      const unsigned mid = lo + ((hi - lo) >> 1);
+      int c = 0;
+#pragma unroll
+      for (int j = 0; j < kPer; ++j) c += __popc(__ballot_sync(0xffffffffu, bv[j] <= mid));
+      if (c >= need) hi = mid; else lo = mid + 1;
+    }
+    return hi;
+  };
+  // keep the buffer entries <= t, in order; returns the new count
+  auto compact = [&](const unsigned (&bv)[kPer], unsigned t, int n) {
+    int nc = 0;
+#pragma unroll
+    for (int j = 0; j < kPer; ++j) {
+      if (32 * j >= n) break;                                  // warp-uniform
+      const int e = 32 * j + lane;
+      const int iv = e < n ? bi[e] : 0;
+      const bool pass = e < n && bv[j] <= t;
+      const unsigned mask = __ballot_sync(0xffffffffu, pass);  // every lane has read chunk j before any lane overwrites it
+      if (pass) { const int slot = nc + __popc(mask & lt_mask); bd[slot] = bv[j]; bi[slot] = iv; }
+      nc += __popc(mask);
+      __syncwarp();
+    }
+    return nc;
+  };
+  auto load_buffer = [&](unsigned (&bv)[kPer], int n) {
+#pragma unroll
+    for (int j = 0; j < kPer; ++j) bv[j] = 32 * j + lane < n ? bd[32 * j + lane] : 0xffffffffu;
+  };
+
+  bool over = false;                                           // more than kCap entries tie within the bound: exact fallback
+  // the buffer's own k-th distance is a bound too: when the buffer is about to overflow (a dense neighbourhood), bisect
+  // it, keep the entries within the new bound and go on (the buffer holds >= k entries then: kCap >= 2 k)
+  auto tighten = [&]() {
+    __syncwarp();
+    unsigned bv[kPer];
+    load_buffer(bv, cnt);
+    thr = bisect(bv, thr, k, 32);
+    cnt = compact(bv, thr, cnt);
+  };
+  // append the lanes' candidates (d2 bits v, atom m) that pass
+  auto append = [&](unsigned v, int m, bool pass) {
+    if (over) return;
+    unsigned mask = __ballot_sync(0xffffffffu, pass);
+    if (cnt + __popc(mask) > kCap) {
+      tighten();
+      pass = pass && v <= thr;
+      mask = __ballot_sync(0xffffffffu, pass);
+      if (cnt + __popc(mask) > kCap) { over = true; return; }
+    }
+    if (pass) { const int slot = cnt + __popc(mask & lt_mask); bd[slot] = v; bi[slot] = m; }
+    cnt += __popc(mask);
+  };
 
   for (int tt = 0; tt < n_tiles; ++tt) {
     const int tile = tt == 0 ? own : (tt <= own ? tt - 1 : tt);
@@ -229,68 +296,73 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
     __syncthreads();
     const int n_here = (L - t0 < kTile ? L - t0 : kTile);
     if (tt == 0) {
-      // ---- 1. distances to the own tile in registers, bisection for T
-      unsigned db[kTile / 32];
+      // ---- 1a. the r smallest distances of each lane's share of the own tile
+      const int need = k < n_here ? k : n_here;
+      const int r = (need + 31) >> 5;                          // <= 8 (k <= 256)
+      unsigned sm[8];
 #pragma unroll
+      for (int j = 0; j < 8; ++j) sm[j] = kInfBits;
+#pragma unroll 4
       for (int i = 0; i < kTile / 32; ++i) {
         const int e = 32 * i + lane;
-        const float a0 = __fsub_rn(sx[e], q0), a1 = __fsub_rn(sy[e], q1), a2 = __fsub_rn(sz[e], q2);
-        const float dd = __fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2));
-        db[i] = e < n_here ? __float_as_uint(dd) : 0x7f800000u;
+        unsigned v = e < n_here ? dist_bits(e) : kInfBits;
+        if (__any_sync(0xffffffffu, v < sm[7])) {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) { const unsigned lo = min(sm[j], v); v = max(sm[j], v); sm[j] = lo; }
+        }
       }
-      unsigned lo = 0u, hi = 0x7f800000u;                      // invariant: #{db <= hi} >= min(k, n_here)
-      const int need = k < n_here ? k : n_here;
-      for (int it = 0; it < 14 && lo < hi; ++it) {
-        const unsigned mid = lo + ((hi - lo) >> 1);
-        int c = 0;
+      unsigned sr = sm[0];
 #pragma unroll
-        for (int i = 0; i < kTile / 32; ++i) c += db[i] <= mid ? 1 : 0;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
-        if (c >= need) hi = mid; else lo = mid + 1;
-      }
-      thr = n_here >= k ? hi : 0x7f800000u;                    // fewer than k atoms in the tile: no bound from it
-      // ---- 2a. the own tile's candidates come straight from the registers
-#pragma unroll
+      for (int j = 1; j < 8; ++j) sr = j == r - 1 ? sm[j] : sr;
+      thr = n_here >= k ? __reduce_max_sync(0xffffffffu, sr) : kInfBits;   // T1; fewer than k atoms: no bound
+      // ---- 1b. the own tile's entries <= T1 -> buffer
+#pragma unroll 4
       for (int i = 0; i < kTile / 32; ++i) {
-        const bool pass = db[i] <= thr && 32 * i + lane < n_here;
-        const unsigned mask = __ballot_sync(0xffffffffu, pass);
-        const int slot = cnt + __popc(mask & lt_mask);
-        if (pass && slot < kCap) { bd[slot] = __uint_as_float(db[i]); bi[slot] = t0 + 32 * i + lane; }
-        cnt += __popc(mask);
+        const int e = 32 * i + lane;
+        const unsigned v = e < n_here ? dist_bits(e) : kInfBits;
+        append(v, t0 + e, e < n_here && v <= thr);
+      }
+      __syncwarp();
+      if (!over && thr != kInfBits) {
+        // ---- 1c. tighten the bound over the buffer, keep what is within it
+        unsigned bv[kPer];
+        load_buffer(bv, cnt);
+        thr = bisect(bv, thr, need, 14);
+        cnt = compact(bv, thr, cnt);
       }
     } else {
-      // ---- 2b. every other tile: four chunks per step
+      // ---- 2. every other tile: four chunks per step
       for (int c0 = 0; c0 < n_here; c0 += 128) {
         unsigned dbv[4], mk[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           const int e = (c0 + 32 * u + lane) & (kTile - 1);
-          const float a0 = __fsub_rn(sx[e], q0), a1 = __fsub_rn(sy[e], q1), a2 = __fsub_rn(sz[e], q2);
-          const float dd = __fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2));
-          dbv[u] = __float_as_uint(dd);
+          dbv[u] = dist_bits(e);
           mk[u] = __ballot_sync(0xffffffffu, dbv[u] <= thr && c0 + 32 * u + lane < n_here);
         }
         if ((mk[0] | mk[1] | mk[2] | mk[3]) == 0) continue;
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const bool pass = (mk[u] >> lane) & 1u;
-          const int slot = cnt + __popc(mk[u] & lt_mask);
-          if (pass && slot < kCap) { bd[slot] = __uint_as_float(dbv[u]); bi[slot] = t0 + c0 + 32 * u + lane; }
-          cnt += __popc(mk[u]);
-        }
+        for (int u = 0; u < 4; ++u)
+          if (mk[u]) append(dbv[u], t0 + c0 + 32 * u + lane, (mk[u] >> lane) & 1u);
       }
     }
   }
   if (!active) return;
-  if (cnt > kCap) {                                            // very dense neighbourhood: exact fallback
+  if (over) {                                                  // > kCap entries tie within the bound: exact fallback
     knn_insert_global<NRF>(x, idx, L, k, l, lane);
     return;
   }
-  // ---- 3. bitonic sort of the buffer by (d2, index), padded to a power of two
+  // ---- 3. the exact k-th distance over the buffer, then a sort of the entries within it (k of them unless distances tie)
+  __syncwarp();
+  {
+    unsigned bv[kPer];
+    load_buffer(bv, cnt);
+    const unsigned dk = bisect(bv, thr, k < cnt ? k : cnt, 32);
+    cnt = compact(bv, dk, cnt);
+  }
   int P = 32;
   while (P < cnt) P <<= 1;
-  for (int e = cnt + lane; e < P; e += 32) { bd[e] = kInf; bi[e] = 0x7fffffff; }
+  for (int e = cnt + lane; e < P; e += 32) { bd[e] = 0xffffffffu; bi[e] = 0x7fffffff; }
   __syncwarp();
   for (int size = 2; size <= P; size <<= 1) {
     for (int stride = size >> 1; stride > 0; stride >>= 1) {
@@ -298,7 +370,7 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
         const int pos = 2 * i - (i & (stride - 1));
         const int par = pos + stride;
         const bool asc = (pos & size) == 0;
-        const float da = bd[pos], dbb = bd[par];
+        const unsigned da = bd[pos], dbb = bd[par];
         const int ia = bi[pos], ib = bi[par];
         const bool a_after_b = da > dbb || (da == dbb && ia > ib);
         if (a_after_b == asc) { bd[pos] = dbb; bd[par] = da; bi[pos] = ib; bi[par] = ia; }

@@ -47,6 +47,24 @@ def test_knn_dense_cluster_takes_the_exact_fallback():
     assert np.array_equal(got[7], np.arange(128))
 
 
+def test_knn_dense_cluster_tightens_the_threshold():
+    """A cluster of 1500 distinct points far denser than the queries' own tile: the bound from the own tile lets the whole
+    cluster through, the candidate buffer (512) would overflow, and the kernel re-derives the bound from the buffer
+    instead of falling back.  Queries inside the cluster, next to it and far from it."""
+    dcp = _dcp()
+    g = torch.Generator(device="cpu").manual_seed(11)
+    x = torch.rand(9000, 3, generator=g) * 100.0
+    centre = torch.tensor([50.0, 50.0, 50.0])
+    x[4000:5500] = centre + (torch.rand(1500, 3, generator=g) - 0.5) * 2.0
+    x[5] = centre
+    x[6] = centre + 3.0
+    x = x.to(DEV)
+    for k in (128, 256, 40):
+        got = dcp.dcp_knn(x, k).cpu().numpy()
+        rows = [5, 6, 7, 100, 2047, 2048, 4000, 4700, 5499, 5500, 8999]
+        assert np.array_equal(got[rows], ko.knn_rows(x.cpu().numpy(), k, rows))
+
+
 def test_knn_structured_atoms_sampled_rows():
     """C4's synthetic assembly (L = 24000), k = 128: sampled queries against the oracle."""
     dcp = _dcp()
