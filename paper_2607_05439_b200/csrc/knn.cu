@@ -530,6 +530,246 @@ __global__ void __launch_bounds__(256) knn_budget_kernel(const float* __restrict
   for (int j = lane; j < k; j += 32) idx[(int64_t)l * k + j] = bi[j];
 }
 
+// ---- structured budget, threshold-select variant (k <= 256): the two classes keep candidate BUFFERS instead of sorted
+// register lists.  A buffer starts unbounded; when it is about to overflow, the k-th smallest key it holds becomes the
+// class's bound (exact bisection of the 32-bit key over the buffer, counted with ballots) and only the entries within it
+// stay -- the own tile is visited first, so the bounds settle after a few such steps and the scan appends little.  After
+// the scan the quotas are known; each class keeps the entries within its exact n-th key, sorts them by (key, index),
+// and the chosen prefixes are sorted together by (d2, index).  More than kCap entries tying within a bound (coincident
+// atoms) send the query to the register-list scan over global memory, which fills the same buffers.
+template <int kPer>
+__device__ __forceinline__ void buf_load(unsigned (&bv)[kPer], const unsigned* key, int n, int lane) {
+#pragma unroll
+  for (int j = 0; j < kPer; ++j) bv[j] = 32 * j + lane < n ? key[32 * j + lane] : 0xffffffffu;
+}
+// smallest key T <= hi0 with #{entries <= T} >= need (hi0 itself must satisfy it)
+template <int kPer>
+__device__ __forceinline__ unsigned buf_bisect(const unsigned (&bv)[kPer], unsigned hi0, int need) {
+  unsigned lo = 0u, hi = hi0;
+  while (lo < hi) {
+    const unsigned mid = lo + ((hi - lo) >> 1);
+    int c = 0;
+#pragma unroll
+    for (int j = 0; j < kPer; ++j) c += __popc(__ballot_sync(0xffffffffu, bv[j] <= mid));
+    if (c >= need) hi = mid; else lo = mid + 1;
+  }
+  return hi;
+}
+// keep the entries <= t, in order; returns the new count
+template <int kPer>
+__device__ __forceinline__ int buf_compact(const unsigned (&bv)[kPer], unsigned* key, int* id, unsigned t, int n, int lane) {
+  int nc = 0;
+#pragma unroll
+  for (int j = 0; j < kPer; ++j) {
+    if (32 * j >= n) break;                                    // warp-uniform
+    const int e = 32 * j + lane;
+    const int iv = e < n ? id[e] : 0;
+    const bool pass = e < n && bv[j] <= t;
+    const unsigned mask = __ballot_sync(0xffffffffu, pass);    // every lane has read chunk j before any lane overwrites it
+    if (pass) { const int slot = nc + __popc(mask & ((1u << lane) - 1u)); key[slot] = bv[j]; id[slot] = iv; }
+    nc += __popc(mask);
+    __syncwarp();
+  }
+  return nc;
+}
+// bitonic sort of n entries by (key, index), padded to a power of two (the buffer has room for it)
+__device__ __forceinline__ void buf_sort(unsigned* key, int* id, int n, int lane) {
+  int P = 32;
+  while (P < n) P <<= 1;
+  for (int e = n + lane; e < P; e += 32) { key[e] = 0xffffffffu; id[e] = 0x7fffffff; }
+  __syncwarp();
+  for (int size = 2; size <= P; size <<= 1) {
+    for (int stride = size >> 1; stride > 0; stride >>= 1) {
+      for (int i = lane; i < (P >> 1); i += 32) {
+        const int pos = 2 * i - (i & (stride - 1));
+        const int par = pos + stride;
+        const bool asc = (pos & size) == 0;
+        const unsigned da = key[pos], dbb = key[par];
+        const int ia = id[pos], ib = id[par];
+        const bool a_after_b = da > dbb || (da == dbb && ia > ib);
+        if (a_after_b == asc) { key[pos] = dbb; key[par] = da; id[pos] = ib; id[par] = ia; }
+      }
+      __syncwarp();
+    }
+  }
+}
+
+// exact fallback of one query: the two-list insertion scan over global memory; leaves each class's first min(k, size)
+// entries, sorted, in its buffer
+template <int NR>
+__device__ __noinline__ void budget_insert_global(const float* __restrict__ x, const int32_t* __restrict__ rid,
+                                                  const int32_t* __restrict__ cid, int L, int k, int l, int n_seq, int split,
+                                                  int lane, unsigned* ak, int* ai, unsigned* bk, int* bi, int* na, int* nb) {
+  const float q0 = __ldg(x + 3 * (int64_t)l), q1 = __ldg(x + 3 * (int64_t)l + 1), q2 = __ldg(x + 3 * (int64_t)l + 2);
+  const int qr = __ldg(rid + l), qc = __ldg(cid + l), win = n_seq - 1;
+  TopList<NR> la, lb;
+  la.init(k);
+  lb.init(k);
+  int cnt_a = 0, cnt_b = 0;
+  for (int c0 = 0; c0 < L; c0 += 32) {
+    const int m = c0 + lane;
+    const bool valid = m < L;
+    const int mm = valid ? m : L - 1;
+    const float a0 = __fsub_rn(__ldg(x + 3 * (int64_t)mm), q0), a1 = __fsub_rn(__ldg(x + 3 * (int64_t)mm + 1), q1);
+    const float a2 = __fsub_rn(__ldg(x + 3 * (int64_t)mm + 2), q2);
+    const unsigned db = __float_as_uint(__fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2)));
+    const bool same = __ldg(cid + mm) == qc;
+    int dr = __ldg(rid + mm) - qr;
+    dr = dr < 0 ? -dr : dr;
+    const bool local = same && dr <= win;
+    const bool in_a = valid && (same || !split), in_b = valid && !same && split;
+    const unsigned ka = db | (local ? 0u : 0x80000000u);
+    cnt_a += __popc(__ballot_sync(0xffffffffu, in_a));
+    cnt_b += __popc(__ballot_sync(0xffffffffu, in_b));
+    const unsigned mka = __ballot_sync(0xffffffffu, in_a && la.beats(ka, m));
+    const unsigned mkb = __ballot_sync(0xffffffffu, in_b && lb.beats(db, m));
+    if (mka) la.insert_chunk(c0, ka, mka, lane);
+    if (mkb) lb.insert_chunk(c0, db, mkb, lane);
+  }
+  *na = cnt_a < k ? cnt_a : k;
+  *nb = cnt_b < k ? cnt_b : k;
+#pragma unroll
+  for (int r = 0; r < NR; ++r) {
+    const int pos = lane * NR + r;
+    if (pos < *na) { ak[pos] = la.key[r]; ai[pos] = la.li[r]; }
+    if (pos < *nb) { bk[pos] = lb.key[r]; bi[pos] = lb.li[r]; }
+  }
+  __syncwarp();
+}
+
+template <int kCap, int NRF>
+__global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __restrict__ x, const int32_t* __restrict__ rid,
+                                                                const int32_t* __restrict__ cid, int32_t* __restrict__ idx,
+                                                                int L, int k, int n_seq, int split, int q_out) {
+  extern __shared__ float smem_knn[];
+  float* sx = smem_knn;
+  float* sy = sx + kTile;
+  float* sz = sy + kTile;
+  int* sr = reinterpret_cast<int*>(sz + kTile);
+  int* sc = sr + kTile;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  constexpr int kPer = kCap / 32;
+  unsigned* ak = reinterpret_cast<unsigned*>(sc + kTile) + wib * (4 * kCap);   // per warp: class A keys, indices, class B keys, indices
+  int* ai = reinterpret_cast<int*>(ak + kCap);
+  unsigned* bk = ak + 2 * kCap;
+  int* bi = reinterpret_cast<int*>(bk + kCap);
+  const int lq = blockIdx.x * 8 + wib;
+  const bool active = lq < L;
+  const int l = active ? lq : L - 1;
+  const float q0 = __ldg(x + 3 * (int64_t)l), q1 = __ldg(x + 3 * (int64_t)l + 1), q2 = __ldg(x + 3 * (int64_t)l + 2);
+  const int qr = __ldg(rid + l), qc = __ldg(cid + l), win = n_seq - 1;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  unsigned thr_a = 0xffffffffu, thr_b = 0xffffffffu;           // the classes' bounds (keys <= bound are kept)
+  int na = 0, nb = 0;                                          // buffer fill
+  int ca = 0, cb = 0;                                          // this lane's share of the class sizes
+  bool over = false;
+  // append the lanes' candidates (key v, atom m) of `mask` to a class buffer; re-bound the buffer when it would overflow
+  auto append = [&](unsigned* key, int* id, int& n, unsigned& thr, unsigned mask, bool pass, unsigned v, int m) {
+    if (over) return;
+    if (n + __popc(mask) > kCap) {
+      __syncwarp();
+      unsigned bv[kPer];
+      buf_load(bv, key, n, lane);
+      thr = buf_bisect(bv, thr, k);                            // the buffer holds more than kCap - 32 >= k entries
+      n = buf_compact(bv, key, id, thr, n, lane);
+      pass = pass && v <= thr;
+      mask = __ballot_sync(0xffffffffu, pass);
+      if (n + __popc(mask) > kCap) { over = true; return; }
+    }
+    if (pass) { const int slot = n + __popc(mask & lt_mask); key[slot] = v; id[slot] = m; }
+    n += __popc(mask);
+  };
+  const int n_tiles = (L + kTile - 1) / kTile;
+  const int own = (blockIdx.x * 8) / kTile;
+  for (int tt = 0; tt < n_tiles; ++tt) {
+    const int tile = tt == 0 ? own : (tt <= own ? tt - 1 : tt);
+    const int t0 = tile * kTile;
+    __syncthreads();
+    for (int e = threadIdx.x; e < kTile; e += blockDim.x) {
+      const int m = t0 + e;
+      sx[e] = m < L ? __ldg(x + 3 * (int64_t)m) : 0.f;
+      sy[e] = m < L ? __ldg(x + 3 * (int64_t)m + 1) : 0.f;
+      sz[e] = m < L ? __ldg(x + 3 * (int64_t)m + 2) : 0.f;
+      sr[e] = m < L ? __ldg(rid + m) : 0;
+      sc[e] = m < L ? __ldg(cid + m) : -1;
+    }
+    __syncthreads();
+    if (!active) continue;
+    const int n_here = (L - t0 < kTile ? L - t0 : kTile);
+    for (int c0 = 0; c0 < n_here; c0 += 64) {                   // two chunks per step: independent loads and arithmetic
+      unsigned db[2], ka[2], ma[2], mb[2];
+      bool pa[2], pb[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int e = (c0 + 32 * u + lane) & (kTile - 1);
+        const bool valid = c0 + 32 * u + lane < n_here;
+        const float a0 = __fsub_rn(sx[e], q0), a1 = __fsub_rn(sy[e], q1), a2 = __fsub_rn(sz[e], q2);
+        db[u] = __float_as_uint(__fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2)));
+        const bool same = sc[e] == qc;
+        int dr = sr[e] - qr;
+        dr = dr < 0 ? -dr : dr;
+        const bool local = same && dr <= win;
+        const bool in_a = valid && (same || !split), in_b = valid && !same && split;
+        ka[u] = db[u] | (local ? 0u : 0x80000000u);
+        ca += in_a ? 1 : 0;
+        cb += in_b ? 1 : 0;
+        pa[u] = in_a && ka[u] <= thr_a;
+        pb[u] = in_b && db[u] <= thr_b;
+        ma[u] = __ballot_sync(0xffffffffu, pa[u]);
+        mb[u] = __ballot_sync(0xffffffffu, pb[u]);
+      }
+      if ((ma[0] | ma[1] | mb[0] | mb[1]) == 0) continue;
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int m = t0 + c0 + 32 * u + lane;
+        if (ma[u]) append(ak, ai, na, thr_a, ma[u], pa[u], ka[u], m);
+        if (mb[u]) append(bk, bi, nb, thr_b, mb[u], pb[u], db[u], m);
+      }
+    }
+  }
+  if (!active) return;
+  __syncwarp();
+  int cnt_a = ca, cnt_b = cb;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { cnt_a += __shfl_xor_sync(0xffffffffu, cnt_a, o); cnt_b += __shfl_xor_sync(0xffffffffu, cnt_b, o); }
+  if (over) budget_insert_global<NRF>(x, rid, cid, L, k, l, n_seq, split, lane, ak, ai, bk, bi, &na, &nb);
+  // quotas (oracle/knn_budget.py): the foreign quota first, the own chain gets the rest, leftovers go back
+  int n_out = cnt_b < q_out ? cnt_b : q_out;
+  const int n_in = cnt_a < k - n_out ? cnt_a : k - n_out;
+  n_out = cnt_b < k - n_in ? cnt_b : k - n_in;
+  // each class: the entries within its exact n-th key, sorted by (key, index); the first n are the class's share
+  if (n_in > 0) {
+    unsigned bv[kPer];
+    buf_load(bv, ak, na, lane);
+    const unsigned t = buf_bisect(bv, thr_a, n_in);
+    na = buf_compact(bv, ak, ai, t, na, lane);
+    buf_sort(ak, ai, na, lane);
+  }
+  if (n_out > 0) {
+    unsigned bv[kPer];
+    buf_load(bv, bk, nb, lane);
+    const unsigned t = buf_bisect(bv, thr_b, n_out);
+    nb = buf_compact(bv, bk, bi, t, nb, lane);
+    buf_sort(bk, bi, nb, lane);
+  }
+  // the two prefixes together, by (d2, index): class A loses its flag bit, class B follows it in A's buffer
+  for (int j = lane; j < n_in; j += 32) ak[j] &= 0x7fffffffu;
+  for (int j = lane; j < n_out; j += 32) { ak[n_in + j] = bk[j]; ai[n_in + j] = bi[j]; }
+  __syncwarp();
+  buf_sort(ak, ai, n_in + n_out, lane);
+  for (int j = lane; j < k; j += 32) idx[(int64_t)l * k + j] = ai[j];
+}
+
+template <int kCap, int NRF>
+cudaError_t launch_budget_select(const float* x, const int32_t* rid, const int32_t* cid, int32_t* idx, int L, int k, int n_seq,
+                                 int split, int q_out, cudaStream_t st) {
+  const size_t smem = (size_t)(5 * kTile + 8 * 4 * kCap) * 4;
+  cudaError_t e = cudaFuncSetAttribute(knn_budget_select_kernel<kCap, NRF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  knn_budget_select_kernel<kCap, NRF><<<(unsigned)((L + 7) / 8), 256, smem, st>>>(x, rid, cid, idx, L, k, n_seq, split, q_out);
+  return cudaGetLastError();
+}
+
 template <int NR>
 cudaError_t launch_budget(const float* x, const int32_t* rid, const int32_t* cid, int32_t* idx, int L, int k, int n_seq, int split,
                           int q_out, cudaStream_t st) {
@@ -548,6 +788,9 @@ cudaError_t launch_knn_budget(const float* x, const int32_t* rid, const int32_t*
   int q_out = k / 4 > 32 ? k / 4 : 32;
   if (q_out > k - 1) q_out = k - 1;
   const int nr = (k + 31) / 32;
+  // threshold-select kernel (candidate buffers of >= 2 k entries per class); larger k: the register-list kernel
+  if (k <= 128) return launch_budget_select<256, 4>(x, rid, cid, idx, (int)L, k, n_seq, split, q_out, st);
+  if (k <= 256) return launch_budget_select<512, 8>(x, rid, cid, idx, (int)L, k, n_seq, split, q_out, st);
   if (nr <= 1) return launch_budget<1>(x, rid, cid, idx, (int)L, k, n_seq, split, q_out, st);
   if (nr <= 2) return launch_budget<2>(x, rid, cid, idx, (int)L, k, n_seq, split, q_out, st);
   if (nr <= 4) return launch_budget<4>(x, rid, cid, idx, (int)L, k, n_seq, split, q_out, st);

@@ -111,6 +111,9 @@ def _topology(L, n_chains, atoms_per_residue, seed):
     (700, 300, 9, 10, 2),     # NR = 16 lists
     (1000, 512, 5, 8, 2),     # the largest budget
     (40, 1, 4, 4, 2),         # k = 1: the query itself
+    (5000, 128, 12, 8, 2),    # select kernel, 256-entry buffers re-bounded many times
+    (3000, 200, 8, 8, 2),     # select kernel with 512-entry buffers
+    (2500, 256, 3, 8, 2),     # no split, k = 256
 ])
 def test_knn_budget_bit_exact(L, k, n_chains, apr, n_seq):
     dcp = _dcp()
@@ -134,6 +137,20 @@ def test_knn_budget_ties_and_short_chains():
     for k, n_seq in ((96, 2), (40, 1), (400, 2)):
         got = dcp.dcp_knn_budget(x.to(DEV), rid.to(DEV), cid.to(DEV), k, 6, n_seq=n_seq).cpu().numpy()
         assert np.array_equal(got, kbo.knn_budget(x.numpy(), rid.numpy(), cid.numpy(), k, n_seq=n_seq))
+
+
+def test_knn_budget_coincident_atoms_take_the_exact_fallback():
+    """900 coincident atoms spread over four chains (+ a few others): more entries tie within a class bound than a
+    candidate buffer holds, so the queries take the register-list fallback; order = (flag, distance, index)."""
+    dcp = _dcp()
+    L = 1000
+    x = torch.zeros(L, 3)
+    x[900:] = torch.arange(100, dtype=torch.float32)[:, None] * 0.5 + 2.0
+    cid = (torch.arange(L) // 250).to(torch.int32)
+    rid = (torch.arange(L) // 6).to(torch.int32)
+    for k in (128, 200):
+        got = dcp.dcp_knn_budget(x.to(DEV), rid.to(DEV), cid.to(DEV), k, 4, n_seq=2).cpu().numpy()
+        assert np.array_equal(got, kbo.knn_budget(x.numpy(), rid.numpy(), cid.numpy(), k, n_seq=2))
 
 
 def test_knn_budget_reduces_to_plain_knn_on_the_device():
