@@ -17,6 +17,8 @@
 // moves + one shuffle).  A window of indices around the query is scanned first, which tightens the k-th distance
 // early (same-chain atoms are close in space), so that few of the remaining L candidates are ever inserted and the
 // scan (about a dozen instructions per 32 candidates) dominates.
+#include <type_traits>
+
 #include "kernels.h"
 
 namespace dcp {
@@ -645,11 +647,10 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
   float* sx = smem_knn;
   float* sy = sx + kTile;
   float* sz = sy + kTile;
-  int* sr = reinterpret_cast<int*>(sz + kTile);
-  int* sc = sr + kTile;
+  int2* scr = reinterpret_cast<int2*>(sz + kTile);             // (chain id, residue id) per candidate: one 64-bit load
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   constexpr int kPer = kCap / 32;
-  unsigned* ak = reinterpret_cast<unsigned*>(sc + kTile) + wib * (4 * kCap);   // per warp: class A keys, indices, class B keys, indices
+  unsigned* ak = reinterpret_cast<unsigned*>(scr + kTile) + wib * (4 * kCap);   // per warp: class A keys, indices, class B keys, indices
   int* ai = reinterpret_cast<int*>(ak + kCap);
   unsigned* bk = ak + 2 * kCap;
   int* bi = reinterpret_cast<int*>(bk + kCap);
@@ -661,7 +662,9 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
   const unsigned lt_mask = (1u << lane) - 1u;
   unsigned thr_a = 0xffffffffu, thr_b = 0xffffffffu;           // the classes' bounds (keys <= bound are kept)
   int na = 0, nb = 0;                                          // buffer fill
-  int ca = 0, cb = 0;                                          // this lane's share of the class sizes
+  int cs = 0;                                                  // this lane's share of the own chain's size
+  const bool has_win = win >= 0;                               // n_seq = 0: no atom is sequence-local
+  const unsigned win2 = has_win ? 2u * (unsigned)win : 0u;
   bool over = false;
   // append the lanes' candidates (key v, atom m) of `mask` to a class buffer; re-bound the buffer when it would overflow
   auto append = [&](unsigned* key, int* id, int& n, unsigned& thr, unsigned mask, bool pass, unsigned v, int m) {
@@ -690,48 +693,50 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
       sx[e] = m < L ? __ldg(x + 3 * (int64_t)m) : 0.f;
       sy[e] = m < L ? __ldg(x + 3 * (int64_t)m + 1) : 0.f;
       sz[e] = m < L ? __ldg(x + 3 * (int64_t)m + 2) : 0.f;
-      sr[e] = m < L ? __ldg(rid + m) : 0;
-      sc[e] = m < L ? __ldg(cid + m) : -1;
+      scr[e] = m < L ? make_int2(__ldg(cid + m), __ldg(rid + m)) : make_int2(-1, 0);
     }
     __syncthreads();
     if (!active) continue;
     const int n_here = (L - t0 < kTile ? L - t0 : kTile);
-    for (int c0 = 0; c0 < n_here; c0 += 64) {                   // two chunks per step: independent loads and arithmetic
-      unsigned db[2], ka[2], ma[2], mb[2];
-      bool pa[2], pb[2];
+    // four chunks per step: independent loads and arithmetic; only the last tile can be ragged, the others check no bounds
+    auto scan = [&](auto RAGGED) {
+      for (int c0 = 0; c0 < n_here; c0 += 128) {
+        unsigned db[4], ka[4], ma[4], mb[4];
+        bool pa[4], pb[4];
 #pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        const int e = (c0 + 32 * u + lane) & (kTile - 1);
-        const bool valid = c0 + 32 * u + lane < n_here;
-        const float a0 = __fsub_rn(sx[e], q0), a1 = __fsub_rn(sy[e], q1), a2 = __fsub_rn(sz[e], q2);
-        db[u] = __float_as_uint(__fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2)));
-        const bool same = sc[e] == qc;
-        int dr = sr[e] - qr;
-        dr = dr < 0 ? -dr : dr;
-        const bool local = same && dr <= win;
-        const bool in_a = valid && (same || !split), in_b = valid && !same && split;
-        ka[u] = db[u] | (local ? 0u : 0x80000000u);
-        ca += in_a ? 1 : 0;
-        cb += in_b ? 1 : 0;
-        pa[u] = in_a && ka[u] <= thr_a;
-        pb[u] = in_b && db[u] <= thr_b;
-        ma[u] = __ballot_sync(0xffffffffu, pa[u]);
-        mb[u] = __ballot_sync(0xffffffffu, pb[u]);
-      }
-      if ((ma[0] | ma[1] | mb[0] | mb[1]) == 0) continue;
+        for (int u = 0; u < 4; ++u) {
+          const int e = c0 + 32 * u + lane;                     // < kTile
+          const float a0 = __fsub_rn(sx[e], q0), a1 = __fsub_rn(sy[e], q1), a2 = __fsub_rn(sz[e], q2);
+          db[u] = __float_as_uint(__fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2)));
+          const int2 cr = scr[e];
+          const bool valid = !decltype(RAGGED)::value || e < n_here;
+          const bool same = cr.x == qc && valid;
+          const bool local = same && has_win && (unsigned)(cr.y - qr + win) <= win2;   // |residue - query's| <= win
+          cs += same ? 1 : 0;
+          ka[u] = local ? db[u] : (db[u] | 0x80000000u);
+          pa[u] = valid && (same || !split) && ka[u] <= thr_a;
+          pb[u] = valid && !same && split && db[u] <= thr_b;
+          ma[u] = __ballot_sync(0xffffffffu, pa[u]);
+          mb[u] = __ballot_sync(0xffffffffu, pb[u]);
+        }
+        if (((ma[0] | ma[1]) | (ma[2] | ma[3]) | (mb[0] | mb[1]) | (mb[2] | mb[3])) == 0) continue;
 #pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        const int m = t0 + c0 + 32 * u + lane;
-        if (ma[u]) append(ak, ai, na, thr_a, ma[u], pa[u], ka[u], m);
-        if (mb[u]) append(bk, bi, nb, thr_b, mb[u], pb[u], db[u], m);
+        for (int u = 0; u < 4; ++u) {
+          const int m = t0 + c0 + 32 * u + lane;
+          if (ma[u]) append(ak, ai, na, thr_a, ma[u], pa[u], ka[u], m);
+          if (mb[u]) append(bk, bi, nb, thr_b, mb[u], pb[u], db[u], m);
+        }
       }
-    }
+    };
+    if (n_here == kTile) scan(std::false_type{}); else scan(std::true_type{});
   }
   if (!active) return;
   __syncwarp();
-  int cnt_a = ca, cnt_b = cb;
+  // class sizes: the own chain's count; every atom without a split
+  int n_same = cs;
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) { cnt_a += __shfl_xor_sync(0xffffffffu, cnt_a, o); cnt_b += __shfl_xor_sync(0xffffffffu, cnt_b, o); }
+  for (int o = 16; o > 0; o >>= 1) n_same += __shfl_xor_sync(0xffffffffu, n_same, o);
+  const int cnt_a = split ? n_same : L, cnt_b = split ? L - n_same : 0;
   if (over) budget_insert_global<NRF>(x, rid, cid, L, k, l, n_seq, split, lane, ak, ai, bk, bi, &na, &nb);
   // quotas (oracle/knn_budget.py): the foreign quota first, the own chain gets the rest, leftovers go back
   int n_out = cnt_b < q_out ? cnt_b : q_out;
