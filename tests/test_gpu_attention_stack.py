@@ -195,6 +195,38 @@ def test_attention_stack_cached_matches_oracle_and_streaming(I, copies, c, n_blo
     assert torch.equal(again, a_c)
 
 
+def test_attention_stack_cached_full_size_block_sampled():
+    """The configuration bench.py --workload D2 --cached times (I = 3000, c_token = 768: 94 x 188 cache tiles per block,
+    282 work units with three key segments each, two bias passes when 18 blocks are given): 17 blocks on the device --
+    one pass of 15 and one of 2 --, block 17 checked on sampled rows against the oracle started from the device's own
+    latent after 16 blocks, and the call as a whole equal to 16 + 1 blocks in two calls."""
+    dcp = _dcp()
+    cfg = syn.small_config("D2", I=3000, c_s=768, c_z=128, H=16, c=48, dtype="bf16", seed=2, structured=True, copies=60)
+    a0, z = syn.make_s(cfg, DEV), syn.make_z(cfg, DEV)
+    blocks = _blocks(cfg, 17)
+    cache = torch.empty(dcp.dcp_attention_stack_cache_bytes(cfg.I, 17), dtype=torch.uint8, device=DEV)
+    a16 = a0.clone()
+    dcp.dcp_attention_stack_cached(a16, z, blocks[:16], cfg.H, cfg.c, bias_cache=cache)
+    a17 = a16.clone()
+    dcp.dcp_attention_stack_cached(a17, z, blocks[16:], cfg.H, cfg.c, bias_cache=cache)
+    full = a0.clone()
+    dcp.dcp_attention_stack_cached(full, z, blocks, cfg.H, cfg.c, bias_cache=cache)
+    assert torch.equal(full, a17)
+    assert bool(torch.isfinite(full.float()).all())
+    rows = syn.sample_rows(cfg.I, 32, boundaries=(32, 1000, 2976), seed=6)
+    idx = torch.as_tensor(rows, device=DEV)
+    upd_ref = orc.pair_bias_attention_rows(util.np64(a16), util.np32(z.index_select(0, idx)), rows, util.weights_np(blocks[16]),
+                                           cfg.H, cfg.c)
+    a16r = util.np64(a16.index_select(0, idx))
+    ref = _bf(a16r + upd_ref)
+    got = util.np64(a17.index_select(0, idx))
+    rel = np.linalg.norm((got - a16r) - upd_ref) / np.linalg.norm(upd_ref)
+    assert rel <= 2e-2, f"update rel-L2 {rel:.3e}"
+    assert np.all(np.abs(got - ref) <= util.TOL_BF16_MAXABS + 2.0 ** -7 * np.abs(ref)), np.abs(got - ref).max()
+    del z, cache
+    torch.cuda.empty_cache()
+
+
 def test_attention_stack_cached_error_paths():
     dcp = _dcp()
     cfg = syn.small_config("cserr", I=64, c_s=768, c_z=128, H=16, c=48, dtype="bf16", seed=5)
