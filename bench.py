@@ -867,10 +867,13 @@ def run_knn(args, rank, world, local_rank):
     peak = probe_pairs / (p0.elapsed_ms(p1) / 5 * 1e-3) / 1e9
     roofline = {"bound": "alu", "achieved": pairs / (kms * 1e-3) / 1e9, "peak": peak, "unit": "Gpair/s",
                 "frac": pairs / (kms * 1e-3) / 1e9 / peak, "traffic": None,
-                "kernel": "knn_budget_kernel" if budget else "knn_select_kernel" if k <= 256 else "knn_kernel",
+                "kernel": ("knn_budget_select_kernel" if k <= 256 else "knn_budget_kernel") if budget else "knn_select_kernel",
                 "peak_source": "measured in this run: dcp_probe_scan (the candidate scan without selection); the instruction-count "
                                "bound 148 SMs x 128 lanes x 1.965 GHz / 12 would be %.0f Gpair/s" % derived,
-                "kernel_ms": kms, "kernel_share_of_step": 1.0}
+                "kernel_ms": kms, "kernel_share_of_step": 1.0,
+                "note": "pairs = L x L (every query against every atom, the paper's cdist); the peak is the brute-force scan of "
+                        "all of them -- knn_select_kernel skips 128-atom chunks whose bounding box lies beyond the query's "
+                        "current bound (exactly, by monotone rounding), so frac can exceed 1 on spatially coherent inputs"}
     cpu = None
     if rank == 0 and not args.no_cpu_baseline:
         rows = syn.sample_rows(L, args.cpu_rows or 3000, seed=0)

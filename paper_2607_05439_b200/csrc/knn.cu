@@ -10,13 +10,15 @@
 // arithmetic is pinned: IEEE binary32, round to nearest, NO fused multiply-add, t = x_m - x_l per coordinate,
 // d2 = (t0 t0 + t1 t1) + t2 t2 -- the oracle (oracle/knn.py) uses the same operations and the result is bit-exact.
 //
-// knn_kernel (k > 256; knn_select_kernel below serves k <= 256): one warp per query.  The list of k (d2, index)
-// pairs, sorted lexicographically, lives in registers, NR = k / 32
-// (rounded up) consecutive positions per lane.  Candidates are visited 128 at a time; a ballot picks those that beat
-// the current k-th entry, and each is inserted by a ballot-count of its position and a one-place shift (register
-// moves + one shuffle).  A window of indices around the query is scanned first, which tightens the k-th distance
-// early (same-chain atoms are close in space), so that few of the remaining L candidates are ever inserted and the
-// scan (about a dozen instructions per 32 candidates) dominates.
+// One warp per query, 8 queries per CTA sharing shared-memory tiles of 2048 candidates (three coordinate planes:
+// conflict-free reads; the [L][3] rows in global memory cost 3-4 L1 wavefronts per 32-candidate load).  The tile of the
+// CTA's own atoms comes first (atoms close in index are mostly close in space, so the bound on the k-th distance tightens
+// early); the (d2, index) order makes the result independent of the visiting order.
+//   knn_select_kernel      threshold select with candidate buffers (below)
+//   knn_insert_global      exact fallback of a single query: the sorted list of k (d2, index) pairs lives in registers
+//                          (NR = k / 32 per lane); candidates that beat the k-th entry (one ballot per 32) are inserted by a
+//                          ballot-count of their position and a one-place shift.  Round 1's first kernel worked this way for
+//                          every query (2.81 ms at L = 24000, k = 128).
 #include <type_traits>
 
 #include "kernels.h"
@@ -28,115 +30,16 @@ namespace {
 constexpr float kInf = __builtin_huge_valf();
 constexpr int kTile = 2048;   // candidates per shared-memory tile (3 x 8 KB)
 
-template <int NR>
-__global__ void __launch_bounds__(256) knn_kernel(const float* __restrict__ x, int32_t* __restrict__ idx, int L, int k) {
-  const int lane = threadIdx.x & 31;
-  __shared__ float sx[kTile], sy[kTile], sz[kTile];
-  const int lq = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  const bool active = lq < L;                           // inactive warps still help staging the tiles
-  const int l = active ? lq : L - 1;
-  const float q0 = __ldg(x + 3 * (int64_t)l), q1 = __ldg(x + 3 * (int64_t)l + 1), q2 = __ldg(x + 3 * (int64_t)l + 2);
-  float ld[NR];       // list position lane * NR + r, sorted by (d2, index)
-  int li[NR];
-#pragma unroll
-  for (int r = 0; r < NR; ++r) { ld[r] = kInf; li[r] = 0x7fffffff; }
-  const int last_lane = (k - 1) / NR, last_r = (k - 1) % NR;
-  float tau = kInf;   // (d2, index) of list position k - 1: the current k-th best
-  int tau_i = 0x7fffffff;
-
-  // insert the candidates of one 32-wide chunk that beat the k-th entry, in increasing index
-  auto insert_chunk = [&](int c0, float d, unsigned mask) {
-    while (mask) {
-      const int b = __ffs(mask) - 1;
-      mask &= mask - 1;
-      const float dn = __shfl_sync(0xffffffffu, d, b);
-      const int mn = c0 + b;
-      if (!(dn < tau || (dn == tau && mn < tau_i))) continue;      // the k-th entry moved meanwhile (warp-uniform)
-      // position = number of entries that come before (dn, mn) in (d2, index) order
-      int pos = 0;
-#pragma unroll
-      for (int r = 0; r < NR; ++r) pos += __popc(__ballot_sync(0xffffffffu, ld[r] < dn || (ld[r] == dn && li[r] < mn)));
-      const int pl = pos / NR, pr = pos % NR;
-      // shift positions pos .. one place to the right (the old k-th entry falls off), insert at pos
-      const float up_d = __shfl_up_sync(0xffffffffu, ld[NR - 1], 1);
-      const int up_i = __shfl_up_sync(0xffffffffu, li[NR - 1], 1);
-      if (lane > pl) {
-#pragma unroll
-        for (int r = NR - 1; r > 0; --r) { ld[r] = ld[r - 1]; li[r] = li[r - 1]; }
-        ld[0] = up_d; li[0] = up_i;
-      } else if (lane == pl) {
-#pragma unroll
-        for (int r = NR - 1; r > 0; --r)
-          if (r > pr) { ld[r] = ld[r - 1]; li[r] = li[r - 1]; }
-#pragma unroll
-        for (int r = 0; r < NR; ++r)
-          if (r == pr) { ld[r] = dn; li[r] = mn; }
-      }
-      float tl = ld[0];
-      int ti = li[0];
-#pragma unroll
-      for (int r = 1; r < NR; ++r) { tl = r == last_r ? ld[r] : tl; ti = r == last_r ? li[r] : ti; }
-      tau = __shfl_sync(0xffffffffu, tl, last_lane);
-      tau_i = __shfl_sync(0xffffffffu, ti, last_lane);
-    }
-  };
-  // The 8 queries of a block scan the same candidates: tiles of kTile atoms are staged once per block in shared memory
-  // as three coordinate planes (conflict-free reads; the [L][3] rows in global memory cost 3-4 L1 wavefronts per
-  // 32-candidate load and made the scan L1-bound).  Tile order: the tile of the block's own atoms first (atoms close
-  // in index are mostly close in space, so the k-th distance tightens early and few later candidates are inserted),
-  // then the others; the (d2, index) order of the list makes the result independent of the visiting order.
-  const int n_tiles = (L + kTile - 1) / kTile;
-  const int own = (blockIdx.x * (blockDim.x >> 5)) / kTile;
-  for (int tt = 0; tt < n_tiles; ++tt) {
-    const int tile = tt == 0 ? own : (tt <= own ? tt - 1 : tt);
-    const int t0 = tile * kTile;
-    __syncthreads();                                   // every warp is done with the previous tile
-    for (int e = threadIdx.x; e < kTile; e += blockDim.x) {
-      const int m = t0 + e;
-      sx[e] = m < L ? __ldg(x + 3 * (int64_t)m) : 0.f;
-      sy[e] = m < L ? __ldg(x + 3 * (int64_t)m + 1) : 0.f;
-      sz[e] = m < L ? __ldg(x + 3 * (int64_t)m + 2) : 0.f;
-    }
-    __syncthreads();
-    if (!active) continue;
-    const int n_here = (L - t0 < kTile ? L - t0 : kTile);
-    for (int c0 = 0; c0 < n_here; c0 += 128) {          // four chunks per step: independent loads and arithmetic
-      float d[4];
-      unsigned mk[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int e = (c0 + 32 * u + lane) & (kTile - 1);   // c0 + 128 may run past the tile when n_here is ragged
-        const float a0 = __fsub_rn(sx[e], q0), a1 = __fsub_rn(sy[e], q1), a2 = __fsub_rn(sz[e], q2);
-        const float dd = __fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2));
-        d[u] = c0 + 32 * u + lane < n_here ? dd : kInf;
-      }
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        const int m = t0 + c0 + 32 * u + lane;
-        mk[u] = __ballot_sync(0xffffffffu, d[u] < tau || (d[u] == tau && m < tau_i));
-      }
-      if ((mk[0] | mk[1] | mk[2] | mk[3]) == 0) continue;
-#pragma unroll 1
-      for (int u = 0; u < 4; ++u)
-        if (mk[u]) insert_chunk(t0 + c0 + 32 * u, d[u], mk[u]);
-    }
-  }
-  if (!active) return;
-#pragma unroll
-  for (int r = 0; r < NR; ++r) {
-    const int pos = lane * NR + r;
-    if (pos < k) idx[(int64_t)l * k + pos] = li[r];
-  }
-}
-
-// ---- threshold-select variant (k <= 256): no sorted list is maintained while scanning.
+// ---- threshold select (k <= 512): no sorted list is maintained while scanning.
 //   1. own tile (2048 atoms): each lane keeps the r = ceil(k / 32) smallest of its 64 distances while they stream past
 //      (nothing else stays in registers); the largest of the lanes' r-th smallest is a bound T1 with at least k of the
 //      tile's distances <= T1.  A second pass appends the tile's entries <= T1 to the per-warp shared-memory buffer,
 //      a bisection of the binary32 bit pattern over the BUFFER (16 values per lane, counted with ballots) tightens the
 //      bound to a threshold T a few percent above the tile's own k-th distance, and the buffer is compacted to <= T;
 //   2. one scan over the other tiles appends every (d2, index) with d2 <= T (one ballot + one prefix popcount per 32
-//      candidates; typically 1.5 k .. 2 k entries in the end);
+//      candidates; typically 1.5 k .. 2 k entries in the end) -- but only over the 128-atom chunks whose bounding box
+//      reaches within T: the bound applies the pinned arithmetic to the query-to-box gaps, rounding is monotone, so a
+//      skipped chunk provably holds no candidate; a buffer about to overflow is re-bounded by its own k-th distance;
 //   3. a full bisection over the buffer finds the exact k-th distance D, the entries <= D (k of them unless distances
 //      tie) are compacted and sorted by (d2, index) with a bitonic network: the first k are the answer.
 // Same distances, same (d2, index) order as knn_kernel: the result is identical.  A query whose buffer overflows
@@ -214,6 +117,8 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
   unsigned* bd = reinterpret_cast<unsigned*>(sz + kTile) + wib * (2 * kCap);   // per-warp buffer: kCap distances (bit patterns),
   int* bi = reinterpret_cast<int*>(bd + kCap);                                 // kCap indices
   constexpr int kPer = kCap / 32;                              // buffer entries per lane
+  constexpr int NS = kCap / 64;                                // per-lane smallest-values slots of step 1a: >= ceil(k / 32)
+  float* box = sz + kTile + 8 * (2 * kCap);                    // per tile: bounding boxes of its 16 chunks of 128 atoms, [16][lo xyz, hi xyz]
   constexpr unsigned kInfBits = 0x7f800000u;
   const int lq = blockIdx.x * 8 + wib;
   const bool active = lq < L;
@@ -237,6 +142,7 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
 #pragma unroll
       for (int j = 0; j < kPer; ++j) c += __popc(__ballot_sync(0xffffffffu, bv[j] <= mid));
       if (c >= need) hi = mid; else lo = mid + 1;
+      if (c == need) break;                                    // exactly `need` entries are <= mid: the set is settled
     }
     return hi;
   };
@@ -297,25 +203,54 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
     }
     __syncthreads();
     const int n_here = (L - t0 < kTile ? L - t0 : kTile);
+    if (tt != 0) {
+      // bounding boxes of the tile's 128-atom chunks (atoms close in index are mostly close in space): warp w takes
+      // chunks 2 w and 2 w + 1; an empty chunk gets lo = +inf, hi = -inf
+#pragma unroll
+      for (int cc = 0; cc < 2; ++cc) {
+        const int ch = 2 * wib + cc;
+        float lo0 = kInf, lo1 = kInf, lo2 = kInf, hi0 = -kInf, hi1 = -kInf, hi2 = -kInf;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int e = ch * 128 + 32 * i + lane;
+          if (e < n_here) {
+            lo0 = fminf(lo0, sx[e]); hi0 = fmaxf(hi0, sx[e]);
+            lo1 = fminf(lo1, sy[e]); hi1 = fmaxf(hi1, sy[e]);
+            lo2 = fminf(lo2, sz[e]); hi2 = fmaxf(hi2, sz[e]);
+          }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          lo0 = fminf(lo0, __shfl_xor_sync(0xffffffffu, lo0, o)); hi0 = fmaxf(hi0, __shfl_xor_sync(0xffffffffu, hi0, o));
+          lo1 = fminf(lo1, __shfl_xor_sync(0xffffffffu, lo1, o)); hi1 = fmaxf(hi1, __shfl_xor_sync(0xffffffffu, hi1, o));
+          lo2 = fminf(lo2, __shfl_xor_sync(0xffffffffu, lo2, o)); hi2 = fmaxf(hi2, __shfl_xor_sync(0xffffffffu, hi2, o));
+        }
+        if (lane == 0) {
+          box[ch * 6] = lo0; box[ch * 6 + 1] = lo1; box[ch * 6 + 2] = lo2;
+          box[ch * 6 + 3] = hi0; box[ch * 6 + 4] = hi1; box[ch * 6 + 5] = hi2;
+        }
+      }
+      __syncthreads();
+    }
     if (tt == 0) {
       // ---- 1a. the r smallest distances of each lane's share of the own tile
       const int need = k < n_here ? k : n_here;
-      const int r = (need + 31) >> 5;                          // <= 8 (k <= 256)
-      unsigned sm[8];
+      const int r = (need + 31) >> 5;                          // <= NS (k <= kCap / 2)
+      unsigned sm[NS];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) sm[j] = kInfBits;
+      for (int j = 0; j < NS; ++j) sm[j] = kInfBits;
 #pragma unroll 4
       for (int i = 0; i < kTile / 32; ++i) {
         const int e = 32 * i + lane;
         unsigned v = e < n_here ? dist_bits(e) : kInfBits;
-        if (__any_sync(0xffffffffu, v < sm[7])) {
+        if (__any_sync(0xffffffffu, v < sm[NS - 1])) {
 #pragma unroll
-          for (int j = 0; j < 8; ++j) { const unsigned lo = min(sm[j], v); v = max(sm[j], v); sm[j] = lo; }
+          for (int j = 0; j < NS; ++j) { const unsigned lo = min(sm[j], v); v = max(sm[j], v); sm[j] = lo; }
         }
       }
       unsigned sr = sm[0];
 #pragma unroll
-      for (int j = 1; j < 8; ++j) sr = j == r - 1 ? sm[j] : sr;
+      for (int j = 1; j < NS; ++j) sr = j == r - 1 ? sm[j] : sr;
       thr = n_here >= k ? __reduce_max_sync(0xffffffffu, sr) : kInfBits;   // T1; fewer than k atoms: no bound
       // ---- 1b. the own tile's entries <= T1 -> buffer
 #pragma unroll 4
@@ -333,14 +268,28 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
         cnt = compact(bv, thr, cnt);
       }
     } else {
-      // ---- 2. every other tile: four chunks per step
-      for (int c0 = 0; c0 < n_here; c0 += 128) {
+      // ---- 2. every other tile: the chunks whose bounding box reaches within the bound, four 32-candidate pieces per step.
+      // Lane c < 16 takes chunk c: lb = the pinned distance arithmetic applied to the per-axis gaps between the query and
+      // the box (sub, mul, add, add, each rounded to nearest, no FMA).  Rounding is monotone, so every atom of the chunk has
+      // a computed d2 >= lb: a chunk with lb > T holds no candidate, and skipping it changes no bit of the result.
+      float lb = kInf;
+      if (lane < 16) {
+        const float* bx = box + lane * 6;
+        const float g0 = fmaxf(fmaxf(__fsub_rn(bx[0], q0), __fsub_rn(q0, bx[3])), 0.f);
+        const float g1 = fmaxf(fmaxf(__fsub_rn(bx[1], q1), __fsub_rn(q1, bx[4])), 0.f);
+        const float g2 = fmaxf(fmaxf(__fsub_rn(bx[2], q2), __fsub_rn(q2, bx[5])), 0.f);
+        lb = __fadd_rn(__fadd_rn(__fmul_rn(g0, g0), __fmul_rn(g1, g1)), __fmul_rn(g2, g2));
+      }
+      unsigned todo = __ballot_sync(0xffffffffu, lane < 16 && __float_as_uint(lb) <= thr);
+      while (todo) {
+        const int c0 = (__ffs(todo) - 1) * 128;
+        todo &= todo - 1;
         unsigned dbv[4], mk[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-          const int e = (c0 + 32 * u + lane) & (kTile - 1);
+          const int e = c0 + 32 * u + lane;
           dbv[u] = dist_bits(e);
-          mk[u] = __ballot_sync(0xffffffffu, dbv[u] <= thr && c0 + 32 * u + lane < n_here);
+          mk[u] = __ballot_sync(0xffffffffu, dbv[u] <= thr && e < n_here);
         }
         if ((mk[0] | mk[1] | mk[2] | mk[3]) == 0) continue;
 #pragma unroll
@@ -810,19 +759,19 @@ cudaError_t launch_knn(const float* x, int32_t* idx, int64_t L, int k, cudaStrea
   const unsigned blocks = (unsigned)((L + 7) / 8);
   // threshold-select kernel: shared tiles (24 KB) + 8 per-warp candidate buffers (8 bytes per entry)
   if (k <= 256) {
-    const size_t smem = (size_t)(3 * kTile + 8 * 2 * 512) * sizeof(float);
+    const size_t smem = (size_t)(3 * kTile + 8 * 2 * 512 + 96) * sizeof(float);
     cudaError_t e = cudaFuncSetAttribute(knn_select_kernel<512, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     knn_select_kernel<512, 8><<<blocks, 256, smem, st>>>(x, idx, (int)L, k);
     return cudaGetLastError();
   }
-  // k > 256: the buffered candidates would outgrow shared memory too often; the register-list kernel serves them
-  if (nr <= 1) knn_kernel<1><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);
-  else if (nr <= 2) knn_kernel<2><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);
-  else if (nr <= 4) knn_kernel<4><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);
-  else if (nr <= 8) knn_kernel<8><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);
-  else knn_kernel<16><<<blocks, 256, 0, st>>>(x, idx, (int)L, k);
-  return cudaGetLastError();
+  {   // k <= 512: 1024-entry buffers (88 KB per CTA)
+    const size_t smem = (size_t)(3 * kTile + 8 * 2 * 1024 + 96) * sizeof(float);
+    cudaError_t e = cudaFuncSetAttribute(knn_select_kernel<1024, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    knn_select_kernel<1024, 16><<<blocks, 256, smem, st>>>(x, idx, (int)L, k);
+    return cudaGetLastError();
+  }
 }
 
 }  // namespace dcp
