@@ -503,6 +503,7 @@ __device__ __forceinline__ unsigned buf_bisect(const unsigned (&bv)[kPer], unsig
 #pragma unroll
     for (int j = 0; j < kPer; ++j) c += __popc(__ballot_sync(0xffffffffu, bv[j] <= mid));
     if (c >= need) hi = mid; else lo = mid + 1;
+    if (c == need) break;                                      // exactly `need` entries are <= mid: the set is settled
   }
   return hi;
 }
@@ -603,6 +604,9 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
   int* ai = reinterpret_cast<int*>(ak + kCap);
   unsigned* bk = ak + 2 * kCap;
   int* bi = reinterpret_cast<int*>(bk + kCap);
+  // per tile: its 16 chunks of 128 atoms -- bounding box [lo xyz, hi xyz], chain-id range, residue-id range
+  float* box = reinterpret_cast<float*>(scr + kTile) + 8 * (4 * kCap);
+  int* meta = reinterpret_cast<int*>(box + 16 * 6);
   const int lq = blockIdx.x * 8 + wib;
   const bool active = lq < L;
   const int l = active ? lq : L - 1;
@@ -612,6 +616,7 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
   unsigned thr_a = 0xffffffffu, thr_b = 0xffffffffu;           // the classes' bounds (keys <= bound are kept)
   int na = 0, nb = 0;                                          // buffer fill
   int cs = 0;                                                  // this lane's share of the own chain's size
+  int cs_w = 0;                                                // ... and the part counted per chunk (warp-uniform)
   const bool has_win = win >= 0;                               // n_seq = 0: no atom is sequence-local
   const unsigned win2 = has_win ? 2u * (unsigned)win : 0u;
   bool over = false;
@@ -645,11 +650,85 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
       scr[e] = m < L ? make_int2(__ldg(cid + m), __ldg(rid + m)) : make_int2(-1, 0);
     }
     __syncthreads();
-    if (!active) continue;
     const int n_here = (L - t0 < kTile ? L - t0 : kTile);
-    // four chunks per step: independent loads and arithmetic; only the last tile can be ragged, the others check no bounds
+    {
+      // chunk metadata: warp w takes chunks 2 w and 2 w + 1; an empty chunk gets an empty box and empty id ranges
+#pragma unroll
+      for (int cc = 0; cc < 2; ++cc) {
+        const int ch = 2 * wib + cc;
+        float lo0 = kInf, lo1 = kInf, lo2 = kInf, hi0 = -kInf, hi1 = -kInf, hi2 = -kInf;
+        int cmin = 0x7fffffff, cmax = (int)0x80000000, rmin = 0x7fffffff, rmax = (int)0x80000000;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int e = ch * 128 + 32 * i + lane;
+          if (e < n_here) {
+            lo0 = fminf(lo0, sx[e]); hi0 = fmaxf(hi0, sx[e]);
+            lo1 = fminf(lo1, sy[e]); hi1 = fmaxf(hi1, sy[e]);
+            lo2 = fminf(lo2, sz[e]); hi2 = fmaxf(hi2, sz[e]);
+            const int2 cr = scr[e];
+            cmin = min(cmin, cr.x); cmax = max(cmax, cr.x);
+            rmin = min(rmin, cr.y); rmax = max(rmax, cr.y);
+          }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          lo0 = fminf(lo0, __shfl_xor_sync(0xffffffffu, lo0, o)); hi0 = fmaxf(hi0, __shfl_xor_sync(0xffffffffu, hi0, o));
+          lo1 = fminf(lo1, __shfl_xor_sync(0xffffffffu, lo1, o)); hi1 = fmaxf(hi1, __shfl_xor_sync(0xffffffffu, hi1, o));
+          lo2 = fminf(lo2, __shfl_xor_sync(0xffffffffu, lo2, o)); hi2 = fmaxf(hi2, __shfl_xor_sync(0xffffffffu, hi2, o));
+        }
+        cmin = __reduce_min_sync(0xffffffffu, cmin); cmax = __reduce_max_sync(0xffffffffu, cmax);
+        rmin = __reduce_min_sync(0xffffffffu, rmin); rmax = __reduce_max_sync(0xffffffffu, rmax);
+        if (lane == 0) {
+          box[ch * 6] = lo0; box[ch * 6 + 1] = lo1; box[ch * 6 + 2] = lo2;
+          box[ch * 6 + 3] = hi0; box[ch * 6 + 4] = hi1; box[ch * 6 + 5] = hi2;
+          meta[ch * 4] = cmin; meta[ch * 4 + 1] = cmax; meta[ch * 4 + 2] = rmin; meta[ch * 4 + 3] = rmax;
+        }
+      }
+      __syncthreads();
+    }
+    if (!active) continue;
+    // Which chunks to scan (lane c < 16 decides for chunk c).  A chunk can be skipped when none of its atoms can enter a
+    // buffer: no atom can be sequence-local (those pass whatever their distance) and the pinned distance arithmetic applied
+    // to the query-to-box gaps -- a lower bound of every atom's computed d2, rounding being monotone -- exceeds both
+    // classes' distance bounds.  The own chain's size is then counted per chunk: all of it, none of it, or (a chunk that
+    // straddles chains) by a pass over the chain ids alone.
+    unsigned todo, count_only;
+    {
+      bool scan_it = false, count_it = false;
+      int whole = 0;
+      if (lane < 16 && lane * 128 < n_here) {
+        const float* bx = box + lane * 6;
+        const float g0 = fmaxf(fmaxf(__fsub_rn(bx[0], q0), __fsub_rn(q0, bx[3])), 0.f);
+        const float g1 = fmaxf(fmaxf(__fsub_rn(bx[1], q1), __fsub_rn(q1, bx[4])), 0.f);
+        const float g2 = fmaxf(fmaxf(__fsub_rn(bx[2], q2), __fsub_rn(q2, bx[5])), 0.f);
+        const unsigned lb = __float_as_uint(__fadd_rn(__fadd_rn(__fmul_rn(g0, g0), __fmul_rn(g1, g1)), __fmul_rn(g2, g2)));
+        const int cmin = meta[lane * 4], cmax = meta[lane * 4 + 1], rmin = meta[lane * 4 + 2], rmax = meta[lane * 4 + 3];
+        const bool may_same = cmin <= qc && qc <= cmax, all_same = cmin == qc && cmax == qc;
+        const bool may_local = may_same && has_win && (int64_t)rmin <= (int64_t)qr + win && (int64_t)rmax >= (int64_t)qr - win;
+        const unsigned lim_a = thr_a & 0x7fffffffu, lim_b = split ? thr_b : 0u;
+        scan_it = may_local || lb <= (lim_a > lim_b ? lim_a : lim_b);
+        count_it = !scan_it && may_same && !all_same;
+        const int n_ch = n_here - lane * 128 < 128 ? n_here - lane * 128 : 128;
+        whole = (!scan_it && all_same) ? n_ch : 0;
+      }
+      todo = __ballot_sync(0xffffffffu, scan_it);
+      count_only = __ballot_sync(0xffffffffu, count_it);
+      cs_w += __reduce_add_sync(0xffffffffu, whole);
+    }
+    while (count_only) {
+      const int c0 = (__ffs(count_only) - 1) * 128;
+      count_only &= count_only - 1;
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int e = c0 + 32 * u + lane;
+        cs += (e < n_here && scr[e].x == qc) ? 1 : 0;
+      }
+    }
+    // four 32-candidate pieces per step: independent loads and arithmetic; only the last tile can be ragged
     auto scan = [&](auto RAGGED) {
-      for (int c0 = 0; c0 < n_here; c0 += 128) {
+      while (todo) {
+        const int c0 = (__ffs(todo) - 1) * 128;
+        todo &= todo - 1;
         unsigned db[4], ka[4], ma[4], mb[4];
         bool pa[4], pb[4];
 #pragma unroll
@@ -685,6 +764,7 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
   int n_same = cs;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) n_same += __shfl_xor_sync(0xffffffffu, n_same, o);
+  n_same += cs_w;
   const int cnt_a = split ? n_same : L, cnt_b = split ? L - n_same : 0;
   if (over) budget_insert_global<NRF>(x, rid, cid, L, k, l, n_seq, split, lane, ak, ai, bk, bi, &na, &nb);
   // quotas (oracle/knn_budget.py): the foreign quota first, the own chain gets the rest, leftovers go back
@@ -717,7 +797,7 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
 template <int kCap, int NRF>
 cudaError_t launch_budget_select(const float* x, const int32_t* rid, const int32_t* cid, int32_t* idx, int L, int k, int n_seq,
                                  int split, int q_out, cudaStream_t st) {
-  const size_t smem = (size_t)(5 * kTile + 8 * 4 * kCap) * 4;
+  const size_t smem = (size_t)(5 * kTile + 8 * 4 * kCap + 16 * 10) * 4;
   cudaError_t e = cudaFuncSetAttribute(knn_budget_select_kernel<kCap, NRF>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
   knn_budget_select_kernel<kCap, NRF><<<(unsigned)((L + 7) / 8), 256, smem, st>>>(x, rid, cid, idx, L, k, n_seq, split, q_out);
