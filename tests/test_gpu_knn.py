@@ -139,6 +139,32 @@ def test_knn_budget_ties_and_short_chains():
         assert np.array_equal(got, kbo.knn_budget(x.numpy(), rid.numpy(), cid.numpy(), k, n_seq=n_seq))
 
 
+def test_knn_budget_interleaved_chains_and_clustered_space():
+    """Chain and residue ids that are NOT contiguous in index (every 128-atom chunk straddles chains: the chunk test can
+    neither skip on ids nor count whole chunks) over spatially clustered atoms (chunks far from a query are skipped on
+    distance), L not a multiple of 128 or of the tile."""
+    dcp = _dcp()
+    g = torch.Generator(device="cpu").manual_seed(31)
+    L = 4500
+    centres = torch.rand(36, 3, generator=g) * 200.0
+    x = centres[torch.arange(L) // 125] + torch.randn(L, 3, generator=g) * 3.0          # coherent in index, like an assembly
+    cid = torch.randint(0, 7, (L,), generator=g).to(torch.int32)                        # interleaved chains
+    rid = torch.randint(0, 40, (L,), generator=g).to(torch.int32)                       # arbitrary residue ids
+    for k, n_seq in ((128, 2), (64, 1), (200, 2)):
+        got = dcp.dcp_knn_budget(x.to(DEV), rid.to(DEV), cid.to(DEV), k, 7, n_seq=n_seq).cpu().numpy()
+        rows = list(range(0, L, 97)) + [L - 1, 2047, 2048, 4095, 4096]
+        assert np.array_equal(got[rows], kbo.knn_budget_rows(x.numpy(), rid.numpy(), cid.numpy(), k, rows, n_seq=n_seq))
+    # the same atoms with contiguous chains: whole chunks are counted without a scan
+    cid2 = (torch.arange(L) // 700).to(torch.int32)
+    rid2 = (torch.arange(L) // 9).to(torch.int32)
+    got = dcp.dcp_knn_budget(x.to(DEV), rid2.to(DEV), cid2.to(DEV), 128, 7, n_seq=2).cpu().numpy()
+    rows = list(range(0, L, 61)) + [L - 1]
+    assert np.array_equal(got[rows], kbo.knn_budget_rows(x.numpy(), rid2.numpy(), cid2.numpy(), 128, rows, n_seq=2))
+    # and the plain lists on the clustered cloud (chunk skipping in knn_select_kernel)
+    gk = dcp.dcp_knn(x.to(DEV), 128).cpu().numpy()
+    assert np.array_equal(gk[rows], ko.knn_rows(x.numpy(), 128, rows))
+
+
 def test_knn_budget_coincident_atoms_take_the_exact_fallback():
     """900 coincident atoms spread over four chains (+ a few others): more entries tie within a class bound than a
     candidate buffer holds, so the queries take the register-list fallback; order = (flag, distance, index)."""
