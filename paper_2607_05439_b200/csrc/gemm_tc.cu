@@ -143,7 +143,9 @@ __global__ void __launch_bounds__(kTcThreads, 2) gemm_tc_kernel(const __grid_con
     const int quad = warp & 3, half = (warp - 2) >> 2, et = threadIdx.x - 64;   // et: 0..255 among the epilogue threads
     const int row = quad * 32 + lane;                       // tile row of this thread = its TMEM lane
     const int mode = p.mode[seg];
-    __nv_bfloat16* Cs = reinterpret_cast<__nv_bfloat16*>(smem);   // [128][kCsPitch], aliases the drained pipeline stages
+    // C tile [128][kCsPitch] bf16, aliases the drained pipeline stages; (head, head dim) table of the tile's columns.
+    // Both are read and written with explicit shared-memory instructions (generic loads of shared memory are slower).
+    const uint32_t s_cs = s_base, s_hd = smem_u32(smem + Cfg::kSmemHd);
     short2* hd = reinterpret_cast<short2*>(smem + Cfg::kSmemHd);
     if (et < TBN && p.c > 0) hd[et] = make_short2((short)((n0 + et) / p.c), (short)((n0 + et) % p.c));   // one division per column
     mbar_wait(bar_acc, 0);
@@ -178,11 +180,12 @@ __global__ void __launch_bounds__(kTcThreads, 2) gemm_tc_kernel(const __grid_con
           }
         }
       }
-      uint4* dst = reinterpret_cast<uint4*>(Cs + row * kCsPitch + ch * 32);
+      const uint32_t dst = s_cs + (row * kCsPitch + ch * 32) * 2;
 #pragma unroll
       for (int i = 0; i < 4; ++i)
-        dst[i] = make_uint4(pack_bf16(v[8 * i] * scale, v[8 * i + 1] * scale), pack_bf16(v[8 * i + 2] * scale, v[8 * i + 3] * scale),
-                            pack_bf16(v[8 * i + 4] * scale, v[8 * i + 5] * scale), pack_bf16(v[8 * i + 6] * scale, v[8 * i + 7] * scale));
+        sts_u32x4(dst + 16 * i,
+                  make_uint4(pack_bf16(v[8 * i] * scale, v[8 * i + 1] * scale), pack_bf16(v[8 * i + 2] * scale, v[8 * i + 3] * scale),
+                             pack_bf16(v[8 * i + 4] * scale, v[8 * i + 5] * scale), pack_bf16(v[8 * i + 6] * scale, v[8 * i + 7] * scale)));
     }
     tc_fence_before();
     asm volatile("bar.sync 1, 256;" ::: "memory");
@@ -193,14 +196,15 @@ __global__ void __launch_bounds__(kTcThreads, 2) gemm_tc_kernel(const __grid_con
       for (int u = et; u < TBM * (TBN / 8); u += 256) {
         const int r = u / (TBN / 8), c8 = u % (TBN / 8);
         if (m0 + r < p.M)
-          *reinterpret_cast<uint4*>(C + (int64_t)(m0 + r) * ldc + n0 + c8 * 8) = *reinterpret_cast<const uint4*>(Cs + r * kCsPitch + c8 * 8);
+          *reinterpret_cast<uint4*>(C + (int64_t)(m0 + r) * ldc + n0 + c8 * 8) = lds_u32x4(s_cs + (r * kCsPitch + c8 * 8) * 2);
       }
     } else if (mode == GEMM_OUT_HEADPAD) {
       for (int u = et; u < TBM * (TBN / 2); u += 256) {
         const int r = u / (TBN / 2), col = (u % (TBN / 2)) * 2;
         if (m0 + r < p.M) {
-          const int h = hd[col].x, d = hd[col].y;  // c even, col even: the pair stays inside one head
-          *reinterpret_cast<uint32_t*>(C + ((int64_t)(m0 + r) * p.H + h) * p.cp + d) = *reinterpret_cast<const uint32_t*>(Cs + r * kCsPitch + col);
+          const uint32_t hw = lds_u32(s_hd + col * 4);
+          const int h = (short)(hw & 0xffffu), d = (short)(hw >> 16);  // c even, col even: the pair stays inside one head
+          *reinterpret_cast<uint32_t*>(C + ((int64_t)(m0 + r) * p.H + h) * p.cp + d) = lds_u32(s_cs + (r * kCsPitch + col) * 2);
         }
       }
     } else {
@@ -215,14 +219,15 @@ __global__ void __launch_bounds__(kTcThreads, 2) gemm_tc_kernel(const __grid_con
         int col;
         if (is_k) {
           col = grp * 16 + 4 * tt;
-          v = *reinterpret_cast<const uint2*>(Cs + (kt * 16 + 4 * (gg >> 1) + (gg & 1) + 2 * b) * kCsPitch + col);
+          v = lds_u32x2(s_cs + ((kt * 16 + 4 * (gg >> 1) + (gg & 1) + 2 * b) * kCsPitch + col) * 2);
         } else {
           col = grp * 16 + 8 * b + gg;
-          const unsigned short* src = reinterpret_cast<const unsigned short*>(Cs + (kt * 16 + 4 * tt) * kCsPitch + col);
-          const uint32_t e0 = src[0], e1 = src[kCsPitch], e2 = src[2 * kCsPitch], e3 = src[3 * kCsPitch];
+          const uint32_t src = s_cs + ((kt * 16 + 4 * tt) * kCsPitch + col) * 2;
+          const uint32_t e0 = lds_u16(src), e1 = lds_u16(src + 2 * kCsPitch), e2 = lds_u16(src + 4 * kCsPitch), e3 = lds_u16(src + 6 * kCsPitch);
           v = make_uint2(e0 | (e1 << 16), e2 | (e3 << 16));
         }
-        const int h = hd[col].x, d = hd[col].y;
+        const uint32_t hw = lds_u32(s_hd + col * 4);
+        const int h = (short)(hw & 0xffffu), d = (short)(hw >> 16);
         int64_t idx;
         if (is_k) idx = (((tile * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + gg * 4 + ((d & 15) >> 2)) * 8 + b * 4;
         else idx = (((tile * p.H + h) * (p.cp >> 4) + (d >> 4)) * 32 + (d & 7) * 4 + tt) * 8 + ((d >> 3) & 1) * 4;

@@ -116,6 +116,19 @@ __device__ __forceinline__ uint2 lds_u32x2(uint32_t addr) {
   asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
   return v;
 }
+__device__ __forceinline__ uint32_t lds_u32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t addr) {
+  uint16_t v;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ void sts_u32x4(uint32_t addr, uint4 v) {
+  asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
 // acc_lo += lo(w)^2, acc_hi += hi(w)^2 for a bf16x2 word: mixed-precision FMA (bf16 x bf16 + f32, PTX ISA 8.6, sm_100:
 // SASS FHFMA.BF16 with .H0/.H1 operand selectors), exact products, fp32 accumulation, no unpacking instructions
 __device__ __forceinline__ void fma_sq_bf16x2(float& acc_lo, float& acc_hi, uint32_t w) {
