@@ -102,10 +102,20 @@ __global__ void __launch_bounds__(256) merge_vec4_kernel(const MergeParams p) {
   if (p.g != nullptr) {
     const T* gp = reinterpret_cast<const T*>(p.g) + row * p.D + e;
     T* out = reinterpret_cast<T*>(p.gated) + row * p.D + e;
-    out[0] = from_f32<T>(to_f32(gp[0]) * (a.x / l));
-    out[1] = from_f32<T>(to_f32(gp[1]) * (a.y / l));
-    out[2] = from_f32<T>(to_f32(gp[2]) * (a.z / l));
-    out[3] = from_f32<T>(to_f32(gp[3]) * (a.w / l));
+    if constexpr (sizeof(T) == 2) {
+      // bf16: the four gates and the four results as one 8-byte access each (e % 4 == 0, rows are 8-byte aligned)
+      const uint2 gw = *reinterpret_cast<const uint2*>(gp);
+      const float g0 = __uint_as_float(gw.x << 16), g1 = __uint_as_float(gw.x & 0xffff0000u);
+      const float g2 = __uint_as_float(gw.y << 16), g3 = __uint_as_float(gw.y & 0xffff0000u);
+      const __nv_bfloat162 o01 = __floats2bfloat162_rn(g0 * (a.x / l), g1 * (a.y / l));
+      const __nv_bfloat162 o23 = __floats2bfloat162_rn(g2 * (a.z / l), g3 * (a.w / l));
+      *reinterpret_cast<uint2*>(out) = make_uint2(*reinterpret_cast<const uint32_t*>(&o01), *reinterpret_cast<const uint32_t*>(&o23));
+    } else {
+      out[0] = from_f32<T>(to_f32(gp[0]) * (a.x / l));
+      out[1] = from_f32<T>(to_f32(gp[1]) * (a.y / l));
+      out[2] = from_f32<T>(to_f32(gp[2]) * (a.z / l));
+      out[3] = from_f32<T>(to_f32(gp[3]) * (a.w / l));
+    }
   } else {
     *reinterpret_cast<float4*>(p.acc_out + row * p.D + e) = a;
     if (e % p.c == 0) { p.m_out[row * p.H + h] = m; p.l_out[row * p.H + h] = l; }
@@ -136,7 +146,8 @@ cudaError_t launch_vec4(const MergeParams& p, unsigned blocks, cudaStream_t st) 
 cudaError_t launch_merge(dcp_dtype dt, const MergeParams& p, cudaStream_t st) {
   const int64_t total = p.rows * p.D;
   if (total <= 0) return cudaSuccess;
-  if (p.c % 4 == 0 && ((uintptr_t)p.st_acc & 15) == 0 && (p.g != nullptr || ((uintptr_t)p.acc_out & 15) == 0)) {
+  if (p.c % 4 == 0 && ((uintptr_t)p.st_acc & 15) == 0 &&
+      (p.g != nullptr ? (((uintptr_t)p.g | (uintptr_t)p.gated) & 7) == 0 : ((uintptr_t)p.acc_out & 15) == 0)) {
     const unsigned vblocks = (unsigned)((total / 4 + 255) / 256);
     return dt == DCP_F32 ? launch_vec4<float>(p, vblocks, st) : launch_vec4<__nv_bfloat16>(p, vblocks, st);
   }
