@@ -621,13 +621,23 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
   const unsigned win2 = has_win ? 2u * (unsigned)win : 0u;
   bool over = false;
   // append the lanes' candidates (key v, atom m) of `mask` to a class buffer; re-bound the buffer when it would overflow
-  auto append = [&](unsigned* key, int* id, int& n, unsigned& thr, unsigned mask, bool pass, unsigned v, int m) {
+  // A class never contributes more than k entries; the foreign class B no more than max(q_out, k - |own chain|) (the
+  // quota arithmetic at the end), and the part of the own chain counted so far bounds that from above: once the own tile
+  // has shown k - q_out own atoms, B's bound is its q_out-th (32nd) key instead of its k-th -- a much shorter radius, so
+  // most foreign chunks are skipped afterwards.
+  auto append = [&](unsigned* key, int* id, int& n, unsigned& thr, unsigned mask, bool pass, unsigned v, int m, bool class_b) {
     if (over) return;
     if (n + __popc(mask) > kCap) {
       __syncwarp();
+      int need = k;
+      if (class_b) {
+        const int own_lb = __reduce_add_sync(0xffffffffu, cs) + cs_w;        // own-chain atoms seen so far
+        need = k - own_lb > q_out ? k - own_lb : q_out;
+        need = need < k ? need : k;
+      }
       unsigned bv[kPer];
       buf_load(bv, key, n, lane);
-      thr = buf_bisect(bv, thr, k);                            // the buffer holds more than kCap - 32 >= k entries
+      thr = buf_bisect(bv, thr, need);                         // the buffer holds more than kCap - 32 >= k >= need entries
       n = buf_compact(bv, key, id, thr, n, lane);
       pass = pass && v <= thr;
       mask = __ballot_sync(0xffffffffu, pass);
@@ -706,7 +716,8 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
         const bool may_same = cmin <= qc && qc <= cmax, all_same = cmin == qc && cmax == qc;
         const bool may_local = may_same && has_win && (int64_t)rmin <= (int64_t)qr + win && (int64_t)rmax >= (int64_t)qr - win;
         const unsigned lim_a = thr_a & 0x7fffffffu, lim_b = split ? thr_b : 0u;
-        scan_it = may_local || lb <= (lim_a > lim_b ? lim_a : lim_b);
+        // class A lives only in chunks that hold own-chain atoms (every chunk without a split), class B in the others
+        scan_it = may_local || ((may_same || !split) && lb <= lim_a) || (split && !all_same && lb <= lim_b);
         count_it = !scan_it && may_same && !all_same;
         const int n_ch = n_here - lane * 128 < 128 ? n_here - lane * 128 : 128;
         whole = (!scan_it && all_same) ? n_ch : 0;
@@ -751,8 +762,8 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           const int m = t0 + c0 + 32 * u + lane;
-          if (ma[u]) append(ak, ai, na, thr_a, ma[u], pa[u], ka[u], m);
-          if (mb[u]) append(bk, bi, nb, thr_b, mb[u], pb[u], db[u], m);
+          if (ma[u]) append(ak, ai, na, thr_a, ma[u], pa[u], ka[u], m, false);
+          if (mb[u]) append(bk, bi, nb, thr_b, mb[u], pb[u], db[u], m, true);
         }
       }
     };
