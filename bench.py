@@ -74,7 +74,7 @@ def parse():
     ap.add_argument("--kernel", default="auto", choices=["auto", "generic", "mma"])
     ap.add_argument("--blocks", type=int, default=2, help="P2: Pairformer blocks in the stack (PAPER.md:293: two); D2 | D3: attention blocks (default there: 18, PAPER.md:294)")
     ap.add_argument("--cached", action="store_true",
-                    help="D2 | D3: dcp_attention_stack_cached (bias cache: one pass over z per 15 blocks, DESIGN.md 6.8)")
+                    help="D2 | D3: dcp_attention_stack_cached (bias cache: one pass over z per 23 blocks, DESIGN.md 6.8)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-rows", type=int, default=0, help="oracle sample rows (0: sized for ~10-20 s)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -730,10 +730,10 @@ def run_attention_stack(args, rank, world, local_rank):
                 "note": "kernel_ms: fused kernel of single layer calls on the same shapes (event pair around it); "
                         "call_frac: blocks x z bytes over the whole stack call"}
     if args.cached:
-        # this mode's own algorithmic bytes: z once per pass of <= 15 blocks, every block's fp16 bias tiles
+        # this mode's own algorithmic bytes: z once per pass of <= 23 blocks, every block's fp16 bias tiles
         # (H * 2 = 32 bytes per pair over the 32 x 16 tile grid) written once and read once.  The whole call is the unit:
         # the per-launch times of its two kernels are in the committed ncu launch list.
-        passes = -(-nb // 15)
+        passes = -(-nb // 23)            # bias_tiles_kernel takes up to 23 blocks per pass over z
         tiles = (-(-cfg.I // 32)) * (-(-cfg.I // 16)) * 32 * 16
         cb = passes * zb + 2.0 * nb * tiles * cfg.H * 2
         roofline = {"bound": "hbm", "achieved": cb / (step_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",

@@ -185,7 +185,7 @@ dcp_status dcp_attention_stack(void *a, const void *z, int64_t ldz, const dcp_we
                                void *stream);
 
 /* The same stack with a BIAS CACHE: every block derives its bias LN_b(z) W_b^b from the same read-only
- * pair tensor, so one pass over z per 15 blocks computes the LayerNorm statistics once per pair and writes every block's
+ * pair tensor, so one pass over z per 23 blocks computes the LayerNorm statistics once per pair and writes every block's
  * bias as fp16 tiles (H * 2 = 32 bytes per pair and block; PAPER.md:81 materialises B in R^{I x I x H} per block too);
  * each block then streams its 32 bytes per pair instead of the 256 bytes of z.  Same result as dcp_attention_stack up
  * to the fp16 rounding of the bias (2^-11 relative, below the bf16 rounding of P that follows).

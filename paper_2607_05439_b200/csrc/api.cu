@@ -631,7 +631,7 @@ dcp_status dcp_attention_stack(void* a, const void* z, int64_t ldz, const dcp_we
   return DCP_OK;
 }
 
-// ---- the same stack with a bias cache: one pass over z per 15 blocks writes every block's bias tiles, then each block
+// ---- the same stack with a bias cache: one pass over z per 23 blocks writes every block's bias tiles, then each block
 // streams 32 bytes per pair instead of 256
 dcp_status dcp_attention_stack_cache_bytes(int64_t I, int n_blocks, size_t* bytes) {
   if (!bytes || I <= 0 || n_blocks <= 0) return DCP_ERR_INVALID_ARG;

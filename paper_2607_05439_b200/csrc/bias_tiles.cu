@@ -1,6 +1,6 @@
 // Bias cache for the attention stack on a read-only pair tensor ("cached" mode).
 // Every block b of the stack derives its own bias  LN_b(z_ij) W_b^b  from the SAME pair tensor; one pass over z computes
-// the biases of up to 15 blocks at once -- LayerNorm statistics once per pair, one tcgen05 projection with
+// the biases of up to 23 blocks at once -- LayerNorm statistics once per pair, one tcgen05 projection with
 // N = 16 heads x n_blocks + the ones column -- and writes them as fp16 tiles in exactly the layout the attention kernel
 // consumes ([query tile of 32][key tile of 16][head pair][32 queries][16 keys] half2, 16 KB per tile), so that each block
 // afterwards streams 32 bytes per pair instead of the 256 bytes of z (the paper's own stack materialises
@@ -19,14 +19,30 @@ namespace {
 constexpr int bCz = 128, bH = 16, bTileQ = 32, bTileK = 16, bSubQ = 8, bNZ = 3, bNT = 2;
 constexpr int bStageBytes = bSubQ * bTileK * bCz * 2;      // 32 KB
 constexpr int bHalfBytes = bStageBytes / 2;
-constexpr int bMaxBlocks = 15;                              // 16 * 15 + 16 = 256 projection columns
-constexpr int bMaxN = 256;
+constexpr int bOneBuf = 15;                                 // 16 * 15 + 16 = 256 projection columns: one MMA, two accumulator buffers
+constexpr int bMaxBlocks = 23;                              // 16 * 23 + 16 = 384 columns in the X / Y split (below)
+constexpr int bMaxN = 384;                                  // rows of W''
 constexpr int bThreads = 256;
 constexpr size_t bSmemZ = 0;
-constexpr size_t bSmemWt = bSmemZ + (size_t)bNZ * bStageBytes;            // 2 halves x 256 rows x 128 B = 64 KB
-constexpr size_t bSmemC = bSmemWt + 2 * (size_t)bMaxN * 128;              // c1, c0: [15][16] floats each
+constexpr size_t bSmemWt = bSmemZ + (size_t)bNZ * bStageBytes;            // 2 halves x 384 rows x 128 B = 96 KB
+constexpr size_t bSmemC = bSmemWt + 2 * (size_t)bMaxN * 128;              // c1, c0: [23][16] floats each
 constexpr size_t bSmemBar = bSmemC + 2 * bMaxBlocks * bH * 4;
-constexpr size_t bSmemAlloc = bSmemBar + (2 * bNZ + 2 * bNT) * 8 + 16 + 1024;
+constexpr int bNumBars = 2 * bNZ + 2 * bNT + 2;             // z full / empty, X full / empty (two buffers), Y full / empty
+constexpr size_t bSmemAlloc = bSmemBar + bNumBars * 8 + 16 + 1024;
+
+// Column plan of a pass of nb blocks.  Up to 15 blocks everything is one region X = [blocks | ones] of 16 nb + 16 <= 256
+// columns, double buffered in tensor memory (NY = 0).  16 .. 23 blocks need 272 .. 384 columns, which do not fit twice into
+// the 512 columns: the columns are split into Y = [ones | the first blocks] (NY columns, ONE buffer) and X = [the other
+// blocks] (NX columns, two buffers), 2 NX + NY <= 512.  Y's MMA is issued first and its columns are read first, so the
+// next stage's Y MMA waits only for that part of the epilogue; X stays double buffered.
+struct ColPlan { int NX, NY, y_blocks; };
+__host__ __device__ inline ColPlan col_plan(int nb) {
+  if (nb <= bOneBuf) return ColPlan{16 * nb + 16, 0, 0};
+  const int T = 16 * nb + 16;
+  const int NX = (512 - T) / 64 * 64;                        // the widest double-buffered part that leaves room for Y; buffers
+                                                             // start at multiples of 64 columns
+  return ColPlan{NX, T - NX, (T - NX) / 16 - 1};
+}
 
 struct BiasTilesParams {
   const void* wfold;       // [n_blocks][16][128] bf16
@@ -46,24 +62,34 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
   const uint32_t s_c = smem_u32(smem + bSmemC);
   float* s_c0 = s_c1 + bMaxBlocks * bH;
   const uint32_t bar_zfull = s_bar, bar_zempty = s_bar + 8 * bNZ, bar_tfull = s_bar + 16 * bNZ, bar_tempty = bar_tfull + 8 * bNT;
-  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + bSmemBar + (2 * bNZ + 2 * bNT) * 8);
+  const uint32_t bar_yfull = bar_tempty + 8 * bNT, bar_yempty = bar_yfull + 8;
+  volatile uint32_t* s_tmem = reinterpret_cast<volatile uint32_t*>(smem + bSmemBar + bNumBars * 8);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int NP = 16 * p.n_blocks + 16;                       // projection columns: heads of every block, ones, zero rows
+  const ColPlan cp = col_plan(p.n_blocks);
+  const int NX = cp.NX, NY = cp.NY, yb = cp.y_blocks;        // Y holds the ones column and blocks [0, yb); X blocks [yb, nb)
 
   pdl_trigger();
   if (threadIdx.x == 0) {
-    for (int s = 0; s < bNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, 1 + 4); }
+    // z_empty: the commits of the stage's MMAs (one thread's, or the Y and the X thread's) + the four epilogue warps
+    for (int s = 0; s < bNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, (NY > 0 ? 2 : 1) + 4); }
     for (int b = 0; b < bNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
+    mbar_init(bar_yfull, 1);
+    mbar_init(bar_yempty, 4);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), 512);
   pdl_wait();
-  // W'': row n < 16 nb = head n % 16 of block n / 16, row 16 nb = ones, others 0; K-major, 128-byte swizzle by hand
+  // W'' rows in column order, K-major, 128-byte swizzle by hand.  One region: row n < 16 nb = head n % 16 of block n / 16,
+  // row 16 nb = ones, others 0.  Split: rows [0, NY) = Y = [ones, 15 zero rows | blocks 0 .. yb), rows [NY, NY + NX) = X.
   for (int e = threadIdx.x; e < NP * (bCz / 8); e += bThreads) {
     const int n = e / (bCz / 8), ch16 = e % (bCz / 8);
+    int src = -2;                                            // -2: zero row, -1: ones, >= 0: row of wfold
+    if (NY == 0) src = n < 16 * p.n_blocks ? n : (n == 16 * p.n_blocks ? -1 : -2);
+    else src = n == 0 ? -1 : (n < 16 ? -2 : n - 16);
     uint4 v = make_uint4(0u, 0u, 0u, 0u);
-    if (n < 16 * p.n_blocks) v = __ldg(reinterpret_cast<const uint4*>(p.wfold) + n * (bCz / 8) + ch16);
-    else if (n == 16 * p.n_blocks) v = make_uint4(0x3f803f80u, 0x3f803f80u, 0x3f803f80u, 0x3f803f80u);
+    if (src >= 0) v = __ldg(reinterpret_cast<const uint4*>(p.wfold) + src * (bCz / 8) + ch16);
+    else if (src == -1) v = make_uint4(0x3f803f80u, 0x3f803f80u, 0x3f803f80u, 0x3f803f80u);
     const int half = ch16 >> 3, c = ch16 & 7;
     *reinterpret_cast<uint4*>(smem + bSmemWt + half * (bMaxN * 128) + n * 128 + ((c ^ (n & 7)) << 4)) = v;
   }
@@ -96,23 +122,52 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
     if (warp <= 2 && lane == 0) {
       // =============================================================== tcgen05 issuers (stage n -> issuer n % 2: with two
       // accumulator buffers a buffer's consecutive users are then the same thread, so its parity waits cannot alias)
-      const uint32_t idesc = umma_idesc_bf16(128, NP);
+      const uint32_t idesc_x = umma_idesc_bf16(128, NX), idesc_y = umma_idesc_bf16(128, NY > 0 ? NY : 16);
+      const uint32_t x_stride = NY == 0 ? 256u : (uint32_t)NX;          // tensor-memory columns between the two X buffers
       const uint32_t me = warp - 1;
       uint32_t it = 0;
       for (int tile = blockIdx.x; tile < p.n_tiles; tile += gridDim.x) {
         for (int sub = 0; sub < bTileQ / bSubQ; ++sub, ++it) {
-          if (it % 2 != me) continue;
           const int stage = it % bNZ, tb = it % bNT;
-          mbar_wait(bar_tempty + 8 * tb, ((it / bNT) & 1) ^ 1);
-          mbar_wait(bar_zfull + 8 * stage, (it / bNZ) & 1);
-          tc_fence_after();
           const uint32_t zs = s_z + stage * bStageBytes;
+          if (NY == 0) {
+            // one region: stage n -> issuer n % 2 (with two accumulator buffers a buffer's consecutive users are then the
+            // same thread, so its parity waits cannot alias)
+            if (it % 2 != me) continue;
+            mbar_wait(bar_tempty + 8 * tb, ((it / bNT) & 1) ^ 1);
+            mbar_wait(bar_zfull + 8 * stage, (it / bNZ) & 1);
+            tc_fence_after();
 #pragma unroll
-          for (int ks = 0; ks < 8; ++ks)
-            umma_bf16(tmem_base + tb * bMaxN, umma_desc_sw128(zs + (ks >> 2) * bHalfBytes + (ks & 3) * 32),
-                      umma_desc_sw128(s_wt + (ks >> 2) * (bMaxN * 128) + (ks & 3) * 32), idesc, ks > 0);
-          umma_commit(bar_zempty + 8 * stage);
-          umma_commit(bar_tfull + 8 * tb);
+            for (int ks = 0; ks < 8; ++ks)
+              umma_bf16(tmem_base + tb * x_stride, umma_desc_sw128(zs + (ks >> 2) * bHalfBytes + (ks & 3) * 32),
+                        umma_desc_sw128(s_wt + (ks >> 2) * (bMaxN * 128) + (ks & 3) * 32), idesc_x, ks > 0);
+            umma_commit(bar_zempty + 8 * stage);
+            umma_commit(bar_tfull + 8 * tb);
+          } else if (me == 0) {
+            // split columns: this thread issues every stage's Y MMA.  Y has ONE buffer, so its users must be one thread: a
+            // thread that alternated stages with another could be two phases ahead of y_empty and its parity wait would
+            // pass early.  The buffer is free once the epilogue of the previous stage has read it (completion it - 1).
+            mbar_wait(bar_zfull + 8 * stage, (it / bNZ) & 1);
+            mbar_wait(bar_yempty, (it & 1) ^ 1);
+            tc_fence_after();
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks)
+              umma_bf16(tmem_base + 2 * NX, umma_desc_sw128(zs + (ks >> 2) * bHalfBytes + (ks & 3) * 32),
+                        umma_desc_sw128(s_wt + (ks >> 2) * (bMaxN * 128) + (ks & 3) * 32), idesc_y, ks > 0);
+            umma_commit(bar_zempty + 8 * stage);
+            umma_commit(bar_yfull);
+          } else {
+            // ... and this one every stage's X MMA (two buffers)
+            mbar_wait(bar_zfull + 8 * stage, (it / bNZ) & 1);
+            mbar_wait(bar_tempty + 8 * tb, ((it / bNT) & 1) ^ 1);
+            tc_fence_after();
+#pragma unroll
+            for (int ks = 0; ks < 8; ++ks)
+              umma_bf16(tmem_base + tb * x_stride, umma_desc_sw128(zs + (ks >> 2) * bHalfBytes + (ks & 3) * 32),
+                        umma_desc_sw128(s_wt + (ks >> 2) * (bMaxN * 128) + NY * 128 + (ks & 3) * 32), idesc_x, ks > 0);
+            umma_commit(bar_zempty + 8 * stage);
+            umma_commit(bar_tfull + 8 * tb);
+          }
         }
       }
     }
@@ -144,12 +199,11 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
         asm volatile("" : "+f"(zsq));
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_zempty + 8 * stage);
-        mbar_wait(bar_tfull + 8 * tb, (it / bNT) & 1);
+        // the ones column (sum_k z) comes first: from Y when the columns are split, else from the X buffer
+        const uint32_t t_x = t_lane + tb * (NY == 0 ? 256u : (uint32_t)NX), t_y = t_lane + 2 * NX;
+        if (NY > 0) mbar_wait(bar_yfull, it & 1); else mbar_wait(bar_tfull + 8 * tb, (it / bNT) & 1);
         tc_fence_after();
-        const uint32_t t_p = t_lane + tb * bMaxN;
-        float accA[16], accB[16];
-        const float zsum = tmem_ld_x1(t_p + 16 * p.n_blocks);
-        tmem_ld_x16(t_p, accA);
+        const float zsum = tmem_ld_x1(NY > 0 ? t_y : t_x + 16 * p.n_blocks);
         tmem_ld_wait();
         const float mu = zsum * (1.f / bCz);
         const float var = fmaf(-mu, mu, zsq * (1.f / bCz));      // one rounding; exactly 0 for a constant row (fused_mma.cu)
@@ -157,7 +211,6 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
         const float nm = -mu * rstd;
         // tile layout [sub 4][head pair 8][8 queries][16 keys] words: a stage writes one contiguous 4 KB piece per block
         uint32_t* dst = p.cache + (int64_t)tile * (8 * 512) + sub * (8 * bSubQ * bTileK) + prow;
-        // block b's 16 columns are processed while block b + 1's are in flight (one tcgen05.ld ahead)
         auto emit = [&](float (&acc)[16], int b) {
 #pragma unroll
           for (int i = 0; i < 16; ++i) asm volatile("" : "+f"(acc[i]));        // not before the wait that completes the load
@@ -171,16 +224,31 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
             d[(2 * h4 + 1) * 128] = pack_f16(fmaf(acc[4 * h4 + 2], rstd, fmaf(nm, a1.z, a0.z)), fmaf(acc[4 * h4 + 3], rstd, fmaf(nm, a1.w, a0.w)));
           }
         };
-        for (int b = 0; b < p.n_blocks; b += 2) {
-          tmem_ld_wait();
-          if (b + 1 < p.n_blocks) tmem_ld_x16(t_p + 16 * (b + 1), accB);
-          emit(accA, b);
-          if (b + 1 < p.n_blocks) {
+        // blocks [b0, b0 + n) live in 16-column groups from t_col on; block b's columns are processed while block b + 1's are
+        // in flight (one tcgen05.ld ahead)
+        auto region = [&](uint32_t t_col, int b0, int n) {
+          float accA[16], accB[16];
+          if (n > 0) tmem_ld_x16(t_col, accA);
+          for (int j = 0; j < n; j += 2) {
             tmem_ld_wait();
-            if (b + 2 < p.n_blocks) tmem_ld_x16(t_p + 16 * (b + 2), accA);
-            emit(accB, b + 1);
+            if (j + 1 < n) tmem_ld_x16(t_col + 16 * (j + 1), accB);
+            emit(accA, b0 + j);
+            if (j + 1 < n) {
+              tmem_ld_wait();
+              if (j + 2 < n) tmem_ld_x16(t_col + 16 * (j + 2), accA);
+              emit(accB, b0 + j + 1);
+            }
           }
+        };
+        if (NY > 0) {
+          region(t_y + 16, 0, yb);                               // Y = [ones | blocks 0 .. yb): read first, freed first
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(bar_yempty);
+          mbar_wait(bar_tfull + 8 * tb, (it / bNT) & 1);
+          tc_fence_after();
         }
+        region(t_x, yb, p.n_blocks - yb);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(bar_tempty + 8 * tb);
@@ -216,7 +284,7 @@ int bias_tiles_max_blocks() { return bMaxBlocks; }
 int64_t bias_tiles_block_words(int64_t I) { return ((I + bTileQ - 1) / bTileQ) * ((I + bTileK - 1) / bTileK) * 8 * 512; }
 size_t bias_tiles_fold_bytes(int n_blocks) { return (size_t)n_blocks * (bH * bCz * 2 + 2 * bH * 4) + 512; }
 
-// Biases of blocks [0, n_blocks) (n_blocks <= 15) of one pass: fold (one small launch) + the streaming kernel.
+// Biases of blocks [0, n_blocks) (n_blocks <= 23) of one pass: fold (one small launch) + the streaming kernel.
 cudaError_t launch_bias_tiles(const void* z, int64_t ldz, int64_t I, const dcp_weights* blocks, int n_blocks, float eps,
                               void* fold_ws, void* cache, cudaStream_t st) {
   if (n_blocks < 1 || n_blocks > bMaxBlocks) return cudaErrorInvalidValue;

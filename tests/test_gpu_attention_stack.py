@@ -152,7 +152,11 @@ def test_attention_stack_error_paths():
     (96, 12, 48, 1),
     (75, 15, 48, 3),       # ragged I: the last query / key tiles of the cache are partly out of range
     (131, 1, 24, 4),
-    (60, 60, 48, 18),      # two passes over z (15 + 3 blocks)
+    (60, 60, 48, 18),      # the paper's depth in ONE pass: 304 projection columns, split into a single-buffered Y part
+                           # (ones + 6 blocks) and a double-buffered X part (12 blocks) of tensor memory
+    (40, 1, 48, 16),       # the smallest split: Y = ones + 4 blocks, X = 12 blocks
+    (48, 12, 48, 23),      # the widest pass: Y = 256 columns (ones + 15 blocks), X = 128 (8 blocks)
+    (36, 12, 48, 25),      # two passes over z (23 + 2 blocks)
     (300, 60, 32, 16),
 ])
 def test_attention_stack_cached_matches_oracle_and_streaming(I, copies, c, n_blocks):
@@ -197,8 +201,8 @@ def test_attention_stack_cached_matches_oracle_and_streaming(I, copies, c, n_blo
 
 def test_attention_stack_cached_full_size_block_sampled():
     """The configuration bench.py --workload D2 --cached times (I = 3000, c_token = 768: 94 x 188 cache tiles per block,
-    282 work units with three key segments each, two bias passes when 18 blocks are given): 17 blocks on the device --
-    one pass of 15 and one of 2 --, block 17 checked on sampled rows against the oracle started from the device's own
+    282 work units with three key segments each): 17 blocks on the device, in one pass with split projection columns and,
+    as 16 + 1 blocks, in two calls; block 17 checked on sampled rows against the oracle started from the device's own
     latent after 16 blocks, and the call as a whole equal to 16 + 1 blocks in two calls."""
     dcp = _dcp()
     cfg = syn.small_config("D2", I=3000, c_s=768, c_z=128, H=16, c=48, dtype="bf16", seed=2, structured=True, copies=60)
