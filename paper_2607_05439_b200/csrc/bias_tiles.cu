@@ -6,8 +6,8 @@
 // afterwards streams 32 bytes per pair instead of the 256 bytes of z (the paper's own stack materialises
 // B in R^{I x I x H} per block).  Values are in the exp2 domain (W' carries log2 e), like the fused kernel's.
 //
-// One persistent CTA per SM, 8 warps: warp 0 TMA producer (z boxes as in fused_mma.cu), warps 1-2 tcgen05 issuers
-// (stage n -> issuer n % 2), warps 4-7 statistics + epilogue (thread = pair).
+// One persistent CTA per SM, 12 warps: warp 0 TMA producer (z boxes as in fused_mma.cu), warps 1-2 tcgen05 issuers,
+// warps 4-11 statistics + epilogue (thread = pair; warps w and w + 4 of a tensor-memory lane quadrant take every other block).
 #include "fold.cuh"
 #include "kernels.h"
 #include "mma_ptx.cuh"
@@ -22,7 +22,8 @@ constexpr int bHalfBytes = bStageBytes / 2;
 constexpr int bOneBuf = 15;                                 // 16 * 15 + 16 = 256 projection columns: one MMA, two accumulator buffers
 constexpr int bMaxBlocks = 23;                              // 16 * 23 + 16 = 384 columns in the X / Y split (below)
 constexpr int bMaxN = 384;                                  // rows of W''
-constexpr int bThreads = 256;
+constexpr int bThreads = 384;
+constexpr int bEpiWarps = 8;                                // warps w and w + 4 share a lane quadrant and alternate blocks
 constexpr size_t bSmemZ = 0;
 constexpr size_t bSmemWt = bSmemZ + (size_t)bNZ * bStageBytes;            // 2 halves x 384 rows x 128 B = 96 KB
 constexpr size_t bSmemC = bSmemWt + 2 * (size_t)bMaxN * 128;              // c1, c0: [23][16] floats each
@@ -72,10 +73,10 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
   pdl_trigger();
   if (threadIdx.x == 0) {
     // z_empty: the commits of the stage's MMAs (one thread's, or the Y and the X thread's) + the four epilogue warps
-    for (int s = 0; s < bNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, (NY > 0 ? 2 : 1) + 4); }
-    for (int b = 0; b < bNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, 4); }
+    for (int s = 0; s < bNZ; ++s) { mbar_init(bar_zfull + 8 * s, 1); mbar_init(bar_zempty + 8 * s, (NY > 0 ? 2 : 1) + bEpiWarps); }
+    for (int b = 0; b < bNT; ++b) { mbar_init(bar_tfull + 8 * b, 1); mbar_init(bar_tempty + 8 * b, bEpiWarps); }
     mbar_init(bar_yfull, 1);
-    mbar_init(bar_yempty, 4);
+    mbar_init(bar_yempty, bEpiWarps);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) tmem_alloc(smem_u32(const_cast<uint32_t*>(s_tmem)), 512);
@@ -173,7 +174,7 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
     }
   } else {
     // =============================================================== LayerNorm statistics + epilogue, thread = pair
-    const int pw = warp - 4;
+    const int pw = warp & 3, par = (warp - 4) >> 2;        // lane quadrant; which of every two blocks this thread writes
     const uint32_t t_lane = tmem_base + ((uint32_t)(pw * 32) << 16);
     const int prow = pw * 32 + lane;
     const uint32_t zrow = s_z + prow * 128, zsw = (uint32_t)(prow & 7);
@@ -228,15 +229,15 @@ __global__ void __launch_bounds__(bThreads, 1) bias_tiles_kernel(const __grid_co
         // in flight (one tcgen05.ld ahead)
         auto region = [&](uint32_t t_col, int b0, int n) {
           float accA[16], accB[16];
-          if (n > 0) tmem_ld_x16(t_col, accA);
-          for (int j = 0; j < n; j += 2) {
+          if (par < n) tmem_ld_x16(t_col + 16 * par, accA);
+          for (int j = par; j < n; j += 4) {
             tmem_ld_wait();
-            if (j + 1 < n) tmem_ld_x16(t_col + 16 * (j + 1), accB);
+            if (j + 2 < n) tmem_ld_x16(t_col + 16 * (j + 2), accB);
             emit(accA, b0 + j);
-            if (j + 1 < n) {
+            if (j + 2 < n) {
               tmem_ld_wait();
-              if (j + 2 < n) tmem_ld_x16(t_col + 16 * (j + 2), accA);
-              emit(accB, b0 + j + 1);
+              if (j + 4 < n) tmem_ld_x16(t_col + 16 * (j + 4), accA);
+              emit(accB, b0 + j + 2);
             }
           }
         };
