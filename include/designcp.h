@@ -191,7 +191,8 @@ dcp_status dcp_attention_stack(void *a, const void *z, int64_t ldz, const dcp_we
  * to the fp16 rounding of the bias (2^-11 relative, below the bf16 rounding of P that follows).
  * bias_cache: device, 16-byte aligned, >= dcp_attention_stack_cache_bytes(I, n_blocks) (I = 3000, 18 blocks: 5.2 GB);
  * it is scratch, valid only during the call.  H = 16, c_z = 128, DCP_BF16, all blocks with the same ln_eps
- * (DCP_ERR_UNSUPPORTED otherwise).  workspace >= dcp_attention_stack_cached_workspace_bytes. */
+ * (DCP_ERR_UNSUPPORTED otherwise).  workspace >= dcp_attention_stack_cached_workspace_bytes.  Launches only, no host
+ * synchronisation: capturable into a CUDA graph like dcp_attention_stack (tests/test_gpu_graph.py). */
 dcp_status dcp_attention_stack_cache_bytes(int64_t I, int n_blocks, size_t *bytes);
 dcp_status dcp_attention_stack_cached_workspace_bytes(int64_t I, int c_s, int H, int c, int c_z, dcp_dtype dtype, size_t *bytes);
 dcp_status dcp_attention_stack_cached(void *a, const void *z, int64_t ldz, const dcp_weights *blocks, int n_blocks, int64_t I,
