@@ -203,7 +203,7 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
     }
     __syncthreads();
     const int n_here = (L - t0 < kTile ? L - t0 : kTile);
-    if (tt != 0) {
+    {
       // bounding boxes of the tile's 128-atom chunks (atoms close in index are mostly close in space): warp w takes
       // chunks 2 w and 2 w + 1; an empty chunk gets lo = +inf, hi = -inf
 #pragma unroll
@@ -232,17 +232,26 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
       }
       __syncthreads();
     }
+    unsigned skip = 0u;                                        // chunks of this tile that step 1 has already taken
     if (tt == 0) {
-      // ---- 1a. the r smallest distances of each lane's share of the own tile
-      const int need = k < n_here ? k : n_here;
+      // ---- 1a. the home window: the kWin chunks of the own tile around the query (the whole tile when the window does not
+      // hold k atoms); the r smallest distances of each lane's share of it
+      constexpr int kWin = kCap <= 512 ? 4 : 16;               // 4 chunks = 512 atoms >= 2 k (k <= 256); larger k: the whole tile
+      int h0 = ((lq - t0) >> 7) - kWin / 2;
+      h0 = h0 < 0 ? 0 : (h0 > 16 - kWin ? 16 - kWin : h0);
+      int e0 = h0 * 128, e1 = e0 + kWin * 128;
+      e1 = e1 < n_here ? e1 : n_here;
+      if (e1 - e0 < k) { e0 = 0; e1 = n_here; }                // ragged tile end: take everything the tile has
+      const int n_win = e1 - e0;
+      skip = e1 - e0 == n_here ? 0xffffu : (((1u << kWin) - 1u) << h0);
+      const int need = k < n_win ? k : n_win;
       const int r = (need + 31) >> 5;                          // <= NS (k <= kCap / 2)
       unsigned sm[NS];
 #pragma unroll
       for (int j = 0; j < NS; ++j) sm[j] = kInfBits;
-#pragma unroll 4
-      for (int i = 0; i < kTile / 32; ++i) {
-        const int e = 32 * i + lane;
-        unsigned v = e < n_here ? dist_bits(e) : kInfBits;
+      for (int eb = e0; eb < e1; eb += 32) {
+        const int e = eb + lane;
+        unsigned v = e < e1 ? dist_bits(e) : kInfBits;
         if (__any_sync(0xffffffffu, v < sm[NS - 1])) {
 #pragma unroll
           for (int j = 0; j < NS; ++j) { const unsigned lo = min(sm[j], v); v = max(sm[j], v); sm[j] = lo; }
@@ -251,13 +260,12 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
       unsigned sr = sm[0];
 #pragma unroll
       for (int j = 1; j < NS; ++j) sr = j == r - 1 ? sm[j] : sr;
-      thr = n_here >= k ? __reduce_max_sync(0xffffffffu, sr) : kInfBits;   // T1; fewer than k atoms: no bound
-      // ---- 1b. the own tile's entries <= T1 -> buffer
-#pragma unroll 4
-      for (int i = 0; i < kTile / 32; ++i) {
-        const int e = 32 * i + lane;
-        const unsigned v = e < n_here ? dist_bits(e) : kInfBits;
-        append(v, t0 + e, e < n_here && v <= thr);
+      thr = n_win >= k ? __reduce_max_sync(0xffffffffu, sr) : kInfBits;   // T1; fewer than k atoms: no bound
+      // ---- 1b. the window's entries <= T1 -> buffer
+      for (int eb = e0; eb < e1; eb += 32) {
+        const int e = eb + lane;
+        const unsigned v = e < e1 ? dist_bits(e) : kInfBits;
+        append(v, t0 + e, e < e1 && v <= thr);
       }
       __syncwarp();
       if (!over && thr != kInfBits) {
@@ -267,8 +275,10 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
         thr = bisect(bv, thr, need, 14);
         cnt = compact(bv, thr, cnt);
       }
-    } else {
-      // ---- 2. every other tile: the chunks whose bounding box reaches within the bound, four 32-candidate pieces per step.
+    }
+    {
+      // ---- 2. the chunks (of the own tile: the ones outside the home window) whose bounding box reaches within the bound,
+      // four 32-candidate pieces per step.
       // Lane c < 16 takes chunk c: lb = the pinned distance arithmetic applied to the per-axis gaps between the query and
       // the box (sub, mul, add, add, each rounded to nearest, no FMA).  Rounding is monotone, so every atom of the chunk has
       // a computed d2 >= lb: a chunk with lb > T holds no candidate, and skipping it changes no bit of the result.
@@ -280,7 +290,7 @@ __global__ void __launch_bounds__(256) knn_select_kernel(const float* __restrict
         const float g2 = fmaxf(fmaxf(__fsub_rn(bx[2], q2), __fsub_rn(q2, bx[5])), 0.f);
         lb = __fadd_rn(__fadd_rn(__fmul_rn(g0, g0), __fmul_rn(g1, g1)), __fmul_rn(g2, g2));
       }
-      unsigned todo = __ballot_sync(0xffffffffu, lane < 16 && __float_as_uint(lb) <= thr);
+      unsigned todo = __ballot_sync(0xffffffffu, lane < 16 && __float_as_uint(lb) <= thr) & ~skip;
       while (todo) {
         const int c0 = (__ffs(todo) - 1) * 128;
         todo &= todo - 1;
