@@ -712,11 +712,21 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
     // to the query-to-box gaps -- a lower bound of every atom's computed d2, rounding being monotone -- exceeds both
     // classes' distance bounds.  The own chain's size is then counted per chunk: all of it, none of it, or (a chunk that
     // straddles chains) by a pass over the chain ids alone.
+    // The own tile goes in two rounds: the four chunks around the query first, so that both bounds are tight before the
+    // rest of the tile (and every other tile) is tested.
+    unsigned home = 0xffffu;
+    if (tt == 0) {
+      int h0 = ((lq - t0) >> 7) - 2;
+      h0 = h0 < 0 ? 0 : (h0 > 12 ? 12 : h0);
+      home = 0xfu << h0;
+    }
+    for (int round = 0; round < (tt == 0 ? 2 : 1); ++round) {
+    const unsigned allowed = round == 0 ? home : ~home;
     unsigned todo, count_only;
     {
       bool scan_it = false, count_it = false;
       int whole = 0;
-      if (lane < 16 && lane * 128 < n_here) {
+      if (lane < 16 && lane * 128 < n_here && ((allowed >> lane) & 1u)) {
         const float* bx = box + lane * 6;
         const float g0 = fmaxf(fmaxf(__fsub_rn(bx[0], q0), __fsub_rn(q0, bx[3])), 0.f);
         const float g1 = fmaxf(fmaxf(__fsub_rn(bx[1], q1), __fsub_rn(q1, bx[4])), 0.f);
@@ -778,6 +788,7 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
       }
     };
     if (n_here == kTile) scan(std::false_type{}); else scan(std::true_type{});
+    }
   }
   if (!active) return;
   __syncwarp();
