@@ -722,9 +722,9 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
     }
     for (int round = 0; round < (tt == 0 ? 2 : 1); ++round) {
     const unsigned allowed = round == 0 ? home : ~home;
-    unsigned todo, count_only;
+    unsigned todo, count_only, pure_b;
     {
-      bool scan_it = false, count_it = false;
+      bool scan_it = false, count_it = false, foreign = false;
       int whole = 0;
       if (lane < 16 && lane * 128 < n_here && ((allowed >> lane) & 1u)) {
         const float* bx = box + lane * 6;
@@ -739,11 +739,13 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
         // class A lives only in chunks that hold own-chain atoms (every chunk without a split), class B in the others
         scan_it = may_local || ((may_same || !split) && lb <= lim_a) || (split && !all_same && lb <= lim_b);
         count_it = !scan_it && may_same && !all_same;
+        foreign = split && !may_same;                          // no own-chain atom in the chunk: every atom is class B
         const int n_ch = n_here - lane * 128 < 128 ? n_here - lane * 128 : 128;
         whole = (!scan_it && all_same) ? n_ch : 0;
       }
       todo = __ballot_sync(0xffffffffu, scan_it);
       count_only = __ballot_sync(0xffffffffu, count_it);
+      pure_b = __ballot_sync(0xffffffffu, foreign);
       cs_w += __reduce_add_sync(0xffffffffu, whole);
     }
     while (count_only) {
@@ -758,8 +760,24 @@ __global__ void __launch_bounds__(256) knn_budget_select_kernel(const float* __r
     // four 32-candidate pieces per step: independent loads and arithmetic; only the last tile can be ragged
     auto scan = [&](auto RAGGED) {
       while (todo) {
-        const int c0 = (__ffs(todo) - 1) * 128;
+        const int ch = __ffs(todo) - 1, c0 = ch * 128;
         todo &= todo - 1;
+        if ((pure_b >> ch) & 1u) {
+          // a chunk of foreign atoms only (most of them): distances and one compare, no ids, no class A
+          unsigned dbf[4], mf[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int e = c0 + 32 * u + lane;
+            const float a0 = __fsub_rn(sx[e], q0), a1 = __fsub_rn(sy[e], q1), a2 = __fsub_rn(sz[e], q2);
+            dbf[u] = __float_as_uint(__fadd_rn(__fadd_rn(__fmul_rn(a0, a0), __fmul_rn(a1, a1)), __fmul_rn(a2, a2)));
+            mf[u] = __ballot_sync(0xffffffffu, dbf[u] <= thr_b && (!decltype(RAGGED)::value || e < n_here));
+          }
+          if ((mf[0] | mf[1] | mf[2] | mf[3]) == 0) continue;
+#pragma unroll
+          for (int u = 0; u < 4; ++u)
+            if (mf[u]) append(bk, bi, nb, thr_b, mf[u], (mf[u] >> lane) & 1u, dbf[u], t0 + c0 + 32 * u + lane, true);
+          continue;
+        }
         unsigned db[4], ka[4], ma[4], mb[4];
         bool pa[4], pb[4];
 #pragma unroll
