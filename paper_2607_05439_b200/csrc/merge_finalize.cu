@@ -133,7 +133,9 @@ cudaError_t launch_vec4(const MergeParams& p, unsigned blocks, cudaStream_t st) 
     case 2: return launch_vec4_n<T, 2>(p, blocks, st);
     case 3: return launch_vec4_n<T, 3>(p, blocks, st);
     case 4: return launch_vec4_n<T, 4>(p, blocks, st);
+    case 5: return launch_vec4_n<T, 5>(p, blocks, st);
     case 6: return launch_vec4_n<T, 6>(p, blocks, st);
+    case 7: return launch_vec4_n<T, 7>(p, blocks, st);
     case 8: return launch_vec4_n<T, 8>(p, blocks, st);
     case 12: return launch_vec4_n<T, 12>(p, blocks, st);
     case 16: return launch_vec4_n<T, 16>(p, blocks, st);
