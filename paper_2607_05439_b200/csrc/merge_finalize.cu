@@ -137,6 +137,7 @@ cudaError_t launch_vec4(const MergeParams& p, unsigned blocks, cudaStream_t st) 
     case 6: return launch_vec4_n<T, 6>(p, blocks, st);
     case 7: return launch_vec4_n<T, 7>(p, blocks, st);
     case 8: return launch_vec4_n<T, 8>(p, blocks, st);
+    case 9: return launch_vec4_n<T, 9>(p, blocks, st);
     case 12: return launch_vec4_n<T, 12>(p, blocks, st);
     case 16: return launch_vec4_n<T, 16>(p, blocks, st);
     default: return launch_vec4_n<T, 0>(p, blocks, st);
