@@ -193,33 +193,43 @@ __global__ void __launch_bounds__(cThreads, 1) cached_attn_kernel(const MmaParam
         }
       }
       uint32_t pf[2][4];
+      if (partial) {
 #pragma unroll
-      for (int mb = 0; mb < 2; ++mb) {
-        if (partial) {
+        for (int mb = 0; mb < 2; ++mb) {
           const int k0 = j0 + 4 * t;
           if (k0 < un.ks || k0 >= un.ke) { sA[mb][0] = -INFINITY; sA[mb][2] = -INFINITY; }
           if (k0 + 1 < un.ks || k0 + 1 >= un.ke) { sA[mb][1] = -INFINITY; sA[mb][3] = -INFINITY; }
           if (k0 + 2 < un.ks || k0 + 2 >= un.ke) { sB[mb][0] = -INFINITY; sB[mb][2] = -INFINITY; }
           if (k0 + 3 < un.ks || k0 + 3 >= un.ke) { sB[mb][1] = -INFINITY; sB[mb][3] = -INFINITY; }
         }
-        // ---- a5: online softmax (exp2 domain), rows g (x = 0) and g + 8 (x = 1); the reference m of a row moves only
-        // when the tile maximum exceeds it by more than kLazy (reading 19; fused_mma.cu)
-        constexpr float kLazy = 8.f;
-        const float mx0 = quad_max(fmaxf(fmaxf(sA[mb][0], sA[mb][1]), fmaxf(sB[mb][0], sB[mb][1])));
-        const float mx1 = quad_max(fmaxf(fmaxf(sA[mb][2], sA[mb][3]), fmaxf(sB[mb][2], sB[mb][3])));
-        const float mo0 = m_run[mb][0], mo1 = m_run[mb][1];
-        const bool mv0 = mx0 > mo0 + kLazy, mv1 = mx1 > mo1 + kLazy;
-        const float mn0 = mv0 ? mx0 : mo0, mn1 = mv1 ? mx1 : mo1;
-        m_run[mb][0] = mn0;
-        m_run[mb][1] = mn1;
-        sA[mb][0] = fast_exp2(sA[mb][0] - mn0); sA[mb][1] = fast_exp2(sA[mb][1] - mn0);
-        sB[mb][0] = fast_exp2(sB[mb][0] - mn0); sB[mb][1] = fast_exp2(sB[mb][1] - mn0);
-        sA[mb][2] = fast_exp2(sA[mb][2] - mn1); sA[mb][3] = fast_exp2(sA[mb][3] - mn1);
-        sB[mb][2] = fast_exp2(sB[mb][2] - mn1); sB[mb][3] = fast_exp2(sB[mb][3] - mn1);
-        const float sum0 = (sA[mb][0] + sA[mb][1]) + (sB[mb][0] + sB[mb][1]);
-        const float sum1 = (sA[mb][2] + sA[mb][3]) + (sB[mb][2] + sB[mb][3]);
-        if (__any_sync(0xffffffffu, mv0 || mv1)) {
-          const float al0 = mv0 ? fast_exp2(mo0 - mn0) : 1.f, al1 = mv1 ? fast_exp2(mo1 - mn1) : 1.f;
+      }
+      // ---- a5: online softmax (exp2 domain), rows g (x = 0) and g + 8 (x = 1); the reference m of a row moves only when
+      // the tile maximum exceeds it by more than kLazy (reading 19; fused_mma.cu).  After the first tiles that is
+      // rare, so the common tile only ASKS whether any logit exceeds its row's reference + kLazy (sixteen compares, one
+      // vote) and skips the maxima, their two shuffle rounds and the rescale; the answer is the same predicate the maxima
+      // would give, so no bit changes.
+      constexpr float kLazy = 8.f;
+      bool exceed = false;
+#pragma unroll
+      for (int mb = 0; mb < 2; ++mb) {
+        const float t0 = m_run[mb][0] + kLazy, t1 = m_run[mb][1] + kLazy;
+        exceed = exceed || sA[mb][0] > t0 || sA[mb][1] > t0 || sB[mb][0] > t0 || sB[mb][1] > t0 ||
+                 sA[mb][2] > t1 || sA[mb][3] > t1 || sB[mb][2] > t1 || sB[mb][3] > t1;
+      }
+      const bool moved = __any_sync(0xffffffffu, exceed);
+#pragma unroll
+      for (int mb = 0; mb < 2; ++mb) {
+        float mn0 = m_run[mb][0], mn1 = m_run[mb][1];
+        if (moved) {
+          const float mx0 = quad_max(fmaxf(fmaxf(sA[mb][0], sA[mb][1]), fmaxf(sB[mb][0], sB[mb][1])));
+          const float mx1 = quad_max(fmaxf(fmaxf(sA[mb][2], sA[mb][3]), fmaxf(sB[mb][2], sB[mb][3])));
+          const float mo0 = mn0, mo1 = mn1;
+          const bool mv0 = mx0 > mo0 + kLazy, mv1 = mx1 > mo1 + kLazy;
+          mn0 = mv0 ? mx0 : mo0;
+          mn1 = mv1 ? mx1 : mo1;
+          m_run[mb][0] = mn0;
+          m_run[mb][1] = mn1;
+          const float al0 = mv0 ? fast_exp2(mo0 - mn0) : 1.f, al1 = mv1 ? fast_exp2(mo1 - mn1) : 1.f;   // rows that stay: x 1
           l_run[mb][0] *= al0;
           l_run[mb][1] *= al1;
 #pragma unroll
@@ -228,8 +238,12 @@ __global__ void __launch_bounds__(cThreads, 1) cached_attn_kernel(const MmaParam
             o[mb][nd][2] *= al1; o[mb][nd][3] *= al1;
           }
         }
-        l_run[mb][0] += sum0;
-        l_run[mb][1] += sum1;
+        sA[mb][0] = fast_exp2(sA[mb][0] - mn0); sA[mb][1] = fast_exp2(sA[mb][1] - mn0);
+        sB[mb][0] = fast_exp2(sB[mb][0] - mn0); sB[mb][1] = fast_exp2(sB[mb][1] - mn0);
+        sA[mb][2] = fast_exp2(sA[mb][2] - mn1); sA[mb][3] = fast_exp2(sA[mb][3] - mn1);
+        sB[mb][2] = fast_exp2(sB[mb][2] - mn1); sB[mb][3] = fast_exp2(sB[mb][3] - mn1);
+        l_run[mb][0] += (sA[mb][0] + sA[mb][1]) + (sB[mb][0] + sB[mb][1]);
+        l_run[mb][1] += (sA[mb][2] + sA[mb][3]) + (sB[mb][2] + sB[mb][3]);
         pf[mb][0] = pack_bf16(sA[mb][0], sA[mb][1]); pf[mb][1] = pack_bf16(sA[mb][2], sA[mb][3]);
         pf[mb][2] = pack_bf16(sB[mb][0], sB[mb][1]); pf[mb][3] = pack_bf16(sB[mb][2], sB[mb][3]);
       }
